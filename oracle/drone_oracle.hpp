@@ -1,0 +1,663 @@
+// oracle/drone_oracle.hpp — TEST INFRASTRUCTURE: the plain, slow, float64 CPU oracle of the batched
+// drone-environment step of arxiv/paper_2606_08039 ("MuJoCo-Drones-Gym").
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may
+// import, link or execute anything under oracle/.  It shares no code, header, table or constant
+// generator with the CUDA path (paper_2606_08039_b200/csrc/, include/mdg.h); the enum VALUES below
+// are restated because they are the interface both sides receive from the workload recipes.
+//
+// The method is a time-stepping iteration, so this file follows the algorithm step by step in the
+// paper's order: scalar loops env -> drone, no blocking, no fusion, no reordering.  Each function cites
+// the PAPER.md passage it follows; where the paper is silent the reading Qn of SURVEY.md §8(c) /
+// DESIGN.md §3 is named.  The scalar type R is a template parameter: R=double is the oracle,
+// R=Counted (oracle_capi.cpp) yields the algorithmic flop tally used by bench.py's roofline.
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): O1 constants, free fall, hover equilibrium, uniform
+// thrust / pure yaw closed forms, torque-free rotation invariants + axisymmetric top + convergence
+// order, ground / drag / downwash closed forms, symmetries, PID fixed point + linear z recurrence +
+// allocation round trip, wind statistics, obs/reward/termination on hand-built states, Philox KATs.
+// PARITY UNPINNED (the oracle itself is the reference): the coupled PID transient in x/y and the
+// multi-config trajectories beyond the invariants above; parity against MuJoCo's own RK4 (MuJoCo is
+// not in the container, reading Q11).
+#pragma once
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#include "philox_ref.hpp"
+
+namespace orc {
+
+// ---- interface enums (values are the interface; Table 1, 179-187 Table 3) -------
+enum { AERO_GND = 1, AERO_DRAG = 2, AERO_DW = 4, AERO_WIND = 8 };
+enum { INTEG_RK4 = 0, INTEG_EULER = 1 };
+enum { PHYS_MJC = 0, PHYS_MJC_GND = 1, PHYS_MJC_DRAG = 2, PHYS_MJC_DW = 3, PHYS_MJC_GND_DRAG_DW = 4, PHYS_DYN = 5 };
+enum { ACT_RPM = 0, ACT_PID = 1, ACT_VEL = 2 };
+enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1 };
+enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3 };
+enum { TERM_NONE = 0, TERM_HOVER = 1, TERM_TILT_DIST = 2, TERM_FORMATION = 3 };
+enum { LAYOUT_NONE = 0, LAYOUT_GRID = 1, LAYOUT_CIRCLE = 2 };
+enum { TGT_FIXED = 0, TGT_SPAWN_LINSPACE = 1, TGT_BOX = 2, TGT_CIRCLE = 3 };
+enum { MODEL_CF2X = 0, MODEL_RACE = 2 };
+
+static const double PI = 3.14159265358979323846;
+
+// ---- parameters --------------------------------------------------------------------------------
+struct Params {
+    // Table 2; units per reading Q1: n in RPM, k_f and k_m per RPM^2.
+    double m, g, L, k_f, k_m, J[3], r_p, tw_ratio;
+    // aero; values absent from the paper are reading Q5/Q6/Q9.
+    double C_gnd, h_clip, c_xy, c_z, dw_C1, dw_C2, dw_C3, dw_dz_clip;
+    // wind (readings Q27, Q28)
+    double k_wind, wind_sigma, wind_tau;
+    int sim_freq, ctrl_freq;
+    int aero_mask, integrator;        // -1: take from physics_mode (Table 1)
+    // cascaded PID (Table 6; readings Q17-Q21)
+    double Kp_pos[3], Ki_pos[3], Kd_pos[3], Kp_att[3], Ki_att[3], Kd_att[3];
+    double int_clamp_pos, int_clamp_att;
+    int dsl;                          // DSL-PID setpoint rate limits
+    double pos_rate_limit, yaw_rate_limit, a_ff[3], tilt_max, tau_xy_max, tau_z_max;
+    // observation / reward / termination
+    int obs_mode; double adj_radius;
+    int reward_mode; double at_target_radius;
+    int term_mode; double term_tilt, term_dist, term_center[3], z_max;
+    double episode_len_s; int auto_reset;
+    // reset distribution and per-episode targets (workload recipe)
+    int reset_layout; double reset_center[3], reset_half[3], reset_z_lo, reset_z_hi;
+    int grid_cols; double grid_spacing, circle_radius;
+    int target_mode; double target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi,
+        form_center[3], form_radius;
+};
+
+inline void default_params(int model, Params& P) {
+    std::memset(&P, 0, sizeof(P));
+    if (model == MODEL_RACE) {        // Table 2, RACE column
+        P.m = 0.250; P.L = 0.125; P.tw_ratio = 4.0; P.J[0] = P.J[1] = 4.86e-4; P.J[2] = 8.80e-4;
+        P.k_f = 1.28e-8; P.k_m = 5.96e-10; P.r_p = 0.0635;
+    } else {                          // Table 2, CF2X column
+        P.m = 0.027; P.L = 0.0397; P.tw_ratio = 2.25; P.J[0] = P.J[1] = 1.4e-5; P.J[2] = 2.17e-5;
+        P.k_f = 3.16e-10; P.k_m = 7.94e-12; P.r_p = 0.02325;
+    }
+    P.g = 9.81;                                                   // Q2
+    P.C_gnd = 11.36859; P.c_xy = 9.1785e-7; P.c_z = 10.311e-7;   // Q5
+    P.h_clip = 0.25 * P.r_p * std::sqrt(15.0 * P.C_gnd / 4.0);    // Q6
+    P.dw_C1 = 2267.18; P.dw_C2 = 0.16; P.dw_C3 = -0.11;
+    P.dw_dz_clip = 0.1;                                           // Q9
+    P.k_wind = 0.5 * 1.225 * 1.0 * 0.01;                          // Q28
+    P.wind_sigma = 0.5; P.wind_tau = 1.0;
+    P.sim_freq = 240; P.ctrl_freq = 48;
+    P.aero_mask = -1; P.integrator = -1;
+    const double kp[3] = {0.4, 0.4, 1.0}, ki[3] = {0.01, 0.01, 0.01}, kd[3] = {0.9, 0.9, 2.0};     // Table 6
+    const double ap[3] = {2e-3, 2e-3, 1e-3}, ai[3] = {0, 0, 1e-4}, ad[3] = {5e-4, 5e-4, 2e-4};
+    for (int i = 0; i < 3; ++i) {
+        P.Kp_pos[i] = kp[i]; P.Ki_pos[i] = ki[i]; P.Kd_pos[i] = kd[i];
+        P.Kp_att[i] = ap[i]; P.Ki_att[i] = ai[i]; P.Kd_att[i] = ad[i];
+    }
+    P.int_clamp_pos = 2.0; P.int_clamp_att = 0.5; P.dsl = 0;
+    P.pos_rate_limit = 2.0; P.yaw_rate_limit = PI; P.tilt_max = 0.5;
+    const double s_hover = P.m * P.g / 4.0;                       // Q17
+    P.tau_xy_max = 4.0 * (P.L / std::sqrt(2.0)) * s_hover / 3.0;
+    P.tau_z_max = 4.0 * (P.k_m / P.k_f) * s_hover / 3.0;
+    P.obs_mode = OBS_KIN12; P.adj_radius = 0.5;
+    P.reward_mode = REW_HOVER; P.at_target_radius = 0.05;         // Q24
+    P.term_mode = TERM_HOVER; P.term_tilt = PI / 2; P.term_dist = 3.0; P.z_max = 3.0;
+    P.episode_len_s = 10.0; P.auto_reset = 1;
+    P.reset_layout = LAYOUT_NONE; P.reset_center[2] = 1.0;
+    P.reset_half[0] = P.reset_half[1] = P.reset_half[2] = 0.1;
+    P.grid_cols = 4; P.grid_spacing = 0.3; P.circle_radius = 0.3;
+    P.target_mode = TGT_FIXED; P.target_fixed[2] = 1.0;
+    P.target_lo[0] = P.target_lo[1] = -1; P.target_lo[2] = 0.2;
+    P.target_hi[0] = P.target_hi[1] = 1; P.target_hi[2] = 2.0;
+    P.mh_z_lo = 0.7; P.mh_z_hi = 1.2;
+    P.form_center[2] = 1.0; P.form_radius = 0.3;                  // PAPER.md:325, Q26
+}
+
+// O1 derived constants (reading Q4)
+struct Derived {
+    double W, hover_rpm, max_rpm, l, kappa, s_max, h, dt_c; int K, ep_steps, aero, integ;
+};
+inline Derived derive(const Params& P, int physics_mode) {
+    Derived d;
+    d.W = P.m * P.g;
+    d.hover_rpm = std::sqrt(d.W / (4.0 * P.k_f));
+    d.max_rpm = std::sqrt(P.tw_ratio * d.W / (4.0 * P.k_f));
+    d.l = P.L / std::sqrt(2.0);
+    d.kappa = P.k_m / P.k_f;
+    d.s_max = P.k_f * d.max_rpm * d.max_rpm;
+    d.h = 1.0 / P.sim_freq;
+    d.dt_c = 1.0 / P.ctrl_freq;
+    d.K = P.sim_freq / P.ctrl_freq;
+    d.ep_steps = (int)std::llround(P.episode_len_s * P.ctrl_freq);
+    int aero = 0, integ = INTEG_RK4;                              // Table 1
+    switch (physics_mode) {
+        case PHYS_MJC_GND: aero = AERO_GND; break;
+        case PHYS_MJC_DRAG: aero = AERO_DRAG; break;
+        case PHYS_MJC_DW: aero = AERO_DW; break;
+        case PHYS_MJC_GND_DRAG_DW: aero = AERO_GND | AERO_DRAG | AERO_DW; break;
+        case PHYS_DYN: integ = INTEG_EULER; break;
+        default: break;
+    }
+    d.aero = P.aero_mask >= 0 ? P.aero_mask : aero;
+    d.integ = P.integrator >= 0 ? P.integrator : integ;
+    return d;
+}
+
+// ---- small linear algebra on scalar type R -----------------------------------------------------
+template <class R> inline double to_d(const R& x) { return (double)x; }
+
+// body->world rotation matrix of q=[w,x,y,z]
+template <class R> inline void rotmat(const R q[4], R M[3][3]) {
+    const R w = q[0], x = q[1], y = q[2], z = q[3];
+    M[0][0] = 1.0 - 2.0 * (y * y + z * z); M[0][1] = 2.0 * (x * y - w * z); M[0][2] = 2.0 * (x * z + w * y);
+    M[1][0] = 2.0 * (x * y + w * z); M[1][1] = 1.0 - 2.0 * (x * x + z * z); M[1][2] = 2.0 * (y * z - w * x);
+    M[2][0] = 2.0 * (x * z - w * y); M[2][1] = 2.0 * (y * z + w * x); M[2][2] = 1.0 - 2.0 * (x * x + y * y);
+}
+template <class R> inline void mat_vec(const R M[3][3], const R a[3], R out[3]) {
+    for (int i = 0; i < 3; ++i) out[i] = M[i][0] * a[0] + M[i][1] * a[1] + M[i][2] * a[2];
+}
+template <class R> inline void matT_vec(const R M[3][3], const R a[3], R out[3]) {
+    for (int i = 0; i < 3; ++i) out[i] = M[0][i] * a[0] + M[1][i] * a[1] + M[2][i] * a[2];
+}
+template <class R> inline void cross(const R a[3], const R b[3], R out[3]) {
+    out[0] = a[1] * b[2] - a[2] * b[1]; out[1] = a[2] * b[0] - a[0] * b[2]; out[2] = a[0] * b[1] - a[1] * b[0];
+}
+template <class R> inline void quat_mul(const R a[4], const R b[4], R out[4]) {
+    out[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
+    out[1] = a[0] * b[1] + b[0] * a[1] + (a[2] * b[3] - a[3] * b[2]);
+    out[2] = a[0] * b[2] + b[0] * a[2] + (a[3] * b[1] - a[1] * b[3]);
+    out[3] = a[0] * b[3] + b[0] * a[3] + (a[1] * b[2] - a[2] * b[1]);
+}
+// Eq.7, readings Q13: Exp(q, phi) = q (x) [cos(|phi|/2), sin(|phi|/2) phi/|phi|];
+// phi = omega_body * dt multiplies on the right; series form below 1e-8.
+template <class R> inline void quat_exp_step(const R q[4], const R phi[3], R out[4]) {
+    const R n2 = phi[0] * phi[0] + phi[1] * phi[1] + phi[2] * phi[2];
+    const R n = sqrt(n2);
+    R dq[4];
+    if (n < 1e-8) {
+        dq[0] = 1.0; dq[1] = 0.5 * phi[0]; dq[2] = 0.5 * phi[1]; dq[3] = 0.5 * phi[2];
+    } else {
+        const R half = 0.5 * n;
+        const R s = sin(half) / n;
+        dq[0] = cos(half); dq[1] = s * phi[0]; dq[2] = s * phi[1]; dq[3] = s * phi[2];
+    }
+    quat_mul(q, dq, out);
+}
+template <class R> inline void quat_normalise(R q[4]) {
+    const R n = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+    for (int i = 0; i < 4; ++i) q[i] = q[i] / n;
+}
+// ZYX Euler angles (O3.1): roll phi, pitch theta, yaw psi
+template <class R> inline void euler_zyx(const R q[4], R eta[3]) {
+    const R w = q[0], x = q[1], y = q[2], z = q[3];
+    eta[0] = atan2(2.0 * (w * x + y * z), 1.0 - 2.0 * (x * x + y * y));
+    R sp = 2.0 * (w * y - z * x);
+    if (sp > 1.0) sp = 1.0;
+    if (sp < -1.0) sp = -1.0;
+    eta[1] = asin(sp);
+    eta[2] = atan2(2.0 * (w * z + x * y), 1.0 - 2.0 * (y * y + z * z));
+}
+template <class R> inline R clampR(const R& x, double lo, double hi) {
+    R y = x;
+    if (y < lo) y = lo;
+    if (y > hi) y = hi;
+    return y;
+}
+template <class R> inline R wrap_pi(const R& x) {     // (-pi, pi]
+    const double xd = to_d(x);
+    const double k = std::ceil((xd - PI) / (2.0 * PI));
+    return x - (2.0 * PI) * k;
+}
+
+// ---- per-drone working set ---------------------------------------------------------------------
+template <class R> struct Drone {
+    R p[3], q[4], v[3], w[3];     // A1 state; w is body-frame (Q22)
+    R Ip[3], Ie[3], sp[4];        // PID memory: position / attitude integrals, held setpoint (DSL)
+    double tg[4];                 // per-episode target (x, y, z, psi)
+    R n[4];                       // rotor speeds in RPM, held over the K substeps (Q21)
+    R T, tau_b[3], Om;            // O4: collective thrust, body torque, sum of 2 pi n / 60
+    R Fwind[3];                   // O9 wind force, held over the K substeps (Q28)
+    R Fw[3], tw[3];               // substep wrench, world frame
+    bool hit;                     // sticky floor-hit flag for this control step (Q15)
+    double min_abs_pz;            // threshold margin bookkeeping (not part of the method)
+};
+
+// O4 motor model (Eq.1-3; Q3 yaw pattern m=(1,0,1,0))
+template <class R>
+inline void motor_wrench(const Params& P, const Derived& D, const R n[4], R& T, R tau[3], R& Om) {
+    R s[4];
+    for (int i = 0; i < 4; ++i) s[i] = P.k_f * (n[i] * n[i]);
+    T = s[0] + s[1] + s[2] + s[3];
+    tau[0] = D.l * (s[0] + s[1] - s[2] - s[3]);
+    tau[1] = D.l * (-s[0] + s[1] + s[2] - s[3]);
+    tau[2] = D.kappa * (-s[0] + s[1] - s[2] + s[3]);
+    Om = (2.0 * PI / 60.0) * (n[0] + n[1] + n[2] + n[3]);      // Eq.5's rotor-speed sum
+}
+
+// O3.7 closed-form allocation inverse: per-rotor thrusts from (T, tau)
+template <class R>
+inline void alloc_inverse(const Derived& D, const R& T, const R tau[3], R s[4]) {
+    const R a = tau[0] / D.l, b = tau[1] / D.l, c = tau[2] / D.kappa;
+    s[0] = 0.25 * (T + a - b - c);
+    s[1] = 0.25 * (T + a + b + c);
+    s[2] = 0.25 * (T - a + b - c);
+    s[3] = 0.25 * (T - a - b + c);
+}
+
+// O2/O3 action decode -> RPM (Table 3; cascaded PID PAPER.md:347-357, 372-376)
+template <class R>
+inline void decode_action(const Params& P, const Derived& D, int action_type, const float a_in[4], Drone<R>& d) {
+    if (action_type == ACT_RPM) {                                  // Q16: raw RPM, clipped
+        for (int i = 0; i < 4; ++i) d.n[i] = clampR(R((double)a_in[i]), 0.0, D.max_rpm);
+        return;
+    }
+    const double dt = D.dt_c;                                      // Q21: once per control step
+    R eta[3];
+    euler_zyx(d.q, eta);                                           // O3.1
+    const R psi = eta[2];
+    R p_ref[3], v_ref[3], psi_ref;
+    if (action_type == ACT_PID) {                                  // O3.2 waypoint [x,y,z,psi]
+        const double pc[3] = {(double)a_in[0], (double)a_in[1], (double)a_in[2]};
+        const double psic = (double)a_in[3];
+        if (P.dsl) {                                               // rate-limited held setpoint
+            R dv[3] = {pc[0] - d.sp[0], pc[1] - d.sp[1], pc[2] - d.sp[2]};
+            const R dist = sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]);
+            const double max_step = P.pos_rate_limit * dt;
+            if (dist > max_step) {
+                const R f = max_step / dist;
+                for (int i = 0; i < 3; ++i) d.sp[i] = d.sp[i] + dv[i] * f;
+            } else {
+                for (int i = 0; i < 3; ++i) d.sp[i] = pc[i];
+            }
+            R dpsi = wrap_pi(R(psic) - d.sp[3]);
+            dpsi = clampR(dpsi, -P.yaw_rate_limit * dt, P.yaw_rate_limit * dt);
+            d.sp[3] = wrap_pi(d.sp[3] + dpsi);
+        } else {
+            for (int i = 0; i < 3; ++i) d.sp[i] = pc[i];
+            d.sp[3] = psic;
+        }
+        for (int i = 0; i < 3; ++i) { p_ref[i] = d.sp[i]; v_ref[i] = 0.0; }
+        psi_ref = d.sp[3];
+    } else {                                                       // ACT_VEL, Q20: heading frame
+        const R c = cos(psi), s = sin(psi);
+        const double ax = a_in[0], ay = a_in[1], az = a_in[2], wz = a_in[3];
+        for (int i = 0; i < 3; ++i) p_ref[i] = d.p[i];
+        v_ref[0] = c * ax - s * ay; v_ref[1] = s * ax + c * ay; v_ref[2] = az;
+        psi_ref = psi + wz * dt;
+    }
+    // O3.3 position loop, Eq.9
+    R acc[3];
+    for (int i = 0; i < 3; ++i) {
+        const R e = p_ref[i] - d.p[i];
+        d.Ip[i] = clampR(d.Ip[i] + e * dt, -P.int_clamp_pos, P.int_clamp_pos);
+        acc[i] = P.Kp_pos[i] * e + P.Ki_pos[i] * d.Ip[i] + P.Kd_pos[i] * (v_ref[i] - d.v[i]) + P.a_ff[i];
+    }
+    acc[2] = acc[2] + P.g;
+    // O3.4 thrust T = m |a*| (Q18)
+    const R T = clampR(P.m * sqrt(acc[0] * acc[0] + acc[1] * acc[1] + acc[2] * acc[2]), 0.0, 4.0 * D.s_max);
+    // O3.5 small-angle attitude target (Q17)
+    const R cps = cos(psi), sps = sin(psi);
+    const R phi_ref = clampR((acc[0] * sps - acc[1] * cps) / P.g, -P.tilt_max, P.tilt_max);
+    const R th_ref = clampR((acc[0] * cps + acc[1] * sps) / P.g, -P.tilt_max, P.tilt_max);
+    // O3.6 attitude PID, D on measurement
+    R e_eta[3] = {phi_ref - eta[0], th_ref - eta[1], wrap_pi(psi_ref - psi)};
+    R tau[3];
+    for (int i = 0; i < 3; ++i) {
+        d.Ie[i] = clampR(d.Ie[i] + e_eta[i] * dt, -P.int_clamp_att, P.int_clamp_att);
+        tau[i] = P.Kp_att[i] * e_eta[i] + P.Ki_att[i] * d.Ie[i] - P.Kd_att[i] * d.w[i];
+    }
+    tau[0] = clampR(tau[0], -P.tau_xy_max, P.tau_xy_max);
+    tau[1] = clampR(tau[1], -P.tau_xy_max, P.tau_xy_max);
+    tau[2] = clampR(tau[2], -P.tau_z_max, P.tau_z_max);
+    // O3.7 allocation inverse and per-rotor clip
+    R s[4];
+    alloc_inverse(D, T, tau, s);
+    for (int i = 0; i < 4; ++i) d.n[i] = sqrt(clampR(s[i], 0.0, D.s_max) / P.k_f);
+}
+
+// O5-O7: world-frame wrench of drone i from the start-of-substep state of all M drones of the env
+// (PAPER.md:86-102, 106).
+template <class R>
+inline void substep_wrench(const Params& P, const Derived& D, Drone<R>* dr, int M, int i) {
+    Drone<R>& d = dr[i];
+    R Rm[3][3];
+    rotmat(d.q, Rm);
+    d.Fw[0] = Rm[0][2] * d.T; d.Fw[1] = Rm[1][2] * d.T; d.Fw[2] = Rm[2][2] * d.T;   // R (0,0,T)
+    mat_vec(Rm, d.tau_b, d.tw);                                                      // R tau_b
+    if (D.aero & AERO_GND) {                       // Eq.4; Q7 body height, Q8 gate R22 > 0
+        if (Rm[2][2] > 0.0) {
+            R hgt = d.p[2];
+            if (hgt < P.h_clip) hgt = P.h_clip;
+            const R ratio = P.r_p / (4.0 * hgt);
+            d.Fw[2] = d.Fw[2] + P.C_gnd * d.T * (ratio * ratio);
+        }
+    }
+    if (D.aero & AERO_DRAG) {                      // Eq.5
+        R vb[3], fb[3], fw[3];
+        matT_vec(Rm, d.v, vb);
+        fb[0] = -(P.c_xy * d.Om) * vb[0]; fb[1] = -(P.c_xy * d.Om) * vb[1]; fb[2] = -(P.c_z * d.Om) * vb[2];
+        mat_vec(Rm, fb, fw);
+        for (int a = 0; a < 3; ++a) d.Fw[a] = d.Fw[a] + fw[a];
+    }
+    if (D.aero & AERO_DW) {                        // Eq.6 with the regularisation of Q9, reaction per Q10
+        for (int k = 0; k < M; ++k) {
+            if (k == i) continue;
+            const R dz = dr[k].p[2] - d.p[2];
+            if (!(dz > 0.0)) continue;
+            const R dx = dr[k].p[0] - d.p[0], dy = dr[k].p[1] - d.p[1];
+            const R dxy2 = dx * dx + dy * dy;
+            if (!(dxy2 < 100.0)) continue;
+            R dze = dz, ramp = 1.0;
+            if (P.dw_dz_clip > 0.0) {
+                if (dze < P.dw_dz_clip) dze = P.dw_dz_clip;
+                ramp = dz / P.dw_dz_clip;
+                if (ramp > 1.0) ramp = 1.0;
+            }
+            const R ratio = P.r_p / (4.0 * dze);
+            const R alpha = P.dw_C1 * (ratio * ratio);
+            const R beta = P.dw_C2 * dze + P.dw_C3;
+            const R b2 = beta * beta;
+            R e;
+            if (b2 < 1e-12) e = (to_d(dxy2) == 0.0) ? 1.0 : 0.0;
+            else e = exp(-0.5 * dxy2 / b2);
+            d.Fw[2] = d.Fw[2] - ramp * alpha * e;
+        }
+    }
+    if (D.aero & AERO_WIND)
+        for (int a = 0; a < 3; ++a) d.Fw[a] = d.Fw[a] + d.Fwind[a];
+}
+
+// angular acceleration f(q, w) = J^-1 (R(q)^T tau_w - w x J w)  (O8, Q11)
+template <class R>
+inline void ang_acc(const Params& P, const R q[4], const R w[3], const R tau_w[3], R out[3]) {
+    R Rm[3][3], tb[3], Jw[3], c[3];
+    rotmat(q, Rm);
+    matT_vec(Rm, tau_w, tb);
+    for (int a = 0; a < 3; ++a) Jw[a] = P.J[a] * w[a];
+    cross(w, Jw, c);
+    for (int a = 0; a < 3; ++a) out[a] = (tb[a] - c[a]) / P.J[a];
+}
+
+// O8: one physics substep with the wrench frozen in the world frame (Table 1)
+template <class R>
+inline void integrate(const Params& P, const Derived& D, Drone<R>& d) {
+    const double h = D.h;
+    R a[3] = {d.Fw[0] / P.m, d.Fw[1] / P.m, d.Fw[2] / P.m - P.g};
+    if (D.integ == INTEG_RK4) {
+        // translation: classical RK4 on (p, v) with constant acceleration reduces exactly to this
+        for (int i = 0; i < 3; ++i) {
+            d.p[i] = d.p[i] + h * d.v[i] + (0.5 * h * h) * a[i];
+            d.v[i] = d.v[i] + h * a[i];
+        }
+        // rotation: classical RK4 tableau on (q, w_body), stage orientations by Eq.7 from q0
+        R k1[3], k2[3], k3[3], k4[3], q2[4], q3[4], q4[4], w2[3], w3[3], w4[3], ph[3];
+        ang_acc(P, d.q, d.w, d.tw, k1);
+        for (int i = 0; i < 3; ++i) { ph[i] = (0.5 * h) * d.w[i]; w2[i] = d.w[i] + (0.5 * h) * k1[i]; }
+        quat_exp_step(d.q, ph, q2);
+        ang_acc(P, q2, w2, d.tw, k2);
+        for (int i = 0; i < 3; ++i) { ph[i] = (0.5 * h) * w2[i]; w3[i] = d.w[i] + (0.5 * h) * k2[i]; }
+        quat_exp_step(d.q, ph, q3);
+        ang_acc(P, q3, w3, d.tw, k3);
+        for (int i = 0; i < 3; ++i) { ph[i] = h * w3[i]; w4[i] = d.w[i] + h * k3[i]; }
+        quat_exp_step(d.q, ph, q4);
+        ang_acc(P, q4, w4, d.tw, k4);
+        for (int i = 0; i < 3; ++i) ph[i] = (h / 6.0) * (d.w[i] + 2.0 * w2[i] + 2.0 * w3[i] + w4[i]);
+        R qn[4];
+        quat_exp_step(d.q, ph, qn);
+        for (int i = 0; i < 3; ++i) d.w[i] = d.w[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+        for (int i = 0; i < 4; ++i) d.q[i] = qn[i];
+        quat_normalise(d.q);                                       // Q14
+    } else {                                                       // DYN: explicit Euler (Q12)
+        for (int i = 0; i < 3; ++i) { d.v[i] = d.v[i] + h * a[i]; d.p[i] = d.p[i] + h * d.v[i]; }
+        R k1[3], ph[3], qn[4];
+        ang_acc(P, d.q, d.w, d.tw, k1);                            // R(q0)^T tau_w = tau_b
+        for (int i = 0; i < 3; ++i) { d.w[i] = d.w[i] + h * k1[i]; ph[i] = h * d.w[i]; }
+        quat_exp_step(d.q, ph, qn);
+        for (int i = 0; i < 4; ++i) d.q[i] = qn[i];
+        quat_normalise(d.q);
+    }
+    // floor (Q15)
+    const double apz = std::fabs(to_d(d.p[2]));
+    if (apz < d.min_abs_pz) d.min_abs_pz = apz;
+    if (d.p[2] < 0.0) {
+        d.hit = true;
+        d.p[2] = 0.0;
+        if (d.v[2] < 0.0) d.v[2] = 0.0;
+    }
+}
+
+// ---- batched simulator ------------------------------------------------------------------------
+struct Sim {
+    int N, M, physics_mode, action_type;
+    Params P; Derived D;
+    uint64_t seed; uint32_t gstep;
+    std::vector<double> state;    // [D][13] p q v w
+    std::vector<double> pid;      // [D][10] Ip Ie sp
+    std::vector<double> target;   // [D][4]
+    std::vector<double> wind;     // [N][3]
+    std::vector<uint32_t> ep_step;  // [N]
+    std::vector<double> obs;      // [N][M*opd]
+    std::vector<double> reward;   // [N]
+    std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
+    std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
+
+    int opd() const { return 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
+    int obs_dim() const { return M * opd(); }
+
+    void init(int n_envs, int n_drones, int phys, int act, const Params& p) {
+        N = n_envs; M = n_drones; physics_mode = phys; action_type = act; P = p; D = derive(P, phys);
+        seed = 0; gstep = 0;
+        const size_t Dn = (size_t)N * M;
+        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0);
+        wind.assign((size_t)N * 3, 0.0); ep_step.assign(N, 0);
+        obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); done.assign(N, 0);
+        margin.assign((size_t)N * 3, 1e30);
+        for (size_t i = 0; i < Dn; ++i) state[i * 13 + 3] = 1.0;
+    }
+
+    // O11/O12: draw the initial state of env e at control-step index t (K2 `_single_reset`)
+    void reset_env(int e, uint32_t t) {
+        const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+        for (int i = 0; i < M; ++i) {
+            const size_t di = (size_t)e * M + i;
+            double base[3] = {P.reset_center[0], P.reset_center[1], P.reset_center[2]};
+            if (P.reset_layout == LAYOUT_GRID) {
+                const int cols = P.grid_cols, rows = (M + cols - 1) / cols;
+                base[0] += ((i % cols) - 0.5 * (cols - 1)) * P.grid_spacing;
+                base[1] += ((i / cols) - 0.5 * (rows - 1)) * P.grid_spacing;
+            } else if (P.reset_layout == LAYOUT_CIRCLE) {
+                const double ang = 2.0 * PI * i / M;
+                base[0] += P.circle_radius * std::cos(ang);
+                base[1] += P.circle_radius * std::sin(ang);
+            }
+            const PhiloxOut r = philox4x32_10((uint32_t)e, (uint32_t)i, t, STREAM_RESET_POS, k0, k1);
+            double* s = &state[di * 13];
+            s[0] = base[0] + (-P.reset_half[0] + 2.0 * P.reset_half[0] * u01(r.x[0]));
+            s[1] = base[1] + (-P.reset_half[1] + 2.0 * P.reset_half[1] * u01(r.x[1]));
+            if (P.reset_z_hi > P.reset_z_lo) s[2] = P.reset_z_lo + (P.reset_z_hi - P.reset_z_lo) * u01(r.x[2]);
+            else s[2] = base[2] + (-P.reset_half[2] + 2.0 * P.reset_half[2] * u01(r.x[2]));
+            s[3] = 1.0; s[4] = s[5] = s[6] = 0.0;                   // identity attitude
+            for (int a = 7; a < 13; ++a) s[a] = 0.0;                // at rest
+            double* tg = &target[di * 4];
+            tg[3] = 0.0;
+            if (P.target_mode == TGT_FIXED) {
+                tg[0] = P.target_fixed[0]; tg[1] = P.target_fixed[1]; tg[2] = P.target_fixed[2];
+            } else if (P.target_mode == TGT_SPAWN_LINSPACE) {
+                tg[0] = s[0]; tg[1] = s[1];
+                tg[2] = (M > 1) ? P.mh_z_lo + (P.mh_z_hi - P.mh_z_lo) * i / (M - 1) : P.mh_z_lo;
+            } else if (P.target_mode == TGT_BOX) {                  // Q32
+                const PhiloxOut r2 = philox4x32_10((uint32_t)e, (uint32_t)i, t, STREAM_RESET_EXTRA, k0, k1);
+                for (int a = 0; a < 3; ++a) tg[a] = P.target_lo[a] + (P.target_hi[a] - P.target_lo[a]) * u01(r2.x[a]);
+            } else {                                                // TGT_CIRCLE, Q26
+                const double ang = 2.0 * PI * i / M;
+                tg[0] = P.form_center[0] + P.form_radius * std::cos(ang);
+                tg[1] = P.form_center[1] + P.form_radius * std::sin(ang);
+                tg[2] = P.form_center[2];
+            }
+            double* pm = &pid[di * 10];
+            for (int a = 0; a < 6; ++a) pm[a] = 0.0;
+            pm[6] = s[0]; pm[7] = s[1]; pm[8] = s[2]; pm[9] = 0.0;  // held setpoint starts at the spawn pose
+        }
+        wind[(size_t)e * 3 + 0] = wind[(size_t)e * 3 + 1] = wind[(size_t)e * 3 + 2] = 0.0;
+        ep_step[e] = 0;
+    }
+
+    template <class R> void load(int e, Drone<R>* dr) const {
+        for (int i = 0; i < M; ++i) {
+            const size_t di = (size_t)e * M + i;
+            const double* s = &state[di * 13]; const double* pm = &pid[di * 10];
+            Drone<R>& d = dr[i];
+            for (int a = 0; a < 3; ++a) { d.p[a] = s[a]; d.v[a] = s[7 + a]; d.w[a] = s[10 + a]; d.Ip[a] = pm[a]; d.Ie[a] = pm[3 + a]; }
+            for (int a = 0; a < 4; ++a) { d.q[a] = s[3 + a]; d.sp[a] = pm[6 + a]; d.tg[a] = target[di * 4 + a]; }
+            for (int a = 0; a < 3; ++a) d.Fwind[a] = 0.0;
+            d.hit = false; d.min_abs_pz = 1e30;
+        }
+    }
+    template <class R> void store(int e, const Drone<R>* dr) {
+        for (int i = 0; i < M; ++i) {
+            const size_t di = (size_t)e * M + i;
+            double* s = &state[di * 13]; double* pm = &pid[di * 10];
+            const Drone<R>& d = dr[i];
+            for (int a = 0; a < 3; ++a) { s[a] = to_d(d.p[a]); s[7 + a] = to_d(d.v[a]); s[10 + a] = to_d(d.w[a]); pm[a] = to_d(d.Ip[a]); pm[3 + a] = to_d(d.Ie[a]); }
+            for (int a = 0; a < 4; ++a) { s[3 + a] = to_d(d.q[a]); pm[6 + a] = to_d(d.sp[a]); }
+        }
+    }
+
+    // O10: observation of env e from dr (S9: [p, eta, v, w] per drone (+ adjacency row, Q23))
+    template <class R> void write_obs(int e, const Drone<R>* dr, double& adj_margin) {
+        const int od = opd();
+        double* o = &obs[(size_t)e * obs_dim()];
+        adj_margin = 1e30;
+        for (int i = 0; i < M; ++i) {
+            R eta[3];
+            euler_zyx(dr[i].q, eta);
+            double* oi = o + (size_t)i * od;
+            for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[3 + a] = to_d(eta[a]); oi[6 + a] = to_d(dr[i].v[a]); oi[9 + a] = to_d(dr[i].w[a]); }
+            if (P.obs_mode == OBS_KIN12_ADJ) {
+                for (int k = 0; k < M; ++k) {
+                    if (k == i) { oi[12 + k] = 1.0; continue; }
+                    const R dx = dr[i].p[0] - dr[k].p[0], dy = dr[i].p[1] - dr[k].p[1], dz = dr[i].p[2] - dr[k].p[2];
+                    const R dist = sqrt(dx * dx + dy * dy + dz * dz);
+                    oi[12 + k] = (dist < P.adj_radius) ? 1.0 : 0.0;
+                    const double mg = std::fabs(to_d(dist) - P.adj_radius);
+                    if (mg < adj_margin) adj_margin = mg;
+                }
+            }
+        }
+    }
+
+    // one control step of env e (call stack (a)/(b) of SURVEY.md §3)
+    template <class R> void step_env(int e, const float* actions, uint32_t t) {
+        std::vector<Drone<R>> buf(M);
+        Drone<R>* dr = buf.data();
+        load(e, dr);
+        const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+        // O9 wind gust (PAPER.md:203 recursion, Q27), once per control step, before the substeps
+        if (D.aero & AERO_WIND) {
+            const PhiloxOut r = philox4x32_10((uint32_t)e, ENV_LEVEL, t, STREAM_WIND, k0, k1);
+            const double ua = u01(r.x[0]), ub = u01(r.x[1]), uc = u01(r.x[2]), ud = u01(r.x[3]);
+            const R r1 = sqrt(-2.0 * log(R(1.0 - ua))), r2 = sqrt(-2.0 * log(R(1.0 - uc)));   // Box-Muller
+            const R xi[3] = {r1 * cos(R(2.0 * PI * ub)), r1 * sin(R(2.0 * PI * ub)), r2 * cos(R(2.0 * PI * ud))};
+            const double alpha = std::exp(-D.dt_c / P.wind_tau);
+            const double gain = P.wind_sigma * std::sqrt(1.0 - alpha * alpha);
+            R w[3];
+            for (int a = 0; a < 3; ++a) { w[a] = alpha * R(wind[(size_t)e * 3 + a]) + gain * xi[a]; wind[(size_t)e * 3 + a] = to_d(w[a]); }
+            for (int i = 0; i < M; ++i) {                          // PAPER.md:201 drag law, Q28
+                R rel[3] = {w[0] - dr[i].v[0], w[1] - dr[i].v[1], w[2] - dr[i].v[2]};
+                const R nr = sqrt(rel[0] * rel[0] + rel[1] * rel[1] + rel[2] * rel[2]);
+                for (int a = 0; a < 3; ++a) dr[i].Fwind[a] = (P.k_wind * nr) * rel[a];
+            }
+        }
+        // O2/O3 decode, O4 motor model
+        for (int i = 0; i < M; ++i) {
+            decode_action(P, D, action_type, actions + ((size_t)e * M + i) * 4, dr[i]);
+            motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om);
+        }
+        // K substeps: all wrenches from the same start-of-substep state, then integrate
+        for (int k = 0; k < D.K; ++k) {
+            for (int i = 0; i < M; ++i) substep_wrench(P, D, dr, M, i);
+            for (int i = 0; i < M; ++i) integrate(P, D, dr[i]);
+        }
+        store(e, dr);
+        // O10 reward / termination from the end-of-step state
+        const bool use_floor = P.term_mode == TERM_HOVER || P.term_mode == TERM_FORMATION;
+        const bool use_tilt = P.term_mode != TERM_NONE;
+        const bool use_zmax = use_floor;
+        const bool use_dist = P.term_mode == TERM_TILT_DIST || P.term_mode == TERM_FORMATION;
+        double m_done = 1e30, m_rew = 1e30;
+        bool terminated = false;
+        R rew = 0.0;
+        for (int i = 0; i < M; ++i) {
+            const Drone<R>& d = dr[i];
+            R eta[3];
+            euler_zyx(d.q, eta);
+            const R aphi = fabs(eta[0]), ath = fabs(eta[1]);
+            bool crash = false;
+            if (use_floor) { if (d.hit) { terminated = true; crash = true; } if (d.min_abs_pz < m_done) m_done = d.min_abs_pz; }
+            if (use_tilt) {                                         // PAPER.md:309 / config 3
+                if (aphi > P.term_tilt || ath > P.term_tilt) { terminated = true; crash = true; }
+                m_done = std::fmin(m_done, std::fmin(std::fabs(to_d(aphi) - P.term_tilt), std::fabs(to_d(ath) - P.term_tilt)));
+            }
+            if (use_zmax) {
+                if (d.p[2] > P.z_max) terminated = true;
+                m_done = std::fmin(m_done, std::fabs(to_d(d.p[2]) - P.z_max));
+            }
+            if (use_dist) {
+                const R dx = d.p[0] - P.term_center[0], dy = d.p[1] - P.term_center[1], dz = d.p[2] - P.term_center[2];
+                const R dist = sqrt(dx * dx + dy * dy + dz * dz);
+                if (dist > P.term_dist) terminated = true;
+                m_done = std::fmin(m_done, std::fabs(to_d(dist) - P.term_dist));
+            }
+            const R ex = d.p[0] - d.tg[0], ey = d.p[1] - d.tg[1], ez = d.p[2] - d.tg[2];
+            if (P.reward_mode == REW_HOVER || P.reward_mode == REW_MULTI_HOVER) {      // Eq.8, 317
+                const R dist = sqrt(ex * ex + ey * ey + ez * ez);
+                const R speed = sqrt(d.v[0] * d.v[0] + d.v[1] * d.v[1] + d.v[2] * d.v[2]);
+                R r = -fabs(ez) - 0.1 * sqrt(ex * ex + ey * ey) - 0.05 * speed - 0.05 * (aphi + ath);
+                if (dist < P.at_target_radius) r = r + 0.5;
+                if (crash) r = r - 100.0;
+                m_rew = std::fmin(m_rew, std::fabs(to_d(dist) - P.at_target_radius));
+                rew = rew + r;
+            } else if (P.reward_mode == REW_NEG_SQ_DIST) {          // config 3
+                rew = rew - (ex * ex + ey * ey + ez * ez);
+            } else {                                                // REW_FORMATION (Q26)
+                rew = rew - sqrt(ex * ex + ey * ey + ez * ez);
+                for (int k = i + 1; k < M; ++k) {
+                    const R ax = d.p[0] - dr[k].p[0], ay = d.p[1] - dr[k].p[1], az = d.p[2] - dr[k].p[2];
+                    const double bx = d.tg[0] - dr[k].tg[0], by = d.tg[1] - dr[k].tg[1], bz = d.tg[2] - dr[k].tg[2];
+                    const R dact = sqrt(ax * ax + ay * ay + az * az);
+                    const double ddes = std::sqrt(bx * bx + by * by + bz * bz);
+                    rew = rew - 0.5 * fabs(dact - ddes);
+                }
+            }
+        }
+        ep_step[e] += 1;
+        const bool truncated = D.ep_steps > 0 && (int)ep_step[e] >= D.ep_steps;
+        reward[e] = to_d(rew);
+        done[e] = (uint8_t)((terminated ? 1 : 0) | (truncated ? 2 : 0));
+        // O11 auto-reset (Q29): reward/done describe the finished transition, obs opens the new episode
+        if (done[e] && P.auto_reset) {
+            reset_env(e, t);
+            load(e, dr);
+        }
+        double m_adj;
+        write_obs(e, dr, m_adj);
+        margin[(size_t)e * 3 + 0] = m_done; margin[(size_t)e * 3 + 1] = m_rew; margin[(size_t)e * 3 + 2] = m_adj;
+    }
+
+    void reset_all(uint64_t s) {
+        seed = s; gstep = 0;
+        std::vector<Drone<double>> buf(M);
+        for (int e = 0; e < N; ++e) {
+            reset_env(e, 0);
+            load(e, buf.data());
+            double m_adj;
+            write_obs(e, buf.data(), m_adj);
+            reward[e] = 0.0; done[e] = 0;
+            margin[(size_t)e * 3 + 0] = margin[(size_t)e * 3 + 1] = 1e30; margin[(size_t)e * 3 + 2] = m_adj;
+        }
+    }
+    template <class R> void step_range(int e0, int e1, const float* actions, uint32_t t) {
+        for (int e = e0; e < e1; ++e) step_env<R>(e, actions, t);
+    }
+};
+
+}  // namespace orc

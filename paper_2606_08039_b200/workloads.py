@@ -1,0 +1,80 @@
+"""Seeded synthetic workload recipes — data only.
+
+This module serves both the CUDA path and the oracle and therefore holds none of the method's
+arithmetic: each recipe is the constructor arguments plus a dict of parameter overrides keyed by the
+field names that `include/mdg.h:mdg_params` and the oracle's parameter block both use, and a
+description of how the harness draws actions.  It imports neither side.
+"""
+import math
+
+BASE_SEED = 260608039
+
+# interface enum values (include/mdg.h; Table 1, 179-187 Table 3)
+AERO_GND, AERO_DRAG, AERO_DW, AERO_WIND = 1, 2, 4, 8
+INTEG_RK4, INTEG_EULER = 0, 1
+PHYS_MJC, PHYS_MJC_GND, PHYS_MJC_DRAG, PHYS_MJC_DW, PHYS_MJC_GND_DRAG_DW, PHYS_DYN = range(6)
+ACT_RPM, ACT_PID, ACT_VEL = 0, 1, 2
+OBS_KIN12, OBS_KIN12_ADJ = 0, 1
+REW_HOVER, REW_NEG_SQ_DIST, REW_MULTI_HOVER, REW_FORMATION = 0, 1, 2, 3
+TERM_NONE, TERM_HOVER, TERM_TILT_DIST, TERM_FORMATION = 0, 1, 2, 3
+LAYOUT_NONE, LAYOUT_GRID, LAYOUT_CIRCLE = 0, 1, 2
+TGT_FIXED, TGT_SPAWN_LINSPACE, TGT_BOX, TGT_CIRCLE = 0, 1, 2, 3
+MODEL_CF2X, MODEL_RACE = 0, 2
+
+_DSL = dict(dsl=1, int_clamp_pos=1.0, int_clamp_att=0.25)      # halved clamps + rate limits
+
+
+class Workload:
+    def __init__(self, name, n_envs, n_drones, physics_mode, action_type, params, actions, steps, seed):
+        self.name, self.n_envs, self.n_drones = name, n_envs, n_drones
+        self.physics_mode, self.action_type = physics_mode, action_type
+        self.params = params          # {field: scalar | list}
+        self.actions = actions        # ("hover_scale", lo, hi) | ("uniform", lo, hi) | ("targets",)
+        self.steps, self.seed = steps, seed
+
+    def scaled(self, n_envs):
+        return Workload(self.name, n_envs, self.n_drones, self.physics_mode, self.action_type,
+                        dict(self.params), self.actions, self.steps, self.seed)
+
+
+def config(c: int) -> Workload:
+    """The five BASELINE.json configs, c = 1..5 (seed = BASE_SEED + c)."""
+    s = BASE_SEED + c
+    if c == 1:      # 1 env x 1 CF2X, pure rigid body, RPM = hover x U[0.95, 1.05]
+        return Workload("c1", 1, 1, PHYS_MJC, ACT_RPM, dict(
+            reset_layout=LAYOUT_NONE, reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1],
+            reward_mode=REW_HOVER, term_mode=TERM_HOVER, target_mode=TGT_FIXED, target_fixed=[0, 0, 1],
+            episode_len_s=10.0, auto_reset=1), ("hover_scale", 0.95, 1.05), 1000, s)
+    if c == 2:      # 4,096 x 1, ground effect + drag, z0 ~ U[0.05, 1.5]
+        return Workload("c2", 4096, 1, PHYS_MJC, ACT_RPM, dict(
+            aero_mask=AERO_GND | AERO_DRAG,
+            reset_layout=LAYOUT_NONE, reset_center=[0, 0, 0], reset_half=[0, 0, 0], reset_z_lo=0.05, reset_z_hi=1.5,
+            reward_mode=REW_HOVER, term_mode=TERM_HOVER, target_mode=TGT_FIXED, target_fixed=[0, 0, 1],
+            episode_len_s=10.0, auto_reset=1), ("hover_scale", 0.9, 1.1), 2000, s)
+    if c == 3:      # 16,384 x 1, PID waypoint (DSL flags), -|p-p*|^2, config-3 termination
+        return Workload("c3", 16384, 1, PHYS_MJC, ACT_PID, dict(
+            reset_layout=LAYOUT_NONE, reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1],
+            reward_mode=REW_NEG_SQ_DIST, term_mode=TERM_TILT_DIST, term_tilt=0.4, term_dist=3.0, term_center=[0, 0, 0],
+            target_mode=TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
+            episode_len_s=10.0, auto_reset=1, **_DSL), ("targets",), 1000, s)
+    if c == 4:      # 1,024 x 8, all-pairs downwash + ground + drag, 4x2 grid, multi-hover
+        return Workload("c4", 1024, 8, PHYS_MJC_GND_DRAG_DW, ACT_RPM, dict(
+            reset_layout=LAYOUT_GRID, grid_cols=4, grid_spacing=0.3, reset_center=[0, 0, 0],
+            reset_half=[0.05, 0.05, 0], reset_z_lo=0.3, reset_z_hi=1.2,
+            reward_mode=REW_MULTI_HOVER, term_mode=TERM_HOVER, target_mode=TGT_SPAWN_LINSPACE, mh_z_lo=0.7, mh_z_hi=1.2,
+            episode_len_s=10.0, auto_reset=1), ("hover_scale", 0.9, 1.1), 2000, s)
+    if c == 5:      # 65,536 x 4, all aero + wind, VEL through the PID, adjacency obs, formation
+        return Workload("c5", 65536, 4, PHYS_MJC_GND_DRAG_DW, ACT_VEL, dict(
+            aero_mask=AERO_GND | AERO_DRAG | AERO_DW | AERO_WIND, wind_sigma=0.5, wind_tau=1.0,
+            reset_layout=LAYOUT_CIRCLE, circle_radius=0.3, reset_center=[0, 0, 1], reset_half=[0.05, 0.05, 0.05],
+            obs_mode=OBS_KIN12_ADJ, adj_radius=0.5,
+            reward_mode=REW_FORMATION, term_mode=TERM_FORMATION, term_center=[0, 0, 1], term_dist=3.0,
+            target_mode=TGT_CIRCLE, form_center=[0, 0, 1], form_radius=0.3,
+            episode_len_s=30.0, auto_reset=1, **_DSL), ("uniform", -1.0, 1.0), 500, s)
+    raise ValueError(c)
+
+
+def hover_rpm_f32(m=0.027, g=9.81, k_f=3.16e-10):
+    """Harness scale for ("hover_scale", ...) actions: the CF2X hover rotor speed rounded to fp32."""
+    import struct
+    return struct.unpack("f", struct.pack("f", math.sqrt(m * g / (4.0 * k_f))))[0]
