@@ -1,0 +1,138 @@
+/* mdg.h — C ABI of the B200-native batched drone-environment step (libmdg.so).
+ *
+ * One call advances thousands of independent environments, each holding M Crazyflie-class quadrotors,
+ * by one control step of arxiv/paper_2606_08039 ("MuJoCo-Drones-Gym"): action decode (PAPER.md:171-187
+ * Table 3; cascaded PID PAPER.md:347-376), rotor model (Eq.1-3), ground effect / blade
+ * drag / downwash (Eq.4-6), wind gust, free-body integration over
+ * sim_freq/ctrl_freq substeps, observation, reward, termination and
+ * auto-reset.  The interface follows the paper's statement of the
+ * simulator: constructor options, `reset(rng) -> state`,
+ * `step(state, action) -> state, obs, reward, done`.
+ *
+ * Conventions
+ *  - Every function returns 0 (MDG_OK) or a negative error code; no exception or abort crosses the ABI.
+ *    mdg_last_error() returns a thread-local description of the last failure.
+ *  - "dev" pointers are CUDA device pointers on the device that was current at mdg_create; "host"
+ *    pointers are ordinary host memory.  Library-owned buffers stay valid until mdg_destroy.
+ *  - mdg_step / mdg_step_many / mdg_reset / mdg_gen_actions are asynchronous on the bound stream
+ *    (default: the legacy default stream) and never synchronise.  mdg_get_* / mdg_set_* synchronise it.
+ *  - A handle is not thread-safe; distinct handles are independent.
+ *  - There is no CPU fallback: without a CUDA device mdg_create fails with MDG_ECUDA.
+ */
+#ifndef MDG_H
+#define MDG_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MDG_OK 0
+#define MDG_EINVAL (-1) /* bad argument (n_envs<1, n_drones<1 or >32, unknown enum, sim_freq not a multiple of ctrl_freq) */
+#define MDG_ECUDA (-2)  /* CUDA runtime error */
+#define MDG_ENOMEM (-3) /* allocation failed */
+
+/* aerodynamic feature mask ("toggled independently") */
+enum { MDG_AERO_GND = 1, MDG_AERO_DRAG = 2, MDG_AERO_DW = 4, MDG_AERO_WIND = 8 };
+enum { MDG_INTEG_RK4 = 0, MDG_INTEG_EULER = 1 };
+/* Table 1 */
+enum { MDG_PHYS_MJC = 0, MDG_PHYS_MJC_GND = 1, MDG_PHYS_MJC_DRAG = 2, MDG_PHYS_MJC_DW = 3,
+       MDG_PHYS_MJC_GND_DRAG_DW = 4, MDG_PHYS_DYN = 5 };
+/* Table 3; ONE_D_RPM and ATTITUDE are not built yet */
+enum { MDG_ACT_RPM = 0, MDG_ACT_PID = 1, MDG_ACT_VEL = 2 };
+enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1 };
+enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3 };
+enum { MDG_TERM_NONE = 0, MDG_TERM_HOVER = 1, MDG_TERM_TILT_DIST = 2, MDG_TERM_FORMATION = 3 };
+enum { MDG_LAYOUT_NONE = 0, MDG_LAYOUT_GRID = 1, MDG_LAYOUT_CIRCLE = 2 };
+enum { MDG_TGT_FIXED = 0, MDG_TGT_SPAWN_LINSPACE = 1, MDG_TGT_BOX = 2, MDG_TGT_CIRCLE = 3 };
+enum { MDG_MODEL_CF2X = 0, MDG_MODEL_RACE = 2 };                /* Table 2 */
+
+/* Plain-old-data parameter block.  struct_size must equal sizeof(mdg_params) (set by
+ * mdg_default_params); units SI, rotor speeds in RPM, k_f and k_m per RPM^2 (DESIGN.md §3 Q1). */
+typedef struct mdg_params {
+    uint32_t struct_size;
+    int32_t drone_model;
+    /* Table 2 */
+    float m, g, L, k_f, k_m, J[3], r_p, tw_ratio;
+    /* Eq.4-6 coefficients; h_clip and dw_dz_clip regularise the h->0 and dz->0 singularities */
+    float C_gnd, h_clip, c_xy, c_z, dw_C1, dw_C2, dw_C3, dw_dz_clip;
+    /* wind gust: F = k_wind |w - v| (w - v); w <- a w + sigma sqrt(1-a^2) xi, a = exp(-dt_c/tau) */
+    float k_wind, wind_sigma, wind_tau;
+    int32_t sim_freq, ctrl_freq;   /* substeps per step = sim_freq / ctrl_freq */
+    int32_t aero_mask, integrator; /* -1: derive from physics_mode (Table 1) */
+    /* cascaded PID (Eq.9, Table 6) */
+    float Kp_pos[3], Ki_pos[3], Kd_pos[3], Kp_att[3], Ki_att[3], Kd_att[3];
+    float int_clamp_pos, int_clamp_att;
+    int32_t dsl;                   /* 1: DSL-PID setpoint rate limits */
+    float pos_rate_limit, yaw_rate_limit, a_ff[3], tilt_max, tau_xy_max, tau_z_max;
+    /* observation, reward, termination */
+    int32_t obs_mode; float adj_radius;
+    int32_t reward_mode; float at_target_radius;
+    int32_t term_mode; float term_tilt, term_dist, term_center[3], z_max;
+    float episode_len_s; int32_t auto_reset;
+    /* reset distribution and per-episode targets */
+    int32_t reset_layout; float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi;
+    int32_t grid_cols; float grid_spacing, circle_radius;
+    int32_t target_mode; float target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi,
+        form_center[3], form_radius;
+} mdg_params;
+
+typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */
+
+/* Fill *out with Table 2 (drone_model), Table 6 and the documented defaults.  host pointer. */
+int mdg_default_params(int drone_model, mdg_params* out);
+
+/* Create n_envs environments of n_drones (1..32) drones each.  physics_mode: Table 1; action_type:
+ * Table 3.  params (host, copied) may be NULL for the CF2X defaults.  *out receives the handle. */
+int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, const mdg_params* params,
+               mdg_env** out);
+void mdg_destroy(mdg_env* env);
+
+/* Draw every env's initial state from Philox4x32-10 keyed by seed (counter = env, drone, 0, stream);
+ * zero controller memory, wind and step counters; obs is valid afterwards (reward 0, done 0). */
+int mdg_reset(mdg_env* env, uint64_t seed);
+
+/* One control step.  actions_dev: [n_envs*n_drones][4] fp32, caller-owned device memory, read only.
+ * RPM: raw rotor speeds (clipped to [0, MAX_RPM]); PID: waypoint [x,y,z,psi]; VEL: [vx,vy,vz,wz]. */
+int mdg_step(mdg_env* env, const float* actions_dev);
+
+/* n_steps control steps replayed as one CUDA graph: step k reads actions_dev + k*stride_floats.
+ * The graph is cached per (pointer, n_steps, stride).  Outputs hold the last step's values. */
+int mdg_step_many(mdg_env* env, const float* actions_dev, int n_steps, int64_t stride_floats);
+
+/* Device pointers to the library-owned outputs of the last reset/step:
+ * obs [n_envs][mdg_obs_dim] fp32 (per drone: p, roll/pitch/yaw, v, body rates [, adjacency row]);
+ * reward [n_envs] fp32; done [n_envs] u8 (bit0 terminated, bit1 truncated).  Any may be NULL. */
+int mdg_outputs(mdg_env* env, const float** obs_dev, const float** reward_dev, const uint8_t** done_dev);
+int mdg_obs_dim(const mdg_env* env); /* floats per env */
+
+/* Device pointer to the per-episode targets [n_envs*n_drones][4] = (x, y, z, psi), fp32. */
+int mdg_targets(mdg_env* env, const float** targets_dev);
+
+/* Harness action generator (Philox stream 3, counter = env, drone, t, 3):
+ * out_dev[(e*n_drones+i)*4 + c] = base * fma(hi - lo, u_c, lo), every operation rounded to fp32. */
+int mdg_gen_actions(mdg_env* env, uint64_t seed, uint32_t t, float base, float lo, float hi, float* out_dev);
+
+/* Checkpoint / test hooks (host pointers; synchronise the stream).
+ * state: [D][13] = p(3) q(4, w x y z) v(3) body rates(3);  ctrl: [D][10] = I_p(3) I_eta(3) held
+ * setpoint(4);  targets: [D][4];  wind: [n_envs][3];  ep_step: [n_envs] u32.  D = n_envs*n_drones.
+ * NULL pointers are skipped.  mdg_set_state recomputes obs. */
+int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float* wind, uint32_t* ep_step);
+int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
+                  const float* wind, const uint32_t* ep_step);
+
+/* Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) used by later calls. */
+int mdg_set_stream(mdg_env* env, void* cuda_stream);
+
+/* Introspection: kernels launched so far through this handle; name of the step kernel specialisation. */
+int64_t mdg_launch_count(const mdg_env* env);
+const char* mdg_kernel_name(const mdg_env* env);
+/* Launch shape tuning (0 keeps the current value): threads per block, and a cap on resident blocks per SM. */
+int mdg_set_launch(mdg_env* env, int block_threads, int max_blocks_per_sm);
+
+const char* mdg_last_error(void);
+int mdg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MDG_H */

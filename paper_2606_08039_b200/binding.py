@@ -1,0 +1,216 @@
+"""Thin ctypes binding of libmdg.so — argument marshalling only; every step of the path runs in the
+CUDA kernels behind the C ABI of include/mdg.h.  Function names mirror the C names (mdg_step -> step).
+"""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libmdg.so")
+
+MDG_OK, MDG_EINVAL, MDG_ECUDA, MDG_ENOMEM = 0, -1, -2, -3
+
+
+class mdg_params(C.Structure):
+    """Mirror of `struct mdg_params` (include/mdg.h)."""
+    _F3 = C.c_float * 3
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("drone_model", C.c_int32),
+        ("m", C.c_float), ("g", C.c_float), ("L", C.c_float), ("k_f", C.c_float), ("k_m", C.c_float),
+        ("J", _F3), ("r_p", C.c_float), ("tw_ratio", C.c_float),
+        ("C_gnd", C.c_float), ("h_clip", C.c_float), ("c_xy", C.c_float), ("c_z", C.c_float),
+        ("dw_C1", C.c_float), ("dw_C2", C.c_float), ("dw_C3", C.c_float), ("dw_dz_clip", C.c_float),
+        ("k_wind", C.c_float), ("wind_sigma", C.c_float), ("wind_tau", C.c_float),
+        ("sim_freq", C.c_int32), ("ctrl_freq", C.c_int32), ("aero_mask", C.c_int32), ("integrator", C.c_int32),
+        ("Kp_pos", _F3), ("Ki_pos", _F3), ("Kd_pos", _F3), ("Kp_att", _F3), ("Ki_att", _F3), ("Kd_att", _F3),
+        ("int_clamp_pos", C.c_float), ("int_clamp_att", C.c_float), ("dsl", C.c_int32),
+        ("pos_rate_limit", C.c_float), ("yaw_rate_limit", C.c_float), ("a_ff", _F3),
+        ("tilt_max", C.c_float), ("tau_xy_max", C.c_float), ("tau_z_max", C.c_float),
+        ("obs_mode", C.c_int32), ("adj_radius", C.c_float), ("reward_mode", C.c_int32), ("at_target_radius", C.c_float),
+        ("term_mode", C.c_int32), ("term_tilt", C.c_float), ("term_dist", C.c_float), ("term_center", _F3), ("z_max", C.c_float),
+        ("episode_len_s", C.c_float), ("auto_reset", C.c_int32),
+        ("reset_layout", C.c_int32), ("reset_center", _F3), ("reset_half", _F3), ("reset_z_lo", C.c_float), ("reset_z_hi", C.c_float),
+        ("grid_cols", C.c_int32), ("grid_spacing", C.c_float), ("circle_radius", C.c_float),
+        ("target_mode", C.c_int32), ("target_fixed", _F3), ("target_lo", _F3), ("target_hi", _F3),
+        ("mh_z_lo", C.c_float), ("mh_z_hi", C.c_float), ("form_center", _F3), ("form_radius", C.c_float),
+    ]
+
+    def update(self, d):
+        for k, v in d.items():
+            cur = getattr(self, k)          # raises AttributeError on an unknown field
+            if isinstance(cur, C.Array):
+                for i, x in enumerate(v):
+                    cur[i] = x
+            else:
+                setattr(self, k, v)
+        return self
+
+
+EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_outputs",
+           "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
+           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_last_error", "mdg_version"]
+
+_lib = None
+
+
+def lib():
+    """Load libmdg.so; fails loudly when the CUDA extension has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_08039_b200.build` "
+                               "(nvcc, sm_100a). There is no CPU fallback.")
+        L = C.CDLL(LIB_PATH)
+        vp, PP = C.c_void_p, C.POINTER(mdg_params)
+        L.mdg_default_params.argtypes = [C.c_int, PP]
+        L.mdg_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, PP, C.POINTER(vp)]
+        L.mdg_destroy.argtypes = [vp]
+        L.mdg_destroy.restype = None
+        L.mdg_reset.argtypes = [vp, C.c_uint64]
+        L.mdg_step.argtypes = [vp, vp]
+        L.mdg_step_many.argtypes = [vp, vp, C.c_int, C.c_int64]
+        L.mdg_outputs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+        L.mdg_obs_dim.argtypes = [vp]
+        L.mdg_targets.argtypes = [vp, C.POINTER(vp)]
+        L.mdg_gen_actions.argtypes = [vp, C.c_uint64, C.c_uint32, C.c_float, C.c_float, C.c_float, vp]
+        L.mdg_get_state.argtypes = [vp] * 6
+        L.mdg_set_state.argtypes = [vp] * 6
+        L.mdg_set_stream.argtypes = [vp, vp]
+        L.mdg_launch_count.argtypes = [vp]
+        L.mdg_launch_count.restype = C.c_int64
+        L.mdg_kernel_name.argtypes = [vp]
+        L.mdg_kernel_name.restype = C.c_char_p
+        L.mdg_set_launch.argtypes = [vp, C.c_int, C.c_int]
+        L.mdg_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+class MdgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"mdg error {code}: {msg}")
+        self.code = code
+
+
+def _check(rc):
+    if rc != MDG_OK:
+        raise MdgError(rc, lib().mdg_last_error().decode())
+
+
+def default_params(drone_model=0, **overrides) -> mdg_params:
+    p = mdg_params()
+    _check(lib().mdg_default_params(drone_model, C.byref(p)))
+    return p.update(overrides)
+
+
+class _DevArray:
+    """Zero-copy view of library-owned device memory for torch.as_tensor (CUDA array interface v3)."""
+
+    def __init__(self, ptr, shape, typestr, owner):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (int(ptr), False),
+                                         "version": 3, "strides": None}
+        self._owner = owner
+
+
+class Env:
+    """create / reset / step of the batched drone env on the current CUDA device.
+
+    PyTorch supplies device memory and streams only: `step(actions)` takes a CUDA float32 tensor of
+    shape [n_envs*n_drones, 4] (or anything reshapeable to it) and `obs`, `reward`, `done` are zero-copy
+    tensor views of the library's output buffers.
+    """
+
+    def __init__(self, n_envs, n_drones, physics_mode, action_type, params: mdg_params = None, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_08039_b200 needs a CUDA device: there is no CPU fallback")
+        self._torch = torch
+        self.n_envs, self.n_drones = n_envs, n_drones
+        self.params = params if params is not None else default_params()
+        h = C.c_void_p()
+        _check(lib().mdg_create(n_envs, n_drones, physics_mode, action_type, C.byref(self.params), C.byref(h)))
+        self._h = h
+        self.obs_dim = lib().mdg_obs_dim(h)
+        o, r, d, t = C.c_void_p(), C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _check(lib().mdg_outputs(h, C.byref(o), C.byref(r), C.byref(d)))
+        _check(lib().mdg_targets(h, C.byref(t)))
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.obs = torch.as_tensor(_DevArray(o.value, (n_envs, self.obs_dim), "<f4", self), device=dev)
+        self.reward = torch.as_tensor(_DevArray(r.value, (n_envs,), "<f4", self), device=dev)
+        self.done = torch.as_tensor(_DevArray(d.value, (n_envs,), "|u1", self), device=dev)
+        self.targets = torch.as_tensor(_DevArray(t.value, (n_envs * n_drones, 4), "<f4", self), device=dev)
+        self.set_stream(stream if stream is not None else torch.cuda.current_stream())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().mdg_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_stream(self, stream):
+        _check(lib().mdg_set_stream(self._h, C.c_void_p(stream.cuda_stream)))
+
+    def set_launch(self, block_threads=0, max_blocks_per_sm=0):
+        _check(lib().mdg_set_launch(self._h, block_threads, max_blocks_per_sm))
+
+    def reset(self, seed):
+        _check(lib().mdg_reset(self._h, int(seed)))
+        return self.obs
+
+    def _act_ptr(self, actions, steps=1):
+        t = self._torch
+        if not (isinstance(actions, t.Tensor) and actions.is_cuda and actions.dtype == t.float32 and actions.is_contiguous()):
+            raise TypeError("actions must be a contiguous CUDA float32 tensor")
+        if actions.numel() != steps * self.n_envs * self.n_drones * 4:
+            raise ValueError("actions must hold n_envs*n_drones*4 floats per step")
+        return C.c_void_p(actions.data_ptr())
+
+    def step(self, actions):
+        _check(lib().mdg_step(self._h, self._act_ptr(actions)))
+        return self.obs, self.reward, self.done
+
+    def step_many(self, actions, n_steps):
+        """n_steps control steps replayed as one CUDA graph; actions: [n_steps, n_envs*n_drones, 4]."""
+        _check(lib().mdg_step_many(self._h, self._act_ptr(actions, n_steps), n_steps, self.n_envs * self.n_drones * 4))
+        return self.obs, self.reward, self.done
+
+    def gen_actions(self, seed, t, base, lo, hi, out=None):
+        if out is None:
+            out = self._torch.empty((self.n_envs * self.n_drones, 4), dtype=self._torch.float32, device=self.obs.device)
+        _check(lib().mdg_gen_actions(self._h, int(seed), int(t), float(base), float(lo), float(hi), C.c_void_p(out.data_ptr())))
+        return out
+
+    def get_state(self):
+        import numpy as np
+        D = self.n_envs * self.n_drones
+        st, ct, tg = np.zeros((D, 13), np.float32), np.zeros((D, 10), np.float32), np.zeros((D, 4), np.float32)
+        wd, ep = np.zeros((self.n_envs, 3), np.float32), np.zeros(self.n_envs, np.uint32)
+        _check(lib().mdg_get_state(self._h, *[C.c_void_p(a.ctypes.data) for a in (st, ct, tg, wd, ep)]))
+        return dict(state=st, ctrl=ct, targets=tg, wind=wd, ep_step=ep)
+
+    def set_state(self, state=None, ctrl=None, targets=None, wind=None, ep_step=None):
+        import numpy as np
+        D = self.n_envs * self.n_drones
+        spec = ((state, (D, 13), np.float32), (ctrl, (D, 10), np.float32), (targets, (D, 4), np.float32),
+                (wind, (self.n_envs, 3), np.float32), (ep_step, (self.n_envs,), np.uint32))
+        keep, ptrs = [], []
+        for a, shape, dt in spec:
+            if a is None:
+                ptrs.append(C.c_void_p(None))
+            else:
+                b = np.ascontiguousarray(a, dtype=dt).reshape(shape)
+                keep.append(b)
+                ptrs.append(C.c_void_p(b.ctypes.data))
+        _check(lib().mdg_set_state(self._h, *ptrs))
+
+    @property
+    def launch_count(self):
+        return int(lib().mdg_launch_count(self._h))
+
+    @property
+    def kernel_name(self):
+        return lib().mdg_kernel_name(self._h).decode()

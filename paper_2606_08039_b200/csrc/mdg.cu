@@ -1,0 +1,432 @@
+// mdg.cu — host side of libmdg.so: the C ABI of include/mdg.h, the SoA allocator, parameter
+// preprocessing, kernel dispatch and CUDA-graph replay.  No CPU fallback: every step runs in the
+// kernels of mdg_kernels.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "../../include/mdg.h"
+#include "mdg_kernels.cuh"
+
+using namespace mdg;
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t _e = (call);                                                                   \
+        if (_e != cudaSuccess)                                                                     \
+            return fail(_e == cudaErrorMemoryAllocation ? MDG_ENOMEM : MDG_ECUDA,                  \
+                        std::string(#call) + ": " + cudaGetErrorString(_e));                       \
+    } while (0)
+
+typedef void (*step_fn)(const DevParams, const DevBuffers, const float4*);
+typedef void (*aux_fn)(const DevParams, const DevBuffers);
+
+struct mdg_env {
+    int N, M, G, physics_mode, action_type;
+    mdg_params hp;
+    DevParams P;
+    DevBuffers B;
+    void* arena = nullptr;
+    size_t arena_bytes = 0;
+    cudaStream_t stream = 0;
+    cudaStream_t capture_stream = nullptr;
+    step_fn step = nullptr;
+    aux_fn reset = nullptr, refresh = nullptr;
+    std::string kernel_name;
+    int block = 128, max_blocks_per_sm = 0, smem = 0;
+    int64_t launches = 0;
+    std::map<std::tuple<const void*, int, int64_t>, cudaGraphExec_t> graphs;
+};
+
+static int feature_word(const mdg_params& p, int physics_mode, int action_type) {
+    int aero = 0, integ = MDG_INTEG_RK4;                  // Table 1
+    switch (physics_mode) {
+        case MDG_PHYS_MJC_GND: aero = MDG_AERO_GND; break;
+        case MDG_PHYS_MJC_DRAG: aero = MDG_AERO_DRAG; break;
+        case MDG_PHYS_MJC_DW: aero = MDG_AERO_DW; break;
+        case MDG_PHYS_MJC_GND_DRAG_DW: aero = MDG_AERO_GND | MDG_AERO_DRAG | MDG_AERO_DW; break;
+        case MDG_PHYS_DYN: integ = MDG_INTEG_EULER; break;
+        default: break;
+    }
+    if (p.aero_mask >= 0) aero = p.aero_mask & 15;
+    if (p.integrator >= 0) integ = p.integrator;
+    int f = aero;
+    if (integ == MDG_INTEG_EULER) f |= F_EULER;
+    f |= action_type << F_ACT_SHIFT;
+    if (action_type == MDG_ACT_PID && p.dsl) f |= F_DSL;
+    if (p.obs_mode == MDG_OBS_KIN12_ADJ) f |= F_ADJ;
+    f |= p.reward_mode << F_REW_SHIFT;
+    f |= p.term_mode << F_TERM_SHIFT;
+    return f;
+}
+
+// host double -> device fp32 constants (O1 of DESIGN.md §2)
+static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevParams& D) {
+    std::memset(&D, 0, sizeof(D));
+    const double W = (double)p.m * p.g;
+    const double hover2 = W / (4.0 * p.k_f);
+    const double max_rpm = std::sqrt((double)p.tw_ratio * hover2);
+    const double h = 1.0 / p.sim_freq, dtc = 1.0 / p.ctrl_freq;
+    D.N = N; D.M = M; D.K = p.sim_freq / p.ctrl_freq;
+    D.ep_steps = (int)std::llround((double)p.episode_len_s * p.ctrl_freq);
+    D.auto_reset = p.auto_reset; D.feat = feat;
+    D.reset_layout = p.reset_layout; D.target_mode = p.target_mode;
+    D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
+    D.opd = 12 + ((feat & F_ADJ) ? M : 0);
+    D.h = (float)h; D.half_h = (float)(0.5 * h); D.h_sixth = (float)(h / 6.0); D.half_h2 = (float)(0.5 * h * h);
+    D.inv_m = (float)(1.0 / p.m); D.g = p.g; D.m = p.m; D.inv_g = (float)(1.0 / p.g);
+    for (int i = 0; i < 3; ++i) { D.J[i] = p.J[i]; D.invJ[i] = (float)(1.0 / p.J[i]); }
+    D.gyro[0] = (float)(((double)p.J[2] - p.J[1]) / p.J[0]);
+    D.gyro[1] = (float)(((double)p.J[0] - p.J[2]) / p.J[1]);
+    D.gyro[2] = (float)(((double)p.J[1] - p.J[0]) / p.J[2]);
+    const double l = p.L / std::sqrt(2.0), kappa = (double)p.k_m / p.k_f;
+    D.k_f = p.k_f; D.inv_k_f = (float)(1.0 / p.k_f); D.l = (float)l; D.kappa = (float)kappa;
+    D.inv_l = (float)(1.0 / l); D.inv_kappa = (float)(1.0 / kappa);
+    D.max_rpm = (float)max_rpm; D.s_max = (float)(p.k_f * max_rpm * max_rpm); D.T_max = (float)(4.0 * p.k_f * max_rpm * max_rpm);
+    D.rpm2rad = (float)(2.0 * M_PI / 60.0);
+    D.gnd_coef = (float)((double)p.C_gnd * (p.r_p / 4.0) * (p.r_p / 4.0)); D.h_clip = p.h_clip;
+    D.c_xy = p.c_xy; D.c_z = p.c_z;
+    D.dw_coef = (float)((double)p.dw_C1 * (p.r_p / 4.0) * (p.r_p / 4.0)); D.dw_C2 = p.dw_C2; D.dw_C3 = p.dw_C3;
+    D.dz_clip = p.dw_dz_clip; D.inv_dz_clip = p.dw_dz_clip > 0 ? (float)(1.0 / p.dw_dz_clip) : 0.0f;
+    const double alpha = std::exp(-dtc / p.wind_tau);
+    D.wind_alpha = (float)alpha; D.wind_gain = (float)(p.wind_sigma * std::sqrt(1.0 - alpha * alpha)); D.k_wind = p.k_wind;
+    D.dt_c = (float)dtc;
+    for (int i = 0; i < 3; ++i) {
+        D.Kp_pos[i] = p.Kp_pos[i]; D.Ki_pos[i] = p.Ki_pos[i]; D.Kd_pos[i] = p.Kd_pos[i];
+        D.Kp_att[i] = p.Kp_att[i]; D.Ki_att[i] = p.Ki_att[i]; D.Kd_att[i] = p.Kd_att[i];
+        D.a_ff[i] = p.a_ff[i]; D.term_center[i] = p.term_center[i];
+        D.reset_center[i] = p.reset_center[i]; D.reset_half[i] = p.reset_half[i];
+        D.target_fixed[i] = p.target_fixed[i]; D.target_lo[i] = p.target_lo[i]; D.target_hi[i] = p.target_hi[i];
+        D.form_center[i] = p.form_center[i];
+    }
+    D.int_clamp_pos = p.int_clamp_pos; D.int_clamp_att = p.int_clamp_att;
+    D.pos_step_max = (float)(p.pos_rate_limit * dtc); D.yaw_step_max = (float)(p.yaw_rate_limit * dtc);
+    D.tilt_max = p.tilt_max; D.tau_xy_max = p.tau_xy_max; D.tau_z_max = p.tau_z_max;
+    D.adj_radius = p.adj_radius; D.at_target_radius = p.at_target_radius;
+    D.term_tilt = p.term_tilt; D.term_dist = p.term_dist; D.z_max = p.z_max;
+    D.reset_z_lo = p.reset_z_lo; D.reset_z_hi = p.reset_z_hi; D.grid_spacing = p.grid_spacing; D.circle_radius = p.circle_radius;
+    D.mh_z_lo = p.mh_z_lo; D.mh_z_hi = p.mh_z_hi; D.form_radius = p.form_radius;
+}
+
+// ---- kernel dispatch: specialisations for the five benchmark configs, generic otherwise -------------
+#define FEATW(aero, euler, act, dsl, adj, rew, term) \
+    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) ? F_ADJ : 0) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT))
+static constexpr int FEAT_C1 = FEATW(0, 0, 0, 0, 0, 0, 1);
+static constexpr int FEAT_C2 = FEATW(3, 0, 0, 0, 0, 0, 1);
+static constexpr int FEAT_C3 = FEATW(0, 0, 1, 1, 0, 1, 2);
+static constexpr int FEAT_C4 = FEATW(7, 0, 0, 0, 0, 2, 1);
+static constexpr int FEAT_C5 = FEATW(15, 0, 2, 0, 1, 3, 3);
+
+static void pick_kernels(mdg_env* h) {
+    const int f = h->P.feat;
+    h->step = nullptr;
+#define SPECIAL(g, fw, name) if (h->G == g && f == fw) { h->step = step_kernel<g, fw>; h->kernel_name = name; }
+    SPECIAL(1, FEAT_C1, "step_kernel<G=1,rigid,rpm,hover>")
+    SPECIAL(1, FEAT_C2, "step_kernel<G=1,gnd+drag,rpm,hover>")
+    SPECIAL(1, FEAT_C3, "step_kernel<G=1,rigid,pid+dsl,negsqdist>")
+    SPECIAL(8, FEAT_C4, "step_kernel<G=8,gnd+drag+dw,rpm,multihover>")
+    SPECIAL(4, FEAT_C5, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation>")
+#undef SPECIAL
+#define GENERIC(g) case g: if (!h->step) { h->step = step_kernel<g, -1>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
+                   h->reset = reset_kernel<g>; h->refresh = refresh_obs_kernel<g>; break;
+    switch (h->G) { GENERIC(1) GENERIC(2) GENERIC(4) GENERIC(8) GENERIC(16) GENERIC(32) }
+#undef GENERIC
+}
+
+// ---- helpers --------------------------------------------------------------------------------------
+static int configure_launch(mdg_env* h) {
+    h->smem = 0;
+    if (h->max_blocks_per_sm > 0) {          // cap residency with a dynamic shared-memory reservation
+        int s = (228 * 1024) / h->max_blocks_per_sm - 1024;
+        if (s > 227 * 1024) s = 227 * 1024;
+        h->smem = s & ~127;
+    }
+    CU(cudaFuncSetAttribute((const void*)h->step, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem > 48 * 1024 ? h->smem : 48 * 1024));
+    return MDG_OK;
+}
+static inline unsigned grid_for(const mdg_env* h, int block) {
+    const size_t threads = (size_t)h->N * h->G;
+    return (unsigned)((threads + block - 1) / block);
+}
+static void drop_graphs(mdg_env* h) {
+    for (auto& kv : h->graphs) cudaGraphExecDestroy(kv.second);
+    h->graphs.clear();
+}
+static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s) {
+    h->step<<<grid_for(h, h->block), h->block, h->smem, s>>>(h->P, h->B, reinterpret_cast<const float4*>(actions_dev));
+    CU(cudaGetLastError());
+    return MDG_OK;
+}
+
+extern "C" {
+
+int mdg_version(void) { return 100; }
+const char* mdg_last_error(void) { return g_err.c_str(); }
+
+int mdg_default_params(int drone_model, mdg_params* p) {
+    if (!p) return fail(MDG_EINVAL, "mdg_default_params: out is NULL");
+    if (drone_model != MDG_MODEL_CF2X && drone_model != MDG_MODEL_RACE)
+        return fail(MDG_EINVAL, "mdg_default_params: unknown drone model (CF2P mixing is not built yet)");
+    std::memset(p, 0, sizeof(*p));
+    p->struct_size = (uint32_t)sizeof(mdg_params);
+    p->drone_model = drone_model;
+    if (drone_model == MDG_MODEL_RACE) {     // Table 2, RACE column
+        p->m = 0.250f; p->L = 0.125f; p->tw_ratio = 4.0f; p->J[0] = p->J[1] = 4.86e-4f; p->J[2] = 8.80e-4f;
+        p->k_f = 1.28e-8f; p->k_m = 5.96e-10f; p->r_p = 0.0635f;
+    } else {                                 // Table 2, CF2X column
+        p->m = 0.027f; p->L = 0.0397f; p->tw_ratio = 2.25f; p->J[0] = p->J[1] = 1.4e-5f; p->J[2] = 2.17e-5f;
+        p->k_f = 3.16e-10f; p->k_m = 7.94e-12f; p->r_p = 0.02325f;
+    }
+    p->g = 9.81f;
+    p->C_gnd = 11.36859f; p->c_xy = 9.1785e-7f; p->c_z = 10.311e-7f;
+    p->h_clip = (float)(0.25 * p->r_p * std::sqrt(15.0 * p->C_gnd / 4.0));
+    p->dw_C1 = 2267.18f; p->dw_C2 = 0.16f; p->dw_C3 = -0.11f; p->dw_dz_clip = 0.1f;
+    p->k_wind = 0.5f * 1.225f * 1.0f * 0.01f; p->wind_sigma = 0.5f; p->wind_tau = 1.0f;
+    p->sim_freq = 240; p->ctrl_freq = 48;
+    p->aero_mask = -1; p->integrator = -1;
+    const float kp[3] = {0.4f, 0.4f, 1.0f}, ki[3] = {0.01f, 0.01f, 0.01f}, kd[3] = {0.9f, 0.9f, 2.0f};   // Table 6
+    const float ap[3] = {2e-3f, 2e-3f, 1e-3f}, ai[3] = {0, 0, 1e-4f}, ad[3] = {5e-4f, 5e-4f, 2e-4f};
+    for (int i = 0; i < 3; ++i) {
+        p->Kp_pos[i] = kp[i]; p->Ki_pos[i] = ki[i]; p->Kd_pos[i] = kd[i];
+        p->Kp_att[i] = ap[i]; p->Ki_att[i] = ai[i]; p->Kd_att[i] = ad[i];
+    }
+    p->int_clamp_pos = 2.0f; p->int_clamp_att = 0.5f; p->dsl = 0;
+    p->pos_rate_limit = 2.0f; p->yaw_rate_limit = (float)M_PI; p->tilt_max = 0.5f;
+    const double s_hover = (double)p->m * p->g / 4.0;
+    p->tau_xy_max = (float)(4.0 * (p->L / std::sqrt(2.0)) * s_hover / 3.0);
+    p->tau_z_max = (float)(4.0 * ((double)p->k_m / p->k_f) * s_hover / 3.0);
+    p->obs_mode = MDG_OBS_KIN12; p->adj_radius = 0.5f;
+    p->reward_mode = MDG_REW_HOVER; p->at_target_radius = 0.05f;
+    p->term_mode = MDG_TERM_HOVER; p->term_tilt = (float)(M_PI / 2); p->term_dist = 3.0f; p->z_max = 3.0f;
+    p->episode_len_s = 10.0f; p->auto_reset = 1;
+    p->reset_layout = MDG_LAYOUT_NONE; p->reset_center[2] = 1.0f;
+    p->reset_half[0] = p->reset_half[1] = p->reset_half[2] = 0.1f;
+    p->grid_cols = 4; p->grid_spacing = 0.3f; p->circle_radius = 0.3f;
+    p->target_mode = MDG_TGT_FIXED; p->target_fixed[2] = 1.0f;
+    p->target_lo[0] = p->target_lo[1] = -1.0f; p->target_lo[2] = 0.2f;
+    p->target_hi[0] = p->target_hi[1] = 1.0f; p->target_hi[2] = 2.0f;
+    p->mh_z_lo = 0.7f; p->mh_z_hi = 1.2f; p->form_center[2] = 1.0f; p->form_radius = 0.3f;
+    return MDG_OK;
+}
+
+int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, const mdg_params* params, mdg_env** out) {
+    if (!out) return fail(MDG_EINVAL, "mdg_create: out is NULL");
+    *out = nullptr;
+    mdg_params p;
+    if (params) {
+        if (params->struct_size != sizeof(mdg_params)) return fail(MDG_EINVAL, "mdg_create: params->struct_size mismatch");
+        p = *params;
+    } else mdg_default_params(MDG_MODEL_CF2X, &p);
+    if (n_envs < 1 || n_drones < 1 || n_drones > 32) return fail(MDG_EINVAL, "mdg_create: need n_envs >= 1 and 1 <= n_drones <= 32");
+    if ((int64_t)n_envs * 32 > (int64_t)1 << 31) return fail(MDG_EINVAL, "mdg_create: n_envs too large");
+    if (physics_mode < 0 || physics_mode > MDG_PHYS_DYN) return fail(MDG_EINVAL, "mdg_create: unknown physics_mode");
+    if (action_type < 0 || action_type > MDG_ACT_VEL) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
+    if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
+        return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
+    if (p.obs_mode < 0 || p.obs_mode > 1 || p.reward_mode < 0 || p.reward_mode > 3 || p.term_mode < 0 || p.term_mode > 3 ||
+        p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 3 || p.integrator > 1 || p.aero_mask > 15)
+        return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
+    if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))
+        return fail(MDG_EINVAL, "mdg_create: m, g, k_f, k_m, J, wind_tau must be positive");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(MDG_ECUDA, "mdg_create: no CUDA device (this library has no CPU fallback)");
+    }
+    mdg_env* h = new mdg_env;
+    h->N = n_envs; h->M = n_drones; h->physics_mode = physics_mode; h->action_type = action_type; h->hp = p;
+    int G = 1; while (G < n_drones) G <<= 1;
+    h->G = G;
+    make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type), h->P);
+    pick_kernels(h);
+    // one arena: 7 drone planes, env plane, gstep, obs, reward, done (each 256 B aligned)
+    const size_t D = (size_t)n_envs * n_drones;
+    auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t plane = al(D * sizeof(float4)), eplane = al((size_t)n_envs * sizeof(float4)), gs = al((size_t)n_envs * 4),
+                 ob = al(D * h->P.opd * sizeof(float)), rw = al((size_t)n_envs * 4), dn = al((size_t)n_envs);
+    h->arena_bytes = 7 * plane + eplane + gs + ob + rw + dn;
+    cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
+    if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
+    ce = cudaMemset(h->arena, 0, h->arena_bytes);
+    if (ce != cudaSuccess) { cudaFree(h->arena); delete h; return fail(MDG_ECUDA, std::string("mdg_create: cudaMemset: ") + cudaGetErrorString(ce)); }
+    char* c = (char*)h->arena;
+    float4** planes[7] = {&h->B.P0, &h->B.P1, &h->B.P2, &h->B.P3, &h->B.P4, &h->B.P5, &h->B.P6};
+    for (int i = 0; i < 7; ++i) { *planes[i] = (float4*)c; c += plane; }
+    h->B.E0 = (float4*)c; c += eplane;
+    h->B.gstep = (uint32_t*)c; c += gs;
+    h->B.obs = (float*)c; c += ob;
+    h->B.reward = (float*)c; c += rw;
+    h->B.done = (uint8_t*)c;
+    int rc = configure_launch(h);
+    if (rc != MDG_OK) { cudaFree(h->arena); delete h; return rc; }
+    *out = h;
+    rc = mdg_reset(h, 0);
+    if (rc != MDG_OK) { mdg_destroy(h); *out = nullptr; return rc; }
+    return MDG_OK;
+}
+
+void mdg_destroy(mdg_env* h) {
+    if (!h) return;
+    drop_graphs(h);
+    if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
+    if (h->arena) cudaFree(h->arena);
+    delete h;
+}
+
+int mdg_reset(mdg_env* h, uint64_t seed) {
+    if (!h) return fail(MDG_EINVAL, "mdg_reset: NULL handle");
+    h->P.seed_lo = (uint32_t)seed; h->P.seed_hi = (uint32_t)(seed >> 32);
+    drop_graphs(h);                          // captured launches carry the old seed
+    h->reset<<<grid_for(h, 128), 128, 0, h->stream>>>(h->P, h->B);
+    CU(cudaGetLastError());
+    h->launches += 1;
+    return MDG_OK;
+}
+
+int mdg_step(mdg_env* h, const float* actions_dev) {
+    if (!h || !actions_dev) return fail(MDG_EINVAL, "mdg_step: NULL argument");
+    if ((uintptr_t)actions_dev & 15) return fail(MDG_EINVAL, "mdg_step: actions_dev must be 16-byte aligned");
+    const int rc = launch_step(h, actions_dev, h->stream);
+    if (rc == MDG_OK) h->launches += 1;
+    return rc;
+}
+
+int mdg_step_many(mdg_env* h, const float* actions_dev, int n_steps, int64_t stride_floats) {
+    if (!h || !actions_dev || n_steps < 1) return fail(MDG_EINVAL, "mdg_step_many: bad argument");
+    if (((uintptr_t)actions_dev & 15) || (stride_floats & 3)) return fail(MDG_EINVAL, "mdg_step_many: actions must stay 16-byte aligned");
+    const auto key = std::make_tuple((const void*)actions_dev, n_steps, stride_floats);
+    auto it = h->graphs.find(key);
+    if (it == h->graphs.end()) {
+        if (!h->capture_stream) CU(cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking));
+        CU(cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal));
+        int rc = MDG_OK;
+        for (int k = 0; k < n_steps && rc == MDG_OK; ++k) rc = launch_step(h, actions_dev + (int64_t)k * stride_floats, h->capture_stream);
+        cudaGraph_t g = nullptr;
+        cudaError_t ce = cudaStreamEndCapture(h->capture_stream, &g);
+        if (rc != MDG_OK) { if (g) cudaGraphDestroy(g); return rc; }
+        if (ce != cudaSuccess) return fail(MDG_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce));
+        cudaGraphExec_t ge = nullptr;
+        ce = cudaGraphInstantiate(&ge, g, 0);
+        cudaGraphDestroy(g);
+        if (ce != cudaSuccess) return fail(MDG_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ce));
+        if (h->graphs.size() >= 16) drop_graphs(h);
+        it = h->graphs.emplace(key, ge).first;
+    }
+    CU(cudaGraphLaunch(it->second, h->stream));
+    h->launches += n_steps;
+    return MDG_OK;
+}
+
+int mdg_outputs(mdg_env* h, const float** obs, const float** reward, const uint8_t** done) {
+    if (!h) return fail(MDG_EINVAL, "mdg_outputs: NULL handle");
+    if (obs) *obs = h->B.obs;
+    if (reward) *reward = h->B.reward;
+    if (done) *done = h->B.done;
+    return MDG_OK;
+}
+int mdg_obs_dim(const mdg_env* h) { return h ? h->M * h->P.opd : MDG_EINVAL; }
+int mdg_targets(mdg_env* h, const float** t) {
+    if (!h || !t) return fail(MDG_EINVAL, "mdg_targets: NULL argument");
+    *t = reinterpret_cast<const float*>(h->B.P6);
+    return MDG_OK;
+}
+
+int mdg_gen_actions(mdg_env* h, uint64_t seed, uint32_t t, float base, float lo, float hi, float* out_dev) {
+    if (!h || !out_dev || ((uintptr_t)out_dev & 15)) return fail(MDG_EINVAL, "mdg_gen_actions: bad argument");
+    const size_t D = (size_t)h->N * h->M;
+    gen_actions_kernel<<<(unsigned)((D + 255) / 256), 256, 0, h->stream>>>(D, h->M, (uint32_t)seed, (uint32_t)(seed >> 32), t, base, lo, hi,
+                                                                              reinterpret_cast<float4*>(out_dev));
+    CU(cudaGetLastError());
+    h->launches += 1;
+    return MDG_OK;
+}
+
+int mdg_set_stream(mdg_env* h, void* s) {
+    if (!h) return fail(MDG_EINVAL, "mdg_set_stream: NULL handle");
+    h->stream = (cudaStream_t)s;
+    return MDG_OK;
+}
+int64_t mdg_launch_count(const mdg_env* h) { return h ? h->launches : 0; }
+const char* mdg_kernel_name(const mdg_env* h) { return h ? h->kernel_name.c_str() : ""; }
+int mdg_set_launch(mdg_env* h, int block_threads, int max_blocks_per_sm) {
+    if (!h) return fail(MDG_EINVAL, "mdg_set_launch: NULL handle");
+    if (block_threads) {
+        if (block_threads < 32 || block_threads > 256 || (block_threads & 31)) return fail(MDG_EINVAL, "mdg_set_launch: block must be a multiple of 32 in [32, 256]");
+        h->block = block_threads;
+    }
+    if (max_blocks_per_sm) {
+        if (max_blocks_per_sm < 0 || max_blocks_per_sm > 32) return fail(MDG_EINVAL, "mdg_set_launch: max_blocks_per_sm in [1, 32]");
+        h->max_blocks_per_sm = max_blocks_per_sm;
+    }
+    drop_graphs(h);
+    return configure_launch(h);
+}
+
+}  // extern "C"
+
+// ---- checkpoint / test hooks: host AoS <-> device SoA planes ---------------------------------------
+extern "C" int mdg_get_state(mdg_env* h, float* state, float* ctrl, float* targets, float* wind, uint32_t* ep_step) {
+    if (!h) return fail(MDG_EINVAL, "mdg_get_state: NULL handle");
+    CU(cudaStreamSynchronize(h->stream));
+    const size_t D = (size_t)h->N * h->M;
+    std::vector<float4> pl[7];
+    float4* src[7] = {h->B.P0, h->B.P1, h->B.P2, h->B.P3, h->B.P4, h->B.P5, h->B.P6};
+    for (int i = 0; i < 7; ++i) { pl[i].resize(D); CU(cudaMemcpy(pl[i].data(), src[i], D * sizeof(float4), cudaMemcpyDeviceToHost)); }
+    for (size_t d = 0; d < D; ++d) {
+        const float4 a = pl[0][d], b = pl[1][d], c = pl[2][d], e = pl[3][d], f = pl[4][d], s = pl[5][d], t = pl[6][d];
+        if (state) { float* o = state + d * 13; o[0] = a.x; o[1] = a.y; o[2] = a.z; o[3] = a.w; o[4] = b.x; o[5] = b.y; o[6] = b.z;
+                     o[7] = b.w; o[8] = c.x; o[9] = c.y; o[10] = c.z; o[11] = c.w; o[12] = e.x; }
+        if (ctrl) { float* o = ctrl + d * 10; o[0] = e.y; o[1] = e.z; o[2] = e.w; o[3] = f.x; o[4] = f.y; o[5] = f.z;
+                    o[6] = s.x; o[7] = s.y; o[8] = s.z; o[9] = s.w; }
+        if (targets) { float* o = targets + d * 4; o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w; }
+    }
+    if (wind || ep_step) {
+        std::vector<float4> ev(h->N);
+        CU(cudaMemcpy(ev.data(), h->B.E0, (size_t)h->N * sizeof(float4), cudaMemcpyDeviceToHost));
+        for (int e = 0; e < h->N; ++e) {
+            if (wind) { wind[e * 3 + 0] = ev[e].x; wind[e * 3 + 1] = ev[e].y; wind[e * 3 + 2] = ev[e].z; }
+            if (ep_step) std::memcpy(&ep_step[e], &ev[e].w, 4);
+        }
+    }
+    return MDG_OK;
+}
+
+extern "C" int mdg_set_state(mdg_env* h, const float* state, const float* ctrl, const float* targets, const float* wind,
+                             const uint32_t* ep_step) {
+    if (!h) return fail(MDG_EINVAL, "mdg_set_state: NULL handle");
+    CU(cudaStreamSynchronize(h->stream));
+    const size_t D = (size_t)h->N * h->M;
+    std::vector<float4> pl[7];
+    float4* dst[7] = {h->B.P0, h->B.P1, h->B.P2, h->B.P3, h->B.P4, h->B.P5, h->B.P6};
+    for (int i = 0; i < 7; ++i) { pl[i].resize(D); CU(cudaMemcpy(pl[i].data(), dst[i], D * sizeof(float4), cudaMemcpyDeviceToHost)); }
+    for (size_t d = 0; d < D; ++d) {
+        if (state) { const float* o = state + d * 13;
+                     pl[0][d] = make_float4(o[0], o[1], o[2], o[3]); pl[1][d] = make_float4(o[4], o[5], o[6], o[7]);
+                     pl[2][d] = make_float4(o[8], o[9], o[10], o[11]); pl[3][d].x = o[12]; }
+        if (ctrl) { const float* o = ctrl + d * 10;
+                    pl[3][d].y = o[0]; pl[3][d].z = o[1]; pl[3][d].w = o[2]; pl[4][d] = make_float4(o[3], o[4], o[5], 0.0f);
+                    pl[5][d] = make_float4(o[6], o[7], o[8], o[9]); }
+        if (targets) { const float* o = targets + d * 4; pl[6][d] = make_float4(o[0], o[1], o[2], o[3]); }
+    }
+    for (int i = 0; i < 7; ++i) CU(cudaMemcpy(dst[i], pl[i].data(), D * sizeof(float4), cudaMemcpyHostToDevice));
+    if (wind || ep_step) {
+        std::vector<float4> ev(h->N);
+        CU(cudaMemcpy(ev.data(), h->B.E0, (size_t)h->N * sizeof(float4), cudaMemcpyDeviceToHost));
+        for (int e = 0; e < h->N; ++e) {
+            if (wind) { ev[e].x = wind[e * 3 + 0]; ev[e].y = wind[e * 3 + 1]; ev[e].z = wind[e * 3 + 2]; }
+            if (ep_step) std::memcpy(&ev[e].w, &ep_step[e], 4);
+        }
+        CU(cudaMemcpy(h->B.E0, ev.data(), (size_t)h->N * sizeof(float4), cudaMemcpyHostToDevice));
+    }
+    h->refresh<<<grid_for(h, 128), 128, 0, h->stream>>>(h->P, h->B);
+    CU(cudaGetLastError());
+    h->launches += 1;
+    CU(cudaStreamSynchronize(h->stream));
+    return MDG_OK;
+}

@@ -1,0 +1,137 @@
+// mdg_dev.cuh — device-side parameter block, Philox4x32-10 and small fp32 helpers of the fused
+// drone-env step kernel (sm_100a).  Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mdg {
+
+// Feature word of a kernel specialisation (compile-time when >= 0, read from DevParams when < 0).
+enum : int {
+    F_GND = 1, F_DRAG = 2, F_DW = 4, F_WIND = 8,          // == MDG_AERO_*
+    F_EULER = 16,                                         // DYN integrator (Table 1)
+    F_ACT_SHIFT = 5,                                      // 2 bits: MDG_ACT_*
+    F_DSL = 128,
+    F_ADJ = 256,                                          // MDG_OBS_KIN12_ADJ
+    F_REW_SHIFT = 9,                                      // 2 bits: MDG_REW_*
+    F_TERM_SHIFT = 11,                                    // 2 bits: MDG_TERM_*
+};
+
+// Everything the kernels need, precomputed on the host in double and rounded once to fp32.
+// Passed by value as a __grid_constant__ kernel parameter, so every field is a constant-bank operand.
+struct DevParams {
+    int N, M, K, ep_steps, auto_reset, feat;
+    int reset_layout, target_mode, grid_cols, grid_rows, opd;
+    uint32_t seed_lo, seed_hi;
+    // integrator
+    float h, half_h, h_sixth, half_h2;
+    float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
+    // motor model (Eq.1-3)
+    float k_f, inv_k_f, l, kappa, inv_l, inv_kappa, max_rpm, s_max, T_max, rpm2rad;
+    // aero (Eq.4-6) and wind
+    float gnd_coef, h_clip, c_xy, c_z, dw_coef, dw_C2, dw_C3, dz_clip, inv_dz_clip;
+    float wind_alpha, wind_gain, k_wind;
+    // cascaded PID (Eq.9, Table 6)
+    float dt_c, m, inv_g;
+    float Kp_pos[3], Ki_pos[3], Kd_pos[3], Kp_att[3], Ki_att[3], Kd_att[3];
+    float int_clamp_pos, int_clamp_att, pos_step_max, yaw_step_max, a_ff[3], tilt_max, tau_xy_max, tau_z_max;
+    // epilogue
+    float adj_radius, at_target_radius, term_tilt, term_dist, term_center[3], z_max;
+    // reset / targets
+    float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
+    float target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi, form_center[3], form_radius;
+};
+
+// SoA state planes (float4 per drone) and per-env words.  DESIGN.md §5.
+struct DevBuffers {
+    float4* P0;   // px py pz qw
+    float4* P1;   // qx qy qz vx
+    float4* P2;   // vy vz wx wy
+    float4* P3;   // wz Ipx Ipy Ipz
+    float4* P4;   // Iex Iey Iez -
+    float4* P5;   // held setpoint x y z psi
+    float4* P6;   // target x y z psi
+    float4* E0;   // wind x y z, bits(ep_step)
+    uint32_t* gstep;
+    float* obs;
+    float* reward;
+    uint8_t* done;
+};
+
+static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3;
+
+// Philox4x32-10 (Salmon et al., SC'11).  key = seed halves, counter = (env, drone|~0, step, stream).
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+__device__ __forceinline__ float u01(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }
+
+struct V3 { float x, y, z; };
+__device__ __forceinline__ V3 v3(float x, float y, float z) { V3 r; r.x = x; r.y = y; r.z = z; return r; }
+__device__ __forceinline__ V3 cross(V3 a, V3 b) {
+    return v3(a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x);
+}
+struct Q4 { float w, x, y, z; };
+
+// rotate v by unit quaternion q (body -> world): v + w t + u x t, t = 2 u x v
+__device__ __forceinline__ V3 rot(Q4 q, V3 v) {
+    const V3 u = v3(q.x, q.y, q.z);
+    V3 t = cross(u, v);
+    t.x += t.x; t.y += t.y; t.z += t.z;
+    const V3 c = cross(u, t);
+    return v3(fmaf(q.w, t.x, v.x) + c.x, fmaf(q.w, t.y, v.y) + c.y, fmaf(q.w, t.z, v.z) + c.z);
+}
+// rotate v by the conjugate of q (world -> body)
+__device__ __forceinline__ V3 rot_inv(Q4 q, V3 v) {
+    Q4 c; c.w = q.w; c.x = -q.x; c.y = -q.y; c.z = -q.z;
+    return rot(c, v);
+}
+__device__ __forceinline__ Q4 qmul(Q4 a, Q4 b) {
+    Q4 r;
+    r.w = a.w * b.w - a.x * b.x - a.y * b.y - a.z * b.z;
+    r.x = a.w * b.x + b.w * a.x + (a.y * b.z - a.z * b.y);
+    r.y = a.w * b.y + b.w * a.y + (a.z * b.x - a.x * b.z);
+    r.z = a.w * b.z + b.w * a.z + (a.x * b.y - a.y * b.x);
+    return r;
+}
+// Eq.7 increment: [cos(|phi|/2), sin(|phi|/2) phi/|phi|].  Both factors are even power series in
+// x = |phi|^2, so for x <= 1 (|omega| h <= 1 rad) no sqrt, division or MUFU is needed; truncation
+// error < 3e-10.  Larger angles take the library path.
+__device__ __forceinline__ Q4 exp_half(V3 phi) {
+    const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
+    float c, s;
+    if (x <= 1.0f) {
+        c = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 9.6881200e-8f, -2.1701389e-5f), 2.6041667e-3f), -0.125f), 1.0f);
+        s = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 5.3822889e-9f, -1.5500992e-6f), 2.6041667e-4f), -2.0833333e-2f), 0.5f);
+    } else {
+        const float n = sqrtf(x);
+        float sn, cn;
+        sincosf(0.5f * n, &sn, &cn);
+        c = cn; s = sn / n;
+    }
+    Q4 r; r.w = c; r.x = s * phi.x; r.y = s * phi.y; r.z = s * phi.z;
+    return r;
+}
+__device__ __forceinline__ float clampf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
+__device__ __forceinline__ float wrap_pi(float x) {
+    const float k = ceilf((x - 3.14159265358979f) * 0.159154943091895f);
+    return fmaf(-6.28318530717959f, k, x);
+}
+// ZYX Euler angles (roll, pitch, yaw) of q
+__device__ __forceinline__ V3 euler_zyx(Q4 q) {
+    V3 e;
+    e.x = atan2f(2.0f * (q.w * q.x + q.y * q.z), 1.0f - 2.0f * (q.x * q.x + q.y * q.y));
+    e.y = asinf(clampf(2.0f * (q.w * q.y - q.z * q.x), -1.0f, 1.0f));
+    e.z = atan2f(2.0f * (q.w * q.z + q.x * q.y), 1.0f - 2.0f * (q.y * q.y + q.z * q.z));
+    return e;
+}
+
+}  // namespace mdg

@@ -1,0 +1,180 @@
+// mdg_step.cuh — the fused control-step kernel: one thread per drone, the G = pow2 >= M drones of an
+// env sit in adjacent lanes of one warp, the 13 state words stay in registers over all K substeps,
+// and every intra-env exchange (downwash pairs, adjacency, reward / done reduction) is a warp shuffle.
+// No shared memory, no HBM traffic between substeps.  PAPER.md citations: see include/mdg.h.
+#pragma once
+#include "mdg_dev.cuh"
+
+namespace mdg {
+
+#define MDG_FULL 0xffffffffu
+
+template <int FEAT> struct Feat {
+    __device__ __forceinline__ static int word(const DevParams& P) { return FEAT >= 0 ? FEAT : P.feat; }
+    __device__ __forceinline__ static bool has(const DevParams& P, int bit) { return (word(P) & bit) != 0; }
+    __device__ __forceinline__ static int act(const DevParams& P) { return (word(P) >> F_ACT_SHIFT) & 3; }
+    __device__ __forceinline__ static int rew(const DevParams& P) { return (word(P) >> F_REW_SHIFT) & 3; }
+    __device__ __forceinline__ static int term(const DevParams& P) { return (word(P) >> F_TERM_SHIFT) & 3; }
+};
+
+struct DroneRegs {
+    V3 p; Q4 q; V3 v; V3 w;       // state, w in the body frame
+    V3 Ip, Ie; float4 sp;         // controller memory
+};
+
+// Initial state of drone j of env e at control-step index t (the paper's `_single_reset`)
+__device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint32_t j, uint32_t t,
+                                            DroneRegs& d, float4& tg) {
+    float bx = P.reset_center[0], by = P.reset_center[1], bz = P.reset_center[2];
+    if (P.reset_layout == 1) {            // GRID
+        const int col = (int)j % P.grid_cols, row = (int)j / P.grid_cols;
+        bx += ((float)col - 0.5f * (float)(P.grid_cols - 1)) * P.grid_spacing;
+        by += ((float)row - 0.5f * (float)(P.grid_rows - 1)) * P.grid_spacing;
+    } else if (P.reset_layout == 2) {     // CIRCLE
+        float s, c;
+        sincospif(2.0f * (float)j / (float)P.M, &s, &c);
+        bx = fmaf(P.circle_radius, c, bx); by = fmaf(P.circle_radius, s, by);
+    }
+    const uint4 r = philox4x32_10(e, j, t, STREAM_RESET_POS, P.seed_lo, P.seed_hi);
+    d.p.x = bx + fmaf(2.0f * P.reset_half[0], u01(r.x), -P.reset_half[0]);
+    d.p.y = by + fmaf(2.0f * P.reset_half[1], u01(r.y), -P.reset_half[1]);
+    if (P.reset_z_hi > P.reset_z_lo) d.p.z = fmaf(P.reset_z_hi - P.reset_z_lo, u01(r.z), P.reset_z_lo);
+    else d.p.z = bz + fmaf(2.0f * P.reset_half[2], u01(r.z), -P.reset_half[2]);
+    d.q.w = 1.0f; d.q.x = d.q.y = d.q.z = 0.0f;
+    d.v = v3(0, 0, 0); d.w = v3(0, 0, 0); d.Ip = v3(0, 0, 0); d.Ie = v3(0, 0, 0);
+    d.sp = make_float4(d.p.x, d.p.y, d.p.z, 0.0f);
+    tg.w = 0.0f;
+    if (P.target_mode == 0) {             // FIXED
+        tg.x = P.target_fixed[0]; tg.y = P.target_fixed[1]; tg.z = P.target_fixed[2];
+    } else if (P.target_mode == 1) {      // SPAWN_LINSPACE
+        tg.x = d.p.x; tg.y = d.p.y;
+        tg.z = P.M > 1 ? fmaf(P.mh_z_hi - P.mh_z_lo, (float)j / (float)(P.M - 1), P.mh_z_lo) : P.mh_z_lo;
+    } else if (P.target_mode == 2) {      // BOX
+        const uint4 r2 = philox4x32_10(e, j, t, STREAM_RESET_EXTRA, P.seed_lo, P.seed_hi);
+        tg.x = fmaf(P.target_hi[0] - P.target_lo[0], u01(r2.x), P.target_lo[0]);
+        tg.y = fmaf(P.target_hi[1] - P.target_lo[1], u01(r2.y), P.target_lo[1]);
+        tg.z = fmaf(P.target_hi[2] - P.target_lo[2], u01(r2.z), P.target_lo[2]);
+    } else {                              // CIRCLE slots
+        float s, c;
+        sincospif(2.0f * (float)j / (float)P.M, &s, &c);
+        tg.x = fmaf(P.form_radius, c, P.form_center[0]); tg.y = fmaf(P.form_radius, s, P.form_center[1]);
+        tg.z = P.form_center[2];
+    }
+}
+
+// Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376)
+template <int FEAT>
+__device__ __forceinline__ void decode_action(const DevParams& P, float4 a, DroneRegs& d, float n[4]) {
+    const int act = Feat<FEAT>::act(P);
+    if (act == 0) {                       // RPM, clipped
+        n[0] = clampf(a.x, 0.0f, P.max_rpm); n[1] = clampf(a.y, 0.0f, P.max_rpm);
+        n[2] = clampf(a.z, 0.0f, P.max_rpm); n[3] = clampf(a.w, 0.0f, P.max_rpm);
+        return;
+    }
+    const V3 eta = euler_zyx(d.q);
+    float spsi, cpsi;
+    sincosf(eta.z, &spsi, &cpsi);
+    V3 e_p, v_ref; float psi_ref;
+    if (act == 1) {                       // PID waypoint [x, y, z, psi]
+        if (Feat<FEAT>::has(P, F_DSL)) {
+            const V3 dv = v3(a.x - d.sp.x, a.y - d.sp.y, a.z - d.sp.z);
+            const float dist = sqrtf(fmaf(dv.x, dv.x, fmaf(dv.y, dv.y, dv.z * dv.z)));
+            if (dist > P.pos_step_max) {
+                const float f = P.pos_step_max / dist;
+                d.sp.x = fmaf(dv.x, f, d.sp.x); d.sp.y = fmaf(dv.y, f, d.sp.y); d.sp.z = fmaf(dv.z, f, d.sp.z);
+            } else { d.sp.x = a.x; d.sp.y = a.y; d.sp.z = a.z; }
+            const float dpsi = clampf(wrap_pi(a.w - d.sp.w), -P.yaw_step_max, P.yaw_step_max);
+            d.sp.w = wrap_pi(d.sp.w + dpsi);
+        } else d.sp = a;
+        e_p = v3(d.sp.x - d.p.x, d.sp.y - d.p.y, d.sp.z - d.p.z);
+        v_ref = v3(0, 0, 0); psi_ref = d.sp.w;
+    } else {                              // VEL [vx, vy, vz, wz] in the heading frame
+        e_p = v3(0, 0, 0);
+        v_ref = v3(cpsi * a.x - spsi * a.y, spsi * a.x + cpsi * a.y, a.z);
+        psi_ref = fmaf(a.w, P.dt_c, eta.z);
+    }
+    // position loop, Eq.9
+    d.Ip.x = clampf(fmaf(e_p.x, P.dt_c, d.Ip.x), -P.int_clamp_pos, P.int_clamp_pos);
+    d.Ip.y = clampf(fmaf(e_p.y, P.dt_c, d.Ip.y), -P.int_clamp_pos, P.int_clamp_pos);
+    d.Ip.z = clampf(fmaf(e_p.z, P.dt_c, d.Ip.z), -P.int_clamp_pos, P.int_clamp_pos);
+    const float ax = fmaf(P.Kp_pos[0], e_p.x, fmaf(P.Ki_pos[0], d.Ip.x, fmaf(P.Kd_pos[0], v_ref.x - d.v.x, P.a_ff[0])));
+    const float ay = fmaf(P.Kp_pos[1], e_p.y, fmaf(P.Ki_pos[1], d.Ip.y, fmaf(P.Kd_pos[1], v_ref.y - d.v.y, P.a_ff[1])));
+    const float az = fmaf(P.Kp_pos[2], e_p.z, fmaf(P.Ki_pos[2], d.Ip.z, fmaf(P.Kd_pos[2], v_ref.z - d.v.z, P.a_ff[2]))) + P.g;
+    const float T = clampf(P.m * sqrtf(fmaf(ax, ax, fmaf(ay, ay, az * az))), 0.0f, P.T_max);
+    const float phi_ref = clampf((ax * spsi - ay * cpsi) * P.inv_g, -P.tilt_max, P.tilt_max);
+    const float th_ref = clampf((ax * cpsi + ay * spsi) * P.inv_g, -P.tilt_max, P.tilt_max);
+    const V3 e_eta = v3(phi_ref - eta.x, th_ref - eta.y, wrap_pi(psi_ref - eta.z));
+    d.Ie.x = clampf(fmaf(e_eta.x, P.dt_c, d.Ie.x), -P.int_clamp_att, P.int_clamp_att);
+    d.Ie.y = clampf(fmaf(e_eta.y, P.dt_c, d.Ie.y), -P.int_clamp_att, P.int_clamp_att);
+    d.Ie.z = clampf(fmaf(e_eta.z, P.dt_c, d.Ie.z), -P.int_clamp_att, P.int_clamp_att);
+    const float tx = clampf(fmaf(P.Kp_att[0], e_eta.x, fmaf(P.Ki_att[0], d.Ie.x, -P.Kd_att[0] * d.w.x)), -P.tau_xy_max, P.tau_xy_max);
+    const float ty = clampf(fmaf(P.Kp_att[1], e_eta.y, fmaf(P.Ki_att[1], d.Ie.y, -P.Kd_att[1] * d.w.y)), -P.tau_xy_max, P.tau_xy_max);
+    const float tz = clampf(fmaf(P.Kp_att[2], e_eta.z, fmaf(P.Ki_att[2], d.Ie.z, -P.Kd_att[2] * d.w.z)), -P.tau_z_max, P.tau_z_max);
+    // closed-form allocation inverse, per-rotor clip, back to RPM
+    const float qa = tx * P.inv_l, qb = ty * P.inv_l, qc = tz * P.inv_kappa;
+    const float s0 = 0.25f * (T + qa - qb - qc), s1 = 0.25f * (T + qa + qb + qc);
+    const float s2 = 0.25f * (T - qa + qb - qc), s3 = 0.25f * (T - qa - qb + qc);
+    n[0] = sqrtf(clampf(s0, 0.0f, P.s_max) * P.inv_k_f); n[1] = sqrtf(clampf(s1, 0.0f, P.s_max) * P.inv_k_f);
+    n[2] = sqrtf(clampf(s2, 0.0f, P.s_max) * P.inv_k_f); n[3] = sqrtf(clampf(s3, 0.0f, P.s_max) * P.inv_k_f);
+}
+
+// angular acceleration J^-1 (tau_body - w x J w)
+__device__ __forceinline__ V3 ang_acc(const DevParams& P, V3 tb, V3 w) {
+    return v3(fmaf(P.invJ[0], tb.x, -P.gyro[0] * (w.y * w.z)),
+              fmaf(P.invJ[1], tb.y, -P.gyro[1] * (w.z * w.x)),
+              fmaf(P.invJ[2], tb.z, -P.gyro[2] * (w.x * w.y)));
+}
+
+// Observation row of one drone: [p, eta, v, w (, adjacency)] written as float4s when the row is 16 B aligned
+template <int G>
+__device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict__ obs, size_t drone, const DroneRegs& d,
+                                          V3 eta, const float (&adj)[G], bool with_adj) {
+    float* o = obs + drone * (size_t)P.opd;
+    if ((P.opd & 3) == 0) {
+        float4* o4 = reinterpret_cast<float4*>(o);
+        o4[0] = make_float4(d.p.x, d.p.y, d.p.z, eta.x);
+        o4[1] = make_float4(eta.y, eta.z, d.v.x, d.v.y);
+        o4[2] = make_float4(d.v.z, d.w.x, d.w.y, d.w.z);
+        if (with_adj) {
+            if (G == 4) o4[3] = make_float4(adj[0], adj[1 % G], adj[2 % G], adj[3 % G]);
+            else {
+#pragma unroll
+                for (int k = 0; k < G; ++k) if (k < P.M) o[12 + k] = adj[k];
+            }
+        }
+    } else {
+        o[0] = d.p.x; o[1] = d.p.y; o[2] = d.p.z; o[3] = eta.x; o[4] = eta.y; o[5] = eta.z;
+        o[6] = d.v.x; o[7] = d.v.y; o[8] = d.v.z; o[9] = d.w.x; o[10] = d.w.y; o[11] = d.w.z;
+        if (with_adj) {
+#pragma unroll
+            for (int k = 0; k < G; ++k) if (k < P.M) o[12 + k] = adj[k];
+        }
+    }
+}
+
+// adjacency row of this lane's drone: A_k = 1 if k == j or |p - p_k| < radius (Q23)
+template <int G>
+__device__ __forceinline__ void adjacency(const DevParams& P, V3 p, int lane, int j, float (&adj)[G]) {
+    const int gbase = lane & ~(G - 1);
+#pragma unroll
+    for (int k = 0; k < G; ++k) {
+        const float ox = __shfl_sync(MDG_FULL, p.x, gbase + k), oy = __shfl_sync(MDG_FULL, p.y, gbase + k),
+                    oz = __shfl_sync(MDG_FULL, p.z, gbase + k);
+        const float dx = p.x - ox, dy = p.y - oy, dz = p.z - oz;
+        const float dist = sqrtf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
+        adj[k] = (k == j || dist < P.adj_radius) ? 1.0f : 0.0f;
+    }
+}
+
+template <int G> __device__ __forceinline__ float group_sum(float x) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) x += __shfl_xor_sync(MDG_FULL, x, o);
+    return x;
+}
+template <int G> __device__ __forceinline__ int group_or(int x) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) x |= __shfl_xor_sync(MDG_FULL, x, o);
+    return x;
+}
+
+}  // namespace mdg
