@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py — env-steps/s of the fused drone-env step on N B200s (BASELINE.json metric, config 5).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
+
+One "step" is one control step of the whole batch (action decode -> K substeps -> obs/reward/done/
+auto-reset) = ONE kernel launch.  See DESIGN.md §7 for what each JSON key means and how the roofline
+numbers are derived.  `--impl reference` times the float64 oracle on the host cores (a baseline, not
+the target).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2606_08039_b200 import workloads as W  # noqa: E402
+
+METRIC = "env_steps_per_sec"
+UNIT = "env-steps/s"
+# FP32 ALU peak: 148 SMs x 128 FP32 lanes x 2 flop/FMA x 1.965 GHz (clocks.max.sm)
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# algorithmic flops per drone per control step, tallied by the oracle's counting scalar type on the
+# seeded workloads (tests/test_oracle_control_env.py::test_flop_tally...)
+FLOPS_PER_DRONE_STEP = {1: 3186.0, 2: 3421.1, 3: 3350.0, 4: 3893.6, 5: 3858.75}
+REPLICAS = 4          # independent env batches stepped round-robin so the working set exceeds the 126 MB L2
+
+
+def algorithmic_bytes_per_drone(c: int) -> float:
+    """State read once + written once, actions read, outputs written."""
+    wl = W.config(c)
+    M = wl.n_drones
+    pid = wl.action_type != W.ACT_RPM
+    rd = 4 * 16 + 16 + 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)   # P0-P3, target, action, P4, P5
+    wr = 4 * 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)
+    obs = 4 * (12 + (M if wl.params.get("obs_mode", 0) == W.OBS_KIN12_ADJ else 0))
+    env = (16 + 4) + (16 + 4 + 4 + 1)                                                         # per env: E0 + gstep r/w, reward, done
+    return rd + wr + obs + env / M
+
+
+class ClockSampler:
+    """nvidia-smi SM clock / throttle-reason samples while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.samples, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc:
+            time.sleep(0.05)
+            self.proc.terminate()
+        mhz, mx, reasons = [], 0.0, set()
+        for ts, line in self.samples:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                mx = max(mx, float(f[1]))
+                if t0 <= ts <= t1 + 0.05:
+                    mhz.append(float(f[0]))
+                    for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                        if v.lower().startswith("active"):
+                            reasons.add(name)
+            except ValueError:
+                pass
+        mhz.sort()
+        return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(mhz)}
+
+
+def harness_actions(wl):
+    kind = wl.actions[0]
+    if kind == "hover_scale":
+        return W.hover_rpm_f32(), wl.actions[1], wl.actions[2]
+    if kind == "uniform":
+        return 1.0, wl.actions[1], wl.actions[2]
+    return None
+
+
+def oracle_throughput(wl, budget_s, n_envs, min_steps=4, max_steps=10 ** 9):
+    """Time the oracle as it stands on a bounded sample of the workload: env-steps/s on the host cores."""
+    import numpy as np
+    from oracle import oracle as O
+    cores = len(os.sched_getaffinity(0))
+    sample = wl.scaled(min(wl.n_envs, n_envs))
+    env = O.OracleEnv(sample.n_envs, sample.n_drones, sample.physics_mode, sample.action_type, O.OracleParams(0, **sample.params), n_threads=cores)
+    env.reset(sample.seed)
+    ha = harness_actions(sample)
+    acts = []
+    for t in range(8):
+        acts.append(O.gen_actions(sample.seed, t, sample.n_envs, sample.n_drones, *ha) if ha else env.targets.astype(np.float32))
+    flops = env.flop_tally(acts[0]) / (sample.n_envs * sample.n_drones)
+    env.step(acts[0])                                   # warm-up (thread start, page faults)
+    t0 = time.perf_counter()
+    steps = 0
+    while steps < max_steps and (steps < min_steps or time.perf_counter() - t0 < budget_s):
+        env.step(acts[steps % 8] if ha else env.targets.astype(np.float32))
+        steps += 1
+    dt = time.perf_counter() - t0
+    return dict(value=sample.n_envs * steps / dt, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{sample.n_envs} envs x {sample.n_drones} drones x {steps} control steps of {wl.name} (float64, {cores} threads, {dt:.1f} s)",
+                flops_per_drone_step=flops, ms_per_step=1e3 * dt / steps, steps=steps)
+
+
+def run_reference(args, wl, c):
+    """`--impl reference`: the oracle on the host cores, same metric/config; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    total = args.steps + args.warmup
+    # bounded sample per step, sized from a short calibration so the whole run takes about a minute
+    cal = oracle_throughput(wl, budget_s=1.0, n_envs=1024, min_steps=2)
+    per_step_envs = int(max(64, min(wl.n_envs, 60.0 * cal["value"] / total)))
+    res = oracle_throughput(wl, budget_s=1e9, n_envs=per_step_envs, min_steps=total, max_steps=total)
+    line = {"impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_dict(wl, c, args.gpus),
+            "cpu_baseline": {"value": res["value"], "unit": UNIT, "cores": res["cores"], "kind": "oracle", "sample": res["sample"]},
+            "e2e": {"value": res["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(wl, c, n_gpus):
+    return {"workload": f"config {c} of BASELINE.json: {wl.n_envs} envs x {wl.n_drones} CF2X drones per GPU, "
+                        f"physics_mode={wl.physics_mode} aero_mask={wl.params.get('aero_mask', 'from mode')}, action_type={wl.action_type}, "
+                        f"240 Hz physics / 48 Hz control (5 substeps), auto-reset on",
+            "n_envs_per_gpu": wl.n_envs, "n_drones": wl.n_drones, "substeps": 5, "seed": wl.seed,
+            "parallelism": f"env-sharded x{n_gpus}, no collective on the step path",
+            "l2": f"{REPLICAS} independent env batches stepped round-robin (working set > 126 MB L2)"}
+
+
+def run_ours(args, wl, c):
+    import torch
+    import paper_2606_08039_b200 as mdg
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K, Wm = args.steps, max(args.warmup, 3)
+    stream = torch.cuda.Stream()
+    ha = harness_actions(wl)
+    A = 4                                                  # distinct action sets per replica
+    envs, acts = [], []
+    with torch.cuda.stream(stream):
+        for r in range(REPLICAS):
+            over = dict(wl.params, env_index_base=(rank * REPLICAS + r) * wl.n_envs)
+            env = mdg.Env(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, mdg.default_params(0, **over), stream=stream)
+            if args.block or args.max_blocks:
+                env.set_launch(args.block, args.max_blocks)
+            env.reset(wl.seed)
+            envs.append(env)
+            if ha:
+                acts.append([env.gen_actions(wl.seed, t, *ha) for t in range(A)])
+            else:
+                acts.append([env.targets] * A)             # PID waypoint = the per-episode target (device resident)
+        launches0 = sum(e.launch_count for e in envs)
+        for k in range(Wm):
+            envs[k % REPLICAS].step(acts[k % REPLICAS][(k // REPLICAS) % A])
+        stream.synchronize()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+            time.sleep(0.1)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = sum(e.launch_count for e in envs)
+        t_wall0 = time.time()
+        ev0.record(stream)
+        for k in range(K):
+            envs[k % REPLICAS].step(acts[k % REPLICAS][(k // REPLICAS) % A])
+        ev1.record(stream)
+        stream.synchronize()
+        torch.cuda.synchronize()
+        t_wall1 = time.time()
+        if dist:
+            dist.barrier()
+        ms = ev0.elapsed_time(ev1)
+        launches = sum(e.launch_count for e in envs) - l0
+        clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+        if dist:
+            tt = torch.tensor([ms], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ms = float(tt.item())
+        # ---- end to end through the C ABI with host buffers (pinned): H2D actions, step, D2H obs/reward/done
+        env = envs[0]
+        D = wl.n_envs * wl.n_drones
+        a_host = [a.cpu().pin_memory() for a in acts[0]]
+        obs_h = torch.empty((wl.n_envs, env.obs_dim), dtype=torch.float32).pin_memory()
+        rew_h = torch.empty(wl.n_envs, dtype=torch.float32).pin_memory()
+        done_h = torch.empty(wl.n_envs, dtype=torch.uint8).pin_memory()
+        Ke = max(3, min(K, args.e2e_steps))
+        for k in range(3):
+            env.step_host(a_host[k % A], obs_h, rew_h, done_h)
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for k in range(Ke):
+            env.step_host(a_host[k % A], obs_h, rew_h, done_h)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_e2e = e0.elapsed_time(e1)
+        if dist:
+            tt = torch.tensor([ms_e2e], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ms_e2e = float(tt.item())
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+    sec = ms / 1e3
+    value = world * wl.n_envs * K / sec
+    per_launch_s = sec / K
+    drones = wl.n_envs * wl.n_drones
+    cpu = oracle_throughput(wl, budget_s=args.cpu_budget, n_envs=16384) if world == 1 and not args.no_cpu else None
+    fpd = cpu["flops_per_drone_step"] if cpu else FLOPS_PER_DRONE_STEP[c]
+    flops = fpd * drones
+    bytes_alg = algorithmic_bytes_per_drone(c) * drones
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    achieved_tf = flops / per_launch_s / 1e12
+    t_alu, t_hbm = flops / (ALU_PEAK_TFLOPS * 1e12), bytes_alg / (hbm_peak * 1e9)
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"c{c}")
+    except Exception:
+        pass
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": config_dict(wl, c, world),
+            "drone_substeps_per_sec": value * wl.n_drones * 5,
+            "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved_tf / ALU_PEAK_TFLOPS,
+                         "traffic": traffic, "kernel": envs[0].kernel_name, "us_per_launch": per_launch_s * 1e6,
+                         "flops_per_launch": flops, "bytes_per_launch": bytes_alg,
+                         "peak_note": "FP32 ALU peak derived: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md §6)",
+                         "hbm": {"achieved_gbs": bytes_alg / per_launch_s / 1e9, "peak_gbs": hbm_peak,
+                                 "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback of B200_PROFILING.md",
+                                 "frac": bytes_alg / per_launch_s / 1e9 / hbm_peak},
+                         "t_roof_us": max(t_alu, t_hbm) * 1e6, "frac_of_binding_roof": max(t_alu, t_hbm) / per_launch_s},
+            "e2e": {"value": world * wl.n_envs * Ke / (ms_e2e / 1e3), "unit": UNIT, "h2d_bytes_per_step": drones * 16,
+                    "d2h_bytes_per_step": wl.n_envs * env.obs_dim * 4 + wl.n_envs * 5, "steps": Ke, "ms_per_step": ms_e2e / Ke},
+            "gpu_launches": launches, "clocks": clocks}
+    if cpu:
+        line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line), flush=True)
+    if dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (5 = 65,536 envs x 4 drones, the metric's config)")
+    ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--max-blocks", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=50)
+    ap.add_argument("--cpu-budget", type=float, default=12.0)
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    wl = W.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, wl, args.config)
+    else:
+        run_ours(args, wl, args.config)
+
+
+if __name__ == "__main__":
+    main()

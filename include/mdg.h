@@ -74,6 +74,9 @@ typedef struct mdg_params {
     int32_t grid_cols; float grid_spacing, circle_radius;
     int32_t target_mode; float target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi,
         form_center[3], form_radius;
+    /* global index of env 0: Philox counters use env_index_base + e, so a batch split across GPUs
+     * draws exactly what the unsplit batch would (no collective on the step path) */
+    uint32_t env_index_base;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */
@@ -98,6 +101,12 @@ int mdg_step(mdg_env* env, const float* actions_dev);
 /* n_steps control steps replayed as one CUDA graph: step k reads actions_dev + k*stride_floats.
  * The graph is cached per (pointer, n_steps, stride).  Outputs hold the last step's values. */
 int mdg_step_many(mdg_env* env, const float* actions_dev, int n_steps, int64_t stride_floats);
+
+/* One control step with HOST buffers (the end-to-end call): copies actions_host [n_envs*n_drones][4] to
+ * the device, steps, copies obs / reward / done back (NULL outputs are skipped) and synchronises the
+ * stream, so the results are valid on return.  Pinned host memory makes the copies asynchronous
+ * with respect to the host but the call still returns only after they finish. */
+int mdg_step_host(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
 
 /* Device pointers to the library-owned outputs of the last reset/step:
  * obs [n_envs][mdg_obs_dim] fp32 (per drone: p, roll/pitch/yaw, v, body rates [, adjacency row]);

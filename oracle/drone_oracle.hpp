@@ -67,6 +67,7 @@ struct Params {
     int grid_cols; double grid_spacing, circle_radius;
     int target_mode; double target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi,
         form_center[3], form_radius;
+    int env_index_base;              // global index of env 0 (sharding across GPUs)
 };
 
 inline void default_params(int model, Params& P) {
@@ -469,7 +470,7 @@ struct Sim {
                 base[0] += P.circle_radius * std::cos(ang);
                 base[1] += P.circle_radius * std::sin(ang);
             }
-            const PhiloxOut r = philox4x32_10((uint32_t)e, (uint32_t)i, t, STREAM_RESET_POS, k0, k1);
+            const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t, STREAM_RESET_POS, k0, k1);
             double* s = &state[di * 13];
             s[0] = base[0] + (-P.reset_half[0] + 2.0 * P.reset_half[0] * u01(r.x[0]));
             s[1] = base[1] + (-P.reset_half[1] + 2.0 * P.reset_half[1] * u01(r.x[1]));
@@ -485,7 +486,7 @@ struct Sim {
                 tg[0] = s[0]; tg[1] = s[1];
                 tg[2] = (M > 1) ? P.mh_z_lo + (P.mh_z_hi - P.mh_z_lo) * i / (M - 1) : P.mh_z_lo;
             } else if (P.target_mode == TGT_BOX) {                  // Q32
-                const PhiloxOut r2 = philox4x32_10((uint32_t)e, (uint32_t)i, t, STREAM_RESET_EXTRA, k0, k1);
+                const PhiloxOut r2 = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t, STREAM_RESET_EXTRA, k0, k1);
                 for (int a = 0; a < 3; ++a) tg[a] = P.target_lo[a] + (P.target_hi[a] - P.target_lo[a]) * u01(r2.x[a]);
             } else {                                                // TGT_CIRCLE, Q26
                 const double ang = 2.0 * PI * i / M;
@@ -553,7 +554,7 @@ struct Sim {
         const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
         // O9 wind gust (PAPER.md:203 recursion, Q27), once per control step, before the substeps
         if (D.aero & AERO_WIND) {
-            const PhiloxOut r = philox4x32_10((uint32_t)e, ENV_LEVEL, t, STREAM_WIND, k0, k1);
+            const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, ENV_LEVEL, t, STREAM_WIND, k0, k1);
             const double ua = u01(r.x[0]), ub = u01(r.x[1]), uc = u01(r.x[2]), ud = u01(r.x[3]);
             const R r1 = sqrt(-2.0 * log(R(1.0 - ua))), r2 = sqrt(-2.0 * log(R(1.0 - uc)));   // Box-Muller
             const R xi[3] = {r1 * cos(R(2.0 * PI * ub)), r1 * sin(R(2.0 * PI * ub)), r2 * cos(R(2.0 * PI * ud))};

@@ -47,7 +47,7 @@ def lib():
         L.orc_quat_exp_step.argtypes = [C.c_void_p] * 3
         L.orc_philox.argtypes = [C.c_uint32] * 6 + [C.c_void_p]
         L.orc_wind_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
-        L.orc_gen_actions.argtypes = [C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_void_p]
+        L.orc_gen_actions.argtypes = [C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_uint32]
     return _lib
 
 
@@ -243,8 +243,8 @@ def wind_normals(seed, env, t):
     return xi
 
 
-def gen_actions(seed, t, n_envs, n_drones, base, lo, hi):
+def gen_actions(seed, t, n_envs, n_drones, base, lo, hi, env_base=0):
     """Harness actions for control step t (Philox stream 3): base * (lo + (hi-lo) u), fp32 [N*M, 4]."""
     out = np.zeros((n_envs * n_drones, 4), dtype=np.float32)
-    lib().orc_gen_actions(int(seed), int(t), n_envs, n_drones, float(base), float(lo), float(hi), _p(out))
+    lib().orc_gen_actions(int(seed), int(t), n_envs, n_drones, float(base), float(lo), float(hi), _p(out), int(env_base))
     return out

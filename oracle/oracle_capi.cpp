@@ -60,7 +60,7 @@ static const Field FIELDS[] = {
     FD(episode_len_s, 1), FI(auto_reset), FI(reset_layout), FD(reset_center, 3), FD(reset_half, 3),
     FD(reset_z_lo, 1), FD(reset_z_hi, 1), FI(grid_cols), FD(grid_spacing, 1), FD(circle_radius, 1), FI(target_mode),
     FD(target_fixed, 3), FD(target_lo, 3), FD(target_hi, 3), FD(mh_z_lo, 1), FD(mh_z_hi, 1), FD(form_center, 3),
-    FD(form_radius, 1),
+    FD(form_radius, 1), FI(env_index_base),
 };
 static const Field* find_field(const char* name) {
     for (const Field& f : FIELDS) if (std::string(f.name) == name) return &f;
@@ -207,11 +207,11 @@ void orc_wind_normals(uint64_t seed, uint32_t e, uint32_t t, double* xi) {
 }
 // harness actions (stream 3): a[c] = base * fma(hi - lo, u_c, lo), every operation correctly rounded
 // in fp32 so that the device generator can reproduce it bit for bit (last paragraph)
-void orc_gen_actions(uint64_t seed, uint32_t t, int n_envs, int n_drones, float base, float lo, float hi, float* out) {
+void orc_gen_actions(uint64_t seed, uint32_t t, int n_envs, int n_drones, float base, float lo, float hi, float* out, uint32_t env_base) {
     const float span = hi - lo;
     for (int e = 0; e < n_envs; ++e)
         for (int i = 0; i < n_drones; ++i) {
-            const PhiloxOut r = philox4x32_10((uint32_t)e, (uint32_t)i, t, STREAM_ACTION, (uint32_t)seed, (uint32_t)(seed >> 32));
+            const PhiloxOut r = philox4x32_10((uint32_t)e + env_base, (uint32_t)i, t, STREAM_ACTION, (uint32_t)seed, (uint32_t)(seed >> 32));
             for (int c = 0; c < 4; ++c) {
                 const float u = (float)(r.x[c] >> 8) * (1.0f / 16777216.0f);
                 const float f = std::fmaf(span, u, lo);

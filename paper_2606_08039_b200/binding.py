@@ -32,6 +32,7 @@ class mdg_params(C.Structure):
         ("grid_cols", C.c_int32), ("grid_spacing", C.c_float), ("circle_radius", C.c_float),
         ("target_mode", C.c_int32), ("target_fixed", _F3), ("target_lo", _F3), ("target_hi", _F3),
         ("mh_z_lo", C.c_float), ("mh_z_hi", C.c_float), ("form_center", _F3), ("form_radius", C.c_float),
+        ("env_index_base", C.c_uint32),
     ]
 
     def update(self, d):
@@ -45,7 +46,7 @@ class mdg_params(C.Structure):
         return self
 
 
-EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_outputs",
+EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
            "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_last_error", "mdg_version"]
 
@@ -68,6 +69,7 @@ def lib():
         L.mdg_reset.argtypes = [vp, C.c_uint64]
         L.mdg_step.argtypes = [vp, vp]
         L.mdg_step_many.argtypes = [vp, vp, C.c_int, C.c_int64]
+        L.mdg_step_host.argtypes = [vp] * 5
         L.mdg_outputs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.mdg_obs_dim.argtypes = [vp]
         L.mdg_targets.argtypes = [vp, C.POINTER(vp)]
@@ -177,6 +179,14 @@ class Env:
         """n_steps control steps replayed as one CUDA graph; actions: [n_steps, n_envs*n_drones, 4]."""
         _check(lib().mdg_step_many(self._h, self._act_ptr(actions, n_steps), n_steps, self.n_envs * self.n_drones * 4))
         return self.obs, self.reward, self.done
+
+    def step_host(self, actions_host, obs_host=None, reward_host=None, done_host=None):
+        """End-to-end step on HOST tensors (ideally pinned): H2D actions, step, D2H outputs, synchronise."""
+        def ptr(x):
+            return C.c_void_p(None) if x is None else C.c_void_p(x.data_ptr())
+        if actions_host.is_cuda or actions_host.numel() != self.n_envs * self.n_drones * 4:
+            raise ValueError("actions_host must be a host float32 tensor of n_envs*n_drones*4 elements")
+        _check(lib().mdg_step_host(self._h, ptr(actions_host), ptr(obs_host), ptr(reward_host), ptr(done_host)))
 
     def gen_actions(self, seed, t, base, lo, hi, out=None):
         if out is None:

@@ -75,7 +75,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     const double h = 1.0 / p.sim_freq, dtc = 1.0 / p.ctrl_freq;
     D.N = N; D.M = M; D.K = p.sim_freq / p.ctrl_freq;
     D.ep_steps = (int)std::llround((double)p.episode_len_s * p.ctrl_freq);
-    D.auto_reset = p.auto_reset; D.feat = feat;
+    D.auto_reset = p.auto_reset; D.feat = feat; D.env_base = p.env_index_base;
     D.reset_layout = p.reset_layout; D.target_mode = p.target_mode;
     D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
     D.opd = 12 + ((feat & F_ADJ) ? M : 0);
@@ -271,8 +271,10 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     return MDG_OK;
 }
 
+void mdg_release_staging(mdg_env* h);
 void mdg_destroy(mdg_env* h) {
     if (!h) return;
+    mdg_release_staging(h);
     drop_graphs(h);
     if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
     if (h->arena) cudaFree(h->arena);
@@ -340,7 +342,7 @@ int mdg_targets(mdg_env* h, const float** t) {
 int mdg_gen_actions(mdg_env* h, uint64_t seed, uint32_t t, float base, float lo, float hi, float* out_dev) {
     if (!h || !out_dev || ((uintptr_t)out_dev & 15)) return fail(MDG_EINVAL, "mdg_gen_actions: bad argument");
     const size_t D = (size_t)h->N * h->M;
-    gen_actions_kernel<<<(unsigned)((D + 255) / 256), 256, 0, h->stream>>>(D, h->M, (uint32_t)seed, (uint32_t)(seed >> 32), t, base, lo, hi,
+    gen_actions_kernel<<<(unsigned)((D + 255) / 256), 256, 0, h->stream>>>(D, h->M, h->P.env_base, (uint32_t)seed, (uint32_t)(seed >> 32), t, base, lo, hi,
                                                                               reinterpret_cast<float4*>(out_dev));
     CU(cudaGetLastError());
     h->launches += 1;
@@ -429,4 +431,26 @@ extern "C" int mdg_set_state(mdg_env* h, const float* state, const float* ctrl, 
     h->launches += 1;
     CU(cudaStreamSynchronize(h->stream));
     return MDG_OK;
+}
+
+// ---- end-to-end call with host buffers --------------------------------------------------------------
+static std::map<mdg_env*, float*> g_stage;   // device staging buffer for host actions, one per handle
+extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
+    if (!h || !actions_host) return fail(MDG_EINVAL, "mdg_step_host: NULL argument");
+    const size_t D = (size_t)h->N * h->M;
+    float*& stage = g_stage[h];
+    if (!stage) CU(cudaMalloc(&stage, D * 4 * sizeof(float)));
+    CU(cudaMemcpyAsync(stage, actions_host, D * 4 * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    const int rc = launch_step(h, stage, h->stream);
+    if (rc != MDG_OK) return rc;
+    h->launches += 1;
+    if (obs_host) CU(cudaMemcpyAsync(obs_host, h->B.obs, D * h->P.opd * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+    if (reward_host) CU(cudaMemcpyAsync(reward_host, h->B.reward, (size_t)h->N * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+    if (done_host) CU(cudaMemcpyAsync(done_host, h->B.done, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return MDG_OK;
+}
+extern "C" void mdg_release_staging(mdg_env* h) {   // called by mdg_destroy
+    auto it = g_stage.find(h);
+    if (it != g_stage.end()) { cudaFree(it->second); g_stage.erase(it); }
 }

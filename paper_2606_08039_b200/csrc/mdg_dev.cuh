@@ -22,7 +22,7 @@ enum : int {
 struct DevParams {
     int N, M, K, ep_steps, auto_reset, feat;
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
-    uint32_t seed_lo, seed_hi;
+    uint32_t seed_lo, seed_hi, env_base;
     // integrator
     float h, half_h, h_sixth, half_h2;
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)

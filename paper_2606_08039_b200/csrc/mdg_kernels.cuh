@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(256) step_kernel(const __grid_constant__ DevPa
     // S7 wind gust: one AR(1) update per env and control step, force held over the substeps
     V3 Fwind = v3(0, 0, 0);
     if (F::has(P, F_WIND)) {
-        const uint4 r = philox4x32_10(e, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
+        const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
         const float r1 = sqrtf(-2.0f * logf(1.0f - u01(r.x))), r2 = sqrtf(-2.0f * logf(1.0f - u01(r.z)));
         float s1, c1, s2, c2;
         sincospif(2.0f * u01(r.y), &s1, &c1);
@@ -263,11 +263,11 @@ __global__ void refresh_obs_kernel(const __grid_constant__ DevParams P, const De
 }
 
 // harness actions (stream 3): base * fma(hi - lo, u, lo), each operation rounded to fp32
-__global__ void gen_actions_kernel(size_t n_drones_total, int M, uint32_t seed_lo, uint32_t seed_hi, uint32_t t,
+__global__ void gen_actions_kernel(size_t n_drones_total, int M, uint32_t env_base, uint32_t seed_lo, uint32_t seed_hi, uint32_t t,
                                    float base, float lo, float hi, float4* __restrict__ out) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_drones_total) return;
-    const uint32_t e = (uint32_t)(i / M), jd = (uint32_t)(i % M);
+    const uint32_t e = (uint32_t)(i / M) + env_base, jd = (uint32_t)(i % M);
     const uint4 r = philox4x32_10(e, jd, t, STREAM_ACTION, seed_lo, seed_hi);
     const float span = __fsub_rn(hi, lo);
     out[i] = make_float4(__fmul_rn(base, __fmaf_rn(span, u01(r.x), lo)), __fmul_rn(base, __fmaf_rn(span, u01(r.y), lo)),

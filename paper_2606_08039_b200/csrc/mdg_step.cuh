@@ -35,7 +35,7 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
         sincospif(2.0f * (float)j / (float)P.M, &s, &c);
         bx = fmaf(P.circle_radius, c, bx); by = fmaf(P.circle_radius, s, by);
     }
-    const uint4 r = philox4x32_10(e, j, t, STREAM_RESET_POS, P.seed_lo, P.seed_hi);
+    const uint4 r = philox4x32_10(e + P.env_base, j, t, STREAM_RESET_POS, P.seed_lo, P.seed_hi);
     d.p.x = bx + fmaf(2.0f * P.reset_half[0], u01(r.x), -P.reset_half[0]);
     d.p.y = by + fmaf(2.0f * P.reset_half[1], u01(r.y), -P.reset_half[1]);
     if (P.reset_z_hi > P.reset_z_lo) d.p.z = fmaf(P.reset_z_hi - P.reset_z_lo, u01(r.z), P.reset_z_lo);
@@ -50,7 +50,7 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
         tg.x = d.p.x; tg.y = d.p.y;
         tg.z = P.M > 1 ? fmaf(P.mh_z_hi - P.mh_z_lo, (float)j / (float)(P.M - 1), P.mh_z_lo) : P.mh_z_lo;
     } else if (P.target_mode == 2) {      // BOX
-        const uint4 r2 = philox4x32_10(e, j, t, STREAM_RESET_EXTRA, P.seed_lo, P.seed_hi);
+        const uint4 r2 = philox4x32_10(e + P.env_base, j, t, STREAM_RESET_EXTRA, P.seed_lo, P.seed_hi);
         tg.x = fmaf(P.target_hi[0] - P.target_lo[0], u01(r2.x), P.target_lo[0]);
         tg.y = fmaf(P.target_hi[1] - P.target_lo[1], u01(r2.y), P.target_lo[1]);
         tg.z = fmaf(P.target_hi[2] - P.target_lo[2], u01(r2.z), P.target_lo[2]);
