@@ -39,7 +39,7 @@ struct mdg_env {
     step_fn step = nullptr;
     aux_fn reset = nullptr, refresh = nullptr;
     std::string kernel_name;
-    int block = 128, max_blocks_per_sm = 0, smem = 0;
+    int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
     int64_t launches = 0;
     std::map<std::tuple<const void*, int, int64_t>, cudaGraphExec_t> graphs;
 };
@@ -108,8 +108,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.int_clamp_pos = p.int_clamp_pos; D.int_clamp_att = p.int_clamp_att;
     D.pos_step_max = (float)(p.pos_rate_limit * dtc); D.yaw_step_max = (float)(p.yaw_rate_limit * dtc);
     D.tilt_max = p.tilt_max; D.tau_xy_max = p.tau_xy_max; D.tau_z_max = p.tau_z_max;
-    D.adj_radius = p.adj_radius; D.at_target_radius = p.at_target_radius;
-    D.term_tilt = p.term_tilt; D.term_dist = p.term_dist; D.z_max = p.z_max;
+    D.adj_radius2 = (float)((double)p.adj_radius * p.adj_radius); D.at_target_radius2 = (float)((double)p.at_target_radius * p.at_target_radius);
+    D.term_tilt = p.term_tilt; D.term_dist2 = (float)((double)p.term_dist * p.term_dist); D.z_max = p.z_max;
     D.reset_z_lo = p.reset_z_lo; D.reset_z_hi = p.reset_z_hi; D.grid_spacing = p.grid_spacing; D.circle_radius = p.circle_radius;
     D.mh_z_lo = p.mh_z_lo; D.mh_z_hi = p.mh_z_hi; D.form_radius = p.form_radius;
 }
@@ -123,17 +123,28 @@ static constexpr int FEAT_C3 = FEATW(0, 0, 1, 1, 0, 1, 2);
 static constexpr int FEAT_C4 = FEATW(7, 0, 0, 0, 0, 2, 1);
 static constexpr int FEAT_C5 = FEATW(15, 0, 2, 0, 1, 3, 3);
 
+// register budget variants of one specialisation: MINB resident 128-thread blocks per SM
+template <int G, int FEAT> static step_fn pick_minb(int minb) {
+    switch (minb) {
+        case 5: return step_kernel<G, FEAT, 5>;
+        case 6: return step_kernel<G, FEAT, 6>;
+        case 7: return step_kernel<G, FEAT, 7>;
+        case 8: return step_kernel<G, FEAT, 8>;
+        default: return step_kernel<G, FEAT, 4>;
+    }
+}
+
 static void pick_kernels(mdg_env* h) {
     const int f = h->P.feat;
     h->step = nullptr;
-#define SPECIAL(g, fw, name) if (h->G == g && f == fw) { h->step = step_kernel<g, fw>; h->kernel_name = name; }
+#define SPECIAL(g, fw, name) if (h->G == g && f == fw) { h->step = pick_minb<g, fw>(h->minb); h->kernel_name = name; }
     SPECIAL(1, FEAT_C1, "step_kernel<G=1,rigid,rpm,hover>")
     SPECIAL(1, FEAT_C2, "step_kernel<G=1,gnd+drag,rpm,hover>")
     SPECIAL(1, FEAT_C3, "step_kernel<G=1,rigid,pid+dsl,negsqdist>")
     SPECIAL(8, FEAT_C4, "step_kernel<G=8,gnd+drag+dw,rpm,multihover>")
     SPECIAL(4, FEAT_C5, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation>")
 #undef SPECIAL
-#define GENERIC(g) case g: if (!h->step) { h->step = step_kernel<g, -1>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
+#define GENERIC(g) case g: if (!h->step) { h->step = step_kernel<g, -1, 4>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
                    h->reset = reset_kernel<g>; h->refresh = refresh_obs_kernel<g>; break;
     switch (h->G) { GENERIC(1) GENERIC(2) GENERIC(4) GENERIC(8) GENERIC(16) GENERIC(32) }
 #undef GENERIC
@@ -359,12 +370,16 @@ const char* mdg_kernel_name(const mdg_env* h) { return h ? h->kernel_name.c_str(
 int mdg_set_launch(mdg_env* h, int block_threads, int max_blocks_per_sm) {
     if (!h) return fail(MDG_EINVAL, "mdg_set_launch: NULL handle");
     if (block_threads) {
-        if (block_threads < 32 || block_threads > 256 || (block_threads & 31)) return fail(MDG_EINVAL, "mdg_set_launch: block must be a multiple of 32 in [32, 256]");
+        if (block_threads < 32 || block_threads > 128 || (block_threads & 31)) return fail(MDG_EINVAL, "mdg_set_launch: block must be a multiple of 32 in [32, 128]");
         h->block = block_threads;
     }
     if (max_blocks_per_sm) {
         if (max_blocks_per_sm < 0 || max_blocks_per_sm > 32) return fail(MDG_EINVAL, "mdg_set_launch: max_blocks_per_sm in [1, 32]");
         h->max_blocks_per_sm = max_blocks_per_sm;
+        // register-budget variant: resident 128-thread blocks per SM the allocation must allow (4..8)
+        const int per128 = (max_blocks_per_sm * h->block + 127) / 128;
+        h->minb = per128 < 4 ? 4 : (per128 > 8 ? 8 : per128);
+        pick_kernels(h);
     }
     drop_graphs(h);
     return configure_launch(h);

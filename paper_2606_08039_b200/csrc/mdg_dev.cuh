@@ -36,7 +36,7 @@ struct DevParams {
     float Kp_pos[3], Ki_pos[3], Kd_pos[3], Kp_att[3], Ki_att[3], Kd_att[3];
     float int_clamp_pos, int_clamp_att, pos_step_max, yaw_step_max, a_ff[3], tilt_max, tau_xy_max, tau_z_max;
     // epilogue
-    float adj_radius, at_target_radius, term_tilt, term_dist, term_center[3], z_max;
+    float adj_radius2, at_target_radius2, term_tilt, term_dist2, term_center[3], z_max;   // radii squared
     // reset / targets
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
     float target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi, form_center[3], form_radius;
@@ -74,6 +74,11 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 }
 __device__ __forceinline__ float u01(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }
 
+// MUFU approximations with flush-to-zero: a single SFU instruction each, no denormal rescaling code
+__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_fast(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float ex2_fast(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 struct V3 { float x, y, z; };
 __device__ __forceinline__ V3 v3(float x, float y, float z) { V3 r; r.x = x; r.y = y; r.z = z; return r; }
 __device__ __forceinline__ V3 cross(V3 a, V3 b) {
@@ -84,10 +89,9 @@ struct Q4 { float w, x, y, z; };
 // rotate v by unit quaternion q (body -> world): v + w t + u x t, t = 2 u x v
 __device__ __forceinline__ V3 rot(Q4 q, V3 v) {
     const V3 u = v3(q.x, q.y, q.z);
-    V3 t = cross(u, v);
-    t.x += t.x; t.y += t.y; t.z += t.z;
+    const V3 t = cross(u, v);
     const V3 c = cross(u, t);
-    return v3(fmaf(q.w, t.x, v.x) + c.x, fmaf(q.w, t.y, v.y) + c.y, fmaf(q.w, t.z, v.z) + c.z);
+    return v3(fmaf(2.0f, fmaf(q.w, t.x, c.x), v.x), fmaf(2.0f, fmaf(q.w, t.y, c.y), v.y), fmaf(2.0f, fmaf(q.w, t.z, c.z), v.z));
 }
 // rotate v by the conjugate of q (world -> body)
 __device__ __forceinline__ V3 rot_inv(Q4 q, V3 v) {
@@ -103,23 +107,37 @@ __device__ __forceinline__ Q4 qmul(Q4 a, Q4 b) {
     return r;
 }
 // Eq.7 increment: [cos(|phi|/2), sin(|phi|/2) phi/|phi|].  Both factors are even power series in
-// x = |phi|^2, so for x <= 1 (|omega| h <= 1 rad) no sqrt, division or MUFU is needed; truncation
-// error < 3e-10.  Larger angles take the library path.
+// x = |phi|^2, so no sqrt, division or MUFU is needed.  Degree 4 in x: truncation error < 3e-9 for
+// |phi| <= 1.5 rad.  The caller routes |omega| h > 1 rad to the exact (library sin/cos) path.
 __device__ __forceinline__ Q4 exp_half(V3 phi) {
     const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
-    float c, s;
-    if (x <= 1.0f) {
-        c = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 9.6881200e-8f, -2.1701389e-5f), 2.6041667e-3f), -0.125f), 1.0f);
-        s = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 5.3822889e-9f, -1.5500992e-6f), 2.6041667e-4f), -2.0833333e-2f), 0.5f);
-    } else {
-        const float n = sqrtf(x);
-        float sn, cn;
-        sincosf(0.5f * n, &sn, &cn);
-        c = cn; s = sn / n;
-    }
+    const float c = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 9.6881200e-8f, -2.1701389e-5f), 2.6041667e-3f), -0.125f), 1.0f);
+    const float s = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 5.3822889e-9f, -1.5500992e-6f), 2.6041667e-4f), -2.0833333e-2f), 0.5f);
     Q4 r; r.w = c; r.x = s * phi.x; r.y = s * phi.y; r.z = s * phi.z;
     return r;
 }
+__device__ __forceinline__ Q4 exp_half_exact(V3 phi) {
+    const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
+    if (x <= 1.0f) return exp_half(phi);
+    const float n = sqrtf(x);
+    float sn, cn;
+    sincosf(0.5f * n, &sn, &cn);
+    const float s = sn / n;
+    Q4 r; r.w = cn; r.x = s * phi.x; r.y = s * phi.y; r.z = s * phi.z;
+    return r;
+}
+// R(phi)^T tau for a rotation VECTOR phi (Rodrigues; both coefficients are series in x = |phi|^2,
+// degree 4: error < 2e-7 for |phi| <= 1.5 rad).  Used for the RK4 stage torques.
+__device__ __forceinline__ V3 rotvec_inv(V3 phi, V3 tau) {
+    const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
+    const float A = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 2.7557319e-6f, -1.9841270e-4f), 8.3333333e-3f), -0.16666667f), 1.0f);
+    const float Bc = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 2.7557319e-7f, -2.4801587e-5f), 1.3888889e-3f), -4.1666667e-2f), 0.5f);
+    const V3 c1 = cross(phi, tau);
+    const V3 c2 = cross(phi, c1);
+    return v3(fmaf(Bc, c2.x, fmaf(-A, c1.x, tau.x)), fmaf(Bc, c2.y, fmaf(-A, c1.y, tau.y)), fmaf(Bc, c2.z, fmaf(-A, c1.z, tau.z)));
+}
+// sqrt(x) for x >= 0 to ~2 ulp: one MUFU.RSQ and one multiply
+__device__ __forceinline__ float fast_sqrt(float x) { return x > 1e-30f ? x * rsqrt_fast(x) : 0.0f; }
 __device__ __forceinline__ float clampf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
 __device__ __forceinline__ float wrap_pi(float x) {
     const float k = ceilf((x - 3.14159265358979f) * 0.159154943091895f);

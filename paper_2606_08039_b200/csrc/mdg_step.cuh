@@ -71,10 +71,15 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
         n[2] = clampf(a.z, 0.0f, P.max_rpm); n[3] = clampf(a.w, 0.0f, P.max_rpm);
         return;
     }
-    const V3 eta = euler_zyx(d.q);
-    float spsi, cpsi;
-    sincosf(eta.z, &spsi, &cpsi);
-    V3 e_p, v_ref; float psi_ref;
+    // roll, pitch and the heading direction (cos psi, sin psi) = normalised (1 - 2(y^2+z^2), 2(wz+xy))
+    V3 eta;
+    eta.x = atan2f(2.0f * (d.q.w * d.q.x + d.q.y * d.q.z), 1.0f - 2.0f * (d.q.x * d.q.x + d.q.y * d.q.y));
+    eta.y = asinf(clampf(2.0f * (d.q.w * d.q.y - d.q.z * d.q.x), -1.0f, 1.0f));
+    const float hc = 1.0f - 2.0f * (d.q.y * d.q.y + d.q.z * d.q.z), hs = 2.0f * (d.q.w * d.q.z + d.q.x * d.q.y);
+    const float hn2 = fmaf(hc, hc, hs * hs);
+    const float hr = hn2 > 1e-30f ? rsqrt_fast(hn2) : 0.0f;
+    const float cpsi = hn2 > 1e-30f ? hc * hr : 1.0f, spsi = hs * hr;
+    V3 e_p, v_ref; float e_psi;
     if (act == 1) {                       // PID waypoint [x, y, z, psi]
         if (Feat<FEAT>::has(P, F_DSL)) {
             const V3 dv = v3(a.x - d.sp.x, a.y - d.sp.y, a.z - d.sp.z);
@@ -87,11 +92,11 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
             d.sp.w = wrap_pi(d.sp.w + dpsi);
         } else d.sp = a;
         e_p = v3(d.sp.x - d.p.x, d.sp.y - d.p.y, d.sp.z - d.p.z);
-        v_ref = v3(0, 0, 0); psi_ref = d.sp.w;
+        v_ref = v3(0, 0, 0); e_psi = wrap_pi(d.sp.w - atan2f(hs, hc));
     } else {                              // VEL [vx, vy, vz, wz] in the heading frame
         e_p = v3(0, 0, 0);
         v_ref = v3(cpsi * a.x - spsi * a.y, spsi * a.x + cpsi * a.y, a.z);
-        psi_ref = fmaf(a.w, P.dt_c, eta.z);
+        e_psi = wrap_pi(a.w * P.dt_c);                             // psi* = psi + wz dt
     }
     // position loop, Eq.9
     d.Ip.x = clampf(fmaf(e_p.x, P.dt_c, d.Ip.x), -P.int_clamp_pos, P.int_clamp_pos);
@@ -100,10 +105,10 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     const float ax = fmaf(P.Kp_pos[0], e_p.x, fmaf(P.Ki_pos[0], d.Ip.x, fmaf(P.Kd_pos[0], v_ref.x - d.v.x, P.a_ff[0])));
     const float ay = fmaf(P.Kp_pos[1], e_p.y, fmaf(P.Ki_pos[1], d.Ip.y, fmaf(P.Kd_pos[1], v_ref.y - d.v.y, P.a_ff[1])));
     const float az = fmaf(P.Kp_pos[2], e_p.z, fmaf(P.Ki_pos[2], d.Ip.z, fmaf(P.Kd_pos[2], v_ref.z - d.v.z, P.a_ff[2]))) + P.g;
-    const float T = clampf(P.m * sqrtf(fmaf(ax, ax, fmaf(ay, ay, az * az))), 0.0f, P.T_max);
+    const float T = clampf(P.m * fast_sqrt(fmaf(ax, ax, fmaf(ay, ay, az * az))), 0.0f, P.T_max);
     const float phi_ref = clampf((ax * spsi - ay * cpsi) * P.inv_g, -P.tilt_max, P.tilt_max);
     const float th_ref = clampf((ax * cpsi + ay * spsi) * P.inv_g, -P.tilt_max, P.tilt_max);
-    const V3 e_eta = v3(phi_ref - eta.x, th_ref - eta.y, wrap_pi(psi_ref - eta.z));
+    const V3 e_eta = v3(phi_ref - eta.x, th_ref - eta.y, e_psi);
     d.Ie.x = clampf(fmaf(e_eta.x, P.dt_c, d.Ie.x), -P.int_clamp_att, P.int_clamp_att);
     d.Ie.y = clampf(fmaf(e_eta.y, P.dt_c, d.Ie.y), -P.int_clamp_att, P.int_clamp_att);
     d.Ie.z = clampf(fmaf(e_eta.z, P.dt_c, d.Ie.z), -P.int_clamp_att, P.int_clamp_att);
@@ -114,8 +119,8 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     const float qa = tx * P.inv_l, qb = ty * P.inv_l, qc = tz * P.inv_kappa;
     const float s0 = 0.25f * (T + qa - qb - qc), s1 = 0.25f * (T + qa + qb + qc);
     const float s2 = 0.25f * (T - qa + qb - qc), s3 = 0.25f * (T - qa - qb + qc);
-    n[0] = sqrtf(clampf(s0, 0.0f, P.s_max) * P.inv_k_f); n[1] = sqrtf(clampf(s1, 0.0f, P.s_max) * P.inv_k_f);
-    n[2] = sqrtf(clampf(s2, 0.0f, P.s_max) * P.inv_k_f); n[3] = sqrtf(clampf(s3, 0.0f, P.s_max) * P.inv_k_f);
+    n[0] = fast_sqrt(clampf(s0, 0.0f, P.s_max) * P.inv_k_f); n[1] = fast_sqrt(clampf(s1, 0.0f, P.s_max) * P.inv_k_f);
+    n[2] = fast_sqrt(clampf(s2, 0.0f, P.s_max) * P.inv_k_f); n[3] = fast_sqrt(clampf(s3, 0.0f, P.s_max) * P.inv_k_f);
 }
 
 // angular acceleration J^-1 (tau_body - w x J w)
@@ -161,8 +166,7 @@ __device__ __forceinline__ void adjacency(const DevParams& P, V3 p, int lane, in
         const float ox = __shfl_sync(MDG_FULL, p.x, gbase + k), oy = __shfl_sync(MDG_FULL, p.y, gbase + k),
                     oz = __shfl_sync(MDG_FULL, p.z, gbase + k);
         const float dx = p.x - ox, dy = p.y - oy, dz = p.z - oz;
-        const float dist = sqrtf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
-        adj[k] = (k == j || dist < P.adj_radius) ? 1.0f : 0.0f;
+        adj[k] = (k == j || fmaf(dx, dx, fmaf(dy, dy, dz * dz)) < P.adj_radius2) ? 1.0f : 0.0f;
     }
 }
 
