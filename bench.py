@@ -249,9 +249,12 @@ def run_ours(args, wl, c):
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
     achieved_tf = flops / per_launch_s / 1e12
     t_alu, t_hbm = flops / (ALU_PEAK_TFLOPS * 1e12), bytes_alg / (hbm_peak * 1e9)
-    traffic = None
+    traffic = None                                         # dram read + write bytes per launch, one ncu --set full capture
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"c{c}")
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv"))):
+            if row["config"] == f"c{c}":
+                traffic = float(row["traffic_bytes"])
     except Exception:
         pass
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
