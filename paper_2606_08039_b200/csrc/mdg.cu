@@ -3,6 +3,7 @@
 // kernels of mdg_kernels.cuh.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <string>
@@ -40,11 +41,13 @@ struct mdg_env {
     aux_fn reset = nullptr, refresh = nullptr;
     std::string kernel_name;
     int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
+    int pdl = 1;
+    int n_sms = 0, step_grid = 0;        // persistent step kernel: one block per resident slot, looping over tiles
     int64_t launches = 0;
     std::map<std::tuple<const void*, int, int64_t>, cudaGraphExec_t> graphs;
 };
 
-static int feature_word(const mdg_params& p, int physics_mode, int action_type) {
+static int feature_word(const mdg_params& p, int physics_mode, int action_type, int M, int G) {
     int aero = 0, integ = MDG_INTEG_RK4;                  // Table 1
     switch (physics_mode) {
         case MDG_PHYS_MJC_GND: aero = MDG_AERO_GND; break;
@@ -56,13 +59,14 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type) 
     }
     if (p.aero_mask >= 0) aero = p.aero_mask & 15;
     if (p.integrator >= 0) integ = p.integrator;
-    int f = aero;
+    int f = aero | (M == G ? F_FULL : 0);
     if (integ == MDG_INTEG_EULER) f |= F_EULER;
     f |= action_type << F_ACT_SHIFT;
     if (action_type == MDG_ACT_PID && p.dsl) f |= F_DSL;
     if (p.obs_mode == MDG_OBS_KIN12_ADJ) f |= F_ADJ;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
+    if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
     return f;
 }
 
@@ -80,6 +84,13 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
     D.opd = 12 + ((feat & F_ADJ) ? M : 0);
     D.h = (float)h; D.half_h = (float)(0.5 * h); D.h_sixth = (float)(h / 6.0); D.half_h2 = (float)(0.5 * h * h);
+    D.w2_exact = (float)((0.75 / h) * (0.75 / h));
+    for (int s = 0; s < 2; ++s) {                                  // Rodrigues series of R(c w)^T in y = |w|^2
+        const double c = s ? h : 0.5 * h, c2 = c * c;
+        float* A = s ? D.rotA_full : D.rotA_half; float* Bc = s ? D.rotB_full : D.rotB_half;
+        A[0] = (float)c; A[1] = (float)(-c * c2 / 6.0); A[2] = (float)(c * c2 * c2 / 120.0); A[3] = (float)(-c * c2 * c2 * c2 / 5040.0);
+        Bc[0] = (float)(c2 / 2.0); Bc[1] = (float)(-c2 * c2 / 24.0); Bc[2] = (float)(c2 * c2 * c2 / 720.0); Bc[3] = (float)(-c2 * c2 * c2 * c2 / 40320.0);
+    }
     D.inv_m = (float)(1.0 / p.m); D.g = p.g; D.m = p.m; D.inv_g = (float)(1.0 / p.g);
     for (int i = 0; i < 3; ++i) { D.J[i] = p.J[i]; D.invJ[i] = (float)(1.0 / p.J[i]); }
     D.gyro[0] = (float)(((double)p.J[2] - p.J[1]) / p.J[0]);
@@ -93,7 +104,10 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.gnd_coef = (float)((double)p.C_gnd * (p.r_p / 4.0) * (p.r_p / 4.0)); D.h_clip = p.h_clip;
     D.c_xy = p.c_xy; D.c_z = p.c_z;
     D.dw_coef = (float)((double)p.dw_C1 * (p.r_p / 4.0) * (p.r_p / 4.0)); D.dw_C2 = p.dw_C2; D.dw_C3 = p.dw_C3;
-    D.dz_clip = p.dw_dz_clip; D.inv_dz_clip = p.dw_dz_clip > 0 ? (float)(1.0 / p.dw_dz_clip) : 0.0f;
+    D.dz_clip = p.dw_dz_clip; D.inv_dz_clip = p.dw_dz_clip > 0 ? (float)(1.0 / p.dw_dz_clip) : INFINITY;   // saturate(dz * inf) = [dz > 0]
+    const double s2ln2 = std::sqrt(2.0 * std::log(2.0));
+    D.dw_C2s = (float)(p.dw_C2 * s2ln2); D.dw_C3s = (float)(p.dw_C3 * s2ln2); D.dw_b2_min = (float)(2.0 * std::log(2.0) * 1e-12);
+    D.dz_floor = p.dw_dz_clip > 1e-6f ? p.dw_dz_clip : 1e-6f;
     const double alpha = std::exp(-dtc / p.wind_tau);
     D.wind_alpha = (float)alpha; D.wind_gain = (float)(p.wind_sigma * std::sqrt(1.0 - alpha * alpha)); D.k_wind = p.k_wind;
     D.dt_c = (float)dtc;
@@ -112,16 +126,17 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.term_tilt = p.term_tilt; D.term_dist2 = (float)((double)p.term_dist * p.term_dist); D.z_max = p.z_max;
     D.reset_z_lo = p.reset_z_lo; D.reset_z_hi = p.reset_z_hi; D.grid_spacing = p.grid_spacing; D.circle_radius = p.circle_radius;
     D.mh_z_lo = p.mh_z_lo; D.mh_z_hi = p.mh_z_hi; D.form_radius = p.form_radius;
+    for (int dlt = 0; dlt < 32; ++dlt) D.chord[dlt] = (float)(2.0 * p.form_radius * std::fabs(std::sin(M_PI * dlt / M)));
 }
 
 // ---- kernel dispatch: specialisations for the five benchmark configs, generic otherwise -------------
 #define FEATW(aero, euler, act, dsl, adj, rew, term) \
-    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) ? F_ADJ : 0) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT))
+    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) ? F_ADJ : 0) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT) | F_FULL)
 static constexpr int FEAT_C1 = FEATW(0, 0, 0, 0, 0, 0, 1);
 static constexpr int FEAT_C2 = FEATW(3, 0, 0, 0, 0, 0, 1);
 static constexpr int FEAT_C3 = FEATW(0, 0, 1, 1, 0, 1, 2);
 static constexpr int FEAT_C4 = FEATW(7, 0, 0, 0, 0, 2, 1);
-static constexpr int FEAT_C5 = FEATW(15, 0, 2, 0, 1, 3, 3);
+static constexpr int FEAT_C5 = FEATW(15, 0, 2, 0, 1, 3, 3) | F_TGT_CIRCLE;
 
 // register budget variants of one specialisation: MINB resident 128-thread blocks per SM
 template <int G, int FEAT> static step_fn pick_minb(int minb) {
@@ -159,6 +174,18 @@ static int configure_launch(mdg_env* h) {
         h->smem = s & ~127;
     }
     CU(cudaFuncSetAttribute((const void*)h->step, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem > 48 * 1024 ? h->smem : 48 * 1024));
+    if (!h->n_sms) {
+        int dev = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&h->n_sms, cudaDevAttrMultiProcessorCount, dev));
+    }
+    int resident = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void*)h->step, h->block, h->smem));
+    if (resident < 1) return fail(MDG_ECUDA, "configure_launch: the step kernel does not fit on an SM");
+    const long long epw = 32 / h->G, wpb = h->block / 32;           // envs per work item (one warp), warps per block
+    const long long items = ((long long)h->N + epw - 1) / epw, blocks = (items + wpb - 1) / wpb;
+    const long long slots = (long long)h->n_sms * resident;
+    h->step_grid = (int)(blocks < slots ? blocks : slots);
     return MDG_OK;
 }
 static inline unsigned grid_for(const mdg_env* h, int block) {
@@ -170,8 +197,17 @@ static void drop_graphs(mdg_env* h) {
     h->graphs.clear();
 }
 static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s) {
-    h->step<<<grid_for(h, h->block), h->block, h->smem, s>>>(h->P, h->B, reinterpret_cast<const float4*>(actions_dev));
-    CU(cudaGetLastError());
+    // Programmatic dependent launch: the blocks of this step may become resident while the previous kernel of the
+    // stream drains (it overlaps launch latency, parameter and instruction fetch); the kernel itself waits
+    // (griddepcontrol.wait) for that kernel to complete and flush before it touches memory.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)h->step_grid); cfg.blockDim = dim3((unsigned)h->block);
+    cfg.dynamicSmemBytes = (size_t)h->smem; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = h->pdl ? 1 : 0;
+    CU(cudaLaunchKernelEx(&cfg, h->step, h->P, h->B, reinterpret_cast<const float4*>(actions_dev)));
     return MDG_OK;
 }
 
@@ -254,14 +290,15 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     h->N = n_envs; h->M = n_drones; h->physics_mode = physics_mode; h->action_type = action_type; h->hp = p;
     int G = 1; while (G < n_drones) G <<= 1;
     h->G = G;
-    make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type), h->P);
+    if (const char* ev = std::getenv("MDG_PDL")) h->pdl = ev[0] != '0';   // development knob: MDG_PDL=0 launches plainly
+    make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type, n_drones, G), h->P);
     pick_kernels(h);
     // one arena: 7 drone planes, env plane, gstep, obs, reward, done (each 256 B aligned)
     const size_t D = (size_t)n_envs * n_drones;
     auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const size_t plane = al(D * sizeof(float4)), eplane = al((size_t)n_envs * sizeof(float4)), gs = al((size_t)n_envs * 4),
                  ob = al(D * h->P.opd * sizeof(float)), rw = al((size_t)n_envs * 4), dn = al((size_t)n_envs);
-    h->arena_bytes = 7 * plane + eplane + gs + ob + rw + dn;
+    h->arena_bytes = 7 * plane + eplane + gs + ob + rw + dn + 256;
     cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
     if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
     ce = cudaMemset(h->arena, 0, h->arena_bytes);
@@ -273,7 +310,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     h->B.gstep = (uint32_t*)c; c += gs;
     h->B.obs = (float*)c; c += ob;
     h->B.reward = (float*)c; c += rw;
-    h->B.done = (uint8_t*)c;
+    h->B.done = (uint8_t*)c; c += dn;
+    h->B.ticket = (unsigned*)c;
     int rc = configure_launch(h);
     if (rc != MDG_OK) { cudaFree(h->arena); delete h; return rc; }
     *out = h;
@@ -296,6 +334,7 @@ int mdg_reset(mdg_env* h, uint64_t seed) {
     if (!h) return fail(MDG_EINVAL, "mdg_reset: NULL handle");
     h->P.seed_lo = (uint32_t)seed; h->P.seed_hi = (uint32_t)(seed >> 32);
     drop_graphs(h);                          // captured launches carry the old seed
+    CU(cudaMemsetAsync(h->B.ticket, 0, sizeof(unsigned), h->stream));
     h->reset<<<grid_for(h, 128), 128, 0, h->stream>>>(h->P, h->B);
     CU(cudaGetLastError());
     h->launches += 1;
@@ -469,3 +508,11 @@ extern "C" void mdg_release_staging(mdg_env* h) {   // called by mdg_destroy
     auto it = g_stage.find(h);
     if (it != g_stage.end()) { cudaFree(it->second); g_stage.erase(it); }
 }
+
+#ifdef MDG_TRACE
+extern "C" int mdg_debug_set_trace(void* dev_ptr) {
+    unsigned long long* p = (unsigned long long*)dev_ptr;
+    CU(cudaMemcpyToSymbol(mdg::g_trace, &p, sizeof(p)));
+    return MDG_OK;
+}
+#endif

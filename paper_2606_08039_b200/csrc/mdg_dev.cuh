@@ -15,6 +15,8 @@ enum : int {
     F_ADJ = 256,                                          // MDG_OBS_KIN12_ADJ
     F_REW_SHIFT = 9,                                      // 2 bits: MDG_REW_*
     F_TERM_SHIFT = 11,                                    // 2 bits: MDG_TERM_*
+    F_TGT_CIRCLE = 1 << 13,                               // targets are the formation circle slots (chord table)
+    F_FULL = 1 << 14,                                     // n_drones == G: no padding lanes in a group
 };
 
 // Everything the kernels need, precomputed on the host in double and rounded once to fp32.
@@ -24,12 +26,16 @@ struct DevParams {
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
     uint32_t seed_lo, seed_hi, env_base;
     // integrator
-    float h, half_h, h_sixth, half_h2;
+    float h, half_h, h_sixth, half_h2, w2_exact;          // w2_exact: |omega|^2 above which the exact path runs
+    // Rodrigues coefficients of R(c w)^T as polynomials in y = |w|^2, c = h/2 (stages 2, 3) and h (stage 4):
+    // A(y) = c sin(c|w|)/(c|w|), B(y) = c^2 (1 - cos(c|w|))/(c|w|)^2, degree 3
+    float rotA_half[4], rotB_half[4], rotA_full[4], rotB_full[4];
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
     // motor model (Eq.1-3)
     float k_f, inv_k_f, l, kappa, inv_l, inv_kappa, max_rpm, s_max, T_max, rpm2rad;
     // aero (Eq.4-6) and wind
     float gnd_coef, h_clip, c_xy, c_z, dw_coef, dw_C2, dw_C3, dz_clip, inv_dz_clip;
+    float dw_C2s, dw_C3s, dw_b2_min, dz_floor;            // Eq.6 with beta scaled by sqrt(2 ln 2): exp(-x/2b^2) = 2^(-x/b'^2)
     float wind_alpha, wind_gain, k_wind;
     // cascaded PID (Eq.9, Table 6)
     float dt_c, m, inv_g;
@@ -40,6 +46,7 @@ struct DevParams {
     // reset / targets
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
     float target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi, form_center[3], form_radius;
+    float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 
 // SoA state planes (float4 per drone) and per-env words.  DESIGN.md §5.
@@ -53,6 +60,7 @@ struct DevBuffers {
     float4* P6;   // target x y z psi
     float4* E0;   // wind x y z, bits(ep_step)
     uint32_t* gstep;
+    unsigned* ticket;   // work-item dispenser of the step kernel (0 between launches)
     float* obs;
     float* reward;
     uint8_t* done;
@@ -78,6 +86,36 @@ __device__ __forceinline__ float u01(uint32_t x) { return (float)(x >> 8) * (1.0
 __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float rsqrt_fast(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float ex2_fast(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+__device__ __forceinline__ float lg2_fast(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sin_fast(float x) { float r; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float cos_fast(float x) { float r; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// atan2(y, x) to 2e-7 rad: octant reduction to a = min/max in [0, 1], a P(a^2) with a degree-7 minimax P
+// (fitted for this kernel, max error 9e-8), one MUFU.RCP.  atan2(0, 0) = 0.
+__device__ __forceinline__ float atan2_fast(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mx = fmaxf(fmaxf(ax, ay), 1e-30f), mn = fminf(ax, ay);
+    const float a = mn * rcp_fast(mx), s = a * a;
+    float p = fmaf(s, -4.780359644e-3f, 2.455679293e-2f);
+    p = fmaf(s, p, -5.990426529e-2f); p = fmaf(s, p, 9.942728849e-2f); p = fmaf(s, p, -1.402940935e-1f);
+    p = fmaf(s, p, 1.997137346e-1f); p = fmaf(s, p, -3.333209341e-1f); p = fmaf(s, p, 9.999999114e-1f);
+    float r = a * p;
+    r = ay > ax ? 1.57079632679f - r : r;
+    r = x < 0.0f ? 3.14159265359f - r : r;
+    return copysignf(r, y);
+}
+// asin(s) for |s| <= 1 to 1e-7: z + z t Q(t) on |s| <= 1/2 (t = s^2), pi/2 - 2 asin(sqrt((1 - |s|)/2)) above
+__device__ __forceinline__ float asin_fast(float s) {
+    const float a = fabsf(s);
+    const bool big = a > 0.5f;
+    const float t = big ? fmaf(-0.5f, a, 0.5f) : a * a;
+    const float z = big ? t * rsqrt_fast(fmaxf(t, 1e-30f)) : a;
+    float q = fmaf(t, 3.828223139e-2f, 2.645942860e-2f);
+    q = fmaf(t, q, 4.501529088e-2f); q = fmaf(t, q, 7.498796169e-2f); q = fmaf(t, q, 1.666667248e-1f);
+    const float r = fmaf(z * t, q, z);
+    return copysignf(big ? fmaf(-2.0f, r, 1.57079632679f) : r, s);
+}
 
 struct V3 { float x, y, z; };
 __device__ __forceinline__ V3 v3(float x, float y, float z) { V3 r; r.x = x; r.y = y; r.z = z; return r; }
@@ -107,18 +145,18 @@ __device__ __forceinline__ Q4 qmul(Q4 a, Q4 b) {
     return r;
 }
 // Eq.7 increment: [cos(|phi|/2), sin(|phi|/2) phi/|phi|].  Both factors are even power series in
-// x = |phi|^2, so no sqrt, division or MUFU is needed.  Degree 4 in x: truncation error < 3e-9 for
-// |phi| <= 1.5 rad.  The caller routes |omega| h > 1 rad to the exact (library sin/cos) path.
+// x = |phi|^2, so no sqrt, division or MUFU is needed.  Degree 3 in x: truncation error < 1e-8 for
+// |phi| <= 0.75 rad.  The caller routes |omega| h > 0.75 rad to the exact (library sin/cos) path.
 __device__ __forceinline__ Q4 exp_half(V3 phi) {
     const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
-    const float c = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 9.6881200e-8f, -2.1701389e-5f), 2.6041667e-3f), -0.125f), 1.0f);
-    const float s = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 5.3822889e-9f, -1.5500992e-6f), 2.6041667e-4f), -2.0833333e-2f), 0.5f);
+    const float c = fmaf(x, fmaf(x, fmaf(x, -2.1701389e-5f, 2.6041667e-3f), -0.125f), 1.0f);
+    const float s = fmaf(x, fmaf(x, fmaf(x, -1.5500992e-6f, 2.6041667e-4f), -2.0833333e-2f), 0.5f);
     Q4 r; r.w = c; r.x = s * phi.x; r.y = s * phi.y; r.z = s * phi.z;
     return r;
 }
 __device__ __forceinline__ Q4 exp_half_exact(V3 phi) {
     const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
-    if (x <= 1.0f) return exp_half(phi);
+    if (x <= 0.5f) return exp_half(phi);
     const float n = sqrtf(x);
     float sn, cn;
     sincosf(0.5f * n, &sn, &cn);
@@ -126,14 +164,15 @@ __device__ __forceinline__ Q4 exp_half_exact(V3 phi) {
     Q4 r; r.w = cn; r.x = s * phi.x; r.y = s * phi.y; r.z = s * phi.z;
     return r;
 }
-// R(phi)^T tau for a rotation VECTOR phi (Rodrigues; both coefficients are series in x = |phi|^2,
-// degree 4: error < 2e-7 for |phi| <= 1.5 rad).  Used for the RK4 stage torques.
-__device__ __forceinline__ V3 rotvec_inv(V3 phi, V3 tau) {
-    const float x = fmaf(phi.x, phi.x, fmaf(phi.y, phi.y, phi.z * phi.z));
-    const float A = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 2.7557319e-6f, -1.9841270e-4f), 8.3333333e-3f), -0.16666667f), 1.0f);
-    const float Bc = fmaf(x, fmaf(x, fmaf(x, fmaf(x, 2.7557319e-7f, -2.4801587e-5f), 1.3888889e-3f), -4.1666667e-2f), 0.5f);
-    const V3 c1 = cross(phi, tau);
-    const V3 c2 = cross(phi, c1);
+// R(c w)^T tau for the rotation vector phi = c w (Rodrigues): tau - A(y) (w x tau) + B(y) w x (w x tau) with
+// y = |w|^2 and the step factor c folded into the host-made coefficients cA, cB (DevParams::rotA_*, rotB_*;
+// degree 3 in y, error < 3e-7 relative for c|w| <= 0.75 rad).  Used for the RK4 stage torques.
+__device__ __forceinline__ V3 stage_torque(const float (&cA)[4], const float (&cB)[4], V3 w, V3 tau) {
+    const float y = fmaf(w.x, w.x, fmaf(w.y, w.y, w.z * w.z));
+    const float A = fmaf(y, fmaf(y, fmaf(y, cA[3], cA[2]), cA[1]), cA[0]);
+    const float Bc = fmaf(y, fmaf(y, fmaf(y, cB[3], cB[2]), cB[1]), cB[0]);
+    const V3 c1 = cross(w, tau);
+    const V3 c2 = cross(w, c1);
     return v3(fmaf(Bc, c2.x, fmaf(-A, c1.x, tau.x)), fmaf(Bc, c2.y, fmaf(-A, c1.y, tau.y)), fmaf(Bc, c2.z, fmaf(-A, c1.z, tau.z)));
 }
 // sqrt(x) for x >= 0 to ~2 ulp: one MUFU.RSQ and one multiply
@@ -144,11 +183,13 @@ __device__ __forceinline__ float wrap_pi(float x) {
     return fmaf(-6.28318530717959f, k, x);
 }
 // ZYX Euler angles (roll, pitch, yaw) of q
+__device__ __forceinline__ float roll_of(Q4 q) { return atan2_fast(2.0f * fmaf(q.w, q.x, q.y * q.z), fmaf(-2.0f, fmaf(q.x, q.x, q.y * q.y), 1.0f)); }
+__device__ __forceinline__ float pitch_of(Q4 q) { return asin_fast(clampf(2.0f * fmaf(q.w, q.y, -q.z * q.x), -1.0f, 1.0f)); }
 __device__ __forceinline__ V3 euler_zyx(Q4 q) {
     V3 e;
-    e.x = atan2f(2.0f * (q.w * q.x + q.y * q.z), 1.0f - 2.0f * (q.x * q.x + q.y * q.y));
-    e.y = asinf(clampf(2.0f * (q.w * q.y - q.z * q.x), -1.0f, 1.0f));
-    e.z = atan2f(2.0f * (q.w * q.z + q.x * q.y), 1.0f - 2.0f * (q.y * q.y + q.z * q.z));
+    e.x = roll_of(q);
+    e.y = pitch_of(q);
+    e.z = atan2_fast(2.0f * fmaf(q.w, q.z, q.x * q.y), fmaf(-2.0f, fmaf(q.y, q.y, q.z * q.z), 1.0f));
     return e;
 }
 

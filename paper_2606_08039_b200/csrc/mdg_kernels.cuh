@@ -19,7 +19,7 @@ __device__ __forceinline__ void store_state(const DevBuffers& B, size_t d, const
 // S8 rotation: classical RK4 on (q, w_body) with the torque frozen in the world frame (MJC* modes) or
 // explicit Euler (DYN).  The stage orientation is q0 (x) dq, so the body-frame torque at a stage is
 // R(dq)^T tau_b and q0 itself is only needed for the final update.  EXACT selects the library
-// sin/cos for |omega| h > 2 rad; the hot path uses the branch-free series of exp_half.
+// sin/cos for |omega| h > 0.75 rad; the hot path uses the branch-free series (stage_torque, exp_half).
 template <bool EXACT, bool EULER>
 __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, V3 tau_b, V3 k1_tau) {
     auto ex = [](V3 phi) { return EXACT ? exp_half_exact(phi) : exp_half(phi); };
@@ -28,12 +28,15 @@ __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, 
         const V3 k1 = v3(fmaf(-P.gyro[0], w0.y * w0.z, k1_tau.x), fmaf(-P.gyro[1], w0.z * w0.x, k1_tau.y),
                          fmaf(-P.gyro[2], w0.x * w0.y, k1_tau.z));
         const V3 w2 = v3(fmaf(P.half_h, k1.x, w0.x), fmaf(P.half_h, k1.y, w0.y), fmaf(P.half_h, k1.z, w0.z));
-        auto stage = [&](V3 phi) { return EXACT ? rot_inv(exp_half_exact(phi), tau_b) : rotvec_inv(phi, tau_b); };
-        const V3 k2 = ang_acc(P, stage(v3(P.half_h * w0.x, P.half_h * w0.y, P.half_h * w0.z)), w2);
+        auto stage_half = [&](V3 ws) { return EXACT ? rot_inv(exp_half_exact(v3(P.half_h * ws.x, P.half_h * ws.y, P.half_h * ws.z)), tau_b)
+                                                    : stage_torque(P.rotA_half, P.rotB_half, ws, tau_b); };
+        auto stage_full = [&](V3 ws) { return EXACT ? rot_inv(exp_half_exact(v3(P.h * ws.x, P.h * ws.y, P.h * ws.z)), tau_b)
+                                                    : stage_torque(P.rotA_full, P.rotB_full, ws, tau_b); };
+        const V3 k2 = ang_acc(P, stage_half(w0), w2);
         const V3 w3 = v3(fmaf(P.half_h, k2.x, w0.x), fmaf(P.half_h, k2.y, w0.y), fmaf(P.half_h, k2.z, w0.z));
-        const V3 k3 = ang_acc(P, stage(v3(P.half_h * w2.x, P.half_h * w2.y, P.half_h * w2.z)), w3);
+        const V3 k3 = ang_acc(P, stage_half(w2), w3);
         const V3 w4 = v3(fmaf(P.h, k3.x, w0.x), fmaf(P.h, k3.y, w0.y), fmaf(P.h, k3.z, w0.z));
-        const V3 k4 = ang_acc(P, stage(v3(P.h * w3.x, P.h * w3.y, P.h * w3.z)), w4);
+        const V3 k4 = ang_acc(P, stage_full(w3), w4);
         const V3 phi = v3(P.h_sixth * (w0.x + 2.0f * (w2.x + w3.x) + w4.x), P.h_sixth * (w0.y + 2.0f * (w2.y + w3.y) + w4.y),
                           P.h_sixth * (w0.z + 2.0f * (w2.z + w3.z) + w4.z));
         q = qmul(q, ex(phi));
@@ -47,7 +50,7 @@ __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, 
     const float rn = rsqrt_fast(fmaf(q.w, q.w, fmaf(q.x, q.x, fmaf(q.y, q.y, q.z * q.z))));
     q.w *= rn; q.x *= rn; q.y *= rn; q.z *= rn;
 }
-// out-of-line copy for fast spins (|omega| h > 2 rad): rare, keeps the hot loop free of library calls
+// out-of-line copy for fast spins (|omega| h > 0.75 rad): rare, keeps the hot loop free of library calls
 struct RotState { Q4 q; V3 w; };
 template <bool EULER>
 __device__ __noinline__ RotState integrate_rot_exact(const DevParams& P, Q4 q, V3 w, V3 tau_b, V3 k1_tau) {
@@ -56,46 +59,130 @@ __device__ __noinline__ RotState integrate_rot_exact(const DevParams& P, Q4 q, V
     return r;
 }
 
-// One control step of every env.  Thread -> (env e, lane-in-group j).
+// Shared-memory landing zone of one warp for one work item (32 lanes = 32 / G envs): every lane owns one
+// 16-byte slot per plane, fills it with cp.async and is the only one to read it back, so no barrier of any
+// kind is needed and the warps of a block never wait for each other.
+struct WarpStage {
+    float4 plane[9][32];           // P0..P6, the actions, E0 (the env word, one copy per lane)
+    uint32_t gstep[32];
+};
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Start the asynchronous copies of this lane's slots of work item `wt` (global -> shared, no registers held).
+template <int G>
+__device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffers& B, const float4* actions, WarpStage& S,
+                                              unsigned wt, int lane, int jj, int act) {
+    const unsigned e_raw = wt * (32u / G) + (unsigned)lane / G;
+    const unsigned e = e_raw < (unsigned)P.N ? e_raw : (unsigned)P.N - 1;
+    const size_t drone = (size_t)e * P.M + jj;
+    cp_async16(&S.plane[0][lane], B.P0 + drone);
+    cp_async16(&S.plane[1][lane], B.P1 + drone);
+    cp_async16(&S.plane[2][lane], B.P2 + drone);
+    cp_async16(&S.plane[3][lane], B.P3 + drone);
+    if (act != 0) cp_async16(&S.plane[4][lane], B.P4 + drone);
+    if (act == 1) cp_async16(&S.plane[5][lane], B.P5 + drone);
+    cp_async16(&S.plane[6][lane], B.P6 + drone);
+    cp_async16(&S.plane[7][lane], actions + drone);
+    cp_async16(&S.plane[8][lane], B.E0 + e);
+    cp_async4(&S.gstep[lane], B.gstep + e);
+    cp_async_commit();
+}
+
+#ifdef MDG_TRACE   // development builds only (_work/): per-item clock64 stamps, never compiled into libmdg.so
+__device__ unsigned long long* g_trace = nullptr;
+__device__ __forceinline__ void trace_stamp(unsigned wt, int k, int lane) {
+    if (lane == 0 && g_trace) {
+        g_trace[(size_t)wt * 10 + k] = clock64();
+        if (k == 0 || k == 5) { unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt)); g_trace[(size_t)wt * 10 + (k == 0 ? 6 : 8)] = gt; }
+        if (k == 0) { unsigned sm; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); g_trace[(size_t)wt * 10 + 7] = sm | ((unsigned long long)(threadIdx.x >> 5) << 32); }
+    }
+}
+#define MDG_T(k) trace_stamp(wt, k, lane)
+#else
+#define MDG_T(k)
+#endif
+
+// One control step of every env.  Persistent warps: each loops over work items of
+// 32 / G envs; lane -> (env e, lane-in-group j).  While an item is integrated, the next item's state planes,
+// actions and per-env words are already on their way into shared memory (cp.async, two stages), so HBM
+// latency and bandwidth overlap the arithmetic instead of alternating with it.
 // MINB = resident blocks of 128 threads per SM the register allocation must allow.
 template <int G, int FEAT, int MINB>
 __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__ DevParams P, const DevBuffers B,
                                                          const float4* __restrict__ actions) {
     using F = Feat<FEAT>;
-    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
-    const unsigned e_raw = tid / G;
-    const int j = tid % G;
+    __shared__ __align__(16) WarpStage S[2][4];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const unsigned wpb = blockDim.x >> 5;
+    const unsigned tw = gridDim.x * wpb;                          // persistent warps of this launch
+    const unsigned n_items = ((unsigned)P.N + (32u / G) - 1) / (32u / G);
+    const int j = lane % G;
+    const bool full_group = F::has(P, F_FULL);
+    const int jj = (full_group || j < P.M) ? j : P.M - 1;
+    const bool pid = F::act(P) != 0;
+    // PDL: let the next kernel of the stream start its own preamble, then wait until the previous kernel has
+    // completed and its writes are visible (no memory access above this line)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // Work items are handed out by an atomic ticket (self-resetting: atomicInc wraps to 0 after the n_items + tw
+    // grabs of one launch), so SMs that run faster or host fewer long warps simply take more items.
+    const unsigned wrap = n_items + tw - 1u;
+    auto grab = [&]() { unsigned v = 0; if (lane == 0) v = atomicInc(B.ticket, wrap); return __shfl_sync(MDG_FULL, v, 0); };
+    unsigned wt = grab();
+    if (wt >= n_items) return;
+    prefetch_item<G>(P, B, actions, S[0][wib], wt, lane, jj, F::act(P));
+    int st = 0;
+#pragma unroll 1
+    for (;;) {
+    const unsigned wt_next = grab();
+    const unsigned e_raw = wt * (32u / G) + (unsigned)lane / G;
     const bool env_ok = e_raw < (unsigned)P.N;
     const unsigned e = env_ok ? e_raw : (unsigned)P.N - 1;      // idle lanes shadow the last env (no stores)
-    const bool active = env_ok && j < P.M;
-    const int jj = j < P.M ? j : P.M - 1;
+    const bool active = env_ok && (full_group || j < P.M);
     const size_t drone = (size_t)e * P.M + jj;
-    const bool pid = F::act(P) != 0;
 
+    MDG_T(0);
+    cp_async_wait_all();
+    const WarpStage& W = S[st][wib];
     DroneRegs d;
-    load_state(B, drone, d);
-    if (pid) {
-        const float4 i4 = B.P4[drone];
-        d.Ie = v3(i4.x, i4.y, i4.z);
-        if (F::act(P) == 1) d.sp = B.P5[drone];
+    {
+        const float4 a = W.plane[0][lane], b = W.plane[1][lane], c = W.plane[2][lane], f = W.plane[3][lane];
+        d.p = v3(a.x, a.y, a.z); d.q.w = a.w; d.q.x = b.x; d.q.y = b.y; d.q.z = b.z;
+        d.v = v3(b.w, c.x, c.y); d.w = v3(c.z, c.w, f.x); d.Ip = v3(f.y, f.z, f.w);
     }
-    const float4 act4 = actions[drone];
-    float4 env4 = B.E0[e];
-    const uint32_t t = B.gstep[e] + 1u;
+    if (pid) {
+        const float4 i4 = W.plane[4][lane];
+        d.Ie = v3(i4.x, i4.y, i4.z);
+        if (F::act(P) == 1) d.sp = W.plane[5][lane];
+    }
+    const float4 tg = W.plane[6][lane];
+    const float4 act4 = W.plane[7][lane];
+    float4 env4 = W.plane[8][lane];
+    const uint32_t t = W.gstep[lane] + 1u;
+    if (wt_next < n_items) prefetch_item<G>(P, B, actions, S[st ^ 1][wib], wt_next, lane, jj, F::act(P));
+    MDG_T(1);
 
-    // S7 wind gust: one AR(1) update per env and control step, force held over the substeps
+    // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
+    // Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact in
+    // fp32; cos/sin(2 pi u_b) = -cos/sin(2 pi (u_b - 1/2)) keeps the MUFU argument in [-pi, pi).
     V3 Fwind = v3(0, 0, 0);
     if (F::has(P, F_WIND)) {
         const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
-        const float r1 = sqrtf(-2.0f * logf(1.0f - u01(r.x))), r2 = sqrtf(-2.0f * logf(1.0f - u01(r.z)));
-        float s1, c1, s2, c2;
-        sincospif(2.0f * u01(r.y), &s1, &c1);
-        sincospif(2.0f * u01(r.w), &s2, &c2);
-        env4.x = fmaf(P.wind_alpha, env4.x, P.wind_gain * (r1 * c1));
-        env4.y = fmaf(P.wind_alpha, env4.y, P.wind_gain * (r1 * s1));
-        env4.z = fmaf(P.wind_alpha, env4.z, P.wind_gain * (r2 * c2));
+        const float r1 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.x))), r2 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.z)));
+        const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
+        env4.x = fmaf(P.wind_alpha, env4.x, P.wind_gain * (r1 * cos_fast(a1)));
+        env4.y = fmaf(P.wind_alpha, env4.y, P.wind_gain * (r1 * sin_fast(a1)));
+        env4.z = fmaf(P.wind_alpha, env4.z, P.wind_gain * (r2 * cos_fast(a2)));
         const V3 rel = v3(env4.x - d.v.x, env4.y - d.v.y, env4.z - d.v.z);
-        const float kn = P.k_wind * sqrtf(fmaf(rel.x, rel.x, fmaf(rel.y, rel.y, rel.z * rel.z)));
+        const float kn = P.k_wind * fast_sqrt(fmaf(rel.x, rel.x, fmaf(rel.y, rel.y, rel.z * rel.z)));
         Fwind = v3(kn * rel.x, kn * rel.y, kn * rel.z);
     }
 
@@ -108,11 +195,10 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const float Om = P.rpm2rad * ((n[0] + n[1]) + (n[2] + n[3]));
     const V3 k1_tau = v3(P.invJ[0] * tau_b.x, P.invJ[1] * tau_b.y, P.invJ[2] * tau_b.z);
     const float cxy = -P.c_xy * Om, cz = -P.c_z * Om, gndT = P.gnd_coef * T;
-    const float w2_slow = 1.0f / (P.h * P.h);                     // |omega| h > 1 rad
     const float dcz = cz - cxy;
-    const bool full_group = P.M == G;
 
     bool hit = false;
+    MDG_T(2);
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
         // S4-S7 world-frame force from the start-of-substep state
@@ -124,13 +210,17 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             const float s = fmaf(dcz, fmaf(b.x, d.v.x, fmaf(b.y, d.v.y, b.z * d.v.z)), T);
             Fw = v3(fmaf(s, b.x, cxy * d.v.x), fmaf(s, b.y, cxy * d.v.y), fmaf(s, b.z, cxy * d.v.z));
         } else Fw = v3(T * b.x, T * b.y, T * b.z);
+        if (F::has(P, F_WIND)) { Fw.x += Fwind.x; Fw.y += Fwind.y; Fw.z += Fwind.z; }
         if (F::has(P, F_GND)) {                                   // Eq.4, gated on body z pointing up
-            const float r22 = b.z;
             const float hgt = fmaxf(d.p.z, P.h_clip);
             const float gain = gndT * rcp_fast(hgt * hgt);
-            Fw.z += r22 > 0.0f ? gain : 0.0f;
+            Fw.z += b.z > 0.0f ? gain : 0.0f;
         }
         if (G > 1 && F::has(P, F_DW)) {                           // Eq.6 over every drone above this one
+            // With b' = sqrt(2 ln 2) beta: exp(-dxy^2 / 2 beta^2) = 2^(-dxy^2 / b'^2) and alpha = C1 (r_p/4)^2 / dz_e^2.
+            // One reciprocal r = 1 / (dz_e^2 b'^2) serves both: alpha ~ b'^2 r, exponent = -dxy^2 (dz_e^2 r).
+            // The ramp saturate(dz / dz_clip) is 0 for dz <= 0, which also gates "k above this drone";
+            // b'^2 is floored (beta^2 >= 1e-12), which reproduces the beta -> 0 rule of DESIGN.md Q9.
             float dw = 0.0f;
 #pragma unroll
             for (int kk = 1; kk < G; ++kk) {                      // partner lane = lane ^ kk: every other drone once
@@ -138,24 +228,22 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                             oz = __shfl_xor_sync(MDG_FULL, d.p.z, kk);
                 const float dz = oz - d.p.z, dx = ox - d.p.x, dy = oy - d.p.y;
                 const float dxy2 = fmaf(dx, dx, dy * dy);
-                const float dze = fmaxf(dz, P.dz_clip);
-                const float ramp = P.dz_clip > 0.0f ? fminf(dz * P.inv_dz_clip, 1.0f) : 1.0f;
-                const float beta = fmaf(P.dw_C2, dze, P.dw_C3);
-                const float b2 = beta * beta, z2 = dze * dze;
-                const float rinv = rcp_fast(z2 * b2);                      // one reciprocal serves alpha and the exponent
-                const float alpha = P.dw_coef * (b2 * rinv);
-                const float ex = b2 < 1e-12f ? (dxy2 == 0.0f ? 1.0f : 0.0f) : ex2_fast(-0.72134752f * dxy2 * (z2 * rinv));   // exp(-x/2) = 2^(-x log2(e)/2)
-                const float al = b2 < 1e-12f ? P.dw_coef * rcp_fast(z2) : alpha;
-                const bool on = (full_group || (j ^ kk) < P.M) && dz > 0.0f && dxy2 < 100.0f;
-                dw += on ? ramp * al * ex : 0.0f;
+                const float dze = fmaxf(dz, P.dz_floor);
+                const float ramp = __saturatef(dz * P.inv_dz_clip);
+                const float bs = fmaf(P.dw_C2s, dze, P.dw_C3s);
+                const float b2 = fmaxf(bs * bs, P.dw_b2_min), z2 = dze * dze;
+                const float rinv = rcp_fast(z2 * b2);
+                const float ex = ex2_fast(-dxy2 * (z2 * rinv));
+                const float al = ramp * (b2 * rinv);
+                const bool on = (full_group || (j ^ kk) < P.M) && dxy2 < 100.0f;
+                dw = fmaf(al, on ? ex : 0.0f, dw);
             }
-            Fw.z -= dw;
+            Fw.z = fmaf(-P.dw_coef, dw, Fw.z);
         }
-        if (F::has(P, F_WIND)) { Fw.x += Fwind.x; Fw.y += Fwind.y; Fw.z += Fwind.z; }
         const V3 acc = v3(Fw.x * P.inv_m, Fw.y * P.inv_m, fmaf(Fw.z, P.inv_m, -P.g));
 
         // S8 integrate with the wrench frozen in the world frame
-        const bool fast_spin = fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)) > w2_slow;
+        const bool fast_spin = fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)) > P.w2_exact;
         if (!F::has(P, F_EULER)) {
             d.p.x = fmaf(P.half_h2, acc.x, fmaf(P.h, d.v.x, d.p.x));
             d.p.y = fmaf(P.half_h2, acc.y, fmaf(P.h, d.v.y, d.p.y));
@@ -172,10 +260,9 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         if (d.p.z < 0.0f) { hit = true; d.p.z = 0.0f; d.v.z = fmaxf(d.v.z, 0.0f); }   // floor
     }
 
+    MDG_T(3);
     // S9-S11 epilogue on the end-of-step state
-    const int lane = threadIdx.x & 31;
     const int gbase = lane & ~(G - 1);
-    const float4 tg = B.P6[drone];
     V3 eta = euler_zyx(d.q);
     const int term = F::term(P);
     const float aphi = fabsf(eta.x), ath = fabsf(eta.y);
@@ -200,51 +287,75 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     } else {                                                       // formation: pair term below
         r = -fast_sqrt(e2);
     }
-    if (G > 1 && rew == 3) {
+    // one pass over the env's drones serves the formation pair term and the adjacency row
+    float adj[G];
+#pragma unroll
+    for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
+    const bool pairs = G > 1 && rew == 3;
+    if (pairs || F::has(P, F_ADJ)) {
         float pen = 0.0f;                                          // the self term is |0 - 0| = 0
 #pragma unroll
         for (int kk = 0; kk < G; ++kk) {
             const float ox = __shfl_sync(MDG_FULL, d.p.x, gbase + kk), oy = __shfl_sync(MDG_FULL, d.p.y, gbase + kk),
                         oz = __shfl_sync(MDG_FULL, d.p.z, gbase + kk);
-            const float ux = __shfl_sync(MDG_FULL, tg.x, gbase + kk), uy = __shfl_sync(MDG_FULL, tg.y, gbase + kk),
-                        uz = __shfl_sync(MDG_FULL, tg.z, gbase + kk);
             const float ax = d.p.x - ox, ay = d.p.y - oy, az = d.p.z - oz;
-            const float bx = tg.x - ux, by = tg.y - uy, bz = tg.z - uz;
-            const float dact = fast_sqrt(fmaf(ax, ax, fmaf(ay, ay, az * az))), ddes = fast_sqrt(fmaf(bx, bx, fmaf(by, by, bz * bz)));
-            pen += (full_group || kk < P.M) ? fabsf(dact - ddes) : 0.0f;
+            const float d2 = fmaf(ax, ax, fmaf(ay, ay, az * az));
+            adj[kk] = (kk == j || d2 < P.adj_radius2) ? 1.0f : 0.0f;
+            if (pairs) {
+                float ddes;
+                if (F::has(P, F_TGT_CIRCLE)) ddes = P.chord[abs(j - kk)];
+                else {
+                    const float ux = __shfl_sync(MDG_FULL, tg.x, gbase + kk), uy = __shfl_sync(MDG_FULL, tg.y, gbase + kk),
+                                uz = __shfl_sync(MDG_FULL, tg.z, gbase + kk);
+                    const float bx = tg.x - ux, by = tg.y - uy, bz = tg.z - uz;
+                    ddes = fast_sqrt(fmaf(bx, bx, fmaf(by, by, bz * bz)));
+                }
+                pen += (full_group || kk < P.M) ? fabsf(fast_sqrt(d2) - ddes) : 0.0f;
+            }
         }
-        r = fmaf(-0.25f, pen, r);                                  // each unordered pair is seen from both ends
+        if (pairs) r = fmaf(-0.25f, pen, r);                       // each unordered pair is seen from both ends
     }
-    const float rsum = group_sum<G>(j < P.M ? r : 0.0f);
-    const int gflags = group_or<G>(j < P.M ? flags : 0);
+    const bool mine = full_group || j < P.M;
+    const float rsum = group_sum<G>(mine ? r : 0.0f);
+    const int gflags = group_or<G>(mine ? flags : 0);
     const uint32_t ep = __float_as_uint(env4.w) + 1u;
     const bool truncated = P.ep_steps > 0 && (int)ep >= P.ep_steps;
     const int done = (gflags & 1) | (truncated ? 2 : 0);
     uint32_t ep_out = ep;
-    float4 tg_out = tg;
     const bool do_reset = done != 0 && P.auto_reset != 0;
-    if (do_reset) {                                                // S12 same-call auto-reset
-        reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
-        env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
-        eta = v3(0, 0, 0);
-    }
-    float adj[G];
+    if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp
+        if (do_reset) {
+            float4 tg_out;
+            reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
+            env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
+            eta = v3(0, 0, 0);
+            if (active) B.P6[drone] = tg_out;
+        }
+        if (F::has(P, F_ADJ)) {                                    // the new episode's first observation
+            float adj_new[G];
+            adjacency<G>(P, d.p, lane, j, adj_new);
 #pragma unroll
-    for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
-    if (F::has(P, F_ADJ)) adjacency<G>(P, d.p, lane, j, adj);
-    if (!active) return;
-    store_state(B, drone, d);
-    if (pid) {
-        B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
-        if (F::act(P) == 1) B.P5[drone] = d.sp;
+            for (int kk = 0; kk < G; ++kk) adj[kk] = do_reset ? adj_new[kk] : adj[kk];
+        }
     }
-    if (do_reset) B.P6[drone] = tg_out;
-    write_obs<G>(P, B.obs, drone, d, eta, adj, F::has(P, F_ADJ));
-    if (j == 0) {
-        env4.w = __uint_as_float(ep_out);
-        B.E0[e] = env4; B.gstep[e] = t;
-        B.reward[e] = rsum; B.done[e] = (uint8_t)done;
+    MDG_T(4);
+    if (active) {
+        store_state(B, drone, d);
+        if (pid) {
+            B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
+            if (F::act(P) == 1) B.P5[drone] = d.sp;
+        }
+        write_obs<G>(P, B.obs, drone, d, eta, adj, F::has(P, F_ADJ));
+        if (j == 0) {
+            env4.w = __uint_as_float(ep_out);
+            B.E0[e] = env4; B.gstep[e] = t;
+            B.reward[e] = rsum; B.done[e] = (uint8_t)done;
+        }
     }
+    MDG_T(5);
+    if (wt_next >= n_items) break;
+    wt = wt_next; st ^= 1;
+    }   // work-item loop
 }
 
 // mdg_reset: initial state of every env at step index 0, first observation, zero reward / done

@@ -73,9 +73,9 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     }
     // roll, pitch and the heading direction (cos psi, sin psi) = normalised (1 - 2(y^2+z^2), 2(wz+xy))
     V3 eta;
-    eta.x = atan2f(2.0f * (d.q.w * d.q.x + d.q.y * d.q.z), 1.0f - 2.0f * (d.q.x * d.q.x + d.q.y * d.q.y));
-    eta.y = asinf(clampf(2.0f * (d.q.w * d.q.y - d.q.z * d.q.x), -1.0f, 1.0f));
-    const float hc = 1.0f - 2.0f * (d.q.y * d.q.y + d.q.z * d.q.z), hs = 2.0f * (d.q.w * d.q.z + d.q.x * d.q.y);
+    eta.x = roll_of(d.q);
+    eta.y = pitch_of(d.q);
+    const float hc = fmaf(-2.0f, fmaf(d.q.y, d.q.y, d.q.z * d.q.z), 1.0f), hs = 2.0f * fmaf(d.q.w, d.q.z, d.q.x * d.q.y);
     const float hn2 = fmaf(hc, hc, hs * hs);
     const float hr = hn2 > 1e-30f ? rsqrt_fast(hn2) : 0.0f;
     const float cpsi = hn2 > 1e-30f ? hc * hr : 1.0f, spsi = hs * hr;
@@ -92,7 +92,7 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
             d.sp.w = wrap_pi(d.sp.w + dpsi);
         } else d.sp = a;
         e_p = v3(d.sp.x - d.p.x, d.sp.y - d.p.y, d.sp.z - d.p.z);
-        v_ref = v3(0, 0, 0); e_psi = wrap_pi(d.sp.w - atan2f(hs, hc));
+        v_ref = v3(0, 0, 0); e_psi = wrap_pi(d.sp.w - atan2_fast(hs, hc));
     } else {                              // VEL [vx, vy, vz, wz] in the heading frame
         e_p = v3(0, 0, 0);
         v_ref = v3(cpsi * a.x - spsi * a.y, spsi * a.x + cpsi * a.y, a.z);
@@ -157,19 +157,19 @@ __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict_
     }
 }
 
-// adjacency row of this lane's drone: A_k = 1 if k == j or |p - p_k| < radius (Q23)
+// adjacency row of this lane's drone: A_k = 1 if k == j or |p - p_k| < radius (Q23); whole-warp call
 template <int G>
 __device__ __forceinline__ void adjacency(const DevParams& P, V3 p, int lane, int j, float (&adj)[G]) {
+    const unsigned mask = MDG_FULL;
     const int gbase = lane & ~(G - 1);
 #pragma unroll
     for (int k = 0; k < G; ++k) {
-        const float ox = __shfl_sync(MDG_FULL, p.x, gbase + k), oy = __shfl_sync(MDG_FULL, p.y, gbase + k),
-                    oz = __shfl_sync(MDG_FULL, p.z, gbase + k);
+        const float ox = __shfl_sync(mask, p.x, gbase + k), oy = __shfl_sync(mask, p.y, gbase + k),
+                    oz = __shfl_sync(mask, p.z, gbase + k);
         const float dx = p.x - ox, dy = p.y - oy, dz = p.z - oz;
         adj[k] = (k == j || fmaf(dx, dx, fmaf(dy, dy, dz * dz)) < P.adj_radius2) ? 1.0f : 0.0f;
     }
 }
-
 template <int G> __device__ __forceinline__ float group_sum(float x) {
 #pragma unroll
     for (int o = G / 2; o > 0; o >>= 1) x += __shfl_xor_sync(MDG_FULL, x, o);

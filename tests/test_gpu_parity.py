@@ -36,3 +36,13 @@ def test_config_parity_with_frequent_episodes(c):
     res = run_parity(wl, steps=40, extra=dict(episode_len_s=7 / 48, z_max=1.3), max_ill_frac=0.05 if c == 4 else 0.0)
     print(c, res)
     assert res["n_done"] > wl.n_envs
+
+
+@pytest.mark.parametrize("c,extra", [(3, dict(term_dist=1.06)), (4, dict(z_max=1.0)), (5, dict(term_dist=0.35))])
+def test_config_parity_with_divergent_resets(c, extra):
+    """Envs that terminate one by one at different steps: neighbouring envs of one warp take the auto-reset path at
+    different times (the truncation test above resets whole warps at once)."""
+    wl = W.config(c).scaled(min(W.config(c).n_envs, 2051))
+    res = run_parity(wl, steps=48, extra=extra, max_ill_frac=0.05 if c == 4 else 0.0)
+    print(c, res)
+    assert res["n_done"] > wl.n_envs // 8
