@@ -42,6 +42,10 @@ struct mdg_env {
     std::string kernel_name;
     int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
     int pdl = 1;
+    uint32_t seq = 0;                    // step launches so far (kernel parameter; see "chain" in mdg_kernels.cuh)
+    bool saturating = false;             // the step grid occupies every resident block slot of the device
+    bool chainable = false;              // the last operation on this handle was a stream-launched step
+    cudaStream_t last_stream = nullptr;
     int n_sms = 0, step_grid = 0;        // persistent step kernel: one block per resident slot, looping over tiles
     int64_t launches = 0;
     std::map<std::tuple<const void*, int, int64_t>, cudaGraphExec_t> graphs;
@@ -186,6 +190,10 @@ static int configure_launch(mdg_env* h) {
     const long long items = ((long long)h->N + epw - 1) / epw, blocks = (items + wpb - 1) / wpb;
     const long long slots = (long long)h->n_sms * resident;
     h->step_grid = (int)(blocks < slots ? blocks : slots);
+    // Item-level chaining of consecutive steps needs "at most two step kernels in flight" (two ticket dispensers):
+    // guaranteed when a grid fills every resident slot, because the successor's blocks can then only start in slots
+    // this grid has vacated, and the successor's successor only once all of those have started.
+    h->saturating = blocks >= slots;
     return MDG_OK;
 }
 static inline unsigned grid_for(const mdg_env* h, int block) {
@@ -196,10 +204,11 @@ static void drop_graphs(mdg_env* h) {
     for (auto& kv : h->graphs) cudaGraphExecDestroy(kv.second);
     h->graphs.clear();
 }
-static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s) {
-    // Programmatic dependent launch: the blocks of this step may become resident while the previous kernel of the
-    // stream drains (it overlaps launch latency, parameter and instruction fetch); the kernel itself waits
-    // (griddepcontrol.wait) for that kernel to complete and flush before it touches memory.
+static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s, bool may_chain) {
+    h->seq += 1;
+    h->P.seq = h->seq;
+    h->P.chain = (may_chain && h->pdl && h->saturating && h->chainable && h->last_stream == s) ? 1u : 0u;
+    h->chainable = may_chain; h->last_stream = s;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)h->step_grid); cfg.blockDim = dim3((unsigned)h->block);
     cfg.dynamicSmemBytes = (size_t)h->smem; cfg.stream = s;
@@ -298,7 +307,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const size_t plane = al(D * sizeof(float4)), eplane = al((size_t)n_envs * sizeof(float4)), gs = al((size_t)n_envs * 4),
                  ob = al(D * h->P.opd * sizeof(float)), rw = al((size_t)n_envs * 4), dn = al((size_t)n_envs);
-    h->arena_bytes = 7 * plane + eplane + gs + ob + rw + dn + 256;
+    const size_t n_items_max = (size_t)n_envs;                     // >= work items for any G
+    h->arena_bytes = 7 * plane + eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
     cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
     if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
     ce = cudaMemset(h->arena, 0, h->arena_bytes);
@@ -311,7 +321,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     h->B.obs = (float*)c; c += ob;
     h->B.reward = (float*)c; c += rw;
     h->B.done = (uint8_t*)c; c += dn;
-    h->B.ticket = (unsigned*)c;
+    h->B.ticket = (unsigned*)c; c += 256;
+    h->B.item_seq = (unsigned*)c;
     int rc = configure_launch(h);
     if (rc != MDG_OK) { cudaFree(h->arena); delete h; return rc; }
     *out = h;
@@ -334,7 +345,8 @@ int mdg_reset(mdg_env* h, uint64_t seed) {
     if (!h) return fail(MDG_EINVAL, "mdg_reset: NULL handle");
     h->P.seed_lo = (uint32_t)seed; h->P.seed_hi = (uint32_t)(seed >> 32);
     drop_graphs(h);                          // captured launches carry the old seed
-    CU(cudaMemsetAsync(h->B.ticket, 0, sizeof(unsigned), h->stream));
+    CU(cudaMemsetAsync(h->B.ticket, 0, 2 * sizeof(unsigned), h->stream));
+    h->chainable = false;
     h->reset<<<grid_for(h, 128), 128, 0, h->stream>>>(h->P, h->B);
     CU(cudaGetLastError());
     h->launches += 1;
@@ -344,8 +356,10 @@ int mdg_reset(mdg_env* h, uint64_t seed) {
 int mdg_step(mdg_env* h, const float* actions_dev) {
     if (!h || !actions_dev) return fail(MDG_EINVAL, "mdg_step: NULL argument");
     if ((uintptr_t)actions_dev & 15) return fail(MDG_EINVAL, "mdg_step: actions_dev must be 16-byte aligned");
-    const int rc = launch_step(h, actions_dev, h->stream);
-    if (rc == MDG_OK) h->launches += 1;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;      // a caller-side capture replays baked parameters
+    CU(cudaStreamIsCapturing(h->stream, &cap));
+    const int rc = launch_step(h, actions_dev, h->stream, cap == cudaStreamCaptureStatusNone);
+    if (rc == MDG_OK) h->launches += 1; else h->chainable = false;
     return rc;
 }
 
@@ -358,7 +372,7 @@ int mdg_step_many(mdg_env* h, const float* actions_dev, int n_steps, int64_t str
         if (!h->capture_stream) CU(cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking));
         CU(cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal));
         int rc = MDG_OK;
-        for (int k = 0; k < n_steps && rc == MDG_OK; ++k) rc = launch_step(h, actions_dev + (int64_t)k * stride_floats, h->capture_stream);
+        for (int k = 0; k < n_steps && rc == MDG_OK; ++k) rc = launch_step(h, actions_dev + (int64_t)k * stride_floats, h->capture_stream, false);
         cudaGraph_t g = nullptr;
         cudaError_t ce = cudaStreamEndCapture(h->capture_stream, &g);
         if (rc != MDG_OK) { if (g) cudaGraphDestroy(g); return rc; }
@@ -371,6 +385,7 @@ int mdg_step_many(mdg_env* h, const float* actions_dev, int n_steps, int64_t str
         it = h->graphs.emplace(key, ge).first;
     }
     CU(cudaGraphLaunch(it->second, h->stream));
+    h->chainable = false;                    // replayed kernels carry baked sequence numbers
     h->launches += n_steps;
     return MDG_OK;
 }
@@ -421,6 +436,7 @@ int mdg_set_launch(mdg_env* h, int block_threads, int max_blocks_per_sm) {
         pick_kernels(h);
     }
     drop_graphs(h);
+    h->chainable = false;
     return configure_launch(h);
 }
 
@@ -480,6 +496,7 @@ extern "C" int mdg_set_state(mdg_env* h, const float* state, const float* ctrl, 
         }
         CU(cudaMemcpy(h->B.E0, ev.data(), (size_t)h->N * sizeof(float4), cudaMemcpyHostToDevice));
     }
+    h->chainable = false;
     h->refresh<<<grid_for(h, 128), 128, 0, h->stream>>>(h->P, h->B);
     CU(cudaGetLastError());
     h->launches += 1;
@@ -495,7 +512,7 @@ extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_h
     float*& stage = g_stage[h];
     if (!stage) CU(cudaMalloc(&stage, D * 4 * sizeof(float)));
     CU(cudaMemcpyAsync(stage, actions_host, D * 4 * sizeof(float), cudaMemcpyHostToDevice, h->stream));
-    const int rc = launch_step(h, stage, h->stream);
+    const int rc = launch_step(h, stage, h->stream, true);
     if (rc != MDG_OK) return rc;
     h->launches += 1;
     if (obs_host) CU(cudaMemcpyAsync(obs_host, h->B.obs, D * h->P.opd * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
@@ -510,9 +527,10 @@ extern "C" void mdg_release_staging(mdg_env* h) {   // called by mdg_destroy
 }
 
 #ifdef MDG_TRACE
-extern "C" int mdg_debug_set_trace(void* dev_ptr) {
+extern "C" int mdg_debug_set_trace(void* dev_ptr, unsigned n_items) {
     unsigned long long* p = (unsigned long long*)dev_ptr;
     CU(cudaMemcpyToSymbol(mdg::g_trace, &p, sizeof(p)));
+    CU(cudaMemcpyToSymbol(mdg::g_trace_items, &n_items, sizeof(n_items)));
     return MDG_OK;
 }
 #endif

@@ -25,6 +25,7 @@ struct DevParams {
     int N, M, K, ep_steps, auto_reset, feat;
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
     uint32_t seed_lo, seed_hi, env_base;
+    uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining (mdg_kernels.cuh)
     // integrator
     float h, half_h, h_sixth, half_h2, w2_exact;          // w2_exact: |omega|^2 above which the exact path runs
     // Rodrigues coefficients of R(c w)^T as polynomials in y = |w|^2, c = h/2 (stages 2, 3) and h (stage 4):
@@ -60,7 +61,8 @@ struct DevBuffers {
     float4* P6;   // target x y z psi
     float4* E0;   // wind x y z, bits(ep_step)
     uint32_t* gstep;
-    unsigned* ticket;   // work-item dispenser of the step kernel (0 between launches)
+    unsigned* ticket;   // two work-item dispensers of the step kernel (0 between launches), used alternately
+    unsigned* item_seq; // per work item: sequence number of the last step that finished it
     float* obs;
     float* reward;
     uint8_t* done;

@@ -98,14 +98,16 @@ __device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffe
 
 #ifdef MDG_TRACE   // development builds only (_work/): per-item clock64 stamps, never compiled into libmdg.so
 __device__ unsigned long long* g_trace = nullptr;
-__device__ __forceinline__ void trace_stamp(unsigned wt, int k, int lane) {
+__device__ unsigned g_trace_items = 0;
+__device__ __forceinline__ void trace_stamp(unsigned wt, int k, int lane, unsigned seq) {
     if (lane == 0 && g_trace) {
-        g_trace[(size_t)wt * 10 + k] = clock64();
-        if (k == 0 || k == 5) { unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt)); g_trace[(size_t)wt * 10 + (k == 0 ? 6 : 8)] = gt; }
-        if (k == 0) { unsigned sm; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); g_trace[(size_t)wt * 10 + 7] = sm | ((unsigned long long)(threadIdx.x >> 5) << 32); }
+        unsigned long long* r = g_trace + ((size_t)(seq & 3u) * g_trace_items + wt) * 10;
+        r[k] = clock64();
+        if (k == 0 || k == 5) { unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt)); r[k == 0 ? 6 : 8] = gt; }
+        if (k == 0) { unsigned sm; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); r[7] = sm | ((unsigned long long)(threadIdx.x >> 5) << 32); r[9] = seq; }
     }
 }
-#define MDG_T(k) trace_stamp(wt, k, lane)
+#define MDG_T(k) trace_stamp(wt, k, lane, P.seq)
 #else
 #define MDG_T(k)
 #endif
@@ -128,21 +130,64 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const bool full_group = F::has(P, F_FULL);
     const int jj = (full_group || j < P.M) ? j : P.M - 1;
     const bool pid = F::act(P) != 0;
-    // PDL: let the next kernel of the stream start its own preamble, then wait until the previous kernel has
-    // completed and its writes are visible (no memory access above this line)
+    // Programmatic dependent launch.  P.chain == 0: wait here until the previous kernel of the stream has completed
+    // and its writes are visible (nothing above touches memory).  P.chain == 1 (the previous operation on this
+    // handle was step number P.seq - 1, launched on the same stream): no grid-wide wait at all; the dependency is
+    // per work item instead - item i may start as soon as the previous step has published item i (item_seq[i] ==
+    // P.seq - 1, release/acquire), so the drain of one step overlaps the ramp-up of the next.  Deadlock-free:
+    // this grid only starts once every block of the previous grid is resident (or done), and nothing here is waited on
+    // by that grid.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const bool chain = P.chain != 0;
+    if (!chain) asm volatile("griddepcontrol.wait;" ::: "memory");
     // Work items are handed out by an atomic ticket (self-resetting: atomicInc wraps to 0 after the n_items + tw
-    // grabs of one launch), so SMs that run faster or host fewer long warps simply take more items.
+    // grabs of one launch; two dispensers alternate so that chained launches never share one), so SMs that run
+    // faster or host fewer long warps simply take more items.
     const unsigned wrap = n_items + tw - 1u;
-    auto grab = [&]() { unsigned v = 0; if (lane == 0) v = atomicInc(B.ticket, wrap); return __shfl_sync(MDG_FULL, v, 0); };
-    unsigned wt = grab();
+    unsigned* const dispenser = B.ticket + (P.seq & 1u);
+    // Everything with a long latency on the per-item path is issued one item early and consumed late: the ticket
+    // of item n+2 is drawn (lane 0, atomic) when item n starts and read after its substeps; the "previous step
+    // has published this item" flag of item n+2 is then probed (ld.acquire) and only re-polled at the prefetch
+    // of item n+2 if that probe came too early; an item's own flag is published (fence + st.release) just before
+    // the NEXT item's stores, when its stores have long been acknowledged.
+    const unsigned want = P.seq - 1u;
+    auto draw = [&](bool go) { unsigned v = 0xFFFFFFFFu; if (lane == 0 && go) v = atomicInc(dispenser, wrap); return v; };   // lane 0 holds it
+    auto probe = [&](unsigned item_l0) {                        // lane 0: one acquire load of the item's flag
+        unsigned got = want;
+        if (chain && lane == 0 && item_l0 < n_items) asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(got) : "l"(B.item_seq + item_l0) : "memory");
+        return got;
+    };
+    auto await_item = [&](unsigned item, unsigned probed_l0) {  // the previous step has finished this item
+        if (chain) {
+            if (lane == 0 && probed_l0 != want) {
+                unsigned got, spins = 0;
+                for (;;) {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(got) : "l"(B.item_seq + item) : "memory");
+                    if (got == want) break;
+                    __nanosleep(64);
+                    if (++spins > (1u << 24)) __trap();          // fail loudly instead of hanging
+                }
+            }
+            __syncwarp();
+        }
+    };
+    // publication of an item = fence over every lane's stores (issued before the substeps of the next item, whose
+    // arithmetic hides the fence's round trip to L2) + a relaxed store of the sequence number (after them)
+    auto publish_flag = [&](unsigned item) {
+        __syncwarp();
+        if (lane == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(B.item_seq + item), "r"(P.seq) : "memory");
+    };
+    unsigned wt = __shfl_sync(MDG_FULL, draw(true), 0);
     if (wt >= n_items) return;
+    unsigned wt_next = __shfl_sync(MDG_FULL, draw(true), 0);      // a warp stops drawing after its first miss
+    unsigned probed_next = probe(wt_next);
+    await_item(wt, probe(wt));
     prefetch_item<G>(P, B, actions, S[0][wib], wt, lane, jj, F::act(P));
+    unsigned pending = 0xFFFFFFFFu;                               // item whose flag is still to be published
     int st = 0;
 #pragma unroll 1
     for (;;) {
-    const unsigned wt_next = grab();
+    const unsigned drawn_l0 = draw(wt_next < n_items);            // ticket of the item after next, in flight
     const unsigned e_raw = wt * (32u / G) + (unsigned)lane / G;
     const bool env_ok = e_raw < (unsigned)P.N;
     const unsigned e = env_ok ? e_raw : (unsigned)P.N - 1;      // idle lanes shadow the last env (no stores)
@@ -167,7 +212,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const float4 act4 = W.plane[7][lane];
     float4 env4 = W.plane[8][lane];
     const uint32_t t = W.gstep[lane] + 1u;
-    if (wt_next < n_items) prefetch_item<G>(P, B, actions, S[st ^ 1][wib], wt_next, lane, jj, F::act(P));
+    if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch_item<G>(P, B, actions, S[st ^ 1][wib], wt_next, lane, jj, F::act(P)); }
     MDG_T(1);
 
     // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
@@ -198,6 +243,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const float dcz = cz - cxy;
 
     bool hit = false;
+    if (pending != 0xFFFFFFFFu) __threadfence();
     MDG_T(2);
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
@@ -261,6 +307,9 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     }
 
     MDG_T(3);
+    if (pending != 0xFFFFFFFFu) publish_flag(pending);
+    const unsigned wt_after = __shfl_sync(MDG_FULL, drawn_l0, 0);
+    const unsigned probed_after = probe(wt_after);
     // S9-S11 epilogue on the end-of-step state
     const int gbase = lane & ~(G - 1);
     V3 eta = euler_zyx(d.q);
@@ -353,9 +402,12 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         }
     }
     MDG_T(5);
+    pending = wt;
     if (wt_next >= n_items) break;
-    wt = wt_next; st ^= 1;
+    wt = wt_next; wt_next = wt_after; probed_next = probed_after; st ^= 1;
     }   // work-item loop
+    __threadfence();
+    publish_flag(pending);
 }
 
 // mdg_reset: initial state of every env at step index 0, first observation, zero reward / done
