@@ -71,6 +71,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
     if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
+    if (p.J[0] == p.J[1]) f |= F_AXISYM;
     return f;
 }
 
@@ -94,6 +95,11 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
         float* A = s ? D.rotA_full : D.rotA_half; float* Bc = s ? D.rotB_full : D.rotB_half;
         A[0] = (float)c; A[1] = (float)(-c * c2 / 6.0); A[2] = (float)(c * c2 * c2 / 120.0); A[3] = (float)(-c * c2 * c2 * c2 / 5040.0);
         Bc[0] = (float)(c2 / 2.0); Bc[1] = (float)(-c2 * c2 / 24.0); Bc[2] = (float)(c2 * c2 * c2 / 720.0); Bc[3] = (float)(-c2 * c2 * c2 * c2 / 40320.0);
+    }
+    {                                                             // Eq.7 increment for phi = (h/6) s in y = |s|^2
+        const double c = h / 6.0, c2 = c * c;
+        D.expC[0] = 1.0f; D.expC[1] = (float)(-c2 / 8.0); D.expC[2] = (float)(c2 * c2 / 384.0); D.expC[3] = (float)(-c2 * c2 * c2 / 46080.0);
+        D.expS[0] = (float)(c / 2.0); D.expS[1] = (float)(-c * c2 / 48.0); D.expS[2] = (float)(c * c2 * c2 / 3840.0); D.expS[3] = (float)(-c * c2 * c2 * c2 / 645120.0);
     }
     D.inv_m = (float)(1.0 / p.m); D.g = p.g; D.m = p.m; D.inv_g = (float)(1.0 / p.g);
     for (int i = 0; i < 3; ++i) { D.J[i] = p.J[i]; D.invJ[i] = (float)(1.0 / p.J[i]); }
@@ -135,7 +141,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
 
 // ---- kernel dispatch: specialisations for the five benchmark configs, generic otherwise -------------
 #define FEATW(aero, euler, act, dsl, adj, rew, term) \
-    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) ? F_ADJ : 0) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT) | F_FULL)
+    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) ? F_ADJ : 0) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT) | F_FULL | F_AXISYM)
 static constexpr int FEAT_C1 = FEATW(0, 0, 0, 0, 0, 0, 1);
 static constexpr int FEAT_C2 = FEATW(3, 0, 0, 0, 0, 0, 1);
 static constexpr int FEAT_C3 = FEATW(0, 0, 1, 1, 0, 1, 2);

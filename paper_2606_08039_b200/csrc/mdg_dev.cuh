@@ -16,6 +16,7 @@ enum : int {
     F_REW_SHIFT = 9,                                      // 2 bits: MDG_REW_*
     F_TERM_SHIFT = 11,                                    // 2 bits: MDG_TERM_*
     F_TGT_CIRCLE = 1 << 13,                               // targets are the formation circle slots (chord table)
+    F_AXISYM = 1 << 15,                                   // J_xx == J_yy: no gyroscopic term about body z
     F_FULL = 1 << 14,                                     // n_drones == G: no padding lanes in a group
 };
 
@@ -31,6 +32,8 @@ struct DevParams {
     // Rodrigues coefficients of R(c w)^T as polynomials in y = |w|^2, c = h/2 (stages 2, 3) and h (stage 4):
     // A(y) = c sin(c|w|)/(c|w|), B(y) = c^2 (1 - cos(c|w|))/(c|w|)^2, degree 3
     float rotA_half[4], rotB_half[4], rotA_full[4], rotB_full[4];
+    // Eq.7 increment for phi = (h/6) s, s = w0 + 2 w2 + 2 w3 + w4, as polynomials in |s|^2: cos(|phi|/2) and (h/6) sin(|phi|/2)/|phi|
+    float expC[4], expS[4];
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
     // motor model (Eq.1-3)
     float k_f, inv_k_f, l, kappa, inv_l, inv_kappa, max_rpm, s_max, T_max, rpm2rad;
@@ -154,6 +157,14 @@ __device__ __forceinline__ Q4 exp_half(V3 phi) {
     const float c = fmaf(x, fmaf(x, fmaf(x, -2.1701389e-5f, 2.6041667e-3f), -0.125f), 1.0f);
     const float s = fmaf(x, fmaf(x, fmaf(x, -1.5500992e-6f, 2.6041667e-4f), -2.0833333e-2f), 0.5f);
     Q4 r; r.w = c; r.x = s * phi.x; r.y = s * phi.y; r.z = s * phi.z;
+    return r;
+}
+// the same increment for phi = c s with c folded into host-made coefficients (DevParams::expC, expS; degree 3 in |s|^2)
+__device__ __forceinline__ Q4 exp_half_scaled(const float (&cC)[4], const float (&cS)[4], V3 s) {
+    const float y = fmaf(s.x, s.x, fmaf(s.y, s.y, s.z * s.z));
+    const float c = fmaf(y, fmaf(y, fmaf(y, cC[3], cC[2]), cC[1]), cC[0]);
+    const float f = fmaf(y, fmaf(y, fmaf(y, cS[3], cS[2]), cS[1]), cS[0]);
+    Q4 r; r.w = c; r.x = f * s.x; r.y = f * s.y; r.z = f * s.z;
     return r;
 }
 __device__ __forceinline__ Q4 exp_half_exact(V3 phi) {

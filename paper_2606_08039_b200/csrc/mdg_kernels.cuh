@@ -21,29 +21,28 @@ __device__ __forceinline__ void store_state(const DevBuffers& B, size_t d, const
 // R(dq)^T tau_b and q0 itself is only needed for the final update.  EXACT selects the library
 // sin/cos for |omega| h > 0.75 rad; the hot path uses the branch-free series (stage_torque, exp_half).
 template <bool EXACT, bool EULER>
-__device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, V3 tau_b, V3 k1_tau) {
+__device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, V3 tau_b, V3 k1_tau, bool axisym) {
     auto ex = [](V3 phi) { return EXACT ? exp_half_exact(phi) : exp_half(phi); };
     if (!EULER) {
         const V3 w0 = w;
         const V3 k1 = v3(fmaf(-P.gyro[0], w0.y * w0.z, k1_tau.x), fmaf(-P.gyro[1], w0.z * w0.x, k1_tau.y),
-                         fmaf(-P.gyro[2], w0.x * w0.y, k1_tau.z));
+                         axisym ? k1_tau.z : fmaf(-P.gyro[2], w0.x * w0.y, k1_tau.z));
         const V3 w2 = v3(fmaf(P.half_h, k1.x, w0.x), fmaf(P.half_h, k1.y, w0.y), fmaf(P.half_h, k1.z, w0.z));
         auto stage_half = [&](V3 ws) { return EXACT ? rot_inv(exp_half_exact(v3(P.half_h * ws.x, P.half_h * ws.y, P.half_h * ws.z)), tau_b)
                                                     : stage_torque(P.rotA_half, P.rotB_half, ws, tau_b); };
         auto stage_full = [&](V3 ws) { return EXACT ? rot_inv(exp_half_exact(v3(P.h * ws.x, P.h * ws.y, P.h * ws.z)), tau_b)
                                                     : stage_torque(P.rotA_full, P.rotB_full, ws, tau_b); };
-        const V3 k2 = ang_acc(P, stage_half(w0), w2);
+        const V3 k2 = ang_acc(P, stage_half(w0), w2, axisym);
         const V3 w3 = v3(fmaf(P.half_h, k2.x, w0.x), fmaf(P.half_h, k2.y, w0.y), fmaf(P.half_h, k2.z, w0.z));
-        const V3 k3 = ang_acc(P, stage_half(w2), w3);
+        const V3 k3 = ang_acc(P, stage_half(w2), w3, axisym);
         const V3 w4 = v3(fmaf(P.h, k3.x, w0.x), fmaf(P.h, k3.y, w0.y), fmaf(P.h, k3.z, w0.z));
-        const V3 k4 = ang_acc(P, stage_full(w3), w4);
-        const V3 phi = v3(P.h_sixth * (w0.x + 2.0f * (w2.x + w3.x) + w4.x), P.h_sixth * (w0.y + 2.0f * (w2.y + w3.y) + w4.y),
-                          P.h_sixth * (w0.z + 2.0f * (w2.z + w3.z) + w4.z));
-        q = qmul(q, ex(phi));
+        const V3 k4 = ang_acc(P, stage_full(w3), w4, axisym);
+        const V3 ws = v3(w0.x + 2.0f * (w2.x + w3.x) + w4.x, w0.y + 2.0f * (w2.y + w3.y) + w4.y, w0.z + 2.0f * (w2.z + w3.z) + w4.z);
+        q = qmul(q, EXACT ? exp_half_exact(v3(P.h_sixth * ws.x, P.h_sixth * ws.y, P.h_sixth * ws.z)) : exp_half_scaled(P.expC, P.expS, ws));
         w = v3(fmaf(P.h_sixth, k1.x + 2.0f * (k2.x + k3.x) + k4.x, w0.x), fmaf(P.h_sixth, k1.y + 2.0f * (k2.y + k3.y) + k4.y, w0.y),
                fmaf(P.h_sixth, k1.z + 2.0f * (k2.z + k3.z) + k4.z, w0.z));
     } else {
-        const V3 k1 = ang_acc(P, tau_b, w);
+        const V3 k1 = ang_acc(P, tau_b, w, axisym);
         w = v3(fmaf(P.h, k1.x, w.x), fmaf(P.h, k1.y, w.y), fmaf(P.h, k1.z, w.z));
         q = qmul(q, ex(v3(P.h * w.x, P.h * w.y, P.h * w.z)));
     }
@@ -54,7 +53,7 @@ __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, 
 struct RotState { Q4 q; V3 w; };
 template <bool EULER>
 __device__ __noinline__ RotState integrate_rot_exact(const DevParams& P, Q4 q, V3 w, V3 tau_b, V3 k1_tau) {
-    integrate_rot<true, EULER>(P, q, w, tau_b, k1_tau);
+    integrate_rot<true, EULER>(P, q, w, tau_b, k1_tau, false);
     RotState r; r.q = q; r.w = w;
     return r;
 }
@@ -267,22 +266,32 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             // One reciprocal r = 1 / (dz_e^2 b'^2) serves both: alpha ~ b'^2 r, exponent = -dxy^2 (dz_e^2 r).
             // The ramp saturate(dz / dz_clip) is 0 for dz <= 0, which also gates "k above this drone";
             // b'^2 is floored (beta^2 >= 1e-12), which reproduces the beta -> 0 rule of DESIGN.md Q9.
+            // Pairs are shared out: in round r < G/2 lane j evaluates the pair (j, j + r mod G) once for both ends -
+            // the force goes to whichever drone is lower, the partner's share travels back by one shuffle - and in
+            // round G/2 both ends evaluate their common pair and each keeps its own share.
             float dw = 0.0f;
 #pragma unroll
-            for (int kk = 1; kk < G; ++kk) {                      // partner lane = lane ^ kk: every other drone once
-                const float ox = __shfl_xor_sync(MDG_FULL, d.p.x, kk), oy = __shfl_xor_sync(MDG_FULL, d.p.y, kk),
-                            oz = __shfl_xor_sync(MDG_FULL, d.p.z, kk);
+            for (int r = 1; r <= G / 2; ++r) {
+                const int src = j + r;                             // logical lane inside the G-wide segment (taken mod G)
+                const float ox = __shfl_sync(MDG_FULL, d.p.x, src, G), oy = __shfl_sync(MDG_FULL, d.p.y, src, G),
+                            oz = __shfl_sync(MDG_FULL, d.p.z, src, G);
                 const float dz = oz - d.p.z, dx = ox - d.p.x, dy = oy - d.p.y;
                 const float dxy2 = fmaf(dx, dx, dy * dy);
-                const float dze = fmaxf(dz, P.dz_floor);
-                const float ramp = __saturatef(dz * P.inv_dz_clip);
+                const float adz = fabsf(dz);
+                const float dze = fmaxf(adz, P.dz_floor);
+                const float ramp = __saturatef(adz * P.inv_dz_clip);
                 const float bs = fmaf(P.dw_C2s, dze, P.dw_C3s);
                 const float b2 = fmaxf(bs * bs, P.dw_b2_min), z2 = dze * dze;
                 const float rinv = rcp_fast(z2 * b2);
                 const float ex = ex2_fast(-dxy2 * (z2 * rinv));
                 const float al = ramp * (b2 * rinv);
-                const bool on = (full_group || (j ^ kk) < P.M) && dxy2 < 100.0f;
-                dw = fmaf(al, on ? ex : 0.0f, dw);
+                const bool on = (full_group || (j < P.M && ((j + r) & (G - 1)) < P.M)) && dxy2 < 100.0f;
+                const float f = on ? al * ex : 0.0f;
+                const bool above = dz > 0.0f;                      // the partner is above this drone
+                if (r < G / 2) {
+                    const float back = __shfl_sync(MDG_FULL, above ? 0.0f : f, j + G - r, G);
+                    dw += (above ? f : 0.0f) + back;
+                } else dw += above ? f : 0.0f;
             }
             Fw.z = fmaf(-P.dw_coef, dw, Fw.z);
         }
@@ -296,12 +305,12 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             d.p.z = fmaf(P.half_h2, acc.z, fmaf(P.h, d.v.z, d.p.z));
             d.v.x = fmaf(P.h, acc.x, d.v.x); d.v.y = fmaf(P.h, acc.y, d.v.y); d.v.z = fmaf(P.h, acc.z, d.v.z);
             if (fast_spin) { const RotState rs = integrate_rot_exact<false>(P, d.q, d.w, tau_b, k1_tau); d.q = rs.q; d.w = rs.w; }
-            else integrate_rot<false, false>(P, d.q, d.w, tau_b, k1_tau);
+            else integrate_rot<false, false>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
         } else {                                                   // DYN: explicit Euler
             d.v.x = fmaf(P.h, acc.x, d.v.x); d.v.y = fmaf(P.h, acc.y, d.v.y); d.v.z = fmaf(P.h, acc.z, d.v.z);
             d.p.x = fmaf(P.h, d.v.x, d.p.x); d.p.y = fmaf(P.h, d.v.y, d.p.y); d.p.z = fmaf(P.h, d.v.z, d.p.z);
             if (fast_spin) { const RotState rs = integrate_rot_exact<true>(P, d.q, d.w, tau_b, k1_tau); d.q = rs.q; d.w = rs.w; }
-            else integrate_rot<false, true>(P, d.q, d.w, tau_b, k1_tau);
+            else integrate_rot<false, true>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
         }
         if (d.p.z < 0.0f) { hit = true; d.p.z = 0.0f; d.v.z = fmaxf(d.v.z, 0.0f); }   // floor
     }

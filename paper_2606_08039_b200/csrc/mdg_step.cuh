@@ -123,11 +123,11 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     n[2] = fast_sqrt(clampf(s2, 0.0f, P.s_max) * P.inv_k_f); n[3] = fast_sqrt(clampf(s3, 0.0f, P.s_max) * P.inv_k_f);
 }
 
-// angular acceleration J^-1 (tau_body - w x J w)
-__device__ __forceinline__ V3 ang_acc(const DevParams& P, V3 tb, V3 w) {
+// angular acceleration J^-1 (tau_body - w x J w); axisym: J_xx == J_yy, the z component has no gyroscopic term
+__device__ __forceinline__ V3 ang_acc(const DevParams& P, V3 tb, V3 w, bool axisym) {
     return v3(fmaf(P.invJ[0], tb.x, -P.gyro[0] * (w.y * w.z)),
               fmaf(P.invJ[1], tb.y, -P.gyro[1] * (w.z * w.x)),
-              fmaf(P.invJ[2], tb.z, -P.gyro[2] * (w.x * w.y)));
+              axisym ? P.invJ[2] * tb.z : fmaf(P.invJ[2], tb.z, -P.gyro[2] * (w.x * w.y)));
 }
 
 // Observation row of one drone: [p, eta, v, w (, adjacency)] written as float4s when the row is 16 B aligned
