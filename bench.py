@@ -247,6 +247,10 @@ def run_ours(args, wl, c):
     except Exception:
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    try:
+        ffma_tf = mdg.measure_fp32_peak(stream)              # FFMA microbenchmark on this GPU, this run
+    except Exception:
+        ffma_tf = None
     achieved_tf = flops / per_launch_s / 1e12
     t_alu, t_hbm = flops / (ALU_PEAK_TFLOPS * 1e12), bytes_alg / (hbm_peak * 1e9)
     traffic = None                                         # dram read + write bytes per launch, one ncu --set full capture
@@ -265,6 +269,7 @@ def run_ours(args, wl, c):
                          "traffic": traffic, "kernel": envs[0].kernel_name, "us_per_launch": per_launch_s * 1e6,
                          "flops_per_launch": flops, "bytes_per_launch": bytes_alg,
                          "peak_note": "FP32 ALU peak derived: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md §6)",
+                         "ffma_measured_tflops": ffma_tf, "frac_of_ffma_measured": (achieved_tf / ffma_tf) if ffma_tf else None,
                          "hbm": {"achieved_gbs": bytes_alg / per_launch_s / 1e9, "peak_gbs": hbm_peak,
                                  "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback of B200_PROFILING.md",
                                  "frac": bytes_alg / per_launch_s / 1e9 / hbm_peak},

@@ -129,7 +129,12 @@ int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float
 int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
                   const float* wind, const uint32_t* ep_step);
 
-/* Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) used by later calls. */
+/* Scheduling note for mdg_step: the step is launched with programmatic dependent launch.  When the previous
+ * operation on the handle was a step on the same stream, the new launch does not wait for that kernel as a whole but,
+ * work item by work item, for the sequence flags it publishes; all other stream semantics are unchanged:
+ * any non-PDL operation enqueued after a step (a copy, a kernel reading obs) sees the step complete.
+ *
+ * Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) used by later calls. */
 int mdg_set_stream(mdg_env* env, void* cuda_stream);
 
 /* Introspection: kernels launched so far through this handle; name of the step kernel specialisation. */
@@ -137,6 +142,11 @@ int64_t mdg_launch_count(const mdg_env* env);
 const char* mdg_kernel_name(const mdg_env* env);
 /* Launch shape tuning (0 keeps the current value): threads per block, and a cap on resident blocks per SM. */
 int mdg_set_launch(mdg_env* env, int block_threads, int max_blocks_per_sm);
+
+/* Measurement aid for the roofline denominator: runs a register-only FFMA kernel (8 independent
+ * chains per thread, every SM full) on the current device, times it with CUDA events on `cuda_stream` and writes
+ * the achieved FP32 rate in TFLOP/s (2 flop per FFMA) to *tflops (host pointer).  Synchronises the stream. */
+int mdg_measure_fp32_peak(void* cuda_stream, double* tflops);
 
 const char* mdg_last_error(void);
 int mdg_version(void);

@@ -5,6 +5,6 @@ its thin Python binding plus the seeded workload recipes.  Importing the package
 using `Env` without the built library or without a GPU raises.
 """
 from . import workloads
-from .binding import Env, MdgError, default_params, lib, mdg_params
+from .binding import Env, MdgError, default_params, lib, mdg_params, measure_fp32_peak
 
-__all__ = ["Env", "MdgError", "default_params", "lib", "mdg_params", "workloads"]
+__all__ = ["Env", "MdgError", "default_params", "lib", "mdg_params", "measure_fp32_peak", "workloads"]

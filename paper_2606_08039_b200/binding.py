@@ -48,7 +48,7 @@ class mdg_params(C.Structure):
 
 EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
-           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_last_error", "mdg_version"]
+           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_last_error", "mdg_version"]
 
 _lib = None
 
@@ -83,8 +83,18 @@ def lib():
         L.mdg_kernel_name.restype = C.c_char_p
         L.mdg_set_launch.argtypes = [vp, C.c_int, C.c_int]
         L.mdg_last_error.restype = C.c_char_p
+        L.mdg_measure_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
         _lib = L
     return _lib
+
+
+def measure_fp32_peak(stream=None) -> float:
+    """Achieved FP32 FFMA rate of the current device in TFLOP/s (include/mdg.h: mdg_measure_fp32_peak)."""
+    import torch
+    out = C.c_double(0.0)
+    s = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().mdg_measure_fp32_peak(C.c_void_p(s.cuda_stream), C.byref(out)))
+    return out.value
 
 
 class MdgError(RuntimeError):
