@@ -25,14 +25,14 @@ from paper_2606_08039_b200 import workloads as W
 TOL_P, TOL_V, TOL_Q, TOL_W, TOL_R, TIE = 1e-4, 1e-3, 1e-4, 1e-3, 1e-3, 1e-4
 
 
-def make_pair(wl, extra=None):
+def make_pair(wl, extra=None, model=0):
     import paper_2606_08039_b200 as mdg
     over = dict(wl.params)
     if extra:
         over.update(extra)
-    orc = O.OracleEnv(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, O.OracleParams(0, **over),
+    orc = O.OracleEnv(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, O.OracleParams(model, **over),
                       n_threads=os.cpu_count() or 1)
-    gpu = mdg.Env(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, mdg.default_params(0, **over))
+    gpu = mdg.Env(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, mdg.default_params(model, **over))
     return orc, gpu
 
 
@@ -77,11 +77,11 @@ def shadow_drift(orc, shadow, M):
     return bad
 
 
-def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0):
-    orc, gpu = make_pair(wl, extra)
+def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=0):
+    orc, gpu = make_pair(wl, extra, model)
     over = dict(wl.params)
     over.update(extra or {})
-    shadow = O.OracleEnv(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, O.OracleParams(0, **over),
+    shadow = O.OracleEnv(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, O.OracleParams(model, **over),
                          n_threads=os.cpu_count() or 1)
     N, M = wl.n_envs, wl.n_drones
     orc.reset(wl.seed)

@@ -1,0 +1,103 @@
+"""-m gpu: the runtime-flag (generic) step kernel and the corner shapes against the float64 oracle.
+
+The five BASELINE.json configs run compile-time specialisations; everything else - drone counts that do not
+fill a lane group, the DYN integrator, the RACE airframe, PID without the DSL limits, formation rewards on
+arbitrary targets, termination off - runs the generic instantiation of the same source.  Each case is a
+small synthetic workload in the style of `workloads.py` stepped for 1 s of simulated time.
+"""
+import pytest
+
+from paper_2606_08039_b200 import workloads as W
+from parity_util import run_parity
+
+pytestmark = pytest.mark.gpu
+
+HOVER = ("hover_scale", 0.9, 1.1)
+GRID = dict(reset_layout=W.LAYOUT_GRID, grid_cols=3, grid_spacing=0.3, reset_center=[0, 0, 0], reset_half=[0.05, 0.05, 0],
+            reset_z_lo=0.3, reset_z_hi=1.2, reward_mode=W.REW_MULTI_HOVER, term_mode=W.TERM_HOVER,
+            target_mode=W.TGT_SPAWN_LINSPACE, mh_z_lo=0.7, mh_z_hi=1.2, episode_len_s=10.0, auto_reset=1)
+CIRCLE = dict(reset_layout=W.LAYOUT_CIRCLE, circle_radius=0.4, reset_center=[0, 0, 1], reset_half=[0.05, 0.05, 0.05],
+              obs_mode=W.OBS_KIN12_ADJ, adj_radius=0.5, reward_mode=W.REW_FORMATION, term_mode=W.TERM_FORMATION,
+              term_center=[0, 0, 1], term_dist=3.0, form_center=[0, 0, 1], form_radius=0.4, episode_len_s=30.0, auto_reset=1)
+
+
+def wl(name, n, m, phys, act, params, actions, seed=77):
+    return W.Workload(name, n, m, phys, act, params, actions, 48, W.BASE_SEED + seed)
+
+
+CASES = {
+    # partial lane groups: M = 3 in G = 4, M = 5 and 6 in G = 8, M = 11 in G = 16, M = 20 in G = 32
+    "m3_all_aero": (wl("m3", 1001, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
+    "m5_vel_wind_formation": (wl("m5", 517, 5, W.PHYS_MJC_GND_DRAG_DW, W.ACT_VEL,
+                                 dict(CIRCLE, aero_mask=15, wind_sigma=0.5, wind_tau=1.0, target_mode=W.TGT_CIRCLE),
+                                 ("uniform", -1.0, 1.0)), {}),
+    "m6_dw_only": (wl("m6", 300, 6, W.PHYS_MJC_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
+    "m11_g16": (wl("m11", 130, 11, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID, grid_cols=4), HOVER), {}),
+    "m20_g32": (wl("m20", 67, 20, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID, grid_cols=5), HOVER), {}),
+    # full groups the benchmark configs do not use
+    "m2_dyn_euler": (wl("m2", 777, 2, W.PHYS_DYN, W.ACT_RPM, dict(GRID, aero_mask=W.AERO_DW | W.AERO_DRAG), HOVER), {}),
+    "m16_full": (wl("m16", 64, 16, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID, grid_cols=4), HOVER), {}),
+    "m32_full": (wl("m32", 33, 32, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID, grid_cols=8), HOVER), {}),
+    # formation reward against targets that are not the circle slots (pair distances by shuffle)
+    "m4_formation_box_targets": (wl("m4box", 600, 4, W.PHYS_MJC, W.ACT_VEL,
+                                    dict(CIRCLE, target_mode=W.TGT_BOX, target_lo=[-0.5, -0.5, 0.8], target_hi=[0.5, 0.5, 1.2]),
+                                    ("uniform", -1.0, 1.0)), {}),
+    # single drone: DYN integrator, PID without the DSL limits, ground effect only, no termination / no auto-reset
+    "m1_dyn_rpm": (wl("m1dyn", 2049, 1, W.PHYS_DYN, W.ACT_RPM,
+                      dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_HOVER, term_mode=W.TERM_HOVER,
+                           target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=10.0, auto_reset=1), ("hover_scale", 0.95, 1.05)), {}),
+    "m1_pid_no_dsl": (wl("m1pid", 1500, 1, W.PHYS_MJC_GND, W.ACT_PID,
+                         dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST,
+                              term_tilt=0.4, term_dist=3.0, target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
+                              episode_len_s=10.0, auto_reset=1), ("targets",)), {}),
+    "m1_no_term_no_reset": (wl("m1free", 900, 1, W.PHYS_MJC_DRAG, W.ACT_RPM,
+                               dict(reset_center=[0, 0, 1.5], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_HOVER, term_mode=W.TERM_NONE,
+                                    target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=0.25, auto_reset=0), ("hover_scale", 0.7, 1.0)), {}),
+    # one env, one warp not even full
+    "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
+}
+
+
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_generic_kernel_parity(name):
+    w, extra = CASES[name]
+    res = run_parity(w, steps=48, extra=extra, max_ill_frac=0.08 if w.n_drones > 1 else 0.0)
+    print(name, res)
+    assert "generic" in res["kernel"]
+
+
+def test_race_airframe_parity():
+    """Table 2's RACE column (mass 0.25 kg, k_f 1.28e-8): rotor speeds around its own hover RPM (6,920)."""
+    w = wl("race", 1200, 1, W.PHYS_MJC_GND, W.ACT_RPM,
+           dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_HOVER, term_mode=W.TERM_HOVER,
+                target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=10.0, auto_reset=1), ("uniform", 6300.0, 7500.0))
+    res = run_parity(w, steps=48, model=W.MODEL_RACE)
+    print(res)
+
+
+def test_error_paths_and_step_many():
+    """Argument errors come back as codes (no abort); a CUDA-graph replay of n steps equals n single steps."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    for bad in [dict(n_envs=0, n_drones=1), dict(n_envs=4, n_drones=33), dict(n_envs=4, n_drones=0)]:
+        with pytest.raises(mdg.MdgError):
+            mdg.Env(bad["n_envs"], bad["n_drones"], W.PHYS_MJC, W.ACT_RPM)
+    with pytest.raises(mdg.MdgError):
+        mdg.Env(4, 1, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, sim_freq=250, ctrl_freq=48))   # not a multiple
+    w = W.config(5).scaled(3000)
+    a, b = (mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **w.params)) for _ in range(2))
+    a.reset(w.seed); b.reset(w.seed)
+    acts = torch.stack([a.gen_actions(w.seed, t, 1.0, -1.0, 1.0) for t in range(6)])
+    with pytest.raises(mdg.MdgError):
+        a.step(acts.view(-1)[1:1 + w.n_envs * w.n_drones * 4])                                 # not 16-byte aligned
+    for t in range(6):
+        a.step(acts[t])
+    b.step_many(acts, 6)
+    b.step_many(acts, 6)                                                                       # cached graph, replayed
+    for t in range(6):
+        a.step(acts[t])
+    torch.cuda.synchronize()
+    sa, sb = a.get_state(), b.get_state()
+    assert np.array_equal(sa["state"], sb["state"]) and np.array_equal(sa["ep_step"], sb["ep_step"])
+    assert torch.equal(a.obs, b.obs) and torch.equal(a.reward, b.reward) and torch.equal(a.done, b.done)
