@@ -37,14 +37,26 @@ enum { MDG_INTEG_RK4 = 0, MDG_INTEG_EULER = 1 };
 /* Table 1 */
 enum { MDG_PHYS_MJC = 0, MDG_PHYS_MJC_GND = 1, MDG_PHYS_MJC_DRAG = 2, MDG_PHYS_MJC_DW = 3,
        MDG_PHYS_MJC_GND_DRAG_DW = 4, MDG_PHYS_DYN = 5 };
-/* Table 3; ONE_D_RPM and ATTITUDE are not built yet */
-enum { MDG_ACT_RPM = 0, MDG_ACT_PID = 1, MDG_ACT_VEL = 2 };
-enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1 };
+/* Table 3.  Every action row is 4 floats per drone:
+ *  RPM        raw rotor speeds, clipped to [0, MAX_RPM]
+ *  PID        waypoint [x, y, z, psi] through the cascaded PID
+ *  VEL        heading-frame [v_x, v_y, v_z, omega_z] through the same PID
+ *  RPM_NORM   four rotor commands in [-1, 1] through normalizedActionToRPM: -1 -> 0, 0 -> HOVER_RPM,
+ *             +1 -> MAX_RPM, piecewise linear, clipped (reading Q35)
+ *  ONE_D_RPM  a[0] in [-1, 1] through the same map to all four rotors; a[1..3] ignored
+ *  ATTITUDE   [thrust in [-1, 1] (same map, T = 4 k_f rpm^2), roll* rad, pitch* rad, yaw rate rad/s] through the
+ *             attitude loop and the mixer of the cascaded PID (reading Q36) */
+enum { MDG_ACT_RPM = 0, MDG_ACT_PID = 1, MDG_ACT_VEL = 2, MDG_ACT_RPM_NORM = 3, MDG_ACT_ONE_D_RPM = 4, MDG_ACT_ATTITUDE = 5 };
+/* PAPER.md:177, 13.  KIN12 = [p, eta, v, omega]; KIN12_ADJ appends the adjacency row; KIN20 = [p, q, eta, v, omega,
+ * a_{t-1}] with a_{t-1} the action applied in the step that produced the state (zeros after a reset). */
+enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1, MDG_OBS_KIN20 = 2 };
 enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3 };
 enum { MDG_TERM_NONE = 0, MDG_TERM_HOVER = 1, MDG_TERM_TILT_DIST = 2, MDG_TERM_FORMATION = 3 };
 enum { MDG_LAYOUT_NONE = 0, MDG_LAYOUT_GRID = 1, MDG_LAYOUT_CIRCLE = 2 };
 enum { MDG_TGT_FIXED = 0, MDG_TGT_SPAWN_LINSPACE = 1, MDG_TGT_BOX = 2, MDG_TGT_CIRCLE = 3 };
-enum { MDG_MODEL_CF2X = 0, MDG_MODEL_RACE = 2 };                /* Table 2 */
+/* Table 2.  CF2P has CF2X's parameters and the +-configuration mixing:
+ * tau_x = L (F_1 - F_3), tau_y = L (-F_0 + F_2) (reading Q37). */
+enum { MDG_MODEL_CF2X = 0, MDG_MODEL_CF2P = 1, MDG_MODEL_RACE = 2 };
 
 /* Plain-old-data parameter block.  struct_size must equal sizeof(mdg_params) (set by
  * mdg_default_params); units SI, rotor speeds in RPM, k_f and k_m per RPM^2 (DESIGN.md §3 Q1). */

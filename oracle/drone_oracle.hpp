@@ -32,13 +32,13 @@ namespace orc {
 enum { AERO_GND = 1, AERO_DRAG = 2, AERO_DW = 4, AERO_WIND = 8 };
 enum { INTEG_RK4 = 0, INTEG_EULER = 1 };
 enum { PHYS_MJC = 0, PHYS_MJC_GND = 1, PHYS_MJC_DRAG = 2, PHYS_MJC_DW = 3, PHYS_MJC_GND_DRAG_DW = 4, PHYS_DYN = 5 };
-enum { ACT_RPM = 0, ACT_PID = 1, ACT_VEL = 2 };
-enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1 };
+enum { ACT_RPM = 0, ACT_PID = 1, ACT_VEL = 2, ACT_RPM_NORM = 3, ACT_ONE_D_RPM = 4, ACT_ATTITUDE = 5 };
+enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2 };
 enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3 };
 enum { TERM_NONE = 0, TERM_HOVER = 1, TERM_TILT_DIST = 2, TERM_FORMATION = 3 };
 enum { LAYOUT_NONE = 0, LAYOUT_GRID = 1, LAYOUT_CIRCLE = 2 };
 enum { TGT_FIXED = 0, TGT_SPAWN_LINSPACE = 1, TGT_BOX = 2, TGT_CIRCLE = 3 };
-enum { MODEL_CF2X = 0, MODEL_RACE = 2 };
+enum { MODEL_CF2X = 0, MODEL_CF2P = 1, MODEL_RACE = 2 };
 
 static const double PI = 3.14159265358979323846;
 
@@ -68,6 +68,7 @@ struct Params {
     int target_mode; double target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi,
         form_center[3], form_radius;
     int env_index_base;              // global index of env 0 (sharding across GPUs)
+    int drone_model;                 // MODEL_*: CF2P selects the +-configuration mixing (Q37)
 };
 
 inline void default_params(int model, Params& P) {
@@ -79,6 +80,7 @@ inline void default_params(int model, Params& P) {
         P.m = 0.027; P.L = 0.0397; P.tw_ratio = 2.25; P.J[0] = P.J[1] = 1.4e-5; P.J[2] = 2.17e-5;
         P.k_f = 3.16e-10; P.k_m = 7.94e-12; P.r_p = 0.02325;
     }
+    P.drone_model = model;
     P.g = 9.81;                                                   // Q2
     P.C_gnd = 11.36859; P.c_xy = 9.1785e-7; P.c_z = 10.311e-7;   // Q5
     P.h_clip = 0.25 * P.r_p * std::sqrt(15.0 * P.C_gnd / 4.0);    // Q6
@@ -98,6 +100,7 @@ inline void default_params(int model, Params& P) {
     P.pos_rate_limit = 2.0; P.yaw_rate_limit = PI; P.tilt_max = 0.5;
     const double s_hover = P.m * P.g / 4.0;                       // Q17
     P.tau_xy_max = 4.0 * (P.L / std::sqrt(2.0)) * s_hover / 3.0;
+    if (model == MODEL_CF2P) P.tau_xy_max = 2.0 * P.L * s_hover / 3.0;   // Q37: two rotors per axis, same rule
     P.tau_z_max = 4.0 * (P.k_m / P.k_f) * s_hover / 3.0;
     P.obs_mode = OBS_KIN12; P.adj_radius = 0.5;
     P.reward_mode = REW_HOVER; P.at_target_radius = 0.05;         // Q24
@@ -214,6 +217,7 @@ template <class R> struct Drone {
     R p[3], q[4], v[3], w[3];     // A1 state; w is body-frame (Q22)
     R Ip[3], Ie[3], sp[4];        // PID memory: position / attitude integrals, held setpoint (DSL)
     double tg[4];                 // per-episode target (x, y, z, psi)
+    double act[4];                // the action row applied in this control step (KIN20's a_{t-1}); zeros after a reset
     R n[4];                       // rotor speeds in RPM, held over the K substeps (Q21)
     R T, tau_b[3], Om;            // O4: collective thrust, body torque, sum of 2 pi n / 60
     R Fwind[3];                   // O9 wind force, held over the K substeps (Q28)
@@ -228,20 +232,60 @@ inline void motor_wrench(const Params& P, const Derived& D, const R n[4], R& T, 
     R s[4];
     for (int i = 0; i < 4; ++i) s[i] = P.k_f * (n[i] * n[i]);
     T = s[0] + s[1] + s[2] + s[3];
-    tau[0] = D.l * (s[0] + s[1] - s[2] - s[3]);
-    tau[1] = D.l * (-s[0] + s[1] + s[2] - s[3]);
+    if (P.drone_model == MODEL_CF2P) {                             // +-configuration (Q37)
+        tau[0] = P.L * (s[1] - s[3]);
+        tau[1] = P.L * (s[2] - s[0]);
+    } else {
+        tau[0] = D.l * (s[0] + s[1] - s[2] - s[3]);
+        tau[1] = D.l * (-s[0] + s[1] + s[2] - s[3]);
+    }
     tau[2] = D.kappa * (-s[0] + s[1] - s[2] + s[3]);
     Om = (2.0 * PI / 60.0) * (n[0] + n[1] + n[2] + n[3]);      // Eq.5's rotor-speed sum
 }
 
 // O3.7 closed-form allocation inverse: per-rotor thrusts from (T, tau)
 template <class R>
-inline void alloc_inverse(const Derived& D, const R& T, const R tau[3], R s[4]) {
+inline void alloc_inverse(const Params& P, const Derived& D, const R& T, const R tau[3], R s[4]) {
+    if (P.drone_model == MODEL_CF2P) {                             // inverse of the +-configuration mixing (Q37)
+        const R a = tau[0] / P.L, b = tau[1] / P.L, c = tau[2] / D.kappa;
+        s[0] = 0.25 * (T - 2.0 * b - c);
+        s[1] = 0.25 * (T + 2.0 * a + c);
+        s[2] = 0.25 * (T + 2.0 * b - c);
+        s[3] = 0.25 * (T - 2.0 * a + c);
+        return;
+    }
     const R a = tau[0] / D.l, b = tau[1] / D.l, c = tau[2] / D.kappa;
     s[0] = 0.25 * (T + a - b - c);
     s[1] = 0.25 * (T + a + b + c);
     s[2] = 0.25 * (T - a + b - c);
     s[3] = 0.25 * (T - a - b + c);
+}
+
+// normalizedActionToRPM (reading Q35): [-1, 1] -> [0, MAX_RPM] through HOVER_RPM at 0, piecewise linear
+template <class R>
+inline R normalized_to_rpm(const Derived& D, double a_in) {
+    const R a = clampR(R(a_in), -1.0, 1.0);
+    if (a > 0.0) return D.hover_rpm + (D.max_rpm - D.hover_rpm) * a;
+    return (a + 1.0) * D.hover_rpm;
+}
+
+// O3.6 attitude PID (D on measurement) and O3.7 allocation inverse with per-rotor clip
+template <class R>
+inline void attitude_loop_and_mix(const Params& P, const Derived& D, const R& T, const R& phi_ref, const R& th_ref, const R& psi_ref,
+                                  const R eta[3], Drone<R>& d) {
+    const double dt = D.dt_c;
+    R e_eta[3] = {phi_ref - eta[0], th_ref - eta[1], wrap_pi(psi_ref - eta[2])};
+    R tau[3];
+    for (int i = 0; i < 3; ++i) {
+        d.Ie[i] = clampR(d.Ie[i] + e_eta[i] * dt, -P.int_clamp_att, P.int_clamp_att);
+        tau[i] = P.Kp_att[i] * e_eta[i] + P.Ki_att[i] * d.Ie[i] - P.Kd_att[i] * d.w[i];
+    }
+    tau[0] = clampR(tau[0], -P.tau_xy_max, P.tau_xy_max);
+    tau[1] = clampR(tau[1], -P.tau_xy_max, P.tau_xy_max);
+    tau[2] = clampR(tau[2], -P.tau_z_max, P.tau_z_max);
+    R s[4];
+    alloc_inverse(P, D, T, tau, s);
+    for (int i = 0; i < 4; ++i) d.n[i] = sqrt(clampR(s[i], 0.0, D.s_max) / P.k_f);
 }
 
 // O2/O3 action decode -> RPM (Table 3; cascaded PID PAPER.md:347-357, 372-376)
@@ -251,10 +295,23 @@ inline void decode_action(const Params& P, const Derived& D, int action_type, co
         for (int i = 0; i < 4; ++i) d.n[i] = clampR(R((double)a_in[i]), 0.0, D.max_rpm);
         return;
     }
+    if (action_type == ACT_RPM_NORM || action_type == ACT_ONE_D_RPM) {   // Table 3 / PAPER.md:300, reading Q35
+        for (int i = 0; i < 4; ++i) d.n[i] = normalized_to_rpm<R>(D, (double)a_in[action_type == ACT_ONE_D_RPM ? 0 : i]);
+        return;
+    }
     const double dt = D.dt_c;                                      // Q21: once per control step
     R eta[3];
     euler_zyx(d.q, eta);                                           // O3.1
     const R psi = eta[2];
+    if (action_type == ACT_ATTITUDE) {                             // Table 3, reading Q36: [thrust, roll*, pitch*, yaw rate]
+        const R nt = normalized_to_rpm<R>(D, (double)a_in[0]);
+        const R T = 4.0 * (P.k_f * (nt * nt));
+        const R phi_ref = clampR(R((double)a_in[1]), -P.tilt_max, P.tilt_max);
+        const R th_ref = clampR(R((double)a_in[2]), -P.tilt_max, P.tilt_max);
+        const R psi_ref = psi + (double)a_in[3] * dt;
+        attitude_loop_and_mix(P, D, T, phi_ref, th_ref, psi_ref, eta, d);
+        return;
+    }
     R p_ref[3], v_ref[3], psi_ref;
     if (action_type == ACT_PID) {                                  // O3.2 waypoint [x,y,z,psi]
         const double pc[3] = {(double)a_in[0], (double)a_in[1], (double)a_in[2]};
@@ -299,20 +356,7 @@ inline void decode_action(const Params& P, const Derived& D, int action_type, co
     const R cps = cos(psi), sps = sin(psi);
     const R phi_ref = clampR((acc[0] * sps - acc[1] * cps) / P.g, -P.tilt_max, P.tilt_max);
     const R th_ref = clampR((acc[0] * cps + acc[1] * sps) / P.g, -P.tilt_max, P.tilt_max);
-    // O3.6 attitude PID, D on measurement
-    R e_eta[3] = {phi_ref - eta[0], th_ref - eta[1], wrap_pi(psi_ref - psi)};
-    R tau[3];
-    for (int i = 0; i < 3; ++i) {
-        d.Ie[i] = clampR(d.Ie[i] + e_eta[i] * dt, -P.int_clamp_att, P.int_clamp_att);
-        tau[i] = P.Kp_att[i] * e_eta[i] + P.Ki_att[i] * d.Ie[i] - P.Kd_att[i] * d.w[i];
-    }
-    tau[0] = clampR(tau[0], -P.tau_xy_max, P.tau_xy_max);
-    tau[1] = clampR(tau[1], -P.tau_xy_max, P.tau_xy_max);
-    tau[2] = clampR(tau[2], -P.tau_z_max, P.tau_z_max);
-    // O3.7 allocation inverse and per-rotor clip
-    R s[4];
-    alloc_inverse(D, T, tau, s);
-    for (int i = 0; i < 4; ++i) d.n[i] = sqrt(clampR(s[i], 0.0, D.s_max) / P.k_f);
+    attitude_loop_and_mix(P, D, T, phi_ref, th_ref, psi_ref, eta, d);
 }
 
 // O5-O7: world-frame wrench of drone i from the start-of-substep state of all M drones of the env
@@ -441,7 +485,7 @@ struct Sim {
     std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
     std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
 
-    int opd() const { return 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
+    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
     int obs_dim() const { return M * opd(); }
 
     void init(int n_envs, int n_drones, int phys, int act, const Params& p) {
@@ -510,6 +554,7 @@ struct Sim {
             for (int a = 0; a < 3; ++a) { d.p[a] = s[a]; d.v[a] = s[7 + a]; d.w[a] = s[10 + a]; d.Ip[a] = pm[a]; d.Ie[a] = pm[3 + a]; }
             for (int a = 0; a < 4; ++a) { d.q[a] = s[3 + a]; d.sp[a] = pm[6 + a]; d.tg[a] = target[di * 4 + a]; }
             for (int a = 0; a < 3; ++a) d.Fwind[a] = 0.0;
+            for (int a = 0; a < 4; ++a) d.act[a] = 0.0;
             d.hit = false; d.min_abs_pz = 1e30;
         }
     }
@@ -532,6 +577,11 @@ struct Sim {
             R eta[3];
             euler_zyx(dr[i].q, eta);
             double* oi = o + (size_t)i * od;
+            if (P.obs_mode == OBS_KIN20) {                         // [p, q, eta, v, omega, a_{t-1}]
+                for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[7 + a] = to_d(eta[a]); oi[10 + a] = to_d(dr[i].v[a]); oi[13 + a] = to_d(dr[i].w[a]); }
+                for (int a = 0; a < 4; ++a) { oi[3 + a] = to_d(dr[i].q[a]); oi[16 + a] = dr[i].act[a]; }
+                continue;
+            }
             for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[3 + a] = to_d(eta[a]); oi[6 + a] = to_d(dr[i].v[a]); oi[9 + a] = to_d(dr[i].w[a]); }
             if (P.obs_mode == OBS_KIN12_ADJ) {
                 for (int k = 0; k < M; ++k) {
@@ -571,6 +621,7 @@ struct Sim {
         // O2/O3 decode, O4 motor model
         for (int i = 0; i < M; ++i) {
             decode_action(P, D, action_type, actions + ((size_t)e * M + i) * 4, dr[i]);
+            for (int a = 0; a < 4; ++a) dr[i].act[a] = (double)actions[((size_t)e * M + i) * 4 + a];
             motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om);
         }
         // K substeps: all wrenches from the same start-of-substep state, then integrate

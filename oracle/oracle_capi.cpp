@@ -60,7 +60,7 @@ static const Field FIELDS[] = {
     FD(episode_len_s, 1), FI(auto_reset), FI(reset_layout), FD(reset_center, 3), FD(reset_half, 3),
     FD(reset_z_lo, 1), FD(reset_z_hi, 1), FI(grid_cols), FD(grid_spacing, 1), FD(circle_radius, 1), FI(target_mode),
     FD(target_fixed, 3), FD(target_lo, 3), FD(target_hi, 3), FD(mh_z_lo, 1), FD(mh_z_hi, 1), FD(form_center, 3),
-    FD(form_radius, 1), FI(env_index_base),
+    FD(form_radius, 1), FI(env_index_base), FI(drone_model),
 };
 static const Field* find_field(const char* name) {
     for (const Field& f : FIELDS) if (std::string(f.name) == name) return &f;
@@ -190,7 +190,7 @@ void orc_motor_wrench(const void* params, const double* rpm, double* out5) {   /
 }
 void orc_alloc_inverse(const void* params, double T, const double* tau, double* s4) {
     const Params& P = *(const Params*)params; const Derived D = derive(P, 0);
-    alloc_inverse(D, T, tau, s4);
+    alloc_inverse(*(const Params*)params, D, T, tau, s4);
 }
 void orc_euler_zyx(const double* q, double* eta) { euler_zyx(q, eta); }
 void orc_quat_exp_step(const double* q, const double* phi, double* out) { quat_exp_step(q, phi, out); }

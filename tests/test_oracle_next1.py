@@ -1,0 +1,125 @@
+"""Pins of the oracle's SURVEY.md §8(f) NEXT-1 parts: normalised RPM actions, ONE_D_RPM, ATTITUDE, the 20-dim KIN
+observation and the +-configuration (CF2P) mixing.  Expected values come from the paper's statements and from
+closed forms worked out here, never from the oracle or the CUDA path."""
+import math
+
+import numpy as np
+
+from oracle import oracle as O
+from oracle_util import FREE, make_env, set_state
+from paper_2606_08039_b200 import workloads as W
+
+M, G, KF, KM, L = 0.027, 9.81, 3.16e-10, 7.94e-12, 0.0397          # Table 2, CF2X / CF2P column
+JXX, JZZ = 1.4e-5, 2.17e-5
+HOVER = math.sqrt(M * G / (4 * KF))
+MAXR = math.sqrt(2.25 * M * G / (4 * KF))
+
+
+def test_normalized_rpm_map_endpoints_and_linearity():
+    """PAPER.md:300 (normalizedActionToRPM), reading Q35: -1 -> 0, 0 -> HOVER_RPM, +1 -> MAX_RPM, piecewise linear, clipped."""
+    env, _ = make_env(action=W.ACT_RPM_NORM, **FREE)
+    for a, want in [(-1.0, 0.0), (0.0, HOVER), (1.0, MAXR), (-0.5, 0.5 * HOVER), (0.25, HOVER + 0.25 * (MAXR - HOVER)),
+                    (-7.0, 0.0), (3.0, MAXR)]:
+        rpm = env.probe_decode(np.array([a, a, a, a], dtype=np.float32))
+        assert np.allclose(rpm, want, rtol=1e-12, atol=1e-9), (a, rpm, want)
+    rpm = env.probe_decode(np.array([-1.0, 0.0, 0.5, 1.0], dtype=np.float32))          # the four rotors are independent
+    assert np.allclose(rpm[0], [0.0, HOVER, HOVER + 0.5 * (MAXR - HOVER), MAXR], rtol=1e-12)
+
+
+def test_one_d_rpm_drives_all_rotors_from_the_first_component():
+    env, _ = make_env(action=W.ACT_ONE_D_RPM, **FREE)
+    rpm = env.probe_decode(np.array([0.5, -1.0, 1.0, 0.123], dtype=np.float32))
+    assert np.allclose(rpm, HOVER + 0.5 * (MAXR - HOVER), rtol=1e-12)
+    # a = 0 is hover: stationary to rounding; a > 0 is the uniform-thrust closed form z'' = 4 k_f n^2 / m - g
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    s0 = env.state.copy()
+    for _ in range(48):
+        env.step(np.zeros((1, 4), dtype=np.float32))
+    assert np.abs(env.state - s0).max() < 1e-12
+    n = HOVER + float(np.float32(0.2)) * (MAXR - HOVER)                 # the action is an fp32 number
+    acc = 4 * KF * n * n / M - G
+    for _ in range(48):
+        env.step(np.array([[0.2, 9, 9, 9]], dtype=np.float32))
+    t = 1.0
+    assert abs(env.state[0, 2] - (1.0 + 0.5 * acc * t * t)) < 1e-9 and abs(env.state[0, 9] - acc * t) < 1e-9
+
+
+def test_attitude_action_thrust_channel_targets_and_yaw_rate():
+    """Reading Q36: [thrust (normalised map, T = 4 k_f rpm^2), roll*, pitch*, yaw rate] through the attitude loop + mixer."""
+    env, P = make_env(action=W.ACT_ATTITUDE, **FREE)
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    # level, zero targets, thrust 0 -> every rotor at HOVER_RPM (no torque demanded)
+    assert np.allclose(env.probe_decode(np.array([0, 0, 0, 0], dtype=np.float32)), HOVER, rtol=1e-12)
+    # roll target 0.1 rad from level: tau_x = Kp * 0.1 + Ki * (0.1 dt) (Table 6: 2e-3, 0), split over the X mixer
+    rpm = env.probe_decode(np.array([0, 0.1, 0, 0], dtype=np.float32))[0]
+    s = KF * rpm ** 2
+    l = L / math.sqrt(2)
+    assert abs(l * (s[0] + s[1] - s[2] - s[3]) - 2e-3 * float(np.float32(0.1))) < 1e-12
+    assert abs(s.sum() - M * G) < 1e-12 and abs(-s[0] + s[1] - s[2] + s[3]) < 1e-15
+    # targets are clipped to +-tilt_max (0.5 rad)
+    a = env.probe_decode(np.array([0, 5.0, 0, 0], dtype=np.float32))[0]
+    b = env.probe_decode(np.array([0, 0.5, 0, 0], dtype=np.float32))[0]
+    assert np.allclose(a, b, rtol=1e-14)
+    # yaw rate r: psi* = psi + r dt  ->  tau_z = Kp_z r dt + Ki_z (r dt) dt  (Table 6: 1e-3, 1e-4)
+    r, dt = 1.0, 1 / 48
+    rpm = env.probe_decode(np.array([0, 0, 0, r], dtype=np.float32))[0]
+    s = KF * rpm ** 2
+    assert abs((KM / KF) * (-s[0] + s[1] - s[2] + s[3]) - (1e-3 * r * dt + 1e-4 * r * dt * dt)) < 1e-13
+    # closed loop: hold roll* = 0.2 rad at hover thrust for 1 s -> settles near the target and drifts towards -y
+    for _ in range(48):
+        env.step(np.array([[0, 0.2, 0, 0]], dtype=np.float32))
+    phi = O.euler_zyx(env.state[0, 3:7])[0]
+    assert 0.15 < phi < 0.25 and env.state[0, 8] < -0.5
+
+
+def test_kin20_observation_layout():
+    """KIN = [p, q, eta, v, omega, a_{t-1}] (20 per drone); a_{t-1} is the action of the step that
+    produced the state, zeros after reset."""
+    env, _ = make_env(n_envs=2, n_drones=2, action=W.ACT_RPM, obs_mode=W.OBS_KIN20, **FREE)
+    obs = env.outputs()[0].reshape(2, 2, 20)
+    assert np.all(obs[:, :, 16:20] == 0.0)
+    q = np.array([0.9, 0.1, -0.2, 0.3]); q /= np.linalg.norm(q)
+    set_state(env, p=[0.1, -0.2, 1.3], q=q, v=[0.4, 0.5, -0.6], w=[0.7, -0.8, 0.9])
+    a = (HOVER * np.array([[1.0, 1.01, 0.99, 1.02]] * 4)).astype(np.float32)
+    env.step(a)
+    obs = env.outputs()[0].reshape(2, 2, 20)
+    st = env.state.reshape(2, 2, 13)
+    assert np.array_equal(obs[:, :, 0:3], st[:, :, 0:3]) and np.array_equal(obs[:, :, 3:7], st[:, :, 3:7])
+    assert np.array_equal(obs[:, :, 10:13], st[:, :, 7:10]) and np.array_equal(obs[:, :, 13:16], st[:, :, 10:13])
+    for e in range(2):
+        for i in range(2):
+            assert np.allclose(obs[e, i, 7:10], O.euler_zyx(st[e, i, 3:7]), atol=1e-15)
+    assert np.array_equal(obs[:, :, 16:20].reshape(4, 4), a.astype(np.float64))
+
+
+def test_cf2p_plus_configuration_mixing():
+    """PAPER.md:80, reading Q37: tau_x = L (F_1 - F_3), tau_y = L (F_2 - F_0), yaw as in the X frame; CF2X parameters."""
+    P = O.OracleParams(W.MODEL_CF2P)
+    assert P.get("m") == 0.027 and P.get("L") == 0.0397
+    rng = np.random.default_rng(3)
+    rpm = rng.uniform(0.8, 1.2, 4) * HOVER
+    T, tau, _ = O.motor_wrench(P, rpm)
+    F = KF * rpm ** 2
+    assert abs(T - F.sum()) < 1e-15
+    assert np.allclose(tau, [L * (F[1] - F[3]), L * (F[2] - F[0]), (KM / KF) * (-F[0] + F[1] - F[2] + F[3])], rtol=1e-13, atol=1e-18)
+    # allocation round trip: random wrench -> per-rotor thrusts -> wrench
+    for _ in range(20):
+        T = rng.uniform(0.1, 0.5); tq = rng.uniform(-1, 1, 3) * [1e-3, 1e-3, 1e-4]
+        s = O.alloc_inverse(P, T, tq)
+        T2, tau2, _ = O.motor_wrench(P, np.sqrt(s / KF))
+        assert abs(T2 - T) < 1e-14 and np.allclose(tau2, tq, rtol=1e-11, atol=1e-17)
+    # pure roll torque at hover thrust: omega_x = tau_x t / J_xx exactly (principal axis, torque-free about the others)
+    env, _ = make_env(model=W.MODEL_CF2P, **FREE)
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    s_h = M * G / 4
+    F = np.array([s_h, 1.1 * s_h, s_h, 0.9 * s_h])
+    a = np.sqrt(F / KF).astype(np.float32)[None, :]
+    Fa = KF * a[0].astype(np.float64) ** 2
+    for _ in range(12):
+        env.step(a)
+    t = 12 / 48
+    assert abs(env.state[0, 10] - L * (Fa[1] - Fa[3]) * t / JXX) < 1e-9 * abs(env.state[0, 10])
+    # fp32 rotor speeds leave a tiny yaw torque; it couples into omega_y only through (J_zz - J_xx) omega_z omega_x
+    assert abs(env.state[0, 11]) < 1e-4 and abs(env.state[0, 12] - (KM / KF) * (-Fa[0] + Fa[1] - Fa[2] + Fa[3]) * t / JZZ) < 2e-8   # frozen world-frame torque over a substep mixes tau_y, tau_z at 9 rad/s
+    # the PID default torque clamp follows the same "a third of the hover rotor thrust per axis" rule (Q17/Q37)
+    assert abs(P.get("tau_xy_max") - 2 * L * s_h / 3) < 1e-15
