@@ -36,7 +36,7 @@ def algorithmic_bytes_per_drone(c: int) -> float:
     """State read once + written once, actions read, outputs written."""
     wl = W.config(c)
     M = wl.n_drones
-    pid = wl.action_type != W.ACT_RPM
+    pid = wl.action_type in (W.ACT_PID, W.ACT_VEL, W.ACT_ATTITUDE)       # actions with an attitude loop read/write P4
     rd = 4 * 16 + 16 + 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)   # P0-P3, target, action, P4, P5
     wr = 4 * 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)
     obs = 4 * (12 + (M if wl.params.get("obs_mode", 0) == W.OBS_KIN12_ADJ else 0))

@@ -67,7 +67,8 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     if (integ == MDG_INTEG_EULER) f |= F_EULER;
     f |= action_type << F_ACT_SHIFT;
     if (action_type == MDG_ACT_PID && p.dsl) f |= F_DSL;
-    if (p.obs_mode == MDG_OBS_KIN12_ADJ) f |= F_ADJ;
+    f |= p.obs_mode << F_OBS_SHIFT;
+    if (p.drone_model == MDG_MODEL_CF2P) f |= F_CF2P;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
     if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
@@ -87,7 +88,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.auto_reset = p.auto_reset; D.feat = feat; D.env_base = p.env_index_base;
     D.reset_layout = p.reset_layout; D.target_mode = p.target_mode;
     D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
-    D.opd = 12 + ((feat & F_ADJ) ? M : 0);
+    D.opd = (feat & F_KIN20) ? 20 : 12 + ((feat & F_ADJ) ? M : 0);
     D.h = (float)h; D.half_h = (float)(0.5 * h); D.h_sixth = (float)(h / 6.0); D.half_h2 = (float)(0.5 * h * h);
     D.w2_exact = (float)((0.75 / h) * (0.75 / h));
     for (int s = 0; s < 2; ++s) {                                  // Rodrigues series of R(c w)^T in y = |w|^2
@@ -111,6 +112,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.inv_l = (float)(1.0 / l); D.inv_kappa = (float)(1.0 / kappa);
     D.max_rpm = (float)max_rpm; D.s_max = (float)(p.k_f * max_rpm * max_rpm); D.T_max = (float)(4.0 * p.k_f * max_rpm * max_rpm);
     D.rpm2rad = (float)(2.0 * M_PI / 60.0);
+    D.hover_rpm = (float)std::sqrt(hover2); D.rpm_span = (float)(max_rpm - std::sqrt(hover2));
+    D.arm = p.L; D.inv_arm = (float)(1.0 / p.L);
     D.gnd_coef = (float)((double)p.C_gnd * (p.r_p / 4.0) * (p.r_p / 4.0)); D.h_clip = p.h_clip;
     D.c_xy = p.c_xy; D.c_z = p.c_z;
     D.dw_coef = (float)((double)p.dw_C1 * (p.r_p / 4.0) * (p.r_p / 4.0)); D.dw_C2 = p.dw_C2; D.dw_C3 = p.dw_C3;
@@ -235,8 +238,8 @@ const char* mdg_last_error(void) { return g_err.c_str(); }
 
 int mdg_default_params(int drone_model, mdg_params* p) {
     if (!p) return fail(MDG_EINVAL, "mdg_default_params: out is NULL");
-    if (drone_model != MDG_MODEL_CF2X && drone_model != MDG_MODEL_RACE)
-        return fail(MDG_EINVAL, "mdg_default_params: unknown drone model (CF2P mixing is not built yet)");
+    if (drone_model != MDG_MODEL_CF2X && drone_model != MDG_MODEL_CF2P && drone_model != MDG_MODEL_RACE)
+        return fail(MDG_EINVAL, "mdg_default_params: unknown drone model");
     std::memset(p, 0, sizeof(*p));
     p->struct_size = (uint32_t)sizeof(mdg_params);
     p->drone_model = drone_model;
@@ -264,6 +267,7 @@ int mdg_default_params(int drone_model, mdg_params* p) {
     p->pos_rate_limit = 2.0f; p->yaw_rate_limit = (float)M_PI; p->tilt_max = 0.5f;
     const double s_hover = (double)p->m * p->g / 4.0;
     p->tau_xy_max = (float)(4.0 * (p->L / std::sqrt(2.0)) * s_hover / 3.0);
+    if (drone_model == MDG_MODEL_CF2P) p->tau_xy_max = (float)(2.0 * p->L * s_hover / 3.0);   // two rotors per axis, same rule
     p->tau_z_max = (float)(4.0 * ((double)p->k_m / p->k_f) * s_hover / 3.0);
     p->obs_mode = MDG_OBS_KIN12; p->adj_radius = 0.5f;
     p->reward_mode = MDG_REW_HOVER; p->at_target_radius = 0.05f;
@@ -290,10 +294,10 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (n_envs < 1 || n_drones < 1 || n_drones > 32) return fail(MDG_EINVAL, "mdg_create: need n_envs >= 1 and 1 <= n_drones <= 32");
     if ((int64_t)n_envs * 32 > (int64_t)1 << 31) return fail(MDG_EINVAL, "mdg_create: n_envs too large");
     if (physics_mode < 0 || physics_mode > MDG_PHYS_DYN) return fail(MDG_EINVAL, "mdg_create: unknown physics_mode");
-    if (action_type < 0 || action_type > MDG_ACT_VEL) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
+    if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 1 || p.reward_mode < 0 || p.reward_mode > 3 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 2 || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 3 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 3 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))

@@ -10,14 +10,17 @@ namespace mdg {
 enum : int {
     F_GND = 1, F_DRAG = 2, F_DW = 4, F_WIND = 8,          // == MDG_AERO_*
     F_EULER = 16,                                         // DYN integrator (Table 1)
-    F_ACT_SHIFT = 5,                                      // 2 bits: MDG_ACT_*
-    F_DSL = 128,
-    F_ADJ = 256,                                          // MDG_OBS_KIN12_ADJ
-    F_REW_SHIFT = 9,                                      // 2 bits: MDG_REW_*
-    F_TERM_SHIFT = 11,                                    // 2 bits: MDG_TERM_*
-    F_TGT_CIRCLE = 1 << 13,                               // targets are the formation circle slots (chord table)
-    F_AXISYM = 1 << 15,                                   // J_xx == J_yy: no gyroscopic term about body z
-    F_FULL = 1 << 14,                                     // n_drones == G: no padding lanes in a group
+    F_ACT_SHIFT = 5,                                      // 3 bits: MDG_ACT_*
+    F_DSL = 1 << 8,
+    F_OBS_SHIFT = 9,                                      // 2 bits: MDG_OBS_*
+    F_ADJ = 1 << F_OBS_SHIFT,                             // MDG_OBS_KIN12_ADJ
+    F_KIN20 = 2 << F_OBS_SHIFT,                           // MDG_OBS_KIN20
+    F_REW_SHIFT = 11,                                     // 2 bits: MDG_REW_*
+    F_TERM_SHIFT = 13,                                    // 2 bits: MDG_TERM_*
+    F_TGT_CIRCLE = 1 << 15,                               // targets are the formation circle slots (chord table)
+    F_FULL = 1 << 16,                                     // n_drones == G: no padding lanes in a group
+    F_AXISYM = 1 << 17,                                   // J_xx == J_yy: no gyroscopic term about body z
+    F_CF2P = 1 << 18,                                     // +-configuration mixing
 };
 
 // Everything the kernels need, precomputed on the host in double and rounded once to fp32.
@@ -37,6 +40,7 @@ struct DevParams {
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
     // motor model (Eq.1-3)
     float k_f, inv_k_f, l, kappa, inv_l, inv_kappa, max_rpm, s_max, T_max, rpm2rad;
+    float hover_rpm, rpm_span, arm, inv_arm;              // normalised-RPM map (HOVER, MAX - HOVER); arm length L for CF2P
     // aero (Eq.4-6) and wind
     float gnd_coef, h_clip, c_xy, c_z, dw_coef, dw_C2, dw_C3, dz_clip, inv_dz_clip;
     float dw_C2s, dw_C3s, dw_b2_min, dz_floor;            // Eq.6 with beta scaled by sqrt(2 ln 2): exp(-x/2b^2) = 2^(-x/b'^2)

@@ -86,7 +86,7 @@ __device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffe
     cp_async16(&S.plane[1][lane], B.P1 + drone);
     cp_async16(&S.plane[2][lane], B.P2 + drone);
     cp_async16(&S.plane[3][lane], B.P3 + drone);
-    if (act != 0) cp_async16(&S.plane[4][lane], B.P4 + drone);
+    if (act == 1 || act == 2 || act == 5) cp_async16(&S.plane[4][lane], B.P4 + drone);   // actions with an attitude loop
     if (act == 1) cp_async16(&S.plane[5][lane], B.P5 + drone);
     cp_async16(&S.plane[6][lane], B.P6 + drone);
     cp_async16(&S.plane[7][lane], actions + drone);
@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const int j = lane % G;
     const bool full_group = F::has(P, F_FULL);
     const int jj = (full_group || j < P.M) ? j : P.M - 1;
-    const bool pid = F::act(P) != 0;
+    const bool pid = F::act(P) == 1 || F::act(P) == 2 || F::act(P) == 5;   // actions with an attitude loop (I_eta in P4)
     // Programmatic dependent launch.  P.chain == 0: wait here until the previous kernel of the stream has completed
     // and its writes are visible (nothing above touches memory).  P.chain == 1 (the previous operation on this
     // handle was step number P.seq - 1, launched on the same stream): no grid-wide wait at all; the dependency is
@@ -235,7 +235,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     decode_action<FEAT>(P, act4, d, n);
     const float f0 = P.k_f * (n[0] * n[0]), f1 = P.k_f * (n[1] * n[1]), f2 = P.k_f * (n[2] * n[2]), f3 = P.k_f * (n[3] * n[3]);
     const float T = (f0 + f1) + (f2 + f3);
-    const V3 tau_b = v3(P.l * ((f0 + f1) - (f2 + f3)), P.l * ((f1 + f2) - (f0 + f3)), P.kappa * ((f1 + f3) - (f0 + f2)));
+    const V3 tau_b = F::has(P, F_CF2P) ? v3(P.arm * (f1 - f3), P.arm * (f2 - f0), P.kappa * ((f1 + f3) - (f0 + f2)))
+                                       : v3(P.l * ((f0 + f1) - (f2 + f3)), P.l * ((f1 + f2) - (f0 + f3)), P.kappa * ((f1 + f3) - (f0 + f2)));
     const float Om = P.rpm2rad * ((n[0] + n[1]) + (n[2] + n[3]));
     const V3 k1_tau = v3(P.invJ[0] * tau_b.x, P.invJ[1] * tau_b.y, P.invJ[2] * tau_b.z);
     const float cxy = -P.c_xy * Om, cz = -P.c_z * Om, gndT = P.gnd_coef * T;
@@ -403,7 +404,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
             if (F::act(P) == 1) B.P5[drone] = d.sp;
         }
-        write_obs<G>(P, B.obs, drone, d, eta, adj, F::has(P, F_ADJ));
+        write_obs<G>(P, B.obs, drone, d, eta, adj, F::has(P, F_ADJ), F::has(P, F_KIN20), do_reset ? make_float4(0, 0, 0, 0) : act4);
         if (j == 0) {
             env4.w = __uint_as_float(ep_out);
             B.E0[e] = env4; B.gstep[e] = t;
@@ -441,7 +442,7 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     if (!active) return;
     store_state(B, drone, d);
     B.P4[drone] = make_float4(0, 0, 0, 0); B.P5[drone] = d.sp; B.P6[drone] = tg;
-    write_obs<G>(P, B.obs, drone, d, v3(0, 0, 0), adj, with_adj);
+    write_obs<G>(P, B.obs, drone, d, v3(0, 0, 0), adj, with_adj, (P.feat & F_KIN20) != 0);
     if (j == 0) { B.E0[e] = make_float4(0, 0, 0, __uint_as_float(0u)); B.gstep[e] = 0u; B.reward[e] = 0.0f; B.done[e] = 0; }
 }
 
@@ -465,7 +466,7 @@ __global__ void refresh_obs_kernel(const __grid_constant__ DevParams P, const De
     const bool with_adj = (P.feat & F_ADJ) != 0;
     if (with_adj) adjacency<G>(P, d.p, lane, j, adj);
     if (!active) return;
-    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, with_adj);
+    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, with_adj, (P.feat & F_KIN20) != 0);
 }
 
 // harness actions (stream 3): base * fma(hi - lo, u, lo), each operation rounded to fp32

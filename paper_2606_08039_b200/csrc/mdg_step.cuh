@@ -12,7 +12,7 @@ namespace mdg {
 template <int FEAT> struct Feat {
     __device__ __forceinline__ static int word(const DevParams& P) { return FEAT >= 0 ? FEAT : P.feat; }
     __device__ __forceinline__ static bool has(const DevParams& P, int bit) { return (word(P) & bit) != 0; }
-    __device__ __forceinline__ static int act(const DevParams& P) { return (word(P) >> F_ACT_SHIFT) & 3; }
+    __device__ __forceinline__ static int act(const DevParams& P) { return (word(P) >> F_ACT_SHIFT) & 7; }
     __device__ __forceinline__ static int rew(const DevParams& P) { return (word(P) >> F_REW_SHIFT) & 3; }
     __device__ __forceinline__ static int term(const DevParams& P) { return (word(P) >> F_TERM_SHIFT) & 3; }
 };
@@ -62,6 +62,12 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
     }
 }
 
+// normalizedActionToRPM: [-1, 1] -> [0, MAX_RPM] through HOVER_RPM at 0, piecewise linear, clipped
+__device__ __forceinline__ float norm_rpm(const DevParams& P, float a) {
+    a = clampf(a, -1.0f, 1.0f);
+    return a > 0.0f ? fmaf(P.rpm_span, a, P.hover_rpm) : fmaf(a, P.hover_rpm, P.hover_rpm);
+}
+
 // Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376)
 template <int FEAT>
 __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, DroneRegs& d, float n[4]) {
@@ -69,6 +75,11 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     if (act == 0) {                       // RPM, clipped
         n[0] = clampf(a.x, 0.0f, P.max_rpm); n[1] = clampf(a.y, 0.0f, P.max_rpm);
         n[2] = clampf(a.z, 0.0f, P.max_rpm); n[3] = clampf(a.w, 0.0f, P.max_rpm);
+        return;
+    }
+    if (act == 3 || act == 4) {           // RPM_NORM / ONE_D_RPM through normalizedActionToRPM (Q35)
+        n[0] = norm_rpm(P, a.x);
+        n[1] = act == 4 ? n[0] : norm_rpm(P, a.y); n[2] = act == 4 ? n[0] : norm_rpm(P, a.z); n[3] = act == 4 ? n[0] : norm_rpm(P, a.w);
         return;
     }
     // roll, pitch and the heading direction (cos psi, sin psi) = normalised (1 - 2(y^2+z^2), 2(wz+xy))
@@ -80,6 +91,14 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     const float hr = hn2 > 1e-30f ? rsqrt_fast(hn2) : 0.0f;
     const float cpsi = hn2 > 1e-30f ? hc * hr : 1.0f, spsi = hs * hr;
     V3 e_p, v_ref; float e_psi;
+    float T, phi_ref, th_ref;
+    if (act == 5) {                       // ATTITUDE [thrust, roll*, pitch*, yaw rate] (Q36): attitude loop + mixer only
+        const float nt = norm_rpm(P, a.x);
+        T = 4.0f * (P.k_f * (nt * nt));
+        phi_ref = clampf(a.y, -P.tilt_max, P.tilt_max);
+        th_ref = clampf(a.z, -P.tilt_max, P.tilt_max);
+        e_psi = wrap_pi(a.w * P.dt_c);
+    } else {
     if (act == 1) {                       // PID waypoint [x, y, z, psi]
         if (Feat<FEAT>::has(P, F_DSL)) {
             const V3 dv = v3(a.x - d.sp.x, a.y - d.sp.y, a.z - d.sp.z);
@@ -105,9 +124,10 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     const float ax = fmaf(P.Kp_pos[0], e_p.x, fmaf(P.Ki_pos[0], d.Ip.x, fmaf(P.Kd_pos[0], v_ref.x - d.v.x, P.a_ff[0])));
     const float ay = fmaf(P.Kp_pos[1], e_p.y, fmaf(P.Ki_pos[1], d.Ip.y, fmaf(P.Kd_pos[1], v_ref.y - d.v.y, P.a_ff[1])));
     const float az = fmaf(P.Kp_pos[2], e_p.z, fmaf(P.Ki_pos[2], d.Ip.z, fmaf(P.Kd_pos[2], v_ref.z - d.v.z, P.a_ff[2]))) + P.g;
-    const float T = clampf(P.m * fast_sqrt(fmaf(ax, ax, fmaf(ay, ay, az * az))), 0.0f, P.T_max);
-    const float phi_ref = clampf((ax * spsi - ay * cpsi) * P.inv_g, -P.tilt_max, P.tilt_max);
-    const float th_ref = clampf((ax * cpsi + ay * spsi) * P.inv_g, -P.tilt_max, P.tilt_max);
+    T = clampf(P.m * fast_sqrt(fmaf(ax, ax, fmaf(ay, ay, az * az))), 0.0f, P.T_max);
+    phi_ref = clampf((ax * spsi - ay * cpsi) * P.inv_g, -P.tilt_max, P.tilt_max);
+    th_ref = clampf((ax * cpsi + ay * spsi) * P.inv_g, -P.tilt_max, P.tilt_max);
+    }
     const V3 e_eta = v3(phi_ref - eta.x, th_ref - eta.y, e_psi);
     d.Ie.x = clampf(fmaf(e_eta.x, P.dt_c, d.Ie.x), -P.int_clamp_att, P.int_clamp_att);
     d.Ie.y = clampf(fmaf(e_eta.y, P.dt_c, d.Ie.y), -P.int_clamp_att, P.int_clamp_att);
@@ -116,9 +136,15 @@ __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, Dron
     const float ty = clampf(fmaf(P.Kp_att[1], e_eta.y, fmaf(P.Ki_att[1], d.Ie.y, -P.Kd_att[1] * d.w.y)), -P.tau_xy_max, P.tau_xy_max);
     const float tz = clampf(fmaf(P.Kp_att[2], e_eta.z, fmaf(P.Ki_att[2], d.Ie.z, -P.Kd_att[2] * d.w.z)), -P.tau_z_max, P.tau_z_max);
     // closed-form allocation inverse, per-rotor clip, back to RPM
-    const float qa = tx * P.inv_l, qb = ty * P.inv_l, qc = tz * P.inv_kappa;
-    const float s0 = 0.25f * (T + qa - qb - qc), s1 = 0.25f * (T + qa + qb + qc);
-    const float s2 = 0.25f * (T - qa + qb - qc), s3 = 0.25f * (T - qa - qb + qc);
+    float s0, s1, s2, s3;
+    if (Feat<FEAT>::has(P, F_CF2P)) {     // +-configuration: tau_x = L (s1 - s3), tau_y = L (s2 - s0)
+        const float qa = 2.0f * tx * P.inv_arm, qb = 2.0f * ty * P.inv_arm, qc = tz * P.inv_kappa;
+        s0 = 0.25f * (T - qb - qc); s1 = 0.25f * (T + qa + qc); s2 = 0.25f * (T + qb - qc); s3 = 0.25f * (T - qa + qc);
+    } else {
+        const float qa = tx * P.inv_l, qb = ty * P.inv_l, qc = tz * P.inv_kappa;
+        s0 = 0.25f * (T + qa - qb - qc); s1 = 0.25f * (T + qa + qb + qc);
+        s2 = 0.25f * (T - qa + qb - qc); s3 = 0.25f * (T - qa - qb + qc);
+    }
     n[0] = fast_sqrt(clampf(s0, 0.0f, P.s_max) * P.inv_k_f); n[1] = fast_sqrt(clampf(s1, 0.0f, P.s_max) * P.inv_k_f);
     n[2] = fast_sqrt(clampf(s2, 0.0f, P.s_max) * P.inv_k_f); n[3] = fast_sqrt(clampf(s3, 0.0f, P.s_max) * P.inv_k_f);
 }
@@ -130,11 +156,21 @@ __device__ __forceinline__ V3 ang_acc(const DevParams& P, V3 tb, V3 w, bool axis
               axisym ? P.invJ[2] * tb.z : fmaf(P.invJ[2], tb.z, -P.gyro[2] * (w.x * w.y)));
 }
 
-// Observation row of one drone: [p, eta, v, w (, adjacency)] written as float4s when the row is 16 B aligned
+// Observation row of one drone: [p, eta, v, w (, adjacency)] or KIN20 [p, q, eta, v, w, a], written as
+// float4s when the row is 16 B aligned
 template <int G>
 __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict__ obs, size_t drone, const DroneRegs& d,
-                                          V3 eta, const float (&adj)[G], bool with_adj) {
+                                          V3 eta, const float (&adj)[G], bool with_adj, bool kin20 = false, float4 act = make_float4(0, 0, 0, 0)) {
     float* o = obs + drone * (size_t)P.opd;
+    if (kin20) {
+        float4* o4 = reinterpret_cast<float4*>(o);                 // 20 floats per drone: always 16 B aligned
+        o4[0] = make_float4(d.p.x, d.p.y, d.p.z, d.q.w);
+        o4[1] = make_float4(d.q.x, d.q.y, d.q.z, eta.x);
+        o4[2] = make_float4(eta.y, eta.z, d.v.x, d.v.y);
+        o4[3] = make_float4(d.v.z, d.w.x, d.w.y, d.w.z);
+        o4[4] = act;
+        return;
+    }
     if ((P.opd & 3) == 0) {
         float4* o4 = reinterpret_cast<float4*>(o);
         o4[0] = make_float4(d.p.x, d.p.y, d.p.z, eta.x);

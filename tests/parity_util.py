@@ -130,11 +130,17 @@ def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=
         # observation (kinematic part follows the state tolerances; adjacency is 0/1 with a threshold)
         ob32 = o32.reshape(N, M, opd)
         ob64 = o64.reshape(N, M, opd)
+        if over.get("obs_mode", 0) == W.OBS_KIN20:                  # [p, q, eta, v, w, a]: q up to sign, a exact
+            assert np.array_equal(ob32[alive][:, :, 16:20], ob64[alive][:, :, 16:20]), ("KIN20 action slot", t)
+            dq = np.minimum(np.abs(ob32[:, :, 3:7] - ob64[:, :, 3:7]).max(axis=2), np.abs(ob32[:, :, 3:7] + ob64[:, :, 3:7]).max(axis=2))
+            assert (dq[alive] <= TOL_Q).all(), ("KIN20 quaternion", t, dq[alive].max())
+            ob32 = np.concatenate([ob32[:, :, 0:3], ob32[:, :, 7:16]], axis=2)
+            ob64 = np.concatenate([ob64[:, :, 0:3], ob64[:, :, 7:16]], axis=2)
         kin = np.abs(ob32[:, :, :12] - ob64[:, :, :12])
         kin[:, :, 3:6] = np.minimum(kin[:, :, 3:6], 2 * np.pi - kin[:, :, 3:6])     # angles wrap
         kin_tol = np.array([TOL_P] * 3 + [2 * TOL_Q * 2] * 3 + [TOL_V] * 3 + [TOL_W] * 3)
         assert (kin[alive] <= kin_tol).all(), ("obs mismatch", t, kin[alive].max(axis=(0, 1)))
-        if opd > 12:
+        if over.get("obs_mode", 0) == W.OBS_KIN12_ADJ:
             badadj = alive & (ob32[:, :, 12:] != ob64[:, :, 12:]).any(axis=(1, 2))
             hard = badadj & (margin[:, 2] >= TIE)
             assert not hard.any(), ("adjacency mismatch", t, np.nonzero(hard)[0][:5])

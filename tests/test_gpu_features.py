@@ -21,6 +21,10 @@ CIRCLE = dict(reset_layout=W.LAYOUT_CIRCLE, circle_radius=0.4, reset_center=[0, 
               term_center=[0, 0, 1], term_dist=3.0, form_center=[0, 0, 1], form_radius=0.4, episode_len_s=30.0, auto_reset=1)
 
 
+SINGLE = dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_HOVER, term_mode=W.TERM_HOVER,
+              target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=10.0, auto_reset=1)
+
+
 def wl(name, n, m, phys, act, params, actions, seed=77):
     return W.Workload(name, n, m, phys, act, params, actions, 48, W.BASE_SEED + seed)
 
@@ -53,6 +57,12 @@ CASES = {
     "m1_no_term_no_reset": (wl("m1free", 900, 1, W.PHYS_MJC_DRAG, W.ACT_RPM,
                                dict(reset_center=[0, 0, 1.5], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_HOVER, term_mode=W.TERM_NONE,
                                     target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=0.25, auto_reset=0), ("hover_scale", 0.7, 1.0)), {}),
+    # normalised / one-dimensional / attitude actions, the 20-dim KIN observation
+    "m1_rpm_norm": (wl("m1norm", 1300, 1, W.PHYS_MJC_DRAG, W.ACT_RPM_NORM, dict(SINGLE), ("uniform", -0.25, 0.3)), {}),
+    "m1_one_d_rpm": (wl("m1oned", 1300, 1, W.PHYS_MJC_GND, W.ACT_ONE_D_RPM, dict(SINGLE), ("uniform", -1.3, 1.3)), {}),
+    "m1_attitude": (wl("m1att", 1300, 1, W.PHYS_MJC, W.ACT_ATTITUDE, dict(SINGLE), ("uniform", -0.3, 0.3)), {}),
+    "m4_attitude_kin20": (wl("m4att", 700, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_ATTITUDE, dict(GRID, grid_cols=2, obs_mode=W.OBS_KIN20), ("uniform", -0.2, 0.2)), {}),
+    "m3_kin20_rpm": (wl("m3kin20", 500, 3, W.PHYS_MJC_DW, W.ACT_RPM, dict(GRID, obs_mode=W.OBS_KIN20), HOVER), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
@@ -101,3 +111,18 @@ def test_error_paths_and_step_many():
     sa, sb = a.get_state(), b.get_state()
     assert np.array_equal(sa["state"], sb["state"]) and np.array_equal(sa["ep_step"], sb["ep_step"])
     assert torch.equal(a.obs, b.obs) and torch.equal(a.reward, b.reward) and torch.equal(a.done, b.done)
+
+
+@pytest.mark.parametrize("act", [W.ACT_RPM, W.ACT_PID, W.ACT_ATTITUDE])
+def test_cf2p_airframe_parity(act):
+    """The +-configuration mixing: rotor wrench for raw RPMs, the mixer inverse under PID and ATTITUDE."""
+    params = dict(SINGLE)
+    actions = HOVER
+    if act == W.ACT_PID:
+        params.update(reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST, term_tilt=0.4, term_dist=3.0,
+                      target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0])
+        actions = ("targets",)
+    elif act == W.ACT_ATTITUDE:
+        actions = ("uniform", -0.3, 0.3)
+    res = run_parity(wl("cf2p", 1100, 1, W.PHYS_MJC_DRAG, act, params, actions), steps=48, model=W.MODEL_CF2P)
+    print(res)
