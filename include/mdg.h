@@ -49,8 +49,10 @@ enum { MDG_PHYS_MJC = 0, MDG_PHYS_MJC_GND = 1, MDG_PHYS_MJC_DRAG = 2, MDG_PHYS_M
 enum { MDG_ACT_RPM = 0, MDG_ACT_PID = 1, MDG_ACT_VEL = 2, MDG_ACT_RPM_NORM = 3, MDG_ACT_ONE_D_RPM = 4, MDG_ACT_ATTITUDE = 5 };
 /* PAPER.md:177, 13.  KIN12 = [p, eta, v, omega]; KIN12_ADJ appends the adjacency row; KIN20 = [p, q, eta, v, omega,
  * a_{t-1}] with a_{t-1} the action applied in the step that produced the state (zeros after a reset). */
-enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1, MDG_OBS_KIN20 = 2 };
-enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3 };
+enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1, MDG_OBS_KIN20 = 2, MDG_OBS_KIN12_TGT = 3 /* KIN12 + the 4 target words */ };
+/* VELOCITY (VelocityAviary): target = (v*, omega_z*), r = -|v - v*| - 0.1 |omega_z - omega_z*| - 0.05 (|phi| + |theta|)
+ * + 0.5 [|v - v*| < at_target_radius] summed over the env's drones */
+enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3, MDG_REW_VELOCITY = 4 };
 enum { MDG_TERM_NONE = 0, MDG_TERM_HOVER = 1, MDG_TERM_TILT_DIST = 2, MDG_TERM_FORMATION = 3 };
 enum { MDG_LAYOUT_NONE = 0, MDG_LAYOUT_GRID = 1, MDG_LAYOUT_CIRCLE = 2 };
 enum { MDG_TGT_FIXED = 0, MDG_TGT_SPAWN_LINSPACE = 1, MDG_TGT_BOX = 2, MDG_TGT_CIRCLE = 3 };
@@ -89,6 +91,8 @@ typedef struct mdg_params {
     /* global index of env 0: Philox counters use env_index_base + e, so a batch split across GPUs
      * draws exactly what the unsplit batch would (no collective on the step path) */
     uint32_t env_index_base;
+    /* MDG_TGT_BOX: range of the 4th target word (VelocityAviary's yaw-rate target; 0, 0 by default) */
+    float target_w_lo, target_w_hi;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

@@ -33,8 +33,8 @@ enum { AERO_GND = 1, AERO_DRAG = 2, AERO_DW = 4, AERO_WIND = 8 };
 enum { INTEG_RK4 = 0, INTEG_EULER = 1 };
 enum { PHYS_MJC = 0, PHYS_MJC_GND = 1, PHYS_MJC_DRAG = 2, PHYS_MJC_DW = 3, PHYS_MJC_GND_DRAG_DW = 4, PHYS_DYN = 5 };
 enum { ACT_RPM = 0, ACT_PID = 1, ACT_VEL = 2, ACT_RPM_NORM = 3, ACT_ONE_D_RPM = 4, ACT_ATTITUDE = 5 };
-enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2 };
-enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3 };
+enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2, OBS_KIN12_TGT = 3 };
+enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3, REW_VELOCITY = 4 };
 enum { TERM_NONE = 0, TERM_HOVER = 1, TERM_TILT_DIST = 2, TERM_FORMATION = 3 };
 enum { LAYOUT_NONE = 0, LAYOUT_GRID = 1, LAYOUT_CIRCLE = 2 };
 enum { TGT_FIXED = 0, TGT_SPAWN_LINSPACE = 1, TGT_BOX = 2, TGT_CIRCLE = 3 };
@@ -69,6 +69,7 @@ struct Params {
         form_center[3], form_radius;
     int env_index_base;              // global index of env 0 (sharding across GPUs)
     int drone_model;                 // MODEL_*: CF2P selects the +-configuration mixing (Q37)
+    double target_w_lo, target_w_hi; // TGT_BOX: range of the 4th target component (VelocityAviary's yaw rate)
 };
 
 inline void default_params(int model, Params& P) {
@@ -485,7 +486,7 @@ struct Sim {
     std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
     std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
 
-    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
+    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : P.obs_mode == OBS_KIN12_TGT ? 16 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
     int obs_dim() const { return M * opd(); }
 
     void init(int n_envs, int n_drones, int phys, int act, const Params& p) {
@@ -532,6 +533,7 @@ struct Sim {
             } else if (P.target_mode == TGT_BOX) {                  // Q32
                 const PhiloxOut r2 = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t, STREAM_RESET_EXTRA, k0, k1);
                 for (int a = 0; a < 3; ++a) tg[a] = P.target_lo[a] + (P.target_hi[a] - P.target_lo[a]) * u01(r2.x[a]);
+                tg[3] = P.target_w_lo + (P.target_w_hi - P.target_w_lo) * u01(r2.x[3]);
             } else {                                                // TGT_CIRCLE, Q26
                 const double ang = 2.0 * PI * i / M;
                 tg[0] = P.form_center[0] + P.form_radius * std::cos(ang);
@@ -583,6 +585,8 @@ struct Sim {
                 continue;
             }
             for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[3 + a] = to_d(eta[a]); oi[6 + a] = to_d(dr[i].v[a]); oi[9 + a] = to_d(dr[i].w[a]); }
+            if (P.obs_mode == OBS_KIN12_TGT)                       // [p, eta, v, omega, v*_x, v*_y, v*_z, omega*_z]
+                for (int a = 0; a < 4; ++a) oi[12 + a] = dr[i].tg[a];
             if (P.obs_mode == OBS_KIN12_ADJ) {
                 for (int k = 0; k < M; ++k) {
                     if (k == i) { oi[12 + k] = 1.0; continue; }
@@ -670,6 +674,13 @@ struct Sim {
                 rew = rew + r;
             } else if (P.reward_mode == REW_NEG_SQ_DIST) {          // config 3
                 rew = rew - (ex * ex + ey * ey + ez * ez);
+            } else if (P.reward_mode == REW_VELOCITY) {             // VelocityAviary, target = (v*, omega_z*), Q38
+                const R ux = d.v[0] - d.tg[0], uy = d.v[1] - d.tg[1], uz = d.v[2] - d.tg[2];
+                const R verr = sqrt(ux * ux + uy * uy + uz * uz);
+                R r = -verr - 0.1 * fabs(d.w[2] - d.tg[3]) - 0.05 * (aphi + ath);
+                if (verr < P.at_target_radius) r = r + 0.5;
+                m_rew = std::fmin(m_rew, std::fabs(to_d(verr) - P.at_target_radius));
+                rew = rew + r;
             } else {                                                // REW_FORMATION (Q26)
                 rew = rew - sqrt(ex * ex + ey * ey + ez * ez);
                 for (int k = i + 1; k < M; ++k) {

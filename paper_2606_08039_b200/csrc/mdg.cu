@@ -88,7 +88,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.auto_reset = p.auto_reset; D.feat = feat; D.env_base = p.env_index_base;
     D.reset_layout = p.reset_layout; D.target_mode = p.target_mode;
     D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
-    D.opd = (feat & F_KIN20) ? 20 : 12 + ((feat & F_ADJ) ? M : 0);
+    const int omode = (feat >> F_OBS_SHIFT) & 3;
+    D.opd = omode == MDG_OBS_KIN20 ? 20 : omode == MDG_OBS_KIN12_TGT ? 16 : 12 + (omode == MDG_OBS_KIN12_ADJ ? M : 0);
     D.h = (float)h; D.half_h = (float)(0.5 * h); D.h_sixth = (float)(h / 6.0); D.half_h2 = (float)(0.5 * h * h);
     D.w2_exact = (float)((0.75 / h) * (0.75 / h));
     for (int s = 0; s < 2; ++s) {                                  // Rodrigues series of R(c w)^T in y = |w|^2
@@ -139,12 +140,13 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.term_tilt = p.term_tilt; D.term_dist2 = (float)((double)p.term_dist * p.term_dist); D.z_max = p.z_max;
     D.reset_z_lo = p.reset_z_lo; D.reset_z_hi = p.reset_z_hi; D.grid_spacing = p.grid_spacing; D.circle_radius = p.circle_radius;
     D.mh_z_lo = p.mh_z_lo; D.mh_z_hi = p.mh_z_hi; D.form_radius = p.form_radius;
+    D.target_w_lo = p.target_w_lo; D.target_w_hi = p.target_w_hi;
     for (int dlt = 0; dlt < 32; ++dlt) D.chord[dlt] = (float)(2.0 * p.form_radius * std::fabs(std::sin(M_PI * dlt / M)));
 }
 
 // ---- kernel dispatch: specialisations for the five benchmark configs, generic otherwise -------------
 #define FEATW(aero, euler, act, dsl, adj, rew, term) \
-    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) ? F_ADJ : 0) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT) | F_FULL | F_AXISYM)
+    ((aero) | ((euler) ? F_EULER : 0) | ((act) << F_ACT_SHIFT) | ((dsl) ? F_DSL : 0) | ((adj) << F_OBS_SHIFT) | ((rew) << F_REW_SHIFT) | ((term) << F_TERM_SHIFT) | F_FULL | F_AXISYM)
 static constexpr int FEAT_C1 = FEATW(0, 0, 0, 0, 0, 0, 1);
 static constexpr int FEAT_C2 = FEATW(3, 0, 0, 0, 0, 0, 1);
 static constexpr int FEAT_C3 = FEATW(0, 0, 1, 1, 0, 1, 2);
@@ -297,7 +299,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 2 || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 3 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 3 || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 4 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 3 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))

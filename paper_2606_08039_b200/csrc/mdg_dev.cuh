@@ -12,15 +12,13 @@ enum : int {
     F_EULER = 16,                                         // DYN integrator (Table 1)
     F_ACT_SHIFT = 5,                                      // 3 bits: MDG_ACT_*
     F_DSL = 1 << 8,
-    F_OBS_SHIFT = 9,                                      // 2 bits: MDG_OBS_*
-    F_ADJ = 1 << F_OBS_SHIFT,                             // MDG_OBS_KIN12_ADJ
-    F_KIN20 = 2 << F_OBS_SHIFT,                           // MDG_OBS_KIN20
-    F_REW_SHIFT = 11,                                     // 2 bits: MDG_REW_*
-    F_TERM_SHIFT = 13,                                    // 2 bits: MDG_TERM_*
-    F_TGT_CIRCLE = 1 << 15,                               // targets are the formation circle slots (chord table)
-    F_FULL = 1 << 16,                                     // n_drones == G: no padding lanes in a group
-    F_AXISYM = 1 << 17,                                   // J_xx == J_yy: no gyroscopic term about body z
-    F_CF2P = 1 << 18,                                     // +-configuration mixing
+    F_OBS_SHIFT = 9,                                      // 2 bits: MDG_OBS_* (compare the field: Feat::obs)
+    F_REW_SHIFT = 11,                                     // 3 bits: MDG_REW_*
+    F_TERM_SHIFT = 14,                                    // 2 bits: MDG_TERM_*
+    F_TGT_CIRCLE = 1 << 16,                               // targets are the formation circle slots (chord table)
+    F_FULL = 1 << 17,                                     // n_drones == G: no padding lanes in a group
+    F_AXISYM = 1 << 18,                                   // J_xx == J_yy: no gyroscopic term about body z
+    F_CF2P = 1 << 19,                                     // +-configuration mixing
 };
 
 // Everything the kernels need, precomputed on the host in double and rounded once to fp32.
@@ -53,7 +51,7 @@ struct DevParams {
     float adj_radius2, at_target_radius2, term_tilt, term_dist2, term_center[3], z_max;   // radii squared
     // reset / targets
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
-    float target_fixed[3], target_lo[3], target_hi[3], mh_z_lo, mh_z_hi, form_center[3], form_radius;
+    float target_fixed[3], target_lo[3], target_hi[3], target_w_lo, target_w_hi, mh_z_lo, mh_z_hi, form_center[3], form_radius;
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 

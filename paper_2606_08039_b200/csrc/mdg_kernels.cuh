@@ -343,6 +343,11 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         if (flags & 2) r -= 100.0f;
     } else if (rew == 1) {
         r = -e2;
+    } else if (rew == 4) {                                         // VelocityAviary: target = (v*, omega_z*)
+        const float ux = d.v.x - tg.x, uy = d.v.y - tg.y, uz = d.v.z - tg.z;
+        const float u2 = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
+        r = -fast_sqrt(u2) - 0.1f * fabsf(d.w.z - tg.w) - 0.05f * (aphi + ath);
+        if (u2 < P.at_target_radius2) r += 0.5f;
     } else {                                                       // formation: pair term below
         r = -fast_sqrt(e2);
     }
@@ -351,7 +356,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
 #pragma unroll
     for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
     const bool pairs = G > 1 && rew == 3;
-    if (pairs || F::has(P, F_ADJ)) {
+    if (pairs || F::obs(P) == 1) {
         float pen = 0.0f;                                          // the self term is |0 - 0| = 0
 #pragma unroll
         for (int kk = 0; kk < G; ++kk) {
@@ -382,15 +387,15 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const int done = (gflags & 1) | (truncated ? 2 : 0);
     uint32_t ep_out = ep;
     const bool do_reset = done != 0 && P.auto_reset != 0;
+    float4 tg_out = tg;
     if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp
         if (do_reset) {
-            float4 tg_out;
             reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
             env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
             eta = v3(0, 0, 0);
             if (active) B.P6[drone] = tg_out;
         }
-        if (F::has(P, F_ADJ)) {                                    // the new episode's first observation
+        if (F::obs(P) == 1) {                                      // the new episode's first observation
             float adj_new[G];
             adjacency<G>(P, d.p, lane, j, adj_new);
 #pragma unroll
@@ -404,7 +409,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
             if (F::act(P) == 1) B.P5[drone] = d.sp;
         }
-        write_obs<G>(P, B.obs, drone, d, eta, adj, F::has(P, F_ADJ), F::has(P, F_KIN20), do_reset ? make_float4(0, 0, 0, 0) : act4);
+        write_obs<G>(P, B.obs, drone, d, eta, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
         if (j == 0) {
             env4.w = __uint_as_float(ep_out);
             B.E0[e] = env4; B.gstep[e] = t;
@@ -437,12 +442,12 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     float adj[G];
 #pragma unroll
     for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
-    const bool with_adj = (P.feat & F_ADJ) != 0;
-    if (with_adj) adjacency<G>(P, d.p, lane, j, adj);
+    const int omode = (P.feat >> F_OBS_SHIFT) & 3;
+    if (omode == 1) adjacency<G>(P, d.p, lane, j, adj);
     if (!active) return;
     store_state(B, drone, d);
     B.P4[drone] = make_float4(0, 0, 0, 0); B.P5[drone] = d.sp; B.P6[drone] = tg;
-    write_obs<G>(P, B.obs, drone, d, v3(0, 0, 0), adj, with_adj, (P.feat & F_KIN20) != 0);
+    write_obs<G>(P, B.obs, drone, d, v3(0, 0, 0), adj, omode, make_float4(0, 0, 0, 0), tg);
     if (j == 0) { B.E0[e] = make_float4(0, 0, 0, __uint_as_float(0u)); B.gstep[e] = 0u; B.reward[e] = 0.0f; B.done[e] = 0; }
 }
 
@@ -463,10 +468,10 @@ __global__ void refresh_obs_kernel(const __grid_constant__ DevParams P, const De
     float adj[G];
 #pragma unroll
     for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
-    const bool with_adj = (P.feat & F_ADJ) != 0;
-    if (with_adj) adjacency<G>(P, d.p, lane, j, adj);
+    const int omode = (P.feat >> F_OBS_SHIFT) & 3;
+    if (omode == 1) adjacency<G>(P, d.p, lane, j, adj);
     if (!active) return;
-    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, with_adj, (P.feat & F_KIN20) != 0);
+    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), B.P6[drone]);
 }
 
 // harness actions (stream 3): base * fma(hi - lo, u, lo), each operation rounded to fp32

@@ -13,7 +13,8 @@ template <int FEAT> struct Feat {
     __device__ __forceinline__ static int word(const DevParams& P) { return FEAT >= 0 ? FEAT : P.feat; }
     __device__ __forceinline__ static bool has(const DevParams& P, int bit) { return (word(P) & bit) != 0; }
     __device__ __forceinline__ static int act(const DevParams& P) { return (word(P) >> F_ACT_SHIFT) & 7; }
-    __device__ __forceinline__ static int rew(const DevParams& P) { return (word(P) >> F_REW_SHIFT) & 3; }
+    __device__ __forceinline__ static int rew(const DevParams& P) { return (word(P) >> F_REW_SHIFT) & 7; }
+    __device__ __forceinline__ static int obs(const DevParams& P) { return (word(P) >> F_OBS_SHIFT) & 3; }   // MDG_OBS_*
     __device__ __forceinline__ static int term(const DevParams& P) { return (word(P) >> F_TERM_SHIFT) & 3; }
 };
 
@@ -54,6 +55,7 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
         tg.x = fmaf(P.target_hi[0] - P.target_lo[0], u01(r2.x), P.target_lo[0]);
         tg.y = fmaf(P.target_hi[1] - P.target_lo[1], u01(r2.y), P.target_lo[1]);
         tg.z = fmaf(P.target_hi[2] - P.target_lo[2], u01(r2.z), P.target_lo[2]);
+        tg.w = fmaf(P.target_w_hi - P.target_w_lo, u01(r2.w), P.target_w_lo);
     } else {                              // CIRCLE slots
         float s, c;
         sincospif(2.0f * (float)j / (float)P.M, &s, &c);
@@ -160,9 +162,10 @@ __device__ __forceinline__ V3 ang_acc(const DevParams& P, V3 tb, V3 w, bool axis
 // float4s when the row is 16 B aligned
 template <int G>
 __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict__ obs, size_t drone, const DroneRegs& d,
-                                          V3 eta, const float (&adj)[G], bool with_adj, bool kin20 = false, float4 act = make_float4(0, 0, 0, 0)) {
+                                          V3 eta, const float (&adj)[G], int mode, float4 act, float4 tg) {
+    const bool with_adj = mode == 1;
     float* o = obs + drone * (size_t)P.opd;
-    if (kin20) {
+    if (mode == 2) {
         float4* o4 = reinterpret_cast<float4*>(o);                 // 20 floats per drone: always 16 B aligned
         o4[0] = make_float4(d.p.x, d.p.y, d.p.z, d.q.w);
         o4[1] = make_float4(d.q.x, d.q.y, d.q.z, eta.x);
@@ -176,6 +179,7 @@ __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict_
         o4[0] = make_float4(d.p.x, d.p.y, d.p.z, eta.x);
         o4[1] = make_float4(eta.y, eta.z, d.v.x, d.v.y);
         o4[2] = make_float4(d.v.z, d.w.x, d.w.y, d.w.z);
+        if (mode == 3) o4[3] = tg;                                 // KIN12_TGT
         if (with_adj) {
             if (G == 4) o4[3] = make_float4(adj[0], adj[1 % G], adj[2 % G], adj[3 % G]);
             else {

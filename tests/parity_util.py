@@ -136,6 +136,8 @@ def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=
             assert (dq[alive] <= TOL_Q).all(), ("KIN20 quaternion", t, dq[alive].max())
             ob32 = np.concatenate([ob32[:, :, 0:3], ob32[:, :, 7:16]], axis=2)
             ob64 = np.concatenate([ob64[:, :, 0:3], ob64[:, :, 7:16]], axis=2)
+        if over.get("obs_mode", 0) == W.OBS_KIN12_TGT:             # the 4 target words are copied, not computed
+            assert np.abs(ob32[alive][:, :, 12:16] - ob64[alive][:, :, 12:16]).max(initial=0) < 1e-6, ("KIN12_TGT target slot", t)
         kin = np.abs(ob32[:, :, :12] - ob64[:, :, :12])
         kin[:, :, 3:6] = np.minimum(kin[:, :, 3:6], 2 * np.pi - kin[:, :, 3:6])     # angles wrap
         kin_tol = np.array([TOL_P] * 3 + [2 * TOL_Q * 2] * 3 + [TOL_V] * 3 + [TOL_W] * 3)

@@ -63,6 +63,15 @@ CASES = {
     "m1_attitude": (wl("m1att", 1300, 1, W.PHYS_MJC, W.ACT_ATTITUDE, dict(SINGLE), ("uniform", -0.3, 0.3)), {}),
     "m4_attitude_kin20": (wl("m4att", 700, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_ATTITUDE, dict(GRID, grid_cols=2, obs_mode=W.OBS_KIN20), ("uniform", -0.2, 0.2)), {}),
     "m3_kin20_rpm": (wl("m3kin20", 500, 3, W.PHYS_MJC_DW, W.ACT_RPM, dict(GRID, obs_mode=W.OBS_KIN20), HOVER), {}),
+    # VelocityAviary: normalised RPM action, 16-dim obs with the target, velocity-tracking reward
+    "m1_velocity_aviary": (wl("m1vel", 1700, 1, W.PHYS_MJC, W.ACT_RPM_NORM,
+                              dict(SINGLE, obs_mode=W.OBS_KIN12_TGT, reward_mode=W.REW_VELOCITY, target_mode=W.TGT_BOX,
+                                   target_lo=[-0.5] * 3, target_hi=[0.5] * 3, target_w_lo=-0.25, target_w_hi=0.25, at_target_radius=0.3,
+                                   episode_len_s=0.5), ("uniform", -0.1, 0.12)), {}),
+    "m2_velocity_vel_action": (wl("m2vel", 900, 2, W.PHYS_MJC_DRAG, W.ACT_VEL,
+                                  dict(GRID, grid_cols=2, obs_mode=W.OBS_KIN12_TGT, reward_mode=W.REW_VELOCITY, target_mode=W.TGT_BOX,
+                                       target_lo=[-0.5] * 3, target_hi=[0.5] * 3, target_w_lo=-0.25, target_w_hi=0.25, at_target_radius=0.3),
+                                  ("uniform", -0.5, 0.5)), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }

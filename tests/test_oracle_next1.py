@@ -123,3 +123,35 @@ def test_cf2p_plus_configuration_mixing():
     assert abs(env.state[0, 11]) < 1e-4 and abs(env.state[0, 12] - (KM / KF) * (-Fa[0] + Fa[1] - Fa[2] + Fa[3]) * t / JZZ) < 2e-8   # frozen world-frame torque over a substep mixes tau_y, tau_z at 9 rad/s
     # the PID default torque clamp follows the same "a third of the hover rotor thrust per axis" rule (Q17/Q37)
     assert abs(P.get("tau_xy_max") - 2 * L * s_h / 3) < 1e-15
+
+
+def test_velocity_aviary_reward_target_and_observation():
+    """PAPER.md:313: obs [p, eta, v, omega, v*, omega_z*] (16), r = -|v - v*| - 0.1 |omega_z - omega_z*| - 0.05 (|phi| + |theta|)
+    + 0.5 [tracked], target ~ U(-0.5, 0.5)^3 x U(-0.25, 0.25) per episode (reading Q38: tracked = |v - v*| < 0.05 m/s)."""
+    from scipy.spatial.transform import Rotation
+    from oracle_util import quat_wxyz_from_scipy
+    over = dict(obs_mode=W.OBS_KIN12_TGT, reward_mode=W.REW_VELOCITY, target_mode=W.TGT_BOX, target_lo=[-0.5] * 3, target_hi=[0.5] * 3,
+                target_w_lo=-0.25, target_w_hi=0.25, physics=W.PHYS_MJC)
+    env, _ = make_env(n_envs=4000, **dict(over, **FREE))
+    tg = env.targets
+    assert np.all(np.abs(tg[:, :3]) <= 0.5) and np.all(np.abs(tg[:, 3]) <= 0.25)
+    assert abs(tg[:, :3].std() - 1 / math.sqrt(12)) < 0.01 and abs(tg[:, 3].std() - 0.5 / math.sqrt(12)) < 0.005
+    assert abs(np.corrcoef(tg[:, 0], tg[:, 3])[0, 1]) < 0.05 and np.abs(tg.mean(axis=0)).max() < 0.02
+    obs = env.outputs()[0].reshape(4000, 16)
+    assert np.array_equal(obs[:, 12:16], tg)
+    # hand-built state: the reward is evaluated on the end-of-step state, so recompute it from that state
+    env, _ = make_env(n_envs=1, **dict(over, **FREE))
+    q = quat_wxyz_from_scipy(Rotation.from_euler("ZYX", [0.3, -0.1, 0.2]))
+    set_state(env, p=[0, 0, 1.0], q=q, v=[0.3, -0.2, 0.1], w=[0.1, 0.2, -0.4])
+    env.targets = np.array([[0.25, -0.1, 0.05, 0.1]])
+    env.step((HOVER * np.ones((1, 4))).astype(np.float32))
+    s = env.state[0]
+    eta = O.euler_zyx(s[3:7])
+    verr = np.linalg.norm(s[7:10] - [0.25, -0.1, 0.05])
+    want = -verr - 0.1 * abs(s[12] - 0.1) - 0.05 * (abs(eta[0]) + abs(eta[1])) + (0.5 if verr < 0.05 else 0.0)
+    assert abs(env.outputs()[1][0] - want) < 1e-13 and verr > 0.05
+    # exactly tracked: level, at the target velocity, gravity cancelled by hover thrust -> -0 + 0.5
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0.25, -0.1, 0.05], w=[0, 0, 0])
+    env.targets = np.array([[0.25, -0.1, 0.05, 0.0]])
+    env.step((HOVER * np.ones((1, 4))).astype(np.float32))
+    assert abs(env.outputs()[1][0] - 0.5) < 1e-6
