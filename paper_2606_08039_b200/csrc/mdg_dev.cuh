@@ -190,8 +190,8 @@ __device__ __forceinline__ V3 stage_torque(const float (&cA)[4], const float (&c
     const V3 c2 = cross(w, c1);
     return v3(fmaf(Bc, c2.x, fmaf(-A, c1.x, tau.x)), fmaf(Bc, c2.y, fmaf(-A, c1.y, tau.y)), fmaf(Bc, c2.z, fmaf(-A, c1.z, tau.z)));
 }
-// sqrt(x) for x >= 0 to ~2 ulp: one MUFU.RSQ and one multiply
-__device__ __forceinline__ float fast_sqrt(float x) { return x > 1e-30f ? x * rsqrt_fast(x) : 0.0f; }
+// sqrt(x) for x >= 0: one MUFU.SQRT (sqrt.approx.ftz, 1 ulp; sqrt(0) = 0)
+__device__ __forceinline__ float fast_sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float clampf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
 __device__ __forceinline__ float wrap_pi(float x) {
     const float k = ceilf((x - 3.14159265358979f) * 0.159154943091895f);

@@ -182,7 +182,9 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     unsigned probed_next = probe(wt_next);
     await_item(wt, probe(wt));
     prefetch_item<G>(P, B, actions, S[0][wib], wt, lane, jj, F::act(P));
-    unsigned pending = 0xFFFFFFFFu;                               // item whose flag is still to be published
+    // Items whose flags are still to be published.  One fence covers two items: the consumer (the next step) reaches
+    // an item a whole step later, so publishing it one item late costs nothing and halves the fences.
+    unsigned pending = 0xFFFFFFFFu, pending2 = 0xFFFFFFFFu;
     int st = 0;
 #pragma unroll 1
     for (;;) {
@@ -243,7 +245,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const float dcz = cz - cxy;
 
     bool hit = false;
-    if (pending != 0xFFFFFFFFu) __threadfence();
+    const bool flush = pending2 != 0xFFFFFFFFu;                  // two items wait: fence now, flags after the substeps
+    if (flush) __threadfence();
     MDG_T(2);
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
@@ -317,7 +320,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     }
 
     MDG_T(3);
-    if (pending != 0xFFFFFFFFu) publish_flag(pending);
+    if (flush) { publish_flag(pending); publish_flag(pending2); pending = pending2 = 0xFFFFFFFFu; }
     const unsigned wt_after = __shfl_sync(MDG_FULL, drawn_l0, 0);
     const unsigned probed_after = probe(wt_after);
     // S9-S11 epilogue on the end-of-step state
@@ -417,12 +420,13 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         }
     }
     MDG_T(5);
-    pending = wt;
+    if (pending == 0xFFFFFFFFu) pending = wt; else pending2 = wt;
     if (wt_next >= n_items) break;
     wt = wt_next; wt_next = wt_after; probed_next = probed_after; st ^= 1;
     }   // work-item loop
     __threadfence();
     publish_flag(pending);
+    if (pending2 != 0xFFFFFFFFu) publish_flag(pending2);
 }
 
 // mdg_reset: initial state of every env at step index 0, first observation, zero reward / done
