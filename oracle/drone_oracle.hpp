@@ -70,7 +70,11 @@ struct Params {
     int env_index_base;              // global index of env 0 (sharding across GPUs)
     int drone_model;                 // MODEL_*: CF2P selects the +-configuration mixing (Q37)
     double target_w_lo, target_w_hi; // TGT_BOX: range of the 4th target component (VelocityAviary's yaw rate)
+    // Domain randomisation (Table 4): half-widths a of the per-episode multiplicative factors
+    // U(1 - a, 1 + a) of [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g]; all 0 = off (reading Q39)
+    double dr_alpha[8];
 };
+enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7 };
 
 inline void default_params(int model, Params& P) {
     std::memset(&P, 0, sizeof(P));
@@ -218,6 +222,7 @@ template <class R> struct Drone {
     R p[3], q[4], v[3], w[3];     // A1 state; w is body-frame (Q22)
     R Ip[3], Ie[3], sp[4];        // PID memory: position / attitude integrals, held setpoint (DSL)
     double tg[4];                 // per-episode target (x, y, z, psi)
+    double sc[8];                 // domain-randomisation factors of this episode (DR_*; all 1 when off)
     double act[4];                // the action row applied in this control step (KIN20's a_{t-1}); zeros after a reset
     R n[4];                       // rotor speeds in RPM, held over the K substeps (Q21)
     R T, tau_b[3], Om;            // O4: collective thrust, body torque, sum of 2 pi n / 60
@@ -229,9 +234,11 @@ template <class R> struct Drone {
 
 // O4 motor model (Eq.1-3; Q3 yaw pattern m=(1,0,1,0))
 template <class R>
-inline void motor_wrench(const Params& P, const Derived& D, const R n[4], R& T, R tau[3], R& Om) {
+inline void motor_wrench(const Params& P, const Derived& D, const R n[4], R& T, R tau[3], R& Om, const double* sc = nullptr) {
+    const double kf = sc ? P.k_f * sc[DR_KF] : P.k_f;             // Table 4: k_f, k_m scaled per episode
+    const double kappa = sc ? (P.k_m * sc[DR_KM]) / kf : D.kappa;
     R s[4];
-    for (int i = 0; i < 4; ++i) s[i] = P.k_f * (n[i] * n[i]);
+    for (int i = 0; i < 4; ++i) s[i] = kf * (n[i] * n[i]);
     T = s[0] + s[1] + s[2] + s[3];
     if (P.drone_model == MODEL_CF2P) {                             // +-configuration (Q37)
         tau[0] = P.L * (s[1] - s[3]);
@@ -240,7 +247,7 @@ inline void motor_wrench(const Params& P, const Derived& D, const R n[4], R& T, 
         tau[0] = D.l * (s[0] + s[1] - s[2] - s[3]);
         tau[1] = D.l * (-s[0] + s[1] + s[2] - s[3]);
     }
-    tau[2] = D.kappa * (-s[0] + s[1] - s[2] + s[3]);
+    tau[2] = kappa * (-s[0] + s[1] - s[2] + s[3]);
     Om = (2.0 * PI / 60.0) * (n[0] + n[1] + n[2] + n[3]);      // Eq.5's rotor-speed sum
 }
 
@@ -374,13 +381,14 @@ inline void substep_wrench(const Params& P, const Derived& D, Drone<R>* dr, int 
             R hgt = d.p[2];
             if (hgt < P.h_clip) hgt = P.h_clip;
             const R ratio = P.r_p / (4.0 * hgt);
-            d.Fw[2] = d.Fw[2] + P.C_gnd * d.T * (ratio * ratio);
+            d.Fw[2] = d.Fw[2] + (P.C_gnd * d.sc[DR_GND]) * d.T * (ratio * ratio);
         }
     }
     if (D.aero & AERO_DRAG) {                      // Eq.5
         R vb[3], fb[3], fw[3];
         matT_vec(Rm, d.v, vb);
-        fb[0] = -(P.c_xy * d.Om) * vb[0]; fb[1] = -(P.c_xy * d.Om) * vb[1]; fb[2] = -(P.c_z * d.Om) * vb[2];
+        const double cxy = P.c_xy * d.sc[DR_DRAG], cz = P.c_z * d.sc[DR_DRAG];
+        fb[0] = -(cxy * d.Om) * vb[0]; fb[1] = -(cxy * d.Om) * vb[1]; fb[2] = -(cz * d.Om) * vb[2];
         mat_vec(Rm, fb, fw);
         for (int a = 0; a < 3; ++a) d.Fw[a] = d.Fw[a] + fw[a];
     }
@@ -399,7 +407,7 @@ inline void substep_wrench(const Params& P, const Derived& D, Drone<R>* dr, int 
                 if (ramp > 1.0) ramp = 1.0;
             }
             const R ratio = P.r_p / (4.0 * dze);
-            const R alpha = P.dw_C1 * (ratio * ratio);
+            const R alpha = (P.dw_C1 * d.sc[DR_DW]) * (ratio * ratio);
             const R beta = P.dw_C2 * dze + P.dw_C3;
             const R b2 = beta * beta;
             R e;
@@ -414,20 +422,21 @@ inline void substep_wrench(const Params& P, const Derived& D, Drone<R>* dr, int 
 
 // angular acceleration f(q, w) = J^-1 (R(q)^T tau_w - w x J w)  (O8, Q11)
 template <class R>
-inline void ang_acc(const Params& P, const R q[4], const R w[3], const R tau_w[3], R out[3]) {
+inline void ang_acc(const Params& P, const R q[4], const R w[3], const R tau_w[3], R out[3], double sJ = 1.0) {
     R Rm[3][3], tb[3], Jw[3], c[3];
     rotmat(q, Rm);
     matT_vec(Rm, tau_w, tb);
-    for (int a = 0; a < 3; ++a) Jw[a] = P.J[a] * w[a];
+    for (int a = 0; a < 3; ++a) Jw[a] = (P.J[a] * sJ) * w[a];
     cross(w, Jw, c);
-    for (int a = 0; a < 3; ++a) out[a] = (tb[a] - c[a]) / P.J[a];
+    for (int a = 0; a < 3; ++a) out[a] = (tb[a] - c[a]) / (P.J[a] * sJ);
 }
 
 // O8: one physics substep with the wrench frozen in the world frame (Table 1)
 template <class R>
 inline void integrate(const Params& P, const Derived& D, Drone<R>& d) {
     const double h = D.h;
-    R a[3] = {d.Fw[0] / P.m, d.Fw[1] / P.m, d.Fw[2] / P.m - P.g};
+    const double m = P.m * d.sc[DR_M], g = P.g * d.sc[DR_G], sJ = d.sc[DR_J];
+    R a[3] = {d.Fw[0] / m, d.Fw[1] / m, d.Fw[2] / m - g};
     if (D.integ == INTEG_RK4) {
         // translation: classical RK4 on (p, v) with constant acceleration reduces exactly to this
         for (int i = 0; i < 3; ++i) {
@@ -436,16 +445,16 @@ inline void integrate(const Params& P, const Derived& D, Drone<R>& d) {
         }
         // rotation: classical RK4 tableau on (q, w_body), stage orientations by Eq.7 from q0
         R k1[3], k2[3], k3[3], k4[3], q2[4], q3[4], q4[4], w2[3], w3[3], w4[3], ph[3];
-        ang_acc(P, d.q, d.w, d.tw, k1);
+        ang_acc(P, d.q, d.w, d.tw, k1, sJ);
         for (int i = 0; i < 3; ++i) { ph[i] = (0.5 * h) * d.w[i]; w2[i] = d.w[i] + (0.5 * h) * k1[i]; }
         quat_exp_step(d.q, ph, q2);
-        ang_acc(P, q2, w2, d.tw, k2);
+        ang_acc(P, q2, w2, d.tw, k2, sJ);
         for (int i = 0; i < 3; ++i) { ph[i] = (0.5 * h) * w2[i]; w3[i] = d.w[i] + (0.5 * h) * k2[i]; }
         quat_exp_step(d.q, ph, q3);
-        ang_acc(P, q3, w3, d.tw, k3);
+        ang_acc(P, q3, w3, d.tw, k3, sJ);
         for (int i = 0; i < 3; ++i) { ph[i] = h * w3[i]; w4[i] = d.w[i] + h * k3[i]; }
         quat_exp_step(d.q, ph, q4);
-        ang_acc(P, q4, w4, d.tw, k4);
+        ang_acc(P, q4, w4, d.tw, k4, sJ);
         for (int i = 0; i < 3; ++i) ph[i] = (h / 6.0) * (d.w[i] + 2.0 * w2[i] + 2.0 * w3[i] + w4[i]);
         R qn[4];
         quat_exp_step(d.q, ph, qn);
@@ -455,7 +464,7 @@ inline void integrate(const Params& P, const Derived& D, Drone<R>& d) {
     } else {                                                       // DYN: explicit Euler (Q12)
         for (int i = 0; i < 3; ++i) { d.v[i] = d.v[i] + h * a[i]; d.p[i] = d.p[i] + h * d.v[i]; }
         R k1[3], ph[3], qn[4];
-        ang_acc(P, d.q, d.w, d.tw, k1);                            // R(q0)^T tau_w = tau_b
+        ang_acc(P, d.q, d.w, d.tw, k1, sJ);                        // R(q0)^T tau_w = tau_b
         for (int i = 0; i < 3; ++i) { d.w[i] = d.w[i] + h * k1[i]; ph[i] = h * d.w[i]; }
         quat_exp_step(d.q, ph, qn);
         for (int i = 0; i < 4; ++i) d.q[i] = qn[i];
@@ -477,6 +486,7 @@ struct Sim {
     Params P; Derived D;
     uint64_t seed; uint32_t gstep;
     std::vector<double> state;    // [D][13] p q v w
+    std::vector<double> drs;      // [D][8] domain-randomisation factors of the running episode (DR_*)
     std::vector<double> pid;      // [D][10] Ip Ie sp
     std::vector<double> target;   // [D][4]
     std::vector<double> wind;     // [N][3]
@@ -493,7 +503,7 @@ struct Sim {
         N = n_envs; M = n_drones; physics_mode = phys; action_type = act; P = p; D = derive(P, phys);
         seed = 0; gstep = 0;
         const size_t Dn = (size_t)N * M;
-        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0);
+        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * 8, 1.0);
         wind.assign((size_t)N * 3, 0.0); ep_step.assign(N, 0);
         obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); done.assign(N, 0);
         margin.assign((size_t)N * 3, 1e30);
@@ -540,6 +550,19 @@ struct Sim {
                 tg[1] = P.form_center[1] + P.form_radius * std::sin(ang);
                 tg[2] = P.form_center[2];
             }
+            // Table 4, Q39: per-episode factors 1 + a (2u - 1); vehicle parameters per drone, g per env
+            bool dr_on = false;
+            for (int a = 0; a < 8; ++a) dr_on = dr_on || P.dr_alpha[a] != 0.0;
+            if (dr_on) {
+                const uint32_t eg = (uint32_t)e + (uint32_t)P.env_index_base;
+                const PhiloxOut d0 = philox4x32_10(eg, (uint32_t)i, t, STREAM_DR0, k0, k1);
+                const PhiloxOut d1 = philox4x32_10(eg, (uint32_t)i, t, STREAM_DR1, k0, k1);
+                const PhiloxOut dg = philox4x32_10(eg, ENV_LEVEL, t, STREAM_DR1, k0, k1);
+                double* sc = &drs[di * 8];
+                for (int a = 0; a < 4; ++a) sc[a] = 1.0 + P.dr_alpha[a] * (2.0 * u01(d0.x[a]) - 1.0);
+                for (int a = 0; a < 3; ++a) sc[4 + a] = 1.0 + P.dr_alpha[4 + a] * (2.0 * u01(d1.x[a]) - 1.0);
+                sc[DR_G] = 1.0 + P.dr_alpha[DR_G] * (2.0 * u01(dg.x[0]) - 1.0);
+            }
             double* pm = &pid[di * 10];
             for (int a = 0; a < 6; ++a) pm[a] = 0.0;
             pm[6] = s[0]; pm[7] = s[1]; pm[8] = s[2]; pm[9] = 0.0;  // held setpoint starts at the spawn pose
@@ -557,6 +580,7 @@ struct Sim {
             for (int a = 0; a < 4; ++a) { d.q[a] = s[3 + a]; d.sp[a] = pm[6 + a]; d.tg[a] = target[di * 4 + a]; }
             for (int a = 0; a < 3; ++a) d.Fwind[a] = 0.0;
             for (int a = 0; a < 4; ++a) d.act[a] = 0.0;
+            for (int a = 0; a < 8; ++a) d.sc[a] = drs[di * 8 + a];
             d.hit = false; d.min_abs_pz = 1e30;
         }
     }
@@ -626,7 +650,7 @@ struct Sim {
         for (int i = 0; i < M; ++i) {
             decode_action(P, D, action_type, actions + ((size_t)e * M + i) * 4, dr[i]);
             for (int a = 0; a < 4; ++a) dr[i].act[a] = (double)actions[((size_t)e * M + i) * 4 + a];
-            motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om);
+            motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
         }
         // K substeps: all wrenches from the same start-of-substep state, then integrate
         for (int k = 0; k < D.K; ++k) {

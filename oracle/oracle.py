@@ -32,7 +32,7 @@ def lib():
         L.orc_step.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.orc_flop_tally.restype = C.c_uint64
         L.orc_flop_tally.argtypes = [C.c_void_p, C.c_void_p]
-        for n in ("state", "pid", "targets", "wind", "ep_step"):
+        for n in ("state", "pid", "targets", "wind", "ep_step", "dr"):
             getattr(L, "orc_get_" + n).argtypes = [C.c_void_p, C.c_void_p]
             getattr(L, "orc_set_" + n).argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_gstep.restype = C.c_uint32
@@ -166,6 +166,14 @@ class OracleEnv:
     @wind.setter
     def wind(self, v):
         self._set("wind", v, (self.N, 3))
+
+    @property
+    def dr(self):               # [N*M, 8] domain-randomisation factors [m, J, k_f, k_m, drag, C_gnd, C_1, g]
+        return self._get("dr", (self.N * self.M, 8))
+
+    @dr.setter
+    def dr(self, v):
+        self._set("dr", v, (self.N * self.M, 8))
 
     @property
     def ep_step(self):

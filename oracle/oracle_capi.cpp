@@ -60,7 +60,7 @@ static const Field FIELDS[] = {
     FD(episode_len_s, 1), FI(auto_reset), FI(reset_layout), FD(reset_center, 3), FD(reset_half, 3),
     FD(reset_z_lo, 1), FD(reset_z_hi, 1), FI(grid_cols), FD(grid_spacing, 1), FD(circle_radius, 1), FI(target_mode),
     FD(target_fixed, 3), FD(target_lo, 3), FD(target_hi, 3), FD(mh_z_lo, 1), FD(mh_z_hi, 1), FD(form_center, 3),
-    FD(form_radius, 1), FI(env_index_base), FI(drone_model), FD(target_w_lo, 1), FD(target_w_hi, 1),
+    FD(form_radius, 1), FI(env_index_base), FI(drone_model), FD(target_w_lo, 1), FD(target_w_hi, 1), FD(dr_alpha, 8),
 };
 static const Field* find_field(const char* name) {
     for (const Field& f : FIELDS) if (std::string(f.name) == name) return &f;
@@ -130,6 +130,8 @@ void orc_get_targets(const void* h, double* out) { std::memcpy(out, ((const Sim*
 void orc_set_targets(void* h, const double* in) { std::memcpy(SIM->target.data(), in, SIM->target.size() * 8); }
 void orc_get_wind(const void* h, double* out) { std::memcpy(out, ((const Sim*)h)->wind.data(), ((const Sim*)h)->wind.size() * 8); }
 void orc_set_wind(void* h, const double* in) { std::memcpy(SIM->wind.data(), in, SIM->wind.size() * 8); }
+void orc_get_dr(const void* h, double* out) { std::memcpy(out, ((const Sim*)h)->drs.data(), ((const Sim*)h)->drs.size() * 8); }
+void orc_set_dr(void* h, const double* in) { std::memcpy(SIM->drs.data(), in, SIM->drs.size() * 8); }
 void orc_get_ep_step(const void* h, uint32_t* out) { std::memcpy(out, ((const Sim*)h)->ep_step.data(), ((const Sim*)h)->ep_step.size() * 4); }
 void orc_set_ep_step(void* h, const uint32_t* in) { std::memcpy(SIM->ep_step.data(), in, SIM->ep_step.size() * 4); }
 uint32_t orc_get_gstep(const void* h) { return ((const Sim*)h)->gstep; }

@@ -155,3 +155,58 @@ def test_velocity_aviary_reward_target_and_observation():
     env.targets = np.array([[0.25, -0.1, 0.05, 0.0]])
     env.step((HOVER * np.ones((1, 4))).astype(np.float32))
     assert abs(env.outputs()[1][0] - 0.5) < 1e-6
+
+
+def test_domain_randomisation_factors_draws_and_physics():
+    """Table 4 (PAPER.md:229-248), reading Q39: per-episode factors U(1 - a, 1 + a) on [m, J, k_f, k_m, drag, C_gnd, C_1, g];
+    each one enters the physics exactly where its nominal constant does, the controller keeps the nominal model."""
+    alpha = [0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02]
+    env, _ = make_env(n_envs=3000, n_drones=2, dr_alpha=alpha, **FREE)
+    f = env.dr
+    for a in range(8):
+        assert np.all(np.abs(f[:, a] - 1.0) <= alpha[a] + 1e-12)
+        assert abs(f[:, a].std() - 2 * alpha[a] / math.sqrt(12)) < 0.04 * alpha[a] and abs(f[:, a].mean() - 1.0) < 0.03 * alpha[a]
+    assert np.abs(np.corrcoef(f[:, :7].T) - np.eye(7)).max() < 0.06          # independent draws
+    g = f[:, 7].reshape(3000, 2)
+    assert np.array_equal(g[:, 0], g[:, 1]) and not np.array_equal(f[0::2, 0], f[1::2, 0])   # g per env, vehicle factors per drone
+    env0, _ = make_env(n_envs=8, n_drones=2, **FREE)
+    assert np.all(env0.dr == 1.0)                                              # off by default
+    # uniform thrust, level: z'' = 4 (k_f s_kf) n^2 / (m s_m) - g s_g
+    env, _ = make_env(**FREE)
+    sc = np.array([[1.15, 0.9, 1.1, 0.93, 1.2, 0.8, 1.25, 1.01]])
+    env.dr = sc
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    n = float(np.float32(HOVER))
+    for _ in range(24):
+        env.step(np.full((1, 4), n, dtype=np.float32))
+    acc = 4 * KF * 1.1 * n * n / (M * 1.15) - G * 1.01
+    assert abs(env.state[0, 9] - acc * 0.5) < 1e-12 and abs(env.state[0, 2] - (1.0 + 0.5 * acc * 0.25)) < 1e-12
+    # pure yaw torque: omega_z = (k_m s_km) sum(+-n^2) t / (J_zz s_J)
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    a = np.array([[0.98, 1.02, 0.98, 1.02]], dtype=np.float32) * np.float32(HOVER)
+    nn = a[0].astype(np.float64) ** 2
+    for _ in range(12):
+        env.step(a)
+    want = KM * 0.93 * (-nn[0] + nn[1] - nn[2] + nn[3]) * 0.25 / (JZZ * 0.9)
+    assert abs(env.state[0, 12] - want) < 1e-10 * abs(want) + 1e-13 and abs(env.state[0, 10]) < 1e-12
+    # ground effect, drag and downwash coefficients scale their forces linearly (probe the substep wrench)
+    envg, _ = make_env(n_drones=2, physics=W.PHYS_MJC_GND_DRAG_DW, **FREE)
+    st = envg.state
+    st[0, 0:3] = [0, 0, 0.1]; st[1, 0:3] = [0.05, 0, 0.6]; st[:, 7:10] = [[0.5, 0, 0], [0, 0, 0]]
+    envg.state = st
+    rpm = np.full((2, 4), HOVER)
+    F0, _ = envg.probe_wrench(0, rpm)
+    d = np.ones((2, 8)); d[0, 4:7] = [1.3, 0.7, 1.2]
+    envg.dr = d
+    F1, _ = envg.probe_wrench(0, rpm)
+    T = M * G
+    gnd = 11.36859 * T * (0.02325 / (4 * 0.1)) ** 2
+    drag_x = -9.1785e-7 * 4 * (2 * math.pi * HOVER / 60) * 0.5
+    dz = 0.5; dw = 2267.18 * (0.02325 / (4 * dz)) ** 2 * math.exp(-0.5 * (0.05 / (0.16 * dz - 0.11)) ** 2)
+    assert abs((F1[0, 0] - F0[0, 0]) - 0.3 * drag_x) < 1e-12
+    assert abs((F1[0, 2] - F0[0, 2]) - (-0.3 * gnd - 0.2 * dw)) < 1e-10
+    # the controller keeps the nominal model: the PID decode of a randomised drone equals the nominal one
+    envp, _ = make_env(action=W.ACT_PID, **FREE)
+    r0 = envp.probe_decode(np.array([0.3, -0.2, 1.4, 0.1], dtype=np.float32))
+    envp.dr = sc
+    assert np.array_equal(envp.probe_decode(np.array([0.3, -0.2, 1.4, 0.1], dtype=np.float32)), r0)
