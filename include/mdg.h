@@ -93,6 +93,10 @@ typedef struct mdg_params {
     uint32_t env_index_base;
     /* MDG_TGT_BOX: range of the 4th target word (VelocityAviary's yaw-rate target; 0, 0 by default) */
     float target_w_lo, target_w_hi;
+    /* Domain randomisation (Table 4): half-widths a of the per-episode factors U(1-a, 1+a) applied to
+     * [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g], redrawn at every reset / auto-reset (vehicle factors per
+     * drone, g per env); all 0 = off.  The PID keeps the nominal model (reading Q39). */
+    float dr_alpha[8];
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */
@@ -144,6 +148,11 @@ int mdg_gen_actions(mdg_env* env, uint64_t seed, uint32_t t, float base, float l
 int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float* wind, uint32_t* ep_step);
 int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
                   const float* wind, const uint32_t* ep_step);
+
+/* Domain-randomisation factors of the running episodes, host [D][8] in the order of mdg_params::dr_alpha (synchronise).
+ * mdg_set_dr fails with MDG_EINVAL when every dr_alpha is 0 (the factors are then not read by the step). */
+int mdg_get_dr(mdg_env* env, float* factors);
+int mdg_set_dr(mdg_env* env, const float* factors);
 
 /* Scheduling note for mdg_step: the step is launched with programmatic dependent launch.  When the previous
  * operation on the handle was a step on the same stream, the new launch does not wait for that kernel as a whole but,

@@ -32,7 +32,7 @@ class mdg_params(C.Structure):
         ("grid_cols", C.c_int32), ("grid_spacing", C.c_float), ("circle_radius", C.c_float),
         ("target_mode", C.c_int32), ("target_fixed", _F3), ("target_lo", _F3), ("target_hi", _F3),
         ("mh_z_lo", C.c_float), ("mh_z_hi", C.c_float), ("form_center", _F3), ("form_radius", C.c_float),
-        ("env_index_base", C.c_uint32), ("target_w_lo", C.c_float), ("target_w_hi", C.c_float),
+        ("env_index_base", C.c_uint32), ("target_w_lo", C.c_float), ("target_w_hi", C.c_float), ("dr_alpha", C.c_float * 8),
     ]
 
     def update(self, d):
@@ -48,7 +48,7 @@ class mdg_params(C.Structure):
 
 EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
-           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_last_error", "mdg_version"]
+           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_last_error", "mdg_version"]
 
 _lib = None
 
@@ -77,6 +77,8 @@ def lib():
         L.mdg_get_state.argtypes = [vp] * 6
         L.mdg_set_state.argtypes = [vp] * 6
         L.mdg_set_stream.argtypes = [vp, vp]
+        L.mdg_get_dr.argtypes = [vp, vp]
+        L.mdg_set_dr.argtypes = [vp, vp]
         L.mdg_launch_count.argtypes = [vp]
         L.mdg_launch_count.restype = C.c_int64
         L.mdg_kernel_name.argtypes = [vp]
@@ -211,6 +213,18 @@ class Env:
         wd, ep = np.zeros((self.n_envs, 3), np.float32), np.zeros(self.n_envs, np.uint32)
         _check(lib().mdg_get_state(self._h, *[C.c_void_p(a.ctypes.data) for a in (st, ct, tg, wd, ep)]))
         return dict(state=st, ctrl=ct, targets=tg, wind=wd, ep_step=ep)
+
+    def get_dr(self):
+        """Domain-randomisation factors of the running episodes, [D, 8] float32 (order of mdg_params.dr_alpha)."""
+        import numpy as np
+        out = np.zeros((self.n_envs * self.n_drones, 8), dtype=np.float32)
+        _check(lib().mdg_get_dr(self._h, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def set_dr(self, factors):
+        import numpy as np
+        a = np.ascontiguousarray(factors, dtype=np.float32).reshape(self.n_envs * self.n_drones, 8)
+        _check(lib().mdg_set_dr(self._h, a.ctypes.data_as(C.c_void_p)))
 
     def set_state(self, state=None, ctrl=None, targets=None, wind=None, ep_step=None):
         import numpy as np

@@ -19,6 +19,7 @@ enum : int {
     F_FULL = 1 << 17,                                     // n_drones == G: no padding lanes in a group
     F_AXISYM = 1 << 18,                                   // J_xx == J_yy: no gyroscopic term about body z
     F_CF2P = 1 << 19,                                     // +-configuration mixing
+    F_DR = 1 << 20,                                       // per-episode domain-randomisation factors (Table 4)
 };
 
 // Everything the kernels need, precomputed on the host in double and rounded once to fp32.
@@ -52,6 +53,7 @@ struct DevParams {
     // reset / targets
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
     float target_fixed[3], target_lo[3], target_hi[3], target_w_lo, target_w_hi, mh_z_lo, mh_z_hi, form_center[3], form_radius;
+    float dr_alpha[8];                                    // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g]
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 
@@ -64,6 +66,8 @@ struct DevBuffers {
     float4* P4;   // Iex Iey Iez -
     float4* P5;   // held setpoint x y z psi
     float4* P6;   // target x y z psi
+    float4* R0;   // DR factors m J k_f k_m
+    float4* R1;   // DR factors drag gnd dw g
     float4* E0;   // wind x y z, bits(ep_step)
     uint32_t* gstep;
     unsigned* ticket;   // two work-item dispensers of the step kernel (0 between launches), used alternately
@@ -73,7 +77,7 @@ struct DevBuffers {
     uint8_t* done;
 };
 
-static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3;
+static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5;
 
 // Philox4x32-10 (Salmon et al., SC'11).  key = seed halves, counter = (env, drone|~0, step, stream).
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,

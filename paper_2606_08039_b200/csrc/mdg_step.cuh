@@ -70,6 +70,16 @@ __device__ __forceinline__ float norm_rpm(const DevParams& P, float a) {
     return a > 0.0f ? fmaf(P.rpm_span, a, P.hover_rpm) : fmaf(a, P.hover_rpm, P.hover_rpm);
 }
 
+// Domain-randomisation factors of a new episode (Table 4; vehicle factors per drone, g per env)
+__device__ __forceinline__ void draw_dr(const DevParams& P, uint32_t e, uint32_t j, uint32_t t, float4& r0, float4& r1) {
+    const uint4 a = philox4x32_10(e + P.env_base, j, t, STREAM_DR0, P.seed_lo, P.seed_hi);
+    const uint4 b = philox4x32_10(e + P.env_base, j, t, STREAM_DR1, P.seed_lo, P.seed_hi);
+    const uint4 g = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_DR1, P.seed_lo, P.seed_hi);
+    auto f = [](float alpha, uint32_t x) { return fmaf(alpha, fmaf(2.0f, u01(x), -1.0f), 1.0f); };
+    r0 = make_float4(f(P.dr_alpha[0], a.x), f(P.dr_alpha[1], a.y), f(P.dr_alpha[2], a.z), f(P.dr_alpha[3], a.w));
+    r1 = make_float4(f(P.dr_alpha[4], b.x), f(P.dr_alpha[5], b.y), f(P.dr_alpha[6], b.z), f(P.dr_alpha[7], g.x));
+}
+
 // Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376)
 template <int FEAT>
 __device__ __forceinline__ void decode_action(const DevParams& P, float4 a, DroneRegs& d, float n[4]) {

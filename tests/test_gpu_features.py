@@ -25,6 +25,9 @@ SINGLE = dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.
               target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=10.0, auto_reset=1)
 
 
+DR = [0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02]                       # Table 4
+
+
 def wl(name, n, m, phys, act, params, actions, seed=77):
     return W.Workload(name, n, m, phys, act, params, actions, 48, W.BASE_SEED + seed)
 
@@ -72,6 +75,13 @@ CASES = {
                                   dict(GRID, grid_cols=2, obs_mode=W.OBS_KIN12_TGT, reward_mode=W.REW_VELOCITY, target_mode=W.TGT_BOX,
                                        target_lo=[-0.5] * 3, target_hi=[0.5] * 3, target_w_lo=-0.25, target_w_hi=0.25, at_target_radius=0.3),
                                   ("uniform", -0.5, 0.5)), {}),
+    # Table 4 domain randomisation: per-episode factors on m, J, k_f, k_m, drag, C_gnd, C_1, g (frequent episodes -> redraws)
+    "m1_domain_randomisation_pid": (wl("m1dr", 1500, 1, W.PHYS_MJC_GND, W.ACT_PID,
+                                       dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST,
+                                            term_tilt=0.4, term_dist=3.0, target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
+                                            episode_len_s=0.25, auto_reset=1, dr_alpha=DR), ("targets",)), {}),
+    "m4_domain_randomisation_all_aero": (wl("m4dr", 800, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
+                                            dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR), HOVER), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
@@ -135,3 +145,28 @@ def test_cf2p_airframe_parity(act):
         actions = ("uniform", -0.3, 0.3)
     res = run_parity(wl("cf2p", 1100, 1, W.PHYS_MJC_DRAG, act, params, actions), steps=48, model=W.MODEL_CF2P)
     print(res)
+
+
+def test_domain_randomisation_factors_match_the_oracle_draws():
+    """The factors themselves (Philox streams 4 and 5) after reset and after auto-resets, and mdg_set_dr / mdg_get_dr."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    from oracle import oracle as O
+    w = wl("drdraw", 700, 3, W.PHYS_MJC, W.ACT_RPM, dict(GRID, episode_len_s=3 / 48, dr_alpha=DR), HOVER)
+    gpu = mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **w.params))
+    orc = O.OracleEnv(w.n_envs, w.n_drones, w.physics_mode, w.action_type, O.OracleParams(0, **w.params), n_threads=4)
+    gpu.reset(w.seed); orc.reset(w.seed)
+    assert np.abs(gpu.get_dr() - orc.dr).max() < 2e-7
+    for t in range(7):                                        # truncation every 3 steps -> two redraws
+        a = O.gen_actions(w.seed, t, w.n_envs, w.n_drones, W.hover_rpm_f32(), 0.9, 1.1)
+        gpu.step(torch.from_numpy(a).cuda()); orc.step(a)
+    f = gpu.get_dr()
+    assert np.abs(f - orc.dr).max() < 2e-7 and f.std() > 0.01
+    f2 = np.ones_like(f); f2[:, 0] = 1.1
+    gpu.set_dr(f2)
+    assert np.array_equal(gpu.get_dr(), f2)
+    plain = mdg.Env(8, 1, W.PHYS_MJC, W.ACT_RPM)
+    assert np.all(plain.get_dr() == 1.0)
+    with pytest.raises(mdg.MdgError):
+        plain.set_dr(np.ones((8, 8), dtype=np.float32))
