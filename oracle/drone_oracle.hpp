@@ -73,7 +73,11 @@ struct Params {
     // Domain randomisation (Table 4): half-widths a of the per-episode multiplicative factors
     // U(1 - a, 1 + a) of [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g]; all 0 = off (reading Q39)
     double dr_alpha[8];
+    // Wind components (reading Q40): WIND_DRYDEN = the AR(1) gust above, WIND_CONSTANT = steady air
+    // velocity wind_const (quadratic drag law), WIND_SINE = the force A [sin wt, cos wt, 0.3 sin 2wt] of episode time t
+    int wind_mask; double wind_const[3], wind_sine_amp, wind_sine_omega;
 };
+enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7 };
 
 inline void default_params(int model, Params& P) {
@@ -93,6 +97,7 @@ inline void default_params(int model, Params& P) {
     P.dw_dz_clip = 0.1;                                           // Q9
     P.k_wind = 0.5 * 1.225 * 1.0 * 0.01;                          // Q28
     P.wind_sigma = 0.5; P.wind_tau = 1.0;
+    P.wind_mask = WIND_DRYDEN; P.wind_sine_omega = 2.0 * PI * 0.5;
     P.sim_freq = 240; P.ctrl_freq = 48;
     P.aero_mask = -1; P.integrator = -1;
     const double kp[3] = {0.4, 0.4, 1.0}, ki[3] = {0.01, 0.01, 0.01}, kd[3] = {0.9, 0.9, 2.0};     // Table 6
@@ -632,18 +637,28 @@ struct Sim {
         const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
         // O9 wind gust (PAPER.md:203 recursion, Q27), once per control step, before the substeps
         if (D.aero & AERO_WIND) {
-            const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, ENV_LEVEL, t, STREAM_WIND, k0, k1);
-            const double ua = u01(r.x[0]), ub = u01(r.x[1]), uc = u01(r.x[2]), ud = u01(r.x[3]);
-            const R r1 = sqrt(-2.0 * log(R(1.0 - ua))), r2 = sqrt(-2.0 * log(R(1.0 - uc)));   // Box-Muller
-            const R xi[3] = {r1 * cos(R(2.0 * PI * ub)), r1 * sin(R(2.0 * PI * ub)), r2 * cos(R(2.0 * PI * ud))};
-            const double alpha = std::exp(-D.dt_c / P.wind_tau);
-            const double gain = P.wind_sigma * std::sqrt(1.0 - alpha * alpha);
-            R w[3];
-            for (int a = 0; a < 3; ++a) { w[a] = alpha * R(wind[(size_t)e * 3 + a]) + gain * xi[a]; wind[(size_t)e * 3 + a] = to_d(w[a]); }
+            R w[3] = {0.0, 0.0, 0.0};                              // air velocity seen by the env's drones
+            if (P.wind_mask & WIND_DRYDEN) {
+                const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, ENV_LEVEL, t, STREAM_WIND, k0, k1);
+                const double ua = u01(r.x[0]), ub = u01(r.x[1]), uc = u01(r.x[2]), ud = u01(r.x[3]);
+                const R r1 = sqrt(-2.0 * log(R(1.0 - ua))), r2 = sqrt(-2.0 * log(R(1.0 - uc)));   // Box-Muller
+                const R xi[3] = {r1 * cos(R(2.0 * PI * ub)), r1 * sin(R(2.0 * PI * ub)), r2 * cos(R(2.0 * PI * ud))};
+                const double alpha = std::exp(-D.dt_c / P.wind_tau);
+                const double gain = P.wind_sigma * std::sqrt(1.0 - alpha * alpha);
+                for (int a = 0; a < 3; ++a) { w[a] = alpha * R(wind[(size_t)e * 3 + a]) + gain * xi[a]; wind[(size_t)e * 3 + a] = to_d(w[a]); }
+            }
+            if (P.wind_mask & WIND_CONSTANT)                       // steady wind, same quadratic drag law
+                for (int a = 0; a < 3; ++a) w[a] = w[a] + P.wind_const[a];
+            R fs[3] = {0.0, 0.0, 0.0};
+            if (P.wind_mask & WIND_SINE) {                         // F(t) = A [sin wt, cos wt, 0.3 sin 2wt]
+                const R ph = P.wind_sine_omega * ((double)ep_step[e] * D.dt_c);   // episode time at the start of the step
+                fs[0] = P.wind_sine_amp * sin(ph); fs[1] = P.wind_sine_amp * cos(ph); fs[2] = (0.3 * P.wind_sine_amp) * sin(2.0 * ph);
+            }
+            const bool drag = (P.wind_mask & (WIND_DRYDEN | WIND_CONSTANT)) != 0;
             for (int i = 0; i < M; ++i) {                          // PAPER.md:201 drag law, Q28
                 R rel[3] = {w[0] - dr[i].v[0], w[1] - dr[i].v[1], w[2] - dr[i].v[2]};
                 const R nr = sqrt(rel[0] * rel[0] + rel[1] * rel[1] + rel[2] * rel[2]);
-                for (int a = 0; a < 3; ++a) dr[i].Fwind[a] = (P.k_wind * nr) * rel[a];
+                for (int a = 0; a < 3; ++a) dr[i].Fwind[a] = (drag ? (P.k_wind * nr) * rel[a] : R(0.0)) + fs[a];
             }
         }
         // O2/O3 decode, O4 motor model

@@ -210,3 +210,44 @@ def test_domain_randomisation_factors_draws_and_physics():
     r0 = envp.probe_decode(np.array([0.3, -0.2, 1.4, 0.1], dtype=np.float32))
     envp.dr = sc
     assert np.array_equal(envp.probe_decode(np.array([0.3, -0.2, 1.4, 0.1], dtype=np.float32)), r0)
+
+
+def test_constant_and_sinusoidal_wind_components():
+    """PAPER.md:200, 204 (reading Q40).  CONSTANT: steady air velocity c through the quadratic drag law, evaluated at the start
+    of each control step and held -> exact recurrence v <- v + dt (k/m) |c - v| (c - v).  SINUSOIDAL: the printed force of
+    episode time, also held over the step."""
+    KW, DT = 0.5 * 1.225 * 0.01, 1 / 48
+    hov = np.full((1, 4), HOVER, dtype=np.float32)
+    res = G - 4 * KF * float(hov[0, 0]) ** 2 / M                     # fp32 hover RPM leaves a tiny vertical residual
+    c = np.array([0.9, -0.4, 0.0])
+    env, _ = make_env(physics=W.PHYS_MJC, aero_mask=W.AERO_WIND, wind_mask=2, wind_const=list(c), **FREE)
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    v = np.zeros(3); p = np.array([0, 0, 1.0])
+    for _ in range(96):
+        env.step(hov)
+        rel = c - v
+        a = KW * np.linalg.norm(rel) * rel / M - np.array([0, 0, res])
+        p = p + DT * v + 0.5 * DT * DT * a
+        v = v + DT * a
+    assert np.abs(env.state[0, 7:10] - v).max() < 1e-12 and np.abs(env.state[0, 0:3] - p).max() < 1e-12
+    assert 0.2 < v[0] < 0.9 and np.all(env.wind == 0.0)               # drifting downwind, no gust state touched
+    # sinusoidal force: v after n steps is the sum of the held accelerations
+    A, om = 0.02, 2 * math.pi * 0.7
+    env, _ = make_env(physics=W.PHYS_MJC, aero_mask=W.AERO_WIND, wind_mask=8, wind_sine_amp=A, wind_sine_omega=om, **FREE)
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    v = np.zeros(3)
+    for k in range(60):
+        env.step(hov)
+        t = k * DT
+        v = v + DT * (A * np.array([math.sin(om * t), math.cos(om * t), 0.3 * math.sin(2 * om * t)]) / M - np.array([0, 0, res]))
+    assert np.abs(env.state[0, 7:10] - v).max() < 1e-12 and abs(v[1]) > 0.01
+    # the components add: DRYDEN + CONSTANT + SINE equals the drag on (gust + c) plus the sine force
+    both, _ = make_env(physics=W.PHYS_MJC, aero_mask=W.AERO_WIND, wind_mask=11, wind_const=list(c), wind_sine_amp=A, wind_sine_omega=om, **FREE)
+    gust, _ = make_env(physics=W.PHYS_MJC, aero_mask=W.AERO_WIND, wind_mask=1, **FREE)
+    for e in (both, gust):
+        set_state(e, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+        e.step(hov)
+    assert np.array_equal(both.wind, gust.wind)                       # same Philox draw, the gust state excludes c
+    u = gust.wind[0] + c
+    want = DT * ((KW * np.linalg.norm(u) * u + A * np.array([0.0, 1.0, 0.0])) / M - np.array([0, 0, res]))
+    assert np.abs(both.state[0, 7:10] - want).max() < 1e-13
