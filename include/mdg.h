@@ -34,6 +34,7 @@ extern "C" {
 /* aerodynamic feature mask ("toggled independently") */
 enum { MDG_AERO_GND = 1, MDG_AERO_DRAG = 2, MDG_AERO_DW = 4, MDG_AERO_WIND = 8 };
 enum { MDG_INTEG_RK4 = 0, MDG_INTEG_EULER = 1 };
+enum { MDG_WIND_DRYDEN = 1, MDG_WIND_CONSTANT = 2, MDG_WIND_SINE = 8 };   /* PAPER.md:199-205; GUST is not built */
 /* Table 1 */
 enum { MDG_PHYS_MJC = 0, MDG_PHYS_MJC_GND = 1, MDG_PHYS_MJC_DRAG = 2, MDG_PHYS_MJC_DW = 3,
        MDG_PHYS_MJC_GND_DRAG_DW = 4, MDG_PHYS_DYN = 5 };
@@ -97,6 +98,10 @@ typedef struct mdg_params {
      * [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g], redrawn at every reset / auto-reset (vehicle factors per
      * drone, g per env); all 0 = off.  The PID keeps the nominal model (reading Q39). */
     float dr_alpha[8];
+    /* Wind components (reading Q40), active when MDG_AERO_WIND is set: MDG_WIND_DRYDEN is the
+     * AR(1) gust above (default), MDG_WIND_CONSTANT adds the steady air velocity wind_const (m/s) under the same quadratic
+     * drag law, MDG_WIND_SINE adds the force wind_sine_amp [sin wt, cos wt, 0.3 sin 2wt] (N) of episode time t. */
+    int32_t wind_mask; float wind_const[3], wind_sine_amp, wind_sine_omega;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

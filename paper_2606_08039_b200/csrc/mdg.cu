@@ -70,6 +70,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     f |= p.obs_mode << F_OBS_SHIFT;
     if (p.drone_model == MDG_MODEL_CF2P) f |= F_CF2P;
     for (int i = 0; i < 8; ++i) if (p.dr_alpha[i] != 0.0f) f |= F_DR;
+    if ((aero & MDG_AERO_WIND) && p.wind_mask != MDG_WIND_DRYDEN) f |= F_WIND_MIX;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
     if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
@@ -125,6 +126,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.dz_floor = p.dw_dz_clip > 1e-6f ? p.dw_dz_clip : 1e-6f;
     const double alpha = std::exp(-dtc / p.wind_tau);
     D.wind_alpha = (float)alpha; D.wind_gain = (float)(p.wind_sigma * std::sqrt(1.0 - alpha * alpha)); D.k_wind = p.k_wind;
+    D.wind_mask = p.wind_mask; D.wind_sine_amp = p.wind_sine_amp; D.wind_sine_omega = p.wind_sine_omega;
+    for (int i = 0; i < 3; ++i) D.wind_const[i] = p.wind_const[i];
     D.dt_c = (float)dtc;
     for (int i = 0; i < 3; ++i) {
         D.Kp_pos[i] = p.Kp_pos[i]; D.Ki_pos[i] = p.Ki_pos[i]; D.Kd_pos[i] = p.Kd_pos[i];
@@ -259,6 +262,7 @@ int mdg_default_params(int drone_model, mdg_params* p) {
     p->h_clip = (float)(0.25 * p->r_p * std::sqrt(15.0 * p->C_gnd / 4.0));
     p->dw_C1 = 2267.18f; p->dw_C2 = 0.16f; p->dw_C3 = -0.11f; p->dw_dz_clip = 0.1f;
     p->k_wind = 0.5f * 1.225f * 1.0f * 0.01f; p->wind_sigma = 0.5f; p->wind_tau = 1.0f;
+    p->wind_mask = MDG_WIND_DRYDEN; p->wind_sine_omega = (float)M_PI;
     p->sim_freq = 240; p->ctrl_freq = 48;
     p->aero_mask = -1; p->integrator = -1;
     const float kp[3] = {0.4f, 0.4f, 1.0f}, ki[3] = {0.01f, 0.01f, 0.01f}, kd[3] = {0.9f, 0.9f, 2.0f};   // Table 6
@@ -301,7 +305,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 3 || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 4 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 3 || (p.wind_mask & ~11) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 4 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 3 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))

@@ -19,6 +19,7 @@ enum : int {
     F_FULL = 1 << 17,                                     // n_drones == G: no padding lanes in a group
     F_AXISYM = 1 << 18,                                   // J_xx == J_yy: no gyroscopic term about body z
     F_CF2P = 1 << 19,                                     // +-configuration mixing
+    F_WIND_MIX = 1 << 21,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
     F_DR = 1 << 20,                                       // per-episode domain-randomisation factors (Table 4)
 };
 
@@ -44,6 +45,7 @@ struct DevParams {
     float gnd_coef, h_clip, c_xy, c_z, dw_coef, dw_C2, dw_C3, dz_clip, inv_dz_clip;
     float dw_C2s, dw_C3s, dw_b2_min, dz_floor;            // Eq.6 with beta scaled by sqrt(2 ln 2): exp(-x/2b^2) = 2^(-x/b'^2)
     float wind_alpha, wind_gain, k_wind;
+    int wind_mask; float wind_const[3], wind_sine_amp, wind_sine_omega;   // MDG_WIND_*: 1 AR(1) gust, 2 constant, 8 sinusoidal force
     // cascaded PID (Eq.9, Table 6)
     float dt_c, m, inv_g;
     float Kp_pos[3], Ki_pos[3], Kd_pos[3], Kp_att[3], Ki_att[3], Kd_att[3];

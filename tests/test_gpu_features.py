@@ -82,6 +82,15 @@ CASES = {
                                             episode_len_s=0.25, auto_reset=1, dr_alpha=DR), ("targets",)), {}),
     "m4_domain_randomisation_all_aero": (wl("m4dr", 800, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
                                             dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR), HOVER), {}),
+    # wind components: constant + gust, sinusoidal alone, all three on a config-5-like setup (must leave the specialisation)
+    "m1_wind_constant_plus_gust": (wl("m1wc", 1300, 1, W.PHYS_MJC, W.ACT_VEL, dict(SINGLE, aero_mask=W.AERO_WIND, wind_mask=3,
+                                      wind_const=[0.9, -0.4, 0.1]), ("uniform", -0.5, 0.5)), {}),
+    "m1_wind_sine": (wl("m1ws", 1300, 1, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(SINGLE, aero_mask=W.AERO_WIND | W.AERO_DRAG, wind_mask=8,
+                        wind_sine_amp=0.02, wind_sine_omega=4.4), ("hover_scale", 0.97, 1.03)), {}),
+    "m4_wind_combined_c5_like": (wl("m4wall", 900, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_VEL,
+                                    dict(CIRCLE, circle_radius=0.3, form_radius=0.3, aero_mask=15, wind_sigma=0.5, wind_tau=1.0, target_mode=W.TGT_CIRCLE,
+                                         wind_mask=11, wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0, int_clamp_pos=1.0,
+                                         int_clamp_att=0.25), ("uniform", -1.0, 1.0)), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
