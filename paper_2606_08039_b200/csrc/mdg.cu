@@ -187,13 +187,12 @@ static void pick_kernels(mdg_env* h) {
 
 // ---- helpers --------------------------------------------------------------------------------------
 static int configure_launch(mdg_env* h) {
-    h->smem = 0;
-    if (h->max_blocks_per_sm > 0) {          // cap residency with a dynamic shared-memory reservation on top of the static part
-        cudaFuncAttributes fa;
-        CU(cudaFuncGetAttributes(&fa, (const void*)h->step));
-        int s = (228 * 1024) / h->max_blocks_per_sm - 1024 - (int)fa.sharedSizeBytes;
+    const int stage_bytes = 2 * (h->block / 32) * (int)sizeof(WarpStage);   // two landing zones per warp
+    h->smem = stage_bytes;
+    if (h->max_blocks_per_sm > 0) {          // cap residency by padding the dynamic shared-memory request
+        int s = (228 * 1024) / h->max_blocks_per_sm - 1024;
         if (s > 227 * 1024) s = 227 * 1024;
-        h->smem = s > 0 ? (s & ~127) : 0;
+        if ((s & ~127) > h->smem) h->smem = s & ~127;
     }
     CU(cudaFuncSetAttribute((const void*)h->step, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem > 48 * 1024 ? h->smem : 48 * 1024));
     if (!h->n_sms) {

@@ -120,7 +120,8 @@ template <int G, int FEAT, int MINB>
 __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__ DevParams P, const DevBuffers B,
                                                          const float4* __restrict__ actions) {
     using F = Feat<FEAT>;
-    __shared__ __align__(16) WarpStage S[2][4];
+    extern __shared__ __align__(16) unsigned char smem_raw[];     // [2 stages][warps per block] WarpStage (host sizes it)
+    WarpStage* const S = reinterpret_cast<WarpStage*>(smem_raw);
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const unsigned wpb = blockDim.x >> 5;
     const unsigned tw = gridDim.x * wpb;                          // persistent warps of this launch
@@ -181,7 +182,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     unsigned wt_next = __shfl_sync(MDG_FULL, draw(true), 0);      // a warp stops drawing after its first miss
     unsigned probed_next = probe(wt_next);
     await_item(wt, probe(wt));
-    prefetch_item<G>(P, B, actions, S[0][wib], wt, lane, jj, F::act(P));
+    prefetch_item<G>(P, B, actions, S[wib], wt, lane, jj, F::act(P));
     // Items whose flags are still to be published.  One fence covers two items: the consumer (the next step) reaches
     // an item a whole step later, so publishing it one item late costs nothing and halves the fences.
     unsigned pending = 0xFFFFFFFFu, pending2 = 0xFFFFFFFFu;
@@ -197,7 +198,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
 
     MDG_T(0);
     cp_async_wait_all();
-    const WarpStage& W = S[st][wib];
+    const WarpStage& W = S[st * wpb + wib];
     DroneRegs d;
     {
         const float4 a = W.plane[0][lane], b = W.plane[1][lane], c = W.plane[2][lane], f = W.plane[3][lane];
@@ -215,7 +216,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const uint32_t t = W.gstep[lane] + 1u;
     float4 dr0 = make_float4(1, 1, 1, 1), dr1 = dr0;             // this episode's DR factors (read-mostly, plain loads)
     if (F::has(P, F_DR)) { dr0 = B.R0[drone]; dr1 = B.R1[drone]; }
-    if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch_item<G>(P, B, actions, S[st ^ 1][wib], wt_next, lane, jj, F::act(P)); }
+    if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch_item<G>(P, B, actions, S[(st ^ 1) * wpb + wib], wt_next, lane, jj, F::act(P)); }
     MDG_T(1);
 
     // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
