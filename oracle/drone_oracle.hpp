@@ -33,11 +33,11 @@ enum { AERO_GND = 1, AERO_DRAG = 2, AERO_DW = 4, AERO_WIND = 8 };
 enum { INTEG_RK4 = 0, INTEG_EULER = 1 };
 enum { PHYS_MJC = 0, PHYS_MJC_GND = 1, PHYS_MJC_DRAG = 2, PHYS_MJC_DW = 3, PHYS_MJC_GND_DRAG_DW = 4, PHYS_DYN = 5 };
 enum { ACT_RPM = 0, ACT_PID = 1, ACT_VEL = 2, ACT_RPM_NORM = 3, ACT_ONE_D_RPM = 4, ACT_ATTITUDE = 5 };
-enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2, OBS_KIN12_TGT = 3 };
-enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3, REW_VELOCITY = 4 };
+enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2, OBS_KIN12_TGT = 3, OBS_KIN12_WP = 4 };
+enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3, REW_VELOCITY = 4, REW_FLY_THROUGH = 5 };
 enum { TERM_NONE = 0, TERM_HOVER = 1, TERM_TILT_DIST = 2, TERM_FORMATION = 3 };
 enum { LAYOUT_NONE = 0, LAYOUT_GRID = 1, LAYOUT_CIRCLE = 2 };
-enum { TGT_FIXED = 0, TGT_SPAWN_LINSPACE = 1, TGT_BOX = 2, TGT_CIRCLE = 3 };
+enum { TGT_FIXED = 0, TGT_SPAWN_LINSPACE = 1, TGT_BOX = 2, TGT_CIRCLE = 3, TGT_WAYPOINTS = 4 };
 enum { MODEL_CF2X = 0, MODEL_CF2P = 1, MODEL_RACE = 2 };
 
 static const double PI = 3.14159265358979323846;
@@ -76,6 +76,8 @@ struct Params {
     // Wind components (reading Q40): WIND_DRYDEN = the AR(1) gust above, WIND_CONSTANT = steady air
     // velocity wind_const (quadratic drag law), WIND_SINE = the force A [sin wt, cos wt, 0.3 sin 2wt] of episode time t
     int wind_mask; double wind_const[3], wind_sine_amp, wind_sine_omega;
+    // FlyThroughAviary (reading Q41): ordered waypoints, capture radius
+    int n_waypoints; double waypoints[24], wp_radius;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7 };
@@ -98,6 +100,9 @@ inline void default_params(int model, Params& P) {
     P.k_wind = 0.5 * 1.225 * 1.0 * 0.01;                          // Q28
     P.wind_sigma = 0.5; P.wind_tau = 1.0;
     P.wind_mask = WIND_DRYDEN; P.wind_sine_omega = 2.0 * PI * 0.5;
+    const double wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5, 0, 1, 1, 0, 0, 0.5};     // PAPER.md:321 default list
+    P.n_waypoints = 5; for (int i = 0; i < 15; ++i) P.waypoints[i] = wps[i];
+    P.wp_radius = 0.1;                                            // Q41
     P.sim_freq = 240; P.ctrl_freq = 48;
     P.aero_mask = -1; P.integrator = -1;
     const double kp[3] = {0.4, 0.4, 1.0}, ki[3] = {0.01, 0.01, 0.01}, kd[3] = {0.9, 0.9, 2.0};     // Table 6
@@ -501,7 +506,7 @@ struct Sim {
     std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
     std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
 
-    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : P.obs_mode == OBS_KIN12_TGT ? 16 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
+    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : P.obs_mode == OBS_KIN12_TGT ? 16 : P.obs_mode == OBS_KIN12_WP ? 18 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
     int obs_dim() const { return M * opd(); }
 
     void init(int n_envs, int n_drones, int phys, int act, const Params& p) {
@@ -549,6 +554,8 @@ struct Sim {
                 const PhiloxOut r2 = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t, STREAM_RESET_EXTRA, k0, k1);
                 for (int a = 0; a < 3; ++a) tg[a] = P.target_lo[a] + (P.target_hi[a] - P.target_lo[a]) * u01(r2.x[a]);
                 tg[3] = P.target_w_lo + (P.target_w_hi - P.target_w_lo) * u01(r2.x[3]);
+            } else if (P.target_mode == TGT_WAYPOINTS) {            // chase waypoint 0 first; tg[3] = its index
+                tg[0] = P.waypoints[0]; tg[1] = P.waypoints[1]; tg[2] = P.waypoints[2];
             } else {                                                // TGT_CIRCLE, Q26
                 const double ang = 2.0 * PI * i / M;
                 tg[0] = P.form_center[0] + P.form_radius * std::cos(ang);
@@ -616,6 +623,12 @@ struct Sim {
             for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[3 + a] = to_d(eta[a]); oi[6 + a] = to_d(dr[i].v[a]); oi[9 + a] = to_d(dr[i].w[a]); }
             if (P.obs_mode == OBS_KIN12_TGT)                       // [p, eta, v, omega, v*_x, v*_y, v*_z, omega*_z]
                 for (int a = 0; a < 4; ++a) oi[12 + a] = dr[i].tg[a];
+            if (P.obs_mode == OBS_KIN12_WP) {                      // next waypoint and its position in the body frame
+                R Rm[3][3], rel[3] = {dr[i].tg[0] - dr[i].p[0], dr[i].tg[1] - dr[i].p[1], dr[i].tg[2] - dr[i].p[2]}, rb[3];
+                rotmat(dr[i].q, Rm);
+                matT_vec(Rm, rel, rb);
+                for (int a = 0; a < 3; ++a) { oi[12 + a] = dr[i].tg[a]; oi[15 + a] = to_d(rb[a]); }
+            }
             if (P.obs_mode == OBS_KIN12_ADJ) {
                 for (int k = 0; k < M; ++k) {
                     if (k == i) { oi[12 + k] = 1.0; continue; }
@@ -719,6 +732,23 @@ struct Sim {
                 R r = -verr - 0.1 * fabs(d.w[2] - d.tg[3]) - 0.05 * (aphi + ath);
                 if (verr < P.at_target_radius) r = r + 0.5;
                 m_rew = std::fmin(m_rew, std::fabs(to_d(verr) - P.at_target_radius));
+                rew = rew + r;
+            } else if (P.reward_mode == REW_FLY_THROUGH) {          // PAPER.md:321, Q41
+                const R dist = sqrt(ex * ex + ey * ey + ez * ez);   // to the waypoint being chased
+                const R wn = sqrt(d.w[0] * d.w[0] + d.w[1] * d.w[1] + d.w[2] * d.w[2]);
+                R r = -0.1 * dist - 0.01 * wn;
+                const double mg = std::fabs(to_d(dist) - P.wp_radius);
+                m_rew = std::fmin(m_rew, mg); m_done = std::fmin(m_done, mg);
+                if (dist < P.wp_radius) {                           // capture: +10, move on; the last one ends the episode
+                    r = r + 10.0;
+                    const int k = (int)dr[i].tg[3] + 1;
+                    if (k >= P.n_waypoints) terminated = true;
+                    else {
+                        double* tgs = &target[((size_t)e * M + i) * 4];
+                        tgs[0] = dr[i].tg[0] = P.waypoints[3 * k]; tgs[1] = dr[i].tg[1] = P.waypoints[3 * k + 1];
+                        tgs[2] = dr[i].tg[2] = P.waypoints[3 * k + 2]; tgs[3] = dr[i].tg[3] = (double)k;
+                    }
+                }
                 rew = rew + r;
             } else {                                                // REW_FORMATION (Q26)
                 rew = rew - sqrt(ex * ex + ey * ey + ez * ez);

@@ -11,14 +11,15 @@ BASE_SEED = 260608039
 
 # interface enum values (include/mdg.h; Table 1, 179-187 Table 3)
 AERO_GND, AERO_DRAG, AERO_DW, AERO_WIND = 1, 2, 4, 8
+WIND_DRYDEN, WIND_CONSTANT, WIND_SINE = 1, 2, 8
 INTEG_RK4, INTEG_EULER = 0, 1
 PHYS_MJC, PHYS_MJC_GND, PHYS_MJC_DRAG, PHYS_MJC_DW, PHYS_MJC_GND_DRAG_DW, PHYS_DYN = range(6)
 ACT_RPM, ACT_PID, ACT_VEL, ACT_RPM_NORM, ACT_ONE_D_RPM, ACT_ATTITUDE = 0, 1, 2, 3, 4, 5
-OBS_KIN12, OBS_KIN12_ADJ, OBS_KIN20, OBS_KIN12_TGT = 0, 1, 2, 3
-REW_HOVER, REW_NEG_SQ_DIST, REW_MULTI_HOVER, REW_FORMATION, REW_VELOCITY = 0, 1, 2, 3, 4
+OBS_KIN12, OBS_KIN12_ADJ, OBS_KIN20, OBS_KIN12_TGT, OBS_KIN12_WP = 0, 1, 2, 3, 4
+REW_HOVER, REW_NEG_SQ_DIST, REW_MULTI_HOVER, REW_FORMATION, REW_VELOCITY, REW_FLY_THROUGH = 0, 1, 2, 3, 4, 5
 TERM_NONE, TERM_HOVER, TERM_TILT_DIST, TERM_FORMATION = 0, 1, 2, 3
 LAYOUT_NONE, LAYOUT_GRID, LAYOUT_CIRCLE = 0, 1, 2
-TGT_FIXED, TGT_SPAWN_LINSPACE, TGT_BOX, TGT_CIRCLE = 0, 1, 2, 3
+TGT_FIXED, TGT_SPAWN_LINSPACE, TGT_BOX, TGT_CIRCLE, TGT_WAYPOINTS = 0, 1, 2, 3, 4
 MODEL_CF2X, MODEL_CF2P, MODEL_RACE = 0, 1, 2
 
 _DSL = dict(dsl=1, int_clamp_pos=1.0, int_clamp_att=0.25)      # halved clamps + rate limits

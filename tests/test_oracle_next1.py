@@ -251,3 +251,48 @@ def test_constant_and_sinusoidal_wind_components():
     u = gust.wind[0] + c
     want = DT * ((KW * np.linalg.norm(u) * u + A * np.array([0.0, 1.0, 0.0])) / M - np.array([0, 0, res]))
     assert np.abs(both.state[0, 7:10] - want).max() < 1e-13
+
+
+def test_fly_through_waypoint_capture_reward_and_observation():
+    """PAPER.md:321 (reading Q41): +10 on capture (distance < 0.1 m), -0.1 |d_wp| shaping, -0.01 |omega| smoothness; the
+    default waypoint list; obs = KIN12 + next waypoint + its position in the body frame; the last capture ends the episode."""
+    from scipy.spatial.transform import Rotation
+    from oracle_util import quat_wxyz_from_scipy
+    WPS = np.array([(0, 0, 1), (1, 0, 1), (1, 1, 1.5), (0, 1, 1), (0, 0, 0.5)], dtype=float)
+    over = dict(obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH, target_mode=W.TGT_WAYPOINTS, term_mode=W.TERM_HOVER,
+                episode_len_s=20.0, auto_reset=0)
+    env, _ = make_env(**over)
+    assert np.array_equal(env.targets[0], [0, 0, 1, 0])
+    hov = np.full((1, 4), HOVER, dtype=np.float32)
+    rot = Rotation.from_euler("ZYX", [0.7, 0.0, 0.0])
+    # far from waypoint 0: shaping and smoothness only, target unchanged
+    set_state(env, p=[0.5, 0.2, 1.3], q=quat_wxyz_from_scipy(rot), v=[0, 0, 0], w=[0.0, 0.0, 0.3])
+    env.step(hov)
+    s = env.state[0]
+    d = np.linalg.norm(WPS[0] - s[0:3])
+    obs, rew, done, _ = env.outputs()
+    assert abs(rew[0] - (-0.1 * d - 0.01 * np.linalg.norm(s[10:13]))) < 1e-13 and done[0] == 0
+    assert np.array_equal(env.targets[0], [0, 0, 1, 0])
+    R = Rotation.from_quat([s[4], s[5], s[6], s[3]])
+    assert np.array_equal(obs[0, 12:15], WPS[0]) and np.allclose(obs[0, 15:18], R.inv().apply(WPS[0] - s[0:3]), atol=1e-14)
+    # inside the capture radius of waypoint 0: +10 and the chase moves to waypoint 1 (obs already shows it)
+    set_state(env, p=[0.03, -0.04, 1.05], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    env.step(hov)
+    s = env.state[0]
+    d = np.linalg.norm(WPS[0] - s[0:3])
+    obs, rew, done, _ = env.outputs()
+    assert d < 0.1 and abs(rew[0] - (10.0 - 0.1 * d)) < 1e-9 and done[0] == 0
+    assert np.array_equal(env.targets[0], [1, 0, 1, 1]) and np.array_equal(obs[0, 12:15], WPS[1])
+    assert np.allclose(obs[0, 15:18], WPS[1] - s[0:3], atol=1e-9)
+    # just outside the radius: no capture
+    set_state(env, p=[1.0, 0.0, 1.0 + 0.1005], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    env.step(hov)
+    assert env.outputs()[1][0] < 0 and np.array_equal(env.targets[0], [1, 0, 1, 1])
+    # walk through the rest: the last capture terminates
+    for k in range(1, 5):
+        set_state(env, p=WPS[k] + [0.01, 0, 0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+        env.step(hov)
+        _, rew, done, _ = env.outputs()
+        assert rew[0] > 9.9 and done[0] == (1 if k == 4 else 0)
+        if k < 4:
+            assert np.array_equal(env.targets[0], list(WPS[k + 1]) + [k + 1])
