@@ -50,13 +50,16 @@ enum { MDG_PHYS_MJC = 0, MDG_PHYS_MJC_GND = 1, MDG_PHYS_MJC_DRAG = 2, MDG_PHYS_M
 enum { MDG_ACT_RPM = 0, MDG_ACT_PID = 1, MDG_ACT_VEL = 2, MDG_ACT_RPM_NORM = 3, MDG_ACT_ONE_D_RPM = 4, MDG_ACT_ATTITUDE = 5 };
 /* PAPER.md:177, 13.  KIN12 = [p, eta, v, omega]; KIN12_ADJ appends the adjacency row; KIN20 = [p, q, eta, v, omega,
  * a_{t-1}] with a_{t-1} the action applied in the step that produced the state (zeros after a reset). */
-enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1, MDG_OBS_KIN20 = 2, MDG_OBS_KIN12_TGT = 3 /* KIN12 + the 4 target words */ };
+enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1, MDG_OBS_KIN20 = 2, MDG_OBS_KIN12_TGT = 3 /* KIN12 + the 4 target words */,
+       MDG_OBS_KIN12_WP = 4 /* KIN12 + next waypoint + its position in the body frame */ };
 /* VELOCITY (VelocityAviary): target = (v*, omega_z*), r = -|v - v*| - 0.1 |omega_z - omega_z*| - 0.05 (|phi| + |theta|)
  * + 0.5 [|v - v*| < at_target_radius] summed over the env's drones */
-enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3, MDG_REW_VELOCITY = 4 };
+enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3, MDG_REW_VELOCITY = 4,
+       MDG_REW_FLY_THROUGH = 5 /* FlyThroughAviary: +10 per captured waypoint, -0.1 |d_wp|, -0.01 |omega|; the last capture terminates */ };
 enum { MDG_TERM_NONE = 0, MDG_TERM_HOVER = 1, MDG_TERM_TILT_DIST = 2, MDG_TERM_FORMATION = 3 };
 enum { MDG_LAYOUT_NONE = 0, MDG_LAYOUT_GRID = 1, MDG_LAYOUT_CIRCLE = 2 };
-enum { MDG_TGT_FIXED = 0, MDG_TGT_SPAWN_LINSPACE = 1, MDG_TGT_BOX = 2, MDG_TGT_CIRCLE = 3 };
+enum { MDG_TGT_FIXED = 0, MDG_TGT_SPAWN_LINSPACE = 1, MDG_TGT_BOX = 2, MDG_TGT_CIRCLE = 3,
+       MDG_TGT_WAYPOINTS = 4 /* target = the waypoint being chased, 4th word = its index */ };
 /* Table 2.  CF2P has CF2X's parameters and the +-configuration mixing:
  * tau_x = L (F_1 - F_3), tau_y = L (-F_0 + F_2) (reading Q37). */
 enum { MDG_MODEL_CF2X = 0, MDG_MODEL_CF2P = 1, MDG_MODEL_RACE = 2 };
@@ -102,6 +105,8 @@ typedef struct mdg_params {
      * AR(1) gust above (default), MDG_WIND_CONSTANT adds the steady air velocity wind_const (m/s) under the same quadratic
      * drag law, MDG_WIND_SINE adds the force wind_sine_amp [sin wt, cos wt, 0.3 sin 2wt] (N) of episode time t. */
     int32_t wind_mask; float wind_const[3], wind_sine_amp, wind_sine_omega;
+    /* FlyThroughAviary: up to 8 ordered waypoints (x, y, z each) and the capture radius (reading Q41: 0.1 m) */
+    int32_t n_waypoints; float waypoints[24], wp_radius;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

@@ -90,8 +90,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.auto_reset = p.auto_reset; D.feat = feat; D.env_base = p.env_index_base;
     D.reset_layout = p.reset_layout; D.target_mode = p.target_mode;
     D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
-    const int omode = (feat >> F_OBS_SHIFT) & 3;
-    D.opd = omode == MDG_OBS_KIN20 ? 20 : omode == MDG_OBS_KIN12_TGT ? 16 : 12 + (omode == MDG_OBS_KIN12_ADJ ? M : 0);
+    const int omode = (feat >> F_OBS_SHIFT) & 7;
+    D.opd = omode == MDG_OBS_KIN20 ? 20 : omode == MDG_OBS_KIN12_TGT ? 16 : omode == MDG_OBS_KIN12_WP ? 18 : 12 + (omode == MDG_OBS_KIN12_ADJ ? M : 0);
     D.h = (float)h; D.half_h = (float)(0.5 * h); D.h_sixth = (float)(h / 6.0); D.half_h2 = (float)(0.5 * h * h);
     D.w2_exact = (float)((0.75 / h) * (0.75 / h));
     for (int s = 0; s < 2; ++s) {                                  // Rodrigues series of R(c w)^T in y = |w|^2
@@ -146,6 +146,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.mh_z_lo = p.mh_z_lo; D.mh_z_hi = p.mh_z_hi; D.form_radius = p.form_radius;
     D.target_w_lo = p.target_w_lo; D.target_w_hi = p.target_w_hi;
     for (int i = 0; i < 8; ++i) D.dr_alpha[i] = p.dr_alpha[i];
+    D.n_waypoints = p.n_waypoints; D.wp_radius2 = (float)((double)p.wp_radius * p.wp_radius);
+    for (int i = 0; i < 24; ++i) D.waypoints[i] = p.waypoints[i];
     for (int dlt = 0; dlt < 32; ++dlt) D.chord[dlt] = (float)(2.0 * p.form_radius * std::fabs(std::sin(M_PI * dlt / M)));
 }
 
@@ -262,6 +264,9 @@ int mdg_default_params(int drone_model, mdg_params* p) {
     p->dw_C1 = 2267.18f; p->dw_C2 = 0.16f; p->dw_C3 = -0.11f; p->dw_dz_clip = 0.1f;
     p->k_wind = 0.5f * 1.225f * 1.0f * 0.01f; p->wind_sigma = 0.5f; p->wind_tau = 1.0f;
     p->wind_mask = MDG_WIND_DRYDEN; p->wind_sine_omega = (float)M_PI;
+    const float wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5f, 0, 1, 1, 0, 0, 0.5f};          // PAPER.md:321 default list
+    p->n_waypoints = 5; for (int i = 0; i < 15; ++i) p->waypoints[i] = wps[i];
+    p->wp_radius = 0.1f;
     p->sim_freq = 240; p->ctrl_freq = 48;
     p->aero_mask = -1; p->integrator = -1;
     const float kp[3] = {0.4f, 0.4f, 1.0f}, ki[3] = {0.01f, 0.01f, 0.01f}, kd[3] = {0.9f, 0.9f, 2.0f};   // Table 6
@@ -304,8 +309,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 3 || (p.wind_mask & ~11) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 4 || p.term_mode < 0 || p.term_mode > 3 ||
-        p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 3 || p.integrator > 1 || p.aero_mask > 15)
+    if (p.obs_mode < 0 || p.obs_mode > 4 || p.n_waypoints < 0 || p.n_waypoints > 8 || (p.wind_mask & ~11) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
+        p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))
         return fail(MDG_EINVAL, "mdg_create: m, g, k_f, k_m, J, wind_tau must be positive");

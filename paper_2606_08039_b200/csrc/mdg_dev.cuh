@@ -12,15 +12,15 @@ enum : int {
     F_EULER = 16,                                         // DYN integrator (Table 1)
     F_ACT_SHIFT = 5,                                      // 3 bits: MDG_ACT_*
     F_DSL = 1 << 8,
-    F_OBS_SHIFT = 9,                                      // 2 bits: MDG_OBS_* (compare the field: Feat::obs)
-    F_REW_SHIFT = 11,                                     // 3 bits: MDG_REW_*
-    F_TERM_SHIFT = 14,                                    // 2 bits: MDG_TERM_*
-    F_TGT_CIRCLE = 1 << 16,                               // targets are the formation circle slots (chord table)
-    F_FULL = 1 << 17,                                     // n_drones == G: no padding lanes in a group
-    F_AXISYM = 1 << 18,                                   // J_xx == J_yy: no gyroscopic term about body z
-    F_CF2P = 1 << 19,                                     // +-configuration mixing
-    F_WIND_MIX = 1 << 21,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
-    F_DR = 1 << 20,                                       // per-episode domain-randomisation factors (Table 4)
+    F_OBS_SHIFT = 9,                                      // 3 bits: MDG_OBS_* (compare the field: Feat::obs)
+    F_REW_SHIFT = 12,                                     // 3 bits: MDG_REW_*
+    F_TERM_SHIFT = 15,                                    // 2 bits: MDG_TERM_*
+    F_TGT_CIRCLE = 1 << 17,                               // targets are the formation circle slots (chord table)
+    F_FULL = 1 << 18,                                     // n_drones == G: no padding lanes in a group
+    F_AXISYM = 1 << 19,                                   // J_xx == J_yy: no gyroscopic term about body z
+    F_CF2P = 1 << 20,                                     // +-configuration mixing
+    F_DR = 1 << 21,                                       // per-episode domain-randomisation factors (Table 4)
+    F_WIND_MIX = 1 << 22,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
 };
 
 // Everything the kernels need, precomputed on the host in double and rounded once to fp32.
@@ -55,6 +55,7 @@ struct DevParams {
     // reset / targets
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
     float target_fixed[3], target_lo[3], target_hi[3], target_w_lo, target_w_hi, mh_z_lo, mh_z_hi, form_center[3], form_radius;
+    int n_waypoints; float waypoints[24], wp_radius2;     // FlyThroughAviary
     float dr_alpha[8];                                    // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g]
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };

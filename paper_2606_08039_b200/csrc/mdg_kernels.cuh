@@ -373,6 +373,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         if (flags & 2) r -= 100.0f;
     } else if (rew == 1) {
         r = -e2;
+    } else if (rew == 5) {                                         // FlyThroughAviary: capture handled below
+        r = fmaf(-0.1f, fast_sqrt(e2), -0.01f * fast_sqrt(fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z))));
     } else if (rew == 4) {                                         // VelocityAviary: target = (v*, omega_z*)
         const float ux = d.v.x - tg.x, uy = d.v.y - tg.y, uz = d.v.z - tg.z;
         const float u2 = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
@@ -409,6 +411,12 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         }
         if (pairs) r = fmaf(-0.25f, pen, r);                       // each unordered pair is seen from both ends
     }
+    bool captured = false, last_wp = false;
+    if (rew == 5) {
+        captured = e2 < P.wp_radius2;
+        last_wp = (int)tg.w + 1 >= P.n_waypoints;
+        if (captured) { r += 10.0f; if (last_wp) flags |= 1; }     // the last capture ends the episode
+    }
     const bool mine = full_group || j < P.M;
     const float rsum = group_sum<G>(mine ? r : 0.0f);
     const int gflags = group_or<G>(mine ? flags : 0);
@@ -418,6 +426,11 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     uint32_t ep_out = ep;
     const bool do_reset = done != 0 && P.auto_reset != 0;
     float4 tg_out = tg;
+    if (rew == 5 && captured && !last_wp) {                        // chase the next waypoint; its index rides in the 4th word
+        const int kn = (int)tg.w + 1;
+        tg_out = make_float4(P.waypoints[3 * kn], P.waypoints[3 * kn + 1], P.waypoints[3 * kn + 2], (float)kn);
+        if (active && !do_reset) B.P6[drone] = tg_out;
+    }
     if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp
         if (do_reset) {
             reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
@@ -478,7 +491,7 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     float adj[G];
 #pragma unroll
     for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
-    const int omode = (P.feat >> F_OBS_SHIFT) & 3;
+    const int omode = (P.feat >> F_OBS_SHIFT) & 7;
     if (omode == 1) adjacency<G>(P, d.p, lane, j, adj);
     if (!active) return;
     store_state(B, drone, d);
@@ -507,7 +520,7 @@ __global__ void refresh_obs_kernel(const __grid_constant__ DevParams P, const De
     float adj[G];
 #pragma unroll
     for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
-    const int omode = (P.feat >> F_OBS_SHIFT) & 3;
+    const int omode = (P.feat >> F_OBS_SHIFT) & 7;
     if (omode == 1) adjacency<G>(P, d.p, lane, j, adj);
     if (!active) return;
     write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), B.P6[drone]);

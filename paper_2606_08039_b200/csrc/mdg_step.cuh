@@ -14,7 +14,7 @@ template <int FEAT> struct Feat {
     __device__ __forceinline__ static bool has(const DevParams& P, int bit) { return (word(P) & bit) != 0; }
     __device__ __forceinline__ static int act(const DevParams& P) { return (word(P) >> F_ACT_SHIFT) & 7; }
     __device__ __forceinline__ static int rew(const DevParams& P) { return (word(P) >> F_REW_SHIFT) & 7; }
-    __device__ __forceinline__ static int obs(const DevParams& P) { return (word(P) >> F_OBS_SHIFT) & 3; }   // MDG_OBS_*
+    __device__ __forceinline__ static int obs(const DevParams& P) { return (word(P) >> F_OBS_SHIFT) & 7; }   // MDG_OBS_*
     __device__ __forceinline__ static int term(const DevParams& P) { return (word(P) >> F_TERM_SHIFT) & 3; }
 };
 
@@ -56,6 +56,8 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
         tg.y = fmaf(P.target_hi[1] - P.target_lo[1], u01(r2.y), P.target_lo[1]);
         tg.z = fmaf(P.target_hi[2] - P.target_lo[2], u01(r2.z), P.target_lo[2]);
         tg.w = fmaf(P.target_w_hi - P.target_w_lo, u01(r2.w), P.target_w_lo);
+    } else if (P.target_mode == 4) {      // WAYPOINTS: chase waypoint 0 first
+        tg.x = P.waypoints[0]; tg.y = P.waypoints[1]; tg.z = P.waypoints[2];
     } else {                              // CIRCLE slots
         float s, c;
         sincospif(2.0f * (float)j / (float)P.M, &s, &c);
@@ -200,6 +202,10 @@ __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict_
     } else {
         o[0] = d.p.x; o[1] = d.p.y; o[2] = d.p.z; o[3] = eta.x; o[4] = eta.y; o[5] = eta.z;
         o[6] = d.v.x; o[7] = d.v.y; o[8] = d.v.z; o[9] = d.w.x; o[10] = d.w.y; o[11] = d.w.z;
+        if (mode == 4) {                                           // KIN12_WP: next waypoint, world and body frame
+            const V3 rb = rot_inv(d.q, v3(tg.x - d.p.x, tg.y - d.p.y, tg.z - d.p.z));
+            o[12] = tg.x; o[13] = tg.y; o[14] = tg.z; o[15] = rb.x; o[16] = rb.y; o[17] = rb.z;
+        }
         if (with_adj) {
 #pragma unroll
             for (int k = 0; k < G; ++k) if (k < P.M) o[12 + k] = adj[k];

@@ -126,6 +126,8 @@ def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=
         hard = bad & (margin[:, 1] >= TIE)
         assert not hard.any(), ("reward mismatch", t, np.nonzero(hard)[0][:5], r32[hard][:5], r64[hard][:5])
         ties["reward"] += int(bad.sum())
+        if over.get("reward_mode", 0) == W.REW_FLY_THROUGH:
+            alive &= ~bad                                             # a capture tie also moves the target: drop the env
         worst["rew"] = max(worst["rew"], rerr[alive & ~bad].max(initial=0))
         # observation (kinematic part follows the state tolerances; adjacency is 0/1 with a threshold)
         ob32 = o32.reshape(N, M, opd)
@@ -138,6 +140,9 @@ def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=
             ob64 = np.concatenate([ob64[:, :, 0:3], ob64[:, :, 7:16]], axis=2)
         if over.get("obs_mode", 0) == W.OBS_KIN12_TGT:             # the 4 target words are copied, not computed
             assert np.abs(ob32[alive][:, :, 12:16] - ob64[alive][:, :, 12:16]).max(initial=0) < 1e-6, ("KIN12_TGT target slot", t)
+        if over.get("obs_mode", 0) == W.OBS_KIN12_WP:              # waypoint copied, body-frame offset follows p and q
+            assert np.abs(ob32[alive][:, :, 12:15] - ob64[alive][:, :, 12:15]).max(initial=0) < 1e-6, ("KIN12_WP waypoint", t)
+            assert np.abs(ob32[alive][:, :, 15:18] - ob64[alive][:, :, 15:18]).max(initial=0) < 1e-3, ("KIN12_WP body-frame offset", t)
         kin = np.abs(ob32[:, :, :12] - ob64[:, :, :12])
         kin[:, :, 3:6] = np.minimum(kin[:, :, 3:6], 2 * np.pi - kin[:, :, 3:6])     # angles wrap
         kin_tol = np.array([TOL_P] * 3 + [2 * TOL_Q * 2] * 3 + [TOL_V] * 3 + [TOL_W] * 3)

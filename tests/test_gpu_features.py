@@ -91,6 +91,15 @@ CASES = {
                                     dict(CIRCLE, circle_radius=0.3, form_radius=0.3, aero_mask=15, wind_sigma=0.5, wind_tau=1.0, target_mode=W.TGT_CIRCLE,
                                          wind_mask=11, wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0, int_clamp_pos=1.0,
                                          int_clamp_att=0.25), ("uniform", -1.0, 1.0)), {}),
+    # FlyThroughAviary: ordered waypoints, capture reward, KIN12_WP observation; waypoints close together
+    # and a large capture radius so that captures, target hand-overs and terminal captures all happen within 48 steps
+    "m1_fly_through_pid": (wl("m1fly", 1500, 1, W.PHYS_MJC, W.ACT_VEL,
+                              dict(SINGLE, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH, target_mode=W.TGT_WAYPOINTS,
+                                   n_waypoints=3, waypoints=[0.0, 0.0, 1.0, 0.15, 0.0, 1.05, 0.15, 0.2, 1.0] + [0.0] * 15, wp_radius=0.12,
+                                   episode_len_s=20.0), ("uniform", -1.0, 1.0)), {}),
+    "m2_fly_through_default_list": (wl("m2fly", 800, 2, W.PHYS_MJC_DRAG, W.ACT_RPM,
+                                       dict(GRID, grid_cols=2, reset_z_lo=0.9, reset_z_hi=1.1, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH,
+                                            target_mode=W.TGT_WAYPOINTS, wp_radius=0.25, episode_len_s=20.0), HOVER), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
