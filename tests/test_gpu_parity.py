@@ -94,3 +94,40 @@ def test_back_to_back_steps_without_host_sync(c, n_envs):
     assert np.array_equal(gpu.done.cpu().numpy()[alive], d64[alive])
     rerr = np.abs(gpu.reward.cpu().numpy() - r64) / np.maximum(1.0, np.abs(r64))
     assert (rerr[alive] <= TOL_R).mean() > 0.999
+
+
+def test_interleaved_handles_and_host_step_are_bitwise_the_plain_sequence():
+    """bench.py's pattern: several handles stepped round-robin on one stream with nothing in between (each launch chains
+    on its own handle's previous step, the kernels of different handles overlap).  Results must equal, bit for bit, the
+    same handles stepped one at a time with a host sync after every step; mdg_step_host must equal mdg_step."""
+    import torch
+    import paper_2606_08039_b200 as mdg
+    wl = W.config(5).scaled(20000)                              # saturating grid: the chained path is taken
+    def make(k):
+        e = mdg.Env(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, mdg.default_params(0, **dict(wl.params, env_index_base=k * wl.n_envs)))
+        e.reset(wl.seed + k)
+        return e
+    fast, slow = [make(k) for k in range(3)], [make(k) for k in range(3)]
+    host = make(0)
+    acts = [[fast[k].gen_actions(wl.seed + k, t, 1.0, -1.0, 1.0) for t in range(24)] for k in range(3)]
+    torch.cuda.synchronize()
+    for t in range(24):
+        for k in range(3):
+            fast[k].step(acts[k][t])
+    for t in range(24):
+        for k in range(3):
+            slow[k].step(acts[k][t])
+            torch.cuda.synchronize()
+    obs_h = torch.empty((wl.n_envs, host.obs_dim), dtype=torch.float32).pin_memory()
+    rew_h = torch.empty(wl.n_envs, dtype=torch.float32).pin_memory()
+    done_h = torch.empty(wl.n_envs, dtype=torch.uint8).pin_memory()
+    for t in range(24):
+        host.step_host(acts[0][t].cpu().pin_memory(), obs_h, rew_h, done_h)
+    torch.cuda.synchronize()
+    for k in range(3):
+        a, b = fast[k].get_state(), slow[k].get_state()
+        for key in ("state", "ctrl", "targets", "wind", "ep_step"):
+            assert np.array_equal(a[key], b[key]), (k, key)
+        assert torch.equal(fast[k].obs, slow[k].obs) and torch.equal(fast[k].reward, slow[k].reward) and torch.equal(fast[k].done, slow[k].done)
+    assert np.array_equal(host.get_state()["state"], slow[0].get_state()["state"])
+    assert torch.equal(obs_h, slow[0].obs.cpu().reshape(wl.n_envs, -1)) and torch.equal(rew_h, slow[0].reward.cpu()) and torch.equal(done_h, slow[0].done.cpu())
