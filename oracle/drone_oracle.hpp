@@ -71,8 +71,10 @@ struct Params {
     int drone_model;                 // MODEL_*: CF2P selects the +-configuration mixing (Q37)
     double target_w_lo, target_w_hi; // TGT_BOX: range of the 4th target component (VelocityAviary's yaw rate)
     // Domain randomisation (Table 4): half-widths a of the per-episode multiplicative factors
-    // U(1 - a, 1 + a) of [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g]; all 0 = off (reading Q39)
-    double dr_alpha[8];
+    // U(1 - a, 1 + a) of [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g, per-motor thrust bias (4 draws), arm L,
+    // MAX_RPM, -]; all 0 = off (reading Q39).  Initial-state ranges of the same table: RPY_0 and v_0 half-widths.
+    double dr_alpha[12];
+    double reset_rpy_half[3], reset_vel_half[3];
     // Wind components (reading Q40): WIND_DRYDEN = the AR(1) gust above, WIND_CONSTANT = steady air
     // velocity wind_const (quadratic drag law), WIND_SINE = the force A [sin wt, cos wt, 0.3 sin 2wt] of episode time t
     int wind_mask; double wind_const[3], wind_sine_amp, wind_sine_omega;
@@ -80,7 +82,7 @@ struct Params {
     int n_waypoints; double waypoints[24], wp_radius;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_SINE = 8 };
-enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7 };
+enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_N = 16 };
 
 inline void default_params(int model, Params& P) {
     std::memset(&P, 0, sizeof(P));
@@ -232,7 +234,7 @@ template <class R> struct Drone {
     R p[3], q[4], v[3], w[3];     // A1 state; w is body-frame (Q22)
     R Ip[3], Ie[3], sp[4];        // PID memory: position / attitude integrals, held setpoint (DSL)
     double tg[4];                 // per-episode target (x, y, z, psi)
-    double sc[8];                 // domain-randomisation factors of this episode (DR_*; all 1 when off)
+    double sc[DR_N];              // domain-randomisation factors of this episode (DR_*; all 1 when off)
     double act[4];                // the action row applied in this control step (KIN20's a_{t-1}); zeros after a reset
     R n[4];                       // rotor speeds in RPM, held over the K substeps (Q21)
     R T, tau_b[3], Om;            // O4: collective thrust, body torque, sum of 2 pi n / 60
@@ -247,15 +249,16 @@ template <class R>
 inline void motor_wrench(const Params& P, const Derived& D, const R n[4], R& T, R tau[3], R& Om, const double* sc = nullptr) {
     const double kf = sc ? P.k_f * sc[DR_KF] : P.k_f;             // Table 4: k_f, k_m scaled per episode
     const double kappa = sc ? (P.k_m * sc[DR_KM]) / kf : D.kappa;
+    const double arm = sc ? sc[DR_ARM] : 1.0;
     R s[4];
-    for (int i = 0; i < 4; ++i) s[i] = kf * (n[i] * n[i]);
+    for (int i = 0; i < 4; ++i) s[i] = (sc ? kf * sc[DR_MOTOR + i] : kf) * (n[i] * n[i]);
     T = s[0] + s[1] + s[2] + s[3];
     if (P.drone_model == MODEL_CF2P) {                             // +-configuration (Q37)
-        tau[0] = P.L * (s[1] - s[3]);
-        tau[1] = P.L * (s[2] - s[0]);
+        tau[0] = (P.L * arm) * (s[1] - s[3]);
+        tau[1] = (P.L * arm) * (s[2] - s[0]);
     } else {
-        tau[0] = D.l * (s[0] + s[1] - s[2] - s[3]);
-        tau[1] = D.l * (-s[0] + s[1] + s[2] - s[3]);
+        tau[0] = (D.l * arm) * (s[0] + s[1] - s[2] - s[3]);
+        tau[1] = (D.l * arm) * (-s[0] + s[1] + s[2] - s[3]);
     }
     tau[2] = kappa * (-s[0] + s[1] - s[2] + s[3]);
     Om = (2.0 * PI / 60.0) * (n[0] + n[1] + n[2] + n[3]);      // Eq.5's rotor-speed sum
@@ -496,7 +499,7 @@ struct Sim {
     Params P; Derived D;
     uint64_t seed; uint32_t gstep;
     std::vector<double> state;    // [D][13] p q v w
-    std::vector<double> drs;      // [D][8] domain-randomisation factors of the running episode (DR_*)
+    std::vector<double> drs;      // [D][16] domain-randomisation factors of the running episode (DR_*)
     std::vector<double> pid;      // [D][10] Ip Ie sp
     std::vector<double> target;   // [D][4]
     std::vector<double> wind;     // [N][3]
@@ -513,7 +516,7 @@ struct Sim {
         N = n_envs; M = n_drones; physics_mode = phys; action_type = act; P = p; D = derive(P, phys);
         seed = 0; gstep = 0;
         const size_t Dn = (size_t)N * M;
-        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * 8, 1.0);
+        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * DR_N, 1.0);
         wind.assign((size_t)N * 3, 0.0); ep_step.assign(N, 0);
         obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); done.assign(N, 0);
         margin.assign((size_t)N * 3, 1e30);
@@ -543,6 +546,19 @@ struct Sim {
             else s[2] = base[2] + (-P.reset_half[2] + 2.0 * P.reset_half[2] * u01(r.x[2]));
             s[3] = 1.0; s[4] = s[5] = s[6] = 0.0;                   // identity attitude
             for (int a = 7; a < 13; ++a) s[a] = 0.0;                // at rest
+            // Table 4 "init" row: RPY_0 and v_0 uniform in +- the given half-widths (0 = the paper's default start)
+            if (P.reset_rpy_half[0] != 0.0 || P.reset_rpy_half[1] != 0.0 || P.reset_rpy_half[2] != 0.0) {
+                const PhiloxOut rr = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t, STREAM_INIT_RPY, k0, k1);
+                double hr[3];
+                for (int a = 0; a < 3; ++a) hr[a] = 0.5 * P.reset_rpy_half[a] * (2.0 * u01(rr.x[a]) - 1.0);   // half angles
+                const double cr = std::cos(hr[0]), sr = std::sin(hr[0]), cp = std::cos(hr[1]), sp = std::sin(hr[1]), cy = std::cos(hr[2]), sy = std::sin(hr[2]);
+                s[3] = cr * cp * cy + sr * sp * sy; s[4] = sr * cp * cy - cr * sp * sy;     // ZYX: q = q_z(yaw) q_y(pitch) q_x(roll)
+                s[5] = cr * sp * cy + sr * cp * sy; s[6] = cr * cp * sy - sr * sp * cy;
+            }
+            if (P.reset_vel_half[0] != 0.0 || P.reset_vel_half[1] != 0.0 || P.reset_vel_half[2] != 0.0) {
+                const PhiloxOut rv = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t, STREAM_INIT_VEL, k0, k1);
+                for (int a = 0; a < 3; ++a) s[7 + a] = P.reset_vel_half[a] * (2.0 * u01(rv.x[a]) - 1.0);
+            }
             double* tg = &target[di * 4];
             tg[3] = 0.0;
             if (P.target_mode == TGT_FIXED) {
@@ -564,13 +580,18 @@ struct Sim {
             }
             // Table 4, Q39: per-episode factors 1 + a (2u - 1); vehicle parameters per drone, g per env
             bool dr_on = false;
-            for (int a = 0; a < 8; ++a) dr_on = dr_on || P.dr_alpha[a] != 0.0;
+            for (int a = 0; a < 12; ++a) dr_on = dr_on || P.dr_alpha[a] != 0.0;
             if (dr_on) {
                 const uint32_t eg = (uint32_t)e + (uint32_t)P.env_index_base;
                 const PhiloxOut d0 = philox4x32_10(eg, (uint32_t)i, t, STREAM_DR0, k0, k1);
                 const PhiloxOut d1 = philox4x32_10(eg, (uint32_t)i, t, STREAM_DR1, k0, k1);
                 const PhiloxOut dg = philox4x32_10(eg, ENV_LEVEL, t, STREAM_DR1, k0, k1);
-                double* sc = &drs[di * 8];
+                const PhiloxOut d2 = philox4x32_10(eg, (uint32_t)i, t, STREAM_DR2, k0, k1);
+                const PhiloxOut d3 = philox4x32_10(eg, (uint32_t)i, t, STREAM_DR3, k0, k1);
+                double* sc = &drs[di * DR_N];
+                for (int a = 0; a < 4; ++a) sc[DR_MOTOR + a] = 1.0 + P.dr_alpha[8] * (2.0 * u01(d2.x[a]) - 1.0);
+                sc[DR_ARM] = 1.0 + P.dr_alpha[9] * (2.0 * u01(d3.x[0]) - 1.0);
+                sc[DR_MAXRPM] = 1.0 + P.dr_alpha[10] * (2.0 * u01(d3.x[1]) - 1.0);
                 for (int a = 0; a < 4; ++a) sc[a] = 1.0 + P.dr_alpha[a] * (2.0 * u01(d0.x[a]) - 1.0);
                 for (int a = 0; a < 3; ++a) sc[4 + a] = 1.0 + P.dr_alpha[4 + a] * (2.0 * u01(d1.x[a]) - 1.0);
                 sc[DR_G] = 1.0 + P.dr_alpha[DR_G] * (2.0 * u01(dg.x[0]) - 1.0);
@@ -592,7 +613,7 @@ struct Sim {
             for (int a = 0; a < 4; ++a) { d.q[a] = s[3 + a]; d.sp[a] = pm[6 + a]; d.tg[a] = target[di * 4 + a]; }
             for (int a = 0; a < 3; ++a) d.Fwind[a] = 0.0;
             for (int a = 0; a < 4; ++a) d.act[a] = 0.0;
-            for (int a = 0; a < 8; ++a) d.sc[a] = drs[di * 8 + a];
+            for (int a = 0; a < DR_N; ++a) d.sc[a] = drs[di * DR_N + a];
             d.hit = false; d.min_abs_pz = 1e30;
         }
     }
@@ -678,6 +699,8 @@ struct Sim {
         for (int i = 0; i < M; ++i) {
             decode_action(P, D, action_type, actions + ((size_t)e * M + i) * 4, dr[i]);
             for (int a = 0; a < 4; ++a) dr[i].act[a] = (double)actions[((size_t)e * M + i) * 4 + a];
+            if (dr[i].sc[DR_MAXRPM] != 1.0)                         // Table 4: the true motor saturation of this episode
+                for (int a = 0; a < 4; ++a) if (dr[i].n[a] > D.max_rpm * dr[i].sc[DR_MAXRPM]) dr[i].n[a] = D.max_rpm * dr[i].sc[DR_MAXRPM];
             motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
         }
         // K substeps: all wrenches from the same start-of-substep state, then integrate

@@ -168,12 +168,12 @@ class OracleEnv:
         self._set("wind", v, (self.N, 3))
 
     @property
-    def dr(self):               # [N*M, 8] domain-randomisation factors [m, J, k_f, k_m, drag, C_gnd, C_1, g]
-        return self._get("dr", (self.N * self.M, 8))
+    def dr(self):               # [N*M, 16] DR factors [m, J, k_f, k_m, drag, C_gnd, C_1, g, motor bias x4, arm, MAX_RPM, 1, 1]
+        return self._get("dr", (self.N * self.M, 16))
 
     @dr.setter
     def dr(self, v):
-        self._set("dr", v, (self.N * self.M, 8))
+        self._set("dr", v, (self.N * self.M, 16))
 
     @property
     def ep_step(self):

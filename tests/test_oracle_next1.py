@@ -161,7 +161,7 @@ def test_domain_randomisation_factors_draws_and_physics():
     """Table 4 (PAPER.md:229-248), reading Q39: per-episode factors U(1 - a, 1 + a) on [m, J, k_f, k_m, drag, C_gnd, C_1, g];
     each one enters the physics exactly where its nominal constant does, the controller keeps the nominal model."""
     alpha = [0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02]
-    env, _ = make_env(n_envs=3000, n_drones=2, dr_alpha=alpha, **FREE)
+    env, _ = make_env(n_envs=3000, n_drones=2, dr_alpha=alpha + [0.0] * 4, **FREE)
     f = env.dr
     for a in range(8):
         assert np.all(np.abs(f[:, a] - 1.0) <= alpha[a] + 1e-12)
@@ -173,7 +173,7 @@ def test_domain_randomisation_factors_draws_and_physics():
     assert np.all(env0.dr == 1.0)                                              # off by default
     # uniform thrust, level: z'' = 4 (k_f s_kf) n^2 / (m s_m) - g s_g
     env, _ = make_env(**FREE)
-    sc = np.array([[1.15, 0.9, 1.1, 0.93, 1.2, 0.8, 1.25, 1.01]])
+    sc = np.array([[1.15, 0.9, 1.1, 0.93, 1.2, 0.8, 1.25, 1.01] + [1.0] * 8])
     env.dr = sc
     set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
     n = float(np.float32(HOVER))
@@ -196,7 +196,7 @@ def test_domain_randomisation_factors_draws_and_physics():
     envg.state = st
     rpm = np.full((2, 4), HOVER)
     F0, _ = envg.probe_wrench(0, rpm)
-    d = np.ones((2, 8)); d[0, 4:7] = [1.3, 0.7, 1.2]
+    d = np.ones((2, 16)); d[0, 4:7] = [1.3, 0.7, 1.2]
     envg.dr = d
     F1, _ = envg.probe_wrench(0, rpm)
     T = M * G
@@ -296,3 +296,54 @@ def test_fly_through_waypoint_capture_reward_and_observation():
         assert rew[0] > 9.9 and done[0] == (1 if k == 4 else 0)
         if k < 4:
             assert np.array_equal(env.targets[0], list(WPS[k + 1]) + [k + 1])
+
+
+def test_table4_motor_bias_arm_maxrpm_and_initial_state_ranges():
+    """Table 4 rows beyond the first eight factors (reading Q39): per-motor thrust bias (4 draws), arm length, MAX_RPM,
+    and the "init" row: RPY_0 and v_0 uniform within given half-widths."""
+    from scipy.spatial.transform import Rotation
+    alpha = [0.0] * 8 + [0.05, 0.02, 0.05, 0.0]
+    env, _ = make_env(n_envs=4000, dr_alpha=alpha, reset_rpy_half=[0.1, 0.1, 0.1], reset_vel_half=[0.5, 0.5, 0.5], **FREE)
+    f = env.dr
+    assert np.all(f[:, :8] == 1.0) and np.all(f[:, 14:] == 1.0)
+    assert np.all(np.abs(f[:, 8:12] - 1) <= 0.05) and np.all(np.abs(f[:, 12] - 1) <= 0.02) and np.all(np.abs(f[:, 13] - 1) <= 0.05)
+    assert abs(f[:, 8:12].std() - 0.1 / math.sqrt(12)) < 0.002 and np.abs(np.corrcoef(f[:, 8:14].T) - np.eye(6)).max() < 0.06
+    st = env.state
+    rpy = Rotation.from_quat(st[:, [4, 5, 6, 3]]).as_euler("ZYX")[:, ::-1]           # roll, pitch, yaw
+    assert np.abs(rpy).max() <= 0.1 + 1e-12 and np.abs(rpy.std(axis=0) - 0.2 / math.sqrt(12)).max() < 0.003
+    assert np.abs(np.linalg.norm(st[:, 3:7], axis=1) - 1).max() < 1e-15
+    assert np.abs(st[:, 7:10]).max() <= 0.5 and np.abs(st[:, 7:10].std(axis=0) - 1.0 / math.sqrt(12)).max() < 0.01
+    assert np.abs(np.corrcoef(np.hstack([rpy, st[:, 7:10]]).T) - np.eye(6)).max() < 0.06 and np.all(st[:, 10:13] == 0)
+    # physics: biases scale each rotor's thrust and reaction torque, the arm scales roll / pitch torque only
+    P = O.OracleParams(0)
+    env1, _ = make_env(**FREE)
+    d = np.ones((1, 16)); d[0, 8:12] = [1.04, 0.97, 1.02, 0.96]; d[0, 12] = 1.015
+    env1.dr = d
+    set_state(env1, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    n = float(np.float32(HOVER))
+    for _ in range(6):
+        env1.step(np.full((1, 4), n, dtype=np.float32))
+    F = KF * n * n * d[0, 8:12]
+    l = L / math.sqrt(2) * 1.015
+    t = 6 / 48
+    tx, ty, tz = l * (F[0] + F[1] - F[2] - F[3]), l * (-F[0] + F[1] + F[2] - F[3]), (KM / KF) * (-F[0] + F[1] - F[2] + F[3])
+    s = env1.state[0]
+    assert abs(s[10] - tx * t / JXX) < 0.03 * abs(s[10]) and abs(s[11] - ty * t / JXX) < 0.1 * abs(s[11])   # gyroscopic coupling aside
+    env2, _ = make_env(**FREE)                                  # exact at the first substep: omega = tau h / J
+    env2.dr = d
+    set_state(env2, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    Fw, tw = env2.probe_wrench(0, np.full((1, 4), n))
+    assert abs(Fw[0, 2] - F.sum()) < 1e-15 and np.allclose(tw[0], [tx, ty, tz], rtol=1e-12, atol=1e-20)
+    # MAX_RPM factor < 1 saturates the rotors below the nominal limit; > 1 leaves the nominal command clip in force
+    env3, _ = make_env(**FREE)
+    d = np.ones((1, 16)); d[0, 13] = 0.96
+    env3.dr = d
+    set_state(env3, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    env3.step(np.full((1, 4), 1e6, dtype=np.float32))
+    acc = 4 * KF * (0.96 * MAXR) ** 2 / M - G
+    assert abs(env3.state[0, 9] - acc / 48) < 1e-10
+    d[0, 13] = 1.04
+    env3.dr = d
+    set_state(env3, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    env3.step(np.full((1, 4), 1e6, dtype=np.float32))
+    assert abs(env3.state[0, 9] - (4 * KF * MAXR ** 2 / M - G) / 48) < 1e-10
