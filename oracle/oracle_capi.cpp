@@ -159,7 +159,7 @@ void orc_probe_wrench(const void* h, int e, const double* rpm, double* F, double
     for (int i = 0; i < s.M; ++i) {
         Drone<double>& d = buf[i];
         for (int a = 0; a < 4; ++a) d.n[a] = rpm[i * 4 + a];
-        motor_wrench(s.P, s.D, d.n, d.T, d.tau_b, d.Om);
+        motor_wrench(s.P, s.D, d.n, d.T, d.tau_b, d.Om, d.sc);
         if (s.D.aero & AERO_WIND) {
             double rel[3]; for (int a = 0; a < 3; ++a) rel[a] = s.wind[(size_t)e * 3 + a] - d.v[a];
             const double nr = std::sqrt(rel[0] * rel[0] + rel[1] * rel[1] + rel[2] * rel[2]);
