@@ -98,9 +98,11 @@ typedef struct mdg_params {
     /* MDG_TGT_BOX: range of the 4th target word (VelocityAviary's yaw-rate target; 0, 0 by default) */
     float target_w_lo, target_w_hi;
     /* Domain randomisation (Table 4): half-widths a of the per-episode factors U(1-a, 1+a) applied to
-     * [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g], redrawn at every reset / auto-reset (vehicle factors per
-     * drone, g per env); all 0 = off.  The PID keeps the nominal model (reading Q39). */
-    float dr_alpha[8];
+     * [m, J, k_f, k_m, drag c_xy/c_z, C_gnd, downwash C_1, g, per-motor thrust bias (4 draws), arm L, MAX_RPM, -], redrawn at
+     * every reset / auto-reset (vehicle factors per drone, g per env); all 0 = off.  The PID keeps the nominal model
+     * (reading Q39).  reset_rpy_half / reset_vel_half: the table's initial-state ranges (uniform, 0 = at rest, level). */
+    float dr_alpha[12];
+    float reset_rpy_half[3], reset_vel_half[3];
     /* Wind components (reading Q40), active when MDG_AERO_WIND is set: MDG_WIND_DRYDEN is the
      * AR(1) gust above (default), MDG_WIND_CONSTANT adds the steady air velocity wind_const (m/s) under the same quadratic
      * drag law, MDG_WIND_SINE adds the force wind_sine_amp [sin wt, cos wt, 0.3 sin 2wt] (N) of episode time t. */
@@ -159,7 +161,8 @@ int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float
 int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
                   const float* wind, const uint32_t* ep_step);
 
-/* Domain-randomisation factors of the running episodes, host [D][8] in the order of mdg_params::dr_alpha (synchronise).
+/* Domain-randomisation factors of the running episodes, host [D][16] = [m, J, k_f, k_m, drag, C_gnd, C_1, g, motor bias x4,
+ * arm, MAX_RPM, 1, 1] (synchronise).
  * mdg_set_dr fails with MDG_EINVAL when every dr_alpha is 0 (the factors are then not read by the step). */
 int mdg_get_dr(mdg_env* env, float* factors);
 int mdg_set_dr(mdg_env* env, const float* factors);

@@ -32,7 +32,7 @@ class mdg_params(C.Structure):
         ("grid_cols", C.c_int32), ("grid_spacing", C.c_float), ("circle_radius", C.c_float),
         ("target_mode", C.c_int32), ("target_fixed", _F3), ("target_lo", _F3), ("target_hi", _F3),
         ("mh_z_lo", C.c_float), ("mh_z_hi", C.c_float), ("form_center", _F3), ("form_radius", C.c_float),
-        ("env_index_base", C.c_uint32), ("target_w_lo", C.c_float), ("target_w_hi", C.c_float), ("dr_alpha", C.c_float * 8),
+        ("env_index_base", C.c_uint32), ("target_w_lo", C.c_float), ("target_w_hi", C.c_float), ("dr_alpha", C.c_float * 12), ("reset_rpy_half", _F3), ("reset_vel_half", _F3),
         ("wind_mask", C.c_int32), ("wind_const", _F3), ("wind_sine_amp", C.c_float), ("wind_sine_omega", C.c_float),
         ("n_waypoints", C.c_int32), ("waypoints", C.c_float * 24), ("wp_radius", C.c_float),
     ]
@@ -217,15 +217,15 @@ class Env:
         return dict(state=st, ctrl=ct, targets=tg, wind=wd, ep_step=ep)
 
     def get_dr(self):
-        """Domain-randomisation factors of the running episodes, [D, 8] float32 (order of mdg_params.dr_alpha)."""
+        """Domain-randomisation factors of the running episodes, [D, 16] float32 (include/mdg.h: mdg_get_dr)."""
         import numpy as np
-        out = np.zeros((self.n_envs * self.n_drones, 8), dtype=np.float32)
+        out = np.zeros((self.n_envs * self.n_drones, 16), dtype=np.float32)
         _check(lib().mdg_get_dr(self._h, out.ctypes.data_as(C.c_void_p)))
         return out
 
     def set_dr(self, factors):
         import numpy as np
-        a = np.ascontiguousarray(factors, dtype=np.float32).reshape(self.n_envs * self.n_drones, 8)
+        a = np.ascontiguousarray(factors, dtype=np.float32).reshape(self.n_envs * self.n_drones, 16)
         _check(lib().mdg_set_dr(self._h, a.ctypes.data_as(C.c_void_p)))
 
     def set_state(self, state=None, ctrl=None, targets=None, wind=None, ep_step=None):

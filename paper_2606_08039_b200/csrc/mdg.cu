@@ -69,7 +69,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     if (action_type == MDG_ACT_PID && p.dsl) f |= F_DSL;
     f |= p.obs_mode << F_OBS_SHIFT;
     if (p.drone_model == MDG_MODEL_CF2P) f |= F_CF2P;
-    for (int i = 0; i < 8; ++i) if (p.dr_alpha[i] != 0.0f) f |= F_DR;
+    for (int i = 0; i < 12; ++i) if (p.dr_alpha[i] != 0.0f) f |= F_DR;
     if ((aero & MDG_AERO_WIND) && p.wind_mask != MDG_WIND_DRYDEN) f |= F_WIND_MIX;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
@@ -145,7 +145,8 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.reset_z_lo = p.reset_z_lo; D.reset_z_hi = p.reset_z_hi; D.grid_spacing = p.grid_spacing; D.circle_radius = p.circle_radius;
     D.mh_z_lo = p.mh_z_lo; D.mh_z_hi = p.mh_z_hi; D.form_radius = p.form_radius;
     D.target_w_lo = p.target_w_lo; D.target_w_hi = p.target_w_hi;
-    for (int i = 0; i < 8; ++i) D.dr_alpha[i] = p.dr_alpha[i];
+    for (int i = 0; i < 12; ++i) D.dr_alpha[i] = p.dr_alpha[i];
+    for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
     D.n_waypoints = p.n_waypoints; D.wp_radius2 = (float)((double)p.wp_radius * p.wp_radius);
     for (int i = 0; i < 24; ++i) D.waypoints[i] = p.waypoints[i];
     for (int dlt = 0; dlt < 32; ++dlt) D.chord[dlt] = (float)(2.0 * p.form_radius * std::fabs(std::sin(M_PI * dlt / M)));
@@ -332,14 +333,14 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     const size_t plane = al(D * sizeof(float4)), eplane = al((size_t)n_envs * sizeof(float4)), gs = al((size_t)n_envs * 4),
                  ob = al(D * h->P.opd * sizeof(float)), rw = al((size_t)n_envs * 4), dn = al((size_t)n_envs);
     const size_t n_items_max = (size_t)n_envs;                     // >= work items for any G
-    h->arena_bytes = 9 * plane + eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
+    h->arena_bytes = 11 * plane + eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
     cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
     if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
     ce = cudaMemset(h->arena, 0, h->arena_bytes);
     if (ce != cudaSuccess) { cudaFree(h->arena); delete h; return fail(MDG_ECUDA, std::string("mdg_create: cudaMemset: ") + cudaGetErrorString(ce)); }
     char* c = (char*)h->arena;
-    float4** planes[9] = {&h->B.P0, &h->B.P1, &h->B.P2, &h->B.P3, &h->B.P4, &h->B.P5, &h->B.P6, &h->B.R0, &h->B.R1};
-    for (int i = 0; i < 9; ++i) { *planes[i] = (float4*)c; c += plane; }
+    float4** planes[11] = {&h->B.P0, &h->B.P1, &h->B.P2, &h->B.P3, &h->B.P4, &h->B.P5, &h->B.P6, &h->B.R0, &h->B.R1, &h->B.R2, &h->B.R3};
+    for (int i = 0; i < 11; ++i) { *planes[i] = (float4*)c; c += plane; }
     h->B.E0 = (float4*)c; c += eplane;
     h->B.gstep = (uint32_t*)c; c += gs;
     h->B.obs = (float*)c; c += ob;
@@ -538,10 +539,12 @@ extern "C" int mdg_get_dr(mdg_env* h, float* f) {
     if (!h || !f) return fail(MDG_EINVAL, "mdg_get_dr: NULL argument");
     CU(cudaStreamSynchronize(h->stream));
     const size_t D = (size_t)h->N * h->M;
-    std::vector<float4> a(D), b(D);
-    CU(cudaMemcpy(a.data(), h->B.R0, D * sizeof(float4), cudaMemcpyDeviceToHost));
-    CU(cudaMemcpy(b.data(), h->B.R1, D * sizeof(float4), cudaMemcpyDeviceToHost));
-    for (size_t d = 0; d < D; ++d) { float* o = f + d * 8; o[0] = a[d].x; o[1] = a[d].y; o[2] = a[d].z; o[3] = a[d].w; o[4] = b[d].x; o[5] = b[d].y; o[6] = b[d].z; o[7] = b[d].w; }
+    float4* src[4] = {h->B.R0, h->B.R1, h->B.R2, h->B.R3};
+    std::vector<float4> a(D);
+    for (int k = 0; k < 4; ++k) {
+        CU(cudaMemcpy(a.data(), src[k], D * sizeof(float4), cudaMemcpyDeviceToHost));
+        for (size_t d = 0; d < D; ++d) { float* o = f + d * 16 + k * 4; o[0] = a[d].x; o[1] = a[d].y; o[2] = a[d].z; o[3] = a[d].w; }
+    }
     return MDG_OK;
 }
 extern "C" int mdg_set_dr(mdg_env* h, const float* f) {
@@ -549,10 +552,12 @@ extern "C" int mdg_set_dr(mdg_env* h, const float* f) {
     if (!(h->P.feat & F_DR)) return fail(MDG_EINVAL, "mdg_set_dr: domain randomisation is off for this handle (all dr_alpha are 0)");
     CU(cudaStreamSynchronize(h->stream));
     const size_t D = (size_t)h->N * h->M;
-    std::vector<float4> a(D), b(D);
-    for (size_t d = 0; d < D; ++d) { const float* o = f + d * 8; a[d] = make_float4(o[0], o[1], o[2], o[3]); b[d] = make_float4(o[4], o[5], o[6], o[7]); }
-    CU(cudaMemcpy(h->B.R0, a.data(), D * sizeof(float4), cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(h->B.R1, b.data(), D * sizeof(float4), cudaMemcpyHostToDevice));
+    float4* dst[4] = {h->B.R0, h->B.R1, h->B.R2, h->B.R3};
+    std::vector<float4> a(D);
+    for (int k = 0; k < 4; ++k) {
+        for (size_t d = 0; d < D; ++d) { const float* o = f + d * 16 + k * 4; a[d] = make_float4(o[0], o[1], o[2], o[3]); }
+        CU(cudaMemcpy(dst[k], a.data(), D * sizeof(float4), cudaMemcpyHostToDevice));
+    }
     h->chainable = false;
     return MDG_OK;
 }

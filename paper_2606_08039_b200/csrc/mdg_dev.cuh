@@ -56,7 +56,8 @@ struct DevParams {
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
     float target_fixed[3], target_lo[3], target_hi[3], target_w_lo, target_w_hi, mh_z_lo, mh_z_hi, form_center[3], form_radius;
     int n_waypoints; float waypoints[24], wp_radius2;     // FlyThroughAviary
-    float dr_alpha[8];                                    // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g]
+    float dr_alpha[12];                                   // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g, motor, arm, max_rpm, -]
+    float reset_rpy_half[3], reset_vel_half[3];           // Table 4 "init" row
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 
@@ -71,6 +72,8 @@ struct DevBuffers {
     float4* P6;   // target x y z psi
     float4* R0;   // DR factors m J k_f k_m
     float4* R1;   // DR factors drag gnd dw g
+    float4* R2;   // DR per-motor thrust bias
+    float4* R3;   // DR arm, MAX_RPM, -, -
     float4* E0;   // wind x y z, bits(ep_step)
     uint32_t* gstep;
     unsigned* ticket;   // two work-item dispensers of the step kernel (0 between launches), used alternately
@@ -80,7 +83,7 @@ struct DevBuffers {
     uint8_t* done;
 };
 
-static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5;
+static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9;
 
 // Philox4x32-10 (Salmon et al., SC'11).  key = seed halves, counter = (env, drone|~0, step, stream).
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,

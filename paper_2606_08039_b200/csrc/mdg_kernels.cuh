@@ -214,8 +214,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const float4 act4 = W.plane[7][lane];
     float4 env4 = W.plane[8][lane];
     const uint32_t t = W.gstep[lane] + 1u;
-    float4 dr0 = make_float4(1, 1, 1, 1), dr1 = dr0;             // this episode's DR factors (read-mostly, plain loads)
-    if (F::has(P, F_DR)) { dr0 = B.R0[drone]; dr1 = B.R1[drone]; }
+    float4 dr0 = make_float4(1, 1, 1, 1), dr1 = dr0, dr2 = dr0, dr3 = dr0;   // this episode's DR factors (read-mostly, plain loads)
+    if (F::has(P, F_DR)) { dr0 = B.R0[drone]; dr1 = B.R1[drone]; dr2 = B.R2[drone]; dr3 = B.R3[drone]; }
     if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch_item<G>(P, B, actions, S[(st ^ 1) * wpb + wib], wt_next, lane, jj, F::act(P)); }
     MDG_T(1);
 
@@ -260,11 +260,17 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const float kf_e = dr ? P.k_f * dr0.z : P.k_f, kappa_e = dr ? P.kappa * (dr0.w / dr0.z) : P.kappa;
     const float inv_sJ = dr ? 1.0f / dr0.y : 1.0f, inv_m_e = dr ? P.inv_m / dr0.x : P.inv_m, g_e = dr ? P.g * dr1.w : P.g;
     const float dwc_e = dr ? P.dw_coef * dr1.z : P.dw_coef;
-    const float f0 = kf_e * (n[0] * n[0]), f1 = kf_e * (n[1] * n[1]), f2 = kf_e * (n[2] * n[2]), f3 = kf_e * (n[3] * n[3]);
+    if (dr) {                                                      // true motor saturation of this episode
+        const float nmax = P.max_rpm * dr3.y;
+        n[0] = fminf(n[0], nmax); n[1] = fminf(n[1], nmax); n[2] = fminf(n[2], nmax); n[3] = fminf(n[3], nmax);
+    }
+    const float f0 = (dr ? kf_e * dr2.x : kf_e) * (n[0] * n[0]), f1 = (dr ? kf_e * dr2.y : kf_e) * (n[1] * n[1]),
+                f2 = (dr ? kf_e * dr2.z : kf_e) * (n[2] * n[2]), f3 = (dr ? kf_e * dr2.w : kf_e) * (n[3] * n[3]);
     const float T = (f0 + f1) + (f2 + f3);
+    const float arm_e = dr ? dr3.x : 1.0f;
     V3 tau_b = F::has(P, F_CF2P) ? v3(P.arm * (f1 - f3), P.arm * (f2 - f0), kappa_e * ((f1 + f3) - (f0 + f2)))
                                  : v3(P.l * ((f0 + f1) - (f2 + f3)), P.l * ((f1 + f2) - (f0 + f3)), kappa_e * ((f1 + f3) - (f0 + f2)));
-    if (dr) { tau_b.x *= inv_sJ; tau_b.y *= inv_sJ; tau_b.z *= inv_sJ; }
+    if (dr) { tau_b.x *= inv_sJ * arm_e; tau_b.y *= inv_sJ * arm_e; tau_b.z *= inv_sJ; }
     const float Om = P.rpm2rad * ((n[0] + n[1]) + (n[2] + n[3]));
     const V3 k1_tau = v3(P.invJ[0] * tau_b.x, P.invJ[1] * tau_b.y, P.invJ[2] * tau_b.z);
     const float cxy = (dr ? -P.c_xy * dr1.x : -P.c_xy) * Om, cz = (dr ? -P.c_z * dr1.x : -P.c_z) * Om;
@@ -435,12 +441,12 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         if (do_reset) {
             reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
             if (F::has(P, F_DR)) {
-                float4 n0, n1;
-                draw_dr(P, e, (uint32_t)jj, t, n0, n1);
-                if (active) { B.R0[drone] = n0; B.R1[drone] = n1; }
+                float4 n0, n1, n2, n3;
+                draw_dr(P, e, (uint32_t)jj, t, n0, n1, n2, n3);
+                if (active) { B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3; }
             }
             env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
-            eta = v3(0, 0, 0);
+            eta = euler_zyx(d.q);                                 // zeros unless Table 4's initial attitude range is on
             if (active) B.P6[drone] = tg_out;
         }
         if (F::obs(P) == 1) {                                      // the new episode's first observation
@@ -496,10 +502,10 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     if (!active) return;
     store_state(B, drone, d);
     B.P4[drone] = make_float4(0, 0, 0, 0); B.P5[drone] = d.sp; B.P6[drone] = tg;
-    float4 n0 = make_float4(1, 1, 1, 1), n1 = n0;
-    if (P.feat & F_DR) draw_dr(P, e, (uint32_t)jj, 0u, n0, n1);
-    B.R0[drone] = n0; B.R1[drone] = n1;
-    write_obs<G>(P, B.obs, drone, d, v3(0, 0, 0), adj, omode, make_float4(0, 0, 0, 0), tg);
+    float4 n0 = make_float4(1, 1, 1, 1), n1 = n0, n2 = n0, n3 = n0;
+    if (P.feat & F_DR) draw_dr(P, e, (uint32_t)jj, 0u, n0, n1, n2, n3);
+    B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3;
+    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), tg);
     if (j == 0) { B.E0[e] = make_float4(0, 0, 0, __uint_as_float(0u)); B.gstep[e] = 0u; B.reward[e] = 0.0f; B.done[e] = 0; }
 }
 

@@ -42,7 +42,21 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
     if (P.reset_z_hi > P.reset_z_lo) d.p.z = fmaf(P.reset_z_hi - P.reset_z_lo, u01(r.z), P.reset_z_lo);
     else d.p.z = bz + fmaf(2.0f * P.reset_half[2], u01(r.z), -P.reset_half[2]);
     d.q.w = 1.0f; d.q.x = d.q.y = d.q.z = 0.0f;
-    d.v = v3(0, 0, 0); d.w = v3(0, 0, 0); d.Ip = v3(0, 0, 0); d.Ie = v3(0, 0, 0);
+    d.v = v3(0, 0, 0); d.w = v3(0, 0, 0);
+    if (P.reset_rpy_half[0] != 0.0f || P.reset_rpy_half[1] != 0.0f || P.reset_rpy_half[2] != 0.0f) {   // Table 4 "init" row
+        const uint4 rr = philox4x32_10(e + P.env_base, j, t, STREAM_INIT_RPY, P.seed_lo, P.seed_hi);
+        float sr, cr, sp, cp, sy, cy;
+        sincosf(0.5f * P.reset_rpy_half[0] * fmaf(2.0f, u01(rr.x), -1.0f), &sr, &cr);
+        sincosf(0.5f * P.reset_rpy_half[1] * fmaf(2.0f, u01(rr.y), -1.0f), &sp, &cp);
+        sincosf(0.5f * P.reset_rpy_half[2] * fmaf(2.0f, u01(rr.z), -1.0f), &sy, &cy);
+        d.q.w = cr * cp * cy + sr * sp * sy; d.q.x = sr * cp * cy - cr * sp * sy;       // ZYX: q = q_z(yaw) q_y(pitch) q_x(roll)
+        d.q.y = cr * sp * cy + sr * cp * sy; d.q.z = cr * cp * sy - sr * sp * cy;
+    }
+    if (P.reset_vel_half[0] != 0.0f || P.reset_vel_half[1] != 0.0f || P.reset_vel_half[2] != 0.0f) {
+        const uint4 rv = philox4x32_10(e + P.env_base, j, t, STREAM_INIT_VEL, P.seed_lo, P.seed_hi);
+        d.v = v3(P.reset_vel_half[0] * fmaf(2.0f, u01(rv.x), -1.0f), P.reset_vel_half[1] * fmaf(2.0f, u01(rv.y), -1.0f),
+                 P.reset_vel_half[2] * fmaf(2.0f, u01(rv.z), -1.0f));
+    } d.Ip = v3(0, 0, 0); d.Ie = v3(0, 0, 0);
     d.sp = make_float4(d.p.x, d.p.y, d.p.z, 0.0f);
     tg.w = 0.0f;
     if (P.target_mode == 0) {             // FIXED
@@ -73,13 +87,17 @@ __device__ __forceinline__ float norm_rpm(const DevParams& P, float a) {
 }
 
 // Domain-randomisation factors of a new episode (Table 4; vehicle factors per drone, g per env)
-__device__ __forceinline__ void draw_dr(const DevParams& P, uint32_t e, uint32_t j, uint32_t t, float4& r0, float4& r1) {
+__device__ __forceinline__ void draw_dr(const DevParams& P, uint32_t e, uint32_t j, uint32_t t, float4& r0, float4& r1, float4& r2, float4& r3) {
     const uint4 a = philox4x32_10(e + P.env_base, j, t, STREAM_DR0, P.seed_lo, P.seed_hi);
     const uint4 b = philox4x32_10(e + P.env_base, j, t, STREAM_DR1, P.seed_lo, P.seed_hi);
+    const uint4 c = philox4x32_10(e + P.env_base, j, t, STREAM_DR2, P.seed_lo, P.seed_hi);
+    const uint4 d = philox4x32_10(e + P.env_base, j, t, STREAM_DR3, P.seed_lo, P.seed_hi);
     const uint4 g = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_DR1, P.seed_lo, P.seed_hi);
     auto f = [](float alpha, uint32_t x) { return fmaf(alpha, fmaf(2.0f, u01(x), -1.0f), 1.0f); };
     r0 = make_float4(f(P.dr_alpha[0], a.x), f(P.dr_alpha[1], a.y), f(P.dr_alpha[2], a.z), f(P.dr_alpha[3], a.w));
     r1 = make_float4(f(P.dr_alpha[4], b.x), f(P.dr_alpha[5], b.y), f(P.dr_alpha[6], b.z), f(P.dr_alpha[7], g.x));
+    r2 = make_float4(f(P.dr_alpha[8], c.x), f(P.dr_alpha[8], c.y), f(P.dr_alpha[8], c.z), f(P.dr_alpha[8], c.w));
+    r3 = make_float4(f(P.dr_alpha[9], d.x), f(P.dr_alpha[10], d.y), 1.0f, 1.0f);
 }
 
 // Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376)

@@ -25,7 +25,8 @@ SINGLE = dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.
               target_mode=W.TGT_FIXED, target_fixed=[0, 0, 1], episode_len_s=10.0, auto_reset=1)
 
 
-DR = [0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02]                       # Table 4
+DR = [0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02, 0.05, 0.02, 0.05, 0.0]     # Table 4
+INIT = dict(reset_rpy_half=[0.1, 0.1, 0.1], reset_vel_half=[0.5, 0.5, 0.5])   # its "init" row
 
 
 def wl(name, n, m, phys, act, params, actions, seed=77):
@@ -79,9 +80,11 @@ CASES = {
     "m1_domain_randomisation_pid": (wl("m1dr", 1500, 1, W.PHYS_MJC_GND, W.ACT_PID,
                                        dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST,
                                             term_tilt=0.4, term_dist=3.0, target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
-                                            episode_len_s=0.25, auto_reset=1, dr_alpha=DR), ("targets",)), {}),
+                                            episode_len_s=0.25, auto_reset=1, dr_alpha=DR, **INIT), ("targets",)), {}),
     "m4_domain_randomisation_all_aero": (wl("m4dr", 800, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
-                                            dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR), HOVER), {}),
+                                            dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR, **INIT), HOVER), {}),
+    "m1_domain_randomisation_saturated_rotors": (wl("m1drsat", 900, 1, W.PHYS_MJC, W.ACT_RPM_NORM,
+                                                    dict(SINGLE, episode_len_s=0.4, dr_alpha=DR), ("uniform", 0.8, 1.0)), {}),
     # wind components: constant + gust, sinusoidal alone, all three on a config-5-like setup (must leave the specialisation)
     "m1_wind_constant_plus_gust": (wl("m1wc", 1300, 1, W.PHYS_MJC, W.ACT_VEL, dict(SINGLE, aero_mask=W.AERO_WIND, wind_mask=3,
                                       wind_const=[0.9, -0.4, 0.1]), ("uniform", -0.5, 0.5)), {}),
@@ -187,4 +190,4 @@ def test_domain_randomisation_factors_match_the_oracle_draws():
     plain = mdg.Env(8, 1, W.PHYS_MJC, W.ACT_RPM)
     assert np.all(plain.get_dr() == 1.0)
     with pytest.raises(mdg.MdgError):
-        plain.set_dr(np.ones((8, 8), dtype=np.float32))
+        plain.set_dr(np.ones((8, 16), dtype=np.float32))
