@@ -15,7 +15,9 @@
 // Pins (tests/test_oracle_*.py, -m "not gpu"): O1 constants, free fall, hover equilibrium, uniform
 // thrust / pure yaw closed forms, torque-free rotation invariants + axisymmetric top + convergence
 // order, ground / drag / downwash closed forms, symmetries, PID fixed point + linear z recurrence +
-// allocation round trip, wind statistics, obs/reward/termination on hand-built states, Philox KATs.
+// allocation round trip, wind statistics, obs/reward/termination on hand-built states, Philox KATs;
+// tests/test_oracle_next1.py: normalised / one-dimensional / attitude actions, KIN20, CF2P mixing, the
+// velocity-tracking and fly-through epilogues, Table 4 factors and initial ranges, constant / sinusoidal wind.
 // PARITY UNPINNED (the oracle itself is the reference): the coupled PID transient in x/y and the
 // multi-config trajectories beyond the invariants above; parity against MuJoCo's own RK4 (MuJoCo is
 // not in the container, reading Q11).
