@@ -41,7 +41,7 @@ def algorithmic_bytes_per_drone(c: int) -> float:
     wr = 4 * 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)
     obs = 4 * (12 + (M if wl.params.get("obs_mode", 0) == W.OBS_KIN12_ADJ else 0))
     env = (16 + 4) + (16 + 4 + 4 + 1)                                                         # per env: E0 + gstep r/w, reward, done
-    return rd + wr + obs + env / M
+    return rd + wr + obs + 4 + env / M                                                        # + the per-drone reward share
 
 
 class ClockSampler:

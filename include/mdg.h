@@ -161,6 +161,11 @@ int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float
 int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
                   const float* wind, const uint32_t* ep_step);
 
+/* Per-agent view for multi-agent training (MultiAgentAviary): device pointer to [n_envs*n_drones] fp32, each
+ * drone's share of the last step's reward (its own terms plus half of every pair term it is part of); the shares of an
+ * env add up to its reward.  Library-owned, valid until mdg_destroy; written by every mdg_step. */
+int mdg_reward_per_drone(mdg_env* env, const float** reward_dev);
+
 /* Domain-randomisation factors of the running episodes, host [D][16] = [m, J, k_f, k_m, drag, C_gnd, C_1, g, motor bias x4,
  * arm, MAX_RPM, 1, 1] (synchronise).
  * mdg_set_dr fails with MDG_EINVAL when every dr_alpha is 0 (the factors are then not read by the step). */

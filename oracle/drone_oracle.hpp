@@ -508,6 +508,7 @@ struct Sim {
     std::vector<uint32_t> ep_step;  // [N]
     std::vector<double> obs;      // [N][M*opd]
     std::vector<double> reward;   // [N]
+    std::vector<double> reward_d; // [D] per-drone share of the reward (MultiAgentAviary); sums to reward[e]
     std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
     std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
 
@@ -520,7 +521,7 @@ struct Sim {
         const size_t Dn = (size_t)N * M;
         state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * DR_N, 1.0);
         wind.assign((size_t)N * 3, 0.0); ep_step.assign(N, 0);
-        obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); done.assign(N, 0);
+        obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); reward_d.assign((size_t)N * M, 0.0); done.assign(N, 0);
         margin.assign((size_t)N * 3, 1e30);
         for (size_t i = 0; i < Dn; ++i) state[i * 13 + 3] = 1.0;
     }
@@ -719,6 +720,8 @@ struct Sim {
         double m_done = 1e30, m_rew = 1e30;
         bool terminated = false;
         R rew = 0.0;
+        double* rd = &reward_d[(size_t)e * M];                   // bookkeeping beside the env reward, not part of its arithmetic
+        for (int i = 0; i < M; ++i) rd[i] = 0.0;
         for (int i = 0; i < M; ++i) {
             const Drone<R>& d = dr[i];
             R eta[3];
@@ -748,16 +751,16 @@ struct Sim {
                 if (dist < P.at_target_radius) r = r + 0.5;
                 if (crash) r = r - 100.0;
                 m_rew = std::fmin(m_rew, std::fabs(to_d(dist) - P.at_target_radius));
-                rew = rew + r;
+                rew = rew + r; rd[i] += to_d(r);
             } else if (P.reward_mode == REW_NEG_SQ_DIST) {          // config 3
-                rew = rew - (ex * ex + ey * ey + ez * ez);
+                rew = rew - (ex * ex + ey * ey + ez * ez); rd[i] -= to_d(ex * ex + ey * ey + ez * ez);
             } else if (P.reward_mode == REW_VELOCITY) {             // VelocityAviary, target = (v*, omega_z*), Q38
                 const R ux = d.v[0] - d.tg[0], uy = d.v[1] - d.tg[1], uz = d.v[2] - d.tg[2];
                 const R verr = sqrt(ux * ux + uy * uy + uz * uz);
                 R r = -verr - 0.1 * fabs(d.w[2] - d.tg[3]) - 0.05 * (aphi + ath);
                 if (verr < P.at_target_radius) r = r + 0.5;
                 m_rew = std::fmin(m_rew, std::fabs(to_d(verr) - P.at_target_radius));
-                rew = rew + r;
+                rew = rew + r; rd[i] += to_d(r);
             } else if (P.reward_mode == REW_FLY_THROUGH) {          // PAPER.md:321, Q41
                 const R dist = sqrt(ex * ex + ey * ey + ez * ez);   // to the waypoint being chased
                 const R wn = sqrt(d.w[0] * d.w[0] + d.w[1] * d.w[1] + d.w[2] * d.w[2]);
@@ -774,15 +777,16 @@ struct Sim {
                         tgs[2] = dr[i].tg[2] = P.waypoints[3 * k + 2]; tgs[3] = dr[i].tg[3] = (double)k;
                     }
                 }
-                rew = rew + r;
+                rew = rew + r; rd[i] += to_d(r);
             } else {                                                // REW_FORMATION (Q26)
-                rew = rew - sqrt(ex * ex + ey * ey + ez * ez);
+                rew = rew - sqrt(ex * ex + ey * ey + ez * ez); rd[i] -= to_d(sqrt(ex * ex + ey * ey + ez * ez));
                 for (int k = i + 1; k < M; ++k) {
                     const R ax = d.p[0] - dr[k].p[0], ay = d.p[1] - dr[k].p[1], az = d.p[2] - dr[k].p[2];
                     const double bx = d.tg[0] - dr[k].tg[0], by = d.tg[1] - dr[k].tg[1], bz = d.tg[2] - dr[k].tg[2];
                     const R dact = sqrt(ax * ax + ay * ay + az * az);
                     const double ddes = std::sqrt(bx * bx + by * by + bz * bz);
                     rew = rew - 0.5 * fabs(dact - ddes);
+                    rd[i] -= 0.25 * std::fabs(to_d(dact) - ddes); rd[k] -= 0.25 * std::fabs(to_d(dact) - ddes);   // half of the pair term each
                 }
             }
         }

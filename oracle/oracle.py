@@ -38,6 +38,7 @@ def lib():
         L.orc_get_gstep.restype = C.c_uint32
         L.orc_get_gstep.argtypes = [C.c_void_p]
         L.orc_get_outputs.argtypes = [C.c_void_p] * 5
+        L.orc_get_reward_d.argtypes = [C.c_void_p] * 2
         L.orc_refresh_obs.argtypes = [C.c_void_p]
         L.orc_probe_wrench.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_probe_decode.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
@@ -194,6 +195,10 @@ class OracleEnv:
         margin = np.zeros((self.N, 3))
         lib().orc_get_outputs(self._h, _p(obs), _p(rew), _p(done), _p(margin))
         return obs, rew, done, margin
+
+    @property
+    def reward_per_drone(self):   # [N*M] per-drone share of the last step's reward (sums to the env reward)
+        return self._get("reward_d", (self.N * self.M,))
 
     def probe_wrench(self, env, rpm):
         rpm = _f64(rpm).reshape(self.M, 4)

@@ -135,6 +135,7 @@ void orc_set_dr(void* h, const double* in) { std::memcpy(SIM->drs.data(), in, SI
 void orc_get_ep_step(const void* h, uint32_t* out) { std::memcpy(out, ((const Sim*)h)->ep_step.data(), ((const Sim*)h)->ep_step.size() * 4); }
 void orc_set_ep_step(void* h, const uint32_t* in) { std::memcpy(SIM->ep_step.data(), in, SIM->ep_step.size() * 4); }
 uint32_t orc_get_gstep(const void* h) { return ((const Sim*)h)->gstep; }
+void orc_get_reward_d(const void* h, double* out) { std::memcpy(out, ((const Sim*)h)->reward_d.data(), ((const Sim*)h)->reward_d.size() * 8); }
 void orc_get_outputs(const void* h, double* obs, double* reward, uint8_t* done, double* margin) {
     const Sim& s = *(const Sim*)h;
     if (obs) std::memcpy(obs, s.obs.data(), s.obs.size() * 8);

@@ -50,7 +50,7 @@ class mdg_params(C.Structure):
 
 EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
-           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_last_error", "mdg_version"]
+           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_last_error", "mdg_version"]
 
 _lib = None
 
@@ -79,6 +79,7 @@ def lib():
         L.mdg_get_state.argtypes = [vp] * 6
         L.mdg_set_state.argtypes = [vp] * 6
         L.mdg_set_stream.argtypes = [vp, vp]
+        L.mdg_reward_per_drone.argtypes = [vp, C.POINTER(vp)]
         L.mdg_get_dr.argtypes = [vp, vp]
         L.mdg_set_dr.argtypes = [vp, vp]
         L.mdg_launch_count.argtypes = [vp]
@@ -154,6 +155,9 @@ class Env:
         self.reward = torch.as_tensor(_DevArray(r.value, (n_envs,), "<f4", self), device=dev)
         self.done = torch.as_tensor(_DevArray(d.value, (n_envs,), "|u1", self), device=dev)
         self.targets = torch.as_tensor(_DevArray(t.value, (n_envs * n_drones, 4), "<f4", self), device=dev)
+        rd = C.c_void_p()
+        _check(lib().mdg_reward_per_drone(self._h, C.byref(rd)))
+        self.reward_per_drone = torch.as_tensor(_DevArray(rd.value, (n_envs * n_drones,), "<f4", self), device=dev)
         self.set_stream(stream if stream is not None else torch.cuda.current_stream())
 
     def close(self):

@@ -333,7 +333,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     const size_t plane = al(D * sizeof(float4)), eplane = al((size_t)n_envs * sizeof(float4)), gs = al((size_t)n_envs * 4),
                  ob = al(D * h->P.opd * sizeof(float)), rw = al((size_t)n_envs * 4), dn = al((size_t)n_envs);
     const size_t n_items_max = (size_t)n_envs;                     // >= work items for any G
-    h->arena_bytes = 11 * plane + eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
+    const size_t rd = al(D * sizeof(float));
+    h->arena_bytes = rd + 11 * plane + eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
     cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
     if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
     ce = cudaMemset(h->arena, 0, h->arena_bytes);
@@ -347,6 +348,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     h->B.reward = (float*)c; c += rw;
     h->B.done = (uint8_t*)c; c += dn;
     h->B.ticket = (unsigned*)c; c += 256;
+    h->B.reward_d = (float*)(c + al(n_items_max * 4));
     h->B.item_seq = (unsigned*)c;
     int rc = configure_launch(h);
     if (rc == MDG_OK && h->saturating) {     // throughput-bound batch: the 5-blocks-per-SM register budget measured fastest
@@ -425,6 +427,11 @@ int mdg_outputs(mdg_env* h, const float** obs, const float** reward, const uint8
     if (obs) *obs = h->B.obs;
     if (reward) *reward = h->B.reward;
     if (done) *done = h->B.done;
+    return MDG_OK;
+}
+int mdg_reward_per_drone(mdg_env* h, const float** r) {
+    if (!h || !r) return fail(MDG_EINVAL, "mdg_reward_per_drone: NULL argument");
+    *r = h->B.reward_d;
     return MDG_OK;
 }
 int mdg_obs_dim(const mdg_env* h) { return h ? h->M * h->P.opd : MDG_EINVAL; }

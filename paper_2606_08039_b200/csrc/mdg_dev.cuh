@@ -80,6 +80,7 @@ struct DevBuffers {
     unsigned* item_seq; // per work item: sequence number of the last step that finished it
     float* obs;
     float* reward;
+    float* reward_d;   // [D] per-drone share of the reward
     uint8_t* done;
 };
 

@@ -464,6 +464,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             if (F::act(P) == 1) B.P5[drone] = d.sp;
         }
         write_obs<G>(P, B.obs, drone, d, eta, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
+        B.reward_d[drone] = r;
         if (j == 0) {
             env4.w = __uint_as_float(ep_out);
             B.E0[e] = env4; B.gstep[e] = t;
@@ -506,6 +507,7 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     if (P.feat & F_DR) draw_dr(P, e, (uint32_t)jj, 0u, n0, n1, n2, n3);
     B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3;
     write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), tg);
+    B.reward_d[drone] = 0.0f;
     if (j == 0) { B.E0[e] = make_float4(0, 0, 0, __uint_as_float(0u)); B.gstep[e] = 0u; B.reward[e] = 0.0f; B.done[e] = 0; }
 }
 

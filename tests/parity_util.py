@@ -129,6 +129,13 @@ def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=
         if over.get("reward_mode", 0) == W.REW_FLY_THROUGH:
             alive &= ~bad                                             # a capture tie also moves the target: drop the env
         worst["rew"] = max(worst["rew"], rerr[alive & ~bad].max(initial=0))
+        # per-drone shares (MultiAgentAviary view): same tolerance, and they add up to the env reward
+        rd64 = orc.reward_per_drone.reshape(N, M)
+        rd32 = gpu.reward_per_drone.cpu().numpy().astype(np.float64).reshape(N, M)
+        ok = alive & ~bad
+        derr = np.abs(rd32 - rd64).max(axis=1) / np.maximum(1.0, np.abs(r64))
+        assert (derr[ok] <= TOL_R).all(), ("per-drone reward mismatch", t, derr[ok].max())
+        assert np.abs(rd32.sum(axis=1) - r32)[ok].max(initial=0) <= 1e-4 * np.maximum(1.0, np.abs(r32)).max()
         # observation (kinematic part follows the state tolerances; adjacency is 0/1 with a threshold)
         ob32 = o32.reshape(N, M, opd)
         ob64 = o64.reshape(N, M, opd)

@@ -347,3 +347,26 @@ def test_table4_motor_bias_arm_maxrpm_and_initial_state_ranges():
     set_state(env3, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
     env3.step(np.full((1, 4), 1e6, dtype=np.float32))
     assert abs(env3.state[0, 9] - (4 * KF * MAXR ** 2 / M - G) / 48) < 1e-10
+
+
+def test_per_drone_reward_shares_add_up_and_split_pair_terms():
+    """MultiAgentAviary view: each drone's share = its own terms + half of every pair term it is part of."""
+    over = dict(reward_mode=W.REW_FORMATION, target_mode=W.TGT_CIRCLE, reset_layout=W.LAYOUT_CIRCLE, circle_radius=0.3, form_radius=0.3,
+                form_center=[0, 0, 1], reset_center=[0, 0, 1], **FREE)
+    env, _ = make_env(n_envs=1, n_drones=3, **over)
+    st = env.state
+    st[:, 0:3] = [[0.4, 0.0, 1.0], [-0.1, 0.3, 1.1], [-0.2, -0.2, 0.9]]
+    env.state = st
+    hov = np.full((3, 4), HOVER, dtype=np.float32)
+    env.step(hov)
+    p, tg = env.state[:, 0:3], env.targets[:, 0:3]
+    want = np.zeros(3)
+    for i in range(3):
+        want[i] -= np.linalg.norm(p[i] - tg[i])
+        for k in range(3):
+            if k != i:
+                want[i] -= 0.25 * abs(np.linalg.norm(p[i] - p[k]) - np.linalg.norm(tg[i] - tg[k]))
+    assert np.allclose(env.reward_per_drone, want, atol=1e-13) and abs(env.reward_per_drone.sum() - env.outputs()[1][0]) < 1e-13
+    envh, _ = make_env(n_envs=2, n_drones=2, reward_mode=W.REW_MULTI_HOVER, **FREE)
+    envh.step(np.full((4, 4), HOVER, dtype=np.float32))
+    assert np.allclose(envh.reward_per_drone.reshape(2, 2).sum(axis=1), envh.outputs()[1], atol=1e-13)
