@@ -80,10 +80,13 @@ struct Params {
     // Wind components (reading Q40): WIND_DRYDEN = the AR(1) gust above, WIND_CONSTANT = steady air
     // velocity wind_const (quadratic drag law), WIND_SINE = the force A [sin wt, cos wt, 0.3 sin 2wt] of episode time t
     int wind_mask; double wind_const[3], wind_sine_amp, wind_sine_omega;
+    // WIND_GUST ("random impulses with a smooth sin(pi s) envelope and per-step trigger probability", reading
+    // Q42): trigger probability per control step, largest gust speed (m/s), duration of one impulse (s)
+    double gust_prob, gust_max, gust_duration;
     // FlyThroughAviary (reading Q41): ordered waypoints, capture radius
     int n_waypoints; double waypoints[24], wp_radius;
 };
-enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_SINE = 8 };
+enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_N = 16 };
 
 inline void default_params(int model, Params& P) {
@@ -104,6 +107,7 @@ inline void default_params(int model, Params& P) {
     P.k_wind = 0.5 * 1.225 * 1.0 * 0.01;                          // Q28
     P.wind_sigma = 0.5; P.wind_tau = 1.0;
     P.wind_mask = WIND_DRYDEN; P.wind_sine_omega = 2.0 * PI * 0.5;
+    P.gust_prob = 0.02; P.gust_max = 1.0; P.gust_duration = 0.5;   // Q42
     const double wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5, 0, 1, 1, 0, 0, 0.5};     // PAPER.md:321 default list
     P.n_waypoints = 5; for (int i = 0; i < 15; ++i) P.waypoints[i] = wps[i];
     P.wp_radius = 0.1;                                            // Q41
@@ -505,6 +509,7 @@ struct Sim {
     std::vector<double> pid;      // [D][10] Ip Ie sp
     std::vector<double> target;   // [D][4]
     std::vector<double> wind;     // [N][3]
+    std::vector<double> gust;     // [N][4] running impulse: velocity vector (m/s) and progress s (>= 1: none)
     std::vector<uint32_t> ep_step;  // [N]
     std::vector<double> obs;      // [N][M*opd]
     std::vector<double> reward;   // [N]
@@ -521,6 +526,7 @@ struct Sim {
         const size_t Dn = (size_t)N * M;
         state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * DR_N, 1.0);
         wind.assign((size_t)N * 3, 0.0); ep_step.assign(N, 0);
+        gust.assign((size_t)N * 4, 0.0); for (int e = 0; e < N; ++e) gust[(size_t)e * 4 + 3] = 1.0;
         obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); reward_d.assign((size_t)N * M, 0.0); done.assign(N, 0);
         margin.assign((size_t)N * 3, 1e30);
         for (size_t i = 0; i < Dn; ++i) state[i * 13 + 3] = 1.0;
@@ -604,6 +610,7 @@ struct Sim {
             pm[6] = s[0]; pm[7] = s[1]; pm[8] = s[2]; pm[9] = 0.0;  // held setpoint starts at the spawn pose
         }
         wind[(size_t)e * 3 + 0] = wind[(size_t)e * 3 + 1] = wind[(size_t)e * 3 + 2] = 0.0;
+        gust[(size_t)e * 4 + 0] = gust[(size_t)e * 4 + 1] = gust[(size_t)e * 4 + 2] = 0.0; gust[(size_t)e * 4 + 3] = 1.0;
         ep_step[e] = 0;
     }
 
@@ -686,12 +693,28 @@ struct Sim {
             }
             if (P.wind_mask & WIND_CONSTANT)                       // steady wind, same quadratic drag law
                 for (int a = 0; a < 3; ++a) w[a] = w[a] + P.wind_const[a];
+            if (P.wind_mask & WIND_GUST) {                         // PAPER.md:201, Q42
+                double* gs = &gust[(size_t)e * 4];
+                if (gs[3] >= 1.0) {                                // no impulse running: trigger with probability gust_prob
+                    const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, ENV_LEVEL, t, STREAM_GUST, k0, k1);
+                    if (u01(r.x[0]) < P.gust_prob) {
+                        const double amp = P.gust_max * u01(r.x[1]), z = 2.0 * u01(r.x[2]) - 1.0, ph = 2.0 * PI * u01(r.x[3]);
+                        const double rxy = std::sqrt(1.0 - z * z);  // direction uniform on the sphere
+                        gs[0] = amp * rxy * std::cos(ph); gs[1] = amp * rxy * std::sin(ph); gs[2] = amp * z; gs[3] = 0.0;
+                    }
+                }
+                if (gs[3] < 1.0) {                                 // smooth envelope sin(pi s), s advancing by dt / duration
+                    const R env_s = sin(R(PI * gs[3]));
+                    for (int a = 0; a < 3; ++a) w[a] = w[a] + gs[a] * env_s;
+                    gs[3] += D.dt_c / P.gust_duration;
+                }
+            }
             R fs[3] = {0.0, 0.0, 0.0};
             if (P.wind_mask & WIND_SINE) {                         // F(t) = A [sin wt, cos wt, 0.3 sin 2wt]
                 const R ph = P.wind_sine_omega * ((double)ep_step[e] * D.dt_c);   // episode time at the start of the step
                 fs[0] = P.wind_sine_amp * sin(ph); fs[1] = P.wind_sine_amp * cos(ph); fs[2] = (0.3 * P.wind_sine_amp) * sin(2.0 * ph);
             }
-            const bool drag = (P.wind_mask & (WIND_DRYDEN | WIND_CONSTANT)) != 0;
+            const bool drag = (P.wind_mask & (WIND_DRYDEN | WIND_CONSTANT | WIND_GUST)) != 0;
             for (int i = 0; i < M; ++i) {                          // PAPER.md:201 drag law, Q28
                 R rel[3] = {w[0] - dr[i].v[0], w[1] - dr[i].v[1], w[2] - dr[i].v[2]};
                 const R nr = sqrt(rel[0] * rel[0] + rel[1] * rel[1] + rel[2] * rel[2]);

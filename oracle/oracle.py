@@ -32,7 +32,7 @@ def lib():
         L.orc_step.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.orc_flop_tally.restype = C.c_uint64
         L.orc_flop_tally.argtypes = [C.c_void_p, C.c_void_p]
-        for n in ("state", "pid", "targets", "wind", "ep_step", "dr"):
+        for n in ("state", "pid", "targets", "wind", "ep_step", "dr", "gust"):
             getattr(L, "orc_get_" + n).argtypes = [C.c_void_p, C.c_void_p]
             getattr(L, "orc_set_" + n).argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_gstep.restype = C.c_uint32
@@ -195,6 +195,14 @@ class OracleEnv:
         margin = np.zeros((self.N, 3))
         lib().orc_get_outputs(self._h, _p(obs), _p(rew), _p(done), _p(margin))
         return obs, rew, done, margin
+
+    @property
+    def gust(self):             # [N, 4] running gust impulse: velocity vector and progress s (>= 1: none)
+        return self._get("gust", (self.N, 4))
+
+    @gust.setter
+    def gust(self, v):
+        self._set("gust", v, (self.N, 4))
 
     @property
     def reward_per_drone(self):   # [N*M] per-drone share of the last step's reward (sums to the env reward)

@@ -11,7 +11,7 @@ BASE_SEED = 260608039
 
 # interface enum values (include/mdg.h; Table 1, 179-187 Table 3)
 AERO_GND, AERO_DRAG, AERO_DW, AERO_WIND = 1, 2, 4, 8
-WIND_DRYDEN, WIND_CONSTANT, WIND_SINE = 1, 2, 8
+WIND_DRYDEN, WIND_CONSTANT, WIND_GUST, WIND_SINE = 1, 2, 4, 8
 INTEG_RK4, INTEG_EULER = 0, 1
 PHYS_MJC, PHYS_MJC_GND, PHYS_MJC_DRAG, PHYS_MJC_DW, PHYS_MJC_GND_DRAG_DW, PHYS_DYN = range(6)
 ACT_RPM, ACT_PID, ACT_VEL, ACT_RPM_NORM, ACT_ONE_D_RPM, ACT_ATTITUDE = 0, 1, 2, 3, 4, 5

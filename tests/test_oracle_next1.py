@@ -370,3 +370,37 @@ def test_per_drone_reward_shares_add_up_and_split_pair_terms():
     envh, _ = make_env(n_envs=2, n_drones=2, reward_mode=W.REW_MULTI_HOVER, **FREE)
     envh.step(np.full((4, 4), HOVER, dtype=np.float32))
     assert np.allclose(envh.reward_per_drone.reshape(2, 2).sum(axis=1), envh.outputs()[1], atol=1e-13)
+
+
+def test_gust_wind_impulses_envelope_and_trigger_rate():
+    """PAPER.md:201 (reading Q42): impulses with a sin(pi s) envelope, per-step trigger probability, direction uniform on the
+    sphere, speed U(0, gust_max)."""
+    KW, DT = 0.5 * 1.225 * 0.01, 1 / 48
+    hov = np.full((1, 4), HOVER, dtype=np.float32)
+    res = G - 4 * KF * float(hov[0, 0]) ** 2 / M
+    # a hand-set impulse: the air velocity follows g sin(pi s) with s = k dt / T, then the impulse ends
+    env, _ = make_env(physics=W.PHYS_MJC, aero_mask=W.AERO_WIND, wind_mask=4, gust_prob=0.0, gust_duration=0.25, **FREE)
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    g = np.array([0.8, -0.3, 0.2])
+    env.gust = np.array([[*g, 0.0]])
+    v = np.zeros(3)
+    for k in range(20):
+        env.step(hov)
+        s = k * DT / 0.25
+        u = g * math.sin(math.pi * s) if s < 1.0 else np.zeros(3)
+        rel = u - v
+        v = v + DT * (KW * np.linalg.norm(rel) * rel / M - np.array([0, 0, res]))
+    assert np.abs(env.state[0, 7:10] - v).max() < 1e-12 and env.gust[0, 3] >= 1.0 and abs(v[0]) > 1e-3
+    # trigger statistics over many envs: fraction of envs whose impulse started in the first step = gust_prob;
+    # speeds uniform in [0, gust_max]; directions isotropic
+    N = 20000
+    env, _ = make_env(n_envs=N, physics=W.PHYS_MJC, aero_mask=W.AERO_WIND, wind_mask=4, gust_prob=0.1, gust_max=2.0, gust_duration=10.0, **FREE)
+    env.step(np.tile(hov, (N, 1)))
+    gs = env.gust
+    on = gs[:, 3] < 1.0
+    assert abs(on.mean() - 0.1) < 0.01 and np.all(gs[~on, :3] == 0.0)
+    sp = np.linalg.norm(gs[on, :3], axis=1)
+    assert sp.max() <= 2.0 and abs(sp.mean() - 1.0) < 0.05 and abs(sp.std() - 2 / math.sqrt(12)) < 0.05
+    d = gs[on, :3] / sp[:, None]
+    assert np.abs(d.mean(axis=0)).max() < 0.05 and np.abs((d ** 2).mean(axis=0) - 1 / 3).max() < 0.03
+    assert np.allclose(gs[on, 3], DT / 10.0)                          # progress after the first sample
