@@ -34,7 +34,7 @@ extern "C" {
 /* aerodynamic feature mask ("toggled independently") */
 enum { MDG_AERO_GND = 1, MDG_AERO_DRAG = 2, MDG_AERO_DW = 4, MDG_AERO_WIND = 8 };
 enum { MDG_INTEG_RK4 = 0, MDG_INTEG_EULER = 1 };
-enum { MDG_WIND_DRYDEN = 1, MDG_WIND_CONSTANT = 2, MDG_WIND_SINE = 8 };   /* PAPER.md:199-205; GUST is not built */
+enum { MDG_WIND_DRYDEN = 1, MDG_WIND_CONSTANT = 2, MDG_WIND_GUST = 4, MDG_WIND_SINE = 8 };   /* PAPER.md:199-205; all four = COMBINED */
 /* Table 1 */
 enum { MDG_PHYS_MJC = 0, MDG_PHYS_MJC_GND = 1, MDG_PHYS_MJC_DRAG = 2, MDG_PHYS_MJC_DW = 3,
        MDG_PHYS_MJC_GND_DRAG_DW = 4, MDG_PHYS_DYN = 5 };
@@ -107,6 +107,9 @@ typedef struct mdg_params {
      * AR(1) gust above (default), MDG_WIND_CONSTANT adds the steady air velocity wind_const (m/s) under the same quadratic
      * drag law, MDG_WIND_SINE adds the force wind_sine_amp [sin wt, cos wt, 0.3 sin 2wt] (N) of episode time t. */
     int32_t wind_mask; float wind_const[3], wind_sine_amp, wind_sine_omega;
+    /* MDG_WIND_GUST (reading Q42): trigger probability per control step, largest impulse speed (m/s), impulse duration (s);
+     * an impulse adds g sin(pi s) to the air velocity, direction uniform on the sphere, speed U(0, gust_max) */
+    float gust_prob, gust_max, gust_duration;
     /* FlyThroughAviary: up to 8 ordered waypoints (x, y, z each) and the capture radius (reading Q41: 0.1 m) */
     int32_t n_waypoints; float waypoints[24], wp_radius;
 } mdg_params;

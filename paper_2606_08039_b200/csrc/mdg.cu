@@ -126,6 +126,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.dz_floor = p.dw_dz_clip > 1e-6f ? p.dw_dz_clip : 1e-6f;
     const double alpha = std::exp(-dtc / p.wind_tau);
     D.wind_alpha = (float)alpha; D.wind_gain = (float)(p.wind_sigma * std::sqrt(1.0 - alpha * alpha)); D.k_wind = p.k_wind;
+    D.gust_prob = p.gust_prob; D.gust_max = p.gust_max; D.gust_ds = (float)(dtc / p.gust_duration);
     D.wind_mask = p.wind_mask; D.wind_sine_amp = p.wind_sine_amp; D.wind_sine_omega = p.wind_sine_omega;
     for (int i = 0; i < 3; ++i) D.wind_const[i] = p.wind_const[i];
     D.dt_c = (float)dtc;
@@ -265,6 +266,7 @@ int mdg_default_params(int drone_model, mdg_params* p) {
     p->dw_C1 = 2267.18f; p->dw_C2 = 0.16f; p->dw_C3 = -0.11f; p->dw_dz_clip = 0.1f;
     p->k_wind = 0.5f * 1.225f * 1.0f * 0.01f; p->wind_sigma = 0.5f; p->wind_tau = 1.0f;
     p->wind_mask = MDG_WIND_DRYDEN; p->wind_sine_omega = (float)M_PI;
+    p->gust_prob = 0.02f; p->gust_max = 1.0f; p->gust_duration = 0.5f;
     const float wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5f, 0, 1, 1, 0, 0, 0.5f};          // PAPER.md:321 default list
     p->n_waypoints = 5; for (int i = 0; i < 15; ++i) p->waypoints[i] = wps[i];
     p->wp_radius = 0.1f;
@@ -310,7 +312,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 4 || p.n_waypoints < 0 || p.n_waypoints > 8 || (p.wind_mask & ~11) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 4 || p.n_waypoints < 0 || p.n_waypoints > 8 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))
@@ -334,7 +336,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
                  ob = al(D * h->P.opd * sizeof(float)), rw = al((size_t)n_envs * 4), dn = al((size_t)n_envs);
     const size_t n_items_max = (size_t)n_envs;                     // >= work items for any G
     const size_t rd = al(D * sizeof(float));
-    h->arena_bytes = rd + 11 * plane + eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
+    h->arena_bytes = rd + 11 * plane + 2 * eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
     cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
     if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
     ce = cudaMemset(h->arena, 0, h->arena_bytes);
@@ -343,6 +345,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     float4** planes[11] = {&h->B.P0, &h->B.P1, &h->B.P2, &h->B.P3, &h->B.P4, &h->B.P5, &h->B.P6, &h->B.R0, &h->B.R1, &h->B.R2, &h->B.R3};
     for (int i = 0; i < 11; ++i) { *planes[i] = (float4*)c; c += plane; }
     h->B.E0 = (float4*)c; c += eplane;
+    h->B.E1 = (float4*)c; c += eplane;
     h->B.gstep = (uint32_t*)c; c += gs;
     h->B.obs = (float*)c; c += ob;
     h->B.reward = (float*)c; c += rw;

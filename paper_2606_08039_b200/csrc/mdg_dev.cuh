@@ -45,6 +45,7 @@ struct DevParams {
     float gnd_coef, h_clip, c_xy, c_z, dw_coef, dw_C2, dw_C3, dz_clip, inv_dz_clip;
     float dw_C2s, dw_C3s, dw_b2_min, dz_floor;            // Eq.6 with beta scaled by sqrt(2 ln 2): exp(-x/2b^2) = 2^(-x/b'^2)
     float wind_alpha, wind_gain, k_wind;
+    float gust_prob, gust_max, gust_ds;                   // MDG_WIND_GUST: trigger probability, largest speed, dt_c / duration
     int wind_mask; float wind_const[3], wind_sine_amp, wind_sine_omega;   // MDG_WIND_*: 1 AR(1) gust, 2 constant, 8 sinusoidal force
     // cascaded PID (Eq.9, Table 6)
     float dt_c, m, inv_g;
@@ -75,6 +76,7 @@ struct DevBuffers {
     float4* R2;   // DR per-motor thrust bias
     float4* R3;   // DR arm, MAX_RPM, -, -
     float4* E0;   // wind x y z, bits(ep_step)
+    float4* E1;   // running gust impulse: velocity x y z, progress s (>= 1: none)
     uint32_t* gstep;
     unsigned* ticket;   // two work-item dispensers of the step kernel (0 between launches), used alternately
     unsigned* item_seq; // per work item: sequence number of the last step that finished it
@@ -84,7 +86,7 @@ struct DevBuffers {
     uint8_t* done;
 };
 
-static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9;
+static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9, STREAM_GUST = 10;
 
 // Philox4x32-10 (Salmon et al., SC'11).  key = seed halves, counter = (env, drone|~0, step, stream).
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,

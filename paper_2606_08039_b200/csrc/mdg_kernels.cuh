@@ -223,6 +223,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     // Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact in
     // fp32; cos/sin(2 pi u_b) = -cos/sin(2 pi (u_b - 1/2)) keeps the MUFU argument in [-pi, pi).
     V3 Fwind = v3(0, 0, 0);
+    float4 gust_out = make_float4(0, 0, 0, 1.0f);                  // E1 after this step (generic kernel, MDG_WIND_GUST only)
     if (F::has(P, F_WIND)) {
         // components (MDG_WIND_*): the benchmark configs run the AR(1) gust alone (wmask == 1 folds at compile time)
         const int wmask = FEAT >= 0 ? 1 : P.wind_mask;
@@ -237,7 +238,26 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             u = v3(env4.x, env4.y, env4.z);
         }
         if (wmask & 2) { u.x += P.wind_const[0]; u.y += P.wind_const[1]; u.z += P.wind_const[2]; }
-        if (wmask & 3) {
+        if (wmask & 4) {                                           // PAPER.md:201 impulses (Q42), state in E1
+            float4 gs = B.E1[e];
+            if (gs.w >= 1.0f) {                                    // none running: trigger with probability gust_prob
+                const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_GUST, P.seed_lo, P.seed_hi);
+                if (u01(r.x) < P.gust_prob) {
+                    const float amp = P.gust_max * u01(r.y), z = fmaf(2.0f, u01(r.z), -1.0f);
+                    const float rxy = sqrtf(fmaxf(fmaf(-z, z, 1.0f), 0.0f));
+                    float sp, cp;
+                    sincospif(2.0f * u01(r.w), &sp, &cp);
+                    gs = make_float4(amp * rxy * cp, amp * rxy * sp, amp * z, 0.0f);
+                }
+            }
+            if (gs.w < 1.0f) {                                     // envelope sin(pi s), s advances by dt_c / duration
+                const float es = sinpif(gs.w);
+                u.x = fmaf(gs.x, es, u.x); u.y = fmaf(gs.y, es, u.y); u.z = fmaf(gs.z, es, u.z);
+                gs.w += P.gust_ds;
+            }
+            gust_out = gs;
+        }
+        if (wmask & 7) {
             const V3 rel = v3(u.x - d.v.x, u.y - d.v.y, u.z - d.v.z);
             const float kn = P.k_wind * fast_sqrt(fmaf(rel.x, rel.x, fmaf(rel.y, rel.y, rel.z * rel.z)));
             Fwind = v3(kn * rel.x, kn * rel.y, kn * rel.z);
@@ -469,6 +489,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             env4.w = __uint_as_float(ep_out);
             B.E0[e] = env4; B.gstep[e] = t;
             B.reward[e] = rsum; B.done[e] = (uint8_t)done;
+            if (FEAT < 0 && (P.wind_mask & 4) && F::has(P, F_WIND)) B.E1[e] = do_reset ? make_float4(0, 0, 0, 1.0f) : gust_out;
         }
     }
     MDG_T(5);
@@ -508,6 +529,7 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3;
     write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), tg);
     B.reward_d[drone] = 0.0f;
+    if (j == 0) B.E1[e] = make_float4(0, 0, 0, 1.0f);
     if (j == 0) { B.E0[e] = make_float4(0, 0, 0, __uint_as_float(0u)); B.gstep[e] = 0u; B.reward[e] = 0.0f; B.done[e] = 0; }
 }
 

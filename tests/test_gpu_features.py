@@ -103,6 +103,12 @@ CASES = {
     "m2_fly_through_default_list": (wl("m2fly", 800, 2, W.PHYS_MJC_DRAG, W.ACT_RPM,
                                        dict(GRID, grid_cols=2, reset_z_lo=0.9, reset_z_hi=1.1, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH,
                                             target_mode=W.TGT_WAYPOINTS, wp_radius=0.25, episode_len_s=20.0), HOVER), {}),
+    # gust impulses (frequent, short) alone and the paper's COMBINED = all four wind components
+    "m1_wind_gust": (wl("m1wg", 1500, 1, W.PHYS_MJC, W.ACT_VEL, dict(SINGLE, aero_mask=W.AERO_WIND, wind_mask=4, gust_prob=0.2,
+                        gust_max=2.0, gust_duration=0.2), ("uniform", -0.5, 0.5)), {}),
+    "m2_wind_combined": (wl("m2wall", 900, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, aero_mask=W.AERO_WIND | W.AERO_DRAG, wind_mask=15,
+                            wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0, gust_prob=0.1, gust_max=1.5, gust_duration=0.3,
+                            episode_len_s=0.5), HOVER), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
