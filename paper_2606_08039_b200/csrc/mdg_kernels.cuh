@@ -19,7 +19,7 @@ __device__ __forceinline__ void store_state(const DevBuffers& B, size_t d, const
 // S8 rotation: classical RK4 on (q, w_body) with the torque frozen in the world frame (MJC* modes) or
 // explicit Euler (DYN).  The stage orientation is q0 (x) dq, so the body-frame torque at a stage is
 // R(dq)^T tau_b and q0 itself is only needed for the final update.  EXACT selects the library
-// sin/cos for |omega| h > 0.75 rad; the hot path uses the branch-free series (stage_torque, exp_half).
+// sin/cos for |omega| h > 0.28 rad; the hot path uses the branch-free series (stage_torque, exp_half).
 template <bool EXACT, bool EULER>
 __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, V3 tau_b, V3 k1_tau, bool axisym) {
     auto ex = [](V3 phi) { return EXACT ? exp_half_exact(phi) : exp_half(phi); };
@@ -49,7 +49,7 @@ __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, 
     const float rn = rsqrt_fast(fmaf(q.w, q.w, fmaf(q.x, q.x, fmaf(q.y, q.y, q.z * q.z))));
     q.w *= rn; q.x *= rn; q.y *= rn; q.z *= rn;
 }
-// out-of-line copy for fast spins (|omega| h > 0.75 rad): rare, keeps the hot loop free of library calls
+// out-of-line copy for fast spins (|omega| h > 0.28 rad, i.e. > 67 rad/s at 240 Hz): rare, keeps the hot loop free of library calls
 struct RotState { Q4 q; V3 w; };
 template <bool EULER>
 __device__ __noinline__ RotState integrate_rot_exact(const DevParams& P, Q4 q, V3 w, V3 tau_b, V3 k1_tau) {
