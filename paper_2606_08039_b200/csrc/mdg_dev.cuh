@@ -31,12 +31,14 @@ struct DevParams {
     uint32_t seed_lo, seed_hi, env_base;
     uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining (mdg_kernels.cuh)
     // integrator
-    float h, half_h, h_sixth, half_h2, w2_exact;          // w2_exact: |omega|^2 above which the exact path runs
+    float h, half_h, h_sixth, half_h2, w2_exact[2];          // w2_exact: |omega|^2 above which the exact path runs
     // Rodrigues coefficients of R(c w)^T as polynomials in y = |w|^2, c = h/2 (stages 2, 3) and h (stage 4):
-    // A(y) = c sin(c|w|)/(c|w|), B(y) = c^2 (1 - cos(c|w|))/(c|w|)^2, degree 2 (|w| h <= 0.28 rad: truncation < 1e-7)
-    float rotA_half[3], rotB_half[3], rotA_full[3], rotB_full[3];
+    // A(y) = c sin(c|w|)/(c|w|), B(y) = c^2 (1 - cos(c|w|))/(c|w|)^2.  Degree 2 (first three coefficients) is exact to
+    // 1e-7 for |w| h <= 0.28 rad and is used where a controller keeps the body rates small (PID / VEL actions);
+    // degree 3 holds to 0.75 rad and serves the open-loop action types.  w2_exact[d-2] is the matching |w|^2 bound.
+    float rotA_half[4], rotB_half[4], rotA_full[4], rotB_full[4];
     // Eq.7 increment for phi = (h/6) s, s = w0 + 2 w2 + 2 w3 + w4, as polynomials in |s|^2: cos(|phi|/2) and (h/6) sin(|phi|/2)/|phi|
-    float expC[3], expS[3];
+    float expC[4], expS[4];
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
     // motor model (Eq.1-3)
     float k_f, inv_k_f, l, kappa, inv_l, inv_kappa, max_rpm, s_max, T_max, rpm2rad;
@@ -175,11 +177,12 @@ __device__ __forceinline__ Q4 exp_half(V3 phi) {
     return r;
 }
 // the same increment for phi = c s with c folded into host-made coefficients (DevParams::expC, expS; degree 2 in |s|^2,
-// error < 1e-8 for |phi| <= 0.28 rad)
-__device__ __forceinline__ Q4 exp_half_scaled(const float (&cC)[3], const float (&cS)[3], V3 s) {
+// error < 1e-8 for |phi| <= 0.28 rad; degree 3 for |phi| <= 0.75 rad)
+template <int DEG>
+__device__ __forceinline__ Q4 exp_half_scaled(const float (&cC)[4], const float (&cS)[4], V3 s) {
     const float y = fmaf(s.x, s.x, fmaf(s.y, s.y, s.z * s.z));
-    const float c = fmaf(y, fmaf(y, cC[2], cC[1]), cC[0]);
-    const float f = fmaf(y, fmaf(y, cS[2], cS[1]), cS[0]);
+    const float c = DEG == 2 ? fmaf(y, fmaf(y, cC[2], cC[1]), cC[0]) : fmaf(y, fmaf(y, fmaf(y, cC[3], cC[2]), cC[1]), cC[0]);
+    const float f = DEG == 2 ? fmaf(y, fmaf(y, cS[2], cS[1]), cS[0]) : fmaf(y, fmaf(y, fmaf(y, cS[3], cS[2]), cS[1]), cS[0]);
     Q4 r; r.w = c; r.x = f * s.x; r.y = f * s.y; r.z = f * s.z;
     return r;
 }
@@ -195,11 +198,12 @@ __device__ __forceinline__ Q4 exp_half_exact(V3 phi) {
 }
 // R(c w)^T tau for the rotation vector phi = c w (Rodrigues): tau - A(y) (w x tau) + B(y) w x (w x tau) with
 // y = |w|^2 and the step factor c folded into the host-made coefficients cA, cB (DevParams::rotA_*, rotB_*;
-// degree 2 in y, error < 1e-7 relative for c|w| <= 0.28 rad).  Used for the RK4 stage torques.
-__device__ __forceinline__ V3 stage_torque(const float (&cA)[3], const float (&cB)[3], V3 w, V3 tau) {
+// degree 2 in y: error < 1e-7 relative for c|w| <= 0.28 rad; degree 3: for c|w| <= 0.75 rad).  Used for the RK4 stage torques.
+template <int DEG>
+__device__ __forceinline__ V3 stage_torque(const float (&cA)[4], const float (&cB)[4], V3 w, V3 tau) {
     const float y = fmaf(w.x, w.x, fmaf(w.y, w.y, w.z * w.z));
-    const float A = fmaf(y, fmaf(y, cA[2], cA[1]), cA[0]);
-    const float Bc = fmaf(y, fmaf(y, cB[2], cB[1]), cB[0]);
+    const float A = DEG == 2 ? fmaf(y, fmaf(y, cA[2], cA[1]), cA[0]) : fmaf(y, fmaf(y, fmaf(y, cA[3], cA[2]), cA[1]), cA[0]);
+    const float Bc = DEG == 2 ? fmaf(y, fmaf(y, cB[2], cB[1]), cB[0]) : fmaf(y, fmaf(y, fmaf(y, cB[3], cB[2]), cB[1]), cB[0]);
     const V3 c1 = cross(w, tau);
     const V3 c2 = cross(w, c1);
     return v3(fmaf(Bc, c2.x, fmaf(-A, c1.x, tau.x)), fmaf(Bc, c2.y, fmaf(-A, c1.y, tau.y)), fmaf(Bc, c2.z, fmaf(-A, c1.z, tau.z)));

@@ -20,7 +20,7 @@ __device__ __forceinline__ void store_state(const DevBuffers& B, size_t d, const
 // explicit Euler (DYN).  The stage orientation is q0 (x) dq, so the body-frame torque at a stage is
 // R(dq)^T tau_b and q0 itself is only needed for the final update.  EXACT selects the library
 // sin/cos for |omega| h > 0.28 rad; the hot path uses the branch-free series (stage_torque, exp_half).
-template <bool EXACT, bool EULER>
+template <bool EXACT, bool EULER, int DEG>
 __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, V3 tau_b, V3 k1_tau, bool axisym) {
     auto ex = [](V3 phi) { return EXACT ? exp_half_exact(phi) : exp_half(phi); };
     if (!EULER) {
@@ -29,16 +29,16 @@ __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, 
                          axisym ? k1_tau.z : fmaf(-P.gyro[2], w0.x * w0.y, k1_tau.z));
         const V3 w2 = v3(fmaf(P.half_h, k1.x, w0.x), fmaf(P.half_h, k1.y, w0.y), fmaf(P.half_h, k1.z, w0.z));
         auto stage_half = [&](V3 ws) { return EXACT ? rot_inv(exp_half_exact(v3(P.half_h * ws.x, P.half_h * ws.y, P.half_h * ws.z)), tau_b)
-                                                    : stage_torque(P.rotA_half, P.rotB_half, ws, tau_b); };
+                                                    : stage_torque<DEG>(P.rotA_half, P.rotB_half, ws, tau_b); };
         auto stage_full = [&](V3 ws) { return EXACT ? rot_inv(exp_half_exact(v3(P.h * ws.x, P.h * ws.y, P.h * ws.z)), tau_b)
-                                                    : stage_torque(P.rotA_full, P.rotB_full, ws, tau_b); };
+                                                    : stage_torque<DEG>(P.rotA_full, P.rotB_full, ws, tau_b); };
         const V3 k2 = ang_acc(P, stage_half(w0), w2, axisym);
         const V3 w3 = v3(fmaf(P.half_h, k2.x, w0.x), fmaf(P.half_h, k2.y, w0.y), fmaf(P.half_h, k2.z, w0.z));
         const V3 k3 = ang_acc(P, stage_half(w2), w3, axisym);
         const V3 w4 = v3(fmaf(P.h, k3.x, w0.x), fmaf(P.h, k3.y, w0.y), fmaf(P.h, k3.z, w0.z));
         const V3 k4 = ang_acc(P, stage_full(w3), w4, axisym);
         const V3 ws = v3(w0.x + 2.0f * (w2.x + w3.x) + w4.x, w0.y + 2.0f * (w2.y + w3.y) + w4.y, w0.z + 2.0f * (w2.z + w3.z) + w4.z);
-        q = qmul(q, EXACT ? exp_half_exact(v3(P.h_sixth * ws.x, P.h_sixth * ws.y, P.h_sixth * ws.z)) : exp_half_scaled(P.expC, P.expS, ws));
+        q = qmul(q, EXACT ? exp_half_exact(v3(P.h_sixth * ws.x, P.h_sixth * ws.y, P.h_sixth * ws.z)) : exp_half_scaled<DEG>(P.expC, P.expS, ws));
         w = v3(fmaf(P.h_sixth, k1.x + 2.0f * (k2.x + k3.x) + k4.x, w0.x), fmaf(P.h_sixth, k1.y + 2.0f * (k2.y + k3.y) + k4.y, w0.y),
                fmaf(P.h_sixth, k1.z + 2.0f * (k2.z + k3.z) + k4.z, w0.z));
     } else {
@@ -53,7 +53,7 @@ __device__ __forceinline__ void integrate_rot(const DevParams& P, Q4& q, V3& w, 
 struct RotState { Q4 q; V3 w; };
 template <bool EULER>
 __device__ __noinline__ RotState integrate_rot_exact(const DevParams& P, Q4 q, V3 w, V3 tau_b, V3 k1_tau) {
-    integrate_rot<true, EULER>(P, q, w, tau_b, k1_tau, false);
+    integrate_rot<true, EULER, 3>(P, q, w, tau_b, k1_tau, false);
     RotState r; r.q = q; r.w = w;
     return r;
 }
@@ -120,6 +120,8 @@ template <int G, int FEAT, int MINB>
 __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__ DevParams P, const DevBuffers B,
                                                          const float4* __restrict__ actions) {
     using F = Feat<FEAT>;
+    // series degree of the rotation update: 2 where the specialisation's controller keeps the body rates small (PID / VEL)
+    constexpr int DEG = (FEAT >= 0 && (((FEAT >> F_ACT_SHIFT) & 7) == 1 || ((FEAT >> F_ACT_SHIFT) & 7) == 2)) ? 2 : 3;
     extern __shared__ __align__(16) unsigned char smem_raw[];     // [2 stages][warps per block] WarpStage (host sizes it)
     WarpStage* const S = reinterpret_cast<WarpStage*>(smem_raw);
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -355,19 +357,19 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         const V3 acc = v3(Fw.x * inv_m_e, Fw.y * inv_m_e, fmaf(Fw.z, inv_m_e, -g_e));
 
         // S8 integrate with the wrench frozen in the world frame
-        const bool fast_spin = fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)) > P.w2_exact;
+        const bool fast_spin = fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)) > P.w2_exact[DEG - 2];
         if (!F::has(P, F_EULER)) {
             d.p.x = fmaf(P.half_h2, acc.x, fmaf(P.h, d.v.x, d.p.x));
             d.p.y = fmaf(P.half_h2, acc.y, fmaf(P.h, d.v.y, d.p.y));
             d.p.z = fmaf(P.half_h2, acc.z, fmaf(P.h, d.v.z, d.p.z));
             d.v.x = fmaf(P.h, acc.x, d.v.x); d.v.y = fmaf(P.h, acc.y, d.v.y); d.v.z = fmaf(P.h, acc.z, d.v.z);
             if (fast_spin) { const RotState rs = integrate_rot_exact<false>(P, d.q, d.w, tau_b, k1_tau); d.q = rs.q; d.w = rs.w; }
-            else integrate_rot<false, false>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
+            else integrate_rot<false, false, DEG>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
         } else {                                                   // DYN: explicit Euler
             d.v.x = fmaf(P.h, acc.x, d.v.x); d.v.y = fmaf(P.h, acc.y, d.v.y); d.v.z = fmaf(P.h, acc.z, d.v.z);
             d.p.x = fmaf(P.h, d.v.x, d.p.x); d.p.y = fmaf(P.h, d.v.y, d.p.y); d.p.z = fmaf(P.h, d.v.z, d.p.z);
             if (fast_spin) { const RotState rs = integrate_rot_exact<true>(P, d.q, d.w, tau_b, k1_tau); d.q = rs.q; d.w = rs.w; }
-            else integrate_rot<false, true>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
+            else integrate_rot<false, true, DEG>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
         }
         if (d.p.z < 0.0f) { hit = true; d.p.z = 0.0f; d.v.z = fmaxf(d.v.z, 0.0f); }   // floor
     }
