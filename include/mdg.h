@@ -3,9 +3,10 @@
  * One call advances thousands of independent environments, each holding M Crazyflie-class quadrotors,
  * by one control step of arxiv/paper_2606_08039 ("MuJoCo-Drones-Gym"): action decode (PAPER.md:171-187
  * Table 3; cascaded PID PAPER.md:347-376), rotor model (Eq.1-3), ground effect / blade
- * drag / downwash (Eq.4-6), wind gust, free-body integration over
+ * drag / downwash (Eq.4-6), wind (Dryden-style gust, constant, impulse gusts,
+ * sinusoidal), per-episode domain randomisation (Table 4), free-body integration over
  * sim_freq/ctrl_freq substeps, observation, reward, termination and
- * auto-reset (PAPER.md:177, 254-258, 304-325).  The interface follows the paper's statement of the
+ * auto-reset (PAPER.md:177, 254-258, 304-333).  The interface follows the paper's statement of the
  * simulator: constructor options, `reset(rng) -> state`,
  * `step(state, action) -> state, obs, reward, done`.
  *
@@ -129,8 +130,8 @@ void mdg_destroy(mdg_env* env);
  * zero controller memory, wind and step counters; obs is valid afterwards (reward 0, done 0). */
 int mdg_reset(mdg_env* env, uint64_t seed);
 
-/* One control step.  actions_dev: [n_envs*n_drones][4] fp32, caller-owned device memory, read only.
- * RPM: raw rotor speeds (clipped to [0, MAX_RPM]); PID: waypoint [x,y,z,psi]; VEL: [vx,vy,vz,wz]. */
+/* One control step.  actions_dev: [n_envs*n_drones][4] fp32, caller-owned device memory, 16-byte aligned, read only;
+ * the meaning of the four floats follows the action type (see MDG_ACT_* above).  Asynchronous on the bound stream. */
 int mdg_step(mdg_env* env, const float* actions_dev);
 
 /* n_steps control steps replayed as one CUDA graph: step k reads actions_dev + k*stride_floats.
@@ -144,7 +145,7 @@ int mdg_step_many(mdg_env* env, const float* actions_dev, int n_steps, int64_t s
 int mdg_step_host(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
 
 /* Device pointers to the library-owned outputs of the last reset/step:
- * obs [n_envs][mdg_obs_dim] fp32 (per drone: p, roll/pitch/yaw, v, body rates [, adjacency row]);
+ * obs [n_envs][mdg_obs_dim] fp32 (per drone: the MDG_OBS_* row, e.g. p, roll/pitch/yaw, v, body rates [, adjacency row]);
  * reward [n_envs] fp32; done [n_envs] u8 (bit0 terminated, bit1 truncated).  Any may be NULL. */
 int mdg_outputs(mdg_env* env, const float** obs_dev, const float** reward_dev, const uint8_t** done_dev);
 int mdg_obs_dim(const mdg_env* env); /* floats per env */
