@@ -52,7 +52,8 @@ enum { MDG_ACT_RPM = 0, MDG_ACT_PID = 1, MDG_ACT_VEL = 2, MDG_ACT_RPM_NORM = 3, 
 /* PAPER.md:177, 13.  KIN12 = [p, eta, v, omega]; KIN12_ADJ appends the adjacency row; KIN20 = [p, q, eta, v, omega,
  * a_{t-1}] with a_{t-1} the action applied in the step that produced the state (zeros after a reset). */
 enum { MDG_OBS_KIN12 = 0, MDG_OBS_KIN12_ADJ = 1, MDG_OBS_KIN20 = 2, MDG_OBS_KIN12_TGT = 3 /* KIN12 + the 4 target words */,
-       MDG_OBS_KIN12_WP = 4 /* KIN12 + next waypoint + its position in the body frame */ };
+       MDG_OBS_KIN12_WP = 4 /* KIN12 + next waypoint + its position in the body frame */,
+       MDG_OBS_KIN12_Z = 5 /* KIN12 + the drone's target altitude: the 13-dim rows of MultiHoverAviary / MultiAgentAviary */ };
 /* VELOCITY (VelocityAviary): target = (v*, omega_z*), r = -|v - v*| - 0.1 |omega_z - omega_z*| - 0.05 (|phi| + |theta|)
  * + 0.5 [|v - v*| < at_target_radius] summed over the env's drones */
 enum { MDG_REW_HOVER = 0, MDG_REW_NEG_SQ_DIST = 1, MDG_REW_MULTI_HOVER = 2, MDG_REW_FORMATION = 3, MDG_REW_VELOCITY = 4,

@@ -35,7 +35,7 @@ enum { AERO_GND = 1, AERO_DRAG = 2, AERO_DW = 4, AERO_WIND = 8 };
 enum { INTEG_RK4 = 0, INTEG_EULER = 1 };
 enum { PHYS_MJC = 0, PHYS_MJC_GND = 1, PHYS_MJC_DRAG = 2, PHYS_MJC_DW = 3, PHYS_MJC_GND_DRAG_DW = 4, PHYS_DYN = 5 };
 enum { ACT_RPM = 0, ACT_PID = 1, ACT_VEL = 2, ACT_RPM_NORM = 3, ACT_ONE_D_RPM = 4, ACT_ATTITUDE = 5 };
-enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2, OBS_KIN12_TGT = 3, OBS_KIN12_WP = 4 };
+enum { OBS_KIN12 = 0, OBS_KIN12_ADJ = 1, OBS_KIN20 = 2, OBS_KIN12_TGT = 3, OBS_KIN12_WP = 4, OBS_KIN12_Z = 5 };
 enum { REW_HOVER = 0, REW_NEG_SQ_DIST = 1, REW_MULTI_HOVER = 2, REW_FORMATION = 3, REW_VELOCITY = 4, REW_FLY_THROUGH = 5 };
 enum { TERM_NONE = 0, TERM_HOVER = 1, TERM_TILT_DIST = 2, TERM_FORMATION = 3 };
 enum { LAYOUT_NONE = 0, LAYOUT_GRID = 1, LAYOUT_CIRCLE = 2 };
@@ -517,7 +517,7 @@ struct Sim {
     std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
     std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
 
-    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : P.obs_mode == OBS_KIN12_TGT ? 16 : P.obs_mode == OBS_KIN12_WP ? 18 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
+    int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : P.obs_mode == OBS_KIN12_TGT ? 16 : P.obs_mode == OBS_KIN12_WP ? 18 : P.obs_mode == OBS_KIN12_Z ? 13 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
     int obs_dim() const { return M * opd(); }
 
     void init(int n_envs, int n_drones, int phys, int act, const Params& p) {
@@ -654,6 +654,7 @@ struct Sim {
             for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[3 + a] = to_d(eta[a]); oi[6 + a] = to_d(dr[i].v[a]); oi[9 + a] = to_d(dr[i].w[a]); }
             if (P.obs_mode == OBS_KIN12_TGT)                       // [p, eta, v, omega, v*_x, v*_y, v*_z, omega*_z]
                 for (int a = 0; a < 4; ++a) oi[12 + a] = dr[i].tg[a];
+            if (P.obs_mode == OBS_KIN12_Z) oi[12] = dr[i].tg[2];   // kinematic state plus target altitude (13)
             if (P.obs_mode == OBS_KIN12_WP) {                      // next waypoint and its position in the body frame
                 R Rm[3][3], rel[3] = {dr[i].tg[0] - dr[i].p[0], dr[i].tg[1] - dr[i].p[1], dr[i].tg[2] - dr[i].p[2]}, rb[3];
                 rotmat(dr[i].q, Rm);

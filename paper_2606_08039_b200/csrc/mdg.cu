@@ -91,7 +91,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.reset_layout = p.reset_layout; D.target_mode = p.target_mode;
     D.grid_cols = p.grid_cols > 0 ? p.grid_cols : 1; D.grid_rows = (M + D.grid_cols - 1) / D.grid_cols;
     const int omode = (feat >> F_OBS_SHIFT) & 7;
-    D.opd = omode == MDG_OBS_KIN20 ? 20 : omode == MDG_OBS_KIN12_TGT ? 16 : omode == MDG_OBS_KIN12_WP ? 18 : 12 + (omode == MDG_OBS_KIN12_ADJ ? M : 0);
+    D.opd = omode == MDG_OBS_KIN20 ? 20 : omode == MDG_OBS_KIN12_TGT ? 16 : omode == MDG_OBS_KIN12_WP ? 18 : omode == MDG_OBS_KIN12_Z ? 13 : 12 + (omode == MDG_OBS_KIN12_ADJ ? M : 0);
     D.h = (float)h; D.half_h = (float)(0.5 * h); D.h_sixth = (float)(h / 6.0); D.half_h2 = (float)(0.5 * h * h);
     D.w2_exact[0] = (float)((0.28 / h) * (0.28 / h));      // degree-2 series: exact to 1e-7 up to |omega| h = 0.28 rad
     D.w2_exact[1] = (float)((0.75 / h) * (0.75 / h));      // degree-3 series: up to 0.75 rad
@@ -313,7 +313,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 4 || p.n_waypoints < 0 || p.n_waypoints > 8 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))

@@ -220,6 +220,7 @@ __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict_
     } else {
         o[0] = d.p.x; o[1] = d.p.y; o[2] = d.p.z; o[3] = eta.x; o[4] = eta.y; o[5] = eta.z;
         o[6] = d.v.x; o[7] = d.v.y; o[8] = d.v.z; o[9] = d.w.x; o[10] = d.w.y; o[11] = d.w.z;
+        if (mode == 5) o[12] = tg.z;                               // KIN12_Z
         if (mode == 4) {                                           // KIN12_WP: next waypoint, world and body frame
             const V3 rb = rot_inv(d.q, v3(tg.x - d.p.x, tg.y - d.p.y, tg.z - d.p.z));
             o[12] = tg.x; o[13] = tg.y; o[14] = tg.z; o[15] = rb.x; o[16] = rb.y; o[17] = rb.z;

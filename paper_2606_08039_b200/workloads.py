@@ -15,7 +15,7 @@ WIND_DRYDEN, WIND_CONSTANT, WIND_GUST, WIND_SINE = 1, 2, 4, 8
 INTEG_RK4, INTEG_EULER = 0, 1
 PHYS_MJC, PHYS_MJC_GND, PHYS_MJC_DRAG, PHYS_MJC_DW, PHYS_MJC_GND_DRAG_DW, PHYS_DYN = range(6)
 ACT_RPM, ACT_PID, ACT_VEL, ACT_RPM_NORM, ACT_ONE_D_RPM, ACT_ATTITUDE = 0, 1, 2, 3, 4, 5
-OBS_KIN12, OBS_KIN12_ADJ, OBS_KIN20, OBS_KIN12_TGT, OBS_KIN12_WP = 0, 1, 2, 3, 4
+OBS_KIN12, OBS_KIN12_ADJ, OBS_KIN20, OBS_KIN12_TGT, OBS_KIN12_WP, OBS_KIN12_Z = 0, 1, 2, 3, 4, 5
 REW_HOVER, REW_NEG_SQ_DIST, REW_MULTI_HOVER, REW_FORMATION, REW_VELOCITY, REW_FLY_THROUGH = 0, 1, 2, 3, 4, 5
 TERM_NONE, TERM_HOVER, TERM_TILT_DIST, TERM_FORMATION = 0, 1, 2, 3
 LAYOUT_NONE, LAYOUT_GRID, LAYOUT_CIRCLE = 0, 1, 2

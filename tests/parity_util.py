@@ -147,6 +147,8 @@ def run_parity(wl, steps=48, extra=None, check_every=8, max_ill_frac=0.0, model=
             ob64 = np.concatenate([ob64[:, :, 0:3], ob64[:, :, 7:16]], axis=2)
         if over.get("obs_mode", 0) == W.OBS_KIN12_TGT:             # the 4 target words are copied, not computed
             assert np.abs(ob32[alive][:, :, 12:16] - ob64[alive][:, :, 12:16]).max(initial=0) < 1e-6, ("KIN12_TGT target slot", t)
+        if over.get("obs_mode", 0) == W.OBS_KIN12_Z:
+            assert np.abs(ob32[alive][:, :, 12] - ob64[alive][:, :, 12]).max(initial=0) < 1e-6, ("KIN12_Z target altitude", t)
         if over.get("obs_mode", 0) == W.OBS_KIN12_WP:              # waypoint copied, body-frame offset follows p and q
             assert np.abs(ob32[alive][:, :, 12:15] - ob64[alive][:, :, 12:15]).max(initial=0) < 1e-6, ("KIN12_WP waypoint", t)
             assert np.abs(ob32[alive][:, :, 15:18] - ob64[alive][:, :, 15:18]).max(initial=0) < 1e-3, ("KIN12_WP body-frame offset", t)

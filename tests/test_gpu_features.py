@@ -109,6 +109,8 @@ CASES = {
     "m2_wind_combined": (wl("m2wall", 900, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, aero_mask=W.AERO_WIND | W.AERO_DRAG, wind_mask=15,
                             wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0, gust_prob=0.1, gust_max=1.5, gust_duration=0.3,
                             episode_len_s=0.5), HOVER), {}),
+    # MultiHoverAviary as the paper tabulates it: 13 floats per drone (kinematic state + target altitude), normalised RPM
+    "m3_multi_hover_obs13": (wl("m3mh", 700, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM_NORM, dict(GRID, obs_mode=W.OBS_KIN12_Z), ("uniform", -0.1, 0.12)), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }

@@ -404,3 +404,13 @@ def test_gust_wind_impulses_envelope_and_trigger_rate():
     d = gs[on, :3] / sp[:, None]
     assert np.abs(d.mean(axis=0)).max() < 0.05 and np.abs((d ** 2).mean(axis=0) - 1 / 3).max() < 0.03
     assert np.allclose(gs[on, 3], DT / 10.0)                          # progress after the first sample
+
+
+def test_kin12_z_observation_is_state_plus_target_altitude():
+    """PAPER.md:317 / 333: MultiHoverAviary and MultiAgentAviary observe 13 numbers per drone: KIN12 + its target altitude."""
+    env, _ = make_env(n_envs=3, n_drones=4, obs_mode=W.OBS_KIN12_Z, reward_mode=W.REW_MULTI_HOVER, target_mode=W.TGT_SPAWN_LINSPACE,
+                      mh_z_lo=0.7, mh_z_hi=1.2, **FREE)
+    obs = env.outputs()[0].reshape(3, 4, 13)
+    assert np.allclose(obs[:, :, 12], np.linspace(0.7, 1.2, 4)[None, :], atol=1e-15)
+    st = env.state.reshape(3, 4, 13)
+    assert np.array_equal(obs[:, :, 0:3], st[:, :, 0:3]) and np.array_equal(obs[:, :, 6:9], st[:, :, 7:10]) and np.array_equal(obs[:, :, 9:12], st[:, :, 10:13])
