@@ -114,6 +114,10 @@ typedef struct mdg_params {
     float gust_prob, gust_max, gust_duration;
     /* FlyThroughAviary: up to 8 ordered waypoints (x, y, z each) and the capture radius (reading Q41: 0.1 m) */
     int32_t n_waypoints; float waypoints[24], wp_radius;
+    /* the waypoint-task family behind MDG_REW_FLY_THROUGH (reading Q43): reward per drone = wp_bonus [capture]
+     * - wp_shaping |d_wp| + wp_speed |v| - wp_omega |omega|, the list run wp_laps times.  Defaults = FlyThroughAviary
+     * (10, 0.1, 0, 0.01, 1 lap); RaceAviary = 20, 0.05, 2, 0, 2 laps over its six gates. */
+    float wp_bonus, wp_shaping, wp_speed, wp_omega; int32_t wp_laps;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

@@ -85,6 +85,9 @@ struct Params {
     double gust_prob, gust_max, gust_duration;
     // FlyThroughAviary (reading Q41): ordered waypoints, capture radius
     int n_waypoints; double waypoints[24], wp_radius;
+    // the waypoint-task family (FlyThroughAviary PAPER.md:321, RaceAviary PAPER.md:329; reading Q43): reward per drone =
+    // wp_bonus [capture] - wp_shaping |d_wp| + wp_speed |v| - wp_omega |omega|; the list is run wp_laps times
+    double wp_bonus, wp_shaping, wp_speed, wp_omega; int wp_laps;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_N = 16 };
@@ -111,6 +114,7 @@ inline void default_params(int model, Params& P) {
     const double wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5, 0, 1, 1, 0, 0, 0.5};     // PAPER.md:321 default list
     P.n_waypoints = 5; for (int i = 0; i < 15; ++i) P.waypoints[i] = wps[i];
     P.wp_radius = 0.1;                                            // Q41
+    P.wp_bonus = 10.0; P.wp_shaping = 0.1; P.wp_speed = 0.0; P.wp_omega = 0.01; P.wp_laps = 1;
     P.sim_freq = 240; P.ctrl_freq = 48;
     P.aero_mask = -1; P.integrator = -1;
     const double kp[3] = {0.4, 0.4, 1.0}, ki[3] = {0.01, 0.01, 0.01}, kd[3] = {0.9, 0.9, 2.0};     // Table 6
@@ -788,17 +792,19 @@ struct Sim {
             } else if (P.reward_mode == REW_FLY_THROUGH) {          // PAPER.md:321, Q41
                 const R dist = sqrt(ex * ex + ey * ey + ez * ez);   // to the waypoint being chased
                 const R wn = sqrt(d.w[0] * d.w[0] + d.w[1] * d.w[1] + d.w[2] * d.w[2]);
-                R r = -0.1 * dist - 0.01 * wn;
+                const R speed = sqrt(d.v[0] * d.v[0] + d.v[1] * d.v[1] + d.v[2] * d.v[2]);
+                R r = P.wp_speed * speed - P.wp_shaping * dist - P.wp_omega * wn;
                 const double mg = std::fabs(to_d(dist) - P.wp_radius);
                 m_rew = std::fmin(m_rew, mg); m_done = std::fmin(m_done, mg);
                 if (dist < P.wp_radius) {                           // capture: +10, move on; the last one ends the episode
-                    r = r + 10.0;
-                    const int k = (int)dr[i].tg[3] + 1;
-                    if (k >= P.n_waypoints) terminated = true;
+                    r = r + P.wp_bonus;
+                    const int k = (int)dr[i].tg[3] + 1;             // running index over all laps
+                    if (k >= P.n_waypoints * P.wp_laps) terminated = true;
                     else {
+                        const int kw = k % P.n_waypoints;
                         double* tgs = &target[((size_t)e * M + i) * 4];
-                        tgs[0] = dr[i].tg[0] = P.waypoints[3 * k]; tgs[1] = dr[i].tg[1] = P.waypoints[3 * k + 1];
-                        tgs[2] = dr[i].tg[2] = P.waypoints[3 * k + 2]; tgs[3] = dr[i].tg[3] = (double)k;
+                        tgs[0] = dr[i].tg[0] = P.waypoints[3 * kw]; tgs[1] = dr[i].tg[1] = P.waypoints[3 * kw + 1];
+                        tgs[2] = dr[i].tg[2] = P.waypoints[3 * kw + 2]; tgs[3] = dr[i].tg[3] = (double)k;
                     }
                 }
                 rew = rew + r; rd[i] += to_d(r);

@@ -36,6 +36,7 @@ class mdg_params(C.Structure):
         ("wind_mask", C.c_int32), ("wind_const", _F3), ("wind_sine_amp", C.c_float), ("wind_sine_omega", C.c_float),
         ("gust_prob", C.c_float), ("gust_max", C.c_float), ("gust_duration", C.c_float),
         ("n_waypoints", C.c_int32), ("waypoints", C.c_float * 24), ("wp_radius", C.c_float),
+        ("wp_bonus", C.c_float), ("wp_shaping", C.c_float), ("wp_speed", C.c_float), ("wp_omega", C.c_float), ("wp_laps", C.c_int32),
     ]
 
     def update(self, d):

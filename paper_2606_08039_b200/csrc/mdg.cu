@@ -149,6 +149,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.target_w_lo = p.target_w_lo; D.target_w_hi = p.target_w_hi;
     for (int i = 0; i < 12; ++i) D.dr_alpha[i] = p.dr_alpha[i];
     for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
+    D.wp_total = p.n_waypoints * p.wp_laps; D.wp_bonus = p.wp_bonus; D.wp_shaping = p.wp_shaping; D.wp_speed = p.wp_speed; D.wp_omega = p.wp_omega;
     D.n_waypoints = p.n_waypoints; D.wp_radius2 = (float)((double)p.wp_radius * p.wp_radius);
     for (int i = 0; i < 24; ++i) D.waypoints[i] = p.waypoints[i];
     for (int dlt = 0; dlt < 32; ++dlt) D.chord[dlt] = (float)(2.0 * p.form_radius * std::fabs(std::sin(M_PI * dlt / M)));
@@ -270,7 +271,7 @@ int mdg_default_params(int drone_model, mdg_params* p) {
     p->gust_prob = 0.02f; p->gust_max = 1.0f; p->gust_duration = 0.5f;
     const float wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5f, 0, 1, 1, 0, 0, 0.5f};          // PAPER.md:321 default list
     p->n_waypoints = 5; for (int i = 0; i < 15; ++i) p->waypoints[i] = wps[i];
-    p->wp_radius = 0.1f;
+    p->wp_radius = 0.1f; p->wp_bonus = 10.0f; p->wp_shaping = 0.1f; p->wp_speed = 0.0f; p->wp_omega = 0.01f; p->wp_laps = 1;
     p->sim_freq = 240; p->ctrl_freq = 48;
     p->aero_mask = -1; p->integrator = -1;
     const float kp[3] = {0.4f, 0.4f, 1.0f}, ki[3] = {0.01f, 0.01f, 0.01f}, kd[3] = {0.9f, 0.9f, 2.0f};   // Table 6
@@ -313,7 +314,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || p.wp_laps < 0 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))

@@ -58,7 +58,7 @@ struct DevParams {
     // reset / targets
     float reset_center[3], reset_half[3], reset_z_lo, reset_z_hi, grid_spacing, circle_radius;
     float target_fixed[3], target_lo[3], target_hi[3], target_w_lo, target_w_hi, mh_z_lo, mh_z_hi, form_center[3], form_radius;
-    int n_waypoints; float waypoints[24], wp_radius2;     // FlyThroughAviary
+    int n_waypoints, wp_total; float waypoints[24], wp_radius2, wp_bonus, wp_shaping, wp_speed, wp_omega;   // waypoint tasks
     float dr_alpha[12];                                   // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g, motor, arm, max_rpm, -]
     float reset_rpy_half[3], reset_vel_half[3];           // Table 4 "init" row
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]

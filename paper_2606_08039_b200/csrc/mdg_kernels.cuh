@@ -402,7 +402,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     } else if (rew == 1) {
         r = -e2;
     } else if (rew == 5) {                                         // FlyThroughAviary: capture handled below
-        r = fmaf(-0.1f, fast_sqrt(e2), -0.01f * fast_sqrt(fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z))));
+        r = fmaf(P.wp_speed, fast_sqrt(fmaf(d.v.x, d.v.x, fmaf(d.v.y, d.v.y, d.v.z * d.v.z))),
+                 fmaf(-P.wp_shaping, fast_sqrt(e2), -P.wp_omega * fast_sqrt(fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)))));
     } else if (rew == 4) {                                         // VelocityAviary: target = (v*, omega_z*)
         const float ux = d.v.x - tg.x, uy = d.v.y - tg.y, uz = d.v.z - tg.z;
         const float u2 = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
@@ -442,8 +443,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     bool captured = false, last_wp = false;
     if (rew == 5) {
         captured = e2 < P.wp_radius2;
-        last_wp = (int)tg.w + 1 >= P.n_waypoints;
-        if (captured) { r += 10.0f; if (last_wp) flags |= 1; }     // the last capture ends the episode
+        last_wp = (int)tg.w + 1 >= P.wp_total;                     // running index over all laps
+        if (captured) { r += P.wp_bonus; if (last_wp) flags |= 1; }   // the last capture ends the episode
     }
     const bool mine = full_group || j < P.M;
     const float rsum = group_sum<G>(mine ? r : 0.0f);
@@ -455,8 +456,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const bool do_reset = done != 0 && P.auto_reset != 0;
     float4 tg_out = tg;
     if (rew == 5 && captured && !last_wp) {                        // chase the next waypoint; its index rides in the 4th word
-        const int kn = (int)tg.w + 1;
-        tg_out = make_float4(P.waypoints[3 * kn], P.waypoints[3 * kn + 1], P.waypoints[3 * kn + 2], (float)kn);
+        const int kn = (int)tg.w + 1, kw = kn % P.n_waypoints;
+        tg_out = make_float4(P.waypoints[3 * kw], P.waypoints[3 * kw + 1], P.waypoints[3 * kw + 2], (float)kn);
         if (active && !do_reset) B.P6[drone] = tg_out;
     }
     if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp

@@ -109,6 +109,12 @@ CASES = {
     "m2_wind_combined": (wl("m2wall", 900, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, aero_mask=W.AERO_WIND | W.AERO_DRAG, wind_mask=15,
                             wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0, gust_prob=0.1, gust_max=1.5, gust_duration=0.3,
                             episode_len_s=0.5), HOVER), {}),
+    # RaceAviary parameters of the waypoint family: six gates close together, two laps, speed bonus
+    "m1_race_two_laps": (wl("m1race", 1500, 1, W.PHYS_MJC, W.ACT_VEL,
+                            dict(SINGLE, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH, target_mode=W.TGT_WAYPOINTS, n_waypoints=6,
+                                 waypoints=[0.1, 0.0, 1.0, 0.05, 0.09, 1.0, -0.05, 0.09, 1.0, -0.1, 0.0, 1.0, -0.05, -0.09, 1.0, 0.05, -0.09, 1.0] + [0.0] * 6,
+                                 wp_radius=0.12, wp_bonus=20.0, wp_shaping=0.05, wp_speed=2.0, wp_omega=0.0, wp_laps=2, episode_len_s=30.0),
+                            ("uniform", -1.0, 1.0)), {}),
     # MultiHoverAviary as the paper tabulates it: 13 floats per drone (kinematic state + target altitude), normalised RPM
     "m3_multi_hover_obs13": (wl("m3mh", 700, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM_NORM, dict(GRID, obs_mode=W.OBS_KIN12_Z), ("uniform", -0.1, 0.12)), {}),
     # one env, one warp not even full

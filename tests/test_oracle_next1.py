@@ -414,3 +414,28 @@ def test_kin12_z_observation_is_state_plus_target_altitude():
     assert np.allclose(obs[:, :, 12], np.linspace(0.7, 1.2, 4)[None, :], atol=1e-15)
     st = env.state.reshape(3, 4, 13)
     assert np.array_equal(obs[:, :, 0:3], st[:, :, 0:3]) and np.array_equal(obs[:, :, 6:9], st[:, :, 7:10]) and np.array_equal(obs[:, :, 9:12], st[:, :, 10:13])
+
+
+def test_race_parameters_of_the_waypoint_task_family():
+    """RaceAviary (reading Q43): +20 per gate, +2 |v| speed bonus, -0.05 d_gate shaping, the track run twice."""
+    gates = [1.5, 0.0, 1.0, 0.75, 1.3, 1.0, -0.75, 1.3, 1.0, -1.5, 0.0, 1.0, -0.75, -1.3, 1.0, 0.75, -1.3, 1.0]
+    env, _ = make_env(obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH, target_mode=W.TGT_WAYPOINTS, n_waypoints=6,
+                      waypoints=gates + [0.0] * 6, wp_radius=0.2, wp_bonus=20.0, wp_shaping=0.05, wp_speed=2.0, wp_omega=0.0, wp_laps=2,
+                      term_mode=W.TERM_HOVER, episode_len_s=30.0, auto_reset=0)
+    hov = np.full((1, 4), HOVER, dtype=np.float32)
+    G6 = np.array(gates).reshape(6, 3)
+    set_state(env, p=[1.0, 0.0, 1.0], q=[1, 0, 0, 0], v=[0.6, 0.8, 0.0], w=[0.0, 0.0, 1.0])
+    env.step(hov)
+    s = env.state[0]
+    want = 2.0 * np.linalg.norm(s[7:10]) - 0.05 * np.linalg.norm(G6[0] - s[0:3])
+    assert abs(env.outputs()[1][0] - want) < 1e-12 and abs(np.linalg.norm(s[7:10]) - 1.0) < 1e-6
+    idx = 0
+    for lap in range(2):
+        for k in range(6):
+            set_state(env, p=G6[k] + [0.0, 0.05, 0.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+            env.step(hov)
+            _, rew, done, _ = env.outputs()
+            idx += 1
+            assert abs(rew[0] - (20.0 - 0.05 * 0.05)) < 1e-6 and done[0] == (1 if idx == 12 else 0)
+            if idx < 12:
+                assert np.allclose(env.targets[0], list(G6[idx % 6]) + [idx])
