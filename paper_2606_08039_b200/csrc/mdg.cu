@@ -213,10 +213,13 @@ static int configure_launch(mdg_env* h) {
     const long long items = ((long long)h->N + epw - 1) / epw, blocks = (items + wpb - 1) / wpb;
     const long long slots = (long long)h->n_sms * resident;
     h->step_grid = (int)(blocks < slots ? blocks : slots);
-    // Item-level chaining of consecutive steps needs "at most two step kernels in flight" (two ticket dispensers):
-    // guaranteed when a grid fills every resident slot, because the successor's blocks can then only start in slots
-    // this grid has vacated, and the successor's successor only once all of those have started.
+    // Item-level chaining of consecutive steps.  A grid that fills every resident slot draws its items from a ticket
+    // dispenser; two dispensers alternate, which needs "at most two step kernels in flight": guaranteed there, because the
+    // successor's blocks can only start in slots this grid has vacated, and the successor's successor only once all of
+    // those have started.  A smaller grid gives every warp exactly one item (its index), draws nothing, and may
+    // therefore be chained to any depth.
     h->saturating = blocks >= slots;
+    h->P.static_items = h->saturating ? 0u : 1u;                   // one warp per item, no dispenser: any depth of chained launches is safe
     return MDG_OK;
 }
 static inline unsigned grid_for(const mdg_env* h, int block) {
@@ -230,7 +233,7 @@ static void drop_graphs(mdg_env* h) {
 static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s, bool may_chain) {
     h->seq += 1;
     h->P.seq = h->seq;
-    h->P.chain = (may_chain && h->pdl && h->saturating && h->chainable && h->last_stream == s) ? 1u : 0u;
+    h->P.chain = (may_chain && h->pdl && h->chainable && h->last_stream == s) ? 1u : 0u;
     h->chainable = may_chain; h->last_stream = s;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)h->step_grid); cfg.blockDim = dim3((unsigned)h->block);

@@ -29,6 +29,7 @@ struct DevParams {
     int N, M, K, ep_steps, auto_reset, feat;
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
     uint32_t seed_lo, seed_hi, env_base;
+    uint32_t static_items;                                // grid does not fill the device: one item per warp, item = warp index (no dispenser)
     uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining (mdg_kernels.cuh)
     // integrator
     float h, half_h, h_sixth, half_h2, w2_exact[2];          // w2_exact: |omega|^2 above which the exact path runs

@@ -179,9 +179,12 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         __syncwarp();
         if (lane == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(B.item_seq + item), "r"(P.seq) : "memory");
     };
-    unsigned wt = __shfl_sync(MDG_FULL, draw(true), 0);
+    // Grids that do not fill the device hold one warp per item: the item is the warp's index and no ticket is drawn, so
+    // any number of such launches may be in flight at once (each item still waits for its predecessor's flag).
+    const bool static_items = P.static_items != 0;
+    unsigned wt = static_items ? blockIdx.x * wpb + wib : __shfl_sync(MDG_FULL, draw(true), 0);
     if (wt >= n_items) return;
-    unsigned wt_next = __shfl_sync(MDG_FULL, draw(true), 0);      // a warp stops drawing after its first miss
+    unsigned wt_next = static_items ? 0xFFFFFFFFu : __shfl_sync(MDG_FULL, draw(true), 0);   // a warp stops drawing after its first miss
     unsigned probed_next = probe(wt_next);
     await_item(wt, probe(wt));
     prefetch_item<G>(P, B, actions, S[wib], wt, lane, jj, F::act(P));
