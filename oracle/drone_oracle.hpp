@@ -77,6 +77,9 @@ struct Params {
     // MAX_RPM, -]; all 0 = off (reading Q39).  Initial-state ranges of the same table: RPY_0 and v_0 half-widths.
     double dr_alpha[12];
     double reset_rpy_half[3], reset_vel_half[3];
+    // Table 4 "motor lag tau_mot U[5, 50] ms (per ep.)" (reading Q44): first-order rotor-speed lag, time constant drawn per
+    // drone and episode from U(motor_lag_lo, motor_lag_hi) seconds; 0, 0 = rotors follow the command at once
+    double motor_lag_lo, motor_lag_hi;
     // Wind components (reading Q40): WIND_DRYDEN = the AR(1) gust above, WIND_CONSTANT = steady air
     // velocity wind_const (quadratic drag law), WIND_SINE = the force A [sin wt, cos wt, 0.3 sin 2wt] of episode time t
     int wind_mask; double wind_const[3], wind_sine_amp, wind_sine_omega;
@@ -90,7 +93,7 @@ struct Params {
     double wp_bonus, wp_shaping, wp_speed, wp_omega; int wp_laps;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
-enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_N = 16 };
+enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_LAG = 14 /* tau_mot in seconds, not a factor */, DR_N = 16 };
 
 inline void default_params(int model, Params& P) {
     std::memset(&P, 0, sizeof(P));
@@ -244,6 +247,7 @@ template <class R> struct Drone {
     R p[3], q[4], v[3], w[3];     // A1 state; w is body-frame (Q22)
     R Ip[3], Ie[3], sp[4];        // PID memory: position / attitude integrals, held setpoint (DSL)
     double tg[4];                 // per-episode target (x, y, z, psi)
+    R n_act[4];                   // rotor speeds actually turning (motor lag, Q44); equal to n when the lag is off
     double sc[DR_N];              // domain-randomisation factors of this episode (DR_*; all 1 when off)
     double act[4];                // the action row applied in this control step (KIN20's a_{t-1}); zeros after a reset
     R n[4];                       // rotor speeds in RPM, held over the K substeps (Q21)
@@ -511,6 +515,7 @@ struct Sim {
     std::vector<double> state;    // [D][13] p q v w
     std::vector<double> drs;      // [D][16] domain-randomisation factors of the running episode (DR_*)
     std::vector<double> pid;      // [D][10] Ip Ie sp
+    std::vector<double> rotor;    // [D][4] rotor speeds actually turning (RPM), state of the motor lag
     std::vector<double> target;   // [D][4]
     std::vector<double> wind;     // [N][3]
     std::vector<double> gust;     // [N][4] running impulse: velocity vector (m/s) and progress s (>= 1: none)
@@ -528,7 +533,7 @@ struct Sim {
         N = n_envs; M = n_drones; physics_mode = phys; action_type = act; P = p; D = derive(P, phys);
         seed = 0; gstep = 0;
         const size_t Dn = (size_t)N * M;
-        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * DR_N, 1.0);
+        state.assign(Dn * 13, 0.0); pid.assign(Dn * 10, 0.0); target.assign(Dn * 4, 0.0); drs.assign(Dn * DR_N, 1.0); rotor.assign(Dn * 4, 0.0);
         wind.assign((size_t)N * 3, 0.0); ep_step.assign(N, 0);
         gust.assign((size_t)N * 4, 0.0); for (int e = 0; e < N; ++e) gust[(size_t)e * 4 + 3] = 1.0;
         obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); reward_d.assign((size_t)N * M, 0.0); done.assign(N, 0);
@@ -592,7 +597,9 @@ struct Sim {
                 tg[2] = P.form_center[2];
             }
             // Table 4, Q39: per-episode factors 1 + a (2u - 1); vehicle parameters per drone, g per env
-            bool dr_on = false;
+            const bool lag_on = P.motor_lag_hi > 0.0;
+            for (int a = 0; a < 4; ++a) rotor[di * 4 + a] = derive(P, 0).hover_rpm;   // Q44: an episode starts with the rotors at hover speed
+            bool dr_on = lag_on;
             for (int a = 0; a < 12; ++a) dr_on = dr_on || P.dr_alpha[a] != 0.0;
             if (dr_on) {
                 const uint32_t eg = (uint32_t)e + (uint32_t)P.env_index_base;
@@ -605,6 +612,7 @@ struct Sim {
                 for (int a = 0; a < 4; ++a) sc[DR_MOTOR + a] = 1.0 + P.dr_alpha[8] * (2.0 * u01(d2.x[a]) - 1.0);
                 sc[DR_ARM] = 1.0 + P.dr_alpha[9] * (2.0 * u01(d3.x[0]) - 1.0);
                 sc[DR_MAXRPM] = 1.0 + P.dr_alpha[10] * (2.0 * u01(d3.x[1]) - 1.0);
+                sc[DR_LAG] = lag_on ? P.motor_lag_lo + (P.motor_lag_hi - P.motor_lag_lo) * u01(d3.x[2]) : 1.0;
                 for (int a = 0; a < 4; ++a) sc[a] = 1.0 + P.dr_alpha[a] * (2.0 * u01(d0.x[a]) - 1.0);
                 for (int a = 0; a < 3; ++a) sc[4 + a] = 1.0 + P.dr_alpha[4 + a] * (2.0 * u01(d1.x[a]) - 1.0);
                 sc[DR_G] = 1.0 + P.dr_alpha[DR_G] * (2.0 * u01(dg.x[0]) - 1.0);
@@ -628,6 +636,7 @@ struct Sim {
             for (int a = 0; a < 3; ++a) d.Fwind[a] = 0.0;
             for (int a = 0; a < 4; ++a) d.act[a] = 0.0;
             for (int a = 0; a < DR_N; ++a) d.sc[a] = drs[di * DR_N + a];
+            for (int a = 0; a < 4; ++a) d.n_act[a] = rotor[di * 4 + a];
             d.hit = false; d.min_abs_pz = 1e30;
         }
     }
@@ -637,7 +646,7 @@ struct Sim {
             double* s = &state[di * 13]; double* pm = &pid[di * 10];
             const Drone<R>& d = dr[i];
             for (int a = 0; a < 3; ++a) { s[a] = to_d(d.p[a]); s[7 + a] = to_d(d.v[a]); s[10 + a] = to_d(d.w[a]); pm[a] = to_d(d.Ip[a]); pm[3 + a] = to_d(d.Ie[a]); }
-            for (int a = 0; a < 4; ++a) { s[3 + a] = to_d(d.q[a]); pm[6 + a] = to_d(d.sp[a]); }
+            for (int a = 0; a < 4; ++a) { s[3 + a] = to_d(d.q[a]); pm[6 + a] = to_d(d.sp[a]); rotor[di * 4 + a] = to_d(d.n_act[a]); }
         }
     }
 
@@ -735,7 +744,14 @@ struct Sim {
             motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
         }
         // K substeps: all wrenches from the same start-of-substep state, then integrate
+        const bool lag = P.motor_lag_hi > 0.0;
         for (int k = 0; k < D.K; ++k) {
+            if (lag)                                               // Q44: n <- n + (1 - e^(-h/tau)) (n_cmd - n), then Eq.1-3 with n
+                for (int i = 0; i < M; ++i) {
+                    const double gam = 1.0 - std::exp(-D.h / dr[i].sc[DR_LAG]);
+                    for (int a = 0; a < 4; ++a) dr[i].n_act[a] = dr[i].n_act[a] + gam * (dr[i].n[a] - dr[i].n_act[a]);
+                    motor_wrench(P, D, dr[i].n_act, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
+                }
             for (int i = 0; i < M; ++i) substep_wrench(P, D, dr, M, i);
             for (int i = 0; i < M; ++i) integrate(P, D, dr[i]);
         }

@@ -32,7 +32,7 @@ def lib():
         L.orc_step.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.orc_flop_tally.restype = C.c_uint64
         L.orc_flop_tally.argtypes = [C.c_void_p, C.c_void_p]
-        for n in ("state", "pid", "targets", "wind", "ep_step", "dr", "gust"):
+        for n in ("state", "pid", "targets", "wind", "ep_step", "dr", "gust", "rotor"):
             getattr(L, "orc_get_" + n).argtypes = [C.c_void_p, C.c_void_p]
             getattr(L, "orc_set_" + n).argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_gstep.restype = C.c_uint32
@@ -195,6 +195,14 @@ class OracleEnv:
         margin = np.zeros((self.N, 3))
         lib().orc_get_outputs(self._h, _p(obs), _p(rew), _p(done), _p(margin))
         return obs, rew, done, margin
+
+    @property
+    def rotor(self):            # [N*M, 4] rotor speeds actually turning (RPM): the state of the motor lag
+        return self._get("rotor", (self.N * self.M, 4))
+
+    @rotor.setter
+    def rotor(self, v):
+        self._set("rotor", v, (self.N * self.M, 4))
 
     @property
     def gust(self):             # [N, 4] running gust impulse: velocity vector and progress s (>= 1: none)

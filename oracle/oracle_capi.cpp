@@ -60,7 +60,7 @@ static const Field FIELDS[] = {
     FD(episode_len_s, 1), FI(auto_reset), FI(reset_layout), FD(reset_center, 3), FD(reset_half, 3),
     FD(reset_z_lo, 1), FD(reset_z_hi, 1), FI(grid_cols), FD(grid_spacing, 1), FD(circle_radius, 1), FI(target_mode),
     FD(target_fixed, 3), FD(target_lo, 3), FD(target_hi, 3), FD(mh_z_lo, 1), FD(mh_z_hi, 1), FD(form_center, 3),
-    FD(form_radius, 1), FI(env_index_base), FI(drone_model), FD(target_w_lo, 1), FD(target_w_hi, 1), FD(dr_alpha, 12), FD(reset_rpy_half, 3), FD(reset_vel_half, 3), FI(wind_mask), FD(wind_const, 3), FD(wind_sine_amp, 1), FD(wind_sine_omega, 1), FD(gust_prob, 1), FD(gust_max, 1), FD(gust_duration, 1), FI(n_waypoints), FD(waypoints, 24), FD(wp_radius, 1), FD(wp_bonus, 1), FD(wp_shaping, 1), FD(wp_speed, 1), FD(wp_omega, 1), FI(wp_laps),
+    FD(form_radius, 1), FI(env_index_base), FI(drone_model), FD(target_w_lo, 1), FD(target_w_hi, 1), FD(dr_alpha, 12), FD(reset_rpy_half, 3), FD(reset_vel_half, 3), FD(motor_lag_lo, 1), FD(motor_lag_hi, 1), FI(wind_mask), FD(wind_const, 3), FD(wind_sine_amp, 1), FD(wind_sine_omega, 1), FD(gust_prob, 1), FD(gust_max, 1), FD(gust_duration, 1), FI(n_waypoints), FD(waypoints, 24), FD(wp_radius, 1), FD(wp_bonus, 1), FD(wp_shaping, 1), FD(wp_speed, 1), FD(wp_omega, 1), FI(wp_laps),
 };
 static const Field* find_field(const char* name) {
     for (const Field& f : FIELDS) if (std::string(f.name) == name) return &f;
@@ -135,6 +135,8 @@ void orc_set_dr(void* h, const double* in) { std::memcpy(SIM->drs.data(), in, SI
 void orc_get_ep_step(const void* h, uint32_t* out) { std::memcpy(out, ((const Sim*)h)->ep_step.data(), ((const Sim*)h)->ep_step.size() * 4); }
 void orc_set_ep_step(void* h, const uint32_t* in) { std::memcpy(SIM->ep_step.data(), in, SIM->ep_step.size() * 4); }
 uint32_t orc_get_gstep(const void* h) { return ((const Sim*)h)->gstep; }
+void orc_get_rotor(const void* h, double* out) { std::memcpy(out, ((const Sim*)h)->rotor.data(), ((const Sim*)h)->rotor.size() * 8); }
+void orc_set_rotor(void* h, const double* in) { std::memcpy(SIM->rotor.data(), in, SIM->rotor.size() * 8); }
 void orc_get_gust(const void* h, double* out) { std::memcpy(out, ((const Sim*)h)->gust.data(), ((const Sim*)h)->gust.size() * 8); }
 void orc_set_gust(void* h, const double* in) { std::memcpy(SIM->gust.data(), in, SIM->gust.size() * 8); }
 void orc_get_reward_d(const void* h, double* out) { std::memcpy(out, ((const Sim*)h)->reward_d.data(), ((const Sim*)h)->reward_d.size() * 8); }

@@ -439,3 +439,38 @@ def test_race_parameters_of_the_waypoint_task_family():
             assert abs(rew[0] - (20.0 - 0.05 * 0.05)) < 1e-6 and done[0] == (1 if idx == 12 else 0)
             if idx < 12:
                 assert np.allclose(env.targets[0], list(G6[idx % 6]) + [idx])
+
+
+def test_motor_lag_first_order_rotor_dynamics():
+    """Table 4 "motor lag tau_mot U[5, 50] ms (per ep.)", reading Q44: rotor speeds follow the command through a first-order
+    lag sampled exactly per substep, n <- n + (1 - e^(-h/tau)) (n_cmd - n); episodes start at hover speed."""
+    h = 1 / 240
+    env, _ = make_env(n_envs=3000, motor_lag_lo=0.005, motor_lag_hi=0.05, **FREE)
+    tau = env.dr[:, 14]
+    assert tau.min() >= 0.005 and tau.max() <= 0.05 and abs(tau.mean() - 0.0275) < 0.001 and abs(tau.std() - 0.045 / math.sqrt(12)) < 0.0007
+    assert np.allclose(env.rotor, HOVER, rtol=1e-15) and np.all(env.dr[:, :14] == 1.0)
+    # one drone, tau fixed by hand: a thrust step from hover
+    env, _ = make_env(motor_lag_lo=0.02, motor_lag_hi=0.02, **FREE)
+    assert abs(env.dr[0, 14] - 0.02) < 1e-15
+    set_state(env, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    n1 = float(np.float32(1.2 * HOVER))
+    a = np.full((1, 4), n1, dtype=np.float32)
+    n, v, z = HOVER, 0.0, 1.0
+    gam = 1 - math.exp(-h / 0.02)
+    for step in range(12):
+        env.step(a)
+        for k in range(5):
+            n = n + gam * (n1 - n)
+            acc = 4 * KF * n * n / M - G
+            z = z + h * v + 0.5 * h * h * acc
+            v = v + h * acc
+    assert abs(env.state[0, 9] - v) < 1e-12 and abs(env.state[0, 2] - z) < 1e-12 and np.allclose(env.rotor[0], n, rtol=1e-14)
+    assert abs(n - (n1 + (HOVER - n1) * math.exp(-60 * h / 0.02))) < 1e-9 * n1       # the closed form of the lag itself
+    # the lag applies rotor by rotor: a differential command builds torque gradually (smaller rate than without lag)
+    env2, _ = make_env(**FREE)
+    for e in (env, env2):
+        set_state(e, p=[0, 0, 1.0], q=[1, 0, 0, 0], v=[0, 0, 0], w=[0, 0, 0])
+    env.rotor = np.full((1, 4), HOVER)
+    b = (np.array([[1.05, 1.05, 0.95, 0.95]]) * HOVER).astype(np.float32)
+    env.step(b); env2.step(b)
+    assert 0 < env.state[0, 10] < 0.6 * env2.state[0, 10]
