@@ -105,6 +105,10 @@ typedef struct mdg_params {
      * (reading Q39).  reset_rpy_half / reset_vel_half: the table's initial-state ranges (uniform, 0 = at rest, level). */
     float dr_alpha[12];
     float reset_rpy_half[3], reset_vel_half[3];
+    /* Table 4 motor lag (reading Q44): rotor speeds follow the command through a first-order lag, sampled exactly per
+     * substep; the time constant is drawn per drone and episode from U(motor_lag_lo, motor_lag_hi) seconds (5-50 ms in the
+     * table); 0, 0 = off.  Episodes start with the rotors at HOVER_RPM. */
+    float motor_lag_lo, motor_lag_hi;
     /* Wind components (reading Q40), active when MDG_AERO_WIND is set: MDG_WIND_DRYDEN is the
      * AR(1) gust above (default), MDG_WIND_CONSTANT adds the steady air velocity wind_const (m/s) under the same quadratic
      * drag law, MDG_WIND_SINE adds the force wind_sine_amp [sin wt, cos wt, 0.3 sin 2wt] (N) of episode time t. */
@@ -176,7 +180,7 @@ int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const flo
 int mdg_reward_per_drone(mdg_env* env, const float** reward_dev);
 
 /* Domain-randomisation factors of the running episodes, host [D][16] = [m, J, k_f, k_m, drag, C_gnd, C_1, g, motor bias x4,
- * arm, MAX_RPM, 1, 1] (synchronise).
+ * arm, MAX_RPM, motor-lag time constant (s; 1 when off), 1] (synchronise).
  * mdg_set_dr fails with MDG_EINVAL when every dr_alpha is 0 (the factors are then not read by the step). */
 int mdg_get_dr(mdg_env* env, float* factors);
 int mdg_set_dr(mdg_env* env, const float* factors);

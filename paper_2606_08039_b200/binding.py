@@ -32,7 +32,7 @@ class mdg_params(C.Structure):
         ("grid_cols", C.c_int32), ("grid_spacing", C.c_float), ("circle_radius", C.c_float),
         ("target_mode", C.c_int32), ("target_fixed", _F3), ("target_lo", _F3), ("target_hi", _F3),
         ("mh_z_lo", C.c_float), ("mh_z_hi", C.c_float), ("form_center", _F3), ("form_radius", C.c_float),
-        ("env_index_base", C.c_uint32), ("target_w_lo", C.c_float), ("target_w_hi", C.c_float), ("dr_alpha", C.c_float * 12), ("reset_rpy_half", _F3), ("reset_vel_half", _F3),
+        ("env_index_base", C.c_uint32), ("target_w_lo", C.c_float), ("target_w_hi", C.c_float), ("dr_alpha", C.c_float * 12), ("reset_rpy_half", _F3), ("reset_vel_half", _F3), ("motor_lag_lo", C.c_float), ("motor_lag_hi", C.c_float),
         ("wind_mask", C.c_int32), ("wind_const", _F3), ("wind_sine_amp", C.c_float), ("wind_sine_omega", C.c_float),
         ("gust_prob", C.c_float), ("gust_max", C.c_float), ("gust_duration", C.c_float),
         ("n_waypoints", C.c_int32), ("waypoints", C.c_float * 24), ("wp_radius", C.c_float),

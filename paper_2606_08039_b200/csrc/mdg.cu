@@ -70,6 +70,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     f |= p.obs_mode << F_OBS_SHIFT;
     if (p.drone_model == MDG_MODEL_CF2P) f |= F_CF2P;
     for (int i = 0; i < 12; ++i) if (p.dr_alpha[i] != 0.0f) f |= F_DR;
+    if (p.motor_lag_hi > 0.0f) f |= F_DR | F_MLAG;
     if ((aero & MDG_AERO_WIND) && p.wind_mask != MDG_WIND_DRYDEN) f |= F_WIND_MIX;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
@@ -149,6 +150,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.target_w_lo = p.target_w_lo; D.target_w_hi = p.target_w_hi;
     for (int i = 0; i < 12; ++i) D.dr_alpha[i] = p.dr_alpha[i];
     for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
+    D.motor_lag_lo = p.motor_lag_lo; D.motor_lag_hi = p.motor_lag_hi;
     D.wp_total = p.n_waypoints * p.wp_laps; D.wp_bonus = p.wp_bonus; D.wp_shaping = p.wp_shaping; D.wp_speed = p.wp_speed; D.wp_omega = p.wp_omega;
     D.n_waypoints = p.n_waypoints; D.wp_radius2 = (float)((double)p.wp_radius * p.wp_radius);
     for (int i = 0; i < 24; ++i) D.waypoints[i] = p.waypoints[i];
@@ -317,7 +319,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (action_type < 0 || action_type > MDG_ACT_ATTITUDE) return fail(MDG_EINVAL, "mdg_create: unknown action_type");
     if (p.ctrl_freq < 1 || p.sim_freq < p.ctrl_freq || p.sim_freq % p.ctrl_freq)
         return fail(MDG_EINVAL, "mdg_create: sim_freq must be a positive integer multiple of ctrl_freq (PAPER.md:169)");
-    if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || p.wp_laps < 0 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
+    if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || p.motor_lag_lo < 0 || p.motor_lag_hi < p.motor_lag_lo || p.wp_laps < 0 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))
@@ -344,14 +346,14 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     // The first 2 MiB of the allocation stay unused: the latency-bound configs ran 30-45 % slower (config 4: 9.3 vs 6.6 us
     // per step) with the buffers at the very start of the cudaMalloc block - measured, mechanism not identified.
     const size_t front_pad = (size_t)2 << 20;
-    h->arena_bytes = front_pad + rd + 11 * plane + 2 * eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
+    h->arena_bytes = front_pad + rd + 12 * plane + 2 * eplane + gs + ob + rw + dn + 256 + al(n_items_max * 4);
     cudaError_t ce = cudaMalloc(&h->arena, h->arena_bytes);
     if (ce != cudaSuccess) { delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc: ") + cudaGetErrorString(ce)); }
     ce = cudaMemset(h->arena, 0, h->arena_bytes);
     if (ce != cudaSuccess) { cudaFree(h->arena); delete h; return fail(MDG_ECUDA, std::string("mdg_create: cudaMemset: ") + cudaGetErrorString(ce)); }
     char* c = (char*)h->arena + front_pad;
-    float4** planes[11] = {&h->B.P0, &h->B.P1, &h->B.P2, &h->B.P3, &h->B.P4, &h->B.P5, &h->B.P6, &h->B.R0, &h->B.R1, &h->B.R2, &h->B.R3};
-    for (int i = 0; i < 11; ++i) { *planes[i] = (float4*)c; c += plane; }
+    float4** planes[12] = {&h->B.P0, &h->B.P1, &h->B.P2, &h->B.P3, &h->B.P4, &h->B.P5, &h->B.P6, &h->B.R0, &h->B.R1, &h->B.R2, &h->B.R3, &h->B.N0};
+    for (int i = 0; i < 12; ++i) { *planes[i] = (float4*)c; c += plane; }
     h->B.E0 = (float4*)c; c += eplane;
     h->B.E1 = (float4*)c; c += eplane;
     h->B.gstep = (uint32_t*)c; c += gs;

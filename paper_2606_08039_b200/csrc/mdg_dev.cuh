@@ -20,6 +20,7 @@ enum : int {
     F_AXISYM = 1 << 19,                                   // J_xx == J_yy: no gyroscopic term about body z
     F_CF2P = 1 << 20,                                     // +-configuration mixing
     F_DR = 1 << 21,                                       // per-episode domain-randomisation factors (Table 4)
+    F_MLAG = 1 << 23,                                     // motor lag: rotor-speed state, wrench recomputed every substep
     F_WIND_MIX = 1 << 22,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
 };
 
@@ -62,6 +63,7 @@ struct DevParams {
     int n_waypoints, wp_total; float waypoints[24], wp_radius2, wp_bonus, wp_shaping, wp_speed, wp_omega;   // waypoint tasks
     float dr_alpha[12];                                   // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g, motor, arm, max_rpm, -]
     float reset_rpy_half[3], reset_vel_half[3];           // Table 4 "init" row
+    float motor_lag_lo, motor_lag_hi;                     // Table 4 motor lag: range of the time constant (s)
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 
@@ -77,7 +79,8 @@ struct DevBuffers {
     float4* R0;   // DR factors m J k_f k_m
     float4* R1;   // DR factors drag gnd dw g
     float4* R2;   // DR per-motor thrust bias
-    float4* R3;   // DR arm, MAX_RPM, -, -
+    float4* R3;   // DR arm, MAX_RPM, motor-lag time constant, -
+    float4* N0;   // rotor speeds actually turning (motor lag state)
     float4* E0;   // wind x y z, bits(ep_step)
     float4* E1;   // running gust impulse: velocity x y z, progress s (>= 1: none)
     uint32_t* gstep;

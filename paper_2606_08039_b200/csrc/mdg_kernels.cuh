@@ -289,18 +289,33 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         const float nmax = P.max_rpm * dr3.y;
         n[0] = fminf(n[0], nmax); n[1] = fminf(n[1], nmax); n[2] = fminf(n[2], nmax); n[3] = fminf(n[3], nmax);
     }
-    const float f0 = (dr ? kf_e * dr2.x : kf_e) * (n[0] * n[0]), f1 = (dr ? kf_e * dr2.y : kf_e) * (n[1] * n[1]),
-                f2 = (dr ? kf_e * dr2.z : kf_e) * (n[2] * n[2]), f3 = (dr ? kf_e * dr2.w : kf_e) * (n[3] * n[3]);
-    const float T = (f0 + f1) + (f2 + f3);
-    const float arm_e = dr ? dr3.x : 1.0f;
-    V3 tau_b = F::has(P, F_CF2P) ? v3(P.arm * (f1 - f3), P.arm * (f2 - f0), kappa_e * ((f1 + f3) - (f0 + f2)))
-                                 : v3(P.l * ((f0 + f1) - (f2 + f3)), P.l * ((f1 + f2) - (f0 + f3)), kappa_e * ((f1 + f3) - (f0 + f2)));
-    if (dr) { tau_b.x *= inv_sJ * arm_e; tau_b.y *= inv_sJ * arm_e; tau_b.z *= inv_sJ; }
-    const float Om = P.rpm2rad * ((n[0] + n[1]) + (n[2] + n[3]));
-    const V3 k1_tau = v3(P.invJ[0] * tau_b.x, P.invJ[1] * tau_b.y, P.invJ[2] * tau_b.z);
-    const float cxy = (dr ? -P.c_xy * dr1.x : -P.c_xy) * Om, cz = (dr ? -P.c_z * dr1.x : -P.c_z) * Om;
-    const float gndT = (dr ? P.gnd_coef * dr1.y : P.gnd_coef) * T;
-    const float dcz = cz - cxy;
+    // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag
+    float T, cxy, dcz, gndT;
+    V3 tau_b, k1_tau;
+    auto motor_model = [&](const float (&nn)[4]) {
+        const float f0 = (dr ? kf_e * dr2.x : kf_e) * (nn[0] * nn[0]), f1 = (dr ? kf_e * dr2.y : kf_e) * (nn[1] * nn[1]),
+                    f2 = (dr ? kf_e * dr2.z : kf_e) * (nn[2] * nn[2]), f3 = (dr ? kf_e * dr2.w : kf_e) * (nn[3] * nn[3]);
+        T = (f0 + f1) + (f2 + f3);
+        const float arm_e = dr ? dr3.x : 1.0f;
+        tau_b = F::has(P, F_CF2P) ? v3(P.arm * (f1 - f3), P.arm * (f2 - f0), kappa_e * ((f1 + f3) - (f0 + f2)))
+                                  : v3(P.l * ((f0 + f1) - (f2 + f3)), P.l * ((f1 + f2) - (f0 + f3)), kappa_e * ((f1 + f3) - (f0 + f2)));
+        if (dr) { tau_b.x *= inv_sJ * arm_e; tau_b.y *= inv_sJ * arm_e; tau_b.z *= inv_sJ; }
+        const float Om = P.rpm2rad * ((nn[0] + nn[1]) + (nn[2] + nn[3]));
+        k1_tau = v3(P.invJ[0] * tau_b.x, P.invJ[1] * tau_b.y, P.invJ[2] * tau_b.z);
+        cxy = (dr ? -P.c_xy * dr1.x : -P.c_xy) * Om;
+        const float cz = (dr ? -P.c_z * dr1.x : -P.c_z) * Om;
+        gndT = (dr ? P.gnd_coef * dr1.y : P.gnd_coef) * T;
+        dcz = cz - cxy;
+    };
+    // Table 4 motor lag (Q44): the rotors follow n through a first-order lag sampled exactly per substep
+    const bool lag = F::has(P, F_MLAG);
+    float n_act[4] = {n[0], n[1], n[2], n[3]};
+    float lag_gain = 1.0f;
+    if (lag) {
+        const float4 r = B.N0[drone];
+        n_act[0] = r.x; n_act[1] = r.y; n_act[2] = r.z; n_act[3] = r.w;
+        lag_gain = 1.0f - __expf(-P.h / dr3.z);
+    } else motor_model(n);
 
     bool hit = false;
     const bool flush = pending2 != 0xFFFFFFFFu;                  // two items wait: fence now, flags after the substeps
@@ -308,6 +323,11 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     MDG_T(2);
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
+        if (lag) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) n_act[i] = fmaf(lag_gain, n[i] - n_act[i], n_act[i]);
+            motor_model(n_act);
+        }
         // S4-S7 world-frame force from the start-of-substep state
         // b = R(q) z: thrust is T b, and Eq.5's R diag(c_xy, c_xy, c_z) R^T v = c_xy v + (c_z - c_xy)(b.v) b
         const V3 b = v3(2.0f * fmaf(d.q.x, d.q.z, d.q.w * d.q.y), 2.0f * fmaf(d.q.y, d.q.z, -d.q.w * d.q.x),
@@ -470,6 +490,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                 float4 n0, n1, n2, n3;
                 draw_dr(P, e, (uint32_t)jj, t, n0, n1, n2, n3);
                 if (active) { B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3; }
+                if (lag) n_act[0] = n_act[1] = n_act[2] = n_act[3] = P.hover_rpm;
             }
             env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
             eta = euler_zyx(d.q);                                 // zeros unless Table 4's initial attitude range is on
@@ -491,6 +512,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         }
         write_obs<G>(P, B.obs, drone, d, eta, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
         B.reward_d[drone] = r;
+        if (lag) B.N0[drone] = make_float4(n_act[0], n_act[1], n_act[2], n_act[3]);
         if (j == 0) {
             env4.w = __uint_as_float(ep_out);
             B.E0[e] = env4; B.gstep[e] = t;
@@ -533,6 +555,7 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     float4 n0 = make_float4(1, 1, 1, 1), n1 = n0, n2 = n0, n3 = n0;
     if (P.feat & F_DR) draw_dr(P, e, (uint32_t)jj, 0u, n0, n1, n2, n3);
     B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3;
+    B.N0[drone] = make_float4(P.hover_rpm, P.hover_rpm, P.hover_rpm, P.hover_rpm);
     write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), tg);
     B.reward_d[drone] = 0.0f;
     if (j == 0) B.E1[e] = make_float4(0, 0, 0, 1.0f);

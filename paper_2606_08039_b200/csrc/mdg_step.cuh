@@ -97,7 +97,8 @@ __device__ __forceinline__ void draw_dr(const DevParams& P, uint32_t e, uint32_t
     r0 = make_float4(f(P.dr_alpha[0], a.x), f(P.dr_alpha[1], a.y), f(P.dr_alpha[2], a.z), f(P.dr_alpha[3], a.w));
     r1 = make_float4(f(P.dr_alpha[4], b.x), f(P.dr_alpha[5], b.y), f(P.dr_alpha[6], b.z), f(P.dr_alpha[7], g.x));
     r2 = make_float4(f(P.dr_alpha[8], c.x), f(P.dr_alpha[8], c.y), f(P.dr_alpha[8], c.z), f(P.dr_alpha[8], c.w));
-    r3 = make_float4(f(P.dr_alpha[9], d.x), f(P.dr_alpha[10], d.y), 1.0f, 1.0f);
+    r3 = make_float4(f(P.dr_alpha[9], d.x), f(P.dr_alpha[10], d.y),
+                     P.motor_lag_hi > 0.0f ? fmaf(P.motor_lag_hi - P.motor_lag_lo, u01(d.z), P.motor_lag_lo) : 1.0f, 1.0f);
 }
 
 // Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376)

@@ -117,6 +117,13 @@ CASES = {
                             ("uniform", -1.0, 1.0)), {}),
     # MultiHoverAviary as the paper tabulates it: 13 floats per drone (kinematic state + target altitude), normalised RPM
     "m3_multi_hover_obs13": (wl("m3mh", 700, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM_NORM, dict(GRID, obs_mode=W.OBS_KIN12_Z), ("uniform", -0.1, 0.12)), {}),
+    # Table 4 motor lag: rotor-speed state, wrench recomputed every substep; alone under PID, and with everything else on
+    "m1_motor_lag_pid": (wl("m1lag", 1500, 1, W.PHYS_MJC, W.ACT_PID,
+                            dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST,
+                                 term_tilt=0.4, term_dist=3.0, target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
+                                 episode_len_s=0.5, auto_reset=1, motor_lag_lo=0.005, motor_lag_hi=0.05), ("targets",)), {}),
+    "m4_motor_lag_dr_all_aero": (wl("m4lag", 700, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
+                                    dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR, motor_lag_lo=0.005, motor_lag_hi=0.05, **INIT), HOVER), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
