@@ -7,7 +7,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "oracle_capi.cpp")]
-DEPS = SRC + [os.path.join(HERE, "drone_oracle.hpp"), os.path.join(HERE, "philox_ref.hpp")]
+DEPS = SRC + [os.path.join(HERE, "drone_oracle.hpp"), os.path.join(HERE, "philox_ref.hpp"),
+               os.path.join(HERE, "camera_oracle.hpp")]
 OUT = os.path.join(HERE, "liboracle.so")
 
 

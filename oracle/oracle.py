@@ -49,6 +49,7 @@ def lib():
         L.orc_philox.argtypes = [C.c_uint32] * 6 + [C.c_void_p]
         L.orc_wind_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
         L.orc_gen_actions.argtypes = [C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_uint32]
+        L.orc_render_depth.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
     return _lib
 
 
@@ -277,3 +278,25 @@ def gen_actions(seed, t, n_envs, n_drones, base, lo, hi, env_base=0):
     out = np.zeros((n_envs * n_drones, 4), dtype=np.float32)
     lib().orc_gen_actions(int(seed), int(t), n_envs, n_drones, float(base), float(lo), float(hi), _p(out), int(env_base))
     return out
+
+
+# NEXT-4 camera (camera_oracle.hpp; readings Q45-Q48).  body_a = arm + propeller radius of CF2X (Table 2), body_c = reading Q46.
+CAM_DEFAULTS = dict(H=48, W=64, fovy_deg=60.0, offset=(0.02, 0.0, 0.0), znear=0.01, zfar=50.0, body_a=0.0397 + 0.02325, body_c=0.0125)
+
+
+def render_depth(state, n_envs, n_drones, n_threads=1, with_margin=False, **cam):
+    """Depth [D, H, W] float64 and segmentation [D, H, W] u8 of every drone's camera from state [D, 13] (float64)."""
+    c = dict(CAM_DEFAULTS)
+    for k in cam:
+        if k not in c:
+            raise KeyError(k)
+    c.update(cam)
+    st = _f64(state).reshape(n_envs * n_drones, 13)
+    H, W = int(c["H"]), int(c["W"])
+    vec = np.array([H, W, c["fovy_deg"], *c["offset"], c["znear"], c["zfar"], c["body_a"], c["body_c"]], dtype=np.float64)
+    D = n_envs * n_drones
+    depth = np.empty((D, H, W), np.float64)
+    seg = np.empty((D, H, W), np.uint8)
+    margin = np.empty((D, H, W), np.float64) if with_margin else None
+    lib().orc_render_depth(_p(st), n_envs, n_drones, _p(vec), _p(depth), _p(seg), _p(margin) if with_margin else None, int(n_threads))
+    return (depth, seg, margin) if with_margin else (depth, seg)
