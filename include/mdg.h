@@ -6,7 +6,8 @@
  * drag / downwash (Eq.4-6), wind (Dryden-style gust, constant, impulse gusts,
  * sinusoidal), per-episode domain randomisation (Table 4), free-body integration over
  * sim_freq/ctrl_freq substeps, observation, reward, termination and
- * auto-reset.  The interface follows the paper's statement of the
+ * auto-reset, and, as a separate call, the onboard depth / segmentation camera
+ * (PAPER.md:177).  The interface follows the paper's statement of the
  * simulator: constructor options, `reset(rng) -> state`,
  * `step(state, action) -> state, obs, reward, done`.
  *
@@ -184,6 +185,32 @@ int mdg_reward_per_drone(mdg_env* env, const float** reward_dev);
  * mdg_set_dr fails with MDG_EINVAL when every dr_alpha is 0 (the factors are then not read by the step). */
 int mdg_get_dr(mdg_env* env, float* factors);
 int mdg_set_dr(mdg_env* env, const float* factors);
+
+/* Onboard depth / segmentation camera (48 x 64 frames from each drone's 60-degree-FOV camera positioned at
+ * [0.02, 0, 0] in the body frame; PAPER.md:13 lists RGB / depth / segmentation).  The paper renders with mujoco.Renderer
+ * (OpenGL, unavailable here); this is a CUDA ray caster over analytic primitives (DESIGN.md readings
+ * Q45-Q48): the floor plane z = 0 seen from above and every OTHER drone of the same env as an oblate spheroid with semi-axes
+ * (body_radius, body_radius, body_half_height) in its body frame, front faces only.  Optical axis = body +x, image right =
+ * body -y, image up = body +z; fovy_deg is the vertical field of view; pixel (r, c), row 0 at the top, looks along the body
+ * direction (1, -(c + 1/2 - width/2) s, -(r + 1/2 - height/2) s), s = 2 tan(fovy/2) / height. */
+typedef struct mdg_cam_params {
+    uint32_t struct_size;           /* must equal sizeof(mdg_cam_params) (set by mdg_default_cam_params) */
+    int32_t height, width;          /* 48, 64; width must be a multiple of 4 */
+    float fovy_deg, offset[3];      /* 60; (0.02, 0, 0) m in the body frame */
+    float znear, zfar;              /* 0.01, 50 m: hits outside [znear, zfar) are discarded */
+    float body_radius, body_half_height;   /* arm + propeller radius of the drone model; 0.0125 m */
+} mdg_cam_params;
+
+/* Fill *out with the defaults above; params (host, may be NULL = CF2X) supplies arm length and propeller radius. */
+int mdg_default_cam_params(const mdg_params* params, mdg_cam_params* out);
+
+/* Render every drone's camera from the CURRENT state (after the last reset / step on the bound stream; asynchronous on it).
+ * cam: host pointer, NULL = defaults for the handle's drone model.  depth_dev: [n_envs*n_drones][height][width] fp32, distance
+ * along the optical axis in metres, zfar where nothing is hit; caller-owned device memory, 16-byte aligned.  seg_dev: same
+ * shape, u8: 0 background, 1 floor, 2 + k drone k of the env; caller-owned, 4-byte aligned.  Either may be NULL (not written).
+ * MDG_EINVAL on a NULL handle, both outputs NULL, misaligned pointers, width % 4 != 0, non-positive sizes, fovy outside
+ * (0, 180), znear <= 0 or zfar <= znear, non-positive body axes. */
+int mdg_render_depth(mdg_env* env, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev);
 
 /* Scheduling note for mdg_step: the step is launched with programmatic dependent launch.  When the previous
  * operation on the handle was a step on the same stream, the new launch does not wait for that kernel as a whole but,

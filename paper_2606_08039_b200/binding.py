@@ -50,9 +50,17 @@ class mdg_params(C.Structure):
         return self
 
 
+class mdg_cam_params(C.Structure):
+    """Mirror of `struct mdg_cam_params` (include/mdg.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("height", C.c_int32), ("width", C.c_int32), ("fovy_deg", C.c_float),
+                ("offset", C.c_float * 3), ("znear", C.c_float), ("zfar", C.c_float),
+                ("body_radius", C.c_float), ("body_half_height", C.c_float)]
+    update = mdg_params.update
+
+
 EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
-           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_last_error", "mdg_version"]
+           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_last_error", "mdg_version"]
 
 _lib = None
 
@@ -91,6 +99,8 @@ def lib():
         L.mdg_set_launch.argtypes = [vp, C.c_int, C.c_int]
         L.mdg_last_error.restype = C.c_char_p
         L.mdg_measure_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
+        L.mdg_default_cam_params.argtypes = [PP, C.POINTER(mdg_cam_params)]
+        L.mdg_render_depth.argtypes = [vp, C.POINTER(mdg_cam_params), vp, vp]
         _lib = L
     return _lib
 
@@ -119,6 +129,12 @@ def default_params(drone_model=0, **overrides) -> mdg_params:
     p = mdg_params()
     _check(lib().mdg_default_params(drone_model, C.byref(p)))
     return p.update(overrides)
+
+
+def default_cam_params(params: mdg_params = None, **overrides) -> mdg_cam_params:
+    c = mdg_cam_params()
+    _check(lib().mdg_default_cam_params(C.byref(params) if params is not None else None, C.byref(c)))
+    return c.update(overrides)
 
 
 class _DevArray:
@@ -213,6 +229,23 @@ class Env:
             out = self._torch.empty((self.n_envs * self.n_drones, 4), dtype=self._torch.float32, device=self.obs.device)
         _check(lib().mdg_gen_actions(self._h, int(seed), int(t), float(base), float(lo), float(hi), C.c_void_p(out.data_ptr())))
         return out
+
+    def render_depth(self, cam: mdg_cam_params = None, depth=None, seg=None, want_depth=True, want_seg=True):
+        """Every drone's onboard camera from the current state (include/mdg.h: mdg_render_depth): depth [D, H, W] float32 and
+        segmentation [D, H, W] uint8 CUDA tensors (allocated here unless passed in)."""
+        t = self._torch
+        c = cam if cam is not None else default_cam_params(self.params)
+        shape = (self.n_envs * self.n_drones, c.height, c.width)
+        if depth is None and want_depth:
+            depth = t.empty(shape, dtype=t.float32, device=self.obs.device)
+        if seg is None and want_seg:
+            seg = t.empty(shape, dtype=t.uint8, device=self.obs.device)
+        for x, dt in ((depth, t.float32), (seg, t.uint8)):
+            if x is not None and not (x.is_cuda and x.dtype == dt and x.is_contiguous() and tuple(x.shape) == shape):
+                raise ValueError(f"camera outputs must be contiguous CUDA tensors of shape {shape}")
+        _check(lib().mdg_render_depth(self._h, C.byref(c), C.c_void_p(depth.data_ptr() if depth is not None else None),
+                                      C.c_void_p(seg.data_ptr() if seg is not None else None)))
+        return depth, seg
 
     def get_state(self):
         import numpy as np

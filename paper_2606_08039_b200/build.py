@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libmdg.so")
 SOURCES = [os.path.join(CSRC, "mdg.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mdg_dev.cuh", "mdg_step.cuh", "mdg_kernels.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mdg_dev.cuh", "mdg_step.cuh", "mdg_kernels.cuh", "mdg_camera.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "mdg.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -12,6 +12,7 @@
 
 #include "../../include/mdg.h"
 #include "mdg_kernels.cuh"
+#include "mdg_camera.cuh"
 
 using namespace mdg;
 
@@ -459,6 +460,49 @@ int mdg_gen_actions(mdg_env* h, uint64_t seed, uint32_t t, float base, float lo,
     const size_t D = (size_t)h->N * h->M;
     gen_actions_kernel<<<(unsigned)((D + 255) / 256), 256, 0, h->stream>>>(D, h->M, h->P.env_base, (uint32_t)seed, (uint32_t)(seed >> 32), t, base, lo, hi,
                                                                               reinterpret_cast<float4*>(out_dev));
+    CU(cudaGetLastError());
+    h->launches += 1;
+    return MDG_OK;
+}
+
+int mdg_default_cam_params(const mdg_params* params, mdg_cam_params* out) {
+    if (!out) return fail(MDG_EINVAL, "mdg_default_cam_params: NULL argument");
+    mdg_params cf2x;
+    if (!params) { const int rc = mdg_default_params(MDG_MODEL_CF2X, &cf2x); if (rc != MDG_OK) return rc; params = &cf2x; }
+    std::memset(out, 0, sizeof(*out));
+    out->struct_size = sizeof(mdg_cam_params);
+    out->height = 48; out->width = 64; out->fovy_deg = 60.0f;
+    out->offset[0] = 0.02f; out->offset[1] = 0.0f; out->offset[2] = 0.0f;
+    out->znear = 0.01f; out->zfar = 50.0f;                                    // reading Q47
+    out->body_radius = params->L + params->r_p; out->body_half_height = 0.0125f;   // reading Q46
+    return MDG_OK;
+}
+
+int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev) {
+    if (!h) return fail(MDG_EINVAL, "mdg_render_depth: NULL handle");
+    mdg_cam_params def;
+    if (!cam) { const int rc = mdg_default_cam_params(&h->hp, &def); if (rc != MDG_OK) return rc; cam = &def; }
+    if (cam->struct_size != sizeof(mdg_cam_params)) return fail(MDG_EINVAL, "mdg_render_depth: struct_size mismatch");
+    if (!depth_dev && !seg_dev) return fail(MDG_EINVAL, "mdg_render_depth: both outputs NULL");
+    if (((uintptr_t)depth_dev & 15) || ((uintptr_t)seg_dev & 3)) return fail(MDG_EINVAL, "mdg_render_depth: depth_dev must be 16-byte, seg_dev 4-byte aligned");
+    if (cam->height < 1 || cam->width < 4 || (cam->width & 3) || (int64_t)cam->height * cam->width > (1 << 24))
+        return fail(MDG_EINVAL, "mdg_render_depth: height >= 1, width a positive multiple of 4, height*width <= 2^24");
+    if (!(cam->fovy_deg > 0.0f && cam->fovy_deg < 180.0f) || !(cam->znear > 0.0f) || !(cam->zfar > cam->znear) ||
+        !(cam->body_radius > 0.0f) || !(cam->body_half_height > 0.0f))
+        return fail(MDG_EINVAL, "mdg_render_depth: fovy in (0, 180), 0 < znear < zfar and positive body axes required");
+    CamDev C;
+    C.H = cam->height; C.W = cam->width; C.groups_per_row = cam->width / 4; C.n_groups = C.H * C.groups_per_row;
+    C.s = (float)(2.0 * std::tan(0.5 * (double)cam->fovy_deg * 3.14159265358979323846 / 180.0) / cam->height);
+    C.half_h = 0.5f * cam->height; C.half_w = 0.5f * cam->width; C.inv_gpr = 1.0f / (float)C.groups_per_row;
+    for (int i = 0; i < 3; ++i) C.off[i] = cam->offset[i];
+    C.znear = cam->znear; C.zfar = cam->zfar;
+    C.rb = std::fmax(cam->body_radius, cam->body_half_height);
+    C.inv_a = (float)(1.0 / (double)cam->body_radius); C.inv_c = (float)(1.0 / (double)cam->body_half_height);
+    const int n_cams = h->N * h->M;
+    const unsigned grid = (unsigned)((n_cams + CAM_WARPS - 1) / CAM_WARPS);
+    const size_t smem = (size_t)CAM_WARPS * h->M * sizeof(CamCand);
+    h->chainable = false;                    // a later step must order itself behind this reader as a whole
+    render_depth_kernel<<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
     CU(cudaGetLastError());
     h->launches += 1;
     return MDG_OK;

@@ -79,3 +79,27 @@ def hover_rpm_f32(m=0.027, g=9.81, k_f=3.16e-10):
     """Harness scale for ("hover_scale", ...) actions: the CF2X hover rotor speed rounded to fp32."""
     import struct
     return struct.unpack("f", struct.pack("f", math.sqrt(m * g / (4.0 * k_f))))[0]
+
+
+def camera_scene(seed, n_envs, n_drones, radius=0.6):
+    """Seeded input for the onboard-camera call: state rows [D, 13] float32 with the env's drones
+    on a circle of the given radius at heights U[0.05, 1.4], each yawed towards the centre +- 0.5 rad with roll / pitch
+    U(+-0.35), so that every camera sees floor, sky and some of the other drones (formation flight seen from inside).
+    A tenth of the drones sit on the floor (z = 0), whose camera origin may dip below it.  Velocities are zero."""
+    import numpy as np
+    rng = np.random.Generator(np.random.Philox(seed))
+    D = n_envs * n_drones
+    i = np.tile(np.arange(n_drones), n_envs)
+    ang = 2 * math.pi * i / max(n_drones, 1) + rng.uniform(-0.25, 0.25, D)
+    r = radius * rng.uniform(0.5, 1.5, D)
+    z = np.where(rng.uniform(size=D) < 0.1, 0.0, rng.uniform(0.05, 1.4, D))
+    roll, pitch = rng.uniform(-0.35, 0.35, D), rng.uniform(-0.35, 0.35, D)
+    yaw = ang + math.pi + rng.uniform(-0.5, 0.5, D)
+    cr, sr, cp, sp, cy, sy = np.cos(roll / 2), np.sin(roll / 2), np.cos(pitch / 2), np.sin(pitch / 2), np.cos(yaw / 2), np.sin(yaw / 2)
+    st = np.zeros((D, 13), dtype=np.float32)
+    st[:, 0], st[:, 1], st[:, 2] = r * np.cos(ang), r * np.sin(ang), z
+    st[:, 3] = cr * cp * cy + sr * sp * sy          # ZYX Euler angles -> unit quaternion (w, x, y, z)
+    st[:, 4] = sr * cp * cy - cr * sp * sy
+    st[:, 5] = cr * sp * cy + sr * cp * sy
+    st[:, 6] = cr * cp * sy - sr * sp * cy
+    return st

@@ -77,6 +77,6 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in txt.lower() or f in ("workloads.py", "mdg_dev.cuh", "__init__.py"), f
-    for f in ("drone_oracle.hpp", "oracle_capi.cpp", "philox_ref.hpp", "oracle.py"):
+    for f in ("drone_oracle.hpp", "camera_oracle.hpp", "oracle_capi.cpp", "philox_ref.hpp", "oracle.py"):
         txt = open(os.path.join(ROOT, "oracle", f)).read()
         assert "paper_2606_08039_b200" not in txt.replace("paper_2606_08039_b200/csrc", "") and "mdg.h\"" not in txt
