@@ -120,6 +120,52 @@ def oracle_throughput(wl, budget_s, n_envs, min_steps=4, max_steps=10 ** 9):
                 flops_per_drone_step=flops, ms_per_step=1e3 * dt / steps, steps=steps)
 
 
+def camera_leg(stream, hbm_peak, n_envs=16384, n_drones=4, reps=20, cpu_envs=24):
+    """Secondary measurement: mdg_render_depth, every drone's 48 x 64 depth + segmentation frame.
+    16,384 envs x 4 drones = 65,536 frames = 1.0 GB of output per call (> 126 MB L2, so every call's stores reach HBM).
+    Algorithmic bytes per frame: H W (4 + 1) written + the drone's 32-byte pose read."""
+    import torch
+    import numpy as np
+    import paper_2606_08039_b200 as mdg
+    with torch.cuda.stream(stream):
+        env = mdg.Env(n_envs, n_drones, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, auto_reset=0, term_mode=W.TERM_NONE), stream=stream)
+        env.reset(1)
+        st = W.camera_scene(W.BASE_SEED + 99, n_envs, n_drones)
+        env.set_state(state=st)
+        depth, seg = env.render_depth()
+        for _ in range(3):
+            env.render_depth(depth=depth, seg=seg)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            env.render_depth(depth=depth, seg=seg)
+        e1.record(stream)
+        stream.synchronize()
+    sec = e0.elapsed_time(e1) / 1e3 / reps
+    frames = n_envs * n_drones
+    byt = frames * (48 * 64 * 5 + 32)
+    out = {"workload": f"{n_envs} envs x {n_drones} drones, one 48 x 64 depth (fp32) + segmentation (u8) frame per drone, formation-circle scenes",
+           "frames_per_sec": frames / sec, "us_per_call": sec * 1e6, "gpu_launches": reps,
+           "roofline": {"bound": "hbm", "achieved": byt / sec / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": byt / sec / 1e9 / hbm_peak,
+                        "traffic": None, "kernel": "render_depth_kernel", "bytes_per_launch": byt}}
+    try:
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv"))):
+            if row["config"] == "camera":
+                out["roofline"]["traffic"] = float(row["traffic_bytes"])
+    except Exception:
+        pass
+    from oracle import oracle as O
+    cores = len(os.sched_getaffinity(0))
+    sub = st[: cpu_envs * n_drones].astype(np.float64)
+    t0 = time.perf_counter()
+    O.render_depth(sub, cpu_envs, n_drones, n_threads=cores)
+    dt = time.perf_counter() - t0
+    out["cpu_baseline"] = {"value": cpu_envs * n_drones / dt, "unit": "frames/s", "cores": cores, "kind": "oracle",
+                           "sample": f"{cpu_envs} envs x {n_drones} drones of the same scenes (float64, {cores} threads, {dt:.2f} s)"}
+    return out
+
+
 def run_reference(args, wl, c):
     """`--impl reference`: the oracle on the host cores, same metric/config; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -279,6 +325,10 @@ def run_ours(args, wl, c):
             "gpu_launches": launches, "clocks": clocks}
     if cpu:
         line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    if world == 1 and not args.no_camera:
+        del envs, acts
+        torch.cuda.empty_cache()
+        line["camera"] = camera_leg(stream, hbm_peak)
     print(json.dumps(line), flush=True)
     if dist:
         dist.destroy_process_group()
@@ -296,6 +346,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-camera", action="store_true", help="skip the secondary onboard-camera measurement")
     args = ap.parse_args()
     wl = W.config(args.config)
     if args.impl == "reference":

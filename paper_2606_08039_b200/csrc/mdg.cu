@@ -502,7 +502,8 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
     const unsigned grid = (unsigned)((n_cams + CAM_WARPS - 1) / CAM_WARPS);
     const size_t smem = (size_t)CAM_WARPS * h->M * sizeof(CamCand);
     h->chainable = false;                    // a later step must order itself behind this reader as a whole
-    render_depth_kernel<<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
+    if (depth_dev && seg_dev) render_depth_kernel<true><<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
+    else render_depth_kernel<false><<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
     CU(cudaGetLastError());
     h->launches += 1;
     return MDG_OK;

@@ -4,16 +4,12 @@
 // plane z = 0 and every other drone of the env as an oblate spheroid.  Product code.
 //
 // Mapping.  One warp per camera, no block-level synchronisation.  Lanes 0..M-1 prepare one candidate primitive each
-// (the ray origin and the three columns of S R_k^T R_i in the spheroid's unit-sphere frame, and a conservative pixel
+// (per-candidate constants of the ray / unit-sphere test in the spheroid's own scaled frame, and a conservative pixel
 // bounding box from the bounding sphere); candidates that can be seen are compacted into the warp's shared-memory list.
 // Then the 32 lanes sweep the image, four horizontally adjacent pixels per lane and iteration, so a warp stores 512
-// contiguous bytes of depth (float4 per lane) and 128 of segmentation (uchar4 per lane) at a time: the kernel is bound
-// by those HBM writes (H W 5 bytes per camera against 32 M bytes of state read).  A spheroid is only intersected for
-// pixel groups inside its bounding box, so the common pixel costs the floor test alone.
-//
-// Arithmetic.  The quadratic is solved around the point of closest approach (t_c = -B/A, v = o + t_c d, hit iff |v| < 1,
-// t = t_c - sqrt((1 - |v|^2)/A)), which keeps fp32 accurate when the camera is hundreds of radii away (the textbook
-// discriminant B^2 - A C cancels catastrophically there).
+// contiguous bytes of depth (float4 per lane) and 128 of segmentation (packed u8 x 4 per lane) at a time: the kernel is
+// bound by those HBM writes (H W 5 bytes per camera against 32 M bytes of state read).  Spheroids are only intersected
+// inside their bounding boxes (see TWO_PASS below), so the common pixel costs the floor test alone.
 #pragma once
 #include "mdg_dev.cuh"
 
@@ -25,10 +21,12 @@ struct CamDev {
     float off[3], znear, zfar, rb, inv_a, inv_c;   // rb: radius of the bounding sphere = the larger semi-axis
 };
 
-struct __align__(16) CamCand {                            // one visible spheroid, in its unit-sphere frame
-    float ox, oy, oz;                       // ray origin
-    float m0x, m0y, m0z, m1x, m1y, m1z, m2x, m2y, m2z;   // image of the camera axes (forward, pixel-right * -1, pixel-up): d = m0 + y m1 + z m2
-    int4 box; int id;                       // inclusive pixel bounding box (r0, r1, c0, c1), segmentation id
+struct __align__(16) CamCand {              // one visible spheroid, in its unit-sphere frame (o = ray origin, d = m0 + y m1 + z m2)
+    float w0x, w0y, w0z, w1x, w1y, w1z, w2x, w2y, w2z;   // o x m0, o x m1, o x m2: o x d is linear in (y, z)
+    float c00, c01x2, c02x2, c11, c12x2, c22;             // m_a . m_b: |d|^2 is a quadratic in (y, z)
+    float b0, b1, b2;                                     // o . m_a
+    int id, pad;                                          // segmentation id
+    int4 box;                                             // inclusive pixel bounding box (r0, r1, c0, c1)
 };
 
 static constexpr int CAM_WARPS = 4;         // cameras per block
@@ -39,6 +37,28 @@ __device__ __forceinline__ void cam_rotmat(float w, float x, float y, float z, f
     R[2][0] = 2.0f * (x * z - w * y); R[2][1] = 2.0f * (y * z + w * x); R[2][2] = 1.0f - 2.0f * (x * x + y * y);
 }
 
+// Ray (1, y, z) of the camera against the unit sphere of candidate q.  The ray misses iff its distance from the centre,
+// |o x d| / |d|, exceeds 1; otherwise the front-face parameter is t = -(o.d)/|d|^2 - sqrt((|d|^2 - |o x d|^2)) / |d|^2.
+// Both |o x d|^2 and |d|^2 are evaluated from per-candidate constants (9 + 6 words), 14 FMA-class operations per pixel and
+// no MUFU on the miss path; every component of o x d is a difference of products formed once per candidate, so the test keeps
+// ~1e-5 relative accuracy hundreds of radii away where the textbook discriminant B^2 - A C cancels catastrophically in fp32.
+__device__ __forceinline__ bool cam_hit(const CamCand& q, float y, float z, float& t) {
+    const float wx = fmaf(y, q.w1x, fmaf(z, q.w2x, q.w0x)), wy = fmaf(y, q.w1y, fmaf(z, q.w2y, q.w0y)), wz = fmaf(y, q.w1z, fmaf(z, q.w2z, q.w0z));
+    const float ww = fmaf(wx, wx, fmaf(wy, wy, wz * wz));
+    const float A = fmaf(y, fmaf(y, q.c11, fmaf(z, q.c12x2, q.c01x2)), fmaf(z, fmaf(z, q.c22, q.c02x2), q.c00));
+    if (ww > A) return false;
+    const float rA = rcp_fast(A);
+    const float h2 = fmaxf((A - ww) * rA * rA, 1e-30f);
+    t = fmaf(-h2, rsqrt_fast(h2), -fmaf(y, q.b1, fmaf(z, q.b2, q.b0)) * rA);
+    return true;
+}
+
+// TWO_PASS (both outputs requested): the warp first sweeps the floor over the whole image, then visits each candidate's
+// bounding box with one lane per PIXEL and depth-tests against what it has just written (still in L2), so no lane idles
+// through a spheroid test that cannot concern it.  Otherwise (one output only) a single sweep tests each 4-pixel group
+// against the candidates whose box it touches.  Both use cam_hit and the same visiting order (floor, then drones by index;
+// strict "<"), so they produce identical images.
+template <bool TWO_PASS>
 __global__ void __launch_bounds__(CAM_WARPS * 32)
 render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1, int n_cams, int M, const CamDev C,
                     float* __restrict__ depth, uint8_t* __restrict__ seg) {
@@ -84,18 +104,22 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
         if (vis) {
             // unit-sphere frame of spheroid k: x' = S R_k^T (x - p_k), S = diag(1/a, 1/a, 1/c)
             const float sc[3] = {C.inv_a, C.inv_a, C.inv_c};
-            float o[3], m[3][3];
+            float o[3], m[3][3];                            // m[c] = image of camera axis c (forward, left, up)
 #pragma unroll
             for (int r = 0; r < 3; ++r) {
                 o[r] = (Rk[0][r] * rx + Rk[1][r] * ry + Rk[2][r] * rz) * sc[r];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) m[c][r] = (Rk[0][r] * Ri[0][c] + Rk[1][r] * Ri[1][c] + Rk[2][r] * Ri[2][c]) * sc[r];
             }
-            cd.ox = o[0]; cd.oy = o[1]; cd.oz = o[2];
-            cd.m0x = m[0][0]; cd.m0y = m[0][1]; cd.m0z = m[0][2];
-            cd.m1x = m[1][0]; cd.m1y = m[1][1]; cd.m1z = m[1][2];
-            cd.m2x = m[2][0]; cd.m2y = m[2][1]; cd.m2z = m[2][2];
-            cd.id = 2 + lane;
+            auto crs = [&](const float* v, float& x, float& y, float& z) {
+                x = o[1] * v[2] - o[2] * v[1]; y = o[2] * v[0] - o[0] * v[2]; z = o[0] * v[1] - o[1] * v[0];
+            };
+            auto dot = [](const float* u, const float* v) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; };
+            crs(m[0], cd.w0x, cd.w0y, cd.w0z); crs(m[1], cd.w1x, cd.w1y, cd.w1z); crs(m[2], cd.w2x, cd.w2y, cd.w2z);
+            cd.c00 = dot(m[0], m[0]); cd.c01x2 = 2.0f * dot(m[0], m[1]); cd.c02x2 = 2.0f * dot(m[0], m[2]);
+            cd.c11 = dot(m[1], m[1]); cd.c12x2 = 2.0f * dot(m[1], m[2]); cd.c22 = dot(m[2], m[2]);
+            cd.b0 = dot(o, m[0]); cd.b1 = dot(o, m[1]); cd.b2 = dot(o, m[2]);
+            cd.id = 2 + lane; cd.pad = 0;
         }
     }
     const unsigned ball = __ballot_sync(0xffffffffu, vis);
@@ -112,39 +136,53 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
         const float z = (C.half_h - 0.5f - (float)r) * C.s;      // -((r + 1/2) - H/2) s
         const float y0 = (C.half_w - 0.5f - (float)c4) * C.s;
         float y[4], best[4];
-        int id[4];
+        unsigned ids = 0;
         const float dz0 = fmaf(z, Ri[2][2], Ri[2][0]);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             y[j] = fmaf(-(float)j, C.s, y0);
             const float dz = fmaf(y[j], Ri[2][1], dz0);          // world z of the ray direction (1, y, z)
-            const float t = noz * rcp_fast(dz);                  // floor: o_z + t d_z = 0
-            const bool hit = dz < 0.0f && t >= C.znear && t < C.zfar;
-            best[j] = hit ? t : C.zfar; id[j] = hit ? 1 : 0;
+            const float t = noz * rcp_fast(dz);                  // floor: o_z + t d_z = 0; d_z >= 0 gives t <= 0 (or NaN): no hit
+            const bool hit = t >= C.znear && t < C.zfar;
+            best[j] = hit ? t : C.zfar; ids |= hit ? (1u << (8 * j)) : 0u;
         }
-        for (int k = 0; k < n_cand; ++k) {
-            const CamCand& q = cand[k];
-            const int4 bb = q.box;                               // r0, r1, c0, c1
-            if (r < bb.x || r > bb.y || c4 + 3 < bb.z || c4 > bb.w) continue;
-            const float bx = fmaf(z, q.m2x, q.m0x), by = fmaf(z, q.m2y, q.m0y), bz = fmaf(z, q.m2z, q.m0z);
+        if (!TWO_PASS) {
+            for (int k = 0; k < n_cand; ++k) {
+                const CamCand& q = cand[k];
+                const int4 bb = q.box;
+                if (r < bb.x || r > bb.y || c4 + 3 < bb.z || c4 > bb.w) continue;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const float dx = fmaf(y[j], q.m1x, bx), dy = fmaf(y[j], q.m1y, by), dzz = fmaf(y[j], q.m1z, bz);
-                const float A = fmaf(dx, dx, fmaf(dy, dy, dzz * dzz));
-                const float Bq = fmaf(q.ox, dx, fmaf(q.oy, dy, q.oz * dzz));
-                const float rA = rcp_fast(A);
-                const float tc = -Bq * rA;
-                const float vx = fmaf(tc, dx, q.ox), vy = fmaf(tc, dy, q.oy), vz = fmaf(tc, dzz, q.oz);
-                const float vv = fmaf(vx, vx, fmaf(vy, vy, vz * vz));
-                if (vv <= 1.0f) {
-                    const float h2 = fmaxf((1.0f - vv) * rA, 1e-30f);
-                    const float t = fmaf(-h2, rsqrt_fast(h2), tc);
-                    if (t >= C.znear && t < best[j]) { best[j] = t; id[j] = q.id; }
+                for (int j = 0; j < 4; ++j) {
+                    float t;
+                    if (cam_hit(q, y[j], z, t) && t >= C.znear && t < best[j]) { best[j] = t; ids = (ids & ~(0xffu << (8 * j))) | ((unsigned)q.id << (8 * j)); }
+                }
+            }
+            if (dcam) __stcs(reinterpret_cast<float4*>(dcam) + g, make_float4(best[0], best[1], best[2], best[3]));
+            if (scam) __stcs(reinterpret_cast<unsigned*>(scam) + g, ids);
+        } else {
+            reinterpret_cast<float4*>(dcam)[g] = make_float4(best[0], best[1], best[2], best[3]);
+            reinterpret_cast<unsigned*>(scam)[g] = ids;
+        }
+    }
+    if (TWO_PASS) {
+        for (int k = 0; k < n_cand; ++k) {
+            __syncwarp();                                        // orders the warp's earlier stores before the loads below
+            const CamCand& q = cand[k];
+            const int4 bb = q.box;
+            const int bw = bb.w - bb.z + 1, n_px = bw * (bb.y - bb.x + 1);
+            const float inv_bw = 1.0f / (float)bw;
+            for (int i = lane; i < n_px; i += 32) {
+                const int rr = (int)(((float)i + 0.5f) * inv_bw);
+                const int r = bb.x + rr, c = bb.z + (i - rr * bw);
+                const float z = (C.half_h - 0.5f - (float)r) * C.s;
+                const float y = fmaf(-(float)(c & 3), C.s, (C.half_w - 0.5f - (float)(c & ~3)) * C.s);   // as the sweep forms it
+                float t;
+                if (cam_hit(q, y, z, t) && t >= C.znear) {
+                    const int px = r * C.W + c;
+                    if (t < __ldcg(dcam + px)) { dcam[px] = t; scam[px] = (uint8_t)q.id; }
                 }
             }
         }
-        if (dcam) __stcs(reinterpret_cast<float4*>(dcam) + g, make_float4(best[0], best[1], best[2], best[3]));
-        if (scam) __stcs(reinterpret_cast<unsigned*>(scam) + g, (unsigned)id[0] | ((unsigned)id[1] << 8) | ((unsigned)id[2] << 16) | ((unsigned)id[3] << 24));
     }
 }
 
