@@ -497,6 +497,8 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
     for (int i = 0; i < 3; ++i) C.off[i] = cam->offset[i];
     C.znear = cam->znear; C.zfar = cam->zfar;
     C.rb = std::fmax(cam->body_radius, cam->body_half_height);
+    C.a2 = (float)((double)cam->body_radius * cam->body_radius);
+    C.dac = (float)((double)cam->body_half_height * cam->body_half_height - (double)cam->body_radius * cam->body_radius);
     C.inv_a = (float)(1.0 / (double)cam->body_radius); C.inv_c = (float)(1.0 / (double)cam->body_half_height);
     const int n_cams = h->N * h->M;
     const unsigned grid = (unsigned)((n_cams + CAM_WARPS - 1) / CAM_WARPS);

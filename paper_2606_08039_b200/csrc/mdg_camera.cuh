@@ -19,6 +19,7 @@ struct CamDev {
     int H, W, groups_per_row, n_groups;     // W / 4, H * W / 4
     float s, half_h, half_w, inv_gpr;       // pixel pitch on the image plane at unit distance; H/2, W/2; 1 / groups_per_row
     float off[3], znear, zfar, rb, inv_a, inv_c;   // rb: radius of the bounding sphere = the larger semi-axis
+    float a2, dac;                          // a^2, c^2 - a^2
 };
 
 struct __align__(16) CamCand {              // one visible spheroid, in its unit-sphere frame (o = ray origin, d = m0 + y m1 + z m2)
@@ -93,11 +94,22 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
         cd.box = make_int4(0, C.H - 1, 0, C.W - 1);
         vis = cx + a >= C.znear && cx - a < C.zfar;
         if (vis && cx > 1.5f * a) {
-            // a point c + a n of the sphere projects to y/x with |y/x - cy/cx| <= a sqrt(cx^2 + cy^2) / (cx (cx - a))
-            const float inv = 1.0f / (cx * (cx - a) * C.s);
-            const float du = a * sqrtf(cx * cx + cy * cy) * inv + 1.0f, dv = a * sqrtf(cx * cx + cz * cz) * inv + 1.0f;
-            const float uc = C.half_w - cy / (cx * C.s), vc = C.half_h - cz / (cx * C.s);     // column, row of the centre
-            const float c0 = floorf(uc - du), c1 = ceilf(uc + du), r0 = floorf(vc - dv), r1 = ceilf(vc + dv);
+            // Tight box of the silhouette.  In camera coordinates the spheroid's dual quadric projects to the dual conic
+            // C* = Sigma - p p^T with Sigma = a^2 I + (c^2 - a^2) n n^T (n = its axis, p = its centre); the image lines u = const
+            // (u = Y/X) tangent to the conic solve C*_00 u^2 - 2 C*_01 u + C*_11 = 0, likewise v = Z/X with index 2.  C*_00 < 0
+            // because the body lies wholly in front of the plane X = 0 here.  One pixel of slack covers the fp32 rounding.
+            const float nx = Ri[0][0] * Rk[0][2] + Ri[1][0] * Rk[1][2] + Ri[2][0] * Rk[2][2];
+            const float ny = Ri[0][1] * Rk[0][2] + Ri[1][1] * Rk[1][2] + Ri[2][1] * Rk[2][2];
+            const float nz = Ri[0][2] * Rk[0][2] + Ri[1][2] * Rk[1][2] + Ri[2][2] * Rk[2][2];
+            const float c00 = fmaf(C.dac, nx * nx, C.a2) - cx * cx;
+            const float c01 = C.dac * nx * ny - cx * cy, c11 = fmaf(C.dac, ny * ny, C.a2) - cy * cy;
+            const float c02 = C.dac * nx * nz - cx * cz, c22 = fmaf(C.dac, nz * nz, C.a2) - cz * cz;
+            const float inv = 1.0f / (c00 * C.s);
+            const float su = sqrtf(fmaxf(c01 * c01 - c00 * c11, 0.0f)), sv = sqrtf(fmaxf(c02 * c02 - c00 * c22, 0.0f));
+            // column = W/2 - u / s, row = H/2 - v / s; c00 < 0 so (c01 + su) / c00 is the smaller root
+            const float ua = (c01 + su) * inv, ub = (c01 - su) * inv, va = (c02 + sv) * inv, vb = (c02 - sv) * inv;
+            const float c0 = floorf(C.half_w - ub - 1.0f), c1 = ceilf(C.half_w - ua + 1.0f);
+            const float r0 = floorf(C.half_h - vb - 1.0f), r1 = ceilf(C.half_h - va + 1.0f);
             vis = c1 >= 0.0f && c0 <= (float)(C.W - 1) && r1 >= 0.0f && r0 <= (float)(C.H - 1);
             cd.box = make_int4((int)fmaxf(r0, 0.0f), (int)fminf(r1, (float)(C.H - 1)), (int)fmaxf(c0, 0.0f), (int)fminf(c1, (float)(C.W - 1)));
         }
