@@ -120,7 +120,7 @@ def oracle_throughput(wl, budget_s, n_envs, min_steps=4, max_steps=10 ** 9):
                 flops_per_drone_step=flops, ms_per_step=1e3 * dt / steps, steps=steps)
 
 
-def camera_leg(stream, hbm_peak, n_envs=16384, n_drones=4, reps=20, cpu_envs=24):
+def camera_leg(stream, hbm_peak, n_envs=16384, n_drones=4, reps=20, cpu_envs=8192):
     """Secondary measurement: mdg_render_depth, every drone's 48 x 64 depth + segmentation frame.
     16,384 envs x 4 drones = 65,536 frames = 1.0 GB of output per call (> 126 MB L2, so every call's stores reach HBM).
     Algorithmic bytes per frame: H W (4 + 1) written + the drone's 32-byte pose read."""

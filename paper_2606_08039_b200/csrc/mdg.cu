@@ -497,6 +497,8 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
     for (int i = 0; i < 3; ++i) C.off[i] = cam->offset[i];
     C.znear = cam->znear; C.zfar = cam->zfar;
     C.rb = std::fmax(cam->body_radius, cam->body_half_height);
+    C.tan_h = C.half_w * C.s; C.tan_v = C.half_h * C.s;
+    C.len_h = std::sqrt(1.0f + C.tan_h * C.tan_h) * 1.001f; C.len_v = std::sqrt(1.0f + C.tan_v * C.tan_v) * 1.001f;
     C.a2 = (float)((double)cam->body_radius * cam->body_radius);
     C.dac = (float)((double)cam->body_half_height * cam->body_half_height - (double)cam->body_radius * cam->body_radius);
     C.inv_a = (float)(1.0 / (double)cam->body_radius); C.inv_c = (float)(1.0 / (double)cam->body_half_height);

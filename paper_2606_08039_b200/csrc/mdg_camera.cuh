@@ -20,6 +20,7 @@ struct CamDev {
     float s, half_h, half_w, inv_gpr;       // pixel pitch on the image plane at unit distance; H/2, W/2; 1 / groups_per_row
     float off[3], znear, zfar, rb, inv_a, inv_c;   // rb: radius of the bounding sphere = the larger semi-axis
     float a2, dac;                          // a^2, c^2 - a^2
+    float tan_h, tan_v, len_h, len_v;       // W s / 2, H s / 2 and sqrt(1 + tan^2) of each
 };
 
 struct __align__(16) CamCand {              // one visible spheroid, in its unit-sphere frame (o = ray origin, d = m0 + y m1 + z m2)
@@ -92,7 +93,10 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
         const float cz = -(Ri[0][2] * rx + Ri[1][2] * ry + Ri[2][2] * rz);
         const float a = C.rb * 1.001f;
         cd.box = make_int4(0, C.H - 1, 0, C.W - 1);
-        vis = cx + a >= C.znear && cx - a < C.zfar;
+        // bounding sphere against the near / far planes and the four side planes of the view frustum (inward normals
+        // (tan, -+1, 0) / sqrt(1 + tan^2) and (tan, 0, -+1) / sqrt(1 + tan^2), tan = half the image extent at unit distance)
+        vis = cx + a >= C.znear && cx - a < C.zfar &&
+              fmaf(cx, C.tan_h, -fabsf(cy)) >= -a * C.len_h && fmaf(cx, C.tan_v, -fabsf(cz)) >= -a * C.len_v;
         if (vis && cx > 1.5f * a) {
             // Tight box of the silhouette.  In camera coordinates the spheroid's dual quadric projects to the dual conic
             // C* = Sigma - p p^T with Sigma = a^2 I + (c^2 - a^2) n n^T (n = its axis, p = its centre); the image lines u = const
