@@ -17,7 +17,9 @@
 // order, ground / drag / downwash closed forms, symmetries, PID fixed point + linear z recurrence +
 // allocation round trip, wind statistics, obs/reward/termination on hand-built states, Philox KATs;
 // tests/test_oracle_next1.py: normalised / one-dimensional / attitude actions, KIN20, CF2P mixing, the
-// velocity-tracking and fly-through epilogues, Table 4 factors and initial ranges, constant / sinusoidal wind.
+// velocity-tracking and fly-through epilogues, Table 4 factors and initial ranges, constant / sinusoidal wind;
+// tests/test_oracle_sensors.py: Table 4 sensor noise and the per-episode observation bias (table standard deviations,
+// normality, independence, which columns move, constancy over an episode, keying by global env index).
 // PARITY UNPINNED (the oracle itself is the reference): the coupled PID transient in x/y and the
 // multi-config trajectories beyond the invariants above; parity against MuJoCo's own RK4 (MuJoCo is
 // not in the container, reading Q11).
@@ -91,6 +93,11 @@ struct Params {
     // the waypoint-task family (FlyThroughAviary PAPER.md:321, RaceAviary PAPER.md:329; reading Q43): reward per drone =
     // wp_bonus [capture] - wp_shaping |d_wp| + wp_speed |v| - wp_omega |omega|; the list is run wp_laps times
     double wp_bonus, wp_shaping, wp_speed, wp_omega; int wp_laps;
+    // Table 4 "sensors" rows (position / vel / RPY noise N(0, 1 cm / 5 cm/s / 1 deg), gyro noise
+    // N(0, 0.05 rad/s), per step) and the "sticky per-episode bias on the observation" of PAPER.md:248 (iii) (reading Q49):
+    // standard deviations for [position m, velocity m/s, RPY rad, body rates rad/s]; obs_noise is redrawn every step,
+    // obs_bias once per drone and episode; all 0 = off.  Only the emitted observation is perturbed.
+    double obs_noise[4], obs_bias[4];
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_LAG = 14 /* tau_mot in seconds, not a factor */, DR_N = 16 };
@@ -651,8 +658,30 @@ struct Sim {
     }
 
     // O10: observation of env e from dr (S9: [p, eta, v, w] per drone (+ adjacency row, Q23))
-    template <class R> void write_obs(int e, const Drone<R>* dr, double& adj_margin) {
+    // Table 4 sensor rows (reading Q49): additive terms nz[12] for [p, eta, v, omega] of drone i of env e in the observation
+    // emitted at control-step index t: sigma_g xi (fresh every step) + beta_g b (b drawn at the episode's reset index
+    // t0 = t - ep_step).  Twelve normals = three Philox calls, four Box-Muller values each: (x0, x1) -> r cos, r sin; (x2, x3) likewise.
+    static void normals4(const PhiloxOut& r, double out[4]) {
+        const double r1 = std::sqrt(-2.0 * std::log(1.0 - u01(r.x[0]))), r2 = std::sqrt(-2.0 * std::log(1.0 - u01(r.x[2])));
+        out[0] = r1 * std::cos(2.0 * PI * u01(r.x[1])); out[1] = r1 * std::sin(2.0 * PI * u01(r.x[1]));
+        out[2] = r2 * std::cos(2.0 * PI * u01(r.x[3])); out[3] = r2 * std::sin(2.0 * PI * u01(r.x[3]));
+    }
+    void sensor_terms(int e, int i, uint32_t t, double nz[12]) const {
+        const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32), eg = (uint32_t)e + (uint32_t)P.env_index_base;
+        const int group[12] = {0, 0, 0, 2, 2, 2, 1, 1, 1, 3, 3, 3};   // [p, eta, v, omega] -> index into (pos, vel, RPY, gyro)
+        const uint32_t t0 = t - ep_step[e];                            // index of the reset that opened the running episode
+        for (int c = 0; c < 3; ++c) {
+            double xi[4], b[4];
+            normals4(philox4x32_10(eg, (uint32_t)i, t, STREAM_OBS_NOISE + c, k0, k1), xi);
+            normals4(philox4x32_10(eg, (uint32_t)i, t0, STREAM_OBS_BIAS + c, k0, k1), b);
+            for (int a = 0; a < 4; ++a) nz[4 * c + a] = P.obs_noise[group[4 * c + a]] * xi[a] + P.obs_bias[group[4 * c + a]] * b[a];
+        }
+    }
+    bool sensors_on() const { for (int a = 0; a < 4; ++a) if (P.obs_noise[a] != 0.0 || P.obs_bias[a] != 0.0) return true; return false; }
+
+    template <class R> void write_obs(int e, const Drone<R>* dr, double& adj_margin, uint32_t t) {
         const int od = opd();
+        const bool noisy = sensors_on();
         double* o = &obs[(size_t)e * obs_dim()];
         adj_margin = 1e30;
         for (int i = 0; i < M; ++i) {
@@ -662,9 +691,17 @@ struct Sim {
             if (P.obs_mode == OBS_KIN20) {                         // [p, q, eta, v, omega, a_{t-1}]
                 for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[7 + a] = to_d(eta[a]); oi[10 + a] = to_d(dr[i].v[a]); oi[13 + a] = to_d(dr[i].w[a]); }
                 for (int a = 0; a < 4; ++a) { oi[3 + a] = to_d(dr[i].q[a]); oi[16 + a] = dr[i].act[a]; }
+                if (noisy) {                                        // q and the last action stay exact (Q49)
+                    double nz[12]; sensor_terms(e, i, t, nz);
+                    for (int a = 0; a < 3; ++a) { oi[a] += nz[a]; oi[7 + a] += nz[3 + a]; oi[10 + a] += nz[6 + a]; oi[13 + a] += nz[9 + a]; }
+                }
                 continue;
             }
             for (int a = 0; a < 3; ++a) { oi[a] = to_d(dr[i].p[a]); oi[3 + a] = to_d(eta[a]); oi[6 + a] = to_d(dr[i].v[a]); oi[9 + a] = to_d(dr[i].w[a]); }
+            if (noisy) {                                            // Table 4 sensor rows on the 12 kinematic entries only (Q49)
+                double nz[12]; sensor_terms(e, i, t, nz);
+                for (int a = 0; a < 12; ++a) oi[a] += nz[a];
+            }
             if (P.obs_mode == OBS_KIN12_TGT)                       // [p, eta, v, omega, v*_x, v*_y, v*_z, omega*_z]
                 for (int a = 0; a < 4; ++a) oi[12 + a] = dr[i].tg[a];
             if (P.obs_mode == OBS_KIN12_Z) oi[12] = dr[i].tg[2];   // kinematic state plus target altitude (13)
@@ -846,7 +883,7 @@ struct Sim {
             load(e, dr);
         }
         double m_adj;
-        write_obs(e, dr, m_adj);
+        write_obs(e, dr, m_adj, t);
         margin[(size_t)e * 3 + 0] = m_done; margin[(size_t)e * 3 + 1] = m_rew; margin[(size_t)e * 3 + 2] = m_adj;
     }
 
@@ -857,7 +894,7 @@ struct Sim {
             reset_env(e, 0);
             load(e, buf.data());
             double m_adj;
-            write_obs(e, buf.data(), m_adj);
+            write_obs(e, buf.data(), m_adj, 0);
             reward[e] = 0.0; done[e] = 0;
             margin[(size_t)e * 3 + 0] = margin[(size_t)e * 3 + 1] = 1e30; margin[(size_t)e * 3 + 2] = m_adj;
         }
