@@ -123,6 +123,13 @@ typedef struct mdg_params {
      * - wp_shaping |d_wp| + wp_speed |v| - wp_omega |omega|, the list run wp_laps times.  Defaults = FlyThroughAviary
      * (10, 0.1, 0, 0.01, 1 lap); RaceAviary = 20, 0.05, 2, 0, 2 laps over its six gates. */
     float wp_bonus, wp_shaping, wp_speed, wp_omega; int32_t wp_laps;
+    /* Table 4 "sensors" rows and the sticky per-episode observation bias of PAPER.md:248 (iii) (DESIGN.md
+     * reading Q49): standard deviations for [position m, velocity m/s, roll/pitch/yaw rad, body rates rad/s].  obs_noise is
+     * drawn afresh for every emitted observation (Table 4: 0.01, 0.05, 1 degree = 0.01745, 0.05), obs_bias once per drone and
+     * episode; both are Gaussian, added to the twelve kinematic entries of the MDG_OBS_* row only (quaternion, last action,
+     * targets and adjacency stay exact); the simulated state, the controller, reward and termination see the true values.
+     * All 0 (default) = off.  Negative values are MDG_EINVAL. */
+    float obs_noise[4], obs_bias[4];
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

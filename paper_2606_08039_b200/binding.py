@@ -37,6 +37,7 @@ class mdg_params(C.Structure):
         ("gust_prob", C.c_float), ("gust_max", C.c_float), ("gust_duration", C.c_float),
         ("n_waypoints", C.c_int32), ("waypoints", C.c_float * 24), ("wp_radius", C.c_float),
         ("wp_bonus", C.c_float), ("wp_shaping", C.c_float), ("wp_speed", C.c_float), ("wp_omega", C.c_float), ("wp_laps", C.c_int32),
+        ("obs_noise", C.c_float * 4), ("obs_bias", C.c_float * 4),
     ]
 
     def update(self, d):

@@ -73,6 +73,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     for (int i = 0; i < 12; ++i) if (p.dr_alpha[i] != 0.0f) f |= F_DR;
     if (p.motor_lag_hi > 0.0f) f |= F_DR | F_MLAG;
     if ((aero & MDG_AERO_WIND) && p.wind_mask != MDG_WIND_DRYDEN) f |= F_WIND_MIX;
+    for (int i = 0; i < 4; ++i) if (p.obs_noise[i] != 0.0f || p.obs_bias[i] != 0.0f) f |= F_SENS;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
     if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
@@ -152,6 +153,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     for (int i = 0; i < 12; ++i) D.dr_alpha[i] = p.dr_alpha[i];
     for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
     D.motor_lag_lo = p.motor_lag_lo; D.motor_lag_hi = p.motor_lag_hi;
+    for (int i = 0; i < 4; ++i) { D.obs_noise[i] = p.obs_noise[i]; D.obs_bias[i] = p.obs_bias[i]; }
     D.wp_total = p.n_waypoints * p.wp_laps; D.wp_bonus = p.wp_bonus; D.wp_shaping = p.wp_shaping; D.wp_speed = p.wp_speed; D.wp_omega = p.wp_omega;
     D.n_waypoints = p.n_waypoints; D.wp_radius2 = (float)((double)p.wp_radius * p.wp_radius);
     for (int i = 0; i < 24; ++i) D.waypoints[i] = p.waypoints[i];
@@ -323,6 +325,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || p.motor_lag_lo < 0 || p.motor_lag_hi < p.motor_lag_lo || p.wp_laps < 0 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
+    for (int i = 0; i < 4; ++i)
+        if (!(p.obs_noise[i] >= 0) || !(p.obs_bias[i] >= 0)) return fail(MDG_EINVAL, "mdg_create: obs_noise / obs_bias must be >= 0");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))
         return fail(MDG_EINVAL, "mdg_create: m, g, k_f, k_m, J, wind_tau must be positive");
     int ndev = 0;

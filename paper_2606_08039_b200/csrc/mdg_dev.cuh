@@ -21,6 +21,7 @@ enum : int {
     F_CF2P = 1 << 20,                                     // +-configuration mixing
     F_DR = 1 << 21,                                       // per-episode domain-randomisation factors (Table 4)
     F_MLAG = 1 << 23,                                     // motor lag: rotor-speed state, wrench recomputed every substep
+    F_SENS = 1 << 24,                                     // Table 4 sensor rows: noise / per-episode bias on the emitted observation
     F_WIND_MIX = 1 << 22,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
 };
 
@@ -64,6 +65,7 @@ struct DevParams {
     float dr_alpha[12];                                   // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g, motor, arm, max_rpm, -]
     float reset_rpy_half[3], reset_vel_half[3];           // Table 4 "init" row
     float motor_lag_lo, motor_lag_hi;                     // Table 4 motor lag: range of the time constant (s)
+    float obs_noise[4], obs_bias[4];                      // Table 4 sensor rows: standard deviations for [position, velocity, RPY, body rates]
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 
@@ -92,7 +94,8 @@ struct DevBuffers {
     uint8_t* done;
 };
 
-static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9, STREAM_GUST = 10;
+static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9, STREAM_GUST = 10,
+                      STREAM_OBS_NOISE = 11 /* 11..13 */, STREAM_OBS_BIAS = 14 /* 14..16 */;
 
 // Philox4x32-10 (Salmon et al., SC'11).  key = seed halves, counter = (env, drone|~0, step, stream).
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,

@@ -510,7 +510,9 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
             if (F::act(P) == 1) B.P5[drone] = d.sp;
         }
-        write_obs<G>(P, B.obs, drone, d, eta, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
+        Sensed sn = sensed(d, eta);
+        if (FEAT < 0 && F::has(P, F_SENS)) sense(P, e, (uint32_t)jj, t, ep_out, sn);   // Table 4 sensor rows: the stored state stays exact
+        write_obs<G>(P, B.obs, drone, d, sn, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
         B.reward_d[drone] = r;
         if (lag) B.N0[drone] = make_float4(n_act[0], n_act[1], n_act[2], n_act[3]);
         if (j == 0) {
@@ -556,7 +558,9 @@ __global__ void reset_kernel(const __grid_constant__ DevParams P, const DevBuffe
     if (P.feat & F_DR) draw_dr(P, e, (uint32_t)jj, 0u, n0, n1, n2, n3);
     B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3;
     B.N0[drone] = make_float4(P.hover_rpm, P.hover_rpm, P.hover_rpm, P.hover_rpm);
-    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), tg);
+    Sensed sn = sensed(d, euler_zyx(d.q));
+    if (P.feat & F_SENS) sense(P, e, (uint32_t)jj, 0u, 0u, sn);
+    write_obs<G>(P, B.obs, drone, d, sn, adj, omode, make_float4(0, 0, 0, 0), tg);
     B.reward_d[drone] = 0.0f;
     if (j == 0) B.E1[e] = make_float4(0, 0, 0, 1.0f);
     if (j == 0) { B.E0[e] = make_float4(0, 0, 0, __uint_as_float(0u)); B.gstep[e] = 0u; B.reward[e] = 0.0f; B.done[e] = 0; }
@@ -582,7 +586,9 @@ __global__ void refresh_obs_kernel(const __grid_constant__ DevParams P, const De
     const int omode = (P.feat >> F_OBS_SHIFT) & 7;
     if (omode == 1) adjacency<G>(P, d.p, lane, j, adj);
     if (!active) return;
-    write_obs<G>(P, B.obs, drone, d, euler_zyx(d.q), adj, omode, make_float4(0, 0, 0, 0), B.P6[drone]);
+    Sensed sn = sensed(d, euler_zyx(d.q));
+    if (P.feat & F_SENS) sense(P, e, (uint32_t)jj, B.gstep[e], __float_as_uint(B.E0[e].w), sn);
+    write_obs<G>(P, B.obs, drone, d, sn, adj, omode, make_float4(0, 0, 0, 0), B.P6[drone]);
 }
 
 // harness actions (stream 3): base * fma(hi - lo, u, lo), each operation rounded to fp32

@@ -189,27 +189,57 @@ __device__ __forceinline__ V3 ang_acc(const DevParams& P, V3 tb, V3 w, bool axis
               axisym ? P.invJ[2] * tb.z : fmaf(P.invJ[2], tb.z, -P.gyro[2] * (w.x * w.y)));
 }
 
+// four standard normal values from one Philox draw: Box-Muller on (x, y) and on (z, w), the angle taken in [-pi, pi) so that
+// the MUFU sine / cosine keep their accuracy (cos(a - pi) = -cos a is absorbed in the sign of the radius)
+// The radius uses log1pf: MUFU.LG2's absolute error near 1 would show in the rare small radii (this path is optional, off the
+// benchmark kernels' critical path).
+__device__ __forceinline__ float4 normals4(uint4 r) {
+    const float r1 = -fast_sqrt(-2.0f * log1pf(-u01(r.x))), r2 = -fast_sqrt(-2.0f * log1pf(-u01(r.z)));
+    const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
+    return make_float4(r1 * cos_fast(a1), r1 * sin_fast(a1), r2 * cos_fast(a2), r2 * sin_fast(a2));
+}
+// Table 4 sensor rows (reading Q49): what the observation emitted at step index t reports for
+// [p, eta, v, omega] = the true value + sigma xi (xi fresh every step, streams 11..13) + beta b (b drawn at the reset
+// index t - ep_step of the running episode, streams 14..16).  The twelve values follow the row order p, eta, v, omega.
+struct Sensed { V3 p, eta, v, w; };                               // the twelve kinematic entries as the observation reports them
+__device__ __forceinline__ Sensed sensed(const DroneRegs& d, V3 eta) { Sensed s; s.p = d.p; s.eta = eta; s.v = d.v; s.w = d.w; return s; }
+__device__ __forceinline__ void sense(const DevParams& P, unsigned e, uint32_t j, uint32_t t, uint32_t ep_step, Sensed& s) {
+    const uint32_t eg = e + P.env_base, t0 = t - ep_step;
+    const float4 n0 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE, P.seed_lo, P.seed_hi));
+    const float4 n1 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE + 1, P.seed_lo, P.seed_hi));
+    const float4 n2 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE + 2, P.seed_lo, P.seed_hi));
+    const float4 b0 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS, P.seed_lo, P.seed_hi));
+    const float4 b1 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS + 1, P.seed_lo, P.seed_hi));
+    const float4 b2 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS + 2, P.seed_lo, P.seed_hi));
+    const float sp = P.obs_noise[0], sv = P.obs_noise[1], se = P.obs_noise[2], sw = P.obs_noise[3];
+    const float bp = P.obs_bias[0], bv = P.obs_bias[1], be = P.obs_bias[2], bw = P.obs_bias[3];
+    s.p.x += fmaf(sp, n0.x, bp * b0.x); s.p.y += fmaf(sp, n0.y, bp * b0.y); s.p.z += fmaf(sp, n0.z, bp * b0.z);
+    s.eta.x += fmaf(se, n0.w, be * b0.w); s.eta.y += fmaf(se, n1.x, be * b1.x); s.eta.z += fmaf(se, n1.y, be * b1.y);
+    s.v.x += fmaf(sv, n1.z, bv * b1.z); s.v.y += fmaf(sv, n1.w, bv * b1.w); s.v.z += fmaf(sv, n2.x, bv * b2.x);
+    s.w.x += fmaf(sw, n2.y, bw * b2.y); s.w.y += fmaf(sw, n2.z, bw * b2.z); s.w.z += fmaf(sw, n2.w, bw * b2.w);
+}
+
 // Observation row of one drone: [p, eta, v, w (, adjacency)] or KIN20 [p, q, eta, v, w, a], written as
 // float4s when the row is 16 B aligned
 template <int G>
 __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict__ obs, size_t drone, const DroneRegs& d,
-                                          V3 eta, const float (&adj)[G], int mode, float4 act, float4 tg) {
+                                          const Sensed& s, const float (&adj)[G], int mode, float4 act, float4 tg) {
     const bool with_adj = mode == 1;
     float* o = obs + drone * (size_t)P.opd;
     if (mode == 2) {
         float4* o4 = reinterpret_cast<float4*>(o);                 // 20 floats per drone: always 16 B aligned
-        o4[0] = make_float4(d.p.x, d.p.y, d.p.z, d.q.w);
-        o4[1] = make_float4(d.q.x, d.q.y, d.q.z, eta.x);
-        o4[2] = make_float4(eta.y, eta.z, d.v.x, d.v.y);
-        o4[3] = make_float4(d.v.z, d.w.x, d.w.y, d.w.z);
+        o4[0] = make_float4(s.p.x, s.p.y, s.p.z, d.q.w);
+        o4[1] = make_float4(d.q.x, d.q.y, d.q.z, s.eta.x);
+        o4[2] = make_float4(s.eta.y, s.eta.z, s.v.x, s.v.y);
+        o4[3] = make_float4(s.v.z, s.w.x, s.w.y, s.w.z);
         o4[4] = act;
         return;
     }
     if ((P.opd & 3) == 0) {
         float4* o4 = reinterpret_cast<float4*>(o);
-        o4[0] = make_float4(d.p.x, d.p.y, d.p.z, eta.x);
-        o4[1] = make_float4(eta.y, eta.z, d.v.x, d.v.y);
-        o4[2] = make_float4(d.v.z, d.w.x, d.w.y, d.w.z);
+        o4[0] = make_float4(s.p.x, s.p.y, s.p.z, s.eta.x);
+        o4[1] = make_float4(s.eta.y, s.eta.z, s.v.x, s.v.y);
+        o4[2] = make_float4(s.v.z, s.w.x, s.w.y, s.w.z);
         if (mode == 3) o4[3] = tg;                                 // KIN12_TGT
         if (with_adj) {
             if (G == 4) o4[3] = make_float4(adj[0], adj[1 % G], adj[2 % G], adj[3 % G]);
@@ -219,8 +249,8 @@ __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict_
             }
         }
     } else {
-        o[0] = d.p.x; o[1] = d.p.y; o[2] = d.p.z; o[3] = eta.x; o[4] = eta.y; o[5] = eta.z;
-        o[6] = d.v.x; o[7] = d.v.y; o[8] = d.v.z; o[9] = d.w.x; o[10] = d.w.y; o[11] = d.w.z;
+        o[0] = s.p.x; o[1] = s.p.y; o[2] = s.p.z; o[3] = s.eta.x; o[4] = s.eta.y; o[5] = s.eta.z;
+        o[6] = s.v.x; o[7] = s.v.y; o[8] = s.v.z; o[9] = s.w.x; o[10] = s.w.y; o[11] = s.w.z;
         if (mode == 5) o[12] = tg.z;                               // KIN12_Z
         if (mode == 4) {                                           // KIN12_WP: next waypoint, world and body frame
             const V3 rb = rot_inv(d.q, v3(tg.x - d.p.x, tg.y - d.p.y, tg.z - d.p.z));

@@ -29,6 +29,9 @@ DR = [0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02, 0.05, 0.02, 0.05, 0.0]     # Ta
 INIT = dict(reset_rpy_half=[0.1, 0.1, 0.1], reset_vel_half=[0.5, 0.5, 0.5])   # its "init" row
 
 
+SENS = dict(obs_noise=[0.01, 0.05, 0.0174533, 0.05], obs_bias=[0.02, 0.03, 0.01, 0.04])   # Table 4 "sensors" rows; bias: PAPER.md:248 (iii)
+
+
 def wl(name, n, m, phys, act, params, actions, seed=77):
     return W.Workload(name, n, m, phys, act, params, actions, 48, W.BASE_SEED + seed)
 
@@ -124,6 +127,21 @@ CASES = {
                                  episode_len_s=0.5, auto_reset=1, motor_lag_lo=0.005, motor_lag_hi=0.05), ("targets",)), {}),
     "m4_motor_lag_dr_all_aero": (wl("m4lag", 700, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
                                     dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR, motor_lag_lo=0.005, motor_lag_hi=0.05, **INIT), HOVER), {}),
+    # Table 4 sensor rows: per-step noise and per-episode bias on the observation, in each row layout (short episodes ->
+    # the bias is redrawn at auto-resets); state, reward and done must be untouched by them
+    "m1_sensors_pid": (wl("m1sens", 1500, 1, W.PHYS_MJC, W.ACT_PID,
+                          dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST,
+                               term_tilt=0.4, term_dist=3.0, target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
+                               episode_len_s=0.25, auto_reset=1, **SENS), ("targets",)), {}),
+    "m3_sensors_kin20": (wl("m3sens", 500, 3, W.PHYS_MJC_DW, W.ACT_RPM, dict(GRID, obs_mode=W.OBS_KIN20, episode_len_s=0.3, **SENS), HOVER), {}),
+    "m4_sensors_c5_like": (wl("m4sens", 900, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_VEL,
+                              dict(CIRCLE, circle_radius=0.3, form_radius=0.3, aero_mask=15, wind_sigma=0.5, wind_tau=1.0, target_mode=W.TGT_CIRCLE,
+                                   int_clamp_pos=1.0, int_clamp_att=0.25, episode_len_s=0.4, **SENS), ("uniform", -1.0, 1.0)), {}),
+    "m2_sensors_fly_through": (wl("m2sensfly", 800, 2, W.PHYS_MJC_DRAG, W.ACT_RPM,
+                                  dict(GRID, grid_cols=2, reset_z_lo=0.9, reset_z_hi=1.1, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH,
+                                       target_mode=W.TGT_WAYPOINTS, wp_radius=0.25, episode_len_s=20.0, **SENS), HOVER), {}),
+    "m5_sensors_obs13_dr": (wl("m5sens", 300, 5, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM_NORM,
+                               dict(GRID, obs_mode=W.OBS_KIN12_Z, episode_len_s=0.3, dr_alpha=DR, **INIT, **SENS), ("uniform", -0.1, 0.12)), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
@@ -212,3 +230,49 @@ def test_domain_randomisation_factors_match_the_oracle_draws():
     assert np.all(plain.get_dr() == 1.0)
     with pytest.raises(mdg.MdgError):
         plain.set_dr(np.ones((8, 16), dtype=np.float32))
+
+
+def test_sensor_noise_residual_and_refresh_after_set_state():
+    """Table 4 sensor rows through the C ABI: the noisy handle's state / reward / done are bitwise those of a noise-free handle,
+    the residual obs_noisy - obs_clean equals the oracle's residual (same Philox draws), and mdg_set_state recomputes the
+    row with the draws of the current step index and episode.  A negative standard deviation is MDG_EINVAL."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    from oracle import oracle as O
+    w = wl("sensres", 2000, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, episode_len_s=5 / 48), HOVER)
+    noisy_p = dict(w.params, **SENS)
+    clean = mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **w.params))
+    noisy = mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **noisy_p))
+    orc_c = O.OracleEnv(w.n_envs, w.n_drones, w.physics_mode, w.action_type, O.OracleParams(0, **w.params), n_threads=4)
+    orc_n = O.OracleEnv(w.n_envs, w.n_drones, w.physics_mode, w.action_type, O.OracleParams(0, **noisy_p), n_threads=4)
+    assert "generic" in noisy.kernel_name
+    for env in (clean, noisy, orc_c, orc_n):
+        env.reset(w.seed)
+    for t in range(8):                                                 # truncation after 5 steps: one bias redraw on the way
+        if t > 0:
+            a = O.gen_actions(w.seed, t, w.n_envs, w.n_drones, W.hover_rpm_f32(), 0.9, 1.1)
+            a_dev = torch.from_numpy(a).cuda()
+            for env in (clean, noisy):
+                env.step(a_dev)
+            for env in (orc_c, orc_n):
+                env.step(a)
+        torch.cuda.synchronize()
+        sc, sn = clean.get_state(), noisy.get_state()
+        assert np.array_equal(sc["state"], sn["state"]) and np.array_equal(sc["ep_step"], sn["ep_step"])
+        assert torch.equal(clean.reward, noisy.reward) and torch.equal(clean.done, noisy.done)
+        res32 = (noisy.obs - clean.obs).cpu().numpy().astype(np.float64)
+        res64 = orc_n.outputs()[0] - orc_c.outputs()[0]
+        assert np.abs(res64).max() > 0.1                               # some 4-sigma draws among 48,000
+        assert np.abs(res32 - res64).max() < 2e-6, (t, np.abs(res32 - res64).max())   # fp32 rounding of obs + residual
+    # set_state: same state into both sides, other episode counters -> the row uses (gstep, gstep - ep_step)
+    st = orc_n.state.astype(np.float32)
+    st[:, 0:3] += 0.125
+    eps = (np.arange(w.n_envs) % 3).astype(np.uint32)
+    orc_n.ep_step = eps
+    orc_n.state = st.astype(np.float64)
+    noisy.set_state(state=st, ep_step=eps)
+    torch.cuda.synchronize()
+    assert np.abs(noisy.obs.cpu().numpy() - orc_n.outputs()[0]).max() < 2e-6
+    with pytest.raises(mdg.MdgError):
+        mdg.Env(4, 1, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, obs_noise=[0.01, -0.05, 0.0, 0.0]))
