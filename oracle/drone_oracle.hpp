@@ -19,7 +19,8 @@
 // tests/test_oracle_next1.py: normalised / one-dimensional / attitude actions, KIN20, CF2P mixing, the
 // velocity-tracking and fly-through epilogues, Table 4 factors and initial ranges, constant / sinusoidal wind;
 // tests/test_oracle_sensors.py: Table 4 sensor noise and the per-episode observation bias (table standard deviations,
-// normality, independence, which columns move, constancy over an episode, keying by global env index).
+// normality, independence, which columns move, constancy over an episode, keying by global env index);
+// tests/test_oracle_dryden.py: altitude-dependent Dryden length scale (printed values, first updates, AR(1) statistics by altitude).
 // PARITY UNPINNED (the oracle itself is the reference): the coupled PID transient in x/y and the
 // multi-config trajectories beyond the invariants above; parity against MuJoCo's own RK4 (MuJoCo is
 // not in the container, reading Q11).
@@ -98,6 +99,10 @@ struct Params {
     // standard deviations for [position m, velocity m/s, RPY rad, body rates rad/s]; obs_noise is redrawn every step,
     // obs_bias once per drone and episode; all 0 = off.  Only the emitted observation is perturbed.
     double obs_noise[4], obs_bias[4];
+    // DRYDEN with the altitude-dependent length scale ("L_u = h/(0.177 + 8.23e-4 h)^1.2 at altitude h ...
+    // alpha = e^(-dt V / L)", reading Q50): V = dryden_airspeed (m/s; 0 = the fixed-tau form above), h = mean altitude of the
+    // env's drones at the start of the control step, not below dryden_h_min
+    double dryden_airspeed, dryden_h_min;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_LAG = 14 /* tau_mot in seconds, not a factor */, DR_N = 16 };
@@ -120,6 +125,7 @@ inline void default_params(int model, Params& P) {
     P.k_wind = 0.5 * 1.225 * 1.0 * 0.01;                          // Q28
     P.wind_sigma = 0.5; P.wind_tau = 1.0;
     P.wind_mask = WIND_DRYDEN; P.wind_sine_omega = 2.0 * PI * 0.5;
+    P.dryden_airspeed = 0.0; P.dryden_h_min = 0.05;                // Q50
     P.gust_prob = 0.02; P.gust_max = 1.0; P.gust_duration = 0.5;   // Q42
     const double wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5, 0, 1, 1, 0, 0, 0.5};     // PAPER.md:321 default list
     P.n_waypoints = 5; for (int i = 0; i < 15; ++i) P.waypoints[i] = wps[i];
@@ -738,7 +744,14 @@ struct Sim {
                 const double ua = u01(r.x[0]), ub = u01(r.x[1]), uc = u01(r.x[2]), ud = u01(r.x[3]);
                 const R r1 = sqrt(-2.0 * log(R(1.0 - ua))), r2 = sqrt(-2.0 * log(R(1.0 - uc)));   // Box-Muller
                 const R xi[3] = {r1 * cos(R(2.0 * PI * ub)), r1 * sin(R(2.0 * PI * ub)), r2 * cos(R(2.0 * PI * ud))};
-                const double alpha = std::exp(-D.dt_c / P.wind_tau);
+                double alpha = std::exp(-D.dt_c / P.wind_tau);
+                if (P.dryden_airspeed > 0.0) {                     // PAPER.md:202, Q50: L_u(h), alpha = exp(-dt V / L)
+                    double hm = 0.0;
+                    for (int i = 0; i < M; ++i) hm += to_d(dr[i].p[2]);
+                    hm = std::fmax(hm / M, P.dryden_h_min);
+                    const double L = hm / std::pow(0.177 + 8.23e-4 * hm, 1.2);
+                    alpha = std::exp(-D.dt_c * P.dryden_airspeed / L);
+                }
                 const double gain = P.wind_sigma * std::sqrt(1.0 - alpha * alpha);
                 for (int a = 0; a < 3; ++a) { w[a] = alpha * R(wind[(size_t)e * 3 + a]) + gain * xi[a]; wind[(size_t)e * 3 + a] = to_d(w[a]); }
             }
