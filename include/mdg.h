@@ -130,6 +130,10 @@ typedef struct mdg_params {
      * targets and adjacency stay exact); the simulated state, the controller, reward and termination see the true values.
      * All 0 (default) = off.  Negative values are MDG_EINVAL. */
     float obs_noise[4], obs_bias[4];
+    /* MDG_WIND_DRYDEN with the altitude-dependent length scale (L_u = h / (0.177 + 8.23e-4 h)^1.2,
+     * alpha = exp(-dt V / L); reading Q50): dryden_airspeed = V in m/s (0, the default, keeps the fixed wind_tau),
+     * h = the mean altitude of the env's drones at the start of the control step, not below dryden_h_min (0.05 m). */
+    float dryden_airspeed, dryden_h_min;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

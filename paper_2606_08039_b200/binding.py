@@ -38,6 +38,7 @@ class mdg_params(C.Structure):
         ("n_waypoints", C.c_int32), ("waypoints", C.c_float * 24), ("wp_radius", C.c_float),
         ("wp_bonus", C.c_float), ("wp_shaping", C.c_float), ("wp_speed", C.c_float), ("wp_omega", C.c_float), ("wp_laps", C.c_int32),
         ("obs_noise", C.c_float * 4), ("obs_bias", C.c_float * 4),
+        ("dryden_airspeed", C.c_float), ("dryden_h_min", C.c_float),
     ]
 
     def update(self, d):

@@ -72,7 +72,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     if (p.drone_model == MDG_MODEL_CF2P) f |= F_CF2P;
     for (int i = 0; i < 12; ++i) if (p.dr_alpha[i] != 0.0f) f |= F_DR;
     if (p.motor_lag_hi > 0.0f) f |= F_DR | F_MLAG;
-    if ((aero & MDG_AERO_WIND) && p.wind_mask != MDG_WIND_DRYDEN) f |= F_WIND_MIX;
+    if ((aero & MDG_AERO_WIND) && (p.wind_mask != MDG_WIND_DRYDEN || p.dryden_airspeed > 0.0f)) f |= F_WIND_MIX;
     for (int i = 0; i < 4; ++i) if (p.obs_noise[i] != 0.0f || p.obs_bias[i] != 0.0f) f |= F_SENS;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
@@ -130,6 +130,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.dz_floor = p.dw_dz_clip > 1e-6f ? p.dw_dz_clip : 1e-6f;
     const double alpha = std::exp(-dtc / p.wind_tau);
     D.wind_alpha = (float)alpha; D.wind_gain = (float)(p.wind_sigma * std::sqrt(1.0 - alpha * alpha)); D.k_wind = p.k_wind;
+    D.dryden_x = (float)(dtc * p.dryden_airspeed); D.dryden_h_min = p.dryden_h_min; D.wind_sigma = p.wind_sigma; D.inv_M = (float)(1.0 / M);
     D.gust_prob = p.gust_prob; D.gust_max = p.gust_max; D.gust_ds = (float)(dtc / p.gust_duration);
     D.wind_mask = p.wind_mask; D.wind_sine_amp = p.wind_sine_amp; D.wind_sine_omega = p.wind_sine_omega;
     for (int i = 0; i < 3; ++i) D.wind_const[i] = p.wind_const[i];
@@ -280,6 +281,7 @@ int mdg_default_params(int drone_model, mdg_params* p) {
     const float wps[15] = {0, 0, 1, 1, 0, 1, 1, 1, 1.5f, 0, 1, 1, 0, 0, 0.5f};          // PAPER.md:321 default list
     p->n_waypoints = 5; for (int i = 0; i < 15; ++i) p->waypoints[i] = wps[i];
     p->wp_radius = 0.1f; p->wp_bonus = 10.0f; p->wp_shaping = 0.1f; p->wp_speed = 0.0f; p->wp_omega = 0.01f; p->wp_laps = 1;
+    p->dryden_airspeed = 0.0f; p->dryden_h_min = 0.05f;
     p->sim_freq = 240; p->ctrl_freq = 48;
     p->aero_mask = -1; p->integrator = -1;
     const float kp[3] = {0.4f, 0.4f, 1.0f}, ki[3] = {0.01f, 0.01f, 0.01f}, kd[3] = {0.9f, 0.9f, 2.0f};   // Table 6
@@ -325,6 +327,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || p.motor_lag_lo < 0 || p.motor_lag_hi < p.motor_lag_lo || p.wp_laps < 0 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
+    if (!(p.dryden_airspeed >= 0) || (p.dryden_airspeed > 0 && !(p.dryden_h_min > 0)))
+        return fail(MDG_EINVAL, "mdg_create: dryden_airspeed must be >= 0 and dryden_h_min > 0");
     for (int i = 0; i < 4; ++i)
         if (!(p.obs_noise[i] >= 0) || !(p.obs_bias[i] >= 0)) return fail(MDG_EINVAL, "mdg_create: obs_noise / obs_bias must be >= 0");
     if (!(p.m > 0) || !(p.k_f > 0) || !(p.k_m > 0) || !(p.J[0] > 0) || !(p.J[1] > 0) || !(p.J[2] > 0) || !(p.g > 0) || !(p.wind_tau > 0))

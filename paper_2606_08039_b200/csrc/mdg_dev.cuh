@@ -50,6 +50,7 @@ struct DevParams {
     float gnd_coef, h_clip, c_xy, c_z, dw_coef, dw_C2, dw_C3, dz_clip, inv_dz_clip;
     float dw_C2s, dw_C3s, dw_b2_min, dz_floor;            // Eq.6 with beta scaled by sqrt(2 ln 2): exp(-x/2b^2) = 2^(-x/b'^2)
     float wind_alpha, wind_gain, k_wind;
+    float dryden_x, dryden_h_min, wind_sigma, inv_M;      // altitude-dependent Dryden scale: dt_c V (0 = fixed tau), altitude floor
     float gust_prob, gust_max, gust_ds;                   // MDG_WIND_GUST: trigger probability, largest speed, dt_c / duration
     int wind_mask; float wind_const[3], wind_sine_amp, wind_sine_omega;   // MDG_WIND_*: 1 AR(1) gust, 2 constant, 8 sinusoidal force
     // cascaded PID (Eq.9, Table 6)

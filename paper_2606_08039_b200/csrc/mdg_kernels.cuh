@@ -237,9 +237,16 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
             const float r1 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.x))), r2 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.z)));
             const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
-            env4.x = fmaf(P.wind_alpha, env4.x, P.wind_gain * (r1 * cos_fast(a1)));
-            env4.y = fmaf(P.wind_alpha, env4.y, P.wind_gain * (r1 * sin_fast(a1)));
-            env4.z = fmaf(P.wind_alpha, env4.z, P.wind_gain * (r2 * cos_fast(a2)));
+            float wa = P.wind_alpha, wg = P.wind_gain;
+            if (FEAT < 0 && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
+                const float hm = fmaxf(group_sum<G>((full_group || j < P.M) ? d.p.z : 0.0f) * P.inv_M, P.dryden_h_min);   // alpha = exp(-dt V / L)
+                const float x = P.dryden_x * powf(fmaf(8.23e-4f, hm, 0.177f), 1.2f) / hm;
+                wa = expf(-x);
+                wg = P.wind_sigma * sqrtf(-expm1f(-2.0f * x));    // sigma sqrt(1 - alpha^2) without the cancellation
+            }
+            env4.x = fmaf(wa, env4.x, wg * (r1 * cos_fast(a1)));
+            env4.y = fmaf(wa, env4.y, wg * (r1 * sin_fast(a1)));
+            env4.z = fmaf(wa, env4.z, wg * (r2 * cos_fast(a2)));
             u = v3(env4.x, env4.y, env4.z);
         }
         if (wmask & 2) { u.x += P.wind_const[0]; u.y += P.wind_const[1]; u.z += P.wind_const[2]; }

@@ -142,6 +142,16 @@ CASES = {
                                        target_mode=W.TGT_WAYPOINTS, wp_radius=0.25, episode_len_s=20.0, **SENS), HOVER), {}),
     "m5_sensors_obs13_dr": (wl("m5sens", 300, 5, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM_NORM,
                                dict(GRID, obs_mode=W.OBS_KIN12_Z, episode_len_s=0.3, dr_alpha=DR, **INIT, **SENS), ("uniform", -0.1, 0.12)), {}),
+    # DRYDEN with the altitude-dependent length scale: alone at mixed altitudes (some below the altitude floor,
+    # M = 3 in a 4-lane group for the mean), and inside the paper's COMBINED wind
+    "m3_dryden_altitude": (wl("m3dry", 700, 3, W.PHYS_MJC_GND, W.ACT_VEL,
+                              dict(GRID, reset_z_lo=0.02, reset_z_hi=2.5, aero_mask=W.AERO_WIND | W.AERO_GND, wind_sigma=0.6, dryden_airspeed=7.0,
+                                   reward_mode=W.REW_MULTI_HOVER), ("uniform", -0.5, 0.5)), {}),
+    "m4_dryden_altitude_combined_c5_like": (wl("m4dry", 900, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_VEL,
+                                               dict(CIRCLE, circle_radius=0.3, form_radius=0.3, aero_mask=15, wind_sigma=0.5, dryden_airspeed=8.0,
+                                                    target_mode=W.TGT_CIRCLE, wind_mask=15, wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01,
+                                                    wind_sine_omega=3.0, gust_prob=0.1, gust_max=1.5, gust_duration=0.3, int_clamp_pos=1.0,
+                                                    int_clamp_att=0.25), ("uniform", -1.0, 1.0)), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
@@ -276,3 +286,32 @@ def test_sensor_noise_residual_and_refresh_after_set_state():
     assert np.abs(noisy.obs.cpu().numpy() - orc_n.outputs()[0]).max() < 2e-6
     with pytest.raises(mdg.MdgError):
         mdg.Env(4, 1, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, obs_noise=[0.01, -0.05, 0.0, 0.0]))
+
+
+def test_dryden_altitude_wind_state_matches_the_oracle():
+    """The gust state itself under the altitude-dependent length scale: drones parked at hand-picked altitudes (k_wind = 0, hover
+    thrust), so alpha(h) is the only thing that shapes the sequence; compared with the oracle's wind after every step."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    from oracle import oracle as O
+    N, M = 512, 2
+    over = dict(aero_mask=W.AERO_WIND, dryden_airspeed=8.0, k_wind=0.0, wind_sigma=0.7, term_mode=W.TERM_NONE, auto_reset=0, episode_len_s=0.0)
+    gpu = mdg.Env(N, M, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, **over))
+    orc = O.OracleEnv(N, M, W.PHYS_MJC, W.ACT_RPM, O.OracleParams(0, **over), n_threads=4)
+    assert "generic" in gpu.kernel_name
+    gpu.reset(9); orc.reset(9)
+    st = orc.state.astype(np.float32)
+    h = np.linspace(0.01, 3.0, N * M, dtype=np.float32)                # from below the altitude floor to 3 m
+    st[:, 0:3] = np.stack([np.arange(N * M) % M * 0.7, np.zeros(N * M), h], axis=1)
+    orc.state = st.astype(np.float64)
+    gpu.set_state(state=st)
+    a = np.full((N * M, 4), W.hover_rpm_f32(), dtype=np.float32)
+    a_dev = torch.from_numpy(a).cuda()
+    for t in range(24):
+        gpu.step(a_dev); orc.step(a)
+        w32, w64 = gpu.get_state()["wind"].astype(np.float64), orc.wind
+        assert np.abs(w32 - w64).max() < 5e-6, (t, np.abs(w32 - w64).max())
+    assert w64.std() > 0.2
+    with pytest.raises(mdg.MdgError):
+        mdg.Env(4, 1, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, dryden_airspeed=-1.0))
