@@ -20,7 +20,9 @@
 // velocity-tracking and fly-through epilogues, Table 4 factors and initial ranges, constant / sinusoidal wind;
 // tests/test_oracle_sensors.py: Table 4 sensor noise and the per-episode observation bias (table standard deviations,
 // normality, independence, which columns move, constancy over an episode, keying by global env index);
-// tests/test_oracle_dryden.py: altitude-dependent Dryden length scale (printed values, first updates, AR(1) statistics by altitude).
+// tests/test_oracle_dryden.py: altitude-dependent Dryden length scale (printed values, first updates, AR(1) statistics by altitude);
+// tests/test_oracle_latency.py: action / sensor latency (thrust-step and free-fall closed forms per substep of delay, shift
+// equivalence for the controller action types, uniform per-episode delays).
 // PARITY UNPINNED (the oracle itself is the reference): the coupled PID transient in x/y and the
 // multi-config trajectories beyond the invariants above; parity against MuJoCo's own RK4 (MuJoCo is
 // not in the container, reading Q11).
@@ -103,6 +105,10 @@ struct Params {
     // alpha = e^(-dt V / L)", reading Q50): V = dryden_airspeed (m/s; 0 = the fixed-tau form above), h = mean altitude of the
     // env's drones at the start of the control step, not below dryden_h_min
     double dryden_airspeed, dryden_h_min;
+    // Table 4 latency rows ("action latency U[0, 50] ms (per ep.)", "sensor latency U[0, 20] ms (per ep.)";
+    // reading Q51): ranges in seconds, quantised to physics substeps; one delay per drone and episode, uniform over the
+    // integers round(lo sim_freq) .. round(hi sim_freq).  Action latency at most 3 control steps, sensor latency at most 1.
+    double act_latency_lo, act_latency_hi, obs_latency_lo, obs_latency_hi;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_LAG = 14 /* tau_mot in seconds, not a factor */, DR_N = 16 };
@@ -538,6 +544,7 @@ struct Sim {
     std::vector<double> reward_d; // [D] per-drone share of the reward (MultiAgentAviary); sums to reward[e]
     std::vector<uint8_t> done;    // [N] bit0 terminated, bit1 truncated
     std::vector<double> margin;   // [N][3] smallest distance to a done / reward / adjacency threshold
+    std::vector<float> ahist;     // [D][3][4] the action rows issued 1, 2 and 3 control steps ago (action latency, Q51)
 
     int opd() const { return P.obs_mode == OBS_KIN20 ? 20 : P.obs_mode == OBS_KIN12_TGT ? 16 : P.obs_mode == OBS_KIN12_WP ? 18 : P.obs_mode == OBS_KIN12_Z ? 13 : 12 + (P.obs_mode == OBS_KIN12_ADJ ? M : 0); }
     int obs_dim() const { return M * opd(); }
@@ -551,6 +558,7 @@ struct Sim {
         gust.assign((size_t)N * 4, 0.0); for (int e = 0; e < N; ++e) gust[(size_t)e * 4 + 3] = 1.0;
         obs.assign((size_t)N * obs_dim(), 0.0); reward.assign(N, 0.0); reward_d.assign((size_t)N * M, 0.0); done.assign(N, 0);
         margin.assign((size_t)N * 3, 1e30);
+        ahist.assign(Dn * 12, 0.0f);
         for (size_t i = 0; i < Dn; ++i) state[i * 13 + 3] = 1.0;
     }
 
@@ -685,9 +693,11 @@ struct Sim {
     }
     bool sensors_on() const { for (int a = 0; a < 4; ++a) if (P.obs_noise[a] != 0.0 || P.obs_bias[a] != 0.0) return true; return false; }
 
-    template <class R> void write_obs(int e, const Drone<R>* dr, double& adj_margin, uint32_t t) {
+    // sensed: the state each drone's kinematic entries are read from (sensor latency, Q51); nullptr = the current state
+    template <class R> void write_obs(int e, const Drone<R>* dr_true, double& adj_margin, uint32_t t, const Drone<R>* sensed = nullptr) {
         const int od = opd();
         const bool noisy = sensors_on();
+        const Drone<R>* dr = sensed ? sensed : dr_true;             // [p, q, eta, v, omega]; targets are the same in both
         double* o = &obs[(size_t)e * obs_dim()];
         adj_margin = 1e30;
         for (int i = 0; i < M; ++i) {
@@ -712,15 +722,15 @@ struct Sim {
                 for (int a = 0; a < 4; ++a) oi[12 + a] = dr[i].tg[a];
             if (P.obs_mode == OBS_KIN12_Z) oi[12] = dr[i].tg[2];   // kinematic state plus target altitude (13)
             if (P.obs_mode == OBS_KIN12_WP) {                      // next waypoint and its position in the body frame
-                R Rm[3][3], rel[3] = {dr[i].tg[0] - dr[i].p[0], dr[i].tg[1] - dr[i].p[1], dr[i].tg[2] - dr[i].p[2]}, rb[3];
-                rotmat(dr[i].q, Rm);
+                R Rm[3][3], rel[3] = {dr_true[i].tg[0] - dr_true[i].p[0], dr_true[i].tg[1] - dr_true[i].p[1], dr_true[i].tg[2] - dr_true[i].p[2]}, rb[3];
+                rotmat(dr_true[i].q, Rm);
                 matT_vec(Rm, rel, rb);
-                for (int a = 0; a < 3; ++a) { oi[12 + a] = dr[i].tg[a]; oi[15 + a] = to_d(rb[a]); }
+                for (int a = 0; a < 3; ++a) { oi[12 + a] = dr_true[i].tg[a]; oi[15 + a] = to_d(rb[a]); }
             }
             if (P.obs_mode == OBS_KIN12_ADJ) {
                 for (int k = 0; k < M; ++k) {
                     if (k == i) { oi[12 + k] = 1.0; continue; }
-                    const R dx = dr[i].p[0] - dr[k].p[0], dy = dr[i].p[1] - dr[k].p[1], dz = dr[i].p[2] - dr[k].p[2];
+                    const R dx = dr_true[i].p[0] - dr_true[k].p[0], dy = dr_true[i].p[1] - dr_true[k].p[1], dz = dr_true[i].p[2] - dr_true[k].p[2];
                     const R dist = sqrt(dx * dx + dy * dy + dz * dz);
                     oi[12 + k] = (dist < P.adj_radius) ? 1.0 : 0.0;
                     const double mg = std::fabs(to_d(dist) - P.adj_radius);
@@ -785,17 +795,63 @@ struct Sim {
                 for (int a = 0; a < 3; ++a) dr[i].Fwind[a] = (drag ? (P.k_wind * nr) * rel[a] : R(0.0)) + fs[a];
             }
         }
+        // Table 4 latency rows (Q51): this episode's delays in physics substeps, drawn at the reset index t0 of the episode
+        const bool lat_a = P.act_latency_hi > 0.0, lat_s = P.obs_latency_hi > 0.0;
+        std::vector<int> d_act(M, 0), d_obs(M, 0), sw(M, -1);
+        std::vector<Drone<R>> later(M), snap(M);                   // rotor commands after the switch; sensed state
+        if (lat_a || lat_s) {
+            const int a_lo = (int)std::floor(P.act_latency_lo * P.sim_freq + 0.5), a_hi = (int)std::floor(P.act_latency_hi * P.sim_freq + 0.5);
+            const int s_lo = (int)std::floor(P.obs_latency_lo * P.sim_freq + 0.5), s_hi = (int)std::floor(P.obs_latency_hi * P.sim_freq + 0.5);
+            const uint32_t t0 = (t - 1u) - ep_step[e];
+            for (int i = 0; i < M; ++i) {
+                const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, (uint32_t)i, t0, STREAM_LATENCY, k0, k1);
+                d_act[i] = a_lo + (int)(((uint64_t)(r.x[0] >> 8) * (uint64_t)(a_hi - a_lo + 1)) >> 24);   // uniform over a_lo..a_hi
+                d_obs[i] = s_lo + (int)(((uint64_t)(r.x[1] >> 8) * (uint64_t)(s_hi - s_lo + 1)) >> 24);
+            }
+        }
+        const bool direct = action_type == ACT_RPM || action_type == ACT_RPM_NORM || action_type == ACT_ONE_D_RPM;
         // O2/O3 decode, O4 motor model
         for (int i = 0; i < M; ++i) {
-            decode_action(P, D, action_type, actions + ((size_t)e * M + i) * 4, dr[i]);
-            for (int a = 0; a < 4; ++a) dr[i].act[a] = (double)actions[((size_t)e * M + i) * 4 + a];
+            const float* a_now = actions + ((size_t)e * M + i) * 4;
+            const float* a_first = a_now;                           // the row in effect when the control step starts
+            if (lat_a) {
+                // The row issued at control step t arrives d substeps later: substep k of step t runs the row of step
+                // t + floor((k - d) / K).  With d = (n - 1) K + r, 1 <= r <= K: row t - n for k < r, row t - n + 1 from k = r on.
+                // A controller (PID / VEL / ATTITUDE) decodes once per control step, from the row that has arrived by then.
+                float* H = &ahist[((size_t)e * M + i) * 12];        // H[0..3] = a_{t-1}, H[4..7] = a_{t-2}, H[8..11] = a_{t-3}
+                if (ep_step[e] == 0) for (int r = 0; r < 3; ++r) for (int a = 0; a < 4; ++a) H[4 * r + a] = a_now[a];   // primed with the episode's first row
+                const int n = (d_act[i] + D.K - 1) / D.K, r = d_act[i] - (n - 1) * D.K;
+                float rows[4][4];
+                for (int a = 0; a < 4; ++a) { rows[0][a] = a_now[a]; rows[1][a] = H[a]; rows[2][a] = H[4 + a]; rows[3][a] = H[8 + a]; }
+                float first[4], second[4];
+                for (int a = 0; a < 4; ++a) { first[a] = rows[n][a]; second[a] = rows[n > 0 ? n - 1 : 0][a]; }
+                for (int a = 0; a < 4; ++a) { H[8 + a] = H[4 + a]; H[4 + a] = H[a]; H[a] = a_now[a]; }
+                decode_action(P, D, action_type, first, dr[i]);
+                if (direct && n >= 1 && r < D.K) {
+                    later[i] = dr[i];
+                    decode_action(P, D, action_type, second, later[i]);
+                    sw[i] = r;
+                }
+                a_first = nullptr;
+            }
+            if (a_first) decode_action(P, D, action_type, a_first, dr[i]);
+            for (int a = 0; a < 4; ++a) dr[i].act[a] = (double)a_now[a];   // KIN20 reports the row the policy issued
             if (dr[i].sc[DR_MAXRPM] != 1.0)                         // Table 4: the true motor saturation of this episode
-                for (int a = 0; a < 4; ++a) if (dr[i].n[a] > D.max_rpm * dr[i].sc[DR_MAXRPM]) dr[i].n[a] = D.max_rpm * dr[i].sc[DR_MAXRPM];
+                for (int a = 0; a < 4; ++a) {
+                    if (dr[i].n[a] > D.max_rpm * dr[i].sc[DR_MAXRPM]) dr[i].n[a] = D.max_rpm * dr[i].sc[DR_MAXRPM];
+                    if (sw[i] >= 0 && later[i].n[a] > D.max_rpm * dr[i].sc[DR_MAXRPM]) later[i].n[a] = D.max_rpm * dr[i].sc[DR_MAXRPM];
+                }
             motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
         }
+        if (lat_s) for (int i = 0; i < M; ++i) if (d_obs[i] >= D.K) snap[i] = dr[i];   // a full step old: the state the step starts from
         // K substeps: all wrenches from the same start-of-substep state, then integrate
         const bool lag = P.motor_lag_hi > 0.0;
         for (int k = 0; k < D.K; ++k) {
+            for (int i = 0; i < M; ++i)
+                if (sw[i] == k) {                                  // Q51: the next row arrives at this substep
+                    for (int a = 0; a < 4; ++a) dr[i].n[a] = later[i].n[a];
+                    motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
+                }
             if (lag)                                               // Q44: n <- n + (1 - e^(-h/tau)) (n_cmd - n), then Eq.1-3 with n
                 for (int i = 0; i < M; ++i) {
                     const double gam = 1.0 - std::exp(-D.h / dr[i].sc[DR_LAG]);
@@ -804,6 +860,7 @@ struct Sim {
                 }
             for (int i = 0; i < M; ++i) substep_wrench(P, D, dr, M, i);
             for (int i = 0; i < M; ++i) integrate(P, D, dr[i]);
+            if (lat_s) for (int i = 0; i < M; ++i) if (k + 1 == D.K - d_obs[i]) snap[i] = dr[i];   // what the sensors report d_obs substeps later
         }
         store(e, dr);
         // O10 reward / termination from the end-of-step state
@@ -891,11 +948,17 @@ struct Sim {
         reward[e] = to_d(rew);
         done[e] = (uint8_t)((terminated ? 1 : 0) | (truncated ? 2 : 0));
         // O11 auto-reset (Q29): reward/done describe the finished transition, obs opens the new episode
+        bool fresh = false;
         if (done[e] && P.auto_reset) {
             reset_env(e, t);
             load(e, dr);
+            fresh = true;                                          // the new episode's first row is its initial state
         }
         double m_adj;
+        if (lat_s && !fresh) {
+            for (int i = 0; i < M; ++i) { for (int a = 0; a < 4; ++a) { snap[i].tg[a] = dr[i].tg[a]; snap[i].act[a] = dr[i].act[a]; } }
+            write_obs(e, dr, m_adj, t, snap.data());
+        } else
         write_obs(e, dr, m_adj, t);
         margin[(size_t)e * 3 + 0] = m_done; margin[(size_t)e * 3 + 1] = m_rew; margin[(size_t)e * 3 + 2] = m_adj;
     }

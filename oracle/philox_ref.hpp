@@ -37,7 +37,8 @@ inline PhiloxOut philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
 inline double u01(uint32_t x) { return (double)(x >> 8) * (1.0 / 16777216.0); }
 
 enum : uint32_t { STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9, STREAM_GUST = 10,
-                  STREAM_OBS_NOISE = 11 /* 11..13: three calls = 12 normals per drone and step */, STREAM_OBS_BIAS = 14 /* 14..16, per episode */ };
+                  STREAM_OBS_NOISE = 11 /* 11..13: three calls = 12 normals per drone and step */, STREAM_OBS_BIAS = 14 /* 14..16, per episode */,
+                  STREAM_LATENCY = 17 /* per episode: word 0 action latency, word 1 sensor latency */ };
 static const uint32_t ENV_LEVEL = 0xFFFFFFFFu;
 
 }  // namespace orc
