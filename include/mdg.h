@@ -4,7 +4,8 @@
  * by one control step of arxiv/paper_2606_08039 ("MuJoCo-Drones-Gym"): action decode (PAPER.md:171-187
  * Table 3; cascaded PID PAPER.md:347-376), rotor model (Eq.1-3), ground effect / blade
  * drag / downwash (Eq.4-6), wind (Dryden-style gust, constant, impulse gusts,
- * sinusoidal), per-episode domain randomisation (Table 4), free-body integration over
+ * sinusoidal), per-episode domain randomisation incl. motor lag, action / sensor latency and sensor noise (Table 4,
+ * PAPER.md:229-248), free-body integration over
  * sim_freq/ctrl_freq substeps, observation, reward, termination and
  * auto-reset, and, as a separate call, the onboard depth / segmentation camera
  * (PAPER.md:177).  The interface follows the paper's statement of the
@@ -134,6 +135,15 @@ typedef struct mdg_params {
      * alpha = exp(-dt V / L); reading Q50): dryden_airspeed = V in m/s (0, the default, keeps the fixed wind_tau),
      * h = the mean altitude of the env's drones at the start of the control step, not below dryden_h_min (0.05 m). */
     float dryden_airspeed, dryden_h_min;
+    /* Table 4 latency rows (reading Q51), ranges in seconds, one delay per drone and episode,
+     * uniform over the whole numbers of physics substeps round(lo sim_freq) .. round(hi sim_freq); hi = 0 (default) = off.
+     * Action latency (table: 0 - 0.050; at most 3 control steps): the row issued at a control step takes effect that many
+     * substeps later; rotor-command rows (RPM, RPM_NORM, ONE_D_RPM) switch at the exact substep, the controller types decode
+     * once per control step from the row that has arrived by then; until the episode's first row arrives that row is used.
+     * Sensor latency (table: 0 - 0.020; at most 1 control step): the kinematic entries of the observation (p, quaternion,
+     * roll/pitch/yaw, v, body rates) are the state that many substeps before the end of the step; the first row after a
+     * reset / auto-reset is the initial state.  Both outside their window: MDG_EINVAL. */
+    float act_latency_lo, act_latency_hi, obs_latency_lo, obs_latency_hi;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

@@ -39,6 +39,7 @@ class mdg_params(C.Structure):
         ("wp_bonus", C.c_float), ("wp_shaping", C.c_float), ("wp_speed", C.c_float), ("wp_omega", C.c_float), ("wp_laps", C.c_int32),
         ("obs_noise", C.c_float * 4), ("obs_bias", C.c_float * 4),
         ("dryden_airspeed", C.c_float), ("dryden_h_min", C.c_float),
+        ("act_latency_lo", C.c_float), ("act_latency_hi", C.c_float), ("obs_latency_lo", C.c_float), ("obs_latency_hi", C.c_float),
     ]
 
     def update(self, d):

@@ -35,6 +35,7 @@ struct mdg_env {
     DevParams P;
     DevBuffers B;
     void* arena = nullptr;
+    void* hist = nullptr;   // action-history planes H0..H2 (action latency only; outside the arena so that its layout never moves)
     size_t arena_bytes = 0;
     cudaStream_t stream = 0;
     cudaStream_t capture_stream = nullptr;
@@ -74,6 +75,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     if (p.motor_lag_hi > 0.0f) f |= F_DR | F_MLAG;
     if ((aero & MDG_AERO_WIND) && (p.wind_mask != MDG_WIND_DRYDEN || p.dryden_airspeed > 0.0f)) f |= F_WIND_MIX;
     for (int i = 0; i < 4; ++i) if (p.obs_noise[i] != 0.0f || p.obs_bias[i] != 0.0f) f |= F_SENS;
+    if (p.act_latency_hi > 0.0f || p.obs_latency_hi > 0.0f) f |= F_LAT;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
     if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
@@ -155,6 +157,12 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
     D.motor_lag_lo = p.motor_lag_lo; D.motor_lag_hi = p.motor_lag_hi;
     for (int i = 0; i < 4; ++i) { D.obs_noise[i] = p.obs_noise[i]; D.obs_bias[i] = p.obs_bias[i]; }
+    {   // Table 4 latency rows in substeps (Q51): uniform over round(lo f_sim) .. round(hi f_sim)
+        const int a_lo = (int)std::floor((double)p.act_latency_lo * p.sim_freq + 0.5), a_hi = (int)std::floor((double)p.act_latency_hi * p.sim_freq + 0.5);
+        const int s_lo = (int)std::floor((double)p.obs_latency_lo * p.sim_freq + 0.5), s_hi = (int)std::floor((double)p.obs_latency_hi * p.sim_freq + 0.5);
+        D.lat_a_lo = a_lo; D.lat_a_n = p.act_latency_hi > 0.0f ? a_hi - a_lo + 1 : 0;
+        D.lat_s_lo = s_lo; D.lat_s_n = p.obs_latency_hi > 0.0f ? s_hi - s_lo + 1 : 0;
+    }
     D.wp_total = p.n_waypoints * p.wp_laps; D.wp_bonus = p.wp_bonus; D.wp_shaping = p.wp_shaping; D.wp_speed = p.wp_speed; D.wp_omega = p.wp_omega;
     D.n_waypoints = p.n_waypoints; D.wp_radius2 = (float)((double)p.wp_radius * p.wp_radius);
     for (int i = 0; i < 24; ++i) D.waypoints[i] = p.waypoints[i];
@@ -327,6 +335,13 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (p.obs_mode < 0 || p.obs_mode > 5 || p.n_waypoints < 0 || p.n_waypoints > 8 || p.motor_lag_lo < 0 || p.motor_lag_hi < p.motor_lag_lo || p.wp_laps < 0 || (p.wind_mask & ~15) || !(p.gust_duration > 0) || p.drone_model < 0 || p.drone_model > 2 || p.reward_mode < 0 || p.reward_mode > 5 || p.term_mode < 0 || p.term_mode > 3 ||
         p.reset_layout < 0 || p.reset_layout > 2 || p.target_mode < 0 || p.target_mode > 4 || p.integrator > 1 || p.aero_mask > 15)
         return fail(MDG_EINVAL, "mdg_create: enum field out of range in params");
+    {
+        const int Ks = p.sim_freq / p.ctrl_freq;
+        if (!(p.act_latency_lo >= 0) || !(p.act_latency_hi >= p.act_latency_lo) || std::floor((double)p.act_latency_hi * p.sim_freq + 0.5) > 3 * Ks)
+            return fail(MDG_EINVAL, "mdg_create: action latency must satisfy 0 <= lo <= hi <= 3 control steps");
+        if (!(p.obs_latency_lo >= 0) || !(p.obs_latency_hi >= p.obs_latency_lo) || std::floor((double)p.obs_latency_hi * p.sim_freq + 0.5) > Ks)
+            return fail(MDG_EINVAL, "mdg_create: sensor latency must satisfy 0 <= lo <= hi <= 1 control step");
+    }
     if (!(p.dryden_airspeed >= 0) || (p.dryden_airspeed > 0 && !(p.dryden_h_min > 0)))
         return fail(MDG_EINVAL, "mdg_create: dryden_airspeed must be >= 0 and dryden_h_min > 0");
     for (int i = 0; i < 4; ++i)
@@ -372,13 +387,19 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     h->B.ticket = (unsigned*)c; c += 256;
     h->B.reward_d = (float*)(c + al(n_items_max * 4));
     h->B.item_seq = (unsigned*)c;
+    if (h->P.lat_a_n > 0) {
+        ce = cudaMalloc(&h->hist, 3 * plane);
+        if (ce == cudaSuccess) ce = cudaMemset(h->hist, 0, 3 * plane);
+        if (ce != cudaSuccess) { cudaFree(h->arena); if (h->hist) cudaFree(h->hist); delete h; return fail(MDG_ENOMEM, std::string("mdg_create: cudaMalloc (action history): ") + cudaGetErrorString(ce)); }
+        h->B.H0 = (float4*)h->hist; h->B.H1 = (float4*)((char*)h->hist + plane); h->B.H2 = (float4*)((char*)h->hist + 2 * plane);
+    }
     int rc = configure_launch(h);
     if (rc == MDG_OK && h->saturating) {     // throughput-bound batch: the 5-blocks-per-SM register budget measured fastest
         h->minb = 5;
         pick_kernels(h);
         rc = configure_launch(h);
     }
-    if (rc != MDG_OK) { cudaFree(h->arena); delete h; return rc; }
+    if (rc != MDG_OK) { cudaFree(h->arena); if (h->hist) cudaFree(h->hist); delete h; return rc; }
     *out = h;
     rc = mdg_reset(h, 0);
     if (rc != MDG_OK) { mdg_destroy(h); *out = nullptr; return rc; }
@@ -392,6 +413,7 @@ void mdg_destroy(mdg_env* h) {
     drop_graphs(h);
     if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
     if (h->arena) cudaFree(h->arena);
+    if (h->hist) cudaFree(h->hist);
     delete h;
 }
 

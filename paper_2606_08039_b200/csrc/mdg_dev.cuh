@@ -22,6 +22,7 @@ enum : int {
     F_DR = 1 << 21,                                       // per-episode domain-randomisation factors (Table 4)
     F_MLAG = 1 << 23,                                     // motor lag: rotor-speed state, wrench recomputed every substep
     F_SENS = 1 << 24,                                     // Table 4 sensor rows: noise / per-episode bias on the emitted observation
+    F_LAT = 1 << 25,                                      // Table 4 latency rows: delayed action rows / sensed state (generic kernel)
     F_WIND_MIX = 1 << 22,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
 };
 
@@ -66,6 +67,7 @@ struct DevParams {
     float dr_alpha[12];                                   // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g, motor, arm, max_rpm, -]
     float reset_rpy_half[3], reset_vel_half[3];           // Table 4 "init" row
     float motor_lag_lo, motor_lag_hi;                     // Table 4 motor lag: range of the time constant (s)
+    int lat_a_lo, lat_a_n, lat_s_lo, lat_s_n;             // Table 4 latency rows in substeps: smallest delay and number of values (0 = off)
     float obs_noise[4], obs_bias[4];                      // Table 4 sensor rows: standard deviations for [position, velocity, RPY, body rates]
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
@@ -84,6 +86,9 @@ struct DevBuffers {
     float4* R2;   // DR per-motor thrust bias
     float4* R3;   // DR arm, MAX_RPM, motor-lag time constant, -
     float4* N0;   // rotor speeds actually turning (motor lag state)
+    float4* H0;   // action rows issued 1, 2 and 3 control steps ago (action latency; allocated only when it is on)
+    float4* H1;
+    float4* H2;
     float4* E0;   // wind x y z, bits(ep_step)
     float4* E1;   // running gust impulse: velocity x y z, progress s (>= 1: none)
     uint32_t* gstep;
@@ -96,7 +101,7 @@ struct DevBuffers {
 };
 
 static const uint32_t STREAM_RESET_POS = 0, STREAM_RESET_EXTRA = 1, STREAM_WIND = 2, STREAM_ACTION = 3, STREAM_DR0 = 4, STREAM_DR1 = 5, STREAM_DR2 = 6, STREAM_DR3 = 7, STREAM_INIT_RPY = 8, STREAM_INIT_VEL = 9, STREAM_GUST = 10,
-                      STREAM_OBS_NOISE = 11 /* 11..13 */, STREAM_OBS_BIAS = 14 /* 14..16 */;
+                      STREAM_OBS_NOISE = 11 /* 11..13 */, STREAM_OBS_BIAS = 14 /* 14..16 */, STREAM_LATENCY = 17;
 
 // Philox4x32-10 (Salmon et al., SC'11).  key = seed halves, counter = (env, drone|~0, step, stream).
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,

@@ -283,9 +283,31 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         }
     }
 
+    // Table 4 latency rows (Q51), generic kernel only: this episode's delays in substeps from one Philox draw at the
+    // episode's reset index.  The row issued at step t runs from substep d on: with d = (n - 1) K + r, 1 <= r <= K, substeps
+    // k < r of this step run the row of n steps ago, the rest the row after it.  A controller decodes once, from the first.
+    float4 a_first = act4, a_second = act4;
+    int sw = -1, d_obs = 0;
+    if (FEAT < 0 && F::has(P, F_LAT)) {
+        const uint32_t ep0 = __float_as_uint(env4.w);
+        const uint4 lr = philox4x32_10(e + P.env_base, (uint32_t)jj, (t - 1u) - ep0, STREAM_LATENCY, P.seed_lo, P.seed_hi);
+        d_obs = P.lat_s_lo + (int)(((lr.y >> 8) * (uint32_t)P.lat_s_n) >> 24);
+        if (P.lat_a_n > 0) {
+            const int d_act = P.lat_a_lo + (int)(((lr.x >> 8) * (uint32_t)P.lat_a_n) >> 24);
+            float4 h0 = B.H0[drone], h1 = B.H1[drone], h2 = B.H2[drone];
+            if (ep0 == 0u) h0 = h1 = h2 = act4;                    // primed with the episode's first row
+            const int nb = (d_act + P.K - 1) / P.K, r = d_act - (nb - 1) * P.K;
+            a_first = nb == 0 ? act4 : nb == 1 ? h0 : nb == 2 ? h1 : h2;
+            a_second = nb <= 1 ? act4 : nb == 2 ? h0 : h1;
+            const int at = F::act(P);
+            if ((at == 0 || at == 3 || at == 4) && nb >= 1 && r < P.K) sw = r;
+            if (active) { B.H2[drone] = h1; B.H1[drone] = h0; B.H0[drone] = act4; }
+        }
+    }
     // S1/S2 decode, S3 motor model (Eq.1-3); RPMs are held over the K substeps
-    float n[4];
-    decode_action<FEAT>(P, act4, d, n);
+    float n[4], n_later[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    decode_action<FEAT>(P, a_first, d, n);
+    if (FEAT < 0 && sw >= 0) { DroneRegs dtmp = d; decode_action<FEAT>(P, a_second, dtmp, n_later); }   // direct rotor commands: stateless
     // Domain randomisation (Table 4): this episode's factors scale the true vehicle, not the controller's model above.
     // 1 / s_J is folded into the body torque (every stage torque is linear in it, the gyroscopic ratios do not change).
     const bool dr = F::has(P, F_DR);
@@ -295,6 +317,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     if (dr) {                                                      // true motor saturation of this episode
         const float nmax = P.max_rpm * dr3.y;
         n[0] = fminf(n[0], nmax); n[1] = fminf(n[1], nmax); n[2] = fminf(n[2], nmax); n[3] = fminf(n[3], nmax);
+        n_later[0] = fminf(n_later[0], nmax); n_later[1] = fminf(n_later[1], nmax); n_later[2] = fminf(n_later[2], nmax); n_later[3] = fminf(n_later[3], nmax);
     }
     // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag
     float T, cxy, dcz, gndT;
@@ -328,8 +351,13 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const bool flush = pending2 != 0xFFFFFFFFu;                  // two items wait: fence now, flags after the substeps
     if (flush) __threadfence();
     MDG_T(2);
+    Sensed snap = sensed(d, v3(0, 0, 0));                          // sensor latency of a whole step: the state the step starts from
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
+        if (FEAT < 0 && sw == k) {                                 // Q51: the next row arrives at this substep
+            n[0] = n_later[0]; n[1] = n_later[1]; n[2] = n_later[2]; n[3] = n_later[3];
+            if (!lag) motor_model(n);
+        }
         if (lag) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) n_act[i] = fmaf(lag_gain, n[i] - n_act[i], n_act[i]);
@@ -402,6 +430,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             else integrate_rot<false, true, DEG>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
         }
         if (d.p.z < 0.0f) { hit = true; d.p.z = 0.0f; d.v.z = fmaxf(d.v.z, 0.0f); }   // floor
+        if (FEAT < 0 && F::has(P, F_LAT) && k + 1 == P.K - d_obs) snap = sensed(d, v3(0, 0, 0));   // what the sensors report d_obs substeps later
     }
 
     MDG_T(3);
@@ -518,6 +547,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             if (F::act(P) == 1) B.P5[drone] = d.sp;
         }
         Sensed sn = sensed(d, eta);
+        if (FEAT < 0 && F::has(P, F_LAT) && !do_reset) { sn = snap; sn.eta = euler_zyx(snap.q); }   // a new episode's first row is its initial state
         if (FEAT < 0 && F::has(P, F_SENS)) sense(P, e, (uint32_t)jj, t, ep_out, sn);   // Table 4 sensor rows: the stored state stays exact
         write_obs<G>(P, B.obs, drone, d, sn, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
         B.reward_d[drone] = r;

@@ -201,8 +201,8 @@ __device__ __forceinline__ float4 normals4(uint4 r) {
 // Table 4 sensor rows (reading Q49): what the observation emitted at step index t reports for
 // [p, eta, v, omega] = the true value + sigma xi (xi fresh every step, streams 11..13) + beta b (b drawn at the reset
 // index t - ep_step of the running episode, streams 14..16).  The twelve values follow the row order p, eta, v, omega.
-struct Sensed { V3 p, eta, v, w; };                               // the twelve kinematic entries as the observation reports them
-__device__ __forceinline__ Sensed sensed(const DroneRegs& d, V3 eta) { Sensed s; s.p = d.p; s.eta = eta; s.v = d.v; s.w = d.w; return s; }
+struct Sensed { V3 p, eta, v, w; Q4 q; };                         // the kinematic entries as the observation reports them
+__device__ __forceinline__ Sensed sensed(const DroneRegs& d, V3 eta) { Sensed s; s.p = d.p; s.eta = eta; s.v = d.v; s.w = d.w; s.q = d.q; return s; }
 __device__ __forceinline__ void sense(const DevParams& P, unsigned e, uint32_t j, uint32_t t, uint32_t ep_step, Sensed& s) {
     const uint32_t eg = e + P.env_base, t0 = t - ep_step;
     const float4 n0 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE, P.seed_lo, P.seed_hi));
@@ -228,8 +228,8 @@ __device__ __forceinline__ void write_obs(const DevParams& P, float* __restrict_
     float* o = obs + drone * (size_t)P.opd;
     if (mode == 2) {
         float4* o4 = reinterpret_cast<float4*>(o);                 // 20 floats per drone: always 16 B aligned
-        o4[0] = make_float4(s.p.x, s.p.y, s.p.z, d.q.w);
-        o4[1] = make_float4(d.q.x, d.q.y, d.q.z, s.eta.x);
+        o4[0] = make_float4(s.p.x, s.p.y, s.p.z, s.q.w);
+        o4[1] = make_float4(s.q.x, s.q.y, s.q.z, s.eta.x);
         o4[2] = make_float4(s.eta.y, s.eta.z, s.v.x, s.v.y);
         o4[3] = make_float4(s.v.z, s.w.x, s.w.y, s.w.z);
         o4[4] = act;

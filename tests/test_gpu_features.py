@@ -32,6 +32,9 @@ INIT = dict(reset_rpy_half=[0.1, 0.1, 0.1], reset_vel_half=[0.5, 0.5, 0.5])   # 
 SENS = dict(obs_noise=[0.01, 0.05, 0.0174533, 0.05], obs_bias=[0.02, 0.03, 0.01, 0.04])   # Table 4 "sensors" rows; bias: PAPER.md:248 (iii)
 
 
+LAT = dict(act_latency_lo=0.0, act_latency_hi=0.050, obs_latency_lo=0.0, obs_latency_hi=0.020)   # Table 4 "action latency", "sensor latency"
+
+
 def wl(name, n, m, phys, act, params, actions, seed=77):
     return W.Workload(name, n, m, phys, act, params, actions, 48, W.BASE_SEED + seed)
 
@@ -152,6 +155,25 @@ CASES = {
                                                     target_mode=W.TGT_CIRCLE, wind_mask=15, wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01,
                                                     wind_sine_omega=3.0, gust_prob=0.1, gust_max=1.5, gust_duration=0.3, int_clamp_pos=1.0,
                                                     int_clamp_att=0.25), ("uniform", -1.0, 1.0)), {}),
+    # Table 4 latency rows: action latency 0-50 ms and sensor latency 0-20 ms per episode (short episodes -> redraws); rotor
+    # commands switch at the exact substep, controllers decode from the row that has arrived
+    "m1_latency_rpm": (wl("m1lat", 1500, 1, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(SINGLE, episode_len_s=0.3, **LAT), HOVER), {}),
+    "m1_latency_pid": (wl("m1latpid", 1500, 1, W.PHYS_MJC, W.ACT_PID,
+                          dict(reset_center=[0, 0, 1], reset_half=[0.1, 0.1, 0.1], reward_mode=W.REW_NEG_SQ_DIST, term_mode=W.TERM_TILT_DIST,
+                               term_tilt=0.4, term_dist=3.0, target_mode=W.TGT_BOX, target_lo=[-1, -1, 0.2], target_hi=[1, 1, 2.0],
+                               episode_len_s=0.25, auto_reset=1, **LAT), ("targets",)), {}),
+    "m3_latency_kin20_norm": (wl("m3lat", 500, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM_NORM, dict(GRID, obs_mode=W.OBS_KIN20, episode_len_s=0.3, **LAT),
+                                 ("uniform", -0.1, 0.12)), {}),
+    "m4_latency_c5_like_everything": (wl("m4lat", 900, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_VEL,
+                                         dict(CIRCLE, circle_radius=0.3, form_radius=0.3, aero_mask=15, wind_sigma=0.5, wind_tau=1.0, target_mode=W.TGT_CIRCLE,
+                                              int_clamp_pos=1.0, int_clamp_att=0.25, episode_len_s=0.4, **LAT, **SENS), ("uniform", -1.0, 1.0)), {}),
+    "m4_latency_motor_lag_dr": (wl("m4latlag", 700, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
+                                   dict(GRID, grid_cols=2, episode_len_s=0.3, dr_alpha=DR, motor_lag_lo=0.005, motor_lag_hi=0.05, **INIT, **LAT), HOVER), {}),
+    "m1_latency_action_only_one_d": (wl("m1lat1d", 1300, 1, W.PHYS_MJC_GND, W.ACT_ONE_D_RPM, dict(SINGLE, episode_len_s=0.5, act_latency_lo=0.004, act_latency_hi=0.06),
+                                        ("uniform", -0.3, 0.3)), {}),
+    "m2_latency_sensor_only_fly_through": (wl("m2latfly", 800, 2, W.PHYS_MJC_DRAG, W.ACT_RPM,
+                                              dict(GRID, grid_cols=2, reset_z_lo=0.9, reset_z_hi=1.1, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH,
+                                                   target_mode=W.TGT_WAYPOINTS, wp_radius=0.25, episode_len_s=20.0, obs_latency_lo=0.0, obs_latency_hi=0.0208), HOVER), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
@@ -315,3 +337,25 @@ def test_dryden_altitude_wind_state_matches_the_oracle():
     assert w64.std() > 0.2
     with pytest.raises(mdg.MdgError):
         mdg.Env(4, 1, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, dryden_airspeed=-1.0))
+
+
+def test_latency_error_paths_and_graph_replay():
+    """Latency windows outside what the history planes hold are MDG_EINVAL; a CUDA-graph replay of the latency path equals single steps."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    for over in (dict(act_latency_hi=0.070), dict(obs_latency_hi=0.030), dict(act_latency_lo=0.02, act_latency_hi=0.01), dict(obs_latency_lo=-0.01)):
+        with pytest.raises(mdg.MdgError):
+            mdg.Env(4, 1, W.PHYS_MJC, W.ACT_RPM, mdg.default_params(0, **over))
+    w = wl("latgraph", 3000, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, episode_len_s=0.1, **LAT, **SENS), HOVER)
+    a, b = (mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **w.params)) for _ in range(2))
+    a.reset(w.seed); b.reset(w.seed)
+    acts = torch.stack([a.gen_actions(w.seed, t, W.hover_rpm_f32(), 0.9, 1.1) for t in range(6)])
+    for rep in range(2):
+        for t in range(6):
+            a.step(acts[t])
+        b.step_many(acts, 6)
+    torch.cuda.synchronize()
+    sa, sb = a.get_state(), b.get_state()
+    assert np.array_equal(sa["state"], sb["state"]) and np.array_equal(sa["ep_step"], sb["ep_step"])
+    assert torch.equal(a.obs, b.obs) and torch.equal(a.reward, b.reward) and torch.equal(a.done, b.done)
