@@ -175,6 +175,14 @@ int mdg_step_many(mdg_env* env, const float* actions_dev, int n_steps, int64_t s
  * with respect to the host but the call still returns only after they finish. */
 int mdg_step_host(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
 
+/* The same call split in two, for double-buffering several handles (each bound to its own stream with mdg_set_stream) so that
+ * one batch's device-to-host copy overlaps another batch's host-to-device copy and step: mdg_step_host_async enqueues the copy
+ * of the actions, the step and the copies of the outputs on the bound stream and returns at once; the host buffers must be
+ * pinned (page-locked) for the copies to be asynchronous and must not be touched until mdg_wait on the same handle has
+ * returned.  mdg_wait blocks until everything enqueued on the handle's stream has finished.  mdg_step_host = async + wait. */
+int mdg_step_host_async(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
+int mdg_wait(mdg_env* env);
+
 /* Device pointers to the library-owned outputs of the last reset/step:
  * obs [n_envs][mdg_obs_dim] fp32 (per drone: the MDG_OBS_* row, e.g. p, roll/pitch/yaw, v, body rates [, adjacency row]);
  * reward [n_envs] fp32; done [n_envs] u8 (bit0 terminated, bit1 truncated).  Any may be NULL. */

@@ -61,7 +61,7 @@ class mdg_cam_params(C.Structure):
     update = mdg_params.update
 
 
-EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_outputs",
+EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_wait", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
            "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_last_error", "mdg_version"]
 
@@ -85,6 +85,8 @@ def lib():
         L.mdg_step.argtypes = [vp, vp]
         L.mdg_step_many.argtypes = [vp, vp, C.c_int, C.c_int64]
         L.mdg_step_host.argtypes = [vp] * 5
+        L.mdg_step_host_async.argtypes = [vp] * 5
+        L.mdg_wait.argtypes = [vp]
         L.mdg_outputs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.mdg_obs_dim.argtypes = [vp]
         L.mdg_targets.argtypes = [vp, C.POINTER(vp)]
@@ -219,13 +221,19 @@ class Env:
         _check(lib().mdg_step_many(self._h, self._act_ptr(actions, n_steps), n_steps, self.n_envs * self.n_drones * 4))
         return self.obs, self.reward, self.done
 
-    def step_host(self, actions_host, obs_host=None, reward_host=None, done_host=None):
-        """End-to-end step on HOST tensors (ideally pinned): H2D actions, step, D2H outputs, synchronise."""
+    def step_host(self, actions_host, obs_host=None, reward_host=None, done_host=None, asynchronous=False):
+        """End-to-end step on HOST tensors (ideally pinned): H2D actions, step, D2H outputs, synchronise.
+        asynchronous=True only enqueues (mdg_step_host_async); call wait() before reading the host tensors."""
         def ptr(x):
             return C.c_void_p(None) if x is None else C.c_void_p(x.data_ptr())
         if actions_host.is_cuda or actions_host.numel() != self.n_envs * self.n_drones * 4:
             raise ValueError("actions_host must be a host float32 tensor of n_envs*n_drones*4 elements")
-        _check(lib().mdg_step_host(self._h, ptr(actions_host), ptr(obs_host), ptr(reward_host), ptr(done_host)))
+        fn = lib().mdg_step_host_async if asynchronous else lib().mdg_step_host
+        _check(fn(self._h, ptr(actions_host), ptr(obs_host), ptr(reward_host), ptr(done_host)))
+
+    def wait(self):
+        """Block until everything enqueued on this handle's stream has finished (include/mdg.h: mdg_wait)."""
+        _check(lib().mdg_wait(self._h))
 
     def gen_actions(self, seed, t, base, lo, hi, out=None):
         if out is None:

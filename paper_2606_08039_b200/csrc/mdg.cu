@@ -663,7 +663,7 @@ extern "C" int mdg_set_dr(mdg_env* h, const float* f) {
 
 // ---- end-to-end call with host buffers --------------------------------------------------------------
 static std::map<mdg_env*, float*> g_stage;   // device staging buffer for host actions, one per handle
-extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
+extern "C" int mdg_step_host_async(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
     if (!h || !actions_host) return fail(MDG_EINVAL, "mdg_step_host: NULL argument");
     const size_t D = (size_t)h->N * h->M;
     float*& stage = g_stage[h];
@@ -675,8 +675,16 @@ extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_h
     if (obs_host) CU(cudaMemcpyAsync(obs_host, h->B.obs, D * h->P.opd * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
     if (reward_host) CU(cudaMemcpyAsync(reward_host, h->B.reward, (size_t)h->N * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
     if (done_host) CU(cudaMemcpyAsync(done_host, h->B.done, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
+    return MDG_OK;
+}
+extern "C" int mdg_wait(mdg_env* h) {
+    if (!h) return fail(MDG_EINVAL, "mdg_wait: NULL handle");
     CU(cudaStreamSynchronize(h->stream));
     return MDG_OK;
+}
+extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
+    const int rc = mdg_step_host_async(h, actions_host, obs_host, reward_host, done_host);
+    return rc != MDG_OK ? rc : mdg_wait(h);
 }
 extern "C" void mdg_release_staging(mdg_env* h) {   // called by mdg_destroy
     auto it = g_stage.find(h);

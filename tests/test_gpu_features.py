@@ -359,3 +359,32 @@ def test_latency_error_paths_and_graph_replay():
     sa, sb = a.get_state(), b.get_state()
     assert np.array_equal(sa["state"], sb["state"]) and np.array_equal(sa["ep_step"], sb["ep_step"])
     assert torch.equal(a.obs, b.obs) and torch.equal(a.reward, b.reward) and torch.equal(a.done, b.done)
+
+
+def test_async_host_step_on_two_streams_equals_the_synchronous_call():
+    """mdg_step_host_async / mdg_wait: two handles double-buffered on two streams produce, bit for bit, what mdg_step_host does."""
+    import torch
+    import paper_2606_08039_b200 as mdg
+    w = W.config(5).scaled(5000)
+    mk = lambda base: mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **dict(w.params, env_index_base=base)))
+    sync = [mk(0), mk(w.n_envs)]
+    asy = [mk(0), mk(w.n_envs)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for i in range(2):
+        asy[i].set_stream(streams[i])
+        sync[i].reset(w.seed); asy[i].reset(w.seed)
+    torch.cuda.synchronize()
+    acts = [[sync[i].gen_actions(w.seed, t, 1.0, -1.0, 1.0).cpu().pin_memory() for t in range(5)] for i in range(2)]
+    def bufs():
+        return (torch.empty((w.n_envs, sync[0].obs_dim)).pin_memory(), torch.empty(w.n_envs).pin_memory(), torch.empty(w.n_envs, dtype=torch.uint8).pin_memory())
+    bs, ba = [bufs(), bufs()], [bufs(), bufs()]
+    for t in range(5):
+        for i in range(2):
+            sync[i].step_host(acts[i][t], *bs[i])
+        asy[0].step_host(acts[0][t], *ba[0], asynchronous=True)
+        asy[1].step_host(acts[1][t], *ba[1], asynchronous=True)
+        asy[0].wait(); asy[1].wait()
+        for i in range(2):
+            for x, y in zip(bs[i], ba[i]):
+                assert torch.equal(x, y), (t, i)
+    assert bs[0][0].abs().max() > 0.1 and not torch.equal(bs[0][0], bs[1][0])
