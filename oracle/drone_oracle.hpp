@@ -23,7 +23,9 @@
 // tests/test_oracle_dryden.py: altitude-dependent Dryden length scale (printed values, first updates, AR(1) statistics by altitude);
 // tests/test_oracle_latency.py: action / sensor latency (thrust-step and free-fall closed forms per substep of delay, shift
 // equivalence for the controller action types, uniform per-episode delays).
-// PARITY UNPINNED (the oracle itself is the reference): the coupled PID transient in x/y and the
+// tests/test_oracle_pid_transient.py: the coupled x / y PID transient against the linearised cascade (a 6-state discrete
+// linear system iterated in numpy) at several yaw angles and directions.
+// PARITY UNPINNED (the oracle itself is the reference): the large-amplitude (nonlinear) PID transient and the
 // multi-config trajectories beyond the invariants above; parity against MuJoCo's own RK4 (MuJoCo is
 // not in the container, reading Q11).
 #pragma once
