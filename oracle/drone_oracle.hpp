@@ -111,6 +111,10 @@ struct Params {
     // reading Q51): ranges in seconds, quantised to physics substeps; one delay per drone and episode, uniform over the
     // integers round(lo sim_freq) .. round(hi sim_freq).  Action latency at most 3 control steps, sensor latency at most 1.
     double act_latency_lo, act_latency_hi, obs_latency_lo, obs_latency_hi;
+    // FormationAviary's moving centre ("the formation centre tracks a closed polygonal path"; reading Q52): up to 8
+    // vertices (x, y, z each), traversed at form_speed m/s from vertex 0 at episode time 0 and closed back to it;
+    // form_path_n < 2 or form_speed = 0 = the static centre form_center (Q26)
+    int form_path_n; double form_path[24], form_speed;
 };
 enum { WIND_DRYDEN = 1, WIND_CONSTANT = 2, WIND_GUST = 4, WIND_SINE = 8 };
 enum { DR_M = 0, DR_J = 1, DR_KF = 2, DR_KM = 3, DR_DRAG = 4, DR_GND = 5, DR_DW = 6, DR_G = 7, DR_MOTOR = 8 /* 8..11 */, DR_ARM = 12, DR_MAXRPM = 13, DR_LAG = 14 /* tau_mot in seconds, not a factor */, DR_N = 16 };
@@ -278,6 +282,33 @@ template <class R> struct Drone {
     bool hit;                     // sticky floor-hit flag for this control step (Q15)
     double min_abs_pz;            // threshold margin bookkeeping (not part of the method)
 };
+
+// PAPER.md:325, reading Q52: centre of the formation at episode time tau, a point moving at constant speed along the closed
+// polygon V_0 -> V_1 -> ... -> V_{n-1} -> V_0
+inline bool path_on(const Params& P) { return P.target_mode == TGT_CIRCLE && P.form_path_n >= 2 && P.form_speed > 0.0; }
+inline void path_centre(const Params& P, double tau, double c[3]) {
+    for (int a = 0; a < 3; ++a) c[a] = P.form_center[a];
+    if (!path_on(P)) return;
+    const int n = P.form_path_n;
+    double len[8], perimeter = 0.0;
+    for (int k = 0; k < n; ++k) {
+        const double* A = &P.form_path[3 * k]; const double* B = &P.form_path[3 * ((k + 1) % n)];
+        len[k] = std::sqrt((B[0] - A[0]) * (B[0] - A[0]) + (B[1] - A[1]) * (B[1] - A[1]) + (B[2] - A[2]) * (B[2] - A[2]));
+        perimeter += len[k];
+    }
+    for (int a = 0; a < 3; ++a) c[a] = P.form_path[a];
+    if (!(perimeter > 0.0)) return;
+    double s = std::fmod(P.form_speed * tau, perimeter);         // arc length travelled on the current lap
+    for (int k = 0; k < n; ++k) {
+        if (len[k] > 0.0 && (s < len[k] || k == n - 1)) {
+            const double* A = &P.form_path[3 * k]; const double* B = &P.form_path[3 * ((k + 1) % n)];
+            const double f = s / len[k];
+            for (int a = 0; a < 3; ++a) c[a] = A[a] + f * (B[a] - A[a]);
+            return;
+        }
+        s -= len[k];
+    }
+}
 
 // O4 motor model (Eq.1-3; Q3 yaw pattern m=(1,0,1,0))
 template <class R>
@@ -615,9 +646,11 @@ struct Sim {
                 tg[0] = P.waypoints[0]; tg[1] = P.waypoints[1]; tg[2] = P.waypoints[2];
             } else {                                                // TGT_CIRCLE, Q26
                 const double ang = 2.0 * PI * i / M;
-                tg[0] = P.form_center[0] + P.form_radius * std::cos(ang);
-                tg[1] = P.form_center[1] + P.form_radius * std::sin(ang);
-                tg[2] = P.form_center[2];
+                double c[3];
+                path_centre(P, 0.0, c);                             // Q52: the path's first vertex when a path is given
+                tg[0] = c[0] + P.form_radius * std::cos(ang);
+                tg[1] = c[1] + P.form_radius * std::sin(ang);
+                tg[2] = c[2];
             }
             // Table 4, Q39: per-episode factors 1 + a (2u - 1); vehicle parameters per drone, g per env
             const bool lag_on = P.motor_lag_hi > 0.0;
@@ -870,6 +903,17 @@ struct Sim {
         const bool use_tilt = P.term_mode != TERM_NONE;
         const bool use_zmax = use_floor;
         const bool use_dist = P.term_mode == TERM_TILT_DIST || P.term_mode == TERM_FORMATION;
+        double centre[3] = {P.term_center[0], P.term_center[1], P.term_center[2]};
+        if (path_on(P)) {                                          // PAPER.md:325, Q52: slots ride on the moving centre; evaluated at the end-of-step time
+            path_centre(P, (double)(ep_step[e] + 1u) * D.dt_c, centre);
+            for (int i = 0; i < M; ++i) {
+                const double ang = 2.0 * PI * i / M;
+                double* tgs = &target[((size_t)e * M + i) * 4];
+                tgs[0] = dr[i].tg[0] = centre[0] + P.form_radius * std::cos(ang);
+                tgs[1] = dr[i].tg[1] = centre[1] + P.form_radius * std::sin(ang);
+                tgs[2] = dr[i].tg[2] = centre[2];
+            }
+        }
         double m_done = 1e30, m_rew = 1e30;
         bool terminated = false;
         R rew = 0.0;
@@ -891,7 +935,7 @@ struct Sim {
                 m_done = std::fmin(m_done, std::fabs(to_d(d.p[2]) - P.z_max));
             }
             if (use_dist) {
-                const R dx = d.p[0] - P.term_center[0], dy = d.p[1] - P.term_center[1], dz = d.p[2] - P.term_center[2];
+                const R dx = d.p[0] - centre[0], dy = d.p[1] - centre[1], dz = d.p[2] - centre[2];   // the moving centre when a path is on
                 const R dist = sqrt(dx * dx + dy * dy + dz * dz);
                 if (dist > P.term_dist) terminated = true;
                 m_done = std::fmin(m_done, std::fabs(to_d(dist) - P.term_dist));

@@ -61,7 +61,7 @@ static const Field FIELDS[] = {
     FD(episode_len_s, 1), FI(auto_reset), FI(reset_layout), FD(reset_center, 3), FD(reset_half, 3),
     FD(reset_z_lo, 1), FD(reset_z_hi, 1), FI(grid_cols), FD(grid_spacing, 1), FD(circle_radius, 1), FI(target_mode),
     FD(target_fixed, 3), FD(target_lo, 3), FD(target_hi, 3), FD(mh_z_lo, 1), FD(mh_z_hi, 1), FD(form_center, 3),
-    FD(form_radius, 1), FI(env_index_base), FI(drone_model), FD(target_w_lo, 1), FD(target_w_hi, 1), FD(dr_alpha, 12), FD(reset_rpy_half, 3), FD(reset_vel_half, 3), FD(motor_lag_lo, 1), FD(motor_lag_hi, 1), FI(wind_mask), FD(wind_const, 3), FD(wind_sine_amp, 1), FD(wind_sine_omega, 1), FD(gust_prob, 1), FD(gust_max, 1), FD(gust_duration, 1), FI(n_waypoints), FD(waypoints, 24), FD(wp_radius, 1), FD(wp_bonus, 1), FD(wp_shaping, 1), FD(wp_speed, 1), FD(wp_omega, 1), FI(wp_laps), FD(obs_noise, 4), FD(obs_bias, 4), FD(dryden_airspeed, 1), FD(dryden_h_min, 1), FD(act_latency_lo, 1), FD(act_latency_hi, 1), FD(obs_latency_lo, 1), FD(obs_latency_hi, 1),
+    FD(form_radius, 1), FI(env_index_base), FI(drone_model), FD(target_w_lo, 1), FD(target_w_hi, 1), FD(dr_alpha, 12), FD(reset_rpy_half, 3), FD(reset_vel_half, 3), FD(motor_lag_lo, 1), FD(motor_lag_hi, 1), FI(wind_mask), FD(wind_const, 3), FD(wind_sine_amp, 1), FD(wind_sine_omega, 1), FD(gust_prob, 1), FD(gust_max, 1), FD(gust_duration, 1), FI(n_waypoints), FD(waypoints, 24), FD(wp_radius, 1), FD(wp_bonus, 1), FD(wp_shaping, 1), FD(wp_speed, 1), FD(wp_omega, 1), FI(wp_laps), FD(obs_noise, 4), FD(obs_bias, 4), FD(dryden_airspeed, 1), FD(dryden_h_min, 1), FD(act_latency_lo, 1), FD(act_latency_hi, 1), FD(obs_latency_lo, 1), FD(obs_latency_hi, 1), FI(form_path_n), FD(form_path, 24), FD(form_speed, 1),
 };
 static const Field* find_field(const char* name) {
     for (const Field& f : FIELDS) if (std::string(f.name) == name) return &f;
@@ -104,6 +104,7 @@ void* orc_create(int n_envs, int n_drones, int physics_mode, int action_type, co
     const int K = P.sim_freq / P.ctrl_freq;                       // Q51: at most 3 control steps of action latency, 1 of sensor latency
     if (P.act_latency_lo < 0 || P.act_latency_hi < P.act_latency_lo || std::floor(P.act_latency_hi * P.sim_freq + 0.5) > 3 * K) return nullptr;
     if (P.obs_latency_lo < 0 || P.obs_latency_hi < P.obs_latency_lo || std::floor(P.obs_latency_hi * P.sim_freq + 0.5) > K) return nullptr;
+    if (P.form_path_n < 0 || P.form_path_n > 8 || P.form_speed < 0) return nullptr;
     Sim* s = new Sim;
     s->init(n_envs, n_drones, physics_mode, action_type, P);
     return s;
