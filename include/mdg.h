@@ -144,6 +144,12 @@ typedef struct mdg_params {
      * roll/pitch/yaw, v, body rates) are the state that many substeps before the end of the step; the first row after a
      * reset / auto-reset is the initial state.  Both outside their window: MDG_EINVAL. */
     float act_latency_lo, act_latency_hi, obs_latency_lo, obs_latency_hi;
+    /* FormationAviary's moving centre ("the formation centre tracks a closed polygonal path"; reading Q52),
+     * with MDG_TGT_CIRCLE: form_path_n (2..8) vertices (x, y, z each) traversed at form_speed m/s from vertex 0 at episode time 0
+     * and closed back to it; the circle slots (the per-drone targets, rewritten every step), the formation reward and the
+     * distance rule of MDG_TERM_FORMATION follow the centre at the end-of-step time.  form_path_n < 2 or form_speed = 0
+     * (default) = the static form_center / term_center. */
+    int32_t form_path_n; float form_path[24], form_speed;
 } mdg_params;
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */

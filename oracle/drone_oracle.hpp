@@ -22,7 +22,8 @@
 // normality, independence, which columns move, constancy over an episode, keying by global env index);
 // tests/test_oracle_dryden.py: altitude-dependent Dryden length scale (printed values, first updates, AR(1) statistics by altitude);
 // tests/test_oracle_latency.py: action / sensor latency (thrust-step and free-fall closed forms per substep of delay, shift
-// equivalence for the controller action types, uniform per-episode delays).
+// equivalence for the controller action types, uniform per-episode delays);
+// tests/test_oracle_formation_path.py: the moving formation centre (hand tables for two polygons, reward / termination about it).
 // tests/test_oracle_pid_transient.py: the coupled x / y PID transient against the linearised cascade (a 6-state discrete
 // linear system iterated in numpy) at several yaw angles and directions.
 // PARITY UNPINNED (the oracle itself is the reference): the large-amplitude (nonlinear) PID transient and the

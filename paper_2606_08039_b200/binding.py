@@ -40,6 +40,7 @@ class mdg_params(C.Structure):
         ("obs_noise", C.c_float * 4), ("obs_bias", C.c_float * 4),
         ("dryden_airspeed", C.c_float), ("dryden_h_min", C.c_float),
         ("act_latency_lo", C.c_float), ("act_latency_hi", C.c_float), ("obs_latency_lo", C.c_float), ("obs_latency_hi", C.c_float),
+        ("form_path_n", C.c_int32), ("form_path", C.c_float * 24), ("form_speed", C.c_float),
     ]
 
     def update(self, d):

@@ -76,6 +76,7 @@ static int feature_word(const mdg_params& p, int physics_mode, int action_type, 
     if ((aero & MDG_AERO_WIND) && (p.wind_mask != MDG_WIND_DRYDEN || p.dryden_airspeed > 0.0f)) f |= F_WIND_MIX;
     for (int i = 0; i < 4; ++i) if (p.obs_noise[i] != 0.0f || p.obs_bias[i] != 0.0f) f |= F_SENS;
     if (p.act_latency_hi > 0.0f || p.obs_latency_hi > 0.0f) f |= F_LAT;
+    if (p.target_mode == MDG_TGT_CIRCLE && p.form_path_n >= 2 && p.form_speed > 0.0f) f |= F_PATH;
     f |= p.reward_mode << F_REW_SHIFT;
     f |= p.term_mode << F_TERM_SHIFT;
     if (p.reward_mode == MDG_REW_FORMATION && p.target_mode == MDG_TGT_CIRCLE) f |= F_TGT_CIRCLE;
@@ -157,6 +158,18 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
     D.motor_lag_lo = p.motor_lag_lo; D.motor_lag_hi = p.motor_lag_hi;
     for (int i = 0; i < 4; ++i) { D.obs_noise[i] = p.obs_noise[i]; D.obs_bias[i] = p.obs_bias[i]; }
+    D.path_n = p.form_path_n; D.path_rate = (float)(dtc * p.form_speed);
+    {   // moving formation centre (Q52): side lengths and perimeter of the closed polygon, in double
+        double per = 0.0;
+        for (int k = 0; k < p.form_path_n && k < 8; ++k) {
+            const int kn = (k + 1) % p.form_path_n;
+            double l2 = 0.0;
+            for (int a = 0; a < 3; ++a) { const double dlt = (double)p.form_path[3 * kn + a] - (double)p.form_path[3 * k + a]; l2 += dlt * dlt; }
+            D.path_len[k] = (float)std::sqrt(l2); per += std::sqrt(l2);
+        }
+        D.path_perimeter = (float)per;
+        for (int i = 0; i < 24; ++i) D.path[i] = p.form_path[i];
+    }
     {   // Table 4 latency rows in substeps (Q51): uniform over round(lo f_sim) .. round(hi f_sim)
         const int a_lo = (int)std::floor((double)p.act_latency_lo * p.sim_freq + 0.5), a_hi = (int)std::floor((double)p.act_latency_hi * p.sim_freq + 0.5);
         const int s_lo = (int)std::floor((double)p.obs_latency_lo * p.sim_freq + 0.5), s_hi = (int)std::floor((double)p.obs_latency_hi * p.sim_freq + 0.5);
@@ -342,6 +355,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
         if (!(p.obs_latency_lo >= 0) || !(p.obs_latency_hi >= p.obs_latency_lo) || std::floor((double)p.obs_latency_hi * p.sim_freq + 0.5) > Ks)
             return fail(MDG_EINVAL, "mdg_create: sensor latency must satisfy 0 <= lo <= hi <= 1 control step");
     }
+    if (p.form_path_n < 0 || p.form_path_n > 8 || !(p.form_speed >= 0)) return fail(MDG_EINVAL, "mdg_create: form_path_n in [0, 8], form_speed >= 0");
     if (!(p.dryden_airspeed >= 0) || (p.dryden_airspeed > 0 && !(p.dryden_h_min > 0)))
         return fail(MDG_EINVAL, "mdg_create: dryden_airspeed must be >= 0 and dryden_h_min > 0");
     for (int i = 0; i < 4; ++i)

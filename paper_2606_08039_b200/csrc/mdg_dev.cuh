@@ -23,6 +23,7 @@ enum : int {
     F_MLAG = 1 << 23,                                     // motor lag: rotor-speed state, wrench recomputed every substep
     F_SENS = 1 << 24,                                     // Table 4 sensor rows: noise / per-episode bias on the emitted observation
     F_LAT = 1 << 25,                                      // Table 4 latency rows: delayed action rows / sensed state (generic kernel)
+    F_PATH = 1 << 26,                                     // formation centre on a closed polygonal path (generic kernel)
     F_WIND_MIX = 1 << 22,                                 // wind_mask != MDG_WIND_DRYDEN: only the generic kernel handles it
 };
 
@@ -67,6 +68,7 @@ struct DevParams {
     float dr_alpha[12];                                   // half-widths of the DR factors [m, J, k_f, k_m, drag, gnd, dw, g, motor, arm, max_rpm, -]
     float reset_rpy_half[3], reset_vel_half[3];           // Table 4 "init" row
     float motor_lag_lo, motor_lag_hi;                     // Table 4 motor lag: range of the time constant (s)
+    int path_n; float path[24], path_len[8], path_perimeter, path_rate;   // moving formation centre: vertices, side lengths, form_speed dt_c
     int lat_a_lo, lat_a_n, lat_s_lo, lat_s_n;             // Table 4 latency rows in substeps: smallest delay and number of values (0 = off)
     float obs_noise[4], obs_bias[4];                      // Table 4 sensor rows: standard deviations for [position, velocity, RPY, body rates]
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]

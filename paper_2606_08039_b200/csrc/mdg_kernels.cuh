@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         d.Ie = v3(i4.x, i4.y, i4.z);
         if (F::act(P) == 1) d.sp = W.plane[5][lane];
     }
-    const float4 tg = W.plane[6][lane];
+    float4 tg = W.plane[6][lane];
     const float4 act4 = W.plane[7][lane];
     float4 env4 = W.plane[8][lane];
     const uint32_t t = W.gstep[lane] + 1u;
@@ -440,13 +440,21 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     // S9-S11 epilogue on the end-of-step state
     const int gbase = lane & ~(G - 1);
     V3 eta = euler_zyx(d.q);
+    V3 cen = v3(P.term_center[0], P.term_center[1], P.term_center[2]);
+    const bool on_path = FEAT < 0 && F::has(P, F_PATH);
+    if (on_path) {                                                 // PAPER.md:325 (Q52): slots and the distance rule ride on the moving centre
+        cen = path_centre(P, __float_as_uint(env4.w) + 1u);
+        float sn, cs;
+        sincospif(2.0f * (float)jj / (float)P.M, &sn, &cs);
+        tg = make_float4(fmaf(P.form_radius, cs, cen.x), fmaf(P.form_radius, sn, cen.y), cen.z, tg.w);
+    }
     const int term = F::term(P);
     const float aphi = fabsf(eta.x), ath = fabsf(eta.y);
     int flags = 0;                                                 // bit0 terminated, bit1 crash
     if (term == 1 || term == 3) { if (hit) flags |= 3; if (d.p.z > P.z_max) flags |= 1; }
     if (term != 0 && (aphi > P.term_tilt || ath > P.term_tilt)) flags |= 3;
     if (term == 2 || term == 3) {
-        const float dx = d.p.x - P.term_center[0], dy = d.p.y - P.term_center[1], dz = d.p.z - P.term_center[2];
+        const float dx = d.p.x - cen.x, dy = d.p.y - cen.y, dz = d.p.z - cen.z;
         if (fmaf(dx, dx, fmaf(dy, dy, dz * dz)) > P.term_dist2) flags |= 1;
     }
     const float ex = d.p.x - tg.x, ey = d.p.y - tg.y, ez = d.p.z - tg.z;
@@ -519,6 +527,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         tg_out = make_float4(P.waypoints[3 * kw], P.waypoints[3 * kw + 1], P.waypoints[3 * kw + 2], (float)kn);
         if (active && !do_reset) B.P6[drone] = tg_out;
     }
+    if (on_path && active && !do_reset) B.P6[drone] = tg_out;       // mdg_targets shows the slot of the moment
     if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp
         if (do_reset) {
             reset_drone(P, e, (uint32_t)jj, t, d, tg_out);

@@ -75,9 +75,33 @@ __device__ __forceinline__ void reset_drone(const DevParams& P, uint32_t e, uint
     } else {                              // CIRCLE slots
         float s, c;
         sincospif(2.0f * (float)j / (float)P.M, &s, &c);
-        tg.x = fmaf(P.form_radius, c, P.form_center[0]); tg.y = fmaf(P.form_radius, s, P.form_center[1]);
-        tg.z = P.form_center[2];
+        const bool path = (P.feat & F_PATH) != 0;             // DESIGN.md Q52: an episode starts at the path's first vertex
+        tg.x = fmaf(P.form_radius, c, path ? P.path[0] : P.form_center[0]); tg.y = fmaf(P.form_radius, s, path ? P.path[1] : P.form_center[1]);
+        tg.z = path ? P.path[2] : P.form_center[2];
     }
+}
+
+// PAPER.md:325 (Q52): centre of the formation after ep control steps of the episode, moving at constant speed along the
+// closed polygon path[0] -> path[1] -> ... -> path[0]
+__device__ __forceinline__ V3 path_centre(const DevParams& P, uint32_t ep) {
+    float s = fmodf(P.path_rate * (float)ep, P.path_perimeter);
+    V3 c = v3(P.path[0], P.path[1], P.path[2]);
+    bool found = false;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        if (k < P.path_n && !found) {
+            const float len = P.path_len[k];
+            if (len > 0.0f && (s < len || k == P.path_n - 1)) {
+                const int kn = (k + 1 == P.path_n) ? 0 : k + 1;
+                const float f = s / len;
+                c = v3(fmaf(f, P.path[3 * kn] - P.path[3 * k], P.path[3 * k]), fmaf(f, P.path[3 * kn + 1] - P.path[3 * k + 1], P.path[3 * k + 1]),
+                       fmaf(f, P.path[3 * kn + 2] - P.path[3 * k + 2], P.path[3 * k + 2]));
+                found = true;
+            }
+            s -= len;
+        }
+    }
+    return c;
 }
 
 // normalizedActionToRPM: [-1, 1] -> [0, MAX_RPM] through HOVER_RPM at 0, piecewise linear, clipped

@@ -174,6 +174,15 @@ CASES = {
     "m2_latency_sensor_only_fly_through": (wl("m2latfly", 800, 2, W.PHYS_MJC_DRAG, W.ACT_RPM,
                                               dict(GRID, grid_cols=2, reset_z_lo=0.9, reset_z_hi=1.1, obs_mode=W.OBS_KIN12_WP, reward_mode=W.REW_FLY_THROUGH,
                                                    target_mode=W.TGT_WAYPOINTS, wp_radius=0.25, episode_len_s=20.0, obs_latency_lo=0.0, obs_latency_hi=0.0208), HOVER), {}),
+    # FormationAviary's moving centre: a fast lap round a small square so that 48 steps pass three vertices; the
+    # 3 m rule measured from the moving centre; and a tilted triangle under M = 5 (partial lane group), short episodes
+    "m4_formation_path_c5_like": (wl("m4path", 900, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_VEL,
+                                     dict(CIRCLE, circle_radius=0.3, form_radius=0.3, aero_mask=15, wind_sigma=0.5, wind_tau=1.0, target_mode=W.TGT_CIRCLE,
+                                          int_clamp_pos=1.0, int_clamp_att=0.25, form_path_n=4, form_speed=2.5,
+                                          form_path=[0, 0, 1, 0.6, 0, 1, 0.6, 0.6, 1, 0, 0.6, 1] + [0.0] * 12), ("uniform", -1.0, 1.0)), {}),
+    "m5_formation_path_triangle": (wl("m5path", 517, 5, W.PHYS_MJC_DRAG, W.ACT_VEL,
+                                      dict(CIRCLE, target_mode=W.TGT_CIRCLE, episode_len_s=0.4, term_dist=0.9, form_path_n=3, form_speed=3.0,
+                                           form_path=[0, 0, 1, 0.5, 0.1, 1.2, 0.2, 0.6, 0.9] + [0.0] * 15), ("uniform", -1.0, 1.0)), {}),
     # one env, one warp not even full
     "n1_m3": (wl("n1m3", 1, 3, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM, dict(GRID), HOVER), {}),
 }
@@ -388,3 +397,29 @@ def test_async_host_step_on_two_streams_equals_the_synchronous_call():
             for x, y in zip(bs[i], ba[i]):
                 assert torch.equal(x, y), (t, i)
     assert bs[0][0].abs().max() > 0.1 and not torch.equal(bs[0][0], bs[1][0])
+
+
+def test_formation_path_targets_follow_the_oracle_and_bad_paths_are_rejected():
+    """mdg_targets under the moving formation centre: the slots of the moment, step by step, across a lap and an auto-reset."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    from oracle import oracle as O
+    w = wl("pathtg", 64, 3, W.PHYS_MJC, W.ACT_VEL,
+           dict(CIRCLE, target_mode=W.TGT_CIRCLE, episode_len_s=1.0, form_path_n=3, form_speed=4.0, form_path=[0, 0, 1, 0.5, 0.1, 1.2, 0.2, 0.6, 0.9] + [0.0] * 15),
+           ("uniform", -0.2, 0.2))
+    gpu = mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **w.params))
+    orc = O.OracleEnv(w.n_envs, w.n_drones, w.physics_mode, w.action_type, O.OracleParams(0, **w.params))
+    assert "generic" in gpu.kernel_name
+    gpu.reset(w.seed); orc.reset(w.seed)
+    seen = []
+    for t in range(60):                                                # perimeter 1.74 m at 4 m/s: two laps; truncation after 48 steps
+        a = O.gen_actions(w.seed, t, w.n_envs, w.n_drones, 1.0, -0.2, 0.2)
+        gpu.step(torch.from_numpy(a).cuda()); orc.step(a)
+        tg = gpu.get_state()["targets"].astype(np.float64)
+        assert np.abs(tg[:, :3] - orc.targets[:, :3]).max() < 2e-6, t
+        seen.append(tg[0, :3].copy())
+    assert np.ptp(np.array(seen), axis=0).min() > 0.25                 # the slot really travelled
+    for over in (dict(form_path_n=9), dict(form_path_n=-1), dict(form_speed=-1.0)):
+        with pytest.raises(mdg.MdgError):
+            mdg.Env(4, 2, W.PHYS_MJC, W.ACT_VEL, mdg.default_params(0, **dict(w.params, **over)))
