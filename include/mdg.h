@@ -210,6 +210,16 @@ int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float
 int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
                   const float* wind, const uint32_t* ep_step);
 
+/* Full checkpoint / resume.  mdg_get_state covers the kinematic state for tests; a running simulation also carries the DR
+ * factors, rotor speeds (motor lag), gust impulses, action history (action latency), step counters, the seed and the last
+ * outputs.  mdg_save writes all of it to host memory as one opaque blob of mdg_checkpoint_size bytes; mdg_load restores it
+ * into a handle created with the same n_envs, n_drones, modes and params, after which stepping continues bit for bit as
+ * if never interrupted.  Both synchronise the stream.  MDG_EINVAL: NULL, short buffer, a blob of another library version or
+ * of a handle with another shape / feature set.  mdg_checkpoint_size returns a negative code on a NULL handle. */
+int64_t mdg_checkpoint_size(const mdg_env* env);
+int mdg_save(mdg_env* env, void* host_buf, int64_t buf_bytes);
+int mdg_load(mdg_env* env, const void* host_buf, int64_t buf_bytes);
+
 /* Per-agent view for multi-agent training (MultiAgentAviary): device pointer to [n_envs*n_drones] fp32, each
  * drone's share of the last step's reward (its own terms plus half of every pair term it is part of); the shares of an
  * env add up to its reward.  Library-owned, valid until mdg_destroy; written by every mdg_step. */

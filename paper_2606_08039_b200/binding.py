@@ -62,7 +62,7 @@ class mdg_cam_params(C.Structure):
     update = mdg_params.update
 
 
-EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_wait", "mdg_outputs",
+EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_wait", "mdg_checkpoint_size", "mdg_save", "mdg_load", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
            "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_last_error", "mdg_version"]
 
@@ -88,6 +88,10 @@ def lib():
         L.mdg_step_host.argtypes = [vp] * 5
         L.mdg_step_host_async.argtypes = [vp] * 5
         L.mdg_wait.argtypes = [vp]
+        L.mdg_checkpoint_size.argtypes = [vp]
+        L.mdg_checkpoint_size.restype = C.c_int64
+        L.mdg_save.argtypes = [vp, vp, C.c_int64]
+        L.mdg_load.argtypes = [vp, vp, C.c_int64]
         L.mdg_outputs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.mdg_obs_dim.argtypes = [vp]
         L.mdg_targets.argtypes = [vp, C.POINTER(vp)]
@@ -231,6 +235,22 @@ class Env:
             raise ValueError("actions_host must be a host float32 tensor of n_envs*n_drones*4 elements")
         fn = lib().mdg_step_host_async if asynchronous else lib().mdg_step_host
         _check(fn(self._h, ptr(actions_host), ptr(obs_host), ptr(reward_host), ptr(done_host)))
+
+    def save(self):
+        """Full checkpoint as a numpy uint8 array (include/mdg.h: mdg_save)."""
+        import numpy as np
+        n = lib().mdg_checkpoint_size(self._h)
+        if n < 0:
+            _check(int(n))
+        buf = np.empty(int(n), dtype=np.uint8)
+        _check(lib().mdg_save(self._h, C.c_void_p(buf.ctypes.data), int(n)))
+        return buf
+
+    def load(self, blob):
+        """Restore a checkpoint written by save() on a handle of the same shape and parameters (mdg_load)."""
+        import numpy as np
+        b = np.ascontiguousarray(blob, dtype=np.uint8)
+        _check(lib().mdg_load(self._h, C.c_void_p(b.ctypes.data), int(b.size)))
 
     def wait(self):
         """Block until everything enqueued on this handle's stream has finished (include/mdg.h: mdg_wait)."""

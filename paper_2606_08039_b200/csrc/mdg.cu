@@ -677,6 +677,54 @@ extern "C" int mdg_set_dr(mdg_env* h, const float* f) {
 
 // ---- end-to-end call with host buffers --------------------------------------------------------------
 static std::map<mdg_env*, float*> g_stage;   // device staging buffer for host actions, one per handle
+// ---- full checkpoint: every device buffer a later step reads, as one opaque host blob ---------------------
+namespace {
+struct CkptHeader { uint32_t magic, version; int32_t N, M, feat, opd; uint32_t seed_lo, seed_hi; uint64_t bytes_main, bytes_rd, bytes_hist; };
+const uint32_t CKPT_MAGIC = 0x4347444Du /* "MDGC" */, CKPT_VERSION = 1;
+// main region: the state / DR / rotor planes, per-env words, step counters and outputs, contiguous in the arena up to the
+// scheduler words (ticket dispensers and per-item flags are launch bookkeeping, not simulation state)
+inline size_t ckpt_main_bytes(const mdg_env* h) { return (size_t)((const char*)h->B.ticket - (const char*)h->B.P0); }
+inline size_t ckpt_rd_bytes(const mdg_env* h) { return (size_t)h->N * h->M * sizeof(float); }
+inline size_t ckpt_hist_bytes(const mdg_env* h) { return h->hist ? (size_t)((const char*)h->B.H1 - (const char*)h->B.H0) * 3 : 0; }
+}
+extern "C" int64_t mdg_checkpoint_size(const mdg_env* h) {
+    if (!h) return fail(MDG_EINVAL, "mdg_checkpoint_size: NULL handle");
+    return (int64_t)(sizeof(CkptHeader) + ckpt_main_bytes(h) + ckpt_rd_bytes(h) + ckpt_hist_bytes(h));
+}
+extern "C" int mdg_save(mdg_env* h, void* host_buf, int64_t buf_bytes) {
+    if (!h || !host_buf) return fail(MDG_EINVAL, "mdg_save: NULL argument");
+    if (buf_bytes < mdg_checkpoint_size(h)) return fail(MDG_EINVAL, "mdg_save: buffer smaller than mdg_checkpoint_size");
+    CU(cudaStreamSynchronize(h->stream));
+    CkptHeader hd = {CKPT_MAGIC, CKPT_VERSION, h->N, h->M, h->P.feat, h->P.opd, h->P.seed_lo, h->P.seed_hi,
+                     ckpt_main_bytes(h), ckpt_rd_bytes(h), ckpt_hist_bytes(h)};
+    char* c = (char*)host_buf;
+    std::memcpy(c, &hd, sizeof(hd)); c += sizeof(hd);
+    CU(cudaMemcpy(c, h->B.P0, hd.bytes_main, cudaMemcpyDeviceToHost)); c += hd.bytes_main;
+    CU(cudaMemcpy(c, h->B.reward_d, hd.bytes_rd, cudaMemcpyDeviceToHost)); c += hd.bytes_rd;
+    if (hd.bytes_hist) CU(cudaMemcpy(c, h->hist, hd.bytes_hist, cudaMemcpyDeviceToHost));
+    return MDG_OK;
+}
+extern "C" int mdg_load(mdg_env* h, const void* host_buf, int64_t buf_bytes) {
+    if (!h || !host_buf) return fail(MDG_EINVAL, "mdg_load: NULL argument");
+    if (buf_bytes < (int64_t)sizeof(CkptHeader)) return fail(MDG_EINVAL, "mdg_load: buffer too small for a checkpoint header");
+    CkptHeader hd;
+    std::memcpy(&hd, host_buf, sizeof(hd));
+    if (hd.magic != CKPT_MAGIC || hd.version != CKPT_VERSION) return fail(MDG_EINVAL, "mdg_load: not a checkpoint of this library version");
+    if (hd.N != h->N || hd.M != h->M || hd.feat != h->P.feat || hd.opd != h->P.opd || hd.bytes_main != ckpt_main_bytes(h) ||
+        hd.bytes_rd != ckpt_rd_bytes(h) || hd.bytes_hist != ckpt_hist_bytes(h))
+        return fail(MDG_EINVAL, "mdg_load: the checkpoint was written by a handle of another shape or feature set");
+    if (buf_bytes < mdg_checkpoint_size(h)) return fail(MDG_EINVAL, "mdg_load: truncated checkpoint");
+    CU(cudaStreamSynchronize(h->stream));
+    const char* c = (const char*)host_buf + sizeof(hd);
+    CU(cudaMemcpy(h->B.P0, c, hd.bytes_main, cudaMemcpyHostToDevice)); c += hd.bytes_main;
+    CU(cudaMemcpy(h->B.reward_d, c, hd.bytes_rd, cudaMemcpyHostToDevice)); c += hd.bytes_rd;
+    if (hd.bytes_hist) CU(cudaMemcpy(h->hist, c, hd.bytes_hist, cudaMemcpyHostToDevice));
+    h->P.seed_lo = hd.seed_lo; h->P.seed_hi = hd.seed_hi;
+    drop_graphs(h);                          // captured launches carry the old seed
+    h->chainable = false;                    // the next step waits for the whole stream, not for item flags of a step it never saw
+    return MDG_OK;
+}
+
 extern "C" int mdg_step_host_async(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
     if (!h || !actions_host) return fail(MDG_EINVAL, "mdg_step_host: NULL argument");
     const size_t D = (size_t)h->N * h->M;

@@ -423,3 +423,43 @@ def test_formation_path_targets_follow_the_oracle_and_bad_paths_are_rejected():
     for over in (dict(form_path_n=9), dict(form_path_n=-1), dict(form_speed=-1.0)):
         with pytest.raises(mdg.MdgError):
             mdg.Env(4, 2, W.PHYS_MJC, W.ACT_VEL, mdg.default_params(0, **dict(w.params, **over)))
+
+
+def test_checkpoint_resume_is_bitwise_with_every_stateful_feature_on():
+    """mdg_save / mdg_load: DR factors, rotor speeds, gust impulses, action history, counters, seed and outputs travel in the blob;
+    a second handle that loads it continues exactly like the first (chained steps and a graph replay included)."""
+    import numpy as np
+    import torch
+    import paper_2606_08039_b200 as mdg
+    w = wl("ckpt", 3000, 4, W.PHYS_MJC_GND_DRAG_DW, W.ACT_RPM,
+           dict(GRID, grid_cols=2, episode_len_s=0.3, aero_mask=15, wind_mask=15, wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0,
+                gust_prob=0.2, gust_max=1.5, gust_duration=0.3, dryden_airspeed=6.0, dr_alpha=DR, motor_lag_lo=0.005, motor_lag_hi=0.05, **INIT, **LAT, **SENS), HOVER)
+    mk = lambda: mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type, mdg.default_params(0, **w.params))
+    a, b = mk(), mk()
+    a.reset(w.seed); b.reset(12345)
+    acts = [a.gen_actions(w.seed, t, W.hover_rpm_f32(), 0.9, 1.1) for t in range(30)]
+    for t in range(14):
+        a.step(acts[t])
+    blob = a.save()
+    for t in range(14):
+        b.step(acts[t])                                                # b is somewhere else entirely when the blob arrives
+    b.load(blob)
+    assert torch.equal(a.obs, b.obs) and torch.equal(a.reward, b.reward) and torch.equal(a.done, b.done)
+    for t in range(14, 24):
+        a.step(acts[t]); b.step(acts[t])
+    stack = torch.stack(acts[24:30])
+    a.step_many(stack, 6); b.step_many(stack, 6)
+    torch.cuda.synchronize()
+    sa, sb = a.get_state(), b.get_state()
+    for k in sa:
+        assert np.array_equal(sa[k], sb[k]), k
+    assert np.array_equal(a.get_dr(), b.get_dr())
+    assert torch.equal(a.obs, b.obs) and torch.equal(a.reward, b.reward) and torch.equal(a.done, b.done)
+    assert torch.equal(a.reward_per_drone, b.reward_per_drone)
+    assert np.array_equal(a.save(), b.save())
+    # error paths: another shape, another feature set, a truncated or foreign blob
+    other = mdg.Env(w.n_envs, 2, w.physics_mode, w.action_type, mdg.default_params(0, **dict(w.params, grid_cols=2)))
+    plain = mdg.Env(w.n_envs, w.n_drones, w.physics_mode, w.action_type)
+    for env, data in ((other, blob), (plain, blob), (b, blob[:1000]), (b, blob[: blob.size - 8]), (b, np.zeros(blob.size, dtype=np.uint8))):
+        with pytest.raises(mdg.MdgError):
+            env.load(data)
