@@ -32,16 +32,33 @@ FLOPS_PER_DRONE_STEP = {1: 3186.0, 2: 3421.1, 3: 3350.0, 4: 3893.6, 5: 3858.75}
 REPLICAS = 4          # independent env batches stepped round-robin so the working set exceeds the 126 MB L2
 
 
-def algorithmic_bytes_per_drone(c: int) -> float:
-    """State read once + written once, actions read, outputs written."""
-    wl = W.config(c)
+# Secondary workloads (`--variant`, never the default line): the metric's config with the DYN integrator of Table 1
+# (SURVEY.md 8(f) NEXT-1 "DYN mode benchmarked"), and with every row of Table 4 switched on (NEXT-2: per-episode parameter
+# planes, motor lag, action / sensor latency, sensor noise) - both run the generic, runtime-flag instantiation of the kernel.
+VARIANTS = {
+    "dyn": dict(integrator=W.INTEG_EULER),
+    "table4": dict(dr_alpha=[0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02, 0.05, 0.02, 0.05, 0.0], reset_rpy_half=[0.1, 0.1, 0.1],
+                   reset_vel_half=[0.5, 0.5, 0.5], motor_lag_lo=0.005, motor_lag_hi=0.05, act_latency_lo=0.0, act_latency_hi=0.05,
+                   obs_latency_lo=0.0, obs_latency_hi=0.02, obs_noise=[0.01, 0.05, 0.0174533, 0.05]),
+}
+
+
+def algorithmic_bytes_per_drone(wl) -> float:
+    """State read once + written once, actions read, outputs written; the optional planes when they are on."""
     M = wl.n_drones
     pid = wl.action_type in (W.ACT_PID, W.ACT_VEL, W.ACT_ATTITUDE)       # actions with an attitude loop read/write P4
     rd = 4 * 16 + 16 + 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)   # P0-P3, target, action, P4, P5
     wr = 4 * 16 + (16 if pid else 0) + (16 if wl.action_type == W.ACT_PID else 0)
     obs = 4 * (12 + (M if wl.params.get("obs_mode", 0) == W.OBS_KIN12_ADJ else 0))
     env = (16 + 4) + (16 + 4 + 4 + 1)                                                         # per env: E0 + gstep r/w, reward, done
-    return rd + wr + obs + 4 + env / M                                                        # + the per-drone reward share
+    extra = 0
+    if any(wl.params.get("dr_alpha", [])) or wl.params.get("motor_lag_hi", 0) > 0:
+        extra += 64                                                                             # R0-R3 read
+    if wl.params.get("motor_lag_hi", 0) > 0:
+        extra += 32                                                                             # N0 read + written
+    if wl.params.get("act_latency_hi", 0) > 0:
+        extra += 96                                                                             # H0-H2 read + written
+    return rd + wr + obs + 4 + env / M + extra                                                # + the per-drone reward share
 
 
 class ClockSampler:
@@ -189,7 +206,8 @@ def run_reference(args, wl, c):
 def config_dict(wl, c, n_gpus):
     return {"workload": f"config {c} of BASELINE.json: {wl.n_envs} envs x {wl.n_drones} CF2X drones per GPU, "
                         f"physics_mode={wl.physics_mode} aero_mask={wl.params.get('aero_mask', 'from mode')}, action_type={wl.action_type}, "
-                        f"240 Hz physics / 48 Hz control (5 substeps), auto-reset on",
+                        f"240 Hz physics / 48 Hz control (5 substeps), auto-reset on"
+                        + (f"; VARIANT {wl.name.split('+', 1)[1]} (secondary workload, generic kernel)" if "+" in wl.name else ""),
             "n_envs_per_gpu": wl.n_envs, "n_drones": wl.n_drones, "substeps": 5, "seed": wl.seed,
             "parallelism": f"env-sharded x{n_gpus}, no collective on the step path",
             "l2": f"{REPLICAS} independent env batches stepped round-robin (working set > 126 MB L2)"}
@@ -319,7 +337,7 @@ def run_ours(args, wl, c):
     cpu = oracle_throughput(wl, budget_s=args.cpu_budget, n_envs=16384) if world == 1 and not args.no_cpu else None
     fpd = cpu["flops_per_drone_step"] if cpu else FLOPS_PER_DRONE_STEP[c]
     flops = fpd * drones
-    bytes_alg = algorithmic_bytes_per_drone(c) * drones
+    bytes_alg = algorithmic_bytes_per_drone(wl) * drones
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -336,7 +354,7 @@ def run_ours(args, wl, c):
     try:
         import csv
         for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv"))):
-            if row["config"] == f"c{c}":
+            if row["config"] == f"c{c}" and not args.variant:
                 traffic = float(row["traffic_bytes"])
     except Exception:
         pass
@@ -382,8 +400,14 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-camera", action="store_true", help="skip the secondary onboard-camera measurement")
+    ap.add_argument("--variant", default="", choices=["", "dyn", "table4"], help="secondary workload on the chosen config (see VARIANTS)")
     args = ap.parse_args()
     wl = W.config(args.config)
+    if args.variant:
+        if args.no_cpu:
+            raise SystemExit("--variant needs the oracle leg: its flop tally is the roofline numerator")
+        wl.params.update(VARIANTS[args.variant])
+        wl.name += "+" + args.variant
     if args.impl == "reference":
         run_reference(args, wl, args.config)
     else:

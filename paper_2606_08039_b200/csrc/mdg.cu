@@ -205,14 +205,16 @@ template <int G, int FEAT> static step_fn pick_minb(int minb) {
 static void pick_kernels(mdg_env* h) {
     const int f = h->P.feat;
     h->step = nullptr;
-#define SPECIAL(g, fw, name) if (h->G == g && f == fw) { h->step = pick_minb<g, fw>(h->minb); h->kernel_name = name; }
+#define SPECIAL(g, fw, name) if (h->G == (g) && f == (fw)) { h->step = pick_minb<(g), (fw)>(h->minb); h->kernel_name = name; }
     SPECIAL(1, FEAT_C1, "step_kernel<G=1,rigid,rpm,hover>")
     SPECIAL(1, FEAT_C2, "step_kernel<G=1,gnd+drag,rpm,hover>")
     SPECIAL(1, FEAT_C3, "step_kernel<G=1,rigid,pid+dsl,negsqdist>")
     SPECIAL(8, FEAT_C4, "step_kernel<G=8,gnd+drag+dw,rpm,multihover>")
     SPECIAL(4, FEAT_C5, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation>")
+    SPECIAL(4, FEAT_C5 | F_EULER, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation,dyn>")   // Table 1's DYN integrator on the metric's config
+    SPECIAL(4, FEAT_C5 | F_DR | F_MLAG | F_SENS | F_LAT, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation,table4>")   // every row of Table 4 on it
 #undef SPECIAL
-#define GENERIC(g) case g: if (!h->step) { h->step = step_kernel<g, -1, 4>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
+#define GENERIC(g) case g: if (!h->step) { h->step = h->minb <= 3 ? step_kernel<g, -1, 3> : step_kernel<g, -1, 4>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
                    h->reset = reset_kernel<g>; h->refresh = refresh_obs_kernel<g>; break;
     switch (h->G) { GENERIC(1) GENERIC(2) GENERIC(4) GENERIC(8) GENERIC(16) GENERIC(32) }
 #undef GENERIC
@@ -408,8 +410,11 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
         h->B.H0 = (float4*)h->hist; h->B.H1 = (float4*)((char*)h->hist + plane); h->B.H2 = (float4*)((char*)h->hist + 2 * plane);
     }
     int rc = configure_launch(h);
-    if (rc == MDG_OK && h->saturating) {     // throughput-bound batch: the 5-blocks-per-SM register budget measured fastest
-        h->minb = 5;
+    if (rc == MDG_OK && h->saturating) {     // throughput-bound batch: register budget (resident 128-thread blocks per SM) as measured fastest
+        const bool generic = h->kernel_name.find("generic") != std::string::npos;
+        // 5 for the benchmark specialisations (96 registers); 6 for the lighter DYN integrator; 4 where Table 4's planes and draws
+        // would spill at 96; the runtime-flag kernel needs 162 registers to stay out of local memory (3)
+        h->minb = generic ? 3 : (h->P.feat & (F_DR | F_MLAG | F_LAT | F_SENS)) ? 4 : (h->P.feat & F_EULER) ? 6 : 5;
         pick_kernels(h);
         rc = configure_launch(h);
     }
@@ -575,7 +580,7 @@ int mdg_set_launch(mdg_env* h, int block_threads, int max_blocks_per_sm) {
         h->max_blocks_per_sm = max_blocks_per_sm;
         // register-budget variant: resident 128-thread blocks per SM the allocation must allow (4..8)
         const int per128 = (max_blocks_per_sm * h->block + 127) / 128;
-        h->minb = per128 < 4 ? 4 : (per128 > 8 ? 8 : per128);
+        h->minb = per128 < 3 ? 3 : (per128 > 8 ? 8 : per128);   // 3 exists for the generic kernel only (specialisations fall back to 4)
         pick_kernels(h);
     }
     drop_graphs(h);

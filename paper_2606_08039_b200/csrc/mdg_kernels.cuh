@@ -231,14 +231,14 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     float4 gust_out = make_float4(0, 0, 0, 1.0f);                  // E1 after this step (generic kernel, MDG_WIND_GUST only)
     if (F::has(P, F_WIND)) {
         // components (MDG_WIND_*): the benchmark configs run the AR(1) gust alone (wmask == 1 folds at compile time)
-        const int wmask = FEAT >= 0 ? 1 : P.wind_mask;
+        const int wmask = F::has(P, F_WIND_MIX) ? P.wind_mask : 1;
         V3 u = v3(0, 0, 0);                                        // air velocity
         if (wmask & 1) {
             const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
             const float r1 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.x))), r2 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.z)));
             const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
             float wa = P.wind_alpha, wg = P.wind_gain;
-            if (FEAT < 0 && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
+            if (F::has(P, F_WIND_MIX) && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
                 const float hm = fmaxf(group_sum<G>((full_group || j < P.M) ? d.p.z : 0.0f) * P.inv_M, P.dryden_h_min);   // alpha = exp(-dt V / L)
                 const float x = P.dryden_x * powf(fmaf(8.23e-4f, hm, 0.177f), 1.2f) / hm;
                 wa = expf(-x);
@@ -283,12 +283,12 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         }
     }
 
-    // Table 4 latency rows (Q51), generic kernel only: this episode's delays in substeps from one Philox draw at the
+    // Table 4 latency rows (Q51): this episode's delays in substeps from one Philox draw at the
     // episode's reset index.  The row issued at step t runs from substep d on: with d = (n - 1) K + r, 1 <= r <= K, substeps
     // k < r of this step run the row of n steps ago, the rest the row after it.  A controller decodes once, from the first.
     float4 a_first = act4, a_second = act4;
     int sw = -1, d_obs = 0;
-    if (FEAT < 0 && F::has(P, F_LAT)) {
+    if (F::has(P, F_LAT)) {
         const uint32_t ep0 = __float_as_uint(env4.w);
         const uint4 lr = philox4x32_10(e + P.env_base, (uint32_t)jj, (t - 1u) - ep0, STREAM_LATENCY, P.seed_lo, P.seed_hi);
         d_obs = P.lat_s_lo + (int)(((lr.y >> 8) * (uint32_t)P.lat_s_n) >> 24);
@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     // S1/S2 decode, S3 motor model (Eq.1-3); RPMs are held over the K substeps
     float n[4], n_later[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     decode_action<FEAT>(P, a_first, d, n);
-    if (FEAT < 0 && sw >= 0) { DroneRegs dtmp = d; decode_action<FEAT>(P, a_second, dtmp, n_later); }   // direct rotor commands: stateless
+    if (F::has(P, F_LAT) && sw >= 0) { DroneRegs dtmp = d; decode_action<FEAT>(P, a_second, dtmp, n_later); }   // direct rotor commands: stateless
     // Domain randomisation (Table 4): this episode's factors scale the true vehicle, not the controller's model above.
     // 1 / s_J is folded into the body torque (every stage torque is linear in it, the gyroscopic ratios do not change).
     const bool dr = F::has(P, F_DR);
@@ -354,7 +354,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     Sensed snap = sensed(d, v3(0, 0, 0));                          // sensor latency of a whole step: the state the step starts from
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
-        if (FEAT < 0 && sw == k) {                                 // Q51: the next row arrives at this substep
+        if (F::has(P, F_LAT) && sw == k) {                                 // Q51: the next row arrives at this substep
             n[0] = n_later[0]; n[1] = n_later[1]; n[2] = n_later[2]; n[3] = n_later[3];
             if (!lag) motor_model(n);
         }
@@ -430,7 +430,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             else integrate_rot<false, true, DEG>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
         }
         if (d.p.z < 0.0f) { hit = true; d.p.z = 0.0f; d.v.z = fmaxf(d.v.z, 0.0f); }   // floor
-        if (FEAT < 0 && F::has(P, F_LAT) && k + 1 == P.K - d_obs) snap = sensed(d, v3(0, 0, 0));   // what the sensors report d_obs substeps later
+        if (F::has(P, F_LAT) && k + 1 == P.K - d_obs) snap = sensed(d, v3(0, 0, 0));   // what the sensors report d_obs substeps later
     }
 
     MDG_T(3);
@@ -441,7 +441,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const int gbase = lane & ~(G - 1);
     V3 eta = euler_zyx(d.q);
     V3 cen = v3(P.term_center[0], P.term_center[1], P.term_center[2]);
-    const bool on_path = FEAT < 0 && F::has(P, F_PATH);
+    const bool on_path = F::has(P, F_PATH);
     if (on_path) {                                                 // PAPER.md:325 (Q52): slots and the distance rule ride on the moving centre
         cen = path_centre(P, __float_as_uint(env4.w) + 1u);
         float sn, cs;
@@ -556,8 +556,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             if (F::act(P) == 1) B.P5[drone] = d.sp;
         }
         Sensed sn = sensed(d, eta);
-        if (FEAT < 0 && F::has(P, F_LAT) && !do_reset) { sn = snap; sn.eta = euler_zyx(snap.q); }   // a new episode's first row is its initial state
-        if (FEAT < 0 && F::has(P, F_SENS)) sense(P, e, (uint32_t)jj, t, ep_out, sn);   // Table 4 sensor rows: the stored state stays exact
+        if (F::has(P, F_LAT) && !do_reset) { sn = snap; sn.eta = euler_zyx(snap.q); }   // a new episode's first row is its initial state
+        if (F::has(P, F_SENS)) sense(P, e, (uint32_t)jj, t, ep_out, sn);   // Table 4 sensor rows: the stored state stays exact
         write_obs<G>(P, B.obs, drone, d, sn, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
         B.reward_d[drone] = r;
         if (lag) B.N0[drone] = make_float4(n_act[0], n_act[1], n_act[2], n_act[3]);
@@ -565,7 +565,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             env4.w = __uint_as_float(ep_out);
             B.E0[e] = env4; B.gstep[e] = t;
             B.reward[e] = rsum; B.done[e] = (uint8_t)done;
-            if (FEAT < 0 && (P.wind_mask & 4) && F::has(P, F_WIND)) B.E1[e] = do_reset ? make_float4(0, 0, 0, 1.0f) : gust_out;
+            if (F::has(P, F_WIND_MIX) && (P.wind_mask & 4) && F::has(P, F_WIND)) B.E1[e] = do_reset ? make_float4(0, 0, 0, 1.0f) : gust_out;
         }
     }
     MDG_T(5);
