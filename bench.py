@@ -354,7 +354,7 @@ def run_ours(args, wl, c):
     try:
         import csv
         for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv"))):
-            if row["config"] == f"c{c}" and not args.variant:
+            if row["config"] == (f"c{c}+{args.variant}" if args.variant else f"c{c}"):
                 traffic = float(row["traffic_bytes"])
     except Exception:
         pass
