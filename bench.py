@@ -400,13 +400,20 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-camera", action="store_true", help="skip the secondary onboard-camera measurement")
-    ap.add_argument("--variant", default="", choices=["", "dyn", "table4"], help="secondary workload on the chosen config (see VARIANTS)")
+    ap.add_argument("--variant", default="", choices=["", "dyn", "table4", "paper_mjx"], help="secondary workload on the chosen config (see VARIANTS)")
     args = ap.parse_args()
     wl = W.config(args.config)
     if args.variant:
         if args.no_cpu:
             raise SystemExit("--variant needs the oracle leg: its flop tally is the roofline numerator")
-        wl.params.update(VARIANTS[args.variant])
+        if args.variant == "paper_mjx":
+            # the workload of the paper's own MJX back end (hover, rigid body only, normalised rotor commands,
+            # PAPER.md:300), at 2^20 envs ("the only practical limit is GPU memory") instead of its default 4,096
+            args.config = 1
+            base = W.config(1)
+            wl = W.Workload("c1", 1 << 20, 1, W.PHYS_MJC, W.ACT_RPM_NORM, dict(base.params), ("uniform", -0.05, 0.06), 1000, base.seed)
+        else:
+            wl.params.update(VARIANTS[args.variant])
         wl.name += "+" + args.variant
     if args.impl == "reference":
         run_reference(args, wl, args.config)

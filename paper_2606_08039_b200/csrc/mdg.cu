@@ -207,6 +207,7 @@ static void pick_kernels(mdg_env* h) {
     h->step = nullptr;
 #define SPECIAL(g, fw, name) if (h->G == (g) && f == (fw)) { h->step = pick_minb<(g), (fw)>(h->minb); h->kernel_name = name; }
     SPECIAL(1, FEAT_C1, "step_kernel<G=1,rigid,rpm,hover>")
+    SPECIAL(1, FEATW(0, 0, 3, 0, 0, 0, 1), "step_kernel<G=1,rigid,rpm_norm,hover>")   // the paper's own MJX workload
     SPECIAL(1, FEAT_C2, "step_kernel<G=1,gnd+drag,rpm,hover>")
     SPECIAL(1, FEAT_C3, "step_kernel<G=1,rigid,pid+dsl,negsqdist>")
     SPECIAL(8, FEAT_C4, "step_kernel<G=8,gnd+drag+dw,rpm,multihover>")

@@ -479,3 +479,11 @@ def test_config5_variant_specialisations_parity(variant, tag):
     res = run_parity(w, steps=48, extra=over, max_ill_frac=0.08)
     print(variant, res)
     assert res["kernel"].endswith(tag), res["kernel"]
+
+
+def test_paper_mjx_workload_specialisation_parity():
+    """HoverAviary as the paper's MJX back end runs it (rigid body only, normalised rotor commands PAPER.md:300):
+    its own compile-time specialisation (bench.py --variant paper_mjx)."""
+    res = run_parity(wl("mjx", 4099, 1, W.PHYS_MJC, W.ACT_RPM_NORM, dict(SINGLE), ("uniform", -0.05, 0.06)), steps=48)
+    print(res)
+    assert res["kernel"] == "step_kernel<G=1,rigid,rpm_norm,hover>"
