@@ -37,6 +37,7 @@ REPLICAS = 4          # independent env batches stepped round-robin so the worki
 # planes, motor lag, action / sensor latency, sensor noise) - both run the generic, runtime-flag instantiation of the kernel.
 VARIANTS = {
     "dyn": dict(integrator=W.INTEG_EULER),
+    "noise": dict(obs_noise=[0.01, 0.05, 0.0174533, 0.05]),      # no precompiled specialisation: instantiated at mdg_create (MDG_JIT=0: generic kernel)
     "table4": dict(dr_alpha=[0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02, 0.05, 0.02, 0.05, 0.0], reset_rpy_half=[0.1, 0.1, 0.1],
                    reset_vel_half=[0.5, 0.5, 0.5], motor_lag_lo=0.005, motor_lag_hi=0.05, act_latency_lo=0.0, act_latency_hi=0.05,
                    obs_latency_lo=0.0, obs_latency_hi=0.02, obs_noise=[0.01, 0.05, 0.0174533, 0.05]),
@@ -400,7 +401,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-camera", action="store_true", help="skip the secondary onboard-camera measurement")
-    ap.add_argument("--variant", default="", choices=["", "dyn", "table4", "paper_mjx"], help="secondary workload on the chosen config (see VARIANTS)")
+    ap.add_argument("--variant", default="", choices=["", "dyn", "table4", "noise", "paper_mjx"], help="secondary workload on the chosen config (see VARIANTS)")
     args = ap.parse_args()
     wl = W.config(args.config)
     if args.variant:

@@ -157,7 +157,12 @@ typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its devic
 /* Fill *out with Table 2 (drone_model), Table 6 and the documented defaults.  host pointer. */
 int mdg_default_params(int drone_model, mdg_params* out);
 
-/* Create n_envs environments of n_drones (1..32) drones each.  physics_mode: Table 1; action_type:
+/* Kernel selection: the five BASELINE configs and a few variants have precompiled instances of the step kernel; for any other
+ * combination of modes and params mdg_create compiles an instance for exactly that combination with NVRTC (about a second, cached
+ * per process; the sources are the csrc/ files beside the library) and falls back to a runtime-flag generic kernel if that is not
+ * possible.  Environment variable MDG_JIT=0 forces the generic kernel.  mdg_kernel_name tells which one runs.
+ *
+ * Create n_envs environments of n_drones (1..32) drones each.  physics_mode: Table 1; action_type:
  * Table 3.  params (host, copied) may be NULL for the CF2X defaults.  *out receives the handle. */
 int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, const mdg_params* params,
                mdg_env** out);

@@ -1,6 +1,8 @@
 // mdg.cu — host side of libmdg.so: the C ABI of include/mdg.h, the SoA allocator, parameter
 // preprocessing, kernel dispatch and CUDA-graph replay.  No CPU fallback: every step runs in the
 // kernels of mdg_kernels.cuh.
+#include <nvrtc.h>
+#include <dlfcn.h>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -44,6 +46,7 @@ struct mdg_env {
     std::string kernel_name;
     int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
     int pdl = 1;
+    int jit = 1;                         // MDG_JIT=0: never compile at run time, use the generic kernel
     uint32_t seq = 0;                    // step launches so far (kernel parameter; see "chain" in mdg_kernels.cuh)
     bool saturating = false;             // the step grid occupies every resident block slot of the device
     bool chainable = false;              // the last operation on this handle was a stream-launched step
@@ -202,6 +205,53 @@ template <int G, int FEAT> static step_fn pick_minb(int minb) {
     }
 }
 
+// ---- run-time specialisation: the handle's own feature word instantiated with NVRTC over the same source ---------------------
+// A feature word without a precompiled specialisation would run the runtime-flag generic kernel at 1.7-2.1x the time
+// (DESIGN.md 6).  Instead, step_kernel<G, FEAT, MINB> is compiled for exactly this word (about a second, cached per process);
+// the sources are the .cuh files beside the library.  Any failure falls back to the generic kernel.  MDG_JIT=0 disables it.
+extern "C" int mdg_version(void);
+static std::map<std::tuple<int, int, int>, step_fn> g_jit;
+static step_fn jit_step_kernel(int G, int feat, int minb) {
+    const auto key = std::make_tuple(G, feat, minb);
+    auto it = g_jit.find(key);
+    if (it != g_jit.end()) return it->second;
+    step_fn result = nullptr;
+    g_jit[key] = nullptr;                                        // a failed attempt is not repeated
+    Dl_info info;
+    if (!dladdr((void*)&mdg_version, &info) || !info.dli_fname) return nullptr;
+    std::string dir(info.dli_fname);
+    const size_t slash = dir.find_last_of('/');
+    dir = (slash == std::string::npos ? std::string(".") : dir.substr(0, slash)) + "/csrc";
+    const std::string src = "#include \"mdg_kernels.cuh\"\n";
+    const char* hdr_names[2] = {"stdint.h", "cuda_runtime.h"};   // NVRTC has the CUDA built-ins; only the fixed-width names are missing
+    const char* hdr_src[2] = {"#pragma once\ntypedef unsigned char uint8_t; typedef unsigned int uint32_t; typedef int int32_t; "
+                              "typedef unsigned long long uint64_t; typedef long long int64_t; typedef unsigned long uintptr_t;\n",
+                              "#pragma once\n"};
+    nvrtcProgram prog = nullptr;
+    if (nvrtcCreateProgram(&prog, src.c_str(), "mdg_jit.cu", 2, hdr_src, hdr_names) != NVRTC_SUCCESS) return nullptr;
+    const std::string expr = "mdg::step_kernel<" + std::to_string(G) + ", " + std::to_string(feat) + ", " + std::to_string(minb) + ">";
+    const std::string inc = "-I" + dir;
+    const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", inc.c_str()};
+    std::vector<char> cubin;
+    if (nvrtcAddNameExpression(prog, expr.c_str()) == NVRTC_SUCCESS && nvrtcCompileProgram(prog, 4, opts) == NVRTC_SUCCESS) {
+        const char* lowered = nullptr;
+        size_t nb = 0;
+        if (nvrtcGetLoweredName(prog, expr.c_str(), &lowered) == NVRTC_SUCCESS && lowered && nvrtcGetCUBINSize(prog, &nb) == NVRTC_SUCCESS && nb > 0) {
+            cubin.resize(nb);
+            cudaLibrary_t lib = nullptr;
+            cudaKernel_t kern = nullptr;
+            if (nvrtcGetCUBIN(prog, cubin.data()) == NVRTC_SUCCESS &&
+                cudaLibraryLoadData(&lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0) == cudaSuccess &&
+                cudaLibraryGetKernel(&kern, lib, lowered) == cudaSuccess)
+                result = reinterpret_cast<step_fn>(kern);       // kernel handles are accepted wherever the runtime takes a function pointer
+            else cudaGetLastError();
+        }
+    }
+    nvrtcDestroyProgram(&prog);
+    g_jit[key] = result;
+    return result;
+}
+
 static void pick_kernels(mdg_env* h) {
     const int f = h->P.feat;
     h->step = nullptr;
@@ -215,6 +265,11 @@ static void pick_kernels(mdg_env* h) {
     SPECIAL(4, FEAT_C5 | F_EULER, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation,dyn>")   // Table 1's DYN integrator on the metric's config
     SPECIAL(4, FEAT_C5 | F_DR | F_MLAG | F_SENS | F_LAT, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation,table4>")   // every row of Table 4 on it
 #undef SPECIAL
+    if (!h->step && h->jit) {                                        // no precompiled specialisation: instantiate this word now
+        const int mb = h->minb < 4 ? 4 : (h->minb > 8 ? 8 : h->minb);
+        h->step = jit_step_kernel(h->G, f, mb);
+        if (h->step) h->kernel_name = "step_kernel<G=" + std::to_string(h->G) + ",jit:" + std::to_string(f) + ">";
+    }
 #define GENERIC(g) case g: if (!h->step) { h->step = h->minb <= 3 ? step_kernel<g, -1, 3> : step_kernel<g, -1, 4>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
                    h->reset = reset_kernel<g>; h->refresh = refresh_obs_kernel<g>; break;
     switch (h->G) { GENERIC(1) GENERIC(2) GENERIC(4) GENERIC(8) GENERIC(16) GENERIC(32) }
@@ -374,7 +429,8 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     h->N = n_envs; h->M = n_drones; h->physics_mode = physics_mode; h->action_type = action_type; h->hp = p;
     int G = 1; while (G < n_drones) G <<= 1;
     h->G = G;
-    if (const char* ev = std::getenv("MDG_PDL")) h->pdl = ev[0] != '0';   // development knob: MDG_PDL=0 launches plainly
+    if (const char* ev = std::getenv("MDG_PDL")) h->pdl = ev[0] != '0';
+    if (const char* ev = std::getenv("MDG_JIT")) h->jit = ev[0] != '0';   // development knob: MDG_PDL=0 launches plainly
     make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type, n_drones, G), h->P);
     pick_kernels(h);
     // one arena: 7 drone planes, env plane, gstep, obs, reward, done (each 256 B aligned)
@@ -415,7 +471,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
         const bool generic = h->kernel_name.find("generic") != std::string::npos;
         // 5 for the benchmark specialisations (96 registers); 6 for the lighter DYN integrator; 4 where Table 4's planes and draws
         // would spill at 96; the runtime-flag kernel needs 162 registers to stay out of local memory (3)
-        h->minb = generic ? 3 : (h->P.feat & (F_DR | F_MLAG | F_LAT | F_SENS)) ? 4 : (h->P.feat & F_EULER) ? 6 : 5;
+        h->minb = generic ? 3 : (h->P.feat & (F_DR | F_MLAG | F_LAT | F_SENS)) ? 4 : (h->P.feat & F_EULER) ? 6 : 5;   // jit kernels follow the same rule
         pick_kernels(h);
         rc = configure_launch(h);
     }
