@@ -1,6 +1,7 @@
 // mdg.cu — host side of libmdg.so: the C ABI of include/mdg.h, the SoA allocator, parameter
 // preprocessing, kernel dispatch and CUDA-graph replay.  No CPU fallback: every step runs in the
 // kernels of mdg_kernels.cuh.
+#include <mutex>
 #include <nvrtc.h>
 #include <dlfcn.h>
 #include <cmath>
@@ -211,7 +212,9 @@ template <int G, int FEAT> static step_fn pick_minb(int minb) {
 // the sources are the .cuh files beside the library.  Any failure falls back to the generic kernel.  MDG_JIT=0 disables it.
 extern "C" int mdg_version(void);
 static std::map<std::tuple<int, int, int>, step_fn> g_jit;
+static std::mutex g_jit_mutex;                                   // distinct handles may be created from different threads
 static step_fn jit_step_kernel(int G, int feat, int minb) {
+    std::lock_guard<std::mutex> guard(g_jit_mutex);
     const auto key = std::make_tuple(G, feat, minb);
     auto it = g_jit.find(key);
     if (it != g_jit.end()) return it->second;
