@@ -4,9 +4,10 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
 
 One "step" is one control step of the whole batch (action decode -> K substeps -> obs/reward/done/
-auto-reset) = ONE kernel launch.  See DESIGN.md §7 for what each JSON key means and how the roofline
-numbers are derived.  `--impl reference` times the float64 oracle on the host cores (a baseline, not
-the target).
+auto-reset) = ONE kernel launch.  The timed region is R back-to-back repeats of K steps, one CUDA-event pair
+per repeat; `ms_per_step` is the MEDIAN repeat (min / max / repeats beside it).  See DESIGN.md §7 for what
+each JSON key means and how the roofline numbers are derived.  `--impl reference` times the float64 oracle
+on the host cores (a baseline, not the target).
 """
 import argparse
 import json
@@ -21,6 +22,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 from paper_2606_08039_b200 import workloads as W  # noqa: E402
+from paper_2606_08039_b200.sharding import max_over_ranks, replica_base  # noqa: E402
 
 METRIC = "env_steps_per_sec"
 UNIT = "env-steps/s"
@@ -29,19 +31,12 @@ ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # algorithmic flops per drone per control step, tallied by the oracle's counting scalar type on the
 # seeded workloads (tests/test_oracle_control_env.py::test_flop_tally...)
 FLOPS_PER_DRONE_STEP = {1: 3186.0, 2: 3421.1, 3: 3350.0, 4: 3893.6, 5: 3858.75}
+SURVEY_FLOPS_PER_DRONE_STEP = {1: 2750.0, 2: 2960.0, 3: 2870.0, 4: 3800.0, 5: 3540.0}   # SURVEY.md 8(d) hand tally (DESIGN.md 6 reconciles the two)
 REPLICAS = 4          # independent env batches stepped round-robin so the working set exceeds the 126 MB L2
 
 
-# Secondary workloads (`--variant`, never the default line): the metric's config with the DYN integrator of Table 1
-# (SURVEY.md 8(f) NEXT-1 "DYN mode benchmarked"), and with every row of Table 4 switched on (NEXT-2: per-episode parameter
-# planes, motor lag, action / sensor latency, sensor noise) - both run the generic, runtime-flag instantiation of the kernel.
-VARIANTS = {
-    "dyn": dict(integrator=W.INTEG_EULER),
-    "noise": dict(obs_noise=[0.01, 0.05, 0.0174533, 0.05]),      # no precompiled specialisation: instantiated at mdg_create (MDG_JIT=0: generic kernel)
-    "table4": dict(dr_alpha=[0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02, 0.05, 0.02, 0.05, 0.0], reset_rpy_half=[0.1, 0.1, 0.1],
-                   reset_vel_half=[0.5, 0.5, 0.5], motor_lag_lo=0.005, motor_lag_hi=0.05, act_latency_lo=0.0, act_latency_hi=0.05,
-                   obs_latency_lo=0.0, obs_latency_hi=0.02, obs_noise=[0.01, 0.05, 0.0174533, 0.05]),
-}
+VARIANTS = W.VARIANTS      # secondary workloads (`--variant`, never the default line): the overrides the parity tests run too
+GRAPH_STEPS = 48          # steps per captured CUDA graph (REPLICAS batches x 12 steps, round-robin)
 
 
 def algorithmic_bytes_per_drone(wl) -> float:
@@ -113,11 +108,11 @@ def harness_actions(wl):
     return None
 
 
-def oracle_throughput(wl, budget_s, n_envs, min_steps=4, max_steps=10 ** 9):
-    """Time the oracle as it stands on a bounded sample of the workload: env-steps/s on the host cores."""
+def oracle_throughput(wl, budget_s, n_envs, min_steps=4, max_steps=10 ** 9, threads=None):
+    """Time the oracle as it stands on a bounded sample of the workload: env-steps/s on `threads` host cores (default: all)."""
     import numpy as np
     from oracle import oracle as O
-    cores = len(os.sched_getaffinity(0))
+    cores = threads or len(os.sched_getaffinity(0))
     sample = wl.scaled(min(wl.n_envs, n_envs))
     env = O.OracleEnv(sample.n_envs, sample.n_drones, sample.physics_mode, sample.action_type, O.OracleParams(0, **sample.params), n_threads=cores)
     env.reset(sample.seed)
@@ -214,6 +209,33 @@ def config_dict(wl, c, n_gpus):
             "l2": f"{REPLICAS} independent env batches stepped round-robin (working set > 126 MB L2)"}
 
 
+def capture_round_robin(torch, envs, acts, stream, n_steps):
+    """One CUDA graph of n_steps chained steps over the env batches, round-robin (caller-side capture of mdg_step_chained:
+    launch numbers live on the device, so the graph can be replayed any number of times)."""
+    A = len(acts[0])
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=stream):
+        cs = torch.cuda.current_stream()
+        for e in envs:
+            e.set_stream(cs)
+        for k in range(n_steps):
+            envs[k % len(envs)].step_chained(acts[k % len(envs)][(k // len(envs)) % A])
+    for e in envs:
+        e.set_stream(stream)
+    return g
+
+
+def timed_repeats(torch, stream, body, repeats):
+    """R back-to-back repeats of body() on `stream`, one event pair per repeat; returns the per-repeat milliseconds."""
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(repeats + 1)]
+    evs[0].record(stream)
+    for r in range(repeats):
+        body()
+        evs[r + 1].record(stream)
+    stream.synchronize()
+    return [evs[r].elapsed_time(evs[r + 1]) for r in range(repeats)]
+
+
 def run_ours(args, wl, c):
     import torch
     import paper_2606_08039_b200 as mdg
@@ -227,13 +249,16 @@ def run_ours(args, wl, c):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     K, Wm = args.steps, max(args.warmup, 3)
+    use_graph = args.mode == "graph" or (args.mode == "auto" and c != 5)    # the latency-bound configs: no host launch rate in the number
+    if use_graph:
+        K = -(-K // GRAPH_STEPS) * GRAPH_STEPS                              # whole graphs
     stream = torch.cuda.Stream()
     ha = harness_actions(wl)
     A = 4                                                  # distinct action sets per replica
     envs, acts = [], []
     with torch.cuda.stream(stream):
         for r in range(REPLICAS):
-            over = dict(wl.params, env_index_base=(rank * REPLICAS + r) * wl.n_envs)
+            over = dict(wl.params, env_index_base=replica_base(rank, r, REPLICAS, wl.n_envs))
             env = mdg.Env(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, mdg.default_params(0, **over), stream=stream)
             if args.block or args.max_blocks:
                 env.set_launch(args.block, args.max_blocks)
@@ -242,37 +267,56 @@ def run_ours(args, wl, c):
             if ha:
                 acts.append([env.gen_actions(wl.seed, t, *ha) for t in range(A)])
             else:
-                acts.append([env.targets] * A)             # PID waypoint = the per-episode target (device resident)
-        launches0 = sum(e.launch_count for e in envs)
-        for k in range(Wm):
-            envs[k % REPLICAS].step(acts[k % REPLICAS][(k // REPLICAS) % A])
+                acts.append([env.targets] * A)             # PID waypoint = the live per-episode target plane (written by the step itself, item by item)
         stream.synchronize()
+
+        # The actions are complete before the first step is enqueued, which is mdg_step_chained's contract: consecutive steps
+        # of a batch order themselves item by item, the steps of the other batches in between overlap.
+        def run_stream(n):
+            for k in range(n):
+                envs[k % REPLICAS].step_chained(acts[k % REPLICAS][(k // REPLICAS) % A])
+
+        graph = capture_round_robin(torch, envs, acts, stream, GRAPH_STEPS)
+
+        def run_graph(n):
+            with torch.cuda.stream(stream):
+                for _ in range(n // GRAPH_STEPS):
+                    graph.replay()
+
+        run = run_graph if use_graph else run_stream
+        run(max(Wm, GRAPH_STEPS) if use_graph else Wm)
+        # size the block of repeats: at least 7, and long enough (0.6 s) for the clock sampler to see the GPU under this load
+        pre = timed_repeats(torch, stream, lambda: run(K), 3)
+        est = sorted(pre)[1] / 1e3
+        R = int(max(7, min(args.max_repeats, 0.6 / max(est, 1e-6))))
         if dist:
+            rt = torch.tensor([R], device="cuda")
+            dist.all_reduce(rt, op=dist.ReduceOp.MAX)
+            R = int(rt.item())
             dist.barrier()
         torch.cuda.synchronize()
         sampler = ClockSampler(local)
         if rank == 0:
             sampler.start()
             time.sleep(0.1)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         l0 = sum(e.launch_count for e in envs)
         t_wall0 = time.time()
-        ev0.record(stream)
-        for k in range(K):
-            envs[k % REPLICAS].step(acts[k % REPLICAS][(k // REPLICAS) % A])
-        ev1.record(stream)
-        stream.synchronize()
+        per_repeat = timed_repeats(torch, stream, lambda: run(K), R)
         torch.cuda.synchronize()
         t_wall1 = time.time()
         if dist:
             dist.barrier()
-        ms = ev0.elapsed_time(ev1)
-        launches = sum(e.launch_count for e in envs) - l0
+        launches = (R * K) if use_graph else (sum(e.launch_count for e in envs) - l0)
         clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-        if dist:
-            tt = torch.tensor([ms], device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ms = float(tt.item())
+        srt = sorted(per_repeat)
+        ms, ms_min, ms_max = srt[len(srt) // 2], srt[0], srt[-1]
+        ms, ms_min, ms_max = (max_over_ranks(x, dist, "cuda") for x in (ms, ms_min, ms_max))
+        # the other launch path beside the headline one: K steps as replays of one captured graph / as a stream of launches
+        other = run_stream if use_graph else run_graph
+        Ko = -(-K // GRAPH_STEPS) * GRAPH_STEPS
+        other(Ko)
+        alt = sorted(timed_repeats(torch, stream, lambda: other(Ko), 7))[3]
+        alt = max_over_ranks(alt, dist, "cuda")
         # ---- end to end through the C ABI with host buffers (pinned): H2D actions, step, D2H obs/reward/done, every step.
         # (a) one batch, the synchronous call (mdg_step_host); (b) two batches double-buffered on two streams
         # (mdg_step_host_async / mdg_wait): the host consumes batch A's results while batch B is in flight, so one batch's
@@ -336,6 +380,7 @@ def run_ours(args, wl, c):
     per_launch_s = sec / K
     drones = wl.n_envs * wl.n_drones
     cpu = oracle_throughput(wl, budget_s=args.cpu_budget, n_envs=16384) if world == 1 and not args.no_cpu else None
+    cpu1 = oracle_throughput(wl, budget_s=args.cpu_budget / 3, n_envs=2048, threads=1) if cpu else None
     fpd = cpu["flops_per_drone_step"] if cpu else FLOPS_PER_DRONE_STEP[c]
     flops = fpd * drones
     bytes_alg = algorithmic_bytes_per_drone(wl) * drones
@@ -359,12 +404,26 @@ def run_ours(args, wl, c):
                 traffic = float(row["traffic_bytes"])
     except Exception:
         pass
+    traffic_timed = None                                   # the same, summed over four consecutive launches of the four batches / 4
+    try:
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv"))):
+            if row["config"] == (f"c{c}+{args.variant}_timed" if args.variant else f"c{c}_timed"):
+                traffic_timed = float(row["traffic_bytes"])
+    except Exception:
+        pass
+    cfg = config_dict(wl, c, world)
+    cfg["launch_path"] = (f"replays of one CUDA graph of {GRAPH_STEPS} chained steps (caller-side capture of mdg_step_chained)" if use_graph
+                          else "a stream of mdg_step_chained launches (actions pre-generated and resident: its contract)")
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
+            "repeats": R, "ms_per_step_min": ms_min / K, "ms_per_step_max": ms_max / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": config_dict(wl, c, world),
+            "config": cfg,
+            ("stream" if use_graph else "graph"): {"ms_per_step": alt / Ko, "steps_per_graph": GRAPH_STEPS, "steps": Ko, "repeats": 7,
+                                                     "value": world * wl.n_envs * Ko / (alt / 1e3)},
             "drone_substeps_per_sec": value * wl.n_drones * 5,
             "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved_tf / ALU_PEAK_TFLOPS,
-                         "traffic": traffic, "kernel": envs[0].kernel_name, "us_per_launch": per_launch_s * 1e6,
+                         "traffic": traffic, "traffic_timed": traffic_timed, "kernel": envs[0].kernel_name,
+                         "frac_survey_tally": SURVEY_FLOPS_PER_DRONE_STEP[c] * drones / per_launch_s / 1e12 / ALU_PEAK_TFLOPS, "us_per_launch": per_launch_s * 1e6,
                          "flops_per_launch": flops, "bytes_per_launch": bytes_alg,
                          "peak_note": "FP32 ALU peak derived: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md §6)",
                          "ffma_measured_tflops": ffma_tf, "frac_of_ffma_measured": (achieved_tf / ffma_tf) if ffma_tf else None,
@@ -379,6 +438,8 @@ def run_ours(args, wl, c):
             "gpu_launches": launches, "clocks": clocks}
     if cpu:
         line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"]["single_thread_value"] = cpu1["value"]
+        line["cpu_baseline"]["single_thread_sample"] = cpu1["sample"]
     if world == 1 and not args.no_camera:
         del envs, acts
         torch.cuda.empty_cache()
@@ -391,13 +452,17 @@ def run_ours(args, wl, c):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20000)
-    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (5 = 65,536 envs x 4 drones, the metric's config)")
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--max-blocks", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=50)
+    ap.add_argument("--mode", default="auto", choices=["auto", "stream", "graph"],
+                    help="launch path of the timed region: a stream of mdg_step_chained calls, or replays of one captured CUDA graph "
+                         "(auto: stream for config 5, graph for the latency-bound configs 1-4); the other one is reported beside it")
+    ap.add_argument("--max-repeats", type=int, default=2000)
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-camera", action="store_true", help="skip the secondary onboard-camera measurement")

@@ -160,7 +160,10 @@ int mdg_default_params(int drone_model, mdg_params* out);
 /* Kernel selection: the five BASELINE configs and a few variants have precompiled instances of the step kernel; for any other
  * combination of modes and params mdg_create compiles an instance for exactly that combination with NVRTC (about a second, cached
  * per process; the sources are the csrc/ files beside the library) and falls back to a runtime-flag generic kernel if that is not
- * possible.  Environment variable MDG_JIT=0 forces the generic kernel.  mdg_kernel_name tells which one runs.
+ * possible.  The fallback is 1.7-2.1x slower but not an error: mdg_create still returns MDG_OK, mdg_kernel_name says
+ * "generic", and mdg_last_error() right after mdg_create holds the reason.  Environment variable MDG_JIT=0 forces the generic
+ * kernel, MDG_JIT=require makes mdg_create fail with MDG_ECUDA instead of falling back; MDG_JIT_SRC overrides the directory
+ * the sources are read from.
  *
  * Create n_envs environments of n_drones (1..32) drones each.  physics_mode: Table 1; action_type:
  * Table 3.  params (host, copied) may be NULL for the CF2X defaults.  *out receives the handle. */
@@ -172,12 +175,34 @@ void mdg_destroy(mdg_env* env);
  * zero controller memory, wind and step counters; obs is valid afterwards (reward 0, done 0). */
 int mdg_reset(mdg_env* env, uint64_t seed);
 
-/* One control step.  actions_dev: [n_envs*n_drones][4] fp32, caller-owned device memory, 16-byte aligned, read only;
- * the meaning of the four floats follows the action type (see MDG_ACT_* above).  Asynchronous on the bound stream. */
+/* One control step: the paper's `step(state, action) -> state, obs, reward, done` for every env, i.e. action
+ * decode (Table 3; PID PAPER.md:347-376), Eq.1-6 wrench, sim_freq/ctrl_freq integration
+ * substeps, observation / reward / termination and same-call auto-reset
+ * (PAPER.md:254-258), in one kernel launch.  actions_dev: [n_envs*n_drones][4] fp32, caller-owned device memory, 16-byte
+ * aligned, read only; the meaning of the four floats follows the action type (see MDG_ACT_* above).  Asynchronous on the bound
+ * stream, with plain stream semantics: the step starts after everything enqueued before it on that stream has completed
+ * (so a policy kernel or mdg_gen_actions may write actions_dev right before it), and everything enqueued after
+ * it sees its outputs complete.  MDG_EINVAL: NULL or misaligned argument. */
 int mdg_step(mdg_env* env, const float* actions_dev);
 
-/* n_steps control steps replayed as one CUDA graph: step k reads actions_dev + k*stride_floats.
- * The graph is cached per (pointer, n_steps, stride).  Outputs hold the last step's values. */
+/* The same step for callers whose actions do not come from the stream: the step is launched with programmatic dependent launch
+ * and, when the previous operation on this handle was a step on the same stream, does NOT wait for the previous kernel of the
+ * stream as a whole; it orders itself behind the previous step of this handle work item by work item, so the drain
+ * of one step overlaps the ramp-up of the next, and steps of other handles enqueued in between overlap as well.
+ * CONTRACT: the contents of actions_dev must have been complete and visible before the previous step of this handle was enqueued
+ * (pre-generated action sets, buffers whose producer a full stream / event dependency ordered before that step).  With an
+ * in-stream producer between two steps use mdg_step.  Everything enqueued after the step still sees it complete.  The first step
+ * after any other operation on the handle (reset, set_state, load, render, set_stream, a graph replay) behaves like mdg_step.
+ * The paper's counterpart is the jitted `lax.scan` of K sub-steps inside one call: work queued ahead, no host
+ * round trip.  Same arguments and errors as mdg_step. */
+int mdg_step_chained(mdg_env* env, const float* actions_dev);
+
+/* n_steps control steps (each exactly mdg_step) replayed as one CUDA graph: step k reads actions_dev +
+ * k*stride_floats; all n_steps action sets must be complete before the call.  Inside the graph the steps chain like
+ * mdg_step_chained; the first waits for whatever precedes the replay.  The graph is cached per (pointer, n_steps, stride) and can
+ * be replayed any number of times, between other steps; mdg_reset / mdg_load / mdg_set_launch drop the cache (seed and launch
+ * shape are kernel parameters).  Outputs hold the last step's values.
+ * MDG_EINVAL: NULL, n_steps < 1, misaligned pointer or stride. */
 int mdg_step_many(mdg_env* env, const float* actions_dev, int n_steps, int64_t stride_floats);
 
 /* One control step with HOST buffers (the end-to-end call): copies actions_host [n_envs*n_drones][4] to
@@ -262,12 +287,10 @@ int mdg_default_cam_params(const mdg_params* params, mdg_cam_params* out);
  * (0, 180), znear <= 0 or zfar <= znear, non-positive body axes. */
 int mdg_render_depth(mdg_env* env, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev);
 
-/* Scheduling note for mdg_step: the step is launched with programmatic dependent launch.  When the previous
- * operation on the handle was a step on the same stream, the new launch does not wait for that kernel as a whole but,
- * work item by work item, for the sequence flags it publishes; all other stream semantics are unchanged:
- * any non-PDL operation enqueued after a step (a copy, a kernel reading obs) sees the step complete.
- *
- * Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) used by later calls. */
+/* Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) used by later calls.  Work already queued
+ * on the previously bound stream (the clear and reset of mdg_create, earlier steps) is ordered before whatever is enqueued on
+ * the new one afterwards (an event on the old stream, waited on by the new; skipped when either stream is being captured:
+ * inside a capture the ordering is the caller's graph).  MDG_EINVAL: NULL handle.  (The simulator itself has no notion of streams; this serves PAPER.md:292, keeping the loop on the device.) */
 int mdg_set_stream(mdg_env* env, void* cuda_stream);
 
 /* Introspection: kernels launched so far through this handle; name of the step kernel specialisation. */

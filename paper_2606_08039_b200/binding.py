@@ -62,7 +62,7 @@ class mdg_cam_params(C.Structure):
     update = mdg_params.update
 
 
-EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_wait", "mdg_checkpoint_size", "mdg_save", "mdg_load", "mdg_outputs",
+EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_chained", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_wait", "mdg_checkpoint_size", "mdg_save", "mdg_load", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
            "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_last_error", "mdg_version"]
 
@@ -84,6 +84,7 @@ def lib():
         L.mdg_destroy.restype = None
         L.mdg_reset.argtypes = [vp, C.c_uint64]
         L.mdg_step.argtypes = [vp, vp]
+        L.mdg_step_chained.argtypes = [vp, vp]
         L.mdg_step_many.argtypes = [vp, vp, C.c_int, C.c_int64]
         L.mdg_step_host.argtypes = [vp] * 5
         L.mdg_step_host_async.argtypes = [vp] * 5
@@ -219,6 +220,11 @@ class Env:
 
     def step(self, actions):
         _check(lib().mdg_step(self._h, self._act_ptr(actions)))
+        return self.obs, self.reward, self.done
+
+    def step_chained(self, actions):
+        """mdg_step_chained: `actions` must have been complete before the previous step of this env was enqueued (include/mdg.h)."""
+        _check(lib().mdg_step_chained(self._h, self._act_ptr(actions)))
         return self.obs, self.reward, self.done
 
     def step_many(self, actions, n_steps):

@@ -3,6 +3,7 @@
 // kernels of mdg_kernels.cuh.
 #include <mutex>
 #include <nvrtc.h>
+#include <nvtx3/nvToolsExt.h>
 #include <dlfcn.h>
 #include <cmath>
 #include <cstdio>
@@ -47,11 +48,15 @@ struct mdg_env {
     std::string kernel_name;
     int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
     int pdl = 1;
-    int jit = 1;                         // MDG_JIT=0: never compile at run time, use the generic kernel
-    uint32_t seq = 0;                    // step launches so far (kernel parameter; see "chain" in mdg_kernels.cuh)
+    int jit = 1;                         // MDG_JIT=0: never compile at run time, use the generic kernel; MDG_JIT=require: fail instead of falling back
+    std::string jit_note;                // why the run-time specialisation was not possible (empty: it was, or was not needed)
     bool saturating = false;             // the step grid occupies every resident block slot of the device
-    bool chainable = false;              // the last operation on this handle was a stream-launched step
+    uint32_t seq = 0;                    // step launches issued so far (kernel parameter: flags and dispenser parity, mdg_kernels.cuh)
+    bool chainable = false;              // the last operation on this handle was a step (launched on last_stream, in capture last_capture)
     cudaStream_t last_stream = nullptr;
+    unsigned long long last_capture = 0;
+    float* stage = nullptr;              // device staging buffer of mdg_step_host (lazily allocated)
+    cudaEvent_t order_event = nullptr;   // mdg_set_stream: orders the new stream behind work queued on the old one
     int n_sms = 0, step_grid = 0;        // persistent step kernel: one block per resident slot, looping over tiles
     int64_t launches = 0;
     std::map<std::tuple<const void*, int, int64_t>, cudaGraphExec_t> graphs;
@@ -111,6 +116,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
         A[0] = (float)c; A[1] = (float)(-c * c2 / 6.0); A[2] = (float)(c * c2 * c2 / 120.0); A[3] = (float)(-c * c2 * c2 * c2 / 5040.0);
         Bc[0] = (float)(c2 / 2.0); Bc[1] = (float)(-c2 * c2 / 24.0); Bc[2] = (float)(c2 * c2 * c2 / 720.0); Bc[3] = (float)(-c2 * c2 * c2 * c2 / 40320.0);
     }
+    for (int i = 0; i < 4; ++i) { D.rotnA_half[i] = -D.rotA_half[i]; D.rotnA_full[i] = -D.rotA_full[i]; }
     {                                                             // Eq.7 increment for phi = (h/6) s in y = |s|^2
         const double c = h / 6.0, c2 = c * c;
         D.expC[0] = 1.0f; D.expC[1] = (float)(-c2 / 8.0); D.expC[2] = (float)(c2 * c2 / 384.0); D.expC[3] = (float)(-c2 * c2 * c2 / 46080.0);
@@ -121,6 +127,7 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     D.gyro[0] = (float)(((double)p.J[2] - p.J[1]) / p.J[0]);
     D.gyro[1] = (float)(((double)p.J[0] - p.J[2]) / p.J[1]);
     D.gyro[2] = (float)(((double)p.J[1] - p.J[0]) / p.J[2]);
+    for (int i = 0; i < 3; ++i) D.ngyro[i] = -D.gyro[i];
     const double l = p.L / std::sqrt(2.0), kappa = (double)p.k_m / p.k_f;
     D.k_f = p.k_f; D.inv_k_f = (float)(1.0 / p.k_f); D.l = (float)l; D.kappa = (float)kappa;
     D.inv_l = (float)(1.0 / l); D.inv_kappa = (float)(1.0 / kappa);
@@ -211,32 +218,40 @@ template <int G, int FEAT> static step_fn pick_minb(int minb) {
 // (DESIGN.md 6).  Instead, step_kernel<G, FEAT, MINB> is compiled for exactly this word (about a second, cached per process);
 // the sources are the .cuh files beside the library.  Any failure falls back to the generic kernel.  MDG_JIT=0 disables it.
 extern "C" int mdg_version(void);
-static std::map<std::tuple<int, int, int>, step_fn> g_jit;
+static std::map<std::tuple<int, int, int>, std::pair<step_fn, std::string>> g_jit;   // kernel or, on failure, why
 static std::mutex g_jit_mutex;                                   // distinct handles may be created from different threads
-static step_fn jit_step_kernel(int G, int feat, int minb) {
+static step_fn jit_step_kernel(int G, int feat, int minb, std::string& why) {
     std::lock_guard<std::mutex> guard(g_jit_mutex);
     const auto key = std::make_tuple(G, feat, minb);
     auto it = g_jit.find(key);
-    if (it != g_jit.end()) return it->second;
+    if (it != g_jit.end()) { why = it->second.second; return it->second.first; }   // a failed attempt is not repeated
     step_fn result = nullptr;
-    g_jit[key] = nullptr;                                        // a failed attempt is not repeated
+    auto done = [&](const std::string& msg) { why = msg; g_jit[key] = std::make_pair(result, msg); return result; };
     Dl_info info;
-    if (!dladdr((void*)&mdg_version, &info) || !info.dli_fname) return nullptr;
+    if (!dladdr((void*)&mdg_version, &info) || !info.dli_fname) return done("dladdr cannot locate libmdg.so");
     std::string dir(info.dli_fname);
     const size_t slash = dir.find_last_of('/');
     dir = (slash == std::string::npos ? std::string(".") : dir.substr(0, slash)) + "/csrc";
+    if (const char* ev = std::getenv("MDG_JIT_SRC")) dir = ev;   // where the .cuh sources are (default: csrc/ beside the library)
     const std::string src = "#include \"mdg_kernels.cuh\"\n";
     const char* hdr_names[2] = {"stdint.h", "cuda_runtime.h"};   // NVRTC has the CUDA built-ins; only the fixed-width names are missing
     const char* hdr_src[2] = {"#pragma once\ntypedef unsigned char uint8_t; typedef unsigned int uint32_t; typedef int int32_t; "
                               "typedef unsigned long long uint64_t; typedef long long int64_t; typedef unsigned long uintptr_t;\n",
                               "#pragma once\n"};
     nvrtcProgram prog = nullptr;
-    if (nvrtcCreateProgram(&prog, src.c_str(), "mdg_jit.cu", 2, hdr_src, hdr_names) != NVRTC_SUCCESS) return nullptr;
+    if (nvrtcCreateProgram(&prog, src.c_str(), "mdg_jit.cu", 2, hdr_src, hdr_names) != NVRTC_SUCCESS) return done("nvrtcCreateProgram failed");
     const std::string expr = "mdg::step_kernel<" + std::to_string(G) + ", " + std::to_string(feat) + ", " + std::to_string(minb) + ">";
     const std::string inc = "-I" + dir;
     const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", inc.c_str()};
     std::vector<char> cubin;
-    if (nvrtcAddNameExpression(prog, expr.c_str()) == NVRTC_SUCCESS && nvrtcCompileProgram(prog, 4, opts) == NVRTC_SUCCESS) {
+    std::string msg;
+    if (nvrtcAddNameExpression(prog, expr.c_str()) != NVRTC_SUCCESS) msg = "nvrtcAddNameExpression failed";
+    else if (nvrtcCompileProgram(prog, 4, opts) != NVRTC_SUCCESS) {
+        size_t ln = 0;
+        std::string log;
+        if (nvrtcGetProgramLogSize(prog, &ln) == NVRTC_SUCCESS && ln > 1) { log.resize(ln); nvrtcGetProgramLog(prog, &log[0]); }
+        msg = "NVRTC could not compile " + expr + " from " + dir + ": " + log.substr(0, 300);
+    } else {
         const char* lowered = nullptr;
         size_t nb = 0;
         if (nvrtcGetLoweredName(prog, expr.c_str(), &lowered) == NVRTC_SUCCESS && lowered && nvrtcGetCUBINSize(prog, &nb) == NVRTC_SUCCESS && nb > 0) {
@@ -247,12 +262,11 @@ static step_fn jit_step_kernel(int G, int feat, int minb) {
                 cudaLibraryLoadData(&lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0) == cudaSuccess &&
                 cudaLibraryGetKernel(&kern, lib, lowered) == cudaSuccess)
                 result = reinterpret_cast<step_fn>(kern);       // kernel handles are accepted wherever the runtime takes a function pointer
-            else cudaGetLastError();
-        }
+            else { cudaGetLastError(); msg = "the compiled cubin could not be loaded (cudaLibraryLoadData / cudaLibraryGetKernel)"; }
+        } else msg = "NVRTC produced no cubin";
     }
     nvrtcDestroyProgram(&prog);
-    g_jit[key] = result;
-    return result;
+    return done(msg);
 }
 
 static void pick_kernels(mdg_env* h) {
@@ -268,9 +282,10 @@ static void pick_kernels(mdg_env* h) {
     SPECIAL(4, FEAT_C5 | F_EULER, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation,dyn>")   // Table 1's DYN integrator on the metric's config
     SPECIAL(4, FEAT_C5 | F_DR | F_MLAG | F_SENS | F_LAT, "step_kernel<G=4,gnd+drag+dw+wind,vel,adj,formation,table4>")   // every row of Table 4 on it
 #undef SPECIAL
+    h->jit_note.clear();
     if (!h->step && h->jit) {                                        // no precompiled specialisation: instantiate this word now
         const int mb = h->minb < 4 ? 4 : (h->minb > 8 ? 8 : h->minb);
-        h->step = jit_step_kernel(h->G, f, mb);
+        h->step = jit_step_kernel(h->G, f, mb, h->jit_note);
         if (h->step) h->kernel_name = "step_kernel<G=" + std::to_string(h->G) + ",jit:" + std::to_string(f) + ">";
     }
 #define GENERIC(g) case g: if (!h->step) { h->step = h->minb <= 3 ? step_kernel<g, -1, 3> : step_kernel<g, -1, 4>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
@@ -301,12 +316,13 @@ static int configure_launch(mdg_env* h) {
     const long long items = ((long long)h->N + epw - 1) / epw, blocks = (items + wpb - 1) / wpb;
     const long long slots = (long long)h->n_sms * resident;
     h->step_grid = (int)(blocks < slots ? blocks : slots);
-    // Item-level chaining of consecutive steps.  A grid that fills every resident slot draws its items from a ticket
-    // dispenser; two dispensers alternate, which needs "at most two step kernels in flight": guaranteed there, because the
-    // successor's blocks can only start in slots this grid has vacated, and the successor's successor only once all of
-    // those have started.  A smaller grid gives every warp exactly one item (its index), draws nothing, and may
-    // therefore be chained to any depth.
-    h->saturating = blocks >= slots;
+    // Item-level chaining of consecutive steps.  A grid that fills every resident slot gives each warp the item of its own
+    // index first and hands the others out through a ticket dispenser (which therefore needs items >= warps); two dispensers
+    // alternate, which needs "at most two step kernels in flight": the successor's blocks can only start in slots this grid
+    // has vacated, and the successor's successor only once all of those have started (a warp of this grid would have to
+    // stall for a whole step to be still drawing then).  A smaller grid gives every warp exactly one item (its index), draws
+    // nothing, and may therefore be chained to any depth.
+    h->saturating = items >= slots * wpb;
     h->P.static_items = h->saturating ? 0u : 1u;                   // one warp per item, no dispenser: any depth of chained launches is safe
     return MDG_OK;
 }
@@ -318,11 +334,19 @@ static void drop_graphs(mdg_env* h) {
     for (auto& kv : h->graphs) cudaGraphExecDestroy(kv.second);
     h->graphs.clear();
 }
-static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s, bool may_chain) {
+// One launch of the fused step.  want_chain: the caller vouches that the actions were complete before the previous step of this
+// handle was enqueued (mdg_step_chained, the inner launches of mdg_step_many); the kernel then skips the grid-wide wait behind
+// the previous kernel of the stream and orders itself item by item behind the previous step (mdg_kernels.cuh) - but only if that
+// previous step really is the previous operation of this handle, on this stream and in the same capture (or both outside one).
+static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s, bool want_chain) {
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    unsigned long long cap_id = 0;
+    CU(cudaStreamGetCaptureInfo(s, &cap, &cap_id));
+    if (cap != cudaStreamCaptureStatusActive) cap_id = 0;
     h->seq += 1;
     h->P.seq = h->seq;
-    h->P.chain = (may_chain && h->pdl && h->chainable && h->last_stream == s) ? 1u : 0u;
-    h->chainable = may_chain; h->last_stream = s;
+    h->P.chain = (want_chain && h->pdl && h->chainable && h->last_stream == s && h->last_capture == cap_id) ? 1u : 0u;
+    h->chainable = true; h->last_stream = s; h->last_capture = cap_id;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)h->step_grid); cfg.blockDim = dim3((unsigned)h->block);
     cfg.dynamicSmemBytes = (size_t)h->smem; cfg.stream = s;
@@ -330,7 +354,11 @@ static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s, boo
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = h->pdl ? 1 : 0;
-    CU(cudaLaunchKernelEx(&cfg, h->step, h->P, h->B, reinterpret_cast<const float4*>(actions_dev)));
+    nvtxRangePushA("mdg_step");                                     // visible in Nsight timelines, free without a tool attached
+    const cudaError_t ce = cudaLaunchKernelEx(&cfg, h->step, h->P, h->B, reinterpret_cast<const float4*>(actions_dev));
+    nvtxRangePop();
+    if (ce != cudaSuccess) { h->chainable = false; return fail(MDG_ECUDA, std::string("cudaLaunchKernelEx(step_kernel): ") + cudaGetErrorString(ce)); }
+    h->launches += 1;
     return MDG_OK;
 }
 
@@ -433,7 +461,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     int G = 1; while (G < n_drones) G <<= 1;
     h->G = G;
     if (const char* ev = std::getenv("MDG_PDL")) h->pdl = ev[0] != '0';
-    if (const char* ev = std::getenv("MDG_JIT")) h->jit = ev[0] != '0';   // development knob: MDG_PDL=0 launches plainly
+    if (const char* ev = std::getenv("MDG_JIT")) h->jit = ev[0] == '0' ? 0 : (ev[0] == 'r' ? 2 : 1);   // 0: generic kernel only; require: no silent fallback
     make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type, n_drones, G), h->P);
     pick_kernels(h);
     // one arena: 7 drone planes, env plane, gstep, obs, reward, done (each 256 B aligned)
@@ -478,18 +506,24 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
         pick_kernels(h);
         rc = configure_launch(h);
     }
+    if (rc == MDG_OK && h->jit == 2 && !h->jit_note.empty())
+        rc = fail(MDG_ECUDA, "mdg_create: MDG_JIT=require and the run-time specialisation failed: " + h->jit_note);
     if (rc != MDG_OK) { cudaFree(h->arena); if (h->hist) cudaFree(h->hist); delete h; return rc; }
     *out = h;
     rc = mdg_reset(h, 0);
     if (rc != MDG_OK) { mdg_destroy(h); *out = nullptr; return rc; }
+    // a fallback to the 1.7-2.1x slower runtime-flag kernel is not an error, but it is not silent either: the text is
+    // readable through mdg_last_error() right after mdg_create, and mdg_kernel_name() says "generic"
+    if (!h->jit_note.empty()) g_err = "mdg_create: run-time specialisation unavailable, using the generic kernel: " + h->jit_note;
+    else g_err.clear();
     return MDG_OK;
 }
 
-void mdg_release_staging(mdg_env* h);
 void mdg_destroy(mdg_env* h) {
     if (!h) return;
-    mdg_release_staging(h);
     drop_graphs(h);
+    if (h->stage) cudaFree(h->stage);
+    if (h->order_event) cudaEventDestroy(h->order_event);
     if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
     if (h->arena) cudaFree(h->arena);
     if (h->hist) cudaFree(h->hist);
@@ -500,8 +534,7 @@ int mdg_reset(mdg_env* h, uint64_t seed) {
     if (!h) return fail(MDG_EINVAL, "mdg_reset: NULL handle");
     h->P.seed_lo = (uint32_t)seed; h->P.seed_hi = (uint32_t)(seed >> 32);
     drop_graphs(h);                          // captured launches carry the old seed
-    CU(cudaMemsetAsync(h->B.ticket, 0, 2 * sizeof(unsigned), h->stream));
-    h->chainable = false;
+    h->chainable = false;                    // the dispensers are back at 0 after every launch: nothing to clear
     h->reset<<<grid_for(h, 128), 128, 0, h->stream>>>(h->P, h->B);
     CU(cudaGetLastError());
     h->launches += 1;
@@ -511,11 +544,13 @@ int mdg_reset(mdg_env* h, uint64_t seed) {
 int mdg_step(mdg_env* h, const float* actions_dev) {
     if (!h || !actions_dev) return fail(MDG_EINVAL, "mdg_step: NULL argument");
     if ((uintptr_t)actions_dev & 15) return fail(MDG_EINVAL, "mdg_step: actions_dev must be 16-byte aligned");
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;      // a caller-side capture replays baked parameters
-    CU(cudaStreamIsCapturing(h->stream, &cap));
-    const int rc = launch_step(h, actions_dev, h->stream, cap == cudaStreamCaptureStatusNone);
-    if (rc == MDG_OK) h->launches += 1; else h->chainable = false;
-    return rc;
+    return launch_step(h, actions_dev, h->stream, false);
+}
+
+int mdg_step_chained(mdg_env* h, const float* actions_dev) {
+    if (!h || !actions_dev) return fail(MDG_EINVAL, "mdg_step_chained: NULL argument");
+    if ((uintptr_t)actions_dev & 15) return fail(MDG_EINVAL, "mdg_step_chained: actions_dev must be 16-byte aligned");
+    return launch_step(h, actions_dev, h->stream, true);
 }
 
 int mdg_step_many(mdg_env* h, const float* actions_dev, int n_steps, int64_t stride_floats) {
@@ -525,11 +560,16 @@ int mdg_step_many(mdg_env* h, const float* actions_dev, int n_steps, int64_t str
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         if (!h->capture_stream) CU(cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking));
+        const int64_t launches0 = h->launches;
         CU(cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal));
         int rc = MDG_OK;
-        for (int k = 0; k < n_steps && rc == MDG_OK; ++k) rc = launch_step(h, actions_dev + (int64_t)k * stride_floats, h->capture_stream, false);
+        // the first launch waits for whatever precedes the replay and publishes its (baked) sequence number for every item;
+        // the others chain item by item behind their predecessor in the graph, exactly like a stream of mdg_step_chained calls
+        for (int k = 0; k < n_steps && rc == MDG_OK; ++k) rc = launch_step(h, actions_dev + (int64_t)k * stride_floats, h->capture_stream, k > 0);
         cudaGraph_t g = nullptr;
         cudaError_t ce = cudaStreamEndCapture(h->capture_stream, &g);
+        h->launches = launches0;                 // capturing launches nothing
+        h->chainable = false;
         if (rc != MDG_OK) { if (g) cudaGraphDestroy(g); return rc; }
         if (ce != cudaSuccess) return fail(MDG_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce));
         cudaGraphExec_t ge = nullptr;
@@ -539,8 +579,11 @@ int mdg_step_many(mdg_env* h, const float* actions_dev, int n_steps, int64_t str
         if (h->graphs.size() >= 16) drop_graphs(h);
         it = h->graphs.emplace(key, ge).first;
     }
-    CU(cudaGraphLaunch(it->second, h->stream));
-    h->chainable = false;                    // replayed kernels carry baked sequence numbers
+    nvtxRangePushA("mdg_step_many");
+    const cudaError_t ce = cudaGraphLaunch(it->second, h->stream);
+    nvtxRangePop();
+    if (ce != cudaSuccess) return fail(MDG_ECUDA, std::string("cudaGraphLaunch: ") + cudaGetErrorString(ce));
+    h->chainable = false;                    // a step after the replay waits for all of it
     h->launches += n_steps;
     return MDG_OK;
 }
@@ -624,7 +667,20 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
 
 int mdg_set_stream(mdg_env* h, void* s) {
     if (!h) return fail(MDG_EINVAL, "mdg_set_stream: NULL handle");
-    h->stream = (cudaStream_t)s;
+    cudaStream_t ns = (cudaStream_t)s;
+    if (ns != h->stream) {
+        // what is already queued on the old stream (the create-time clear and reset, earlier steps) stays ahead of what follows
+        cudaStreamCaptureStatus c0 = cudaStreamCaptureStatusNone, c1 = cudaStreamCaptureStatusNone;
+        CU(cudaStreamIsCapturing(h->stream, &c0));
+        CU(cudaStreamIsCapturing(ns, &c1));
+        if (c0 == cudaStreamCaptureStatusNone && c1 == cudaStreamCaptureStatusNone) {   // inside a capture the ordering is the caller's graph
+            if (!h->order_event) CU(cudaEventCreateWithFlags(&h->order_event, cudaEventDisableTiming));
+            CU(cudaEventRecord(h->order_event, h->stream));
+            CU(cudaStreamWaitEvent(ns, h->order_event, 0));
+        }
+        h->stream = ns;
+    }
+    h->chainable = false;
     return MDG_OK;
 }
 int64_t mdg_launch_count(const mdg_env* h) { return h ? h->launches : 0; }
@@ -741,7 +797,6 @@ extern "C" int mdg_set_dr(mdg_env* h, const float* f) {
 }
 
 // ---- end-to-end call with host buffers --------------------------------------------------------------
-static std::map<mdg_env*, float*> g_stage;   // device staging buffer for host actions, one per handle
 // ---- full checkpoint: every device buffer a later step reads, as one opaque host blob ---------------------
 namespace {
 struct CkptHeader { uint32_t magic, version; int32_t N, M, feat, opd; uint32_t seed_lo, seed_hi; uint64_t bytes_main, bytes_rd, bytes_hist; };
@@ -793,12 +848,10 @@ extern "C" int mdg_load(mdg_env* h, const void* host_buf, int64_t buf_bytes) {
 extern "C" int mdg_step_host_async(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
     if (!h || !actions_host) return fail(MDG_EINVAL, "mdg_step_host: NULL argument");
     const size_t D = (size_t)h->N * h->M;
-    float*& stage = g_stage[h];
-    if (!stage) CU(cudaMalloc(&stage, D * 4 * sizeof(float)));
-    CU(cudaMemcpyAsync(stage, actions_host, D * 4 * sizeof(float), cudaMemcpyHostToDevice, h->stream));
-    const int rc = launch_step(h, stage, h->stream, true);
+    if (!h->stage) CU(cudaMalloc(&h->stage, D * 4 * sizeof(float)));
+    CU(cudaMemcpyAsync(h->stage, actions_host, D * 4 * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    const int rc = launch_step(h, h->stage, h->stream, false);
     if (rc != MDG_OK) return rc;
-    h->launches += 1;
     if (obs_host) CU(cudaMemcpyAsync(obs_host, h->B.obs, D * h->P.opd * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
     if (reward_host) CU(cudaMemcpyAsync(reward_host, h->B.reward, (size_t)h->N * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
     if (done_host) CU(cudaMemcpyAsync(done_host, h->B.done, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
@@ -813,11 +866,6 @@ extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_h
     const int rc = mdg_step_host_async(h, actions_host, obs_host, reward_host, done_host);
     return rc != MDG_OK ? rc : mdg_wait(h);
 }
-extern "C" void mdg_release_staging(mdg_env* h) {   // called by mdg_destroy
-    auto it = g_stage.find(h);
-    if (it != g_stage.end()) { cudaFree(it->second); g_stage.erase(it); }
-}
-
 // ---- FP32 peak microbenchmark (roofline denominator check) ------------------------------------------
 __global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int iters, float a, float b) {
     float x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
@@ -858,12 +906,3 @@ extern "C" int mdg_measure_fp32_peak(void* cuda_stream, double* tflops) {
     *tflops = 2.0 * 64.0 * iters * (double)blocks * threads / (best_ms * 1e-3) / 1e12;
     return MDG_OK;
 }
-
-#ifdef MDG_TRACE
-extern "C" int mdg_debug_set_trace(void* dev_ptr, unsigned n_items) {
-    unsigned long long* p = (unsigned long long*)dev_ptr;
-    CU(cudaMemcpyToSymbol(mdg::g_trace, &p, sizeof(p)));
-    CU(cudaMemcpyToSymbol(mdg::g_trace_items, &n_items, sizeof(n_items)));
-    return MDG_OK;
-}
-#endif

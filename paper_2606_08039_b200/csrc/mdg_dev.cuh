@@ -34,7 +34,7 @@ struct DevParams {
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
     uint32_t seed_lo, seed_hi, env_base;
     uint32_t static_items;                                // grid does not fill the device: one item per warp, item = warp index (no dispenser)
-    uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining (mdg_kernels.cuh)
+    uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining behind step seq - 1 (mdg_kernels.cuh)
     // integrator
     float h, half_h, h_sixth, half_h2, w2_exact[2];          // w2_exact: |omega|^2 above which the exact path runs
     // Rodrigues coefficients of R(c w)^T as polynomials in y = |w|^2, c = h/2 (stages 2, 3) and h (stage 4):
@@ -42,6 +42,7 @@ struct DevParams {
     // 1e-7 for |w| h <= 0.28 rad and is used where a controller keeps the body rates small (PID / VEL actions);
     // degree 3 holds to 0.75 rad and serves the open-loop action types.  w2_exact[d-2] is the matching |w|^2 bound.
     float rotA_half[4], rotB_half[4], rotA_full[4], rotB_full[4];
+    float rotnA_half[4], rotnA_full[4], ngyro[3];            // -A's coefficients and -gyro: the lane-generic substep loop never negates
     // Eq.7 increment for phi = (h/6) s, s = w0 + 2 w2 + 2 w3 + w4, as polynomials in |s|^2: cos(|phi|/2) and (h/6) sin(|phi|/2)/|phi|
     float expC[4], expS[4];
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
@@ -94,7 +95,7 @@ struct DevBuffers {
     float4* E0;   // wind x y z, bits(ep_step)
     float4* E1;   // running gust impulse: velocity x y z, progress s (>= 1: none)
     uint32_t* gstep;
-    unsigned* ticket;   // two work-item dispensers of the step kernel (0 between launches), used alternately
+    unsigned* ticket;   // [0..1] two work-item dispensers of the step kernel (0 between launches), used alternately; [2..3] their owner stamps
     unsigned* item_seq; // per work item: sequence number of the last step that finished it
     float* obs;
     float* reward;
@@ -223,6 +224,119 @@ __device__ __forceinline__ V3 stage_torque(const float (&cA)[4], const float (&c
     const V3 c2 = cross(w, c1);
     return v3(fmaf(Bc, c2.x, fmaf(-A, c1.x, tau.x)), fmaf(Bc, c2.y, fmaf(-A, c1.y, tau.y)), fmaf(Bc, c2.z, fmaf(-A, c1.z, tau.z)));
 }
+// ---- lane-generic arithmetic of the substep loop ----------------------------------------------------------------------
+// The substep loop is written once over a value type T: float (one drone per thread) or F2, a pair of floats in one 64-bit
+// register holding the same quantity of TWO drones (two envs per lane group).  sm_100 executes fma / mul / add on such pairs
+// as single instructions (FFMA2 / FMUL2 / FADD2: one issue slot, two cycles of the FP32 pipe), which is what an issue-bound
+// kernel needs; everything else (MUFU, min / max, compares, selects, shuffles) works on the halves, which are ordinary
+// registers.  Every operation is spelled out (no operator the compiler could contract differently), so both instantiations
+// round identically: the two-drones-per-thread kernel is bit for bit the one-drone kernel.
+struct F2 { unsigned long long v; };
+__device__ __forceinline__ F2 pk(float lo, float hi) { F2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float lo_(F2 a) { float l, h; asm("mov.b64 {%0, %1}, %2;" : "=f"(l), "=f"(h) : "l"(a.v)); return l; }
+__device__ __forceinline__ float hi_(F2 a) { float l, h; asm("mov.b64 {%0, %1}, %2;" : "=f"(l), "=f"(h) : "l"(a.v)); return h; }
+struct B2 { bool lo, hi; };
+template <class T> struct LaneOps;
+template <> struct LaneOps<float> {
+    typedef bool mask;
+    static __device__ __forceinline__ float bc(float s) { return s; }
+};
+template <> struct LaneOps<F2> {
+    typedef B2 mask;
+    static __device__ __forceinline__ F2 bc(float s) { return pk(s, s); }
+};
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ float mul_(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add_(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub_(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float neg_(float a) { return -a; }
+__device__ __forceinline__ F2 fma_(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
+__device__ __forceinline__ F2 mul_(F2 a, F2 b) { F2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ F2 add_(F2 a, F2 b) { F2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ F2 sub_(F2 a, F2 b) { F2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ F2 neg_(F2 a) { F2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(0xBF800000BF800000ull)); return r; }   // x * -1: exact, one FMUL2
+// uniform (float) operands broadcast to both halves
+__device__ __forceinline__ F2 fma_(float a, F2 b, F2 c) { return fma_(pk(a, a), b, c); }
+__device__ __forceinline__ F2 fma_(F2 a, float b, F2 c) { return fma_(a, pk(b, b), c); }
+__device__ __forceinline__ F2 fma_(F2 a, F2 b, float c) { return fma_(a, b, pk(c, c)); }
+__device__ __forceinline__ F2 fma_(float a, F2 b, float c) { return fma_(pk(a, a), b, pk(c, c)); }
+__device__ __forceinline__ F2 fma_(F2 a, float b, float c) { return fma_(a, pk(b, b), pk(c, c)); }
+__device__ __forceinline__ F2 mul_(float a, F2 b) { return mul_(pk(a, a), b); }
+__device__ __forceinline__ F2 mul_(F2 a, float b) { return mul_(a, pk(b, b)); }
+// per-half operations
+#define MDG_MAP1(name, expr) \
+    __device__ __forceinline__ float name(float x) { return expr; } \
+    __device__ __forceinline__ F2 name(F2 a) { float x = lo_(a); const float l = expr; x = hi_(a); const float h = expr; return pk(l, h); }
+MDG_MAP1(rcp_, rcp_fast(x))
+MDG_MAP1(rsqrt_, rsqrt_fast(x))
+MDG_MAP1(ex2_, ex2_fast(x))
+MDG_MAP1(abs_, fabsf(x))
+MDG_MAP1(sat_, __saturatef(x))
+#undef MDG_MAP1
+__device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ F2 max_(F2 a, float b) { return pk(fmaxf(lo_(a), b), fmaxf(hi_(a), b)); }
+__device__ __forceinline__ bool gt_(float a, float b) { return a > b; }
+__device__ __forceinline__ bool lt_(float a, float b) { return a < b; }
+__device__ __forceinline__ B2 gt_(F2 a, float b) { B2 m; m.lo = lo_(a) > b; m.hi = hi_(a) > b; return m; }
+__device__ __forceinline__ B2 lt_(F2 a, float b) { B2 m; m.lo = lo_(a) < b; m.hi = hi_(a) < b; return m; }
+__device__ __forceinline__ bool and_(bool a, bool b) { return a && b; }
+__device__ __forceinline__ B2 and_(B2 a, bool b) { B2 m; m.lo = a.lo && b; m.hi = a.hi && b; return m; }
+__device__ __forceinline__ float sel_(bool m, float a, float b) { return m ? a : b; }
+__device__ __forceinline__ F2 sel_(B2 m, F2 a, F2 b) { return pk(m.lo ? lo_(a) : lo_(b), m.hi ? hi_(a) : hi_(b)); }
+__device__ __forceinline__ F2 sel_(B2 m, F2 a, float b) { return pk(m.lo ? lo_(a) : b, m.hi ? hi_(a) : b); }
+__device__ __forceinline__ F2 sel_(B2 m, float a, F2 b) { return pk(m.lo ? a : lo_(b), m.hi ? a : hi_(b)); }
+__device__ __forceinline__ float shfl_(float x, int src, int width) { return __shfl_sync(0xffffffffu, x, src, width); }
+__device__ __forceinline__ F2 shfl_(F2 a, int src, int width) { return pk(__shfl_sync(0xffffffffu, lo_(a), src, width), __shfl_sync(0xffffffffu, hi_(a), src, width)); }
+
+template <class T> struct V3T { T x, y, z; };
+template <class T> struct Q4T { T w, x, y, z; };
+template <class T> __device__ __forceinline__ V3T<T> v3t(T x, T y, T z) { V3T<T> r; r.x = x; r.y = y; r.z = z; return r; }
+template <class T> __device__ __forceinline__ V3T<T> neg3(V3T<T> a) { return v3t<T>(neg_(a.x), neg_(a.y), neg_(a.z)); }
+// a x b, given na = -a: each component is one multiply and one fma
+template <class T> __device__ __forceinline__ V3T<T> cross_n(V3T<T> a, V3T<T> na, V3T<T> b) {
+    return v3t<T>(fma_(a.y, b.z, mul_(na.z, b.y)), fma_(a.z, b.x, mul_(na.x, b.z)), fma_(a.x, b.y, mul_(na.y, b.x)));
+}
+template <class T> __device__ __forceinline__ T dot3(V3T<T> a, V3T<T> b) { return fma_(a.x, b.x, fma_(a.y, b.y, mul_(a.z, b.z))); }
+// a (x) b (Hamilton product)
+template <class T> __device__ __forceinline__ Q4T<T> qmul_t(Q4T<T> a, Q4T<T> b) {
+    const T nx = neg_(a.x), ny = neg_(a.y), nz = neg_(a.z);
+    Q4T<T> r;
+    r.w = fma_(nz, b.z, fma_(ny, b.y, fma_(nx, b.x, mul_(a.w, b.w))));
+    r.x = fma_(a.w, b.x, fma_(b.w, a.x, fma_(a.y, b.z, mul_(nz, b.y))));
+    r.y = fma_(a.w, b.y, fma_(b.w, a.y, fma_(a.z, b.x, mul_(nx, b.z))));
+    r.z = fma_(a.w, b.z, fma_(b.w, a.z, fma_(a.x, b.y, mul_(ny, b.x))));
+    return r;
+}
+// polynomial c0 + y (c1 + y (c2 [+ y c3])) with uniform coefficients
+template <int DEG, class T> __device__ __forceinline__ T poly_(const float (&c)[4], T y) {
+    return DEG == 2 ? fma_(y, fma_(y, c[2], c[1]), c[0]) : fma_(y, fma_(y, fma_(y, c[3], c[2]), c[1]), c[0]);
+}
+// Eq.7 increment [cos(|phi|/2), sin(|phi|/2) phi/|phi|] for phi = c s with c folded into host-made coefficients (DevParams::expC, expS)
+template <int DEG, class T> __device__ __forceinline__ Q4T<T> exp_half_scaled_t(const float (&cC)[4], const float (&cS)[4], V3T<T> s) {
+    const T y = dot3(s, s);
+    const T f = poly_<DEG>(cS, y);
+    Q4T<T> r; r.w = poly_<DEG>(cC, y); r.x = mul_(f, s.x); r.y = mul_(f, s.y); r.z = mul_(f, s.z);
+    return r;
+}
+// the same increment for an explicit rotation vector phi (degree 3, |phi| <= 0.75 rad): the DYN integrator's update
+template <class T> __device__ __forceinline__ Q4T<T> exp_half_t(V3T<T> phi) {
+    const T x = dot3(phi, phi);
+    const T c = fma_(x, fma_(x, fma_(x, -2.1701389e-5f, 2.6041667e-3f), -0.125f), 1.0f);
+    const T f = fma_(x, fma_(x, fma_(x, -1.5500992e-6f, 2.6041667e-4f), -2.0833333e-2f), 0.5f);
+    Q4T<T> r; r.w = c; r.x = mul_(f, phi.x); r.y = mul_(f, phi.y); r.z = mul_(f, phi.z);
+    return r;
+}
+// R(c w)^T tau for the rotation vector phi = c w (Rodrigues): tau - A(y) (w x tau) + B(y) w x (w x tau), y = |w|^2, the step
+// factor c folded into the host-made coefficients; cnA holds -A's coefficients so that no negation is needed
+template <int DEG, class T> __device__ __forceinline__ V3T<T> stage_torque_t(const float (&cnA)[4], const float (&cB)[4], V3T<T> w, V3T<T> tau) {
+    const T y = dot3(w, w);
+    const T nA = poly_<DEG>(cnA, y), Bc = poly_<DEG>(cB, y);
+    const V3T<T> nw = neg3(w);
+    const V3T<T> c1 = cross_n(w, nw, tau);
+    const V3T<T> c2 = cross_n(w, nw, c1);
+    return v3t<T>(fma_(Bc, c2.x, fma_(nA, c1.x, tau.x)), fma_(Bc, c2.y, fma_(nA, c1.y, tau.y)), fma_(Bc, c2.z, fma_(nA, c1.z, tau.z)));
+}
+
 // sqrt(x) for x >= 0: one MUFU.SQRT (sqrt.approx.ftz, 1 ulp; sqrt(0) = 0)
 __device__ __forceinline__ float fast_sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float clampf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }

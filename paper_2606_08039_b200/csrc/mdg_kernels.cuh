@@ -95,21 +95,6 @@ __device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffe
     cp_async_commit();
 }
 
-#ifdef MDG_TRACE   // development builds only (_work/): per-item clock64 stamps, never compiled into libmdg.so
-__device__ unsigned long long* g_trace = nullptr;
-__device__ unsigned g_trace_items = 0;
-__device__ __forceinline__ void trace_stamp(unsigned wt, int k, int lane, unsigned seq) {
-    if (lane == 0 && g_trace) {
-        unsigned long long* r = g_trace + ((size_t)(seq & 3u) * g_trace_items + wt) * 10;
-        r[k] = clock64();
-        if (k == 0 || k == 5) { unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt)); r[k == 0 ? 6 : 8] = gt; }
-        if (k == 0) { unsigned sm; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); r[7] = sm | ((unsigned long long)(threadIdx.x >> 5) << 32); r[9] = seq; }
-    }
-}
-#define MDG_T(k) trace_stamp(wt, k, lane, P.seq)
-#else
-#define MDG_T(k)
-#endif
 
 // One control step of every env.  Persistent warps: each loops over work items of
 // 32 / G envs; lane -> (env e, lane-in-group j).  While an item is integrated, the next item's state planes,
@@ -133,27 +118,33 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const int jj = (full_group || j < P.M) ? j : P.M - 1;
     const bool pid = F::act(P) == 1 || F::act(P) == 2 || F::act(P) == 5;   // actions with an attitude loop (I_eta in P4)
     // Programmatic dependent launch.  P.chain == 0: wait here until the previous kernel of the stream has completed
-    // and its writes are visible (nothing above touches memory).  P.chain == 1 (the previous operation on this
-    // handle was step number P.seq - 1, launched on the same stream): no grid-wide wait at all; the dependency is
-    // per work item instead - item i may start as soon as the previous step has published item i (item_seq[i] ==
-    // P.seq - 1, release/acquire), so the drain of one step overlaps the ramp-up of the next.  Deadlock-free:
-    // this grid only starts once every block of the previous grid is resident (or done), and nothing here is waited on
-    // by that grid.
+    // and its writes are visible (nothing above touches memory).  P.chain == 1 (mdg_step_chained / the inner launches of
+    // mdg_step_many: the previous operation on this handle was step number P.seq - 1, launched on the same stream or in the
+    // same capture, and the caller guarantees that the actions were complete before that step was enqueued): no grid-wide
+    // wait at all; the dependency is per work item instead - item i may start as soon as the previous step has published
+    // item i (item_seq[i] == P.seq - 1, release/acquire), so the drain of one step overlaps the ramp-up of the next.
+    // Deadlock-free: this grid only starts once every block of the previous grid is resident (or done), and nothing here
+    // is waited on by that grid.  Sequence numbers are kernel parameters: in a replayed CUDA graph the first launch has
+    // chain == 0 and publishes its (baked) number for every item, so the second finds what it expects in every replay.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const uint32_t seq = P.seq;
     const bool chain = P.chain != 0;
     if (!chain) asm volatile("griddepcontrol.wait;" ::: "memory");
-    // Work items are handed out by an atomic ticket (self-resetting: atomicInc wraps to 0 after the n_items + tw
-    // grabs of one launch; two dispensers alternate so that chained launches never share one), so SMs that run
-    // faster or host fewer long warps simply take more items.
-    const unsigned wrap = n_items + tw - 1u;
-    unsigned* const dispenser = B.ticket + (P.seq & 1u);
+    // Every warp starts on the item of its own index (known without a memory round trip: the blocks of a launch start
+    // within a microsecond of each other, whatever they wait for first is paid by all of them); the others are handed out
+    // by an atomic ticket (item = tw + ticket; self-resetting: atomicInc wraps to 0 after the n_items grabs of one launch -
+    // n_items - tw items and one miss per warp; two dispensers alternate so that chained launches never share one), so SMs
+    // that run faster or host fewer long warps simply take more items.
+    const unsigned wrap = n_items - 1u;
+    unsigned* const dispenser = B.ticket + (seq & 1u);
     // Everything with a long latency on the per-item path is issued one item early and consumed late: the ticket
     // of item n+2 is drawn (lane 0, atomic) when item n starts and read after its substeps; the "previous step
     // has published this item" flag of item n+2 is then probed (ld.acquire) and only re-polled at the prefetch
     // of item n+2 if that probe came too early; an item's own flag is published (fence + st.release) just before
     // the NEXT item's stores, when its stores have long been acknowledged.
-    const unsigned want = P.seq - 1u;
-    auto draw = [&](bool go) { unsigned v = 0xFFFFFFFFu; if (lane == 0 && go) v = atomicInc(dispenser, wrap); return v; };   // lane 0 holds it
+    const unsigned want = seq - 1u;
+    auto draw = [&](bool go) { unsigned v = 0xFFFFFFFFu; if (lane == 0 && go) v = tw + atomicInc(dispenser, wrap); return v; };   // lane 0 holds it
+    auto take = [&](unsigned drawn_l0) { return __shfl_sync(MDG_FULL, drawn_l0, 0); };
     auto probe = [&](unsigned item_l0) {                        // lane 0: one acquire load of the item's flag
         unsigned got = want;
         if (chain && lane == 0 && item_l0 < n_items) asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(got) : "l"(B.item_seq + item_l0) : "memory");
@@ -177,14 +168,14 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     // arithmetic hides the fence's round trip to L2) + a relaxed store of the sequence number (after them)
     auto publish_flag = [&](unsigned item) {
         __syncwarp();
-        if (lane == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(B.item_seq + item), "r"(P.seq) : "memory");
+        if (lane == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(B.item_seq + item), "r"(seq) : "memory");
     };
-    // Grids that do not fill the device hold one warp per item: the item is the warp's index and no ticket is drawn, so
-    // any number of such launches may be in flight at once (each item still waits for its predecessor's flag).
+    // Grids that do not fill the device hold one warp per item: no ticket is drawn at all, so any number of such launches
+    // may be in flight at once (each item still waits for its predecessor's flag).
     const bool static_items = P.static_items != 0;
-    unsigned wt = static_items ? blockIdx.x * wpb + wib : __shfl_sync(MDG_FULL, draw(true), 0);
-    if (wt >= n_items) return;
-    unsigned wt_next = static_items ? 0xFFFFFFFFu : __shfl_sync(MDG_FULL, draw(true), 0);   // a warp stops drawing after its first miss
+    unsigned wt = blockIdx.x * wpb + wib;
+    if (wt >= n_items) return;                                    // only in grids that do not fill the device (static_items)
+    unsigned wt_next = static_items ? 0xFFFFFFFFu : take(draw(true));   // a warp stops drawing after its first miss
     unsigned probed_next = probe(wt_next);
     await_item(wt, probe(wt));
     prefetch_item<G>(P, B, actions, S[wib], wt, lane, jj, F::act(P));
@@ -201,7 +192,6 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const bool active = env_ok && (full_group || j < P.M);
     const size_t drone = (size_t)e * P.M + jj;
 
-    MDG_T(0);
     cp_async_wait_all();
     const WarpStage& W = S[st * wpb + wib];
     DroneRegs d;
@@ -222,7 +212,6 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     float4 dr0 = make_float4(1, 1, 1, 1), dr1 = dr0, dr2 = dr0, dr3 = dr0;   // this episode's DR factors (read-mostly, plain loads)
     if (F::has(P, F_DR)) { dr0 = B.R0[drone]; dr1 = B.R1[drone]; dr2 = B.R2[drone]; dr3 = B.R3[drone]; }
     if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch_item<G>(P, B, actions, S[(st ^ 1) * wpb + wib], wt_next, lane, jj, F::act(P)); }
-    MDG_T(1);
 
     // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
     // Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact in
@@ -350,7 +339,6 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     bool hit = false;
     const bool flush = pending2 != 0xFFFFFFFFu;                  // two items wait: fence now, flags after the substeps
     if (flush) __threadfence();
-    MDG_T(2);
     Sensed snap = sensed(d, v3(0, 0, 0));                          // sensor latency of a whole step: the state the step starts from
 #pragma unroll 1
     for (int k = 0; k < P.K; ++k) {
@@ -433,9 +421,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         if (F::has(P, F_LAT) && k + 1 == P.K - d_obs) snap = sensed(d, v3(0, 0, 0));   // what the sensors report d_obs substeps later
     }
 
-    MDG_T(3);
     if (flush) { publish_flag(pending); publish_flag(pending2); pending = pending2 = 0xFFFFFFFFu; }
-    const unsigned wt_after = __shfl_sync(MDG_FULL, drawn_l0, 0);
+    const unsigned wt_after = take(drawn_l0);
     const unsigned probed_after = probe(wt_after);
     // S9-S11 epilogue on the end-of-step state
     const int gbase = lane & ~(G - 1);
@@ -548,7 +535,6 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             for (int kk = 0; kk < G; ++kk) adj[kk] = do_reset ? adj_new[kk] : adj[kk];
         }
     }
-    MDG_T(4);
     if (active) {
         store_state(B, drone, d);
         if (pid) {
@@ -568,7 +554,6 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             if (F::has(P, F_WIND_MIX) && (P.wind_mask & 4) && F::has(P, F_WIND)) B.E1[e] = do_reset ? make_float4(0, 0, 0, 1.0f) : gust_out;
         }
     }
-    MDG_T(5);
     if (pending == 0xFFFFFFFFu) pending = wt; else pending2 = wt;
     if (wt_next >= n_items) break;
     wt = wt_next; wt_next = wt_after; probed_next = probed_after; st ^= 1;

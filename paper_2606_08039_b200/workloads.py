@@ -75,6 +75,22 @@ def config(c: int) -> Workload:
     raise ValueError(c)
 
 
+# Secondary workloads on a config (bench.py --variant, tests/test_gpu_features.py): parameter overrides, data only.
+#  dyn     Table 1's DYN integrator (SURVEY.md 8(f) NEXT-1 "DYN mode benchmarked")
+#  noise   Table 4's sensor-noise rows alone (a feature word without a precompiled kernel instance)
+#  table4  every row of Table 4 except the initial-velocity range: per-episode DR planes, initial attitude,
+#          motor lag, action / sensor latency, sensor noise.  The +-0.5 m/s initial velocities are left out on config 5 because
+#          at its 0.3 m formation they send drones through each other's downwash column, where Eq.6 amplifies rounding by
+#          orders of magnitude (conditioning); the generic-kernel cases of the tests cover that row.
+VARIANTS = {
+    "dyn": dict(integrator=INTEG_EULER),
+    "noise": dict(obs_noise=[0.01, 0.05, 0.0174533, 0.05]),
+    "table4": dict(dr_alpha=[0.2, 0.2, 0.15, 0.15, 0.3, 0.3, 0.3, 0.02, 0.05, 0.02, 0.05, 0.0], reset_rpy_half=[0.1, 0.1, 0.1],
+                   motor_lag_lo=0.005, motor_lag_hi=0.05, act_latency_lo=0.0, act_latency_hi=0.05,
+                   obs_latency_lo=0.0, obs_latency_hi=0.02, obs_noise=[0.01, 0.05, 0.0174533, 0.05]),
+}
+
+
 def hover_rpm_f32(m=0.027, g=9.81, k_f=3.16e-10):
     """Harness scale for ("hover_scale", ...) actions: the CF2X hover rotor speed rounded to fp32."""
     import struct

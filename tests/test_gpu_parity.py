@@ -13,8 +13,8 @@ pytestmark = pytest.mark.gpu
 
 @pytest.mark.parametrize("c", [1, 2, 3, 4])
 def test_config_parity_full_size(c):
-    # c4: close downwash passes are chaotic (parity_util "Conditioning"); measured 13 of 1,024 envs
-    res = run_parity(W.config(c), steps=48, max_ill_frac=0.05 if c == 4 else 0.0)
+    # c4: close downwash passes are chaotic (parity_util "Conditioning"); measured 13 of 1,024 envs on the fixed seed, cap = 2 x that
+    res = run_parity(W.config(c), steps=48, max_ill_frac=26 / 1024 if c == 4 else 0.0)
     print(c, res)
     assert "generic" not in res["kernel"]
 
@@ -35,7 +35,7 @@ def test_config5_parity_full_size():
 def test_config_parity_with_frequent_episodes(c):
     """Short episodes + crashes: exercises truncation, termination and same-call auto-reset every few steps."""
     wl = W.config(c).scaled(min(W.config(c).n_envs, 1500))
-    res = run_parity(wl, steps=40, extra=dict(episode_len_s=7 / 48, z_max=1.3), max_ill_frac=0.05 if c == 4 else 0.0)
+    res = run_parity(wl, steps=40, extra=dict(episode_len_s=7 / 48, z_max=1.3), max_ill_frac=0.0)   # measured: no ill-conditioned env in any config
     print(c, res)
     assert res["n_done"] > wl.n_envs
 
@@ -45,9 +45,14 @@ def test_config_parity_with_divergent_resets(c, extra):
     """Envs that terminate one by one at different steps: neighbouring envs of one warp take the auto-reset path at
     different times (the truncation test above resets whole warps at once)."""
     wl = W.config(c).scaled(min(W.config(c).n_envs, 2051))
-    res = run_parity(wl, steps=48, extra=extra, max_ill_frac=0.05 if c == 4 else 0.0)
+    res = run_parity(wl, steps=48, extra=extra, max_ill_frac=10 / 1024 if c == 4 else 0.0)      # c4: measured 5 of 1,024, cap = 2 x that
     print(c, res)
     assert res["n_done"] > wl.n_envs // 8
+
+
+# Measured with the oracle alone on the fixed seeds (the exclusion depends on nothing else): c4 13 ill-conditioned + 200 envs that
+# came within 1e-4 of a threshold (mostly floor contacts), 210 distinct; c3 and c5: none.  Cap = 2 x ill + near-threshold.
+MAX_EXCLUDED = {5: 0, 4: 226, 3: 0}
 
 
 @pytest.mark.parametrize("c,n_envs", [(5, 65536), (4, 1024), (3, 16384)])
@@ -57,7 +62,7 @@ def test_back_to_back_steps_without_host_sync(c, n_envs):
     the last outputs and the episode counters must match the oracle as in the step-by-step tests."""
     import torch
     from oracle import oracle as O
-    from parity_util import make_pair, compare_state, shadow_drift, TOL_R
+    from parity_util import make_pair, compare_state, shadow_drift, reward_err
     wl = W.config(c).scaled(n_envs)
     orc, gpu = make_pair(wl)
     shadow = O.OracleEnv(wl.n_envs, wl.n_drones, wl.physics_mode, wl.action_type, O.OracleParams(0, **wl.params), n_threads=os.cpu_count() or 1)
@@ -72,8 +77,8 @@ def test_back_to_back_steps_without_host_sync(c, n_envs):
         acts = [O.gen_actions(wl.seed, t, wl.n_envs, wl.n_drones, base, wl.actions[1], wl.actions[2]) for t in range(steps)]
         dev = [gpu.gen_actions(wl.seed, t, base, wl.actions[1], wl.actions[2]) for t in range(steps)]
     torch.cuda.synchronize()
-    for t in range(steps):                       # nothing but launches
-        gpu.step(dev[t])
+    for t in range(steps):                       # nothing but launches; the actions were all there before the first one
+        gpu.step_chained(dev[t])
     ill = np.zeros(wl.n_envs, dtype=bool)
     differ = np.zeros(wl.n_envs, dtype=bool)     # envs whose done history may legitimately differ (threshold ties)
     for t in range(steps):
@@ -86,14 +91,18 @@ def test_back_to_back_steps_without_host_sync(c, n_envs):
         differ |= orc.outputs()[3][:, 0] < 1e-4
     torch.cuda.synchronize()
     alive = ~ill & ~differ
-    assert alive.mean() > (0.7 if c == 4 else 0.995)      # c4: ill-conditioned downwash passes + near-threshold envs
+    # envs left out: ill-conditioned downwash passes (shadow oracle, c4 only) + envs that came within 1e-4 of a termination threshold
+    # at any of the 48 steps (their done history may legitimately differ).
+    print(c, "excluded", int((~alive).sum()), "of", wl.n_envs, "ill", int(ill.sum()), "near-threshold", int(differ.sum()))
+    assert (~alive).sum() <= MAX_EXCLUDED[c], (int(ill.sum()), int(differ.sum()))
     res, g = compare_state(orc, gpu, alive, wl.n_drones, "after 48 queued steps")
     print(c, res, int((~alive).sum()))
     assert np.array_equal(g["ep_step"][alive], orc.ep_step[alive])
     _, r64, d64, _ = orc.outputs()
     assert np.array_equal(gpu.done.cpu().numpy()[alive], d64[alive])
-    rerr = np.abs(gpu.reward.cpu().numpy() - r64) / np.maximum(1.0, np.abs(r64))
-    assert (rerr[alive] <= TOL_R).mean() > 0.999
+    rerr = reward_err(gpu.reward.cpu().numpy().astype(np.float64), r64)
+    margin = orc.outputs()[3]
+    assert (rerr[alive & (margin[:, 1] >= 1e-4)] <= 1.0).all(), rerr[alive].max()      # every reward, at-target threshold ties aside
 
 
 def test_interleaved_handles_and_host_step_are_bitwise_the_plain_sequence():
@@ -113,7 +122,7 @@ def test_interleaved_handles_and_host_step_are_bitwise_the_plain_sequence():
     torch.cuda.synchronize()
     for t in range(24):
         for k in range(3):
-            fast[k].step(acts[k][t])
+            fast[k].step_chained(acts[k][t])
     for t in range(24):
         for k in range(3):
             slow[k].step(acts[k][t])
