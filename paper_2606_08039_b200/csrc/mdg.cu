@@ -48,6 +48,8 @@ struct mdg_env {
     std::string kernel_name;
     int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
     int pdl = 1;
+    int lanes = 1;                       // envs per lane group in the step kernel: 2 = packed FP32 pairs (grids that fill the device; MDG_LANES=1|2 forces)
+    int stages = 1;                      // shared-memory landing zones per warp (MDG_STAGES=1|2)
     int jit = 1;                         // MDG_JIT=0: never compile at run time, use the generic kernel; MDG_JIT=require: fail instead of falling back
     std::string jit_note;                // why the run-time specialisation was not possible (empty: it was, or was not needed)
     bool saturating = false;             // the step grid occupies every resident block slot of the device
@@ -202,14 +204,20 @@ static constexpr int FEAT_C3 = FEATW(0, 0, 1, 1, 0, 1, 2);
 static constexpr int FEAT_C4 = FEATW(7, 0, 0, 0, 0, 2, 1);
 static constexpr int FEAT_C5 = FEATW(15, 0, 2, 0, 1, 3, 3) | F_TGT_CIRCLE;
 
-// register budget variants of one specialisation: MINB resident 128-thread blocks per SM
-template <int G, int FEAT> static step_fn pick_minb(int minb) {
+// Feature words whose substep loop can run two envs per lane as packed FP32 pairs (mdg_kernels.cuh): a compile-time word
+// without rotor commands that change inside the step (motor lag, latency rows).
+static constexpr bool lanes2_capable(int feat) { return feat >= 0 && !(feat & (F_MLAG | F_LAT)); }
+// register budget variants of one specialisation: MINB resident 128-thread blocks per SM; lanes = envs per lane group (1 or 2)
+template <int G, int FEAT> static step_fn pick_minb(int minb, int lanes) {
+    if constexpr (lanes2_capable(FEAT)) {
+        if (lanes == 2) return minb >= 4 ? step_kernel<G, FEAT, 4, 2> : step_kernel<G, FEAT, 3, 2>;
+    }
     switch (minb) {
-        case 5: return step_kernel<G, FEAT, 5>;
-        case 6: return step_kernel<G, FEAT, 6>;
-        case 7: return step_kernel<G, FEAT, 7>;
-        case 8: return step_kernel<G, FEAT, 8>;
-        default: return step_kernel<G, FEAT, 4>;
+        case 5: return step_kernel<G, FEAT, 5, 1>;
+        case 6: return step_kernel<G, FEAT, 6, 1>;
+        case 7: return step_kernel<G, FEAT, 7, 1>;
+        case 8: return step_kernel<G, FEAT, 8, 1>;
+        default: return step_kernel<G, FEAT, 4, 1>;
     }
 }
 
@@ -218,11 +226,11 @@ template <int G, int FEAT> static step_fn pick_minb(int minb) {
 // (DESIGN.md 6).  Instead, step_kernel<G, FEAT, MINB> is compiled for exactly this word (about a second, cached per process);
 // the sources are the .cuh files beside the library.  Any failure falls back to the generic kernel.  MDG_JIT=0 disables it.
 extern "C" int mdg_version(void);
-static std::map<std::tuple<int, int, int>, std::pair<step_fn, std::string>> g_jit;   // kernel or, on failure, why
+static std::map<std::tuple<int, int, int, int>, std::pair<step_fn, std::string>> g_jit;   // kernel or, on failure, why
 static std::mutex g_jit_mutex;                                   // distinct handles may be created from different threads
-static step_fn jit_step_kernel(int G, int feat, int minb, std::string& why) {
+static step_fn jit_step_kernel(int G, int feat, int minb, int lanes, std::string& why) {
     std::lock_guard<std::mutex> guard(g_jit_mutex);
-    const auto key = std::make_tuple(G, feat, minb);
+    const auto key = std::make_tuple(G, feat, minb, lanes);
     auto it = g_jit.find(key);
     if (it != g_jit.end()) { why = it->second.second; return it->second.first; }   // a failed attempt is not repeated
     step_fn result = nullptr;
@@ -240,7 +248,7 @@ static step_fn jit_step_kernel(int G, int feat, int minb, std::string& why) {
                               "#pragma once\n"};
     nvrtcProgram prog = nullptr;
     if (nvrtcCreateProgram(&prog, src.c_str(), "mdg_jit.cu", 2, hdr_src, hdr_names) != NVRTC_SUCCESS) return done("nvrtcCreateProgram failed");
-    const std::string expr = "mdg::step_kernel<" + std::to_string(G) + ", " + std::to_string(feat) + ", " + std::to_string(minb) + ">";
+    const std::string expr = "mdg::step_kernel<" + std::to_string(G) + ", " + std::to_string(feat) + ", " + std::to_string(minb) + ", " + std::to_string(lanes) + ">";
     const std::string inc = "-I" + dir;
     const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", inc.c_str()};
     std::vector<char> cubin;
@@ -272,7 +280,9 @@ static step_fn jit_step_kernel(int G, int feat, int minb, std::string& why) {
 static void pick_kernels(mdg_env* h) {
     const int f = h->P.feat;
     h->step = nullptr;
-#define SPECIAL(g, fw, name) if (h->G == (g) && f == (fw)) { h->step = pick_minb<(g), (fw)>(h->minb); h->kernel_name = name; }
+    if (h->lanes == 2 && !lanes2_capable(f)) h->lanes = 1;
+    const int mb2 = h->minb >= 4 ? 4 : 3;                            // two envs per lane: 128 or 168 registers
+#define SPECIAL(g, fw, name) if (h->G == (g) && f == (fw)) { h->step = pick_minb<(g), (fw)>(h->minb, h->lanes); h->kernel_name = name; }
     SPECIAL(1, FEAT_C1, "step_kernel<G=1,rigid,rpm,hover>")
     SPECIAL(1, FEATW(0, 0, 3, 0, 0, 0, 1), "step_kernel<G=1,rigid,rpm_norm,hover>")   // the paper's own MJX workload
     SPECIAL(1, FEAT_C2, "step_kernel<G=1,gnd+drag,rpm,hover>")
@@ -284,11 +294,13 @@ static void pick_kernels(mdg_env* h) {
 #undef SPECIAL
     h->jit_note.clear();
     if (!h->step && h->jit) {                                        // no precompiled specialisation: instantiate this word now
-        const int mb = h->minb < 4 ? 4 : (h->minb > 8 ? 8 : h->minb);
-        h->step = jit_step_kernel(h->G, f, mb, h->jit_note);
+        const int mb = h->lanes == 2 ? mb2 : (h->minb < 4 ? 4 : (h->minb > 8 ? 8 : h->minb));
+        h->step = jit_step_kernel(h->G, f, mb, h->lanes, h->jit_note);
         if (h->step) h->kernel_name = "step_kernel<G=" + std::to_string(h->G) + ",jit:" + std::to_string(f) + ">";
     }
-#define GENERIC(g) case g: if (!h->step) { h->step = h->minb <= 3 ? step_kernel<g, -1, 3> : step_kernel<g, -1, 4>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
+    if (!h->step) h->lanes = 1;                                      // the runtime-flag kernel: one env per lane
+    if (h->step && h->lanes == 2) h->kernel_name.insert(h->kernel_name.size() - 1, ",x2");   // two envs per lane, packed FP32 pairs
+#define GENERIC(g) case g: if (!h->step) { h->step = h->minb <= 3 ? step_kernel<g, -1, 3, 1> : step_kernel<g, -1, 4, 1>; h->kernel_name = "step_kernel<G=" #g ",generic>"; } \
                    h->reset = reset_kernel<g>; h->refresh = refresh_obs_kernel<g>; break;
     switch (h->G) { GENERIC(1) GENERIC(2) GENERIC(4) GENERIC(8) GENERIC(16) GENERIC(32) }
 #undef GENERIC
@@ -296,7 +308,8 @@ static void pick_kernels(mdg_env* h) {
 
 // ---- helpers --------------------------------------------------------------------------------------
 static int configure_launch(mdg_env* h) {
-    const int stage_bytes = 2 * (h->block / 32) * (int)sizeof(WarpStage);   // two landing zones per warp
+    h->P.n_stages = (uint32_t)h->stages; h->P.zero = 0u;
+    const int stage_bytes = h->stages * (h->block / 32) * h->lanes * (int)sizeof(WarpStage);   // landing zones per warp and env slot
     h->smem = stage_bytes;
     if (h->max_blocks_per_sm > 0) {          // cap residency by padding the dynamic shared-memory request
         int s = (228 * 1024) / h->max_blocks_per_sm - 1024;
@@ -312,7 +325,7 @@ static int configure_launch(mdg_env* h) {
     int resident = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void*)h->step, h->block, h->smem));
     if (resident < 1) return fail(MDG_ECUDA, "configure_launch: the step kernel does not fit on an SM");
-    const long long epw = 32 / h->G, wpb = h->block / 32;           // envs per work item (one warp), warps per block
+    const long long epw = (long long)h->lanes * (32 / h->G), wpb = h->block / 32;   // envs per work item (one warp), warps per block
     const long long items = ((long long)h->N + epw - 1) / epw, blocks = (items + wpb - 1) / wpb;
     const long long slots = (long long)h->n_sms * resident;
     h->step_grid = (int)(blocks < slots ? blocks : slots);
@@ -461,6 +474,7 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     int G = 1; while (G < n_drones) G <<= 1;
     h->G = G;
     if (const char* ev = std::getenv("MDG_PDL")) h->pdl = ev[0] != '0';
+    if (const char* ev = std::getenv("MDG_STAGES")) h->stages = ev[0] == '1' ? 1 : 2;
     if (const char* ev = std::getenv("MDG_JIT")) h->jit = ev[0] == '0' ? 0 : (ev[0] == 'r' ? 2 : 1);   // 0: generic kernel only; require: no silent fallback
     make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type, n_drones, G), h->P);
     pick_kernels(h);
@@ -500,11 +514,28 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     int rc = configure_launch(h);
     if (rc == MDG_OK && h->saturating) {     // throughput-bound batch: register budget (resident 128-thread blocks per SM) as measured fastest
         const bool generic = h->kernel_name.find("generic") != std::string::npos;
-        // 5 for the benchmark specialisations (96 registers); 6 for the lighter DYN integrator; 4 where Table 4's planes and draws
-        // would spill at 96; the runtime-flag kernel needs 162 registers to stay out of local memory (3)
-        h->minb = generic ? 3 : (h->P.feat & (F_DR | F_MLAG | F_LAT | F_SENS)) ? 4 : (h->P.feat & F_EULER) ? 6 : 5;   // jit kernels follow the same rule
+        // 6 for the benchmark specialisations (80 registers: only the integrated state and the frozen wrench live across the substep
+        // loop); 4 where Table 4's planes and draws would spill; the runtime-flag kernel needs 162 registers to stay out of local memory (3)
+        h->minb = generic ? 3 : (h->P.feat & (F_DR | F_MLAG | F_LAT | F_SENS)) ? 4 : 6;   // jit kernels follow the same rule
         pick_kernels(h);
         rc = configure_launch(h);
+    }
+    // Two envs per lane (packed FP32 pairs in the substep loop) when the grid still fills the device with half the warps:
+    // an issue-bound kernel gains from the halved instruction count, a latency-bound one would only lose parallelism.
+    int want_lanes = 0;
+    if (const char* ev = std::getenv("MDG_LANES")) want_lanes = ev[0] == '2' ? 2 : 1;
+    if (rc == MDG_OK && want_lanes != 1 && lanes2_capable(h->P.feat) && (h->saturating || want_lanes == 2) &&
+        h->kernel_name.find("generic") == std::string::npos) {
+        const int minb1 = h->minb;
+        h->lanes = 2; h->minb = 4;
+        if (const char* ev = std::getenv("MDG_X2_MINB")) h->minb = std::atoi(ev) >= 4 ? 4 : 3;   // 128 instead of 168 registers
+        pick_kernels(h);
+        rc = configure_launch(h);
+        if (rc != MDG_OK || h->lanes != 2 || (!h->saturating && want_lanes != 2)) {
+            h->lanes = 1; h->minb = minb1;
+            pick_kernels(h);
+            rc = configure_launch(h);
+        }
     }
     if (rc == MDG_OK && h->jit == 2 && !h->jit_note.empty())
         rc = fail(MDG_ECUDA, "mdg_create: MDG_JIT=require and the run-time specialisation failed: " + h->jit_note);

@@ -34,6 +34,7 @@ struct DevParams {
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
     uint32_t seed_lo, seed_hi, env_base;
     uint32_t static_items;                                // grid does not fill the device: one item per warp, item = warp index (no dispenser)
+    uint32_t n_stages, zero;                              // shared-memory landing zones per warp (1 or 2); zero: always 0, unknown to the compiler
     uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining behind step seq - 1 (mdg_kernels.cuh)
     // integrator
     float h, half_h, h_sixth, half_h2, w2_exact[2];          // w2_exact: |omega|^2 above which the exact path runs
@@ -269,7 +270,7 @@ __device__ __forceinline__ F2 mul_(F2 a, float b) { return mul_(a, pk(b, b)); }
     __device__ __forceinline__ F2 name(F2 a) { float x = lo_(a); const float l = expr; x = hi_(a); const float h = expr; return pk(l, h); }
 MDG_MAP1(rcp_, rcp_fast(x))
 MDG_MAP1(rsqrt_, rsqrt_fast(x))
-MDG_MAP1(ex2_, ex2_fast(x))
+MDG_MAP1(ex2n_, ex2_fast(-x))
 MDG_MAP1(abs_, fabsf(x))
 MDG_MAP1(sat_, __saturatef(x))
 #undef MDG_MAP1

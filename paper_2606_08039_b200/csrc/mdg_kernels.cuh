@@ -75,12 +75,14 @@ __device__ __forceinline__ void cp_async4(void* dst, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// Start the asynchronous copies of this lane's slots of work item `wt` (global -> shared, no registers held).
+// Start the asynchronous copies of this lane's slots of lane-group row `wt` (32 / G envs; global -> shared, no registers held).
+// dep: a zero the hardware cannot know to be zero, derived from the registers last read from S (single-stage staging: the
+// copies may overwrite S only once those reads have returned - a register dependency the address generation must wait for).
 template <int G>
 __device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffers& B, const float4* actions, WarpStage& S,
-                                              unsigned wt, int lane, int jj, int act) {
+                                              unsigned wt, int lane, int jj, int act, unsigned dep) {
     const unsigned e_raw = wt * (32u / G) + (unsigned)lane / G;
-    const unsigned e = e_raw < (unsigned)P.N ? e_raw : (unsigned)P.N - 1;
+    const unsigned e = (e_raw < (unsigned)P.N ? e_raw : (unsigned)P.N - 1) + dep;
     const size_t drone = (size_t)e * P.M + jj;
     cp_async16(&S.plane[0][lane], B.P0 + drone);
     cp_async16(&S.plane[1][lane], B.P1 + drone);
@@ -92,27 +94,227 @@ __device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffe
     cp_async16(&S.plane[7][lane], actions + drone);
     cp_async16(&S.plane[8][lane], B.E0 + e);
     cp_async4(&S.gstep[lane], B.gstep + e);
-    cp_async_commit();
 }
 
 
+// ---- lane-generic rotation update and substep ---------------------------------------------------------------------------
+template <int N> struct NPTag {};
+template <int NP> struct Lanes;
+template <> struct Lanes<1> { typedef float T; };
+template <> struct Lanes<2> { typedef F2 T; };
+__device__ __forceinline__ float pack_lanes(NPTag<1>, float a, float) { return a; }
+__device__ __forceinline__ F2 pack_lanes(NPTag<2>, float a, float b) { return pk(a, b); }
+__device__ __forceinline__ float half_of(float x, int) { return x; }
+__device__ __forceinline__ float half_of(F2 x, int h) { return h ? hi_(x) : lo_(x); }
+__device__ __forceinline__ bool half_of(bool m, int) { return m; }
+__device__ __forceinline__ bool half_of(B2 m, int h) { return h ? m.hi : m.lo; }
+__device__ __forceinline__ bool any_(bool m) { return m; }
+__device__ __forceinline__ bool any_(B2 m) { return m.lo || m.hi; }
+template <class T> __device__ __forceinline__ V3T<float> half3(V3T<T> a, int h) { return v3t<float>(half_of(a.x, h), half_of(a.y, h), half_of(a.z, h)); }
+
+// angular acceleration J^-1 (tau_body - w x J w); axisym: J_xx == J_yy, the z component has no gyroscopic term
+template <class T> __device__ __forceinline__ V3T<T> ang_acc_t(const DevParams& P, V3T<T> tb, V3T<T> w, bool axisym) {
+    return v3t<T>(fma_(P.invJ[0], tb.x, mul_(P.ngyro[0], mul_(w.y, w.z))),
+                  fma_(P.invJ[1], tb.y, mul_(P.ngyro[1], mul_(w.z, w.x))),
+                  axisym ? fma_(P.invJ[2], tb.z, 0.0f) : fma_(P.invJ[2], tb.z, mul_(P.ngyro[2], mul_(w.x, w.y))));   // an fma with a zero addend, not
+    // a multiply: the product is summed with the other stages' right away, and ptxas contracts a PACKED multiply-add pair into one
+    // FFMA2 (it never does so for the scalar mul.rn / add.rn), which would make the two instantiations round differently
+}
+// S8 rotation, series form (the hot path): classical RK4 on (q, w_body) with the torque frozen in the world frame (MJC* modes)
+// or explicit Euler (DYN).  The stage orientation is q0 (x) dq, so the body-frame torque at a stage is R(dq)^T tau_b and q0
+// itself is only needed for the final update.  Valid for |omega| h below P.w2_exact; the caller re-does faster spins exactly.
+template <bool EULER, int DEG, class T>
+__device__ __forceinline__ void integrate_rot_t(const DevParams& P, Q4T<T>& q, V3T<T>& w, V3T<T> tau_b, V3T<T> k1_tau, bool axisym) {
+    if (!EULER) {
+        const V3T<T> w0 = w;
+        const V3T<T> k1 = v3t<T>(fma_(P.ngyro[0], mul_(w0.y, w0.z), k1_tau.x), fma_(P.ngyro[1], mul_(w0.z, w0.x), k1_tau.y),
+                                 axisym ? k1_tau.z : fma_(P.ngyro[2], mul_(w0.x, w0.y), k1_tau.z));
+        const V3T<T> w2 = v3t<T>(fma_(P.half_h, k1.x, w0.x), fma_(P.half_h, k1.y, w0.y), fma_(P.half_h, k1.z, w0.z));
+        const V3T<T> k2 = ang_acc_t(P, stage_torque_t<DEG>(P.rotnA_half, P.rotB_half, w0, tau_b), w2, axisym);
+        const V3T<T> w3 = v3t<T>(fma_(P.half_h, k2.x, w0.x), fma_(P.half_h, k2.y, w0.y), fma_(P.half_h, k2.z, w0.z));
+        const V3T<T> k3 = ang_acc_t(P, stage_torque_t<DEG>(P.rotnA_half, P.rotB_half, w2, tau_b), w3, axisym);
+        const V3T<T> w4 = v3t<T>(fma_(P.h, k3.x, w0.x), fma_(P.h, k3.y, w0.y), fma_(P.h, k3.z, w0.z));
+        const V3T<T> k4 = ang_acc_t(P, stage_torque_t<DEG>(P.rotnA_full, P.rotB_full, w3, tau_b), w4, axisym);
+        const V3T<T> ws = v3t<T>(add_(fma_(add_(w2.x, w3.x), 2.0f, w0.x), w4.x), add_(fma_(add_(w2.y, w3.y), 2.0f, w0.y), w4.y),
+                                 add_(fma_(add_(w2.z, w3.z), 2.0f, w0.z), w4.z));          // w0 + 2 (w2 + w3) + w4
+        q = qmul_t(q, exp_half_scaled_t<DEG>(P.expC, P.expS, ws));
+        w = v3t<T>(fma_(P.h_sixth, add_(fma_(add_(k2.x, k3.x), 2.0f, k1.x), k4.x), w0.x),
+                   fma_(P.h_sixth, add_(fma_(add_(k2.y, k3.y), 2.0f, k1.y), k4.y), w0.y),
+                   fma_(P.h_sixth, add_(fma_(add_(k2.z, k3.z), 2.0f, k1.z), k4.z), w0.z));
+    } else {
+        const V3T<T> k1 = ang_acc_t(P, tau_b, w, axisym);
+        w = v3t<T>(fma_(P.h, k1.x, w.x), fma_(P.h, k1.y, w.y), fma_(P.h, k1.z, w.z));
+        q = qmul_t(q, exp_half_t(v3t<T>(mul_(P.h, w.x), mul_(P.h, w.y), mul_(P.h, w.z))));
+    }
+    const T rn = rsqrt_(fma_(q.w, q.w, fma_(q.x, q.x, fma_(q.y, q.y, mul_(q.z, q.z)))));
+    q.w = mul_(q.w, rn); q.x = mul_(q.x, rn); q.y = mul_(q.y, rn); q.z = mul_(q.z, rn);
+}
+// fast spins (|omega| h above the series' range): redo the rotation update from the start-of-substep values with the library
+// sin / cos, out of line, one lane (half) at a time; never taken by the benchmark workloads
+template <bool EULER> __device__ __forceinline__ void redo_fast_spin(const DevParams& P, bool fast, Q4T<float>& q, V3T<float>& w, Q4T<float> q0, V3T<float> w0,
+                                                                      V3T<float> tau_b, V3T<float> k1_tau) {
+    if (fast) {
+        Q4 a; a.w = q0.w; a.x = q0.x; a.y = q0.y; a.z = q0.z;
+        const RotState rs = integrate_rot_exact<EULER>(P, a, v3(w0.x, w0.y, w0.z), v3(tau_b.x, tau_b.y, tau_b.z), v3(k1_tau.x, k1_tau.y, k1_tau.z));
+        q.w = rs.q.w; q.x = rs.q.x; q.y = rs.q.y; q.z = rs.q.z; w.x = rs.w.x; w.y = rs.w.y; w.z = rs.w.z;
+    }
+}
+template <bool EULER> __device__ __forceinline__ void redo_fast_spin(const DevParams& P, B2 fast, Q4T<F2>& q, V3T<F2>& w, Q4T<F2> q0, V3T<F2> w0,
+                                                                      V3T<F2> tau_b, V3T<F2> k1_tau) {
+    if (fast.lo || fast.hi) {
+        float r[2][7];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            Q4T<float> qh; qh.w = half_of(q.w, h); qh.x = half_of(q.x, h); qh.y = half_of(q.y, h); qh.z = half_of(q.z, h);
+            V3T<float> wh = v3t<float>(half_of(w.x, h), half_of(w.y, h), half_of(w.z, h));
+            Q4T<float> q0h; q0h.w = half_of(q0.w, h); q0h.x = half_of(q0.x, h); q0h.y = half_of(q0.y, h); q0h.z = half_of(q0.z, h);
+            redo_fast_spin<EULER>(P, h ? fast.hi : fast.lo, qh, wh, q0h, v3t<float>(half_of(w0.x, h), half_of(w0.y, h), half_of(w0.z, h)),
+                                  v3t<float>(half_of(tau_b.x, h), half_of(tau_b.y, h), half_of(tau_b.z, h)),
+                                  v3t<float>(half_of(k1_tau.x, h), half_of(k1_tau.y, h), half_of(k1_tau.z, h)));
+            r[h][0] = qh.w; r[h][1] = qh.x; r[h][2] = qh.y; r[h][3] = qh.z; r[h][4] = wh.x; r[h][5] = wh.y; r[h][6] = wh.z;
+        }
+        q.w = pk(r[0][0], r[1][0]); q.x = pk(r[0][1], r[1][1]); q.y = pk(r[0][2], r[1][2]); q.z = pk(r[0][3], r[1][3]);
+        w.x = pk(r[0][4], r[1][4]); w.y = pk(r[0][5], r[1][5]); w.z = pk(r[0][6], r[1][6]);
+    }
+}
+
+// What a lane integrates over the substeps: one drone (T = float) or the same drone index of two envs (T = F2).
+template <class T> struct Body {
+    V3T<T> p; Q4T<T> q; V3T<T> v, w;                              // state, w in the body frame
+    V3T<T> tau_b, k1_tau, Fwind;                                  // frozen over a substep: Eq.1-3 torque, J^-1 tau, wind force
+    T thrust, cxy, dcz, gndT, inv_m, ng, ndwc;                    // thrust, Eq.5 / Eq.4 coefficients x rotor terms, 1/m, -g, -Eq.6 coefficient
+};
+// One physics substep (S4-S8): world-frame force from the start-of-substep state, then the free-body update with the wrench
+// frozen.  Returns "went through the floor" (clamped).  The downwash exchange is a shuffle inside the G-lane group.
+template <class T> struct SubstepFlags { typename LaneOps<T>::mask below, fast; };   // went through the floor (clamped); spun too fast for the series
+__device__ __forceinline__ bool inline_redo(float) { return true; }
+__device__ __forceinline__ bool inline_redo(F2) { return false; }
+template <int G, int FEAT, int DEG, class T>
+__device__ __forceinline__ SubstepFlags<T> substep(const DevParams& P, Body<T>& s, int j, bool full_group) {
+    using F = Feat<FEAT>;
+    // b = R(q) z: thrust is T b, and Eq.5's R diag(c_xy, c_xy, c_z) R^T v = c_xy v + (c_z - c_xy)(b.v) b
+    const T bx = mul_(2.0f, fma_(s.q.x, s.q.z, mul_(s.q.w, s.q.y)));
+    const T by = mul_(2.0f, fma_(s.q.y, s.q.z, mul_(neg_(s.q.w), s.q.x)));
+    const T bz = fma_(-2.0f, fma_(s.q.x, s.q.x, mul_(s.q.y, s.q.y)), 1.0f);
+    V3T<T> Fw;
+    if (F::has(P, F_DRAG)) {
+        const T sc = fma_(s.dcz, fma_(bx, s.v.x, fma_(by, s.v.y, mul_(bz, s.v.z))), s.thrust);
+        Fw = v3t<T>(fma_(sc, bx, mul_(s.cxy, s.v.x)), fma_(sc, by, mul_(s.cxy, s.v.y)), fma_(sc, bz, mul_(s.cxy, s.v.z)));
+    } else Fw = v3t<T>(fma_(s.thrust, bx, 0.0f), fma_(s.thrust, by, 0.0f), fma_(s.thrust, bz, 0.0f));   // (fma, not mul: see ang_acc_t)
+    if (F::has(P, F_WIND)) { Fw.x = add_(Fw.x, s.Fwind.x); Fw.y = add_(Fw.y, s.Fwind.y); Fw.z = add_(Fw.z, s.Fwind.z); }
+    if (F::has(P, F_GND)) {                                       // Eq.4, gated on body z pointing up
+        const T hgt = max_(s.p.z, P.h_clip);
+        const T gain = mul_(s.gndT, rcp_(mul_(hgt, hgt)));
+        Fw.z = add_(Fw.z, sel_(gt_(bz, 0.0f), gain, 0.0f));
+    }
+    if (G > 1 && F::has(P, F_DW)) {                               // Eq.6 over every drone above this one
+        // With b' = sqrt(2 ln 2) beta: exp(-dxy^2 / 2 beta^2) = 2^(-dxy^2 / b'^2) and alpha = C1 (r_p/4)^2 / dz_e^2.
+        // One reciprocal r = 1 / (dz_e^2 b'^2) serves both: alpha ~ b'^2 r, exponent = -dxy^2 (dz_e^2 r).
+        // The ramp saturate(dz / dz_clip) is 0 for dz <= 0, which also gates "k above this drone";
+        // b'^2 is floored (beta^2 >= 1e-12), which reproduces the beta -> 0 rule of DESIGN.md Q9.
+        // Pairs are shared out: in round r < G/2 lane j evaluates the pair (j, j + r mod G) once for both ends -
+        // the force goes to whichever drone is lower, the partner's share travels back by one shuffle - and in
+        // round G/2 both ends evaluate their common pair and each keeps its own share.
+        T dw = LaneOps<T>::bc(0.0f);
+#pragma unroll
+        for (int r = 1; r <= G / 2; ++r) {
+            const int src = j + r;                                 // logical lane inside the G-wide segment (taken mod G)
+            const T ox = shfl_(s.p.x, src, G), oy = shfl_(s.p.y, src, G), oz = shfl_(s.p.z, src, G);
+            const T dz = sub_(oz, s.p.z), dx = sub_(ox, s.p.x), dy = sub_(oy, s.p.y);
+            const T dxy2 = fma_(dx, dx, mul_(dy, dy));
+            const T adz = abs_(dz);
+            const T dze = max_(adz, P.dz_floor);
+            const T ramp = sat_(mul_(adz, P.inv_dz_clip));
+            const T bs = fma_(P.dw_C2s, dze, P.dw_C3s);
+            const T b2 = max_(mul_(bs, bs), P.dw_b2_min), z2 = mul_(dze, dze);
+            const T rinv = rcp_(mul_(z2, b2));
+            const T ex = ex2n_(mul_(dxy2, mul_(z2, rinv)));
+            const T al = mul_(ramp, mul_(b2, rinv));
+            const bool on = full_group || (j < P.M && ((j + r) & (G - 1)) < P.M);
+            const T f = sel_(and_(lt_(dxy2, 100.0f), on), mul_(al, ex), 0.0f);
+            const typename LaneOps<T>::mask above = gt_(dz, 0.0f);   // the partner is above this drone
+            if (r < G / 2) {
+                const T back = shfl_(sel_(above, 0.0f, f), j + G - r, G);
+                dw = add_(dw, add_(sel_(above, f, 0.0f), back));
+            } else dw = add_(dw, sel_(above, f, 0.0f));
+        }
+        Fw.z = fma_(s.ndwc, dw, Fw.z);
+    }
+    const V3T<T> acc = v3t<T>(mul_(Fw.x, s.inv_m), mul_(Fw.y, s.inv_m), fma_(Fw.z, s.inv_m, s.ng));
+
+    // S8 integrate with the wrench frozen in the world frame
+    const typename LaneOps<T>::mask fast_spin = gt_(dot3(s.w, s.w), P.w2_exact[DEG - 2]);
+    const Q4T<T> q0 = s.q;
+    const V3T<T> w0 = s.w;
+    if (!F::has(P, F_EULER)) {
+        s.p.x = fma_(P.half_h2, acc.x, fma_(P.h, s.v.x, s.p.x));
+        s.p.y = fma_(P.half_h2, acc.y, fma_(P.h, s.v.y, s.p.y));
+        s.p.z = fma_(P.half_h2, acc.z, fma_(P.h, s.v.z, s.p.z));
+        s.v.x = fma_(P.h, acc.x, s.v.x); s.v.y = fma_(P.h, acc.y, s.v.y); s.v.z = fma_(P.h, acc.z, s.v.z);
+        integrate_rot_t<false, DEG>(P, s.q, s.w, s.tau_b, s.k1_tau, F::has(P, F_AXISYM));
+        if (inline_redo(s.p.x)) redo_fast_spin<false>(P, fast_spin, s.q, s.w, q0, w0, s.tau_b, s.k1_tau);
+    } else {                                                       // DYN: explicit Euler
+        s.v.x = fma_(P.h, acc.x, s.v.x); s.v.y = fma_(P.h, acc.y, s.v.y); s.v.z = fma_(P.h, acc.z, s.v.z);
+        s.p.x = fma_(P.h, s.v.x, s.p.x); s.p.y = fma_(P.h, s.v.y, s.p.y); s.p.z = fma_(P.h, s.v.z, s.p.z);
+        integrate_rot_t<true, DEG>(P, s.q, s.w, s.tau_b, s.k1_tau, F::has(P, F_AXISYM));
+        if (inline_redo(s.p.x)) redo_fast_spin<true>(P, fast_spin, s.q, s.w, q0, w0, s.tau_b, s.k1_tau);
+    }
+    const typename LaneOps<T>::mask below = lt_(s.p.z, 0.0f);       // floor
+    s.v.z = sel_(below, max_(s.v.z, 0.0f), s.v.z);
+    s.p.z = sel_(below, 0.0f, s.p.z);
+    SubstepFlags<T> fl; fl.below = below; fl.fast = fast_spin;
+    return fl;
+}
+// Two envs per lane keep the hot loop free of the exact path: a warp in which any lane spun too fast during the step redoes the
+// step's K substeps one env slot at a time with the one-drone code (same arithmetic: the result is what one env per lane
+// computes), from the start-of-step state that is still in the warp's landing zone W.  Out of line, never taken by the benchmarks.
+struct RedoOut { float s[13]; bool hit; };
+template <int G, int FEAT, int DEG>
+__device__ __noinline__ RedoOut redo_item_exact(const DevParams& P, const WarpStage& W, Body<float> b, int lane, int j, bool full_group) {
+    const float4 a0 = W.plane[0][lane], a1 = W.plane[1][lane], a2 = W.plane[2][lane], a3 = W.plane[3][lane];
+    b.p = v3t<float>(a0.x, a0.y, a0.z); b.q.w = a0.w; b.q.x = a1.x; b.q.y = a1.y; b.q.z = a1.z;
+    b.v = v3t<float>(a1.w, a2.x, a2.y); b.w = v3t<float>(a2.z, a2.w, a3.x);
+    RedoOut o; o.hit = false;
+    for (int k = 0; k < P.K; ++k) o.hit |= substep<G, FEAT, DEG>(P, b, j, full_group).below;
+    o.s[0] = b.p.x; o.s[1] = b.p.y; o.s[2] = b.p.z; o.s[3] = b.q.w; o.s[4] = b.q.x; o.s[5] = b.q.y; o.s[6] = b.q.z;
+    o.s[7] = b.v.x; o.s[8] = b.v.y; o.s[9] = b.v.z; o.s[10] = b.w.x; o.s[11] = b.w.y; o.s[12] = b.w.z;
+    return o;
+}
+
+// What one lane carries for one of its NP env slots from the prologue to the epilogue of a work item.
+struct Slot {
+    unsigned e; bool active; size_t drone;
+    DroneRegs d; float4 tg, act4, env4; uint32_t t;
+    float4 dr0, dr1, dr2, dr3;                                    // this episode's DR factors (read-mostly, plain loads)
+    V3 Fwind; float4 gust_out;                                    // wind force held over the substeps; E1 after this step (MDG_WIND_GUST)
+    float n[4], n_later[4], n_act[4], lag_gain; int sw, d_obs;    // rotor commands (now / after the latency switch), rotor speeds under lag
+    float kf_e, kappa_e, inv_sJ, inv_m_e, g_e, dwc_e;             // the true vehicle of this episode (Table 4)
+    float T, cxy, dcz, gndT; V3 tau_b, k1_tau;                    // motor model (Eq.1-3) as the substeps use it
+    bool hit; Sensed snap;
+};
+
 // One control step of every env.  Persistent warps: each loops over work items of
-// 32 / G envs; lane -> (env e, lane-in-group j).  While an item is integrated, the next item's state planes,
-// actions and per-env words are already on their way into shared memory (cp.async, two stages), so HBM
-// latency and bandwidth overlap the arithmetic instead of alternating with it.
+// NP * 32 / G envs; lane -> (lane-in-group j, NP envs: slot h holds env (item * NP + h) * 32 / G + lane / G).  With NP = 2 the
+// substeps of a lane's two drones run as packed FP32 pairs (mdg_dev.cuh: F2), everything else once per slot.  While an item is
+// integrated, the next item's state planes, actions and per-env words are already on their way into shared memory (cp.async,
+// two stages), so HBM latency and bandwidth overlap the arithmetic instead of alternating with it.
 // MINB = resident blocks of 128 threads per SM the register allocation must allow.
-template <int G, int FEAT, int MINB>
+template <int G, int FEAT, int MINB, int NP>
 __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__ DevParams P, const DevBuffers B,
                                                          const float4* __restrict__ actions) {
     using F = Feat<FEAT>;
+    using T = typename Lanes<NP>::T;
+    static_assert(NP == 1 || FEAT >= 0, "two envs per lane need a compile-time feature word");
+    static_assert(NP == 1 || !(FEAT & (F_MLAG | F_LAT)), "motor lag and the latency rows switch rotor commands inside the substep loop: one env per lane");
     // series degree of the rotation update: 2 where the specialisation's controller keeps the body rates small (PID / VEL)
     constexpr int DEG = (FEAT >= 0 && (((FEAT >> F_ACT_SHIFT) & 7) == 1 || ((FEAT >> F_ACT_SHIFT) & 7) == 2)) ? 2 : 3;
-    extern __shared__ __align__(16) unsigned char smem_raw[];     // [2 stages][warps per block] WarpStage (host sizes it)
+    extern __shared__ __align__(16) unsigned char smem_raw[];     // [P.n_stages][warps per block][NP] WarpStage (host sizes it)
     WarpStage* const S = reinterpret_cast<WarpStage*>(smem_raw);
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const unsigned wpb = blockDim.x >> 5;
     const unsigned tw = gridDim.x * wpb;                          // persistent warps of this launch
-    const unsigned n_items = ((unsigned)P.N + (32u / G) - 1) / (32u / G);
+    const unsigned epi = NP * (32u / G);                          // envs per work item
+    const unsigned n_items = ((unsigned)P.N + epi - 1) / epi;
     const int j = lane % G;
     const bool full_group = F::has(P, F_FULL);
     const int jj = (full_group || j < P.M) ? j : P.M - 1;
@@ -175,10 +377,22 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const bool static_items = P.static_items != 0;
     unsigned wt = blockIdx.x * wpb + wib;
     if (wt >= n_items) return;                                    // only in grids that do not fill the device (static_items)
-    unsigned wt_next = static_items ? 0xFFFFFFFFu : take(draw(true));   // a warp stops drawing after its first miss
+    // start-up: the first item's flag probe and the first ticket are in flight together, the item's copies start as soon as
+    // the flag is in (every warp of a launch pays this once, a good part of its life when a launch gives it two or three items)
+    const unsigned probed_first = probe(wt);
+    const unsigned drawn_first = draw(!static_items);
+    await_item(wt, probed_first);
+    auto prefetch = [&](unsigned item, int stage, unsigned dep) {
+#pragma unroll
+        for (int h = 0; h < NP; ++h) prefetch_item<G>(P, B, actions, S[(stage * wpb + wib) * NP + h], item * NP + h, lane, jj, F::act(P), dep);
+        cp_async_commit();
+    };
+    // P.n_stages == 1: one landing zone per warp, refilled as soon as its contents have been read into registers (half the
+    // shared memory, room for more resident blocks); 2: the next item lands beside the current one.
+    const int flip = P.n_stages - 1;
+    prefetch(wt, 0, 0u);
+    unsigned wt_next = static_items ? 0xFFFFFFFFu : take(drawn_first);   // a warp stops drawing after its first miss
     unsigned probed_next = probe(wt_next);
-    await_item(wt, probe(wt));
-    prefetch_item<G>(P, B, actions, S[wib], wt, lane, jj, F::act(P));
     // Items whose flags are still to be published.  One fence covers two items: the consumer (the next step) reaches
     // an item a whole step later, so publishing it one item late costs nothing and halves the fences.
     unsigned pending = 0xFFFFFFFFu, pending2 = 0xFFFFFFFFu;
@@ -186,377 +400,442 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
 #pragma unroll 1
     for (;;) {
     const unsigned drawn_l0 = draw(wt_next < n_items);            // ticket of the item after next, in flight
-    const unsigned e_raw = wt * (32u / G) + (unsigned)lane / G;
-    const bool env_ok = e_raw < (unsigned)P.N;
-    const unsigned e = env_ok ? e_raw : (unsigned)P.N - 1;      // idle lanes shadow the last env (no stores)
-    const bool active = env_ok && (full_group || j < P.M);
-    const size_t drone = (size_t)e * P.M + jj;
-
+    Slot sl[NP];
+    unsigned touched = 0u;                                        // OR of one word of every shared-memory read of this item
     cp_async_wait_all();
-    const WarpStage& W = S[st * wpb + wib];
-    DroneRegs d;
-    {
+#pragma unroll
+    for (int h = 0; h < NP; ++h) {
+        Slot& s = sl[h];
+        const unsigned e_raw = (wt * NP + h) * (32u / G) + (unsigned)lane / G;
+        const bool env_ok = e_raw < (unsigned)P.N;
+        s.e = env_ok ? e_raw : (unsigned)P.N - 1;                 // idle lanes shadow the last env (no stores)
+        s.active = env_ok && (full_group || j < P.M);
+        s.drone = (size_t)s.e * P.M + jj;
+        const WarpStage& W = S[(st * wpb + wib) * NP + h];
         const float4 a = W.plane[0][lane], b = W.plane[1][lane], c = W.plane[2][lane], f = W.plane[3][lane];
-        d.p = v3(a.x, a.y, a.z); d.q.w = a.w; d.q.x = b.x; d.q.y = b.y; d.q.z = b.z;
-        d.v = v3(b.w, c.x, c.y); d.w = v3(c.z, c.w, f.x); d.Ip = v3(f.y, f.z, f.w);
+        s.d.p = v3(a.x, a.y, a.z); s.d.q.w = a.w; s.d.q.x = b.x; s.d.q.y = b.y; s.d.q.z = b.z;
+        s.d.v = v3(b.w, c.x, c.y); s.d.w = v3(c.z, c.w, f.x); s.d.Ip = v3(f.y, f.z, f.w);
+        if (pid) {
+            const float4 i4 = W.plane[4][lane];
+            s.d.Ie = v3(i4.x, i4.y, i4.z);
+            if (F::act(P) == 1) s.d.sp = W.plane[5][lane];
+        }
+        s.tg = W.plane[6][lane];
+        s.act4 = W.plane[7][lane];
+        s.env4 = W.plane[8][lane];
+        s.t = W.gstep[lane] + 1u;
+        touched |= __float_as_uint(a.x) | __float_as_uint(b.x) | __float_as_uint(c.x) | __float_as_uint(f.x) | __float_as_uint(s.tg.x) |
+                   __float_as_uint(s.act4.x) | __float_as_uint(s.env4.x) | s.t;
+        if (pid) touched |= __float_as_uint(s.d.Ie.x) | (F::act(P) == 1 ? __float_as_uint(s.d.sp.x) : 0u);
+        s.dr0 = make_float4(1, 1, 1, 1); s.dr1 = s.dr0; s.dr2 = s.dr0; s.dr3 = s.dr0;
+        if (F::has(P, F_DR)) { s.dr0 = B.R0[s.drone]; s.dr1 = B.R1[s.drone]; s.dr2 = B.R2[s.drone]; s.dr3 = B.R3[s.drone]; }
     }
-    if (pid) {
-        const float4 i4 = W.plane[4][lane];
-        d.Ie = v3(i4.x, i4.y, i4.z);
-        if (F::act(P) == 1) d.sp = W.plane[5][lane];
-    }
-    float4 tg = W.plane[6][lane];
-    const float4 act4 = W.plane[7][lane];
-    float4 env4 = W.plane[8][lane];
-    const uint32_t t = W.gstep[lane] + 1u;
-    float4 dr0 = make_float4(1, 1, 1, 1), dr1 = dr0, dr2 = dr0, dr3 = dr0;   // this episode's DR factors (read-mostly, plain loads)
-    if (F::has(P, F_DR)) { dr0 = B.R0[drone]; dr1 = B.R1[drone]; dr2 = B.R2[drone]; dr3 = B.R3[drone]; }
-    if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch_item<G>(P, B, actions, S[(st ^ 1) * wpb + wib], wt_next, lane, jj, F::act(P)); }
+    if (flip && wt_next < n_items) { await_item(wt_next, probed_next); prefetch(wt_next, st ^ 1, 0u); }   // two landing zones: the next item starts coming now
 
-    // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
-    // Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact in
-    // fp32; cos/sin(2 pi u_b) = -cos/sin(2 pi (u_b - 1/2)) keeps the MUFU argument in [-pi, pi).
-    V3 Fwind = v3(0, 0, 0);
-    float4 gust_out = make_float4(0, 0, 0, 1.0f);                  // E1 after this step (generic kernel, MDG_WIND_GUST only)
-    if (F::has(P, F_WIND)) {
-        // components (MDG_WIND_*): the benchmark configs run the AR(1) gust alone (wmask == 1 folds at compile time)
-        const int wmask = F::has(P, F_WIND_MIX) ? P.wind_mask : 1;
-        V3 u = v3(0, 0, 0);                                        // air velocity
-        if (wmask & 1) {
-            const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
-            const float r1 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.x))), r2 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.z)));
-            const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
-            float wa = P.wind_alpha, wg = P.wind_gain;
-            if (F::has(P, F_WIND_MIX) && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
-                const float hm = fmaxf(group_sum<G>((full_group || j < P.M) ? d.p.z : 0.0f) * P.inv_M, P.dryden_h_min);   // alpha = exp(-dt V / L)
-                const float x = P.dryden_x * powf(fmaf(8.23e-4f, hm, 0.177f), 1.2f) / hm;
-                wa = expf(-x);
-                wg = P.wind_sigma * sqrtf(-expm1f(-2.0f * x));    // sigma sqrt(1 - alpha^2) without the cancellation
-            }
-            env4.x = fmaf(wa, env4.x, wg * (r1 * cos_fast(a1)));
-            env4.y = fmaf(wa, env4.y, wg * (r1 * sin_fast(a1)));
-            env4.z = fmaf(wa, env4.z, wg * (r2 * cos_fast(a2)));
-            u = v3(env4.x, env4.y, env4.z);
-        }
-        if (wmask & 2) { u.x += P.wind_const[0]; u.y += P.wind_const[1]; u.z += P.wind_const[2]; }
-        if (wmask & 4) {                                           // PAPER.md:201 impulses (Q42), state in E1
-            float4 gs = B.E1[e];
-            if (gs.w >= 1.0f) {                                    // none running: trigger with probability gust_prob
-                const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_GUST, P.seed_lo, P.seed_hi);
-                if (u01(r.x) < P.gust_prob) {
-                    const float amp = P.gust_max * u01(r.y), z = fmaf(2.0f, u01(r.z), -1.0f);
-                    const float rxy = sqrtf(fmaxf(fmaf(-z, z, 1.0f), 0.0f));
-                    float sp, cp;
-                    sincospif(2.0f * u01(r.w), &sp, &cp);
-                    gs = make_float4(amp * rxy * cp, amp * rxy * sp, amp * z, 0.0f);
-                }
-            }
-            if (gs.w < 1.0f) {                                     // envelope sin(pi s), s advances by dt_c / duration
-                const float es = sinpif(gs.w);
-                u.x = fmaf(gs.x, es, u.x); u.y = fmaf(gs.y, es, u.y); u.z = fmaf(gs.z, es, u.z);
-                gs.w += P.gust_ds;
-            }
-            gust_out = gs;
-        }
-        if (wmask & 7) {
-            const V3 rel = v3(u.x - d.v.x, u.y - d.v.y, u.z - d.v.z);
-            const float kn = P.k_wind * fast_sqrt(fmaf(rel.x, rel.x, fmaf(rel.y, rel.y, rel.z * rel.z)));
-            Fwind = v3(kn * rel.x, kn * rel.y, kn * rel.z);
-        }
-        if (wmask & 8) {                                           // PAPER.md:204, episode time at the start of the step
-            const float ph = P.wind_sine_omega * ((float)__float_as_uint(env4.w) * P.dt_c);
-            float s1, c1;
-            sincosf(ph, &s1, &c1);
-            Fwind.x = fmaf(P.wind_sine_amp, s1, Fwind.x); Fwind.y = fmaf(P.wind_sine_amp, c1, Fwind.y);
-            Fwind.z = fmaf(0.6f * P.wind_sine_amp, s1 * c1, Fwind.z);   // 0.3 sin 2x = 0.6 sin x cos x
-        }
-    }
-
-    // Table 4 latency rows (Q51): this episode's delays in substeps from one Philox draw at the
-    // episode's reset index.  The row issued at step t runs from substep d on: with d = (n - 1) K + r, 1 <= r <= K, substeps
-    // k < r of this step run the row of n steps ago, the rest the row after it.  A controller decodes once, from the first.
-    float4 a_first = act4, a_second = act4;
-    int sw = -1, d_obs = 0;
-    if (F::has(P, F_LAT)) {
-        const uint32_t ep0 = __float_as_uint(env4.w);
-        const uint4 lr = philox4x32_10(e + P.env_base, (uint32_t)jj, (t - 1u) - ep0, STREAM_LATENCY, P.seed_lo, P.seed_hi);
-        d_obs = P.lat_s_lo + (int)(((lr.y >> 8) * (uint32_t)P.lat_s_n) >> 24);
-        if (P.lat_a_n > 0) {
-            const int d_act = P.lat_a_lo + (int)(((lr.x >> 8) * (uint32_t)P.lat_a_n) >> 24);
-            float4 h0 = B.H0[drone], h1 = B.H1[drone], h2 = B.H2[drone];
-            if (ep0 == 0u) h0 = h1 = h2 = act4;                    // primed with the episode's first row
-            const int nb = (d_act + P.K - 1) / P.K, r = d_act - (nb - 1) * P.K;
-            a_first = nb == 0 ? act4 : nb == 1 ? h0 : nb == 2 ? h1 : h2;
-            a_second = nb <= 1 ? act4 : nb == 2 ? h0 : h1;
-            const int at = F::act(P);
-            if ((at == 0 || at == 3 || at == 4) && nb >= 1 && r < P.K) sw = r;
-            if (active) { B.H2[drone] = h1; B.H1[drone] = h0; B.H0[drone] = act4; }
-        }
-    }
-    // S1/S2 decode, S3 motor model (Eq.1-3); RPMs are held over the K substeps
-    float n[4], n_later[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-    decode_action<FEAT>(P, a_first, d, n);
-    if (F::has(P, F_LAT) && sw >= 0) { DroneRegs dtmp = d; decode_action<FEAT>(P, a_second, dtmp, n_later); }   // direct rotor commands: stateless
-    // Domain randomisation (Table 4): this episode's factors scale the true vehicle, not the controller's model above.
-    // 1 / s_J is folded into the body torque (every stage torque is linear in it, the gyroscopic ratios do not change).
     const bool dr = F::has(P, F_DR);
-    const float kf_e = dr ? P.k_f * dr0.z : P.k_f, kappa_e = dr ? P.kappa * (dr0.w / dr0.z) : P.kappa;
-    const float inv_sJ = dr ? 1.0f / dr0.y : 1.0f, inv_m_e = dr ? P.inv_m / dr0.x : P.inv_m, g_e = dr ? P.g * dr1.w : P.g;
-    const float dwc_e = dr ? P.dw_coef * dr1.z : P.dw_coef;
-    if (dr) {                                                      // true motor saturation of this episode
-        const float nmax = P.max_rpm * dr3.y;
-        n[0] = fminf(n[0], nmax); n[1] = fminf(n[1], nmax); n[2] = fminf(n[2], nmax); n[3] = fminf(n[3], nmax);
-        n_later[0] = fminf(n_later[0], nmax); n_later[1] = fminf(n_later[1], nmax); n_later[2] = fminf(n_later[2], nmax); n_later[3] = fminf(n_later[3], nmax);
-    }
-    // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag
-    float T, cxy, dcz, gndT;
-    V3 tau_b, k1_tau;
-    auto motor_model = [&](const float (&nn)[4]) {
-        const float f0 = (dr ? kf_e * dr2.x : kf_e) * (nn[0] * nn[0]), f1 = (dr ? kf_e * dr2.y : kf_e) * (nn[1] * nn[1]),
-                    f2 = (dr ? kf_e * dr2.z : kf_e) * (nn[2] * nn[2]), f3 = (dr ? kf_e * dr2.w : kf_e) * (nn[3] * nn[3]);
-        T = (f0 + f1) + (f2 + f3);
-        const float arm_e = dr ? dr3.x : 1.0f;
-        tau_b = F::has(P, F_CF2P) ? v3(P.arm * (f1 - f3), P.arm * (f2 - f0), kappa_e * ((f1 + f3) - (f0 + f2)))
-                                  : v3(P.l * ((f0 + f1) - (f2 + f3)), P.l * ((f1 + f2) - (f0 + f3)), kappa_e * ((f1 + f3) - (f0 + f2)));
-        if (dr) { tau_b.x *= inv_sJ * arm_e; tau_b.y *= inv_sJ * arm_e; tau_b.z *= inv_sJ; }
-        const float Om = P.rpm2rad * ((nn[0] + nn[1]) + (nn[2] + nn[3]));
-        k1_tau = v3(P.invJ[0] * tau_b.x, P.invJ[1] * tau_b.y, P.invJ[2] * tau_b.z);
-        cxy = (dr ? -P.c_xy * dr1.x : -P.c_xy) * Om;
-        const float cz = (dr ? -P.c_z * dr1.x : -P.c_z) * Om;
-        gndT = (dr ? P.gnd_coef * dr1.y : P.gnd_coef) * T;
-        dcz = cz - cxy;
-    };
-    // Table 4 motor lag (Q44): the rotors follow n through a first-order lag sampled exactly per substep
     const bool lag = F::has(P, F_MLAG);
-    float n_act[4] = {n[0], n[1], n[2], n[3]};
-    float lag_gain = 1.0f;
-    if (lag) {
-        const float4 r = B.N0[drone];
-        n_act[0] = r.x; n_act[1] = r.y; n_act[2] = r.z; n_act[3] = r.w;
-        lag_gain = 1.0f - __expf(-P.h / dr3.z);
-    } else motor_model(n);
+    // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag
+    // (every product and sum spelled out: the compiler must not choose, per instantiation, which of them to contract into
+    // fused multiply-adds - both lane shapes have to round identically)
+    auto motor_model = [&](Slot& s, const float (&nn)[4]) {
+        const float k0 = dr ? __fmul_rn(s.kf_e, s.dr2.x) : s.kf_e, k1 = dr ? __fmul_rn(s.kf_e, s.dr2.y) : s.kf_e,
+                    k2 = dr ? __fmul_rn(s.kf_e, s.dr2.z) : s.kf_e, k3 = dr ? __fmul_rn(s.kf_e, s.dr2.w) : s.kf_e;
+        const float f0 = __fmul_rn(k0, __fmul_rn(nn[0], nn[0])), f1 = __fmul_rn(k1, __fmul_rn(nn[1], nn[1])),
+                    f2 = __fmul_rn(k2, __fmul_rn(nn[2], nn[2])), f3 = __fmul_rn(k3, __fmul_rn(nn[3], nn[3]));
+        const float f01 = __fadd_rn(f0, f1), f23 = __fadd_rn(f2, f3), f12 = __fadd_rn(f1, f2), f03 = __fadd_rn(f0, f3),
+                    f13 = __fadd_rn(f1, f3), f02 = __fadd_rn(f0, f2);
+        s.T = __fadd_rn(f01, f23);
+        const float arm_e = dr ? s.dr3.x : 1.0f;
+        const float tz = __fmul_rn(s.kappa_e, __fsub_rn(f13, f02));
+        s.tau_b = F::has(P, F_CF2P) ? v3(__fmul_rn(P.arm, __fsub_rn(f1, f3)), __fmul_rn(P.arm, __fsub_rn(f2, f0)), tz)
+                                    : v3(__fmul_rn(P.l, __fsub_rn(f01, f23)), __fmul_rn(P.l, __fsub_rn(f12, f03)), tz);
+        if (dr) {
+            const float sxy = __fmul_rn(s.inv_sJ, arm_e);
+            s.tau_b.x = __fmul_rn(s.tau_b.x, sxy); s.tau_b.y = __fmul_rn(s.tau_b.y, sxy); s.tau_b.z = __fmul_rn(s.tau_b.z, s.inv_sJ);
+        }
+        const float Om = __fmul_rn(P.rpm2rad, __fadd_rn(__fadd_rn(nn[0], nn[1]), __fadd_rn(nn[2], nn[3])));
+        s.k1_tau = v3(__fmul_rn(P.invJ[0], s.tau_b.x), __fmul_rn(P.invJ[1], s.tau_b.y), __fmul_rn(P.invJ[2], s.tau_b.z));
+        s.cxy = __fmul_rn(dr ? __fmul_rn(-P.c_xy, s.dr1.x) : -P.c_xy, Om);
+        const float cz = __fmul_rn(dr ? __fmul_rn(-P.c_z, s.dr1.x) : -P.c_z, Om);
+        s.gndT = __fmul_rn(dr ? __fmul_rn(P.gnd_coef, s.dr1.y) : P.gnd_coef, s.T);
+        s.dcz = __fsub_rn(cz, s.cxy);
+    };
+#pragma unroll
+    for (int h = 0; h < NP; ++h) {
+        Slot& s = sl[h];
+        DroneRegs& d = s.d;
+        float4& env4 = s.env4;
+        const unsigned e = s.e;
+        const uint32_t t = s.t;
+        const float4 act4 = s.act4;
+        const size_t drone = s.drone;
+        const bool active = s.active;
+        // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
+        // Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact in
+        // fp32; cos/sin(2 pi u_b) = -cos/sin(2 pi (u_b - 1/2)) keeps the MUFU argument in [-pi, pi).
+        V3 Fwind = v3(0, 0, 0);
+        float4 gust_out = make_float4(0, 0, 0, 1.0f);                  // E1 after this step (generic kernel, MDG_WIND_GUST only)
+        if (F::has(P, F_WIND)) {
+            // components (MDG_WIND_*): the benchmark configs run the AR(1) gust alone (wmask == 1 folds at compile time)
+            const int wmask = F::has(P, F_WIND_MIX) ? P.wind_mask : 1;
+            V3 u = v3(0, 0, 0);                                        // air velocity
+            if (wmask & 1) {
+                const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
+                const float r1 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.x))), r2 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.z)));
+                const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
+                float wa = P.wind_alpha, wg = P.wind_gain;
+                if (F::has(P, F_WIND_MIX) && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
+                    const float hm = fmaxf(group_sum<G>((full_group || j < P.M) ? d.p.z : 0.0f) * P.inv_M, P.dryden_h_min);   // alpha = exp(-dt V / L)
+                    const float x = P.dryden_x * powf(fmaf(8.23e-4f, hm, 0.177f), 1.2f) / hm;
+                    wa = expf(-x);
+                    wg = P.wind_sigma * sqrtf(-expm1f(-2.0f * x));    // sigma sqrt(1 - alpha^2) without the cancellation
+                }
+                env4.x = fmaf(wa, env4.x, wg * (r1 * cos_fast(a1)));
+                env4.y = fmaf(wa, env4.y, wg * (r1 * sin_fast(a1)));
+                env4.z = fmaf(wa, env4.z, wg * (r2 * cos_fast(a2)));
+                u = v3(env4.x, env4.y, env4.z);
+            }
+            if (wmask & 2) { u.x += P.wind_const[0]; u.y += P.wind_const[1]; u.z += P.wind_const[2]; }
+            if (wmask & 4) {                                           // PAPER.md:201 impulses (Q42), state in E1
+                float4 gs = B.E1[e];
+                if (gs.w >= 1.0f) {                                    // none running: trigger with probability gust_prob
+                    const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_GUST, P.seed_lo, P.seed_hi);
+                    if (u01(r.x) < P.gust_prob) {
+                        const float amp = P.gust_max * u01(r.y), z = fmaf(2.0f, u01(r.z), -1.0f);
+                        const float rxy = sqrtf(fmaxf(fmaf(-z, z, 1.0f), 0.0f));
+                        float sp, cp;
+                        sincospif(2.0f * u01(r.w), &sp, &cp);
+                        gs = make_float4(amp * rxy * cp, amp * rxy * sp, amp * z, 0.0f);
+                    }
+                }
+                if (gs.w < 1.0f) {                                     // envelope sin(pi s), s advances by dt_c / duration
+                    const float es = sinpif(gs.w);
+                    u.x = fmaf(gs.x, es, u.x); u.y = fmaf(gs.y, es, u.y); u.z = fmaf(gs.z, es, u.z);
+                    gs.w += P.gust_ds;
+                }
+                gust_out = gs;
+            }
+            if (wmask & 7) {
+                const V3 rel = v3(u.x - d.v.x, u.y - d.v.y, u.z - d.v.z);
+                const float kn = P.k_wind * fast_sqrt(fmaf(rel.x, rel.x, fmaf(rel.y, rel.y, rel.z * rel.z)));
+                Fwind = v3(kn * rel.x, kn * rel.y, kn * rel.z);
+            }
+            if (wmask & 8) {                                           // PAPER.md:204, episode time at the start of the step
+                const float ph = P.wind_sine_omega * ((float)__float_as_uint(env4.w) * P.dt_c);
+                float s1, c1;
+                sincosf(ph, &s1, &c1);
+                Fwind.x = fmaf(P.wind_sine_amp, s1, Fwind.x); Fwind.y = fmaf(P.wind_sine_amp, c1, Fwind.y);
+                Fwind.z = fmaf(0.6f * P.wind_sine_amp, s1 * c1, Fwind.z);   // 0.3 sin 2x = 0.6 sin x cos x
+            }
+        }
 
-    bool hit = false;
+        s.Fwind = Fwind; s.gust_out = gust_out;
+        // Table 4 latency rows (Q51): this episode's delays in substeps from one Philox draw at the
+        // episode's reset index.  The row issued at step t runs from substep d on: with d = (n - 1) K + r, 1 <= r <= K, substeps
+        // k < r of this step run the row of n steps ago, the rest the row after it.  A controller decodes once, from the first.
+        float4 a_first = act4, a_second = act4;
+        int sw = -1, d_obs = 0;
+        if (F::has(P, F_LAT)) {
+            const uint32_t ep0 = __float_as_uint(env4.w);
+            const uint4 lr = philox4x32_10(e + P.env_base, (uint32_t)jj, (t - 1u) - ep0, STREAM_LATENCY, P.seed_lo, P.seed_hi);
+            d_obs = P.lat_s_lo + (int)(((lr.y >> 8) * (uint32_t)P.lat_s_n) >> 24);
+            if (P.lat_a_n > 0) {
+                const int d_act = P.lat_a_lo + (int)(((lr.x >> 8) * (uint32_t)P.lat_a_n) >> 24);
+                float4 h0 = B.H0[drone], h1 = B.H1[drone], h2 = B.H2[drone];
+                if (ep0 == 0u) h0 = h1 = h2 = act4;                    // primed with the episode's first row
+                const int nb = (d_act + P.K - 1) / P.K, r = d_act - (nb - 1) * P.K;
+                a_first = nb == 0 ? act4 : nb == 1 ? h0 : nb == 2 ? h1 : h2;
+                a_second = nb <= 1 ? act4 : nb == 2 ? h0 : h1;
+                const int at = F::act(P);
+                if ((at == 0 || at == 3 || at == 4) && nb >= 1 && r < P.K) sw = r;
+                if (active) { B.H2[drone] = h1; B.H1[drone] = h0; B.H0[drone] = act4; }
+            }
+        }
+        s.sw = sw; s.d_obs = d_obs;
+        // S1/S2 decode, S3 motor model (Eq.1-3); RPMs are held over the K substeps
+        s.n_later[0] = s.n_later[1] = s.n_later[2] = s.n_later[3] = 0.0f;
+        decode_action<FEAT>(P, a_first, d, s.n);
+        if (F::has(P, F_LAT) && s.sw >= 0) { DroneRegs dtmp = d; decode_action<FEAT>(P, a_second, dtmp, s.n_later); }   // direct rotor commands: stateless
+        // Domain randomisation (Table 4): this episode's factors scale the true vehicle, not the controller's model above.
+        // 1 / s_J is folded into the body torque (every stage torque is linear in it, the gyroscopic ratios do not change).
+        s.kf_e = dr ? __fmul_rn(P.k_f, s.dr0.z) : P.k_f; s.kappa_e = dr ? __fmul_rn(P.kappa, __fdiv_rn(s.dr0.w, s.dr0.z)) : P.kappa;
+        s.inv_sJ = dr ? __fdiv_rn(1.0f, s.dr0.y) : 1.0f; s.inv_m_e = dr ? __fdiv_rn(P.inv_m, s.dr0.x) : P.inv_m; s.g_e = dr ? __fmul_rn(P.g, s.dr1.w) : P.g;
+        s.dwc_e = dr ? __fmul_rn(P.dw_coef, s.dr1.z) : P.dw_coef;
+        if (dr) {                                                      // true motor saturation of this episode
+            const float nmax = __fmul_rn(P.max_rpm, s.dr3.y);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { s.n[i] = fminf(s.n[i], nmax); s.n_later[i] = fminf(s.n_later[i], nmax); }
+        }
+        // Table 4 motor lag (Q44): the rotors follow n through a first-order lag sampled exactly per substep
+#pragma unroll
+        for (int i = 0; i < 4; ++i) s.n_act[i] = s.n[i];
+        s.lag_gain = 1.0f;
+        if (lag) {
+            const float4 r = B.N0[s.drone];
+            s.n_act[0] = r.x; s.n_act[1] = r.y; s.n_act[2] = r.z; s.n_act[3] = r.w;
+            s.lag_gain = 1.0f - __expf(-P.h / s.dr3.z);
+        } else motor_model(s, s.n);
+        s.hit = false;
+        s.snap = sensed(d, v3(0, 0, 0));                              // sensor latency of a whole step: the state the step starts from
+        // What only the epilogue needs goes back to the landing zone, which stays intact until the next prefetch into it: the
+        // substep loop then holds nothing but the integrated state and the frozen wrench in registers.
+        WarpStage& Wm = S[(st * wpb + wib) * NP + h];
+        Wm.plane[3][lane] = make_float4(d.w.z, d.Ip.x, d.Ip.y, d.Ip.z);
+        if (pid) {
+            Wm.plane[4][lane] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
+            if (F::act(P) == 1) Wm.plane[5][lane] = d.sp;
+        }
+        Wm.plane[8][lane] = env4;
+    }
+    asm volatile("" ::: "memory");                                // the epilogue re-reads them: no register copies kept across the loop
+
     const bool flush = pending2 != 0xFFFFFFFFu;                  // two items wait: fence now, flags after the substeps
     if (flush) __threadfence();
-    Sensed snap = sensed(d, v3(0, 0, 0));                          // sensor latency of a whole step: the state the step starts from
+    {   // the K substeps, state in registers: one drone per lane (float) or the lane's two drones as packed pairs (F2)
+        const NPTag<NP> np;
+        Slot& s0 = sl[0]; Slot& s1 = sl[NP - 1];
+#define MDG_PK(f) pack_lanes(np, s0.f, s1.f)
+        Body<T> bd;
+        bd.p = v3t<T>(MDG_PK(d.p.x), MDG_PK(d.p.y), MDG_PK(d.p.z));
+        bd.q.w = MDG_PK(d.q.w); bd.q.x = MDG_PK(d.q.x); bd.q.y = MDG_PK(d.q.y); bd.q.z = MDG_PK(d.q.z);
+        bd.v = v3t<T>(MDG_PK(d.v.x), MDG_PK(d.v.y), MDG_PK(d.v.z));
+        bd.w = v3t<T>(MDG_PK(d.w.x), MDG_PK(d.w.y), MDG_PK(d.w.z));
+        bd.Fwind = v3t<T>(MDG_PK(Fwind.x), MDG_PK(Fwind.y), MDG_PK(Fwind.z));
+        bd.inv_m = MDG_PK(inv_m_e); bd.ng = pack_lanes(np, -s0.g_e, -s1.g_e); bd.ndwc = pack_lanes(np, -s0.dwc_e, -s1.dwc_e);
+        auto load_motor = [&]() {
+            bd.tau_b = v3t<T>(MDG_PK(tau_b.x), MDG_PK(tau_b.y), MDG_PK(tau_b.z));
+            bd.k1_tau = v3t<T>(MDG_PK(k1_tau.x), MDG_PK(k1_tau.y), MDG_PK(k1_tau.z));
+            bd.thrust = MDG_PK(T); bd.cxy = MDG_PK(cxy); bd.dcz = MDG_PK(dcz); bd.gndT = MDG_PK(gndT);
+        };
+        load_motor();
+        bool spun = false;                                         // two envs per lane: some substep was outside the series' range
 #pragma unroll 1
-    for (int k = 0; k < P.K; ++k) {
-        if (F::has(P, F_LAT) && sw == k) {                                 // Q51: the next row arrives at this substep
-            n[0] = n_later[0]; n[1] = n_later[1]; n[2] = n_later[2]; n[3] = n_later[3];
-            if (!lag) motor_model(n);
-        }
-        if (lag) {
+        for (int k = 0; k < P.K; ++k) {
+            if (NP == 1) {                                         // rotor commands that change inside the step: one env per lane only
+                if (F::has(P, F_LAT) && s0.sw == k) {              // Q51: the next row arrives at this substep
 #pragma unroll
-            for (int i = 0; i < 4; ++i) n_act[i] = fmaf(lag_gain, n[i] - n_act[i], n_act[i]);
-            motor_model(n_act);
-        }
-        // S4-S7 world-frame force from the start-of-substep state
-        // b = R(q) z: thrust is T b, and Eq.5's R diag(c_xy, c_xy, c_z) R^T v = c_xy v + (c_z - c_xy)(b.v) b
-        const V3 b = v3(2.0f * fmaf(d.q.x, d.q.z, d.q.w * d.q.y), 2.0f * fmaf(d.q.y, d.q.z, -d.q.w * d.q.x),
-                        fmaf(-2.0f, fmaf(d.q.x, d.q.x, d.q.y * d.q.y), 1.0f));
-        V3 Fw;
-        if (F::has(P, F_DRAG)) {
-            const float s = fmaf(dcz, fmaf(b.x, d.v.x, fmaf(b.y, d.v.y, b.z * d.v.z)), T);
-            Fw = v3(fmaf(s, b.x, cxy * d.v.x), fmaf(s, b.y, cxy * d.v.y), fmaf(s, b.z, cxy * d.v.z));
-        } else Fw = v3(T * b.x, T * b.y, T * b.z);
-        if (F::has(P, F_WIND)) { Fw.x += Fwind.x; Fw.y += Fwind.y; Fw.z += Fwind.z; }
-        if (F::has(P, F_GND)) {                                   // Eq.4, gated on body z pointing up
-            const float hgt = fmaxf(d.p.z, P.h_clip);
-            const float gain = gndT * rcp_fast(hgt * hgt);
-            Fw.z += b.z > 0.0f ? gain : 0.0f;
-        }
-        if (G > 1 && F::has(P, F_DW)) {                           // Eq.6 over every drone above this one
-            // With b' = sqrt(2 ln 2) beta: exp(-dxy^2 / 2 beta^2) = 2^(-dxy^2 / b'^2) and alpha = C1 (r_p/4)^2 / dz_e^2.
-            // One reciprocal r = 1 / (dz_e^2 b'^2) serves both: alpha ~ b'^2 r, exponent = -dxy^2 (dz_e^2 r).
-            // The ramp saturate(dz / dz_clip) is 0 for dz <= 0, which also gates "k above this drone";
-            // b'^2 is floored (beta^2 >= 1e-12), which reproduces the beta -> 0 rule of DESIGN.md Q9.
-            // Pairs are shared out: in round r < G/2 lane j evaluates the pair (j, j + r mod G) once for both ends -
-            // the force goes to whichever drone is lower, the partner's share travels back by one shuffle - and in
-            // round G/2 both ends evaluate their common pair and each keeps its own share.
-            float dw = 0.0f;
+                    for (int i = 0; i < 4; ++i) s0.n[i] = s0.n_later[i];
+                    if (!lag) { motor_model(s0, s0.n); load_motor(); }
+                }
+                if (lag) {
 #pragma unroll
-            for (int r = 1; r <= G / 2; ++r) {
-                const int src = j + r;                             // logical lane inside the G-wide segment (taken mod G)
-                const float ox = __shfl_sync(MDG_FULL, d.p.x, src, G), oy = __shfl_sync(MDG_FULL, d.p.y, src, G),
-                            oz = __shfl_sync(MDG_FULL, d.p.z, src, G);
-                const float dz = oz - d.p.z, dx = ox - d.p.x, dy = oy - d.p.y;
-                const float dxy2 = fmaf(dx, dx, dy * dy);
-                const float adz = fabsf(dz);
-                const float dze = fmaxf(adz, P.dz_floor);
-                const float ramp = __saturatef(adz * P.inv_dz_clip);
-                const float bs = fmaf(P.dw_C2s, dze, P.dw_C3s);
-                const float b2 = fmaxf(bs * bs, P.dw_b2_min), z2 = dze * dze;
-                const float rinv = rcp_fast(z2 * b2);
-                const float ex = ex2_fast(-dxy2 * (z2 * rinv));
-                const float al = ramp * (b2 * rinv);
-                const bool on = (full_group || (j < P.M && ((j + r) & (G - 1)) < P.M)) && dxy2 < 100.0f;
-                const float f = on ? al * ex : 0.0f;
-                const bool above = dz > 0.0f;                      // the partner is above this drone
-                if (r < G / 2) {
-                    const float back = __shfl_sync(MDG_FULL, above ? 0.0f : f, j + G - r, G);
-                    dw += (above ? f : 0.0f) + back;
-                } else dw += above ? f : 0.0f;
+                    for (int i = 0; i < 4; ++i) s0.n_act[i] = fmaf(s0.lag_gain, __fsub_rn(s0.n[i], s0.n_act[i]), s0.n_act[i]);
+                    motor_model(s0, s0.n_act);
+                    load_motor();
+                }
             }
-            Fw.z = fmaf(-dwc_e, dw, Fw.z);
+            const SubstepFlags<T> fl = substep<G, FEAT, DEG>(P, bd, j, full_group);
+            s0.hit |= half_of(fl.below, 0);
+            if (NP == 2) { s1.hit |= half_of(fl.below, 1); spun |= any_(fl.fast); }
+            if (NP == 1 && F::has(P, F_LAT) && k + 1 == P.K - s0.d_obs) {   // what the sensors report d_obs substeps later
+                s0.snap.p = v3(half_of(bd.p.x, 0), half_of(bd.p.y, 0), half_of(bd.p.z, 0));
+                s0.snap.v = v3(half_of(bd.v.x, 0), half_of(bd.v.y, 0), half_of(bd.v.z, 0));
+                s0.snap.w = v3(half_of(bd.w.x, 0), half_of(bd.w.y, 0), half_of(bd.w.z, 0));
+                s0.snap.q.w = half_of(bd.q.w, 0); s0.snap.q.x = half_of(bd.q.x, 0); s0.snap.q.y = half_of(bd.q.y, 0); s0.snap.q.z = half_of(bd.q.z, 0);
+                s0.snap.eta = v3(0, 0, 0);
+            }
         }
-        const V3 acc = v3(Fw.x * inv_m_e, Fw.y * inv_m_e, fmaf(Fw.z, inv_m_e, -g_e));
-
-        // S8 integrate with the wrench frozen in the world frame
-        const bool fast_spin = fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)) > P.w2_exact[DEG - 2];
-        if (!F::has(P, F_EULER)) {
-            d.p.x = fmaf(P.half_h2, acc.x, fmaf(P.h, d.v.x, d.p.x));
-            d.p.y = fmaf(P.half_h2, acc.y, fmaf(P.h, d.v.y, d.p.y));
-            d.p.z = fmaf(P.half_h2, acc.z, fmaf(P.h, d.v.z, d.p.z));
-            d.v.x = fmaf(P.h, acc.x, d.v.x); d.v.y = fmaf(P.h, acc.y, d.v.y); d.v.z = fmaf(P.h, acc.z, d.v.z);
-            if (fast_spin) { const RotState rs = integrate_rot_exact<false>(P, d.q, d.w, tau_b, k1_tau); d.q = rs.q; d.w = rs.w; }
-            else integrate_rot<false, false, DEG>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
-        } else {                                                   // DYN: explicit Euler
-            d.v.x = fmaf(P.h, acc.x, d.v.x); d.v.y = fmaf(P.h, acc.y, d.v.y); d.v.z = fmaf(P.h, acc.z, d.v.z);
-            d.p.x = fmaf(P.h, d.v.x, d.p.x); d.p.y = fmaf(P.h, d.v.y, d.p.y); d.p.z = fmaf(P.h, d.v.z, d.p.z);
-            if (fast_spin) { const RotState rs = integrate_rot_exact<true>(P, d.q, d.w, tau_b, k1_tau); d.q = rs.q; d.w = rs.w; }
-            else integrate_rot<false, true, DEG>(P, d.q, d.w, tau_b, k1_tau, F::has(P, F_AXISYM));
+#undef MDG_PK
+        if (NP == 2 && __any_sync(MDG_FULL, spun)) {               // rare: redo this item's substeps with the exact rotation path
+            float r[2][13];
+#pragma unroll
+            for (int h = 0; h < NP; ++h) {
+                Body<float> b1;
+                b1.tau_b = half3(bd.tau_b, h); b1.k1_tau = half3(bd.k1_tau, h); b1.Fwind = half3(bd.Fwind, h);
+                b1.thrust = half_of(bd.thrust, h); b1.cxy = half_of(bd.cxy, h); b1.dcz = half_of(bd.dcz, h); b1.gndT = half_of(bd.gndT, h);
+                b1.inv_m = half_of(bd.inv_m, h); b1.ng = half_of(bd.ng, h); b1.ndwc = half_of(bd.ndwc, h);
+                const RedoOut o = redo_item_exact<G, FEAT, DEG>(P, S[(st * wpb + wib) * NP + h], b1, lane, j, full_group);
+                sl[h].hit = o.hit;
+#pragma unroll
+                for (int i = 0; i < 13; ++i) r[h][i] = o.s[i];
+            }
+            bd.p = v3t<T>(pack_lanes(np, r[0][0], r[NP - 1][0]), pack_lanes(np, r[0][1], r[NP - 1][1]), pack_lanes(np, r[0][2], r[NP - 1][2]));
+            bd.q.w = pack_lanes(np, r[0][3], r[NP - 1][3]); bd.q.x = pack_lanes(np, r[0][4], r[NP - 1][4]);
+            bd.q.y = pack_lanes(np, r[0][5], r[NP - 1][5]); bd.q.z = pack_lanes(np, r[0][6], r[NP - 1][6]);
+            bd.v = v3t<T>(pack_lanes(np, r[0][7], r[NP - 1][7]), pack_lanes(np, r[0][8], r[NP - 1][8]), pack_lanes(np, r[0][9], r[NP - 1][9]));
+            bd.w = v3t<T>(pack_lanes(np, r[0][10], r[NP - 1][10]), pack_lanes(np, r[0][11], r[NP - 1][11]), pack_lanes(np, r[0][12], r[NP - 1][12]));
         }
-        if (d.p.z < 0.0f) { hit = true; d.p.z = 0.0f; d.v.z = fmaxf(d.v.z, 0.0f); }   // floor
-        if (F::has(P, F_LAT) && k + 1 == P.K - d_obs) snap = sensed(d, v3(0, 0, 0));   // what the sensors report d_obs substeps later
+#pragma unroll
+        for (int h = 0; h < NP; ++h) {
+            DroneRegs& d = sl[h].d;
+            d.p = v3(half_of(bd.p.x, h), half_of(bd.p.y, h), half_of(bd.p.z, h));
+            d.q.w = half_of(bd.q.w, h); d.q.x = half_of(bd.q.x, h); d.q.y = half_of(bd.q.y, h); d.q.z = half_of(bd.q.z, h);
+            d.v = v3(half_of(bd.v.x, h), half_of(bd.v.y, h), half_of(bd.v.z, h));
+            d.w = v3(half_of(bd.w.x, h), half_of(bd.w.y, h), half_of(bd.w.z, h));
+        }
     }
 
     if (flush) { publish_flag(pending); publish_flag(pending2); pending = pending2 = 0xFFFFFFFFu; }
     const unsigned wt_after = take(drawn_l0);
     const unsigned probed_after = probe(wt_after);
-    // S9-S11 epilogue on the end-of-step state
-    const int gbase = lane & ~(G - 1);
-    V3 eta = euler_zyx(d.q);
-    V3 cen = v3(P.term_center[0], P.term_center[1], P.term_center[2]);
-    const bool on_path = F::has(P, F_PATH);
-    if (on_path) {                                                 // PAPER.md:325 (Q52): slots and the distance rule ride on the moving centre
-        cen = path_centre(P, __float_as_uint(env4.w) + 1u);
-        float sn, cs;
-        sincospif(2.0f * (float)jj / (float)P.M, &sn, &cs);
-        tg = make_float4(fmaf(P.form_radius, cs, cen.x), fmaf(P.form_radius, sn, cen.y), cen.z, tg.w);
-    }
-    const int term = F::term(P);
-    const float aphi = fabsf(eta.x), ath = fabsf(eta.y);
-    int flags = 0;                                                 // bit0 terminated, bit1 crash
-    if (term == 1 || term == 3) { if (hit) flags |= 3; if (d.p.z > P.z_max) flags |= 1; }
-    if (term != 0 && (aphi > P.term_tilt || ath > P.term_tilt)) flags |= 3;
-    if (term == 2 || term == 3) {
-        const float dx = d.p.x - cen.x, dy = d.p.y - cen.y, dz = d.p.z - cen.z;
-        if (fmaf(dx, dx, fmaf(dy, dy, dz * dz)) > P.term_dist2) flags |= 1;
-    }
-    const float ex = d.p.x - tg.x, ey = d.p.y - tg.y, ez = d.p.z - tg.z;
-    const float e2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
-    float r;
-    const int rew = F::rew(P);
-    if (rew == 0 || rew == 2) {                                    // Eq.8, summed over drones
-        const float speed = fast_sqrt(fmaf(d.v.x, d.v.x, fmaf(d.v.y, d.v.y, d.v.z * d.v.z)));
-        r = -fabsf(ez) - 0.1f * fast_sqrt(fmaf(ex, ex, ey * ey)) - 0.05f * speed - 0.05f * (aphi + ath);
-        if (e2 < P.at_target_radius2) r += 0.5f;
-        if (flags & 2) r -= 100.0f;
-    } else if (rew == 1) {
-        r = -e2;
-    } else if (rew == 5) {                                         // FlyThroughAviary: capture handled below
-        r = fmaf(P.wp_speed, fast_sqrt(fmaf(d.v.x, d.v.x, fmaf(d.v.y, d.v.y, d.v.z * d.v.z))),
-                 fmaf(-P.wp_shaping, fast_sqrt(e2), -P.wp_omega * fast_sqrt(fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)))));
-    } else if (rew == 4) {                                         // VelocityAviary: target = (v*, omega_z*)
-        const float ux = d.v.x - tg.x, uy = d.v.y - tg.y, uz = d.v.z - tg.z;
-        const float u2 = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
-        r = -fast_sqrt(u2) - 0.1f * fabsf(d.w.z - tg.w) - 0.05f * (aphi + ath);
-        if (u2 < P.at_target_radius2) r += 0.5f;
-    } else {                                                       // formation: pair term below
-        r = -fast_sqrt(e2);
-    }
-    // one pass over the env's drones serves the formation pair term and the adjacency row
-    float adj[G];
+    touched = 0u;
 #pragma unroll
-    for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
-    const bool pairs = G > 1 && rew == 3;
-    if (pairs || F::obs(P) == 1) {
-        float pen = 0.0f;                                          // the self term is |0 - 0| = 0
-#pragma unroll
-        for (int kk = 0; kk < G; ++kk) {
-            const float ox = __shfl_sync(MDG_FULL, d.p.x, gbase + kk), oy = __shfl_sync(MDG_FULL, d.p.y, gbase + kk),
-                        oz = __shfl_sync(MDG_FULL, d.p.z, gbase + kk);
-            const float ax = d.p.x - ox, ay = d.p.y - oy, az = d.p.z - oz;
-            const float d2 = fmaf(ax, ax, fmaf(ay, ay, az * az));
-            adj[kk] = (kk == j || d2 < P.adj_radius2) ? 1.0f : 0.0f;
-            if (pairs) {
-                float ddes;
-                if (F::has(P, F_TGT_CIRCLE)) ddes = P.chord[abs(j - kk)];
-                else {
-                    const float ux = __shfl_sync(MDG_FULL, tg.x, gbase + kk), uy = __shfl_sync(MDG_FULL, tg.y, gbase + kk),
-                                uz = __shfl_sync(MDG_FULL, tg.z, gbase + kk);
-                    const float bx = tg.x - ux, by = tg.y - uy, bz = tg.z - uz;
-                    ddes = fast_sqrt(fmaf(bx, bx, fmaf(by, by, bz * bz)));
-                }
-                pen += (full_group || kk < P.M) ? fabsf(fast_sqrt(d2) - ddes) : 0.0f;
-            }
-        }
-        if (pairs) r = fmaf(-0.25f, pen, r);                       // each unordered pair is seen from both ends
-    }
-    bool captured = false, last_wp = false;
-    if (rew == 5) {
-        captured = e2 < P.wp_radius2;
-        last_wp = (int)tg.w + 1 >= P.wp_total;                     // running index over all laps
-        if (captured) { r += P.wp_bonus; if (last_wp) flags |= 1; }   // the last capture ends the episode
-    }
-    const bool mine = full_group || j < P.M;
-    const float rsum = group_sum<G>(mine ? r : 0.0f);
-    const int gflags = group_or<G>(mine ? flags : 0);
-    const uint32_t ep = __float_as_uint(env4.w) + 1u;
-    const bool truncated = P.ep_steps > 0 && (int)ep >= P.ep_steps;
-    const int done = (gflags & 1) | (truncated ? 2 : 0);
-    uint32_t ep_out = ep;
-    const bool do_reset = done != 0 && P.auto_reset != 0;
-    float4 tg_out = tg;
-    if (rew == 5 && captured && !last_wp) {                        // chase the next waypoint; its index rides in the 4th word
-        const int kn = (int)tg.w + 1, kw = kn % P.n_waypoints;
-        tg_out = make_float4(P.waypoints[3 * kw], P.waypoints[3 * kw + 1], P.waypoints[3 * kw + 2], (float)kn);
-        if (active && !do_reset) B.P6[drone] = tg_out;
-    }
-    if (on_path && active && !do_reset) B.P6[drone] = tg_out;       // mdg_targets shows the slot of the moment
-    if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp
-        if (do_reset) {
-            reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
-            if (F::has(P, F_DR)) {
-                float4 n0, n1, n2, n3;
-                draw_dr(P, e, (uint32_t)jj, t, n0, n1, n2, n3);
-                if (active) { B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3; }
-                if (lag) n_act[0] = n_act[1] = n_act[2] = n_act[3] = P.hover_rpm;
-            }
-            env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
-            eta = euler_zyx(d.q);                                 // zeros unless Table 4's initial attitude range is on
-            if (active) B.P6[drone] = tg_out;
-        }
-        if (F::obs(P) == 1) {                                      // the new episode's first observation
-            float adj_new[G];
-            adjacency<G>(P, d.p, lane, j, adj_new);
-#pragma unroll
-            for (int kk = 0; kk < G; ++kk) adj[kk] = do_reset ? adj_new[kk] : adj[kk];
-        }
-    }
-    if (active) {
-        store_state(B, drone, d);
+    for (int h = 0; h < NP; ++h) {                                // back from the landing zone: controller memory, target, action row, env word
+        Slot& s = sl[h];
+        const WarpStage& W = S[(st * wpb + wib) * NP + h];
+        const float4 f = W.plane[3][lane];
+        s.d.Ip = v3(f.y, f.z, f.w);
         if (pid) {
-            B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
-            if (F::act(P) == 1) B.P5[drone] = d.sp;
+            const float4 i4 = W.plane[4][lane];
+            s.d.Ie = v3(i4.x, i4.y, i4.z);
+            touched |= __float_as_uint(i4.x);
+            if (F::act(P) == 1) { s.d.sp = W.plane[5][lane]; touched |= __float_as_uint(s.d.sp.x); }
         }
-        Sensed sn = sensed(d, eta);
-        if (F::has(P, F_LAT) && !do_reset) { sn = snap; sn.eta = euler_zyx(snap.q); }   // a new episode's first row is its initial state
-        if (F::has(P, F_SENS)) sense(P, e, (uint32_t)jj, t, ep_out, sn);   // Table 4 sensor rows: the stored state stays exact
-        write_obs<G>(P, B.obs, drone, d, sn, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
-        B.reward_d[drone] = r;
-        if (lag) B.N0[drone] = make_float4(n_act[0], n_act[1], n_act[2], n_act[3]);
-        if (j == 0) {
-            env4.w = __uint_as_float(ep_out);
-            B.E0[e] = env4; B.gstep[e] = t;
-            B.reward[e] = rsum; B.done[e] = (uint8_t)done;
-            if (F::has(P, F_WIND_MIX) && (P.wind_mask & 4) && F::has(P, F_WIND)) B.E1[e] = do_reset ? make_float4(0, 0, 0, 1.0f) : gust_out;
+        s.tg = W.plane[6][lane];
+        s.act4 = W.plane[7][lane];
+        s.env4 = W.plane[8][lane];
+        touched |= __float_as_uint(f.y) | __float_as_uint(s.tg.x) | __float_as_uint(s.act4.x) | __float_as_uint(s.env4.x);
+    }
+    // one landing zone: it is free now; the next item's copies overlap the epilogue
+    if (!flip && wt_next < n_items) { await_item(wt_next, probed_next); prefetch(wt_next, st, touched & P.zero); }
+#pragma unroll
+    for (int h = 0; h < NP; ++h) {
+        Slot& s = sl[h];
+        DroneRegs& d = s.d;
+        float4& env4 = s.env4;
+        float4& tg = s.tg;
+        const float4 act4 = s.act4;
+        const unsigned e = s.e;
+        const uint32_t t = s.t;
+        const size_t drone = s.drone;
+        const bool active = s.active, hit = s.hit;
+        float (&n_act)[4] = s.n_act;
+        const float4 gust_out = s.gust_out;
+        const Sensed snap = s.snap;
+        // S9-S11 epilogue on the end-of-step state
+        const int gbase = lane & ~(G - 1);
+        V3 eta = euler_zyx(d.q);
+        V3 cen = v3(P.term_center[0], P.term_center[1], P.term_center[2]);
+        const bool on_path = F::has(P, F_PATH);
+        if (on_path) {                                                 // PAPER.md:325 (Q52): slots and the distance rule ride on the moving centre
+            cen = path_centre(P, __float_as_uint(env4.w) + 1u);
+            float sn, cs;
+            sincospif(2.0f * (float)jj / (float)P.M, &sn, &cs);
+            tg = make_float4(fmaf(P.form_radius, cs, cen.x), fmaf(P.form_radius, sn, cen.y), cen.z, tg.w);
+        }
+        const int term = F::term(P);
+        const float aphi = fabsf(eta.x), ath = fabsf(eta.y);
+        int flags = 0;                                                 // bit0 terminated, bit1 crash
+        if (term == 1 || term == 3) { if (hit) flags |= 3; if (d.p.z > P.z_max) flags |= 1; }
+        if (term != 0 && (aphi > P.term_tilt || ath > P.term_tilt)) flags |= 3;
+        if (term == 2 || term == 3) {
+            const float dx = d.p.x - cen.x, dy = d.p.y - cen.y, dz = d.p.z - cen.z;
+            if (fmaf(dx, dx, fmaf(dy, dy, dz * dz)) > P.term_dist2) flags |= 1;
+        }
+        const float ex = d.p.x - tg.x, ey = d.p.y - tg.y, ez = d.p.z - tg.z;
+        const float e2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
+        float r;
+        const int rew = F::rew(P);
+        if (rew == 0 || rew == 2) {                                    // Eq.8, summed over drones
+            const float speed = fast_sqrt(fmaf(d.v.x, d.v.x, fmaf(d.v.y, d.v.y, d.v.z * d.v.z)));
+            r = -fabsf(ez) - 0.1f * fast_sqrt(fmaf(ex, ex, ey * ey)) - 0.05f * speed - 0.05f * (aphi + ath);
+            if (e2 < P.at_target_radius2) r += 0.5f;
+            if (flags & 2) r -= 100.0f;
+        } else if (rew == 1) {
+            r = -e2;
+        } else if (rew == 5) {                                         // FlyThroughAviary: capture handled below
+            r = fmaf(P.wp_speed, fast_sqrt(fmaf(d.v.x, d.v.x, fmaf(d.v.y, d.v.y, d.v.z * d.v.z))),
+                     fmaf(-P.wp_shaping, fast_sqrt(e2), -P.wp_omega * fast_sqrt(fmaf(d.w.x, d.w.x, fmaf(d.w.y, d.w.y, d.w.z * d.w.z)))));
+        } else if (rew == 4) {                                         // VelocityAviary: target = (v*, omega_z*)
+            const float ux = d.v.x - tg.x, uy = d.v.y - tg.y, uz = d.v.z - tg.z;
+            const float u2 = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
+            r = -fast_sqrt(u2) - 0.1f * fabsf(d.w.z - tg.w) - 0.05f * (aphi + ath);
+            if (u2 < P.at_target_radius2) r += 0.5f;
+        } else {                                                       // formation: pair term below
+            r = -fast_sqrt(e2);
+        }
+        // one pass over the env's drones serves the formation pair term and the adjacency row
+        float adj[G];
+    #pragma unroll
+        for (int kk = 0; kk < G; ++kk) adj[kk] = 0.0f;
+        const bool pairs = G > 1 && rew == 3;
+        if (pairs || F::obs(P) == 1) {
+            float pen = 0.0f;                                          // the self term is |0 - 0| = 0
+    #pragma unroll
+            for (int kk = 0; kk < G; ++kk) {
+                const float ox = __shfl_sync(MDG_FULL, d.p.x, gbase + kk), oy = __shfl_sync(MDG_FULL, d.p.y, gbase + kk),
+                            oz = __shfl_sync(MDG_FULL, d.p.z, gbase + kk);
+                const float ax = d.p.x - ox, ay = d.p.y - oy, az = d.p.z - oz;
+                const float d2 = fmaf(ax, ax, fmaf(ay, ay, az * az));
+                adj[kk] = (kk == j || d2 < P.adj_radius2) ? 1.0f : 0.0f;
+                if (pairs) {
+                    float ddes;
+                    if (F::has(P, F_TGT_CIRCLE)) ddes = P.chord[abs(j - kk)];
+                    else {
+                        const float ux = __shfl_sync(MDG_FULL, tg.x, gbase + kk), uy = __shfl_sync(MDG_FULL, tg.y, gbase + kk),
+                                    uz = __shfl_sync(MDG_FULL, tg.z, gbase + kk);
+                        const float bx = tg.x - ux, by = tg.y - uy, bz = tg.z - uz;
+                        ddes = fast_sqrt(fmaf(bx, bx, fmaf(by, by, bz * bz)));
+                    }
+                    pen += (full_group || kk < P.M) ? fabsf(fast_sqrt(d2) - ddes) : 0.0f;
+                }
+            }
+            if (pairs) r = fmaf(-0.25f, pen, r);                       // each unordered pair is seen from both ends
+        }
+        bool captured = false, last_wp = false;
+        if (rew == 5) {
+            captured = e2 < P.wp_radius2;
+            last_wp = (int)tg.w + 1 >= P.wp_total;                     // running index over all laps
+            if (captured) { r += P.wp_bonus; if (last_wp) flags |= 1; }   // the last capture ends the episode
+        }
+        const bool mine = full_group || j < P.M;
+        const float rsum = group_sum<G>(mine ? r : 0.0f);
+        const int gflags = group_or<G>(mine ? flags : 0);
+        const uint32_t ep = __float_as_uint(env4.w) + 1u;
+        const bool truncated = P.ep_steps > 0 && (int)ep >= P.ep_steps;
+        const int done = (gflags & 1) | (truncated ? 2 : 0);
+        uint32_t ep_out = ep;
+        const bool do_reset = done != 0 && P.auto_reset != 0;
+        float4 tg_out = tg;
+        if (rew == 5 && captured && !last_wp) {                        // chase the next waypoint; its index rides in the 4th word
+            const int kn = (int)tg.w + 1, kw = kn % P.n_waypoints;
+            tg_out = make_float4(P.waypoints[3 * kw], P.waypoints[3 * kw + 1], P.waypoints[3 * kw + 2], (float)kn);
+            if (active && !do_reset) B.P6[drone] = tg_out;
+        }
+        if (on_path && active && !do_reset) B.P6[drone] = tg_out;       // mdg_targets shows the slot of the moment
+        if (__any_sync(MDG_FULL, do_reset)) {                          // S12 same-call auto-reset: rare, taken by the whole warp
+            if (do_reset) {
+                reset_drone(P, e, (uint32_t)jj, t, d, tg_out);
+                if (F::has(P, F_DR)) {
+                    float4 n0, n1, n2, n3;
+                    draw_dr(P, e, (uint32_t)jj, t, n0, n1, n2, n3);
+                    if (active) { B.R0[drone] = n0; B.R1[drone] = n1; B.R2[drone] = n2; B.R3[drone] = n3; }
+                    if (lag) n_act[0] = n_act[1] = n_act[2] = n_act[3] = P.hover_rpm;
+                }
+                env4.x = env4.y = env4.z = 0.0f; ep_out = 0u;
+                eta = euler_zyx(d.q);                                 // zeros unless Table 4's initial attitude range is on
+                if (active) B.P6[drone] = tg_out;
+            }
+            if (F::obs(P) == 1) {                                      // the new episode's first observation
+                float adj_new[G];
+                adjacency<G>(P, d.p, lane, j, adj_new);
+    #pragma unroll
+                for (int kk = 0; kk < G; ++kk) adj[kk] = do_reset ? adj_new[kk] : adj[kk];
+            }
+        }
+        if (active) {
+            store_state(B, drone, d);
+            if (pid) {
+                B.P4[drone] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
+                if (F::act(P) == 1) B.P5[drone] = d.sp;
+            }
+            Sensed sn = sensed(d, eta);
+            if (F::has(P, F_LAT) && !do_reset) { sn = snap; sn.eta = euler_zyx(snap.q); }   // a new episode's first row is its initial state
+            if (F::has(P, F_SENS)) sense(P, e, (uint32_t)jj, t, ep_out, sn);   // Table 4 sensor rows: the stored state stays exact
+            write_obs<G>(P, B.obs, drone, d, sn, adj, F::obs(P), do_reset ? make_float4(0, 0, 0, 0) : act4, tg_out);
+            B.reward_d[drone] = r;
+            if (lag) B.N0[drone] = make_float4(n_act[0], n_act[1], n_act[2], n_act[3]);
+            if (j == 0) {
+                env4.w = __uint_as_float(ep_out);
+                B.E0[e] = env4; B.gstep[e] = t;
+                B.reward[e] = rsum; B.done[e] = (uint8_t)done;
+                if (F::has(P, F_WIND_MIX) && (P.wind_mask & 4) && F::has(P, F_WIND)) B.E1[e] = do_reset ? make_float4(0, 0, 0, 1.0f) : gust_out;
+            }
         }
     }
     if (pending == 0xFFFFFFFFu) pending = wt; else pending2 = wt;
     if (wt_next >= n_items) break;
-    wt = wt_next; wt_next = wt_after; probed_next = probed_after; st ^= 1;
+    wt = wt_next; wt_next = wt_after; probed_next = probed_after; st ^= flip;
     }   // work-item loop
     __threadfence();
     publish_flag(pending);
