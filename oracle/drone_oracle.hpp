@@ -202,6 +202,12 @@ inline Derived derive(const Params& P, int physics_mode) {
     return d;
 }
 
+// Phase marker for the flop tally of oracle_capi.cpp (a no-op for the simulation itself)
+#ifndef ORC_PHASE
+#define ORC_PHASE(k)
+#endif
+enum { PH_WIND = 0, PH_DECODE, PH_MOTOR, PH_WRENCH, PH_INTEGRATE, PH_OBS, PH_REWARD, PH_N };
+
 // ---- small linear algebra on scalar type R -----------------------------------------------------
 template <class R> inline double to_d(const R& x) { return (double)x; }
 
@@ -783,6 +789,7 @@ struct Sim {
         load(e, dr);
         const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
         // O9 wind gust (PAPER.md:203 recursion, Q27), once per control step, before the substeps
+        ORC_PHASE(PH_WIND);
         if (D.aero & AERO_WIND) {
             R w[3] = {0.0, 0.0, 0.0};                              // air velocity seen by the env's drones
             if (P.wind_mask & WIND_DRYDEN) {
@@ -831,6 +838,7 @@ struct Sim {
                 for (int a = 0; a < 3; ++a) dr[i].Fwind[a] = (drag ? (P.k_wind * nr) * rel[a] : R(0.0)) + fs[a];
             }
         }
+        ORC_PHASE(PH_DECODE);
         // Table 4 latency rows (Q51): this episode's delays in physics substeps, drawn at the reset index t0 of the episode
         const bool lat_a = P.act_latency_hi > 0.0, lat_s = P.obs_latency_hi > 0.0;
         std::vector<int> d_act(M, 0), d_obs(M, 0), sw(M, -1);
@@ -877,12 +885,15 @@ struct Sim {
                     if (dr[i].n[a] > D.max_rpm * dr[i].sc[DR_MAXRPM]) dr[i].n[a] = D.max_rpm * dr[i].sc[DR_MAXRPM];
                     if (sw[i] >= 0 && later[i].n[a] > D.max_rpm * dr[i].sc[DR_MAXRPM]) later[i].n[a] = D.max_rpm * dr[i].sc[DR_MAXRPM];
                 }
+            ORC_PHASE(PH_MOTOR);
             motor_wrench(P, D, dr[i].n, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
+            ORC_PHASE(PH_DECODE);
         }
         if (lat_s) for (int i = 0; i < M; ++i) if (d_obs[i] >= D.K) snap[i] = dr[i];   // a full step old: the state the step starts from
         // K substeps: all wrenches from the same start-of-substep state, then integrate
         const bool lag = P.motor_lag_hi > 0.0;
         for (int k = 0; k < D.K; ++k) {
+            ORC_PHASE(PH_MOTOR);
             for (int i = 0; i < M; ++i)
                 if (sw[i] == k) {                                  // Q51: the next row arrives at this substep
                     for (int a = 0; a < 4; ++a) dr[i].n[a] = later[i].n[a];
@@ -894,11 +905,14 @@ struct Sim {
                     for (int a = 0; a < 4; ++a) dr[i].n_act[a] = dr[i].n_act[a] + gam * (dr[i].n[a] - dr[i].n_act[a]);
                     motor_wrench(P, D, dr[i].n_act, dr[i].T, dr[i].tau_b, dr[i].Om, dr[i].sc);
                 }
+            ORC_PHASE(PH_WRENCH);
             for (int i = 0; i < M; ++i) substep_wrench(P, D, dr, M, i);
+            ORC_PHASE(PH_INTEGRATE);
             for (int i = 0; i < M; ++i) integrate(P, D, dr[i]);
             if (lat_s) for (int i = 0; i < M; ++i) if (k + 1 == D.K - d_obs[i]) snap[i] = dr[i];   // what the sensors report d_obs substeps later
         }
         store(e, dr);
+        ORC_PHASE(PH_REWARD);
         // O10 reward / termination from the end-of-step state
         const bool use_floor = P.term_mode == TERM_HOVER || P.term_mode == TERM_FORMATION;
         const bool use_tilt = P.term_mode != TERM_NONE;
@@ -1002,6 +1016,7 @@ struct Sim {
             fresh = true;                                          // the new episode's first row is its initial state
         }
         double m_adj;
+        ORC_PHASE(PH_OBS);
         if (lat_s && !fresh) {
             for (int i = 0; i < M; ++i) { for (int a = 0; a < 4; ++a) { snap[i].tg[a] = dr[i].tg[a]; snap[i].act[a] = dr[i].act[a]; } }
             write_obs(e, dr, m_adj, t, snap.data());

@@ -32,6 +32,9 @@ def lib():
         L.orc_step.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.orc_flop_tally.restype = C.c_uint64
         L.orc_flop_tally.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_flop_parts.argtypes = [C.c_void_p]
+        L.orc_count_flops.restype = C.c_uint64
+        L.orc_count_flops.argtypes = [C.c_char_p]
         for n in ("state", "pid", "targets", "wind", "ep_step", "dr", "gust", "rotor"):
             getattr(L, "orc_get_" + n).argtypes = [C.c_void_p, C.c_void_p]
             getattr(L, "orc_set_" + n).argtypes = [C.c_void_p, C.c_void_p]
@@ -97,6 +100,17 @@ class OracleParams:
             self._h = None
 
 
+FLOP_PHASES = ("wind", "decode", "motor", "wrench", "integrate", "obs", "reward")
+
+
+def count_flops(name):
+    """Flops of one call of a building block of the oracle on its counting scalar (oracle_capi.cpp: orc_count_flops)."""
+    n = int(lib().orc_count_flops(name.encode()))
+    if n == 2 ** 64 - 1:
+        raise KeyError(name)
+    return n
+
+
 class OracleEnv:
     """The batched env of SURVEY.md §8(b) computed by the float64 oracle."""
 
@@ -126,6 +140,14 @@ class OracleEnv:
         a = np.ascontiguousarray(actions, dtype=np.float32).reshape(-1)
         assert a.size == self.N * self.M * 4
         return int(lib().orc_flop_tally(self._h, _p(a)))
+
+    def flop_parts(self, actions):
+        """The tally of flop_tally(actions) by phase of the control step (drone_oracle.hpp: PH_*)."""
+        total = self.flop_tally(actions)
+        out = np.zeros(len(FLOP_PHASES), dtype=np.uint64)
+        lib().orc_flop_parts(_p(out))
+        assert int(out.sum()) == total
+        return dict(zip(FLOP_PHASES, (int(x) for x in out)))
 
     def _get(self, name, shape, dtype=np.float64):
         out = np.zeros(shape, dtype=dtype)

@@ -5,6 +5,9 @@
 #include <cstdlib>
 #include <string>
 #include <thread>
+// flop tally by phase of the control step: the oracle's header marks the phases, this file counts (drone_oracle.hpp: ORC_PHASE)
+namespace orc { static thread_local int g_phase = 0; }
+#define ORC_PHASE(k) (::orc::g_phase = (k))
 #include "drone_oracle.hpp"
 #include "camera_oracle.hpp"
 
@@ -13,26 +16,28 @@ namespace orc {
 // Counting scalar: every add, sub, mul, div, compare and elementary function is one flop (an FMA is
 // therefore two); negation, fabs and conversions are free.  SURVEY.md §8(d) counting rule.
 static thread_local uint64_t g_flops = 0;
+static thread_local uint64_t g_parts[PH_N] = {0};
+#define ORC_TICK() (++g_flops, ++g_parts[g_phase])
 struct Counted {
     double v;
     Counted() : v(0) {}
     Counted(double x) : v(x) {}
     explicit operator double() const { return v; }
-    friend Counted operator+(const Counted& a, const Counted& b) { ++g_flops; return Counted(a.v + b.v); }
-    friend Counted operator-(const Counted& a, const Counted& b) { ++g_flops; return Counted(a.v - b.v); }
-    friend Counted operator*(const Counted& a, const Counted& b) { ++g_flops; return Counted(a.v * b.v); }
-    friend Counted operator/(const Counted& a, const Counted& b) { ++g_flops; return Counted(a.v / b.v); }
+    friend Counted operator+(const Counted& a, const Counted& b) { ORC_TICK(); return Counted(a.v + b.v); }
+    friend Counted operator-(const Counted& a, const Counted& b) { ORC_TICK(); return Counted(a.v - b.v); }
+    friend Counted operator*(const Counted& a, const Counted& b) { ORC_TICK(); return Counted(a.v * b.v); }
+    friend Counted operator/(const Counted& a, const Counted& b) { ORC_TICK(); return Counted(a.v / b.v); }
     friend Counted operator-(const Counted& a) { return Counted(-a.v); }
-    friend bool operator<(const Counted& a, const Counted& b) { ++g_flops; return a.v < b.v; }
-    friend bool operator>(const Counted& a, const Counted& b) { ++g_flops; return a.v > b.v; }
+    friend bool operator<(const Counted& a, const Counted& b) { ORC_TICK(); return a.v < b.v; }
+    friend bool operator>(const Counted& a, const Counted& b) { ORC_TICK(); return a.v > b.v; }
 };
-inline Counted sqrt(const Counted& a) { ++g_flops; return Counted(std::sqrt(a.v)); }
-inline Counted sin(const Counted& a) { ++g_flops; return Counted(std::sin(a.v)); }
-inline Counted cos(const Counted& a) { ++g_flops; return Counted(std::cos(a.v)); }
-inline Counted exp(const Counted& a) { ++g_flops; return Counted(std::exp(a.v)); }
-inline Counted log(const Counted& a) { ++g_flops; return Counted(std::log(a.v)); }
-inline Counted asin(const Counted& a) { ++g_flops; return Counted(std::asin(a.v)); }
-inline Counted atan2(const Counted& a, const Counted& b) { ++g_flops; return Counted(std::atan2(a.v, b.v)); }
+inline Counted sqrt(const Counted& a) { ORC_TICK(); return Counted(std::sqrt(a.v)); }
+inline Counted sin(const Counted& a) { ORC_TICK(); return Counted(std::sin(a.v)); }
+inline Counted cos(const Counted& a) { ORC_TICK(); return Counted(std::cos(a.v)); }
+inline Counted exp(const Counted& a) { ORC_TICK(); return Counted(std::exp(a.v)); }
+inline Counted log(const Counted& a) { ORC_TICK(); return Counted(std::log(a.v)); }
+inline Counted asin(const Counted& a) { ORC_TICK(); return Counted(std::asin(a.v)); }
+inline Counted atan2(const Counted& a, const Counted& b) { ORC_TICK(); return Counted(std::atan2(a.v, b.v)); }
 inline Counted fabs(const Counted& a) { return Counted(std::fabs(a.v)); }
 
 static void run_threads(Sim& s, const float* actions, uint32_t t, int n_threads) {
@@ -122,7 +127,47 @@ void orc_step(void* h, const float* actions, int n_threads) {
 uint64_t orc_flop_tally(const void* h, const float* actions) {
     Sim copy = *(const Sim*)h;
     g_flops = 0;
+    for (int k = 0; k < PH_N; ++k) g_parts[k] = 0;
     copy.step_range<Counted>(0, copy.N, actions, copy.gstep + 1);
+    return g_flops;
+}
+// the same tally by phase (PH_* of drone_oracle.hpp: wind, decode, motor model, substep wrench, integrator, observation,
+// reward + termination), filled by the last orc_flop_tally of this thread
+void orc_flop_parts(uint64_t* out) { for (int k = 0; k < PH_N; ++k) out[k] = g_parts[k]; }
+// flops of ONE call of a building block of the oracle on the counting scalar, on generic (non-degenerate) arguments:
+// what tests/test_oracle_flop_tally.py compares with hand counts of the formulas
+uint64_t orc_count_flops(const char* name) {
+    Params P; default_params(MODEL_CF2X, P);
+    const Derived D = derive(P, PHYS_MJC);
+    Counted q[4] = {0.9, 0.1, -0.2, 0.3}, a3[3] = {0.3, -0.4, 0.5}, b3[3] = {0.7, 0.2, -0.6}, o3[3], o4[4], M[3][3];
+    Counted b4[4] = {0.8, -0.3, 0.4, 0.1};
+    const std::string n(name);
+    g_flops = 0;
+    if (n == "cross") cross(a3, b3, o3);
+    else if (n == "mat_vec") { rotmat(q, M); g_flops = 0; mat_vec(M, a3, o3); }
+    else if (n == "matT_vec") { rotmat(q, M); g_flops = 0; matT_vec(M, a3, o3); }
+    else if (n == "rotmat") rotmat(q, M);
+    else if (n == "quat_mul") quat_mul(q, b4, o4);
+    else if (n == "quat_exp_step") quat_exp_step(q, a3, o4);
+    else if (n == "quat_normalise") quat_normalise(q);
+    else if (n == "euler_zyx") euler_zyx(q, o3);
+    else if (n == "ang_acc") ang_acc(P, q, a3, b3, o3);
+    else if (n == "motor_wrench") { Counted nn[4] = {14000.0, 14100.0, 14200.0, 14300.0}, T, tau[3], Om; motor_wrench(P, D, nn, T, tau, Om); }
+    else if (n == "alloc_inverse") { Counted T = 0.26, s[4]; alloc_inverse(P, D, T, a3, s); }
+    else if (n == "clampR_inside") { Counted x = 0.5; (void)clampR(x, 0.0, 1.0); }
+    else if (n == "wrap_pi") { Counted x = 4.0; (void)wrap_pi(x); }
+    else if (n == "integrate_rk4" || n == "integrate_euler") {
+        Params P2 = P; P2.integrator = n == "integrate_rk4" ? INTEG_RK4 : INTEG_EULER;
+        const Derived D2 = derive(P2, PHYS_MJC);
+        Drone<Counted> d;
+        for (int i = 0; i < 3; ++i) { d.p[i] = 1.0 + 0.1 * i; d.v[i] = 0.2 - 0.1 * i; d.w[i] = 0.5 + 0.3 * i; d.Fw[i] = 0.05 * (i + 1); d.tw[i] = 1e-4 * (i + 1); }
+        for (int i = 0; i < 4; ++i) d.q[i] = q[i];
+        for (int i = 0; i < DR_N; ++i) d.sc[i] = 1.0;
+        d.hit = false; d.min_abs_pz = 1e30;
+        quat_normalise(d.q);
+        g_flops = 0;
+        integrate(P2, D2, d);
+    } else return ~0ull;
     return g_flops;
 }
 
