@@ -255,7 +255,7 @@ __device__ __forceinline__ F2 fma_(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %
 __device__ __forceinline__ F2 mul_(F2 a, F2 b) { F2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
 __device__ __forceinline__ F2 add_(F2 a, F2 b) { F2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
 __device__ __forceinline__ F2 sub_(F2 a, F2 b) { F2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ F2 neg_(F2 a) { F2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(0xBF800000BF800000ull)); return r; }   // x * -1: exact, one FMUL2
+__device__ __forceinline__ F2 neg_(F2 a) { F2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(0xBF800000BF800000ull)); return r; }   // x * -1: exact, one FMUL2 (two sign flips on the ALU pipe measured slower)
 // uniform (float) operands broadcast to both halves
 __device__ __forceinline__ F2 fma_(float a, F2 b, F2 c) { return fma_(pk(a, a), b, c); }
 __device__ __forceinline__ F2 fma_(F2 a, float b, F2 c) { return fma_(a, pk(b, b), c); }

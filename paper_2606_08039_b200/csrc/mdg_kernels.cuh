@@ -281,6 +281,17 @@ __device__ __noinline__ RedoOut redo_item_exact(const DevParams& P, const WarpSt
     return o;
 }
 
+// S7: one AR(1) step of an env's gust, w <- alpha w + sigma sqrt(1 - alpha^2) xi, xi from one Philox draw at
+// (env, ~0, t, stream 2).  Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact
+// in fp32; cos / sin(2 pi u_b) = -cos / sin(2 pi (u_b - 1/2)) keeps the MUFU argument in [-pi, pi).
+__device__ __forceinline__ V3 gust_update(const DevParams& P, unsigned e, uint32_t t, V3 w, float wa, float wg) {
+    const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
+    const float r1 = -fast_sqrt(__fmul_rn(-1.38629436f, lg2_fast(__fsub_rn(1.0f, u01(r.x))))), r2 = -fast_sqrt(__fmul_rn(-1.38629436f, lg2_fast(__fsub_rn(1.0f, u01(r.z)))));
+    const float a1 = __fmul_rn(6.28318531f, __fsub_rn(u01(r.y), 0.5f)), a2 = __fmul_rn(6.28318531f, __fsub_rn(u01(r.w), 0.5f));
+    return v3(fmaf(wa, w.x, __fmul_rn(wg, __fmul_rn(r1, cos_fast(a1)))), fmaf(wa, w.y, __fmul_rn(wg, __fmul_rn(r1, sin_fast(a1)))),
+              fmaf(wa, w.z, __fmul_rn(wg, __fmul_rn(r2, cos_fast(a2)))));
+}
+
 // What one lane carries for one of its NP env slots from the prologue to the epilogue of a work item.
 struct Slot {
     unsigned e; bool active; size_t drone;
@@ -460,6 +471,21 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         s.gndT = __fmul_rn(dr ? __fmul_rn(P.gnd_coef, s.dr1.y) : P.gnd_coef, s.T);
         s.dcz = __fsub_rn(cz, s.cxy);
     };
+    // Two envs per lane and at least two lanes per env: the AR(1) gust of an env is the same for all its lanes, so lane j draws
+    // it for env slot j & 1 only and the group's lanes 0 and 1 hand their results round (six shuffles instead of a second
+    // Philox + Box-Muller per lane; the arithmetic is gust_update either way).
+    const bool share_gust = NP == 2 && G >= 2 && F::has(P, F_WIND) && !F::has(P, F_WIND_MIX);
+    float gust_x[NP], gust_y[NP], gust_z[NP];
+    if (share_gust) {
+        const int hs = j & 1;
+        const Slot& s0 = sl[0]; const Slot& s1 = sl[NP - 1];
+        const V3 mine = gust_update(P, hs ? s1.e : s0.e, hs ? s1.t : s0.t,
+                                    hs ? v3(s1.env4.x, s1.env4.y, s1.env4.z) : v3(s0.env4.x, s0.env4.y, s0.env4.z), P.wind_alpha, P.wind_gain);
+#pragma unroll
+        for (int h = 0; h < NP; ++h) {
+            gust_x[h] = __shfl_sync(MDG_FULL, mine.x, h, G); gust_y[h] = __shfl_sync(MDG_FULL, mine.y, h, G); gust_z[h] = __shfl_sync(MDG_FULL, mine.z, h, G);
+        }
+    }
 #pragma unroll
     for (int h = 0; h < NP; ++h) {
         Slot& s = sl[h];
@@ -470,9 +496,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         const float4 act4 = s.act4;
         const size_t drone = s.drone;
         const bool active = s.active;
-        // S7 wind gust: one AR(1) update per env and control step, force held over the substeps.
-        // Box-Muller on (1 - u_a, u_b): r = sqrt(-2 ln(1 - u_a)) = sqrt(-2 ln2 lg2(1 - u_a)); 1 - u_a is exact in
-        // fp32; cos/sin(2 pi u_b) = -cos/sin(2 pi (u_b - 1/2)) keeps the MUFU argument in [-pi, pi).
+        // S7 wind gust: one AR(1) update per env and control step (gust_update), force held over the substeps.
         V3 Fwind = v3(0, 0, 0);
         float4 gust_out = make_float4(0, 0, 0, 1.0f);                  // E1 after this step (generic kernel, MDG_WIND_GUST only)
         if (F::has(P, F_WIND)) {
@@ -480,19 +504,18 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             const int wmask = F::has(P, F_WIND_MIX) ? P.wind_mask : 1;
             V3 u = v3(0, 0, 0);                                        // air velocity
             if (wmask & 1) {
-                const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_WIND, P.seed_lo, P.seed_hi);
-                const float r1 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.x))), r2 = -fast_sqrt(-1.38629436f * lg2_fast(1.0f - u01(r.z)));
-                const float a1 = 6.28318531f * (u01(r.y) - 0.5f), a2 = 6.28318531f * (u01(r.w) - 0.5f);
-                float wa = P.wind_alpha, wg = P.wind_gain;
-                if (F::has(P, F_WIND_MIX) && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
-                    const float hm = fmaxf(group_sum<G>((full_group || j < P.M) ? d.p.z : 0.0f) * P.inv_M, P.dryden_h_min);   // alpha = exp(-dt V / L)
-                    const float x = P.dryden_x * powf(fmaf(8.23e-4f, hm, 0.177f), 1.2f) / hm;
-                    wa = expf(-x);
-                    wg = P.wind_sigma * sqrtf(-expm1f(-2.0f * x));    // sigma sqrt(1 - alpha^2) without the cancellation
+                if (share_gust) { env4.x = gust_x[h]; env4.y = gust_y[h]; env4.z = gust_z[h]; }   // drawn once per env, above
+                else {
+                    float wa = P.wind_alpha, wg = P.wind_gain;
+                    if (F::has(P, F_WIND_MIX) && P.dryden_x > 0.0f) {                  // PAPER.md:202 (Q50): L_u(h) at the env's mean altitude,
+                        const float hm = fmaxf(group_sum<G>((full_group || j < P.M) ? d.p.z : 0.0f) * P.inv_M, P.dryden_h_min);   // alpha = exp(-dt V / L)
+                        const float x = P.dryden_x * powf(fmaf(8.23e-4f, hm, 0.177f), 1.2f) / hm;
+                        wa = expf(-x);
+                        wg = P.wind_sigma * sqrtf(-expm1f(-2.0f * x));    // sigma sqrt(1 - alpha^2) without the cancellation
+                    }
+                    const V3 wn = gust_update(P, e, t, v3(env4.x, env4.y, env4.z), wa, wg);
+                    env4.x = wn.x; env4.y = wn.y; env4.z = wn.z;
                 }
-                env4.x = fmaf(wa, env4.x, wg * (r1 * cos_fast(a1)));
-                env4.y = fmaf(wa, env4.y, wg * (r1 * sin_fast(a1)));
-                env4.z = fmaf(wa, env4.z, wg * (r2 * cos_fast(a2)));
                 u = v3(env4.x, env4.y, env4.z);
             }
             if (wmask & 2) { u.x += P.wind_const[0]; u.y += P.wind_const[1]; u.z += P.wind_const[2]; }
