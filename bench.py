@@ -254,7 +254,7 @@ def run_ours(args, wl, c):
         K = -(-K // GRAPH_STEPS) * GRAPH_STEPS                              # whole graphs
     stream = torch.cuda.Stream()
     ha = harness_actions(wl)
-    A = 4                                                  # distinct action sets per replica
+    A = GRAPH_STEPS // REPLICAS                            # distinct action sets per replica (12: a short period lets open-loop rotor commands pump the body rates)
     envs, acts = [], []
     with torch.cuda.stream(stream):
         for r in range(REPLICAS):
