@@ -515,8 +515,9 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     if (rc == MDG_OK && h->saturating) {     // throughput-bound batch: register budget (resident 128-thread blocks per SM) as measured fastest
         const bool generic = h->kernel_name.find("generic") != std::string::npos;
         // 6 for the benchmark specialisations (80 registers: only the integrated state and the frozen wrench live across the substep
-        // loop); 4 where Table 4's planes and draws would spill; the runtime-flag kernel needs 162 registers to stay out of local memory (3)
-        h->minb = generic ? 3 : (h->P.feat & (F_DR | F_MLAG | F_LAT | F_SENS)) ? 4 : 6;   // jit kernels follow the same rule
+        // loop); 4 where the motor lag / latency rows keep rotor commands and history rows live as well (measured: 45.0 vs 50.9 us at 5);
+        // the runtime-flag kernel needs 162 registers to stay out of local memory (3)
+        h->minb = generic ? 3 : (h->P.feat & (F_MLAG | F_LAT)) ? 4 : 6;   // jit kernels follow the same rule
         pick_kernels(h);
         rc = configure_launch(h);
     }
@@ -524,7 +525,10 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     // an issue-bound kernel gains from the halved instruction count, a latency-bound one would only lose parallelism.
     int want_lanes = 0;
     if (const char* ev = std::getenv("MDG_LANES")) want_lanes = ev[0] == '2' ? 2 : 1;
-    if (rc == MDG_OK && want_lanes != 1 && lanes2_capable(h->P.feat) && (h->saturating || want_lanes == 2) &&
+    // (not with per-drone DR planes or sensor rows: their scalar prologue / epilogue work per env slot outweighs the packed loop;
+    //  measured on config 5: DR 30.6 vs 24.5 us, sensor noise 33.6 vs 28.4 us)
+    const bool lanes2_pays = !(h->P.feat & (F_DR | F_SENS));
+    if (rc == MDG_OK && want_lanes != 1 && lanes2_capable(h->P.feat) && ((h->saturating && lanes2_pays) || want_lanes == 2) &&
         h->kernel_name.find("generic") == std::string::npos) {
         const int minb1 = h->minb;
         h->lanes = 2; h->minb = 4;
