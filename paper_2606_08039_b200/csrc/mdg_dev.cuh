@@ -340,6 +340,13 @@ template <int DEG, class T> __device__ __forceinline__ V3T<T> stage_torque_t(con
 
 // sqrt(x) for x >= 0: one MUFU.SQRT (sqrt.approx.ftz, 1 ulp; sqrt(0) = 0)
 __device__ __forceinline__ float fast_sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ F2 add_(F2 a, float b) { return add_(a, pk(b, b)); }
+__device__ __forceinline__ float clamp_(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
+__device__ __forceinline__ F2 clamp_(F2 a, float lo, float hi) { return pk(fminf(fmaxf(lo_(a), lo), hi), fminf(fmaxf(hi_(a), lo), hi)); }
+__device__ __forceinline__ float min_(float a, float b) { return fminf(a, b); }
+__device__ __forceinline__ F2 min_(F2 a, F2 b) { return pk(fminf(lo_(a), lo_(b)), fminf(hi_(a), hi_(b))); }
+__device__ __forceinline__ float sqrt_(float x) { return fast_sqrt(x); }
+__device__ __forceinline__ F2 sqrt_(F2 a) { return pk(fast_sqrt(lo_(a)), fast_sqrt(hi_(a))); }
 __device__ __forceinline__ float clampf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
 __device__ __forceinline__ float wrap_pi(float x) {
     const float k = ceilf((x - 3.14159265358979f) * 0.159154943091895f);

@@ -299,8 +299,8 @@ struct Slot {
     float4 dr0, dr1, dr2, dr3;                                    // this episode's DR factors (read-mostly, plain loads)
     V3 Fwind; float4 gust_out;                                    // wind force held over the substeps; E1 after this step (MDG_WIND_GUST)
     float n[4], n_later[4], n_act[4], lag_gain; int sw, d_obs;    // rotor commands (now / after the latency switch), rotor speeds under lag
-    float kf_e, kappa_e, inv_sJ, inv_m_e, g_e, dwc_e;             // the true vehicle of this episode (Table 4)
-    float T, cxy, dcz, gndT; V3 tau_b, k1_tau;                    // motor model (Eq.1-3) as the substeps use it
+    float kf_e, kappa_e, inv_sJ, inv_m_e, g_e, dwc_e, nmax;       // the true vehicle of this episode (Table 4)
+    DecodeMid mid;                                                // controller actions: what decode_front leaves for control_loops
     bool hit; Sensed snap;
 };
 
@@ -445,32 +445,6 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
 
     const bool dr = F::has(P, F_DR);
     const bool lag = F::has(P, F_MLAG);
-    // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag
-    // (every product and sum spelled out: the compiler must not choose, per instantiation, which of them to contract into
-    // fused multiply-adds - both lane shapes have to round identically)
-    auto motor_model = [&](Slot& s, const float (&nn)[4]) {
-        const float k0 = dr ? __fmul_rn(s.kf_e, s.dr2.x) : s.kf_e, k1 = dr ? __fmul_rn(s.kf_e, s.dr2.y) : s.kf_e,
-                    k2 = dr ? __fmul_rn(s.kf_e, s.dr2.z) : s.kf_e, k3 = dr ? __fmul_rn(s.kf_e, s.dr2.w) : s.kf_e;
-        const float f0 = __fmul_rn(k0, __fmul_rn(nn[0], nn[0])), f1 = __fmul_rn(k1, __fmul_rn(nn[1], nn[1])),
-                    f2 = __fmul_rn(k2, __fmul_rn(nn[2], nn[2])), f3 = __fmul_rn(k3, __fmul_rn(nn[3], nn[3]));
-        const float f01 = __fadd_rn(f0, f1), f23 = __fadd_rn(f2, f3), f12 = __fadd_rn(f1, f2), f03 = __fadd_rn(f0, f3),
-                    f13 = __fadd_rn(f1, f3), f02 = __fadd_rn(f0, f2);
-        s.T = __fadd_rn(f01, f23);
-        const float arm_e = dr ? s.dr3.x : 1.0f;
-        const float tz = __fmul_rn(s.kappa_e, __fsub_rn(f13, f02));
-        s.tau_b = F::has(P, F_CF2P) ? v3(__fmul_rn(P.arm, __fsub_rn(f1, f3)), __fmul_rn(P.arm, __fsub_rn(f2, f0)), tz)
-                                    : v3(__fmul_rn(P.l, __fsub_rn(f01, f23)), __fmul_rn(P.l, __fsub_rn(f12, f03)), tz);
-        if (dr) {
-            const float sxy = __fmul_rn(s.inv_sJ, arm_e);
-            s.tau_b.x = __fmul_rn(s.tau_b.x, sxy); s.tau_b.y = __fmul_rn(s.tau_b.y, sxy); s.tau_b.z = __fmul_rn(s.tau_b.z, s.inv_sJ);
-        }
-        const float Om = __fmul_rn(P.rpm2rad, __fadd_rn(__fadd_rn(nn[0], nn[1]), __fadd_rn(nn[2], nn[3])));
-        s.k1_tau = v3(__fmul_rn(P.invJ[0], s.tau_b.x), __fmul_rn(P.invJ[1], s.tau_b.y), __fmul_rn(P.invJ[2], s.tau_b.z));
-        s.cxy = __fmul_rn(dr ? __fmul_rn(-P.c_xy, s.dr1.x) : -P.c_xy, Om);
-        const float cz = __fmul_rn(dr ? __fmul_rn(-P.c_z, s.dr1.x) : -P.c_z, Om);
-        s.gndT = __fmul_rn(dr ? __fmul_rn(P.gnd_coef, s.dr1.y) : P.gnd_coef, s.T);
-        s.dcz = __fsub_rn(cz, s.cxy);
-    };
     // Two envs per lane and at least two lanes per env: the AR(1) gust of an env is the same for all its lanes, so lane j draws
     // it for env slot j & 1 only and the group's lanes 0 and 1 hand their results round (six shuffles instead of a second
     // Philox + Box-Muller per lane; the arithmetic is gust_update either way).
@@ -538,7 +512,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                 }
                 gust_out = gs;
             }
-            if (wmask & 7) {
+            if (F::has(P, F_WIND_MIX) && (wmask & 7)) {            // (the plain gust's drag law is evaluated with the lanes' values packed, below)
                 const V3 rel = v3(u.x - d.v.x, u.y - d.v.y, u.z - d.v.z);
                 const float kn = P.k_wind * fast_sqrt(fmaf(rel.x, rel.x, fmaf(rel.y, rel.y, rel.z * rel.z)));
                 Fwind = v3(kn * rel.x, kn * rel.y, kn * rel.z);
@@ -577,17 +551,18 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         s.sw = sw; s.d_obs = d_obs;
         // S1/S2 decode, S3 motor model (Eq.1-3); RPMs are held over the K substeps
         s.n_later[0] = s.n_later[1] = s.n_later[2] = s.n_later[3] = 0.0f;
-        decode_action<FEAT>(P, a_first, d, s.n);
-        if (F::has(P, F_LAT) && s.sw >= 0) { DroneRegs dtmp = d; decode_action<FEAT>(P, a_second, dtmp, s.n_later); }   // direct rotor commands: stateless
+        s.n[0] = s.n[1] = s.n[2] = s.n[3] = 0.0f;
+        decode_front<FEAT>(P, a_first, d, s.n, s.mid);            // controller actions: the loops run on the lanes' values packed, below
+        if (F::has(P, F_LAT) && s.sw >= 0) { DroneRegs dtmp = d; DecodeMid mtmp; decode_front<FEAT>(P, a_second, dtmp, s.n_later, mtmp); }   // direct rotor commands: stateless
         // Domain randomisation (Table 4): this episode's factors scale the true vehicle, not the controller's model above.
         // 1 / s_J is folded into the body torque (every stage torque is linear in it, the gyroscopic ratios do not change).
         s.kf_e = dr ? __fmul_rn(P.k_f, s.dr0.z) : P.k_f; s.kappa_e = dr ? __fmul_rn(P.kappa, __fdiv_rn(s.dr0.w, s.dr0.z)) : P.kappa;
         s.inv_sJ = dr ? __fdiv_rn(1.0f, s.dr0.y) : 1.0f; s.inv_m_e = dr ? __fdiv_rn(P.inv_m, s.dr0.x) : P.inv_m; s.g_e = dr ? __fmul_rn(P.g, s.dr1.w) : P.g;
         s.dwc_e = dr ? __fmul_rn(P.dw_coef, s.dr1.z) : P.dw_coef;
-        if (dr) {                                                      // true motor saturation of this episode
-            const float nmax = __fmul_rn(P.max_rpm, s.dr3.y);
+        s.nmax = dr ? __fmul_rn(P.max_rpm, s.dr3.y) : P.max_rpm;    // true motor saturation of this episode
+        if (dr && !pid) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) { s.n[i] = fminf(s.n[i], nmax); s.n_later[i] = fminf(s.n_later[i], nmax); }
+            for (int i = 0; i < 4; ++i) { s.n[i] = fminf(s.n[i], s.nmax); s.n_later[i] = fminf(s.n_later[i], s.nmax); }
         }
         // Table 4 motor lag (Q44): the rotors follow n through a first-order lag sampled exactly per substep
 #pragma unroll
@@ -597,20 +572,10 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             const float4 r = B.N0[s.drone];
             s.n_act[0] = r.x; s.n_act[1] = r.y; s.n_act[2] = r.z; s.n_act[3] = r.w;
             s.lag_gain = 1.0f - __expf(-P.h / s.dr3.z);
-        } else motor_model(s, s.n);
+        }
         s.hit = false;
         s.snap = sensed(d, v3(0, 0, 0));                              // sensor latency of a whole step: the state the step starts from
-        // What only the epilogue needs goes back to the landing zone, which stays intact until the next prefetch into it: the
-        // substep loop then holds nothing but the integrated state and the frozen wrench in registers.
-        WarpStage& Wm = S[(st * wpb + wib) * NP + h];
-        Wm.plane[3][lane] = make_float4(d.w.z, d.Ip.x, d.Ip.y, d.Ip.z);
-        if (pid) {
-            Wm.plane[4][lane] = make_float4(d.Ie.x, d.Ie.y, d.Ie.z, 0.0f);
-            if (F::act(P) == 1) Wm.plane[5][lane] = d.sp;
-        }
-        Wm.plane[8][lane] = env4;
     }
-    asm volatile("" ::: "memory");                                // the epilogue re-reads them: no register copies kept across the loop
 
     const bool flush = pending2 != 0xFFFFFFFFu;                  // two items wait: fence now, flags after the substeps
     if (flush) __threadfence();
@@ -623,14 +588,78 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         bd.q.w = MDG_PK(d.q.w); bd.q.x = MDG_PK(d.q.x); bd.q.y = MDG_PK(d.q.y); bd.q.z = MDG_PK(d.q.z);
         bd.v = v3t<T>(MDG_PK(d.v.x), MDG_PK(d.v.y), MDG_PK(d.v.z));
         bd.w = v3t<T>(MDG_PK(d.w.x), MDG_PK(d.w.y), MDG_PK(d.w.z));
-        bd.Fwind = v3t<T>(MDG_PK(Fwind.x), MDG_PK(Fwind.y), MDG_PK(Fwind.z));
+        T nn[4] = {MDG_PK(n[0]), MDG_PK(n[1]), MDG_PK(n[2]), MDG_PK(n[3])};
+        if (pid) {                                                 // S2: position and attitude loops, mixer (control_loops)
+            DecodeMidT<T> m;
+            m.roll = MDG_PK(mid.roll); m.pitch = MDG_PK(mid.pitch); m.cpsi = MDG_PK(mid.cpsi); m.spsi = MDG_PK(mid.spsi);
+            m.ncpsi = pack_lanes(np, -s0.mid.cpsi, -s1.mid.cpsi); m.nspsi = pack_lanes(np, -s0.mid.spsi, -s1.mid.spsi);
+            m.e_p = v3t<T>(MDG_PK(mid.e_p.x), MDG_PK(mid.e_p.y), MDG_PK(mid.e_p.z));
+            m.v_cmd = v3t<T>(MDG_PK(mid.v_cmd.x), MDG_PK(mid.v_cmd.y), MDG_PK(mid.v_cmd.z));
+            m.e_psi = MDG_PK(mid.e_psi); m.thrust = MDG_PK(mid.T); m.phi_ref = MDG_PK(mid.phi_ref); m.th_ref = MDG_PK(mid.th_ref);
+            V3T<T> Ip = v3t<T>(MDG_PK(d.Ip.x), MDG_PK(d.Ip.y), MDG_PK(d.Ip.z)), Ie = v3t<T>(MDG_PK(d.Ie.x), MDG_PK(d.Ie.y), MDG_PK(d.Ie.z));
+            control_loops<FEAT>(P, m, bd.v, bd.w, Ip, Ie, nn);
+            if (dr) {
+                const T nmax = MDG_PK(nmax);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) nn[i] = min_(nn[i], nmax);
+            }
+#pragma unroll
+            for (int h = 0; h < NP; ++h) {
+                sl[h].d.Ip = v3(half_of(Ip.x, h), half_of(Ip.y, h), half_of(Ip.z, h));
+                sl[h].d.Ie = v3(half_of(Ie.x, h), half_of(Ie.y, h), half_of(Ie.z, h));
+#pragma unroll
+                for (int i = 0; i < 4; ++i) sl[h].n[i] = half_of(nn[i], h);
+            }
+        }
+        // What only the epilogue needs goes back to the landing zone, which stays intact until the next prefetch into it: the
+        // substep loop then holds nothing but the integrated state and the frozen wrench in registers.
+#pragma unroll
+        for (int h = 0; h < NP; ++h) {
+            const Slot& s = sl[h];
+            WarpStage& Wm = S[(st * wpb + wib) * NP + h];
+            Wm.plane[3][lane] = make_float4(s.d.w.z, s.d.Ip.x, s.d.Ip.y, s.d.Ip.z);
+            if (pid) {
+                Wm.plane[4][lane] = make_float4(s.d.Ie.x, s.d.Ie.y, s.d.Ie.z, 0.0f);
+                if (F::act(P) == 1) Wm.plane[5][lane] = s.d.sp;
+            }
+            Wm.plane[8][lane] = s.env4;
+        }
+        asm volatile("" ::: "memory");                            // the epilogue re-reads them: no register copies kept across the loop
+
+        if (F::has(P, F_WIND) && !F::has(P, F_WIND_MIX)) {        // PAPER.md:201 drag law on the gust just updated: F = k_w |u - v| (u - v) (Q28)
+            const V3T<T> rel = v3t<T>(sub_(MDG_PK(env4.x), bd.v.x), sub_(MDG_PK(env4.y), bd.v.y), sub_(MDG_PK(env4.z), bd.v.z));
+            const T kn = mul_(P.k_wind, sqrt_(dot3(rel, rel)));
+            bd.Fwind = v3t<T>(mul_(kn, rel.x), mul_(kn, rel.y), mul_(kn, rel.z));
+        } else bd.Fwind = v3t<T>(MDG_PK(Fwind.x), MDG_PK(Fwind.y), MDG_PK(Fwind.z));
         bd.inv_m = MDG_PK(inv_m_e); bd.ng = pack_lanes(np, -s0.g_e, -s1.g_e); bd.ndwc = pack_lanes(np, -s0.dwc_e, -s1.dwc_e);
-        auto load_motor = [&]() {
-            bd.tau_b = v3t<T>(MDG_PK(tau_b.x), MDG_PK(tau_b.y), MDG_PK(tau_b.z));
-            bd.k1_tau = v3t<T>(MDG_PK(k1_tau.x), MDG_PK(k1_tau.y), MDG_PK(k1_tau.z));
-            bd.thrust = MDG_PK(T); bd.cxy = MDG_PK(cxy); bd.dcz = MDG_PK(dcz); bd.gndT = MDG_PK(gndT);
+        // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag.  Every
+        // product and sum is spelled out (mdg_dev.cuh: lane-generic arithmetic), so one env per lane and two round identically.
+        auto motor_model = [&](const T (&nn)[4]) {
+            const T kf = MDG_PK(kf_e);
+            const T k0 = dr ? mul_(kf, MDG_PK(dr2.x)) : kf, k1 = dr ? mul_(kf, MDG_PK(dr2.y)) : kf,
+                    k2 = dr ? mul_(kf, MDG_PK(dr2.z)) : kf, k3 = dr ? mul_(kf, MDG_PK(dr2.w)) : kf;
+            // (products that are summed next are written as fma(a, b, 0): ptxas contracts a PACKED multiply-add pair into one FFMA2,
+            //  which it never does for the scalar mul.rn / add.rn - see ang_acc_t)
+            const T f0 = fma_(k0, mul_(nn[0], nn[0]), 0.0f), f1 = fma_(k1, mul_(nn[1], nn[1]), 0.0f), f2 = fma_(k2, mul_(nn[2], nn[2]), 0.0f),
+                    f3 = fma_(k3, mul_(nn[3], nn[3]), 0.0f);
+            const T f01 = add_(f0, f1), f23 = add_(f2, f3), f12 = add_(f1, f2), f03 = add_(f0, f3), f13 = add_(f1, f3), f02 = add_(f0, f2);
+            bd.thrust = add_(f01, f23);
+            const T tz = mul_(MDG_PK(kappa_e), sub_(f13, f02));
+            V3T<T> tau = F::has(P, F_CF2P) ? v3t<T>(mul_(P.arm, sub_(f1, f3)), mul_(P.arm, sub_(f2, f0)), tz)
+                                            : v3t<T>(mul_(P.l, sub_(f01, f23)), mul_(P.l, sub_(f12, f03)), tz);
+            if (dr) {
+                const T isj = MDG_PK(inv_sJ), sxy = mul_(isj, MDG_PK(dr3.x));
+                tau.x = mul_(tau.x, sxy); tau.y = mul_(tau.y, sxy); tau.z = mul_(tau.z, isj);
+            }
+            const T Om = mul_(P.rpm2rad, add_(add_(nn[0], nn[1]), add_(nn[2], nn[3])));
+            bd.tau_b = tau;
+            bd.k1_tau = v3t<T>(mul_(P.invJ[0], tau.x), mul_(P.invJ[1], tau.y), mul_(P.invJ[2], tau.z));
+            bd.cxy = dr ? mul_(mul_(-P.c_xy, MDG_PK(dr1.x)), Om) : mul_(-P.c_xy, Om);
+            const T cz = dr ? fma_(mul_(-P.c_z, MDG_PK(dr1.x)), Om, 0.0f) : fma_(-P.c_z, Om, 0.0f);
+            bd.gndT = dr ? mul_(mul_(P.gnd_coef, MDG_PK(dr1.y)), bd.thrust) : mul_(P.gnd_coef, bd.thrust);
+            bd.dcz = sub_(cz, bd.cxy);
         };
-        load_motor();
+        if (!lag) motor_model(nn);
         bool spun = false;                                         // two envs per lane: some substep was outside the series' range
 #pragma unroll 1
         for (int k = 0; k < P.K; ++k) {
@@ -638,13 +667,14 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                 if (F::has(P, F_LAT) && s0.sw == k) {              // Q51: the next row arrives at this substep
 #pragma unroll
                     for (int i = 0; i < 4; ++i) s0.n[i] = s0.n_later[i];
-                    if (!lag) { motor_model(s0, s0.n); load_motor(); }
+                    const T nn[4] = {MDG_PK(n[0]), MDG_PK(n[1]), MDG_PK(n[2]), MDG_PK(n[3])};
+                    if (!lag) motor_model(nn);
                 }
                 if (lag) {
 #pragma unroll
                     for (int i = 0; i < 4; ++i) s0.n_act[i] = fmaf(s0.lag_gain, __fsub_rn(s0.n[i], s0.n_act[i]), s0.n_act[i]);
-                    motor_model(s0, s0.n_act);
-                    load_motor();
+                    const T nn[4] = {MDG_PK(n_act[0]), MDG_PK(n_act[1]), MDG_PK(n_act[2]), MDG_PK(n_act[3])};
+                    motor_model(nn);
                 }
             }
             const SubstepFlags<T> fl = substep<G, FEAT, DEG>(P, bd, j, full_group);

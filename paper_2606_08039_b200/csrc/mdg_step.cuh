@@ -125,85 +125,105 @@ __device__ __forceinline__ void draw_dr(const DevParams& P, uint32_t e, uint32_t
                      P.motor_lag_hi > 0.0f ? fmaf(P.motor_lag_hi - P.motor_lag_lo, u01(d.z), P.motor_lag_lo) : 1.0f, 1.0f);
 }
 
-// Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376)
+// Action decode -> per-rotor RPM (Table 3; cascaded PID PAPER.md:347-357, DSL PAPER.md:372-376), in two parts.
+// decode_front (per env slot, scalar): rotor-command actions are finished here (returns false); for the controller actions it
+// leaves what the loops need in a DecodeMid - roll, pitch and the heading direction of the current attitude, the position error
+// and commanded velocity (PID / VEL) or thrust and tilt targets (ATTITUDE), the yaw error - and moves the held setpoint (DSL).
+// control_loops (lane-generic, mdg_dev.cuh: one env per lane or two as packed pairs): Eq.9, T = m |a*|, the small-angle tilt
+// target, the attitude PID with its clamps, the closed-form allocation inverse and the per-rotor clip.
+struct DecodeMid {
+    float roll, pitch, cpsi, spsi;        // current attitude: eta_x, eta_y, heading (cos psi, sin psi)
+    V3 e_p, v_cmd;                        // position error; commanded velocity in the heading frame (VEL) or zero (PID)
+    float e_psi, T, phi_ref, th_ref;      // yaw error; ATTITUDE only: thrust and tilt targets
+};
 template <int FEAT>
-__device__ __forceinline__ void decode_action(const DevParams& P, float4 a, DroneRegs& d, float n[4]) {
+__device__ __forceinline__ bool decode_front(const DevParams& P, float4 a, DroneRegs& d, float n[4], DecodeMid& m) {
     const int act = Feat<FEAT>::act(P);
     if (act == 0) {                       // RPM, clipped
         n[0] = clampf(a.x, 0.0f, P.max_rpm); n[1] = clampf(a.y, 0.0f, P.max_rpm);
         n[2] = clampf(a.z, 0.0f, P.max_rpm); n[3] = clampf(a.w, 0.0f, P.max_rpm);
-        return;
+        return false;
     }
     if (act == 3 || act == 4) {           // RPM_NORM / ONE_D_RPM through normalizedActionToRPM (Q35)
         n[0] = norm_rpm(P, a.x);
         n[1] = act == 4 ? n[0] : norm_rpm(P, a.y); n[2] = act == 4 ? n[0] : norm_rpm(P, a.z); n[3] = act == 4 ? n[0] : norm_rpm(P, a.w);
-        return;
+        return false;
     }
     // roll, pitch and the heading direction (cos psi, sin psi) = normalised (1 - 2(y^2+z^2), 2(wz+xy))
-    V3 eta;
-    eta.x = roll_of(d.q);
-    eta.y = pitch_of(d.q);
-    const float hc = fmaf(-2.0f, fmaf(d.q.y, d.q.y, d.q.z * d.q.z), 1.0f), hs = 2.0f * fmaf(d.q.w, d.q.z, d.q.x * d.q.y);
-    const float hn2 = fmaf(hc, hc, hs * hs);
+    m.roll = roll_of(d.q);
+    m.pitch = pitch_of(d.q);
+    const float hc = fmaf(-2.0f, fmaf(d.q.y, d.q.y, __fmul_rn(d.q.z, d.q.z)), 1.0f), hs = __fmul_rn(2.0f, fmaf(d.q.w, d.q.z, __fmul_rn(d.q.x, d.q.y)));
+    const float hn2 = fmaf(hc, hc, __fmul_rn(hs, hs));
     const float hr = hn2 > 1e-30f ? rsqrt_fast(hn2) : 0.0f;
-    const float cpsi = hn2 > 1e-30f ? hc * hr : 1.0f, spsi = hs * hr;
-    V3 e_p, v_ref; float e_psi;
-    float T, phi_ref, th_ref;
+    m.cpsi = hn2 > 1e-30f ? __fmul_rn(hc, hr) : 1.0f; m.spsi = __fmul_rn(hs, hr);
+    m.e_p = v3(0, 0, 0); m.v_cmd = v3(0, 0, 0); m.T = 0.0f; m.phi_ref = 0.0f; m.th_ref = 0.0f;
     if (act == 5) {                       // ATTITUDE [thrust, roll*, pitch*, yaw rate] (Q36): attitude loop + mixer only
         const float nt = norm_rpm(P, a.x);
-        T = 4.0f * (P.k_f * (nt * nt));
-        phi_ref = clampf(a.y, -P.tilt_max, P.tilt_max);
-        th_ref = clampf(a.z, -P.tilt_max, P.tilt_max);
-        e_psi = wrap_pi(a.w * P.dt_c);
-    } else {
-    if (act == 1) {                       // PID waypoint [x, y, z, psi]
+        m.T = __fmul_rn(4.0f, __fmul_rn(P.k_f, __fmul_rn(nt, nt)));
+        m.phi_ref = clampf(a.y, -P.tilt_max, P.tilt_max);
+        m.th_ref = clampf(a.z, -P.tilt_max, P.tilt_max);
+        m.e_psi = wrap_pi(__fmul_rn(a.w, P.dt_c));
+    } else if (act == 1) {                // PID waypoint [x, y, z, psi]
         if (Feat<FEAT>::has(P, F_DSL)) {
-            const V3 dv = v3(a.x - d.sp.x, a.y - d.sp.y, a.z - d.sp.z);
-            const float dist = sqrtf(fmaf(dv.x, dv.x, fmaf(dv.y, dv.y, dv.z * dv.z)));
+            const V3 dv = v3(__fsub_rn(a.x, d.sp.x), __fsub_rn(a.y, d.sp.y), __fsub_rn(a.z, d.sp.z));
+            const float dist = sqrtf(fmaf(dv.x, dv.x, fmaf(dv.y, dv.y, __fmul_rn(dv.z, dv.z))));
             if (dist > P.pos_step_max) {
-                const float f = P.pos_step_max / dist;
+                const float f = __fdiv_rn(P.pos_step_max, dist);
                 d.sp.x = fmaf(dv.x, f, d.sp.x); d.sp.y = fmaf(dv.y, f, d.sp.y); d.sp.z = fmaf(dv.z, f, d.sp.z);
             } else { d.sp.x = a.x; d.sp.y = a.y; d.sp.z = a.z; }
-            const float dpsi = clampf(wrap_pi(a.w - d.sp.w), -P.yaw_step_max, P.yaw_step_max);
-            d.sp.w = wrap_pi(d.sp.w + dpsi);
+            const float dpsi = clampf(wrap_pi(__fsub_rn(a.w, d.sp.w)), -P.yaw_step_max, P.yaw_step_max);
+            d.sp.w = wrap_pi(__fadd_rn(d.sp.w, dpsi));
         } else d.sp = a;
-        e_p = v3(d.sp.x - d.p.x, d.sp.y - d.p.y, d.sp.z - d.p.z);
-        v_ref = v3(0, 0, 0); e_psi = wrap_pi(d.sp.w - atan2_fast(hs, hc));
+        m.e_p = v3(__fsub_rn(d.sp.x, d.p.x), __fsub_rn(d.sp.y, d.p.y), __fsub_rn(d.sp.z, d.p.z));
+        m.e_psi = wrap_pi(__fsub_rn(d.sp.w, atan2_fast(hs, hc)));
     } else {                              // VEL [vx, vy, vz, wz] in the heading frame
-        e_p = v3(0, 0, 0);
-        v_ref = v3(cpsi * a.x - spsi * a.y, spsi * a.x + cpsi * a.y, a.z);
-        e_psi = wrap_pi(a.w * P.dt_c);                             // psi* = psi + wz dt
+        m.v_cmd = v3(a.x, a.y, a.z);
+        m.e_psi = wrap_pi(__fmul_rn(a.w, P.dt_c));                 // psi* = psi + wz dt
     }
-    // position loop, Eq.9
-    d.Ip.x = clampf(fmaf(e_p.x, P.dt_c, d.Ip.x), -P.int_clamp_pos, P.int_clamp_pos);
-    d.Ip.y = clampf(fmaf(e_p.y, P.dt_c, d.Ip.y), -P.int_clamp_pos, P.int_clamp_pos);
-    d.Ip.z = clampf(fmaf(e_p.z, P.dt_c, d.Ip.z), -P.int_clamp_pos, P.int_clamp_pos);
-    const float ax = fmaf(P.Kp_pos[0], e_p.x, fmaf(P.Ki_pos[0], d.Ip.x, fmaf(P.Kd_pos[0], v_ref.x - d.v.x, P.a_ff[0])));
-    const float ay = fmaf(P.Kp_pos[1], e_p.y, fmaf(P.Ki_pos[1], d.Ip.y, fmaf(P.Kd_pos[1], v_ref.y - d.v.y, P.a_ff[1])));
-    const float az = fmaf(P.Kp_pos[2], e_p.z, fmaf(P.Ki_pos[2], d.Ip.z, fmaf(P.Kd_pos[2], v_ref.z - d.v.z, P.a_ff[2]))) + P.g;
-    T = clampf(P.m * fast_sqrt(fmaf(ax, ax, fmaf(ay, ay, az * az))), 0.0f, P.T_max);
-    phi_ref = clampf((ax * spsi - ay * cpsi) * P.inv_g, -P.tilt_max, P.tilt_max);
-    th_ref = clampf((ax * cpsi + ay * spsi) * P.inv_g, -P.tilt_max, P.tilt_max);
+    return true;
+}
+template <class T> struct DecodeMidT {   // DecodeMid of one env slot (float) or of the lane's two (F2)
+    T roll, pitch, cpsi, spsi, ncpsi, nspsi; V3T<T> e_p, v_cmd; T e_psi, thrust, phi_ref, th_ref;
+};
+template <int FEAT, class T>
+__device__ __forceinline__ void control_loops(const DevParams& P, const DecodeMidT<T>& m, V3T<T> v, V3T<T> w, V3T<T>& Ip, V3T<T>& Ie, T (&n)[4]) {
+    const int act = Feat<FEAT>::act(P);
+    T thrust = m.thrust, phi_ref = m.phi_ref, th_ref = m.th_ref;
+    if (act != 5) {
+        // commanded velocity from the heading frame to the world frame (zero for PID)
+        const V3T<T> v_ref = v3t<T>(fma_(m.cpsi, m.v_cmd.x, mul_(m.nspsi, m.v_cmd.y)), fma_(m.spsi, m.v_cmd.x, mul_(m.cpsi, m.v_cmd.y)), m.v_cmd.z);
+        // position loop, Eq.9
+        Ip.x = clamp_(fma_(m.e_p.x, P.dt_c, Ip.x), -P.int_clamp_pos, P.int_clamp_pos);
+        Ip.y = clamp_(fma_(m.e_p.y, P.dt_c, Ip.y), -P.int_clamp_pos, P.int_clamp_pos);
+        Ip.z = clamp_(fma_(m.e_p.z, P.dt_c, Ip.z), -P.int_clamp_pos, P.int_clamp_pos);
+        const T ax = fma_(P.Kp_pos[0], m.e_p.x, fma_(P.Ki_pos[0], Ip.x, fma_(P.Kd_pos[0], sub_(v_ref.x, v.x), P.a_ff[0])));
+        const T ay = fma_(P.Kp_pos[1], m.e_p.y, fma_(P.Ki_pos[1], Ip.y, fma_(P.Kd_pos[1], sub_(v_ref.y, v.y), P.a_ff[1])));
+        const T az = add_(fma_(P.Kp_pos[2], m.e_p.z, fma_(P.Ki_pos[2], Ip.z, fma_(P.Kd_pos[2], sub_(v_ref.z, v.z), P.a_ff[2]))), P.g);
+        thrust = clamp_(mul_(P.m, sqrt_(fma_(ax, ax, fma_(ay, ay, mul_(az, az))))), 0.0f, P.T_max);       // T = m |a*|
+        phi_ref = clamp_(mul_(fma_(ax, m.spsi, mul_(ay, m.ncpsi)), P.inv_g), -P.tilt_max, P.tilt_max);    // small-angle tilt target
+        th_ref = clamp_(mul_(fma_(ax, m.cpsi, mul_(ay, m.spsi)), P.inv_g), -P.tilt_max, P.tilt_max);
     }
-    const V3 e_eta = v3(phi_ref - eta.x, th_ref - eta.y, e_psi);
-    d.Ie.x = clampf(fmaf(e_eta.x, P.dt_c, d.Ie.x), -P.int_clamp_att, P.int_clamp_att);
-    d.Ie.y = clampf(fmaf(e_eta.y, P.dt_c, d.Ie.y), -P.int_clamp_att, P.int_clamp_att);
-    d.Ie.z = clampf(fmaf(e_eta.z, P.dt_c, d.Ie.z), -P.int_clamp_att, P.int_clamp_att);
-    const float tx = clampf(fmaf(P.Kp_att[0], e_eta.x, fmaf(P.Ki_att[0], d.Ie.x, -P.Kd_att[0] * d.w.x)), -P.tau_xy_max, P.tau_xy_max);
-    const float ty = clampf(fmaf(P.Kp_att[1], e_eta.y, fmaf(P.Ki_att[1], d.Ie.y, -P.Kd_att[1] * d.w.y)), -P.tau_xy_max, P.tau_xy_max);
-    const float tz = clampf(fmaf(P.Kp_att[2], e_eta.z, fmaf(P.Ki_att[2], d.Ie.z, -P.Kd_att[2] * d.w.z)), -P.tau_z_max, P.tau_z_max);
-    // closed-form allocation inverse, per-rotor clip, back to RPM
-    float s0, s1, s2, s3;
+    const V3T<T> e_eta = v3t<T>(sub_(phi_ref, m.roll), sub_(th_ref, m.pitch), m.e_psi);
+    Ie.x = clamp_(fma_(e_eta.x, P.dt_c, Ie.x), -P.int_clamp_att, P.int_clamp_att);
+    Ie.y = clamp_(fma_(e_eta.y, P.dt_c, Ie.y), -P.int_clamp_att, P.int_clamp_att);
+    Ie.z = clamp_(fma_(e_eta.z, P.dt_c, Ie.z), -P.int_clamp_att, P.int_clamp_att);
+    const T tx = clamp_(fma_(P.Kp_att[0], e_eta.x, fma_(P.Ki_att[0], Ie.x, mul_(-P.Kd_att[0], w.x))), -P.tau_xy_max, P.tau_xy_max);
+    const T ty = clamp_(fma_(P.Kp_att[1], e_eta.y, fma_(P.Ki_att[1], Ie.y, mul_(-P.Kd_att[1], w.y))), -P.tau_xy_max, P.tau_xy_max);
+    const T tz = clamp_(fma_(P.Kp_att[2], e_eta.z, fma_(P.Ki_att[2], Ie.z, mul_(-P.Kd_att[2], w.z))), -P.tau_z_max, P.tau_z_max);
+    // closed-form allocation inverse, per-rotor clip, back to RPM.  (The clamps above are per-half min / max, so the products
+    // below never sit next to a packed add: nothing for ptxas to contract differently in the two lane shapes.)
+    T s0, s1, s2, s3;
     if (Feat<FEAT>::has(P, F_CF2P)) {     // +-configuration: tau_x = L (s1 - s3), tau_y = L (s2 - s0)
-        const float qa = 2.0f * tx * P.inv_arm, qb = 2.0f * ty * P.inv_arm, qc = tz * P.inv_kappa;
-        s0 = 0.25f * (T - qb - qc); s1 = 0.25f * (T + qa + qc); s2 = 0.25f * (T + qb - qc); s3 = 0.25f * (T - qa + qc);
+        const T qa = fma_(mul_(2.0f, tx), P.inv_arm, 0.0f), qb = fma_(mul_(2.0f, ty), P.inv_arm, 0.0f), qc = fma_(tz, P.inv_kappa, 0.0f);
+        s0 = mul_(0.25f, sub_(sub_(thrust, qb), qc)); s1 = mul_(0.25f, add_(add_(thrust, qa), qc));
+        s2 = mul_(0.25f, sub_(add_(thrust, qb), qc)); s3 = mul_(0.25f, add_(sub_(thrust, qa), qc));
     } else {
-        const float qa = tx * P.inv_l, qb = ty * P.inv_l, qc = tz * P.inv_kappa;
-        s0 = 0.25f * (T + qa - qb - qc); s1 = 0.25f * (T + qa + qb + qc);
-        s2 = 0.25f * (T - qa + qb - qc); s3 = 0.25f * (T - qa - qb + qc);
+        const T qa = fma_(tx, P.inv_l, 0.0f), qb = fma_(ty, P.inv_l, 0.0f), qc = fma_(tz, P.inv_kappa, 0.0f);   // fma(a, b, 0): summed next (see ang_acc_t)
+        s0 = mul_(0.25f, sub_(sub_(add_(thrust, qa), qb), qc)); s1 = mul_(0.25f, add_(add_(add_(thrust, qa), qb), qc));
+        s2 = mul_(0.25f, sub_(add_(sub_(thrust, qa), qb), qc)); s3 = mul_(0.25f, add_(sub_(sub_(thrust, qa), qb), qc));
     }
-    n[0] = fast_sqrt(clampf(s0, 0.0f, P.s_max) * P.inv_k_f); n[1] = fast_sqrt(clampf(s1, 0.0f, P.s_max) * P.inv_k_f);
-    n[2] = fast_sqrt(clampf(s2, 0.0f, P.s_max) * P.inv_k_f); n[3] = fast_sqrt(clampf(s3, 0.0f, P.s_max) * P.inv_k_f);
+    n[0] = sqrt_(mul_(clamp_(s0, 0.0f, P.s_max), P.inv_k_f)); n[1] = sqrt_(mul_(clamp_(s1, 0.0f, P.s_max), P.inv_k_f));
+    n[2] = sqrt_(mul_(clamp_(s2, 0.0f, P.s_max), P.inv_k_f)); n[3] = sqrt_(mul_(clamp_(s3, 0.0f, P.s_max), P.inv_k_f));
 }
 
 // angular acceleration J^-1 (tau_body - w x J w); axisym: J_xx == J_yy, the z component has no gyroscopic term
