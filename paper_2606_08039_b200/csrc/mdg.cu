@@ -49,7 +49,6 @@ struct mdg_env {
     int block = 128, max_blocks_per_sm = 0, smem = 0, minb = 4;
     int pdl = 1;
     int lanes = 1;                       // envs per lane group in the step kernel: 2 = packed FP32 pairs (grids that fill the device; MDG_LANES=1|2 forces)
-    int stages = 1;                      // shared-memory landing zones per warp (MDG_STAGES=1|2)
     int jit = 1;                         // MDG_JIT=0: never compile at run time, use the generic kernel; MDG_JIT=require: fail instead of falling back
     std::string jit_note;                // why the run-time specialisation was not possible (empty: it was, or was not needed)
     bool saturating = false;             // the step grid occupies every resident block slot of the device
@@ -308,8 +307,10 @@ static void pick_kernels(mdg_env* h) {
 
 // ---- helpers --------------------------------------------------------------------------------------
 static int configure_launch(mdg_env* h) {
-    h->P.n_stages = (uint32_t)h->stages; h->P.zero = 0u;
-    const int stage_bytes = h->stages * (h->block / 32) * h->lanes * (int)sizeof(WarpStage);   // landing zones per warp and env slot
+    h->P.zero = 0u;
+    const int act_t = (h->P.feat >> F_ACT_SHIFT) & 7, obs_t = (h->P.feat >> F_OBS_SHIFT) & 7;
+    const int n_stash = 3 + ((act_t == 1 || act_t == 2 || act_t == 5) ? 1 : 0) + (act_t == 1 ? 1 : 0) + (obs_t == 2 ? 1 : 0);   // as the kernel counts them
+    const int stage_bytes = (h->block / 32) * h->lanes * ((int)sizeof(WarpStage) + n_stash * 512);   // landing zone + stash per warp and env slot
     h->smem = stage_bytes;
     if (h->max_blocks_per_sm > 0) {          // cap residency by padding the dynamic shared-memory request
         int s = (228 * 1024) / h->max_blocks_per_sm - 1024;
@@ -474,7 +475,6 @@ int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, cons
     int G = 1; while (G < n_drones) G <<= 1;
     h->G = G;
     if (const char* ev = std::getenv("MDG_PDL")) h->pdl = ev[0] != '0';
-    if (const char* ev = std::getenv("MDG_STAGES")) h->stages = ev[0] == '1' ? 1 : 2;
     if (const char* ev = std::getenv("MDG_JIT")) h->jit = ev[0] == '0' ? 0 : (ev[0] == 'r' ? 2 : 1);   // 0: generic kernel only; require: no silent fallback
     make_dev_params(p, n_envs, n_drones, feature_word(p, physics_mode, action_type, n_drones, G), h->P);
     pick_kernels(h);

@@ -34,7 +34,7 @@ struct DevParams {
     int reset_layout, target_mode, grid_cols, grid_rows, opd;
     uint32_t seed_lo, seed_hi, env_base;
     uint32_t static_items;                                // grid does not fill the device: one item per warp, item = warp index (no dispenser)
-    uint32_t n_stages, zero;                              // shared-memory landing zones per warp (1 or 2); zero: always 0, unknown to the compiler
+    uint32_t zero;                                        // always 0, unknown to the compiler (mdg_kernels.cuh: prefetch_item)
     uint32_t seq, chain;                                  // per launch: step sequence number, item-level chaining behind step seq - 1 (mdg_kernels.cuh)
     // integrator
     float h, half_h, h_sixth, half_h2, w2_exact[2];          // w2_exact: |omega|^2 above which the exact path runs

@@ -76,8 +76,8 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // Start the asynchronous copies of this lane's slots of lane-group row `wt` (32 / G envs; global -> shared, no registers held).
-// dep: a zero the hardware cannot know to be zero, derived from the registers last read from S (single-stage staging: the
-// copies may overwrite S only once those reads have returned - a register dependency the address generation must wait for).
+// dep: a zero the hardware cannot know to be zero, derived from the registers last read from S: the copies may overwrite S
+// only once those reads have returned - a register dependency the address generation must wait for.
 template <int G>
 __device__ __forceinline__ void prefetch_item(const DevParams& P, const DevBuffers& B, const float4* actions, WarpStage& S,
                                               unsigned wt, int lane, int jj, int act, unsigned dep) {
@@ -267,11 +267,12 @@ __device__ __forceinline__ SubstepFlags<T> substep(const DevParams& P, Body<T>& 
 }
 // Two envs per lane keep the hot loop free of the exact path: a warp in which any lane spun too fast during the step redoes the
 // step's K substeps one env slot at a time with the one-drone code (same arithmetic: the result is what one env per lane
-// computes), from the start-of-step state that is still in the warp's landing zone W.  Out of line, never taken by the benchmarks.
+// computes), from the start-of-step state, which is still what global memory holds.  Out of line, never taken by the benchmarks.
 struct RedoOut { float s[13]; bool hit; };
 template <int G, int FEAT, int DEG>
-__device__ __noinline__ RedoOut redo_item_exact(const DevParams& P, const WarpStage& W, Body<float> b, int lane, int j, bool full_group) {
-    const float4 a0 = W.plane[0][lane], a1 = W.plane[1][lane], a2 = W.plane[2][lane], a3 = W.plane[3][lane];
+__device__ __noinline__ RedoOut redo_item_exact(const DevParams& P, const float4* p0, const float4* p1, const float4* p2, const float4* p3, Body<float> b,
+                                                int j, bool full_group) {
+    const float4 a0 = *p0, a1 = *p1, a2 = *p2, a3 = *p3;          // the step's stores have not happened yet
     b.p = v3t<float>(a0.x, a0.y, a0.z); b.q.w = a0.w; b.q.x = a1.x; b.q.y = a1.y; b.q.z = a1.z;
     b.v = v3t<float>(a1.w, a2.x, a2.y); b.w = v3t<float>(a2.z, a2.w, a3.x);
     RedoOut o; o.hit = false;
@@ -307,8 +308,8 @@ struct Slot {
 // One control step of every env.  Persistent warps: each loops over work items of
 // NP * 32 / G envs; lane -> (lane-in-group j, NP envs: slot h holds env (item * NP + h) * 32 / G + lane / G).  With NP = 2 the
 // substeps of a lane's two drones run as packed FP32 pairs (mdg_dev.cuh: F2), everything else once per slot.  While an item is
-// integrated, the next item's state planes, actions and per-env words are already on their way into shared memory (cp.async,
-// two stages), so HBM latency and bandwidth overlap the arithmetic instead of alternating with it.
+// integrated, the next item's state planes, actions and per-env words are already on their way into shared memory (cp.async
+// into the warp's landing zone), so HBM latency and bandwidth overlap the arithmetic instead of alternating with it.
 // MINB = resident blocks of 128 threads per SM the register allocation must allow.
 template <int G, int FEAT, int MINB, int NP>
 __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__ DevParams P, const DevBuffers B,
@@ -319,8 +320,17 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     static_assert(NP == 1 || !(FEAT & (F_MLAG | F_LAT)), "motor lag and the latency rows switch rotor commands inside the substep loop: one env per lane");
     // series degree of the rotation update: 2 where the specialisation's controller keeps the body rates small (PID / VEL)
     constexpr int DEG = (FEAT >= 0 && (((FEAT >> F_ACT_SHIFT) & 7) == 1 || ((FEAT >> F_ACT_SHIFT) & 7) == 2)) ? 2 : 3;
-    extern __shared__ __align__(16) unsigned char smem_raw[];     // [P.n_stages][warps per block][NP] WarpStage (host sizes it)
+    extern __shared__ __align__(16) unsigned char smem_raw[];     // [warps per block][NP] WarpStage, then the stash (host sizes it)
     WarpStage* const S = reinterpret_cast<WarpStage*>(smem_raw);
+    // Behind the landing zones: the warp's stash, one 16-byte slot per lane, env slot and parked quantity.  What only the epilogue
+    // needs (controller memory, target, env word, ...) waits there during the substeps, so the loop holds nothing but the
+    // integrated state and the frozen wrench in registers, and the landing zone is free for the next item right away.
+    const int obs_kin20 = F::obs(P) == 2;
+    const int act1 = F::act(P) == 1;
+    const int pid_i = (F::act(P) == 1 || F::act(P) == 2 || F::act(P) == 5) ? 1 : 0;
+    const int iIP = 0, iTG = 1, iENV = 2, iIE = 3, iSP = 3 + pid_i, iACT = 3 + pid_i + act1;
+    const int n_stash = 3 + pid_i + act1 + obs_kin20;             // the host sizes the shared memory with the same count
+    float4* const stash0 = reinterpret_cast<float4*>(smem_raw + (size_t)(blockDim.x >> 5) * NP * sizeof(WarpStage));
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const unsigned wpb = blockDim.x >> 5;
     const unsigned tw = gridDim.x * wpb;                          // persistent warps of this launch
@@ -393,21 +403,17 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     const unsigned probed_first = probe(wt);
     const unsigned drawn_first = draw(!static_items);
     await_item(wt, probed_first);
-    auto prefetch = [&](unsigned item, int stage, unsigned dep) {
+    auto prefetch = [&](unsigned item, unsigned dep) {
 #pragma unroll
-        for (int h = 0; h < NP; ++h) prefetch_item<G>(P, B, actions, S[(stage * wpb + wib) * NP + h], item * NP + h, lane, jj, F::act(P), dep);
+        for (int h = 0; h < NP; ++h) prefetch_item<G>(P, B, actions, S[wib * NP + h], item * NP + h, lane, jj, F::act(P), dep);
         cp_async_commit();
     };
-    // P.n_stages == 1: one landing zone per warp, refilled as soon as its contents have been read into registers (half the
-    // shared memory, room for more resident blocks); 2: the next item lands beside the current one.
-    const int flip = P.n_stages - 1;
-    prefetch(wt, 0, 0u);
+    prefetch(wt, 0u);
     unsigned wt_next = static_items ? 0xFFFFFFFFu : take(drawn_first);   // a warp stops drawing after its first miss
     unsigned probed_next = probe(wt_next);
     // Items whose flags are still to be published.  One fence covers two items: the consumer (the next step) reaches
     // an item a whole step later, so publishing it one item late costs nothing and halves the fences.
     unsigned pending = 0xFFFFFFFFu, pending2 = 0xFFFFFFFFu;
-    int st = 0;
 #pragma unroll 1
     for (;;) {
     const unsigned drawn_l0 = draw(wt_next < n_items);            // ticket of the item after next, in flight
@@ -422,7 +428,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         s.e = env_ok ? e_raw : (unsigned)P.N - 1;                 // idle lanes shadow the last env (no stores)
         s.active = env_ok && (full_group || j < P.M);
         s.drone = (size_t)s.e * P.M + jj;
-        const WarpStage& W = S[(st * wpb + wib) * NP + h];
+        const WarpStage& W = S[wib * NP + h];
         const float4 a = W.plane[0][lane], b = W.plane[1][lane], c = W.plane[2][lane], f = W.plane[3][lane];
         s.d.p = v3(a.x, a.y, a.z); s.d.q.w = a.w; s.d.q.x = b.x; s.d.q.y = b.y; s.d.q.z = b.z;
         s.d.v = v3(b.w, c.x, c.y); s.d.w = v3(c.z, c.w, f.x); s.d.Ip = v3(f.y, f.z, f.w);
@@ -441,7 +447,9 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         s.dr0 = make_float4(1, 1, 1, 1); s.dr1 = s.dr0; s.dr2 = s.dr0; s.dr3 = s.dr0;
         if (F::has(P, F_DR)) { s.dr0 = B.R0[s.drone]; s.dr1 = B.R1[s.drone]; s.dr2 = B.R2[s.drone]; s.dr3 = B.R3[s.drone]; }
     }
-    if (flip && wt_next < n_items) { await_item(wt_next, probed_next); prefetch(wt_next, st ^ 1, 0u); }   // two landing zones: the next item starts coming now
+    // the next item starts coming now, into the same landing zone: its contents are all in registers (`touched` makes the copies'
+    // addresses depend on them, so no copy can overtake a read)
+    if (wt_next < n_items) { await_item(wt_next, probed_next); prefetch(wt_next, touched & P.zero); }
 
     const bool dr = F::has(P, F_DR);
     const bool lag = F::has(P, F_MLAG);
@@ -611,18 +619,17 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                 for (int i = 0; i < 4; ++i) sl[h].n[i] = half_of(nn[i], h);
             }
         }
-        // What only the epilogue needs goes back to the landing zone, which stays intact until the next prefetch into it: the
-        // substep loop then holds nothing but the integrated state and the frozen wrench in registers.
+        // park what only the epilogue needs
 #pragma unroll
         for (int h = 0; h < NP; ++h) {
             const Slot& s = sl[h];
-            WarpStage& Wm = S[(st * wpb + wib) * NP + h];
-            Wm.plane[3][lane] = make_float4(s.d.w.z, s.d.Ip.x, s.d.Ip.y, s.d.Ip.z);
-            if (pid) {
-                Wm.plane[4][lane] = make_float4(s.d.Ie.x, s.d.Ie.y, s.d.Ie.z, 0.0f);
-                if (F::act(P) == 1) Wm.plane[5][lane] = s.d.sp;
-            }
-            Wm.plane[8][lane] = s.env4;
+            float4* const st4 = stash0 + ((size_t)(wib * NP + h) * n_stash) * 32 + lane;
+            st4[iIP * 32] = make_float4(0.0f, s.d.Ip.x, s.d.Ip.y, s.d.Ip.z);
+            st4[iTG * 32] = s.tg;
+            st4[iENV * 32] = s.env4;
+            if (pid) st4[iIE * 32] = make_float4(s.d.Ie.x, s.d.Ie.y, s.d.Ie.z, 0.0f);
+            if (F::act(P) == 1) st4[iSP * 32] = s.d.sp;
+            if (obs_kin20) st4[iACT * 32] = s.act4;
         }
         asm volatile("" ::: "memory");                            // the epilogue re-reads them: no register copies kept across the loop
 
@@ -697,7 +704,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                 b1.tau_b = half3(bd.tau_b, h); b1.k1_tau = half3(bd.k1_tau, h); b1.Fwind = half3(bd.Fwind, h);
                 b1.thrust = half_of(bd.thrust, h); b1.cxy = half_of(bd.cxy, h); b1.dcz = half_of(bd.dcz, h); b1.gndT = half_of(bd.gndT, h);
                 b1.inv_m = half_of(bd.inv_m, h); b1.ng = half_of(bd.ng, h); b1.ndwc = half_of(bd.ndwc, h);
-                const RedoOut o = redo_item_exact<G, FEAT, DEG>(P, S[(st * wpb + wib) * NP + h], b1, lane, j, full_group);
+                const RedoOut o = redo_item_exact<G, FEAT, DEG>(P, B.P0 + sl[h].drone, B.P1 + sl[h].drone, B.P2 + sl[h].drone, B.P3 + sl[h].drone, b1, j, full_group);
                 sl[h].hit = o.hit;
 #pragma unroll
                 for (int i = 0; i < 13; ++i) r[h][i] = o.s[i];
@@ -721,26 +728,18 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     if (flush) { publish_flag(pending); publish_flag(pending2); pending = pending2 = 0xFFFFFFFFu; }
     const unsigned wt_after = take(drawn_l0);
     const unsigned probed_after = probe(wt_after);
-    touched = 0u;
 #pragma unroll
-    for (int h = 0; h < NP; ++h) {                                // back from the landing zone: controller memory, target, action row, env word
+    for (int h = 0; h < NP; ++h) {                                // back from the stash: controller memory, target, env word, action row
         Slot& s = sl[h];
-        const WarpStage& W = S[(st * wpb + wib) * NP + h];
-        const float4 f = W.plane[3][lane];
+        const float4* const st4 = stash0 + ((size_t)(wib * NP + h) * n_stash) * 32 + lane;
+        const float4 f = st4[iIP * 32];
         s.d.Ip = v3(f.y, f.z, f.w);
-        if (pid) {
-            const float4 i4 = W.plane[4][lane];
-            s.d.Ie = v3(i4.x, i4.y, i4.z);
-            touched |= __float_as_uint(i4.x);
-            if (F::act(P) == 1) { s.d.sp = W.plane[5][lane]; touched |= __float_as_uint(s.d.sp.x); }
-        }
-        s.tg = W.plane[6][lane];
-        s.act4 = W.plane[7][lane];
-        s.env4 = W.plane[8][lane];
-        touched |= __float_as_uint(f.y) | __float_as_uint(s.tg.x) | __float_as_uint(s.act4.x) | __float_as_uint(s.env4.x);
+        s.tg = st4[iTG * 32];
+        s.env4 = st4[iENV * 32];
+        if (pid) { const float4 i4 = st4[iIE * 32]; s.d.Ie = v3(i4.x, i4.y, i4.z); }
+        if (F::act(P) == 1) s.d.sp = st4[iSP * 32];
+        if (obs_kin20) s.act4 = st4[iACT * 32];
     }
-    // one landing zone: it is free now; the next item's copies overlap the epilogue
-    if (!flip && wt_next < n_items) { await_item(wt_next, probed_next); prefetch(wt_next, st, touched & P.zero); }
 #pragma unroll
     for (int h = 0; h < NP; ++h) {
         Slot& s = sl[h];
@@ -888,7 +887,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     }
     if (pending == 0xFFFFFFFFu) pending = wt; else pending2 = wt;
     if (wt_next >= n_items) break;
-    wt = wt_next; wt_next = wt_after; probed_next = probed_after; st ^= flip;
+    wt = wt_next; wt_next = wt_after; probed_next = probed_after;
     }   // work-item loop
     __threadfence();
     publish_flag(pending);
