@@ -154,7 +154,9 @@ typedef struct mdg_params {
 
 typedef struct mdg_env mdg_env; /* opaque; the library owns it and all its device buffers */
 
-/* Fill *out with Table 2 (drone_model), Table 6 and the documented defaults.  host pointer. */
+/* Fill *out (host pointer, caller-owned) with Table 2 of the drone model, the PIDControl gains of Table 6
+ * (PAPER.md:365-372), the Eq.4-6 coefficients and the documented defaults of every other field.
+ * MDG_EINVAL: NULL, unknown drone_model. */
 int mdg_default_params(int drone_model, mdg_params* out);
 
 /* Kernel selection: the five BASELINE configs and a few variants have precompiled instances of the step kernel; for any other
@@ -165,14 +167,21 @@ int mdg_default_params(int drone_model, mdg_params* out);
  * kernel, MDG_JIT=require makes mdg_create fail with MDG_ECUDA instead of falling back; MDG_JIT_SRC overrides the directory
  * the sources are read from.
  *
- * Create n_envs environments of n_drones (1..32) drones each.  physics_mode: Table 1; action_type:
- * Table 3.  params (host, copied) may be NULL for the CF2X defaults.  *out receives the handle. */
+ * Create n_envs environments of n_drones (1..32) drones each: the constructor of PAPER.md:169 (drone model, num_drones,
+ * physics, sim / ctrl frequency, obs and act type) and, for the batch, MJXVectorAviary's num_envs.
+ * physics_mode: Table 1; action_type: Table 3.  params (host, copied) may be NULL for the
+ * CF2X defaults.  *out receives the handle; it owns all device memory (one arena) until mdg_destroy.  The state is that of
+ * mdg_reset(env, 0).  Errors: MDG_EINVAL (see the code's comment above), MDG_ENOMEM, MDG_ECUDA (no device: no CPU fallback). */
 int mdg_create(int n_envs, int n_drones, int physics_mode, int action_type, const mdg_params* params,
                mdg_env** out);
+/* Free the handle and everything it owns (synchronises its stream).  NULL is ignored. */
 void mdg_destroy(mdg_env* env);
 
-/* Draw every env's initial state from Philox4x32-10 keyed by seed (counter = env, drone, 0, stream);
- * zero controller memory, wind and step counters; obs is valid afterwards (reward 0, done 0). */
+/* The paper's `reset(rng) -> state` for the whole batch (per-env PRNG key, step counter and done flag of
+ * MJXState): draw every env's initial state (Table 4's initial-state ranges when set) and
+ * per-episode targets from Philox4x32-10 keyed by seed (counter = env_index_base + env, drone, 0, stream);
+ * zero controller memory, wind and step counters; obs is valid afterwards (reward 0, done 0).  Asynchronous on the bound
+ * stream.  MDG_EINVAL: NULL handle. */
 int mdg_reset(mdg_env* env, uint64_t seed);
 
 /* One control step: the paper's `step(state, action) -> state, obs, reward, done` for every env, i.e. action
@@ -205,10 +214,12 @@ int mdg_step_chained(mdg_env* env, const float* actions_dev);
  * MDG_EINVAL: NULL, n_steps < 1, misaligned pointer or stride. */
 int mdg_step_many(mdg_env* env, const float* actions_dev, int n_steps, int64_t stride_floats);
 
-/* One control step with HOST buffers (the end-to-end call): copies actions_host [n_envs*n_drones][4] to
+/* One control step (exactly mdg_step) with HOST buffers, the end-to-end call a Gymnasium-style host loop
+ * makes: copies actions_host [n_envs*n_drones][4] to
  * the device, steps, copies obs / reward / done back (NULL outputs are skipped) and synchronises the
  * stream, so the results are valid on return.  Pinned host memory makes the copies asynchronous
- * with respect to the host but the call still returns only after they finish. */
+ * with respect to the host but the call still returns only after they finish.  obs_host [n_envs][mdg_obs_dim] fp32,
+ * reward_host [n_envs] fp32, done_host [n_envs] u8; all caller-owned.  MDG_EINVAL: NULL handle or actions. */
 int mdg_step_host(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
 
 /* The same call split in two, for double-buffering several handles (each bound to its own stream with mdg_set_stream) so that
@@ -219,20 +230,26 @@ int mdg_step_host(mdg_env* env, const float* actions_host, float* obs_host, floa
 int mdg_step_host_async(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
 int mdg_wait(mdg_env* env);
 
-/* Device pointers to the library-owned outputs of the last reset/step:
+/* Device pointers to the library-owned outputs of the last reset/step (`obs, reward, done` of PAPER.md:285-289; observation
+ * rows PAPER.md:177, rewards and termination rules PAPER.md:304-333):
  * obs [n_envs][mdg_obs_dim] fp32 (per drone: the MDG_OBS_* row, e.g. p, roll/pitch/yaw, v, body rates [, adjacency row]);
  * reward [n_envs] fp32; done [n_envs] u8 (bit0 terminated, bit1 truncated).  Any may be NULL. */
 int mdg_outputs(mdg_env* env, const float** obs_dev, const float** reward_dev, const uint8_t** done_dev);
-int mdg_obs_dim(const mdg_env* env); /* floats per env */
+int mdg_obs_dim(const mdg_env* env); /* floats per env = n_drones x the MDG_OBS_* row length; negative code on NULL */
 
-/* Device pointer to the per-episode targets [n_envs*n_drones][4] = (x, y, z, psi), fp32. */
+/* Device pointer to the per-episode targets [n_envs*n_drones][4] = (x, y, z, psi), fp32: the task's hover point, velocity
+ * target, waypoint or formation slot.  Library-owned, rewritten by reset / auto-reset (and every step for
+ * waypoint and moving-formation tasks). */
 int mdg_targets(mdg_env* env, const float** targets_dev);
 
-/* Harness action generator (Philox stream 3, counter = env, drone, t, 3):
- * out_dev[(e*n_drones+i)*4 + c] = base * fma(hi - lo, u_c, lo), every operation rounded to fp32. */
+/* Harness action generator, not part of the paper's method (it stands in for the policy of PAPER.md:285-292 so that tests and
+ * bench.py can produce seeded actions on the device).  Philox stream 3, counter = (env_index_base + env, drone, t, 3):
+ * out_dev[(e*n_drones+i)*4 + c] = base * fma(hi - lo, u_c, lo), every operation rounded to fp32.  out_dev: caller-owned
+ * device memory, 16-byte aligned.  Asynchronous on the bound stream. */
 int mdg_gen_actions(mdg_env* env, uint64_t seed, uint32_t t, float base, float lo, float hi, float* out_dev);
 
-/* Checkpoint / test hooks (host pointers; synchronise the stream).
+/* Checkpoint / test hooks (host pointers; synchronise the stream): the kinematic part of the paper's per-env state
+ * (MJXState's qpos / qvel, step counter: PAPER.md:254-258; controller memory of PAPER.md:347-357).
  * state: [D][13] = p(3) q(4, w x y z) v(3) body rates(3);  ctrl: [D][10] = I_p(3) I_eta(3) held
  * setpoint(4);  targets: [D][4];  wind: [n_envs][3];  ep_step: [n_envs] u32.  D = n_envs*n_drones.
  * NULL pointers are skipped.  mdg_set_state recomputes obs. */
@@ -240,7 +257,8 @@ int mdg_get_state(mdg_env* env, float* state, float* ctrl, float* targets, float
 int mdg_set_state(mdg_env* env, const float* state, const float* ctrl, const float* targets,
                   const float* wind, const uint32_t* ep_step);
 
-/* Full checkpoint / resume.  mdg_get_state covers the kinematic state for tests; a running simulation also carries the DR
+/* Full checkpoint / resume of everything MJXState carries (data, step counter, PRNG key, done) and this
+ * library adds.  mdg_get_state covers the kinematic state for tests; a running simulation also carries the DR
  * factors, rotor speeds (motor lag), gust impulses, action history (action latency), step counters, the seed and the last
  * outputs.  mdg_save writes all of it to host memory as one opaque blob of mdg_checkpoint_size bytes; mdg_load restores it
  * into a handle created with the same n_envs, n_drones, modes and params, after which stepping continues bit for bit as
@@ -255,7 +273,7 @@ int mdg_load(mdg_env* env, const void* host_buf, int64_t buf_bytes);
  * env add up to its reward.  Library-owned, valid until mdg_destroy; written by every mdg_step. */
 int mdg_reward_per_drone(mdg_env* env, const float** reward_dev);
 
-/* Domain-randomisation factors of the running episodes, host [D][16] = [m, J, k_f, k_m, drag, C_gnd, C_1, g, motor bias x4,
+/* Domain-randomisation factors of the running episodes (Table 4), host [D][16] = [m, J, k_f, k_m, drag, C_gnd, C_1, g, motor bias x4,
  * arm, MAX_RPM, motor-lag time constant (s; 1 when off), 1] (synchronise).
  * mdg_set_dr fails with MDG_EINVAL when every dr_alpha is 0 (the factors are then not read by the step). */
 int mdg_get_dr(mdg_env* env, float* factors);
@@ -276,7 +294,8 @@ typedef struct mdg_cam_params {
     float body_radius, body_half_height;   /* arm + propeller radius of the drone model; 0.0125 m */
 } mdg_cam_params;
 
-/* Fill *out with the defaults above; params (host, may be NULL = CF2X) supplies arm length and propeller radius. */
+/* Fill *out with the defaults above (48 x 64, 60 degrees, offset [0.02, 0, 0]); params (host, may be NULL =
+ * CF2X) supplies arm length and propeller radius (Table 2).  MDG_EINVAL: NULL out. */
 int mdg_default_cam_params(const mdg_params* params, mdg_cam_params* out);
 
 /* Render every drone's camera from the CURRENT state (after the last reset / step on the bound stream; asynchronous on it).
@@ -293,10 +312,13 @@ int mdg_render_depth(mdg_env* env, const mdg_cam_params* cam, float* depth_dev, 
  * inside a capture the ordering is the caller's graph).  MDG_EINVAL: NULL handle.  (The simulator itself has no notion of streams; this serves PAPER.md:292, keeping the loop on the device.) */
 int mdg_set_stream(mdg_env* env, void* cuda_stream);
 
-/* Introspection: kernels launched so far through this handle; name of the step kernel specialisation. */
+/* Introspection (no counterpart in the paper; bench.py's `gpu_launches` and the tests use them): kernels launched so far
+ * through this handle; name of the step kernel specialisation ("step_kernel<G, feature word, blocks/SM[, x2]>", "jit" or
+ * "generic" inside it says how it was built; the string lives as long as the handle). */
 int64_t mdg_launch_count(const mdg_env* env);
 const char* mdg_kernel_name(const mdg_env* env);
-/* Launch shape tuning (0 keeps the current value): threads per block, and a cap on resident blocks per SM. */
+/* Launch shape tuning (0 keeps the current value): threads per block (a multiple of 32 in [32, 128]), and a cap on resident blocks
+ * per SM (1..32).  Results do not depend on the launch shape.  Drops cached graphs.  MDG_EINVAL: NULL handle, bad block size. */
 int mdg_set_launch(mdg_env* env, int block_threads, int max_blocks_per_sm);
 
 /* Measurement aid for the roofline denominator: runs a register-only FFMA kernel (8 independent
@@ -304,7 +326,10 @@ int mdg_set_launch(mdg_env* env, int block_threads, int max_blocks_per_sm);
  * the achieved FP32 rate in TFLOP/s (2 flop per FFMA) to *tflops (host pointer).  Synchronises the stream. */
 int mdg_measure_fp32_peak(void* cuda_stream, double* tflops);
 
+/* Thread-local text of the last failure in this thread (or the note a successful mdg_create left about a kernel fallback);
+ * never NULL. */
 const char* mdg_last_error(void);
+/* Library version; checkpoints of another version are refused by mdg_load. */
 int mdg_version(void);
 
 #ifdef __cplusplus
