@@ -181,8 +181,8 @@ template <bool EULER> __device__ __forceinline__ void redo_fast_spin(const DevPa
 // What a lane integrates over the substeps: one drone (T = float) or the same drone index of two envs (T = F2).
 template <class T> struct Body {
     V3T<T> p; Q4T<T> q; V3T<T> v, w;                              // state, w in the body frame
-    V3T<T> tau_b, k1_tau, Fwind;                                  // frozen over a substep: Eq.1-3 torque, J^-1 tau, wind force
-    T thrust, cxy, dcz, gndT, inv_m, ng, ndwc;                    // thrust, Eq.5 / Eq.4 coefficients x rotor terms, 1/m, -g, -Eq.6 coefficient
+    V3T<T> tau_b, k1_tau, a0;                                     // frozen over a substep: Eq.1-3 torque, J^-1 tau; wind force / m - g z
+    T thrust, cxy, dcz, gndT, ndwc;                               // thrust, Eq.5 / Eq.4 coefficients x rotor terms, -Eq.6 coefficient: all / m
 };
 // One physics substep (S4-S8): world-frame force from the start-of-substep state, then the free-body update with the wrench
 // frozen.  Returns "went through the floor" (clamped).  The downwash exchange is a shuffle inside the G-lane group.
@@ -196,12 +196,12 @@ __device__ __forceinline__ SubstepFlags<T> substep(const DevParams& P, Body<T>& 
     const T bx = mul_(2.0f, fma_(s.q.x, s.q.z, mul_(s.q.w, s.q.y)));
     const T by = mul_(2.0f, fma_(s.q.y, s.q.z, mul_(neg_(s.q.w), s.q.x)));
     const T bz = fma_(-2.0f, fma_(s.q.x, s.q.x, mul_(s.q.y, s.q.y)), 1.0f);
+    // every coefficient already carries 1 / m and a0 = F_wind / m - g z, so the sums below are the acceleration itself
     V3T<T> Fw;
     if (F::has(P, F_DRAG)) {
         const T sc = fma_(s.dcz, fma_(bx, s.v.x, fma_(by, s.v.y, mul_(bz, s.v.z))), s.thrust);
-        Fw = v3t<T>(fma_(sc, bx, mul_(s.cxy, s.v.x)), fma_(sc, by, mul_(s.cxy, s.v.y)), fma_(sc, bz, mul_(s.cxy, s.v.z)));
-    } else Fw = v3t<T>(fma_(s.thrust, bx, 0.0f), fma_(s.thrust, by, 0.0f), fma_(s.thrust, bz, 0.0f));   // (fma, not mul: see ang_acc_t)
-    if (F::has(P, F_WIND)) { Fw.x = add_(Fw.x, s.Fwind.x); Fw.y = add_(Fw.y, s.Fwind.y); Fw.z = add_(Fw.z, s.Fwind.z); }
+        Fw = v3t<T>(fma_(sc, bx, fma_(s.cxy, s.v.x, s.a0.x)), fma_(sc, by, fma_(s.cxy, s.v.y, s.a0.y)), fma_(sc, bz, fma_(s.cxy, s.v.z, s.a0.z)));
+    } else Fw = v3t<T>(fma_(s.thrust, bx, s.a0.x), fma_(s.thrust, by, s.a0.y), fma_(s.thrust, bz, s.a0.z));
     if (F::has(P, F_GND)) {                                       // Eq.4, gated on body z pointing up
         const T hgt = max_(s.p.z, P.h_clip);
         const T gain = mul_(s.gndT, rcp_(mul_(hgt, hgt)));
@@ -240,7 +240,7 @@ __device__ __forceinline__ SubstepFlags<T> substep(const DevParams& P, Body<T>& 
         }
         Fw.z = fma_(s.ndwc, dw, Fw.z);
     }
-    const V3T<T> acc = v3t<T>(mul_(Fw.x, s.inv_m), mul_(Fw.y, s.inv_m), fma_(Fw.z, s.inv_m, s.ng));
+    const V3T<T> acc = Fw;
 
     // S8 integrate with the wrench frozen in the world frame
     const typename LaneOps<T>::mask fast_spin = gt_(dot3(s.w, s.w), P.w2_exact[DEG - 2]);
@@ -636,9 +636,11 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
         if (F::has(P, F_WIND) && !F::has(P, F_WIND_MIX)) {        // PAPER.md:201 drag law on the gust just updated: F = k_w |u - v| (u - v) (Q28)
             const V3T<T> rel = v3t<T>(sub_(MDG_PK(env4.x), bd.v.x), sub_(MDG_PK(env4.y), bd.v.y), sub_(MDG_PK(env4.z), bd.v.z));
             const T kn = mul_(P.k_wind, sqrt_(dot3(rel, rel)));
-            bd.Fwind = v3t<T>(mul_(kn, rel.x), mul_(kn, rel.y), mul_(kn, rel.z));
-        } else bd.Fwind = v3t<T>(MDG_PK(Fwind.x), MDG_PK(Fwind.y), MDG_PK(Fwind.z));
-        bd.inv_m = MDG_PK(inv_m_e); bd.ng = pack_lanes(np, -s0.g_e, -s1.g_e); bd.ndwc = pack_lanes(np, -s0.dwc_e, -s1.dwc_e);
+            bd.a0 = v3t<T>(mul_(kn, rel.x), mul_(kn, rel.y), mul_(kn, rel.z));
+        } else bd.a0 = v3t<T>(MDG_PK(Fwind.x), MDG_PK(Fwind.y), MDG_PK(Fwind.z));
+        const T inv_m = MDG_PK(inv_m_e);                          // 1 / m folded into everything the substeps sum up
+        bd.a0 = v3t<T>(fma_(bd.a0.x, inv_m, 0.0f), fma_(bd.a0.y, inv_m, 0.0f), fma_(bd.a0.z, inv_m, pack_lanes(np, -s0.g_e, -s1.g_e)));
+        bd.ndwc = mul_(pack_lanes(np, -s0.dwc_e, -s1.dwc_e), inv_m);
         // S3 motor model (Eq.1-3) as a function of the rotor speeds: once per step, or every substep under the motor lag.  Every
         // product and sum is spelled out (mdg_dev.cuh: lane-generic arithmetic), so one env per lane and two round identically.
         auto motor_model = [&](const T (&nn)[4]) {
@@ -650,7 +652,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             const T f0 = fma_(k0, mul_(nn[0], nn[0]), 0.0f), f1 = fma_(k1, mul_(nn[1], nn[1]), 0.0f), f2 = fma_(k2, mul_(nn[2], nn[2]), 0.0f),
                     f3 = fma_(k3, mul_(nn[3], nn[3]), 0.0f);
             const T f01 = add_(f0, f1), f23 = add_(f2, f3), f12 = add_(f1, f2), f03 = add_(f0, f3), f13 = add_(f1, f3), f02 = add_(f0, f2);
-            bd.thrust = add_(f01, f23);
+            const T thrust = add_(f01, f23);
+            bd.thrust = fma_(thrust, inv_m, 0.0f);
             const T tz = mul_(MDG_PK(kappa_e), sub_(f13, f02));
             V3T<T> tau = F::has(P, F_CF2P) ? v3t<T>(mul_(P.arm, sub_(f1, f3)), mul_(P.arm, sub_(f2, f0)), tz)
                                             : v3t<T>(mul_(P.l, sub_(f01, f23)), mul_(P.l, sub_(f12, f03)), tz);
@@ -661,10 +664,11 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             const T Om = mul_(P.rpm2rad, add_(add_(nn[0], nn[1]), add_(nn[2], nn[3])));
             bd.tau_b = tau;
             bd.k1_tau = v3t<T>(mul_(P.invJ[0], tau.x), mul_(P.invJ[1], tau.y), mul_(P.invJ[2], tau.z));
-            bd.cxy = dr ? mul_(mul_(-P.c_xy, MDG_PK(dr1.x)), Om) : mul_(-P.c_xy, Om);
+            const T cxy = dr ? mul_(mul_(-P.c_xy, MDG_PK(dr1.x)), Om) : mul_(-P.c_xy, Om);
             const T cz = dr ? fma_(mul_(-P.c_z, MDG_PK(dr1.x)), Om, 0.0f) : fma_(-P.c_z, Om, 0.0f);
             bd.gndT = dr ? mul_(mul_(P.gnd_coef, MDG_PK(dr1.y)), bd.thrust) : mul_(P.gnd_coef, bd.thrust);
-            bd.dcz = sub_(cz, bd.cxy);
+            bd.cxy = fma_(cxy, inv_m, 0.0f);
+            bd.dcz = mul_(sub_(cz, cxy), inv_m);
         };
         if (!lag) motor_model(nn);
         bool spun = false;                                         // two envs per lane: some substep was outside the series' range
@@ -701,9 +705,9 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
 #pragma unroll
             for (int h = 0; h < NP; ++h) {
                 Body<float> b1;
-                b1.tau_b = half3(bd.tau_b, h); b1.k1_tau = half3(bd.k1_tau, h); b1.Fwind = half3(bd.Fwind, h);
+                b1.tau_b = half3(bd.tau_b, h); b1.k1_tau = half3(bd.k1_tau, h); b1.a0 = half3(bd.a0, h);
                 b1.thrust = half_of(bd.thrust, h); b1.cxy = half_of(bd.cxy, h); b1.dcz = half_of(bd.dcz, h); b1.gndT = half_of(bd.gndT, h);
-                b1.inv_m = half_of(bd.inv_m, h); b1.ng = half_of(bd.ng, h); b1.ndwc = half_of(bd.ndwc, h);
+                b1.ndwc = half_of(bd.ndwc, h);
                 const RedoOut o = redo_item_exact<G, FEAT, DEG>(P, B.P0 + sl[h].drone, B.P1 + sl[h].drone, B.P2 + sl[h].drone, B.P3 + sl[h].drone, b1, j, full_group);
                 sl[h].hit = o.hit;
 #pragma unroll
