@@ -123,6 +123,11 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
         D.expC[0] = 1.0f; D.expC[1] = (float)(-c2 / 8.0); D.expC[2] = (float)(c2 * c2 / 384.0); D.expC[3] = (float)(-c2 * c2 * c2 / 46080.0);
         D.expS[0] = (float)(c / 2.0); D.expS[1] = (float)(-c * c2 / 48.0); D.expS[2] = (float)(c * c2 * c2 / 3840.0); D.expS[3] = (float)(-c * c2 * c2 * c2 / 645120.0);
     }
+    {                                                             // the same for phi = h s (s = the RK4 mean of the stage rates)
+        const double c = h, c2 = c * c;
+        D.expCm[0] = 1.0f; D.expCm[1] = (float)(-c2 / 8.0); D.expCm[2] = (float)(c2 * c2 / 384.0); D.expCm[3] = (float)(-c2 * c2 * c2 / 46080.0);
+        D.expSm[0] = (float)(c / 2.0); D.expSm[1] = (float)(-c * c2 / 48.0); D.expSm[2] = (float)(c * c2 * c2 / 3840.0); D.expSm[3] = (float)(-c * c2 * c2 * c2 / 645120.0);
+    }
     D.inv_m = (float)(1.0 / p.m); D.g = p.g; D.m = p.m; D.inv_g = (float)(1.0 / p.g);
     for (int i = 0; i < 3; ++i) { D.J[i] = p.J[i]; D.invJ[i] = (float)(1.0 / p.J[i]); }
     D.gyro[0] = (float)(((double)p.J[2] - p.J[1]) / p.J[0]);

@@ -45,7 +45,7 @@ struct DevParams {
     float rotA_half[4], rotB_half[4], rotA_full[4], rotB_full[4];
     float rotnA_half[4], rotnA_full[4], ngyro[3];            // -A's coefficients and -gyro: the lane-generic substep loop never negates
     // Eq.7 increment for phi = (h/6) s, s = w0 + 2 w2 + 2 w3 + w4, as polynomials in |s|^2: cos(|phi|/2) and (h/6) sin(|phi|/2)/|phi|
-    float expC[4], expS[4];
+    float expC[4], expS[4], expCm[4], expSm[4];   // Eq.7 series for phi = (h/6) s and for phi = h s
     float inv_m, g, J[3], invJ[3], gyro[3];               // gyro = ((Jz-Jy)/Jx, (Jx-Jz)/Jy, (Jy-Jx)/Jz)
     // motor model (Eq.1-3)
     float k_f, inv_k_f, l, kappa, inv_l, inv_kappa, max_rpm, s_max, T_max, rpm2rad;

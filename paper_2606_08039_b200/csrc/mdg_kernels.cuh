@@ -135,18 +135,20 @@ __device__ __forceinline__ void integrate_rot_t(const DevParams& P, Q4T<T>& q, V
         const V3T<T> k3 = ang_acc_t(P, stage_torque_t<DEG>(P.rotnA_half, P.rotB_half, w2, tau_b), w3, axisym);
         const V3T<T> w4 = v3t<T>(fma_(P.h, k3.x, w0.x), fma_(P.h, k3.y, w0.y), fma_(P.h, k3.z, w0.z));
         const V3T<T> k4 = ang_acc_t(P, stage_torque_t<DEG>(P.rotnA_full, P.rotB_full, w3, tau_b), w4, axisym);
-        const V3T<T> ws = v3t<T>(add_(fma_(add_(w2.x, w3.x), 2.0f, w0.x), w4.x), add_(fma_(add_(w2.y, w3.y), 2.0f, w0.y), w4.y),
-                                 add_(fma_(add_(w2.z, w3.z), 2.0f, w0.z), w4.z));          // w0 + 2 (w2 + w3) + w4
-        q = qmul_t(q, exp_half_scaled_t<DEG>(P.expC, P.expS, ws));
-        w = v3t<T>(fma_(P.h_sixth, add_(fma_(add_(k2.x, k3.x), 2.0f, k1.x), k4.x), w0.x),
-                   fma_(P.h_sixth, add_(fma_(add_(k2.y, k3.y), 2.0f, k1.y), k4.y), w0.y),
-                   fma_(P.h_sixth, add_(fma_(add_(k2.z, k3.z), 2.0f, k1.z), k4.z), w0.z));
+        // Eq.7 with the RK4 mean of the stage rates, (w0 + 2 w2 + 2 w3 + w4) / 6 = w0 + h/6 (k1 + k2 + k3), and the rate update
+        // w0 + h/6 (k1 + 2 k2 + 2 k3 + k4) share k2 + k3 and k1 + k2 + k3
+        const V3T<T> k23 = v3t<T>(add_(k2.x, k3.x), add_(k2.y, k3.y), add_(k2.z, k3.z));
+        const V3T<T> ks = v3t<T>(add_(k1.x, k23.x), add_(k1.y, k23.y), add_(k1.z, k23.z));
+        const V3T<T> wm = v3t<T>(fma_(P.h_sixth, ks.x, w0.x), fma_(P.h_sixth, ks.y, w0.y), fma_(P.h_sixth, ks.z, w0.z));
+        q = qmul_t(q, exp_half_scaled_t<DEG>(P.expCm, P.expSm, wm));
+        w = v3t<T>(fma_(P.h_sixth, add_(add_(ks.x, k23.x), k4.x), w0.x), fma_(P.h_sixth, add_(add_(ks.y, k23.y), k4.y), w0.y),
+                   fma_(P.h_sixth, add_(add_(ks.z, k23.z), k4.z), w0.z));
     } else {
         const V3T<T> k1 = ang_acc_t(P, tau_b, w, axisym);
         w = v3t<T>(fma_(P.h, k1.x, w.x), fma_(P.h, k1.y, w.y), fma_(P.h, k1.z, w.z));
         q = qmul_t(q, exp_half_t(v3t<T>(mul_(P.h, w.x), mul_(P.h, w.y), mul_(P.h, w.z))));
     }
-    const T rn = rsqrt_(fma_(q.w, q.w, fma_(q.x, q.x, fma_(q.y, q.y, mul_(q.z, q.z)))));
+    const T rn = rsqrt_(fma_(q.w, q.w, fma_(q.x, q.x, fma_(q.y, q.y, mul_(q.z, q.z)))));   // (1.5 - 0.5 |q|^2 instead of the MUFU: measured slower, the FP32 pipe is the busy one)
     q.w = mul_(q.w, rn); q.x = mul_(q.x, rn); q.y = mul_(q.y, rn); q.z = mul_(q.z, rn);
 }
 // fast spins (|omega| h above the series' range): redo the rotation update from the start-of-substep values with the library
@@ -208,8 +210,8 @@ __device__ __forceinline__ SubstepFlags<T> substep(const DevParams& P, Body<T>& 
         Fw.z = add_(Fw.z, sel_(gt_(bz, 0.0f), gain, 0.0f));
     }
     if (G > 1 && F::has(P, F_DW)) {                               // Eq.6 over every drone above this one
-        // With b' = sqrt(2 ln 2) beta: exp(-dxy^2 / 2 beta^2) = 2^(-dxy^2 / b'^2) and alpha = C1 (r_p/4)^2 / dz_e^2.
-        // One reciprocal r = 1 / (dz_e^2 b'^2) serves both: alpha ~ b'^2 r, exponent = -dxy^2 (dz_e^2 r).
+        // With b' = sqrt(2 ln 2) beta: exp(-dxy^2 / 2 beta^2) = 2^(-dxy^2 / b'^2) and alpha = C1 (r_p/4)^2 / dz_e^2: two MUFU
+        // reciprocals (the XU pipe is idle most of the time; one shared reciprocal costs three more multiplies on the FP32 pipe).
         // The ramp saturate(dz / dz_clip) is 0 for dz <= 0, which also gates "k above this drone";
         // b'^2 is floored (beta^2 >= 1e-12), which reproduces the beta -> 0 rule of DESIGN.md Q9.
         // Pairs are shared out: in round r < G/2 lane j evaluates the pair (j, j + r mod G) once for both ends -
@@ -227,9 +229,8 @@ __device__ __forceinline__ SubstepFlags<T> substep(const DevParams& P, Body<T>& 
             const T ramp = sat_(mul_(adz, P.inv_dz_clip));
             const T bs = fma_(P.dw_C2s, dze, P.dw_C3s);
             const T b2 = max_(mul_(bs, bs), P.dw_b2_min), z2 = mul_(dze, dze);
-            const T rinv = rcp_(mul_(z2, b2));
-            const T ex = ex2n_(mul_(dxy2, mul_(z2, rinv)));
-            const T al = mul_(ramp, mul_(b2, rinv));
+            const T ex = ex2n_(mul_(dxy2, rcp_(b2)));
+            const T al = mul_(ramp, rcp_(z2));
             const bool on = full_group || (j < P.M && ((j + r) & (G - 1)) < P.M);
             const T f = sel_(and_(lt_(dxy2, 100.0f), on), mul_(al, ex), 0.0f);
             const typename LaneOps<T>::mask above = gt_(dz, 0.0f);   // the partner is above this drone
