@@ -230,6 +230,21 @@ int mdg_step_host(mdg_env* env, const float* actions_host, float* obs_host, floa
 int mdg_step_host_async(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
 int mdg_wait(mdg_env* env);
 
+/* mdg_step_host for callers that must not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same control step with the same arguments, results and
+ * synchronisation as mdg_step_host, but the device staging buffer of the actions is a static device array inside the library
+ * instead of a buffer mdg_step_host cudaMallocs on a handle's first call.  The call allocates and frees nothing, on the host
+ * side of CUDA or the device.  Limits and caveats:
+ *  - the array holds MDG_STATIC_STAGE_MAX_DRONES action rows (4 MiB; every GPU that loads the library holds it until the
+ *    process exits); a handle with n_envs * n_drones beyond that gets MDG_EINVAL and a message naming both numbers;
+ *  - there is ONE array per GPU, shared by every handle and thread of the process: calls that overlap on the GPU (two
+ *    threads, each on its own handle and stream) race on it and step with mixed actions - serialise them, or use
+ *    mdg_step_host, whose staging buffer is per handle.  The call itself returns only after its own work has finished;
+ *  - the array keeps the previous call's rows; nothing in it has to start at zero, the call overwrites every row it reads.
+ * Errors: MDG_EINVAL (NULL handle or actions, too many drones), MDG_ECUDA. */
+#define MDG_STATIC_STAGE_MAX_DRONES 262144
+int mdg_step_host_static(mdg_env* env, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host);
+
 /* Device pointers to the library-owned outputs of the last reset/step (`obs, reward, done` of PAPER.md:285-289; observation
  * rows PAPER.md:177, rewards and termination rules PAPER.md:304-333):
  * obs [n_envs][mdg_obs_dim] fp32 (per drone: the MDG_OBS_* row, e.g. p, roll/pitch/yaw, v, body rates [, adjacency row]);

@@ -6,6 +6,7 @@ import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmdg.so")
+STATIC_STAGE_MAX_DRONES = 262144     # include/mdg.h: MDG_STATIC_STAGE_MAX_DRONES
 
 MDG_OK, MDG_EINVAL, MDG_ECUDA, MDG_ENOMEM = 0, -1, -2, -3
 
@@ -62,7 +63,7 @@ class mdg_cam_params(C.Structure):
     update = mdg_params.update
 
 
-EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_chained", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_wait", "mdg_checkpoint_size", "mdg_save", "mdg_load", "mdg_outputs",
+EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_chained", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_step_host_static", "mdg_wait", "mdg_checkpoint_size", "mdg_save", "mdg_load", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
            "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_last_error", "mdg_version"]
 
@@ -88,6 +89,7 @@ def lib():
         L.mdg_step_many.argtypes = [vp, vp, C.c_int, C.c_int64]
         L.mdg_step_host.argtypes = [vp] * 5
         L.mdg_step_host_async.argtypes = [vp] * 5
+        L.mdg_step_host_static.argtypes = [vp] * 5
         L.mdg_wait.argtypes = [vp]
         L.mdg_checkpoint_size.argtypes = [vp]
         L.mdg_checkpoint_size.restype = C.c_int64
@@ -241,6 +243,15 @@ class Env:
             raise ValueError("actions_host must be a host float32 tensor of n_envs*n_drones*4 elements")
         fn = lib().mdg_step_host_async if asynchronous else lib().mdg_step_host
         _check(fn(self._h, ptr(actions_host), ptr(obs_host), ptr(reward_host), ptr(done_host)))
+
+    def step_host_static(self, actions_host, obs_host=None, reward_host=None, done_host=None):
+        """step_host without any allocation: the actions are staged in the library's static device array (mdg_step_host_static;
+        at most STATIC_STAGE_MAX_DRONES drones per handle, one array per GPU shared by all handles)."""
+        def ptr(x):
+            return C.c_void_p(None) if x is None else C.c_void_p(x.data_ptr())
+        if actions_host.is_cuda or actions_host.numel() != self.n_envs * self.n_drones * 4:
+            raise ValueError("actions_host must be a host float32 tensor of n_envs*n_drones*4 elements")
+        _check(lib().mdg_step_host_static(self._h, ptr(actions_host), ptr(obs_host), ptr(reward_host), ptr(done_host)))
 
     def save(self):
         """Full checkpoint as a numpy uint8 array (include/mdg.h: mdg_save)."""

@@ -906,6 +906,52 @@ extern "C" int mdg_step_host(mdg_env* h, const float* actions_host, float* obs_h
     const int rc = mdg_step_host_async(h, actions_host, obs_host, reward_host, done_host);
     return rc != MDG_OK ? rc : mdg_wait(h);
 }
+// ---- mdg_step_host without any allocation --------------------------------------------------------------------------
+// mdg_step_host_async cudaMallocs its device staging buffer on a handle's first call.  Callers that must not allocate (a serving
+// loop, code under stream capture, harnesses that forbid it) get the same step with the staging buffer in a file-scope device
+// array: MDG_STATIC_STAGE_MAX_DRONES action rows of 16 bytes = 4 MiB, held by every GPU that loads the library until exit.
+// In host code `g_static_stage` is only the host-side stand-in of the symbol, never a device address: the address is looked up
+// once per device, with that device current, and that pointer is what the copy and the kernel get.
+static __device__ __align__(256) float g_static_stage[(size_t)MDG_STATIC_STAGE_MAX_DRONES * 4];
+static constexpr int kMaxDevices = 64;
+static std::mutex g_static_stage_mu;
+static float* g_static_stage_ptr[kMaxDevices] = {};
+
+// Device address of g_static_stage on the CURRENT device (resolved at the first use on that device; allocates nothing).
+static int static_stage_address(float** out) {
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(MDG_EINVAL, "mdg_step_host_static: device ordinal out of range");
+    std::lock_guard<std::mutex> lk(g_static_stage_mu);
+    if (!g_static_stage_ptr[dev]) {
+        float* ptr = nullptr;
+        const cudaError_t ce = cudaGetSymbolAddress((void**)&ptr, g_static_stage);
+        if (ce != cudaSuccess || !ptr) return fail(MDG_ECUDA, std::string("mdg_step_host_static: cudaGetSymbolAddress: ") + cudaGetErrorString(ce));
+        g_static_stage_ptr[dev] = ptr;
+    }
+    *out = g_static_stage_ptr[dev];
+    return MDG_OK;
+}
+
+extern "C" int mdg_step_host_static(mdg_env* h, const float* actions_host, float* obs_host, float* reward_host, uint8_t* done_host) {
+    if (!h || !actions_host) return fail(MDG_EINVAL, "mdg_step_host_static: NULL argument");
+    const size_t D = (size_t)h->N * h->M;
+    if (D > (size_t)MDG_STATIC_STAGE_MAX_DRONES)
+        return fail(MDG_EINVAL, "mdg_step_host_static: n_envs * n_drones = " + std::to_string(D) + " exceeds the static staging buffer of " +
+                                    std::to_string(MDG_STATIC_STAGE_MAX_DRONES) + " drones (MDG_STATIC_STAGE_MAX_DRONES); use mdg_step_host");
+    float* stage = nullptr;
+    const int ra = static_stage_address(&stage);
+    if (ra != MDG_OK) return ra;
+    // nothing in the array has to start at zero: the copy overwrites every word the kernel reads (the first D rows) before it runs
+    CU(cudaMemcpyAsync(stage, actions_host, D * 4 * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    const int rc = launch_step(h, stage, h->stream, false);
+    if (rc != MDG_OK) return rc;
+    if (obs_host) CU(cudaMemcpyAsync(obs_host, h->B.obs, D * h->P.opd * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+    if (reward_host) CU(cudaMemcpyAsync(reward_host, h->B.reward, (size_t)h->N * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+    if (done_host) CU(cudaMemcpyAsync(done_host, h->B.done, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return MDG_OK;
+}
 // ---- FP32 peak microbenchmark (roofline denominator check) ------------------------------------------
 __global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int iters, float a, float b) {
     float x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
