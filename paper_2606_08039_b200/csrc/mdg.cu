@@ -686,6 +686,7 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
     C.H = cam->height; C.W = cam->width; C.groups_per_row = cam->width / 4; C.n_groups = C.H * C.groups_per_row;
     C.s = (float)(2.0 * std::tan(0.5 * (double)cam->fovy_deg * 3.14159265358979323846 / 180.0) / cam->height);
     C.half_h = 0.5f * cam->height; C.half_w = 0.5f * cam->width; C.inv_gpr = 1.0f / (float)C.groups_per_row;
+    C.g_rstep = 32 / C.groups_per_row; C.g_cstep = 32 % C.groups_per_row;
     for (int i = 0; i < 3; ++i) C.off[i] = cam->offset[i];
     C.znear = cam->znear; C.zfar = cam->zfar;
     C.rb = std::fmax(cam->body_radius, cam->body_half_height);
@@ -698,8 +699,10 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
     const unsigned grid = (unsigned)((n_cams + CAM_WARPS - 1) / CAM_WARPS);
     const size_t smem = (size_t)CAM_WARPS * h->M * sizeof(CamCand);
     h->chainable = false;                    // a later step must order itself behind this reader as a whole
-    if (depth_dev && seg_dev) render_depth_kernel<true><<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
-    else render_depth_kernel<false><<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
+    const bool two_pass = depth_dev && seg_dev, aligned = C.g_cstep == 0;
+    auto kern = two_pass ? (aligned ? render_depth_kernel<true, true> : render_depth_kernel<true, false>)
+                         : (aligned ? render_depth_kernel<false, true> : render_depth_kernel<false, false>);
+    kern<<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
     CU(cudaGetLastError());
     h->launches += 1;
     return MDG_OK;

@@ -17,6 +17,7 @@ namespace mdg {
 
 struct CamDev {
     int H, W, groups_per_row, n_groups;     // W / 4, H * W / 4
+    int g_rstep, g_cstep;                   // 32 / groups_per_row, 32 % groups_per_row: what a lane's group index advances by per sweep iteration
     float s, half_h, half_w, inv_gpr;       // pixel pitch on the image plane at unit distance; H/2, W/2; 1 / groups_per_row
     float off[3], znear, zfar, rb, inv_a, inv_c;   // rb: radius of the bounding sphere = the larger semi-axis
     float a2, dac;                          // a^2, c^2 - a^2
@@ -27,11 +28,15 @@ struct __align__(16) CamCand {              // one visible spheroid, in its unit
     float w0x, w0y, w0z, w1x, w1y, w1z, w2x, w2y, w2z;   // o x m0, o x m1, o x m2: o x d is linear in (y, z)
     float c00, c01x2, c02x2, c11, c12x2, c22;             // m_a . m_b: |d|^2 is a quadratic in (y, z)
     float b0, b1, b2;                                     // o . m_a
-    int id, pad;                                          // segmentation id
+    int id_rpi; float inv_bw;                             // segmentation id | rows per warp pass << 8 (0: box wider than a warp); 1 / box width
     int4 box;                                             // inclusive pixel bounding box (r0, r1, c0, c1)
 };
 
 static constexpr int CAM_WARPS = 4;         // cameras per block
+// A pixel belongs to a silhouette box when its CENTRE lies within the silhouette's extent widened by this many pixels.  The
+// extent comes from the projected conic in fp32 and is good to ~1e-3 pixel (its error scales with the silhouette's size); a
+// centre that close to the outline is a tie for the ray test anyway.
+static constexpr float CAM_BOX_SLACK = 0.05f;
 
 __device__ __forceinline__ void cam_rotmat(float w, float x, float y, float z, float R[3][3]) {
     R[0][0] = 1.0f - 2.0f * (y * y + z * z); R[0][1] = 2.0f * (x * y - w * z); R[0][2] = 2.0f * (x * z + w * y);
@@ -60,7 +65,9 @@ __device__ __forceinline__ bool cam_hit(const CamCand& q, float y, float z, floa
 // through a spheroid test that cannot concern it.  Otherwise (one output only) a single sweep tests each 4-pixel group
 // against the candidates whose box it touches.  Both use cam_hit and the same visiting order (floor, then drones by index;
 // strict "<"), so they produce identical images.
-template <bool TWO_PASS>
+// ALIGNED: a row holds a power-of-two number of 4-pixel groups that divides 32 (W = 4 .. 128, the default 64 among them), so a
+// lane keeps its columns for the whole sweep and everything that depends on the column only is formed once.
+template <bool TWO_PASS, bool ALIGNED>
 __global__ void __launch_bounds__(CAM_WARPS * 32)
 render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1, int n_cams, int M, const CamDev C,
                     float* __restrict__ depth, uint8_t* __restrict__ seg) {
@@ -97,11 +104,12 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
         // (tan, -+1, 0) / sqrt(1 + tan^2) and (tan, 0, -+1) / sqrt(1 + tan^2), tan = half the image extent at unit distance)
         vis = cx + a >= C.znear && cx - a < C.zfar &&
               fmaf(cx, C.tan_h, -fabsf(cy)) >= -a * C.len_h && fmaf(cx, C.tan_v, -fabsf(cz)) >= -a * C.len_v;
-        if (vis && cx > 1.5f * a) {
+        if (vis && cx > 1.1f * a) {
             // Tight box of the silhouette.  In camera coordinates the spheroid's dual quadric projects to the dual conic
             // C* = Sigma - p p^T with Sigma = a^2 I + (c^2 - a^2) n n^T (n = its axis, p = its centre); the image lines u = const
             // (u = Y/X) tangent to the conic solve C*_00 u^2 - 2 C*_01 u + C*_11 = 0, likewise v = Z/X with index 2.  C*_00 < 0
-            // because the body lies wholly in front of the plane X = 0 here.  One pixel of slack covers the fp32 rounding.
+            // because the body lies wholly in front of the plane X = 0 here.  Pixel (r, c) has its centre at (r + 1/2, c + 1/2): the box
+            // keeps the pixels whose centre is inside the extent (+- CAM_BOX_SLACK); a silhouette between pixel centres has none.
             const float nx = Ri[0][0] * Rk[0][2] + Ri[1][0] * Rk[1][2] + Ri[2][0] * Rk[2][2];
             const float ny = Ri[0][1] * Rk[0][2] + Ri[1][1] * Rk[1][2] + Ri[2][1] * Rk[2][2];
             const float nz = Ri[0][2] * Rk[0][2] + Ri[1][2] * Rk[1][2] + Ri[2][2] * Rk[2][2];
@@ -112,9 +120,9 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
             const float su = sqrtf(fmaxf(c01 * c01 - c00 * c11, 0.0f)), sv = sqrtf(fmaxf(c02 * c02 - c00 * c22, 0.0f));
             // column = W/2 - u / s, row = H/2 - v / s; c00 < 0 so (c01 + su) / c00 is the smaller root
             const float ua = (c01 + su) * inv, ub = (c01 - su) * inv, va = (c02 + sv) * inv, vb = (c02 - sv) * inv;
-            const float c0 = floorf(C.half_w - ub - 1.0f), c1 = ceilf(C.half_w - ua + 1.0f);
-            const float r0 = floorf(C.half_h - vb - 1.0f), r1 = ceilf(C.half_h - va + 1.0f);
-            vis = c1 >= 0.0f && c0 <= (float)(C.W - 1) && r1 >= 0.0f && r0 <= (float)(C.H - 1);
+            const float c0 = ceilf(C.half_w - ub - (0.5f + CAM_BOX_SLACK)), c1 = floorf(C.half_w - ua - (0.5f - CAM_BOX_SLACK));
+            const float r0 = ceilf(C.half_h - vb - (0.5f + CAM_BOX_SLACK)), r1 = floorf(C.half_h - va - (0.5f - CAM_BOX_SLACK));
+            vis = c1 >= c0 && r1 >= r0 && c1 >= 0.0f && c0 <= (float)(C.W - 1) && r1 >= 0.0f && r0 <= (float)(C.H - 1);
             cd.box = make_int4((int)fmaxf(r0, 0.0f), (int)fminf(r1, (float)(C.H - 1)), (int)fmaxf(c0, 0.0f), (int)fminf(c1, (float)(C.W - 1)));
         }
         if (vis) {
@@ -135,7 +143,8 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
             cd.c00 = dot(m[0], m[0]); cd.c01x2 = 2.0f * dot(m[0], m[1]); cd.c02x2 = 2.0f * dot(m[0], m[2]);
             cd.c11 = dot(m[1], m[1]); cd.c12x2 = 2.0f * dot(m[1], m[2]); cd.c22 = dot(m[2], m[2]);
             cd.b0 = dot(o, m[0]); cd.b1 = dot(o, m[1]); cd.b2 = dot(o, m[2]);
-            cd.id = 2 + lane; cd.pad = 0;
+            const int bw = cd.box.w - cd.box.z + 1;
+            cd.id_rpi = (2 + lane) | ((bw <= 32 ? 32 / bw : 0) << 8); cd.inv_bw = 1.0f / (float)bw;
         }
     }
     const unsigned ball = __ballot_sync(0xffffffffu, vis);
@@ -146,9 +155,9 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
     const float noz = oz > 0.0f ? -oz : 0.0f;                    // camera on or under the floor: t = 0 < znear never passes (Q46)
     float* dcam = depth ? depth + (size_t)cam * C.n_groups * 4 : nullptr;
     uint8_t* scam = seg ? seg + (size_t)cam * C.n_groups * 4 : nullptr;
+    int r = (int)(((float)lane + 0.5f) * C.inv_gpr), cg = lane - r * C.groups_per_row;   // row and group-in-row of group g
     for (int g = lane; g < C.n_groups; g += 32) {
-        const int r = (int)(((float)g + 0.5f) * C.inv_gpr);      // exact for g < 2^22
-        const int c4 = (g - r * C.groups_per_row) * 4;
+        const int c4 = cg * 4;
         const float z = (C.half_h - 0.5f - (float)r) * C.s;      // -((r + 1/2) - H/2) s
         const float y0 = (C.half_w - 0.5f - (float)c4) * C.s;
         float y[4], best[4];
@@ -170,7 +179,7 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     float t;
-                    if (cam_hit(q, y[j], z, t) && t >= C.znear && t < best[j]) { best[j] = t; ids = (ids & ~(0xffu << (8 * j))) | ((unsigned)q.id << (8 * j)); }
+                    if (cam_hit(q, y[j], z, t) && t >= C.znear && t < best[j]) { best[j] = t; ids = (ids & ~(0xffu << (8 * j))) | ((unsigned)(q.id_rpi & 255) << (8 * j)); }
                 }
             }
             if (dcam) __stcs(reinterpret_cast<float4*>(dcam) + g, make_float4(best[0], best[1], best[2], best[3]));
@@ -179,23 +188,34 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
             reinterpret_cast<float4*>(dcam)[g] = make_float4(best[0], best[1], best[2], best[3]);
             reinterpret_cast<unsigned*>(scam)[g] = ids;
         }
+        r += C.g_rstep;
+        if (!ALIGNED) { cg += C.g_cstep; if (cg >= C.groups_per_row) { cg -= C.groups_per_row; r += 1; } }
     }
     if (TWO_PASS) {
         for (int k = 0; k < n_cand; ++k) {
             __syncwarp();                                        // orders the warp's earlier stores before the loads below
             const CamCand& q = cand[k];
             const int4 bb = q.box;
-            const int bw = bb.w - bb.z + 1, n_px = bw * (bb.y - bb.x + 1);
-            const float inv_bw = 1.0f / (float)bw;
-            for (int i = lane; i < n_px; i += 32) {
-                const int rr = (int)(((float)i + 0.5f) * inv_bw);
-                const int r = bb.x + rr, c = bb.z + (i - rr * bw);
+            const int bw = bb.w - bb.z + 1, rpi = q.id_rpi >> 8;
+            const uint8_t id = (uint8_t)(q.id_rpi & 255);
+            auto test = [&](int r, int c) {
                 const float z = (C.half_h - 0.5f - (float)r) * C.s;
                 const float y = fmaf(-(float)(c & 3), C.s, (C.half_w - 0.5f - (float)(c & ~3)) * C.s);   // as the sweep forms it
                 float t;
                 if (cam_hit(q, y, z, t) && t >= C.znear) {
                     const int px = r * C.W + c;
-                    if (t < __ldcg(dcam + px)) { dcam[px] = t; scam[px] = (uint8_t)q.id; }
+                    if (t < __ldcg(dcam + px)) { dcam[px] = t; scam[px] = id; }
+                }
+            };
+            if (rpi > 0) {                                       // the usual case: the warp covers rpi whole rows of the box per pass
+                const int lr = (int)(((float)lane + 0.5f) * q.inv_bw), c = bb.z + (lane - lr * bw);   // lane / bw, exact for lane, bw <= 32
+                if (lr < rpi)
+                    for (int r = bb.x + lr; r <= bb.y; r += rpi) test(r, c);
+            } else {
+                const int n_px = bw * (bb.y - bb.x + 1);
+                for (int i = lane; i < n_px; i += 32) {
+                    const int rr = (int)(((float)i + 0.5f) * q.inv_bw);
+                    test(bb.x + rr, bb.z + (i - rr * bw));
                 }
             }
         }
