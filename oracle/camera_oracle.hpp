@@ -20,11 +20,18 @@
 //   Q47 depth = distance along the optical axis in metres (the ray parameter t of the direction above, whose
 //       axial component is 1), hits with t < znear or t >= zfar are discarded, background depth = zfar.
 //   Q48 segmentation id (u8): 0 background, 1 floor, 2 + k drone k of the env.
+//   Q53 colour frame ("(N, 48, 64, 4) uint8"): flat Lambert shading of the same nearest hit.  One directional
+//       light, the unit vector towards it l = (0.36, 0.48, 0.80) in the world frame; shade = 0.3 + 0.7 max(0, n.l) with n the
+//       outward unit normal of the primitive at the hit point (floor: +z; spheroid: the normalised gradient of its quadric);
+//       albedo (R, G, B) in 0..255: floor (160, 160, 160), drone k (250 - 22 (k mod 8), 60 + 40 ((k div 8) mod 4),
+//       40 + 26 (k mod 8)) - all even, so that the ambient term alone (0.3 x albedo) never lands on a rounding boundary; channel = floor(albedo * shade + 1/2); background = the unshaded sky (135, 206, 235); alpha = 255.
 // Pins (tests/test_oracle_camera.py): floor depth rows of a level camera against the similar-triangles value
 // h / tan(elevation); forward pinhole projection of small spheres at tabulated bearings lands in the pixel the
 // ray caster marks (tests/golden/camera_bearings.txt); on-axis sphere silhouette area and nearest depth d - R;
 // every hit pixel's reconstructed 3-D point lies on its primitive; yaw co-rotation invariance; roll by pi flips
 // the image; occlusion order; a : c aspect of a spheroid seen edge-on; spheroid seen along its axis = disc of radius a.
+// Colour frame (tests/test_oracle_camera_rgba.py): the floor's hand value; a sphere's radial normals; the finite-difference
+// gradient of the defining quadric for tilted spheroids; back-lit faces = the ambient term alone; sky and alpha.
 #pragma once
 #include <cmath>
 #include <cstdint>
@@ -42,8 +49,21 @@ struct CamParams {
 // carries the camera.  depth / seg: [H*W]; margin (may be null): per pixel, the smallest relative distance of any
 // decision taken for it (discriminant sign, near / far clip, ordering of the two nearest hits, floor side) to its
 // threshold, so that a comparison in another precision can tell a tie from an error.
+// rgba (may be null): [H*W][4] u8 of reading Q53; shade_margin (may be null): per pixel, the distance of the channel value
+// closest to a rounding boundary from that boundary, in units of one u8 step (1/2 = as far as it gets; background pixels: 1/2).
+constexpr double LIGHT_DIR[3] = {0.36, 0.48, 0.80};
+constexpr double SHADE_AMBIENT = 0.3, SHADE_DIFFUSE = 0.7;
+inline void albedo_of(int id, double rgb[3]) {
+    if (id == 0) { rgb[0] = 135.0; rgb[1] = 206.0; rgb[2] = 235.0; }
+    else if (id == 1) { rgb[0] = rgb[1] = rgb[2] = 160.0; }
+    else {
+        const int k = id - 2;
+        rgb[0] = 250.0 - 22.0 * (k % 8); rgb[1] = 60.0 + 40.0 * ((k / 8) % 4); rgb[2] = 40.0 + 26.0 * (k % 8);
+    }
+}
+
 inline void render_camera(const double* state, int n_drones, int i, const CamParams& cp, double* depth, uint8_t* seg,
-                          double* margin) {
+                          double* margin, uint8_t* rgba = nullptr, double* shade_margin = nullptr) {
     const double* si = state + 13 * i;
     double Ri[3][3], o[3], off_w[3];
     rotmat(si + 3, Ri);
@@ -91,6 +111,36 @@ inline void render_camera(const double* state, int n_drones, int i, const CamPar
             depth[r * cp.W + c] = best;
             seg[r * cp.W + c] = (uint8_t)id;
             if (margin) margin[r * cp.W + c] = mg;
+            if (rgba) {                                        // Q53
+                double shade = 1.0, alb[3];
+                albedo_of(id, alb);
+                if (id != 0) {
+                    double n[3] = {0.0, 0.0, 1.0};
+                    if (id >= 2) {
+                        const double* sk = state + 13 * (id - 2);
+                        double Rk[3][3], rel[3], b[3], g[3];
+                        rotmat(sk + 3, Rk);
+                        for (int a = 0; a < 3; ++a) rel[a] = o[a] + best * d[a] - sk[a];      // hit point relative to the body's centre
+                        matT_vec(Rk, rel, b);
+                        const double ia2 = 1.0 / (cp.body_a * cp.body_a), ic2 = 1.0 / (cp.body_c * cp.body_c);
+                        const double gb[3] = {b[0] * ia2, b[1] * ia2, b[2] * ic2};              // gradient of x^2/a^2 + y^2/a^2 + z^2/c^2 (halved)
+                        mat_vec(Rk, gb, g);
+                        const double gn = std::sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
+                        for (int a = 0; a < 3; ++a) n[a] = g[a] / gn;
+                    }
+                    const double ndl = n[0] * LIGHT_DIR[0] + n[1] * LIGHT_DIR[1] + n[2] * LIGHT_DIR[2];
+                    shade = SHADE_AMBIENT + SHADE_DIFFUSE * std::fmax(0.0, ndl);
+                }
+                double sm = 0.5;
+                for (int ch = 0; ch < 3; ++ch) {
+                    const double v = alb[ch] * shade;
+                    const double q = std::floor(v + 0.5);
+                    rgba[(r * cp.W + c) * 4 + ch] = (uint8_t)q;
+                    if (id != 0) sm = std::fmin(sm, 0.5 - std::fabs(v - q));
+                }
+                rgba[(r * cp.W + c) * 4 + 3] = 255;
+                if (shade_margin) shade_margin[r * cp.W + c] = sm;
+            }
         }
     }
 }

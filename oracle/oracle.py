@@ -53,6 +53,7 @@ def lib():
         L.orc_wind_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
         L.orc_gen_actions.argtypes = [C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_uint32]
         L.orc_render_depth.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.orc_render_rgba.argtypes = [C.c_void_p, C.c_int, C.c_int] + [C.c_void_p] * 6 + [C.c_int]
     return _lib
 
 
@@ -322,3 +323,21 @@ def render_depth(state, n_envs, n_drones, n_threads=1, with_margin=False, **cam)
     margin = np.empty((D, H, W), np.float64) if with_margin else None
     lib().orc_render_depth(_p(st), n_envs, n_drones, _p(vec), _p(depth), _p(seg), _p(margin) if with_margin else None, int(n_threads))
     return (depth, seg, margin) if with_margin else (depth, seg)
+
+
+def render_rgba(state, n_envs, n_drones, n_threads=1, **cam):
+    """The colour frame of reading Q53 (camera_oracle.hpp): rgba [D, H, W, 4] u8, with depth, segmentation, the tie margin of
+    the hit decisions and the distance of the shaded value from a u8 rounding boundary, all [D, H, W]."""
+    c = dict(CAM_DEFAULTS)
+    for k in cam:
+        if k not in c:
+            raise KeyError(k)
+    c.update(cam)
+    st = _f64(state).reshape(n_envs * n_drones, 13)
+    H, W = int(c["H"]), int(c["W"])
+    vec = np.array([H, W, c["fovy_deg"], *c["offset"], c["znear"], c["zfar"], c["body_a"], c["body_c"]], dtype=np.float64)
+    D = n_envs * n_drones
+    depth, seg, margin = np.empty((D, H, W), np.float64), np.empty((D, H, W), np.uint8), np.empty((D, H, W), np.float64)
+    rgba, sm = np.empty((D, H, W, 4), np.uint8), np.empty((D, H, W), np.float64)
+    lib().orc_render_rgba(_p(st), n_envs, n_drones, _p(vec), _p(depth), _p(seg), _p(margin), _p(rgba), _p(sm), int(n_threads))
+    return rgba, depth, seg, margin, sm

@@ -300,4 +300,27 @@ void orc_render_depth(const double* state, int n_envs, int n_drones, const doubl
         th.emplace_back(work, (int)((int64_t)n_envs * t / n_threads), (int)((int64_t)n_envs * (t + 1) / n_threads));
     for (auto& x : th) x.join();
 }
+
+// The same with the colour frame of reading Q53: rgba [D][H][W][4] u8, shade_margin [D][H][W] float64 or NULL.
+void orc_render_rgba(const double* state, int n_envs, int n_drones, const double* cam, double* depth, uint8_t* seg,
+                     double* margin, uint8_t* rgba, double* shade_margin, int n_threads) {
+    CamParams cp;
+    cp.H = (int)cam[0]; cp.W = (int)cam[1]; cp.fovy_deg = cam[2];
+    cp.offset[0] = cam[3]; cp.offset[1] = cam[4]; cp.offset[2] = cam[5];
+    cp.znear = cam[6]; cp.zfar = cam[7]; cp.body_a = cam[8]; cp.body_c = cam[9];
+    const size_t px = (size_t)cp.H * cp.W;
+    auto work = [&](int e0, int e1) {
+        for (int e = e0; e < e1; ++e)
+            for (int i = 0; i < n_drones; ++i) {
+                const size_t d = (size_t)e * n_drones + i;
+                render_camera(state + (size_t)e * n_drones * 13, n_drones, i, cp, depth + d * px, seg + d * px,
+                              margin ? margin + d * px : nullptr, rgba + d * px * 4, shade_margin ? shade_margin + d * px : nullptr);
+            }
+    };
+    if (n_threads <= 1) { work(0, n_envs); return; }
+    std::vector<std::thread> th;
+    for (int t = 0; t < n_threads; ++t)
+        th.emplace_back(work, (int)((int64_t)n_envs * t / n_threads), (int)((int64_t)n_envs * (t + 1) / n_threads));
+    for (auto& x : th) x.join();
+}
 }  // extern "C"
