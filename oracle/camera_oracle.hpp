@@ -49,8 +49,8 @@ struct CamParams {
 // carries the camera.  depth / seg: [H*W]; margin (may be null): per pixel, the smallest relative distance of any
 // decision taken for it (discriminant sign, near / far clip, ordering of the two nearest hits, floor side) to its
 // threshold, so that a comparison in another precision can tell a tie from an error.
-// rgba (may be null): [H*W][4] u8 of reading Q53; shade_margin (may be null): per pixel, the distance of the channel value
-// closest to a rounding boundary from that boundary, in units of one u8 step (1/2 = as far as it gets; background pixels: 1/2).
+// rgba (may be null): [H*W][4] u8 of reading Q53; shade_out (may be null): per pixel, the shade before quantisation (1 for the
+// background), so that a comparison in another precision can tell a value next to a rounding boundary from an error.
 constexpr double LIGHT_DIR[3] = {0.36, 0.48, 0.80};
 constexpr double SHADE_AMBIENT = 0.3, SHADE_DIFFUSE = 0.7;
 inline void albedo_of(int id, double rgb[3]) {
@@ -63,7 +63,7 @@ inline void albedo_of(int id, double rgb[3]) {
 }
 
 inline void render_camera(const double* state, int n_drones, int i, const CamParams& cp, double* depth, uint8_t* seg,
-                          double* margin, uint8_t* rgba = nullptr, double* shade_margin = nullptr) {
+                          double* margin, uint8_t* rgba = nullptr, double* shade_out = nullptr) {
     const double* si = state + 13 * i;
     double Ri[3][3], o[3], off_w[3];
     rotmat(si + 3, Ri);
@@ -131,15 +131,9 @@ inline void render_camera(const double* state, int n_drones, int i, const CamPar
                     const double ndl = n[0] * LIGHT_DIR[0] + n[1] * LIGHT_DIR[1] + n[2] * LIGHT_DIR[2];
                     shade = SHADE_AMBIENT + SHADE_DIFFUSE * std::fmax(0.0, ndl);
                 }
-                double sm = 0.5;
-                for (int ch = 0; ch < 3; ++ch) {
-                    const double v = alb[ch] * shade;
-                    const double q = std::floor(v + 0.5);
-                    rgba[(r * cp.W + c) * 4 + ch] = (uint8_t)q;
-                    if (id != 0) sm = std::fmin(sm, 0.5 - std::fabs(v - q));
-                }
+                for (int ch = 0; ch < 3; ++ch) rgba[(r * cp.W + c) * 4 + ch] = (uint8_t)std::floor(alb[ch] * shade + 0.5);
                 rgba[(r * cp.W + c) * 4 + 3] = 255;
-                if (shade_margin) shade_margin[r * cp.W + c] = sm;
+                if (shade_out) shade_out[r * cp.W + c] = shade;
             }
         }
     }

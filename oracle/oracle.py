@@ -327,7 +327,7 @@ def render_depth(state, n_envs, n_drones, n_threads=1, with_margin=False, **cam)
 
 def render_rgba(state, n_envs, n_drones, n_threads=1, **cam):
     """The colour frame of reading Q53 (camera_oracle.hpp): rgba [D, H, W, 4] u8, with depth, segmentation, the tie margin of
-    the hit decisions and the distance of the shaded value from a u8 rounding boundary, all [D, H, W]."""
+    the hit decisions and the shade before quantisation (1 for the background), all [D, H, W]."""
     c = dict(CAM_DEFAULTS)
     for k in cam:
         if k not in c:

@@ -301,9 +301,9 @@ void orc_render_depth(const double* state, int n_envs, int n_drones, const doubl
     for (auto& x : th) x.join();
 }
 
-// The same with the colour frame of reading Q53: rgba [D][H][W][4] u8, shade_margin [D][H][W] float64 or NULL.
+// The same with the colour frame of reading Q53: rgba [D][H][W][4] u8, shade [D][H][W] float64 or NULL.
 void orc_render_rgba(const double* state, int n_envs, int n_drones, const double* cam, double* depth, uint8_t* seg,
-                     double* margin, uint8_t* rgba, double* shade_margin, int n_threads) {
+                     double* margin, uint8_t* rgba, double* shade, int n_threads) {
     CamParams cp;
     cp.H = (int)cam[0]; cp.W = (int)cam[1]; cp.fovy_deg = cam[2];
     cp.offset[0] = cam[3]; cp.offset[1] = cam[4]; cp.offset[2] = cam[5];
@@ -314,7 +314,7 @@ void orc_render_rgba(const double* state, int n_envs, int n_drones, const double
             for (int i = 0; i < n_drones; ++i) {
                 const size_t d = (size_t)e * n_drones + i;
                 render_camera(state + (size_t)e * n_drones * 13, n_drones, i, cp, depth + d * px, seg + d * px,
-                              margin ? margin + d * px : nullptr, rgba + d * px * 4, shade_margin ? shade_margin + d * px : nullptr);
+                              margin ? margin + d * px : nullptr, rgba + d * px * 4, shade ? shade + d * px : nullptr);
             }
     };
     if (n_threads <= 1) { work(0, n_envs); return; }

@@ -44,6 +44,12 @@ def hit_points(st, i, depth):
     return o + depth[..., None] * (pixel_dirs(48, 64, 60.0) @ Ri.T)
 
 
+def boundary_distance(alb, shade):
+    """Distance of the channel value closest to a u8 rounding boundary from that boundary (1/2 = as far as it gets)."""
+    v = np.asarray(alb)[None, :] * np.asarray(shade).reshape(-1, 1)
+    return (0.5 - np.abs(v - np.floor(v + 0.5))).min(axis=1)
+
+
 def expected(alb, ndl):
     return np.floor(np.asarray(alb)[None, :] * (0.3 + 0.7 * np.maximum(0.0, ndl))[:, None] + 0.5)
 
@@ -56,7 +62,7 @@ def test_light_is_a_unit_vector_and_the_floor_sky_and_alpha_have_their_hand_valu
     assert np.all(rgba[0][seg[0] == 0][:, :3] == SKY)
     # floor: n = +z, n.l = 0.8, shade = 0.3 + 0.7 * 0.8 = 0.86, 160 * 0.86 = 137.6 -> 138
     assert np.all(rgba[0][seg[0] == 1][:, :3] == 138)
-    assert np.allclose(sm[0][seg[0] == 1], 0.1) and np.all(sm[0][seg[0] == 0] == 0.5)
+    assert np.allclose(sm[0][seg[0] == 1], 0.86, atol=1e-15) and np.all(sm[0][seg[0] == 0] == 1.0)
 
 
 def test_depth_segmentation_and_margin_are_those_of_render_depth():
@@ -82,7 +88,7 @@ def test_sphere_normals_are_radial(k):
     n = (hit_points(st, 0, depth[0])[hit] - ctr) / R
     assert np.abs(np.linalg.norm(n, axis=1) - 1.0).max() < 1e-9
     v = albedo(k)[None, :] * (0.3 + 0.7 * np.maximum(0.0, n @ L))[:, None]
-    safe = sm[0][hit] > 1e-6
+    safe = boundary_distance(albedo(k), sm[0][hit]) > 1e-6
     assert safe.mean() > 0.99
     assert np.array_equal(rgba[0][hit][safe][:, :3], np.floor(v + 0.5)[safe])
     assert (n @ L > 0.2).any() and (n @ L < 0.0).any()       # both the lit and the shadowed side are in view
@@ -105,9 +111,10 @@ def test_spheroid_normals_match_the_finite_difference_gradient_of_the_quadric():
         for i in range(M):
             X = hit_points(st, i, depth[i])
             for k in range(M):
-                hk = (seg[i] == 2 + k) & (sm[i] > 1e-4)
+                hk = seg[i] == 2 + k
                 if not hk.any():
                     continue
+                hk[hk] = boundary_distance(albedo(k), sm[i][hk]) > 1e-4
                 Rk, pk = rot_of(st[k]), st[k, :3]
                 f = lambda x: (((x - pk) @ Rk / np.array([a, a, c])) ** 2).sum(axis=-1)
                 h = 1e-6
