@@ -321,6 +321,16 @@ int mdg_default_cam_params(const mdg_params* params, mdg_cam_params* out);
  * (0, 180), znear <= 0 or zfar <= znear, non-positive body axes. */
 int mdg_render_depth(mdg_env* env, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev);
 
+/* The colour frame of the same cameras: PAPER.md:177's "(N, 48, 64, 4) uint8" observation, [n_envs*n_drones][height][width][4]
+ * u8 = R, G, B, A, caller-owned device memory, 16-byte aligned.  The paper's frame comes from mujoco.Renderer (OpenGL,
+ * unavailable here); this one is flat Lambert shading of the hit mdg_render_depth finds (reading Q53): one directional
+ * light, unit vector towards it l = (0.36, 0.48, 0.80) in the world frame; shade = 0.3 + 0.7 max(0, n.l), n the outward unit
+ * normal at the hit (floor +z; spheroid: normalised gradient of its quadric); albedo 0..255: floor (160, 160, 160), drone k
+ * (250 - 22 (k mod 8), 60 + 40 ((k div 8) mod 4), 40 + 26 (k mod 8)); channel = floor(albedo * shade + 1/2) in fp32;
+ * background = the unshaded sky (135, 206, 235); A = 255.  Same cam argument, scene, clipping, stream behaviour and errors as
+ * mdg_render_depth (MDG_EINVAL also for a NULL or misaligned rgba_dev). */
+int mdg_render_rgba(mdg_env* env, const mdg_cam_params* cam, uint8_t* rgba_dev);
+
 /* Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) used by later calls.  Work already queued
  * on the previously bound stream (the clear and reset of mdg_create, earlier steps) is ordered before whatever is enqueued on
  * the new one afterwards (an event on the old stream, waited on by the new; skipped when either stream is being captured:

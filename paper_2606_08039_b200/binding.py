@@ -65,7 +65,7 @@ class mdg_cam_params(C.Structure):
 
 EXPORTS = ["mdg_default_params", "mdg_create", "mdg_destroy", "mdg_reset", "mdg_step", "mdg_step_chained", "mdg_step_many", "mdg_step_host", "mdg_step_host_async", "mdg_step_host_static", "mdg_wait", "mdg_checkpoint_size", "mdg_save", "mdg_load", "mdg_outputs",
            "mdg_obs_dim", "mdg_targets", "mdg_gen_actions", "mdg_get_state", "mdg_set_state", "mdg_set_stream",
-           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_last_error", "mdg_version"]
+           "mdg_launch_count", "mdg_kernel_name", "mdg_set_launch", "mdg_measure_fp32_peak", "mdg_get_dr", "mdg_set_dr", "mdg_reward_per_drone", "mdg_default_cam_params", "mdg_render_depth", "mdg_render_rgba", "mdg_last_error", "mdg_version"]
 
 _lib = None
 
@@ -114,6 +114,7 @@ def lib():
         L.mdg_measure_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
         L.mdg_default_cam_params.argtypes = [PP, C.POINTER(mdg_cam_params)]
         L.mdg_render_depth.argtypes = [vp, C.POINTER(mdg_cam_params), vp, vp]
+        L.mdg_render_rgba.argtypes = [vp, C.POINTER(mdg_cam_params), vp]
         _lib = L
     return _lib
 
@@ -295,6 +296,18 @@ class Env:
         _check(lib().mdg_render_depth(self._h, C.byref(c), C.c_void_p(depth.data_ptr() if depth is not None else None),
                                       C.c_void_p(seg.data_ptr() if seg is not None else None)))
         return depth, seg
+
+    def render_rgba(self, cam: mdg_cam_params = None, rgba=None):
+        """Every drone's colour frame from the current state (include/mdg.h: mdg_render_rgba): [D, H, W, 4] uint8 CUDA tensor."""
+        t = self._torch
+        c = cam if cam is not None else default_cam_params(self.params)
+        shape = (self.n_envs * self.n_drones, c.height, c.width, 4)
+        if rgba is None:
+            rgba = t.empty(shape, dtype=t.uint8, device=self.obs.device)
+        if not (rgba.is_cuda and rgba.dtype == t.uint8 and rgba.is_contiguous() and tuple(rgba.shape) == shape):
+            raise ValueError(f"rgba must be a contiguous CUDA uint8 tensor of shape {shape}")
+        _check(lib().mdg_render_rgba(self._h, C.byref(c), C.c_void_p(rgba.data_ptr())))
+        return rgba
 
     def get_state(self):
         import numpy as np

@@ -670,13 +670,11 @@ int mdg_default_cam_params(const mdg_params* params, mdg_cam_params* out) {
     return MDG_OK;
 }
 
-int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev) {
-    if (!h) return fail(MDG_EINVAL, "mdg_render_depth: NULL handle");
+// One launch of the camera kernel: depth and / or segmentation (mdg_render_depth), or the colour frame (mdg_render_rgba).
+static int render_camera(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev, uint8_t* rgba_dev) {
     mdg_cam_params def;
     if (!cam) { const int rc = mdg_default_cam_params(&h->hp, &def); if (rc != MDG_OK) return rc; cam = &def; }
     if (cam->struct_size != sizeof(mdg_cam_params)) return fail(MDG_EINVAL, "mdg_render_depth: struct_size mismatch");
-    if (!depth_dev && !seg_dev) return fail(MDG_EINVAL, "mdg_render_depth: both outputs NULL");
-    if (((uintptr_t)depth_dev & 15) || ((uintptr_t)seg_dev & 3)) return fail(MDG_EINVAL, "mdg_render_depth: depth_dev must be 16-byte, seg_dev 4-byte aligned");
     if (cam->height < 1 || cam->width < 4 || (cam->width & 3) || (int64_t)cam->height * cam->width > (1 << 24))
         return fail(MDG_EINVAL, "mdg_render_depth: height >= 1, width a positive multiple of 4, height*width <= 2^24");
     if (!(cam->fovy_deg > 0.0f && cam->fovy_deg < 180.0f) || !(cam->znear > 0.0f) || !(cam->zfar > cam->znear) ||
@@ -697,15 +695,30 @@ int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, ui
     C.inv_a = (float)(1.0 / (double)cam->body_radius); C.inv_c = (float)(1.0 / (double)cam->body_half_height);
     const int n_cams = h->N * h->M;
     const unsigned grid = (unsigned)((n_cams + CAM_WARPS - 1) / CAM_WARPS);
-    const size_t smem = (size_t)CAM_WARPS * h->M * sizeof(CamCand);
+    const size_t smem = (size_t)CAM_WARPS * h->M * (sizeof(CamCand) + (rgba_dev ? sizeof(CamShade) : 0));
     h->chainable = false;                    // a later step must order itself behind this reader as a whole
     const bool two_pass = depth_dev && seg_dev, aligned = C.g_cstep == 0;
-    auto kern = two_pass ? (aligned ? render_depth_kernel<true, true> : render_depth_kernel<true, false>)
-                         : (aligned ? render_depth_kernel<false, true> : render_depth_kernel<false, false>);
-    kern<<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev);
+    auto kern = rgba_dev ? (aligned ? render_depth_kernel<CAM_RGBA, true> : render_depth_kernel<CAM_RGBA, false>)
+              : two_pass ? (aligned ? render_depth_kernel<CAM_TWO_PASS, true> : render_depth_kernel<CAM_TWO_PASS, false>)
+                         : (aligned ? render_depth_kernel<CAM_ONE_PASS, true> : render_depth_kernel<CAM_ONE_PASS, false>);
+    kern<<<grid, CAM_WARPS * 32, smem, h->stream>>>(h->B.P0, h->B.P1, n_cams, h->M, C, depth_dev, seg_dev, reinterpret_cast<uint4*>(rgba_dev));
     CU(cudaGetLastError());
     h->launches += 1;
     return MDG_OK;
+}
+
+int mdg_render_depth(mdg_env* h, const mdg_cam_params* cam, float* depth_dev, uint8_t* seg_dev) {
+    if (!h) return fail(MDG_EINVAL, "mdg_render_depth: NULL handle");
+    if (!depth_dev && !seg_dev) return fail(MDG_EINVAL, "mdg_render_depth: both outputs NULL");
+    if (((uintptr_t)depth_dev & 15) || ((uintptr_t)seg_dev & 3)) return fail(MDG_EINVAL, "mdg_render_depth: depth_dev must be 16-byte, seg_dev 4-byte aligned");
+    return render_camera(h, cam, depth_dev, seg_dev, nullptr);
+}
+
+int mdg_render_rgba(mdg_env* h, const mdg_cam_params* cam, uint8_t* rgba_dev) {
+    if (!h) return fail(MDG_EINVAL, "mdg_render_rgba: NULL handle");
+    if (!rgba_dev) return fail(MDG_EINVAL, "mdg_render_rgba: NULL output");
+    if ((uintptr_t)rgba_dev & 15) return fail(MDG_EINVAL, "mdg_render_rgba: rgba_dev must be 16-byte aligned");
+    return render_camera(h, cam, nullptr, nullptr, rgba_dev);
 }
 
 int mdg_set_stream(mdg_env* h, void* s) {

@@ -32,7 +32,20 @@ struct __align__(16) CamCand {              // one visible spheroid, in its unit
     int4 box;                                             // inclusive pixel bounding box (r0, r1, c0, c1)
 };
 
+// What the colour frame needs on top (reading Q53): the ray direction in the candidate's unit-sphere frame, d = m0 + y m1 + z m2,
+// and L = S R_k^T l, so that for the hit point u (|u| = 1) the shading is n.l = (u.L) / |S u|, |S u|^2 = 1/a^2 + u_z^2 (1/c^2 - 1/a^2).
+struct __align__(16) CamShade { float m0[3], m1[3], m2[3], L[3]; unsigned ovl; float pad[3]; };   // ovl: candidates whose box meets this one's
+
 static constexpr int CAM_WARPS = 4;         // cameras per block
+enum { CAM_ONE_PASS = 0, CAM_TWO_PASS = 1, CAM_RGBA = 2 };
+// Q53: unit vector towards the light, ambient and diffuse weights, sky colour (R | G << 8 | B << 16 | A << 24) and floor albedo
+static constexpr float CAM_LIGHT_X = 0.36f, CAM_LIGHT_Y = 0.48f, CAM_LIGHT_Z = 0.80f;
+static constexpr float CAM_AMBIENT = 0.3f, CAM_DIFFUSE = 0.7f, CAM_FLOOR_ALBEDO = 160.0f;
+static constexpr unsigned CAM_SKY = 135u | (206u << 8) | (235u << 16) | (255u << 24);
+__device__ __forceinline__ unsigned cam_shade_rgba(float ar, float ag, float ab, float ndl) {
+    const float sh = fmaf(CAM_DIFFUSE, fmaxf(ndl, 0.0f), CAM_AMBIENT);
+    return __float2uint_rd(fmaf(ar, sh, 0.5f)) | (__float2uint_rd(fmaf(ag, sh, 0.5f)) << 8) | (__float2uint_rd(fmaf(ab, sh, 0.5f)) << 16) | (255u << 24);
+}
 // A pixel belongs to a silhouette box when its CENTRE lies within the silhouette's extent widened by this many pixels.  The
 // extent comes from the projected conic in fp32 and is good to ~1e-3 pixel (its error scales with the silhouette's size); a
 // centre that close to the outline is a tie for the ray test anyway.
@@ -59,6 +72,20 @@ __device__ __forceinline__ bool cam_hit(const CamCand& q, float y, float z, floa
     t = fmaf(-h2, rsqrt_fast(h2), -fmaf(y, q.b1, fmaf(z, q.b2, q.b0)) * rA);
     return true;
 }
+// n.l at the front hit of ray (1, y, z) on candidate q (the ray is known to hit).  The hit point in the unit-sphere frame is the
+// foot of the perpendicular from the centre, d x (o x d) / |d|^2 (|.| <= 1, formed from the same cancellation-free o x d as the
+// hit test), minus the half-chord h d: no difference of the large vectors o and t d is ever taken.
+__device__ __forceinline__ float cam_ndotl(const CamCand& q, const CamShade& sh, float y, float z, float ia2, float dic) {
+    const float wx = fmaf(y, q.w1x, fmaf(z, q.w2x, q.w0x)), wy = fmaf(y, q.w1y, fmaf(z, q.w2y, q.w0y)), wz = fmaf(y, q.w1z, fmaf(z, q.w2z, q.w0z));
+    const float ww = fmaf(wx, wx, fmaf(wy, wy, wz * wz));
+    const float A = fmaf(y, fmaf(y, q.c11, fmaf(z, q.c12x2, q.c01x2)), fmaf(z, fmaf(z, q.c22, q.c02x2), q.c00));
+    const float rA = rcp_fast(A);
+    const float h2 = fmaxf((A - ww) * rA * rA, 1e-30f);
+    const float h = h2 * rsqrt_fast(h2);
+    const float dx = fmaf(y, sh.m1[0], fmaf(z, sh.m2[0], sh.m0[0])), dy = fmaf(y, sh.m1[1], fmaf(z, sh.m2[1], sh.m0[1])), dz = fmaf(y, sh.m1[2], fmaf(z, sh.m2[2], sh.m0[2]));
+    const float ux = fmaf(fmaf(dy, wz, -dz * wy), rA, -h * dx), uy = fmaf(fmaf(dz, wx, -dx * wz), rA, -h * dy), uz = fmaf(fmaf(dx, wy, -dy * wx), rA, -h * dz);
+    return fmaf(ux, sh.L[0], fmaf(uy, sh.L[1], uz * sh.L[2])) * rsqrt_fast(fmaf(uz * uz, dic, ia2));
+}
 
 // TWO_PASS (both outputs requested): the warp first sweeps the floor over the whole image, then visits each candidate's
 // bounding box with one lane per PIXEL and depth-tests against what it has just written (still in L2), so no lane idles
@@ -67,15 +94,51 @@ __device__ __forceinline__ bool cam_hit(const CamCand& q, float y, float z, floa
 // strict "<"), so they produce identical images.
 // ALIGNED: a row holds a power-of-two number of 4-pixel groups that divides 32 (W = 4 .. 128, the default 64 among them), so a
 // lane keeps its columns for the whole sweep and everything that depends on the column only is formed once.
-template <bool TWO_PASS, bool ALIGNED>
+// The candidates' bounding boxes, one after the other, one lane per box pixel: visit(k, q, row, column, y, z, t) for every pixel
+// whose ray (1, y, z) hits candidate k in front of the near plane.  Lanes of one call touch different pixels; calls are ordered by __syncwarp.
+template <class F>
+__device__ __forceinline__ void cam_box_pass(const CamCand* cand, int n_cand, int lane, const CamDev& C, F&& visit) {
+    for (int k = 0; k < n_cand; ++k) {
+        __syncwarp();                                            // orders the warp's earlier stores before the loads below
+        const CamCand& q = cand[k];
+        const int4 bb = q.box;
+        const int bw = bb.w - bb.z + 1, rpi = q.id_rpi >> 8;
+        auto test = [&](int r, int c) {
+            const float z = (C.half_h - 0.5f - (float)r) * C.s;
+            const float y = fmaf(-(float)(c & 3), C.s, (C.half_w - 0.5f - (float)(c & ~3)) * C.s);   // as the sweep forms it
+            float t;
+            if (cam_hit(q, y, z, t) && t >= C.znear) visit(k, q, r, c, y, z, t);
+        };
+        if (rpi > 0) {                                           // the usual case: the warp covers rpi whole rows of the box per pass
+            const int lr = (int)(((float)lane + 0.5f) * q.inv_bw), c = bb.z + (lane - lr * bw);   // lane / bw, exact for lane, bw <= 32
+            if (lr < rpi)
+                for (int r = bb.x + lr; r <= bb.y; r += rpi) test(r, c);
+        } else {
+            const int n_px = bw * (bb.y - bb.x + 1);
+            for (int i = lane; i < n_px; i += 32) {
+                const int rr = (int)(((float)i + 0.5f) * q.inv_bw);
+                test(bb.x + rr, bb.z + (i - rr * bw));
+            }
+        }
+    }
+}
+
+// MODE = CAM_RGBA: the colour frame (reading Q53) in two passes without any depth buffer.  The sweep writes sky and floor; the
+// box pass then decides every drone pixel in registers - a hit wins its pixel when it is in front of the floor and of the hits of
+// the few candidates whose boxes meet this one's (CamShade::ovl; same tests, same boxes and the same order rule as the depth
+// kernel: the lower drone index wins a tie) - and the winner alone shades and stores its pixel.  Every pixel's final value is
+// written by exactly one lane after the sweep's; nothing is read back.  depth and seg are not written.
+template <int MODE, bool ALIGNED>
 __global__ void __launch_bounds__(CAM_WARPS * 32)
 render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1, int n_cams, int M, const CamDev C,
-                    float* __restrict__ depth, uint8_t* __restrict__ seg) {
+                    float* __restrict__ depth, uint8_t* __restrict__ seg, uint4* __restrict__ rgba) {
+    constexpr bool TWO_PASS = MODE == CAM_TWO_PASS, RGBA = MODE == CAM_RGBA;
     extern __shared__ __align__(16) unsigned char cam_smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int cam = blockIdx.x * CAM_WARPS + wib;
     if (cam >= n_cams) return;
     CamCand* cand = reinterpret_cast<CamCand*>(cam_smem) + (size_t)wib * M;
+    CamShade* shade = reinterpret_cast<CamShade*>(cam_smem + (size_t)CAM_WARPS * M * sizeof(CamCand)) + (size_t)wib * M;   // CAM_RGBA only
     const int env0 = (cam / M) * M, self = cam - env0;
 
     // camera pose (every lane; the loads are warp-uniform broadcasts)
@@ -89,6 +152,7 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
     // candidate list: lane k prepares drone k of the env
     bool vis = false;
     CamCand cd;
+    CamShade sd;
     if (lane < M && lane != self) {
         const float4 b0 = __ldg(P0 + env0 + lane), b1 = __ldg(P1 + env0 + lane);
         float Rk[3][3];
@@ -143,6 +207,13 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
             cd.c00 = dot(m[0], m[0]); cd.c01x2 = 2.0f * dot(m[0], m[1]); cd.c02x2 = 2.0f * dot(m[0], m[2]);
             cd.c11 = dot(m[1], m[1]); cd.c12x2 = 2.0f * dot(m[1], m[2]); cd.c22 = dot(m[2], m[2]);
             cd.b0 = dot(o, m[0]); cd.b1 = dot(o, m[1]); cd.b2 = dot(o, m[2]);
+            if (RGBA) {
+#pragma unroll
+                for (int r = 0; r < 3; ++r) {
+                    sd.m0[r] = m[0][r]; sd.m1[r] = m[1][r]; sd.m2[r] = m[2][r];
+                    sd.L[r] = (Rk[0][r] * CAM_LIGHT_X + Rk[1][r] * CAM_LIGHT_Y + Rk[2][r] * CAM_LIGHT_Z) * sc[r];
+                }
+            }
             const int bw = cd.box.w - cd.box.z + 1;
             cd.id_rpi = (2 + lane) | ((bw <= 32 ? 32 / bw : 0) << 8); cd.inv_bw = 1.0f / (float)bw;
         }
@@ -150,8 +221,21 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
     const unsigned ball = __ballot_sync(0xffffffffu, vis);
     const int n_cand = __popc(ball);
     if (vis) cand[__popc(ball & ((1u << lane) - 1u))] = cd;
+    if (RGBA && vis) shade[__popc(ball & ((1u << lane) - 1u))] = sd;
     __syncwarp();
 
+    if (RGBA) {                                                  // which other candidates can cover a pixel of this one's box
+        if (lane < n_cand) {
+            const int4 b = cand[lane].box;
+            unsigned ovl = 0;
+            for (int k = 0; k < n_cand; ++k) {
+                const int4 o = cand[k].box;
+                if (k != lane && o.x <= b.y && o.y >= b.x && o.z <= b.w && o.w >= b.z) ovl |= 1u << k;
+            }
+            shade[lane].ovl = ovl;
+        }
+        __syncwarp();
+    }
     const float noz = oz > 0.0f ? -oz : 0.0f;                    // camera on or under the floor: t = 0 < znear never passes (Q46)
     float* dcam = depth ? depth + (size_t)cam * C.n_groups * 4 : nullptr;
     uint8_t* scam = seg ? seg + (size_t)cam * C.n_groups * 4 : nullptr;
@@ -171,7 +255,11 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
             const bool hit = t >= C.znear && t < C.zfar;
             best[j] = hit ? t : C.zfar; ids |= hit ? (1u << (8 * j)) : 0u;
         }
-        if (!TWO_PASS) {
+        if (RGBA) {
+            const unsigned floor_px = cam_shade_rgba(CAM_FLOOR_ALBEDO, CAM_FLOOR_ALBEDO, CAM_FLOOR_ALBEDO, CAM_LIGHT_Z);
+            rgba[(size_t)cam * C.n_groups + g] = make_uint4((ids & 1u) ? floor_px : CAM_SKY, (ids & 0x100u) ? floor_px : CAM_SKY,
+                                                            (ids & 0x10000u) ? floor_px : CAM_SKY, (ids & 0x1000000u) ? floor_px : CAM_SKY);
+        } else if (!TWO_PASS) {
             for (int k = 0; k < n_cand; ++k) {
                 const CamCand& q = cand[k];
                 const int4 bb = q.box;
@@ -191,34 +279,30 @@ render_depth_kernel(const float4* __restrict__ P0, const float4* __restrict__ P1
         r += C.g_rstep;
         if (!ALIGNED) { cg += C.g_cstep; if (cg >= C.groups_per_row) { cg -= C.groups_per_row; r += 1; } }
     }
-    if (TWO_PASS) {
-        for (int k = 0; k < n_cand; ++k) {
-            __syncwarp();                                        // orders the warp's earlier stores before the loads below
-            const CamCand& q = cand[k];
-            const int4 bb = q.box;
-            const int bw = bb.w - bb.z + 1, rpi = q.id_rpi >> 8;
-            const uint8_t id = (uint8_t)(q.id_rpi & 255);
-            auto test = [&](int r, int c) {
-                const float z = (C.half_h - 0.5f - (float)r) * C.s;
-                const float y = fmaf(-(float)(c & 3), C.s, (C.half_w - 0.5f - (float)(c & ~3)) * C.s);   // as the sweep forms it
-                float t;
-                if (cam_hit(q, y, z, t) && t >= C.znear) {
-                    const int px = r * C.W + c;
-                    if (t < __ldcg(dcam + px)) { dcam[px] = t; scam[px] = id; }
-                }
-            };
-            if (rpi > 0) {                                       // the usual case: the warp covers rpi whole rows of the box per pass
-                const int lr = (int)(((float)lane + 0.5f) * q.inv_bw), c = bb.z + (lane - lr * bw);   // lane / bw, exact for lane, bw <= 32
-                if (lr < rpi)
-                    for (int r = bb.x + lr; r <= bb.y; r += rpi) test(r, c);
-            } else {
-                const int n_px = bw * (bb.y - bb.x + 1);
-                for (int i = lane; i < n_px; i += 32) {
-                    const int rr = (int)(((float)i + 0.5f) * q.inv_bw);
-                    test(bb.x + rr, bb.z + (i - rr * bw));
-                }
+    if (TWO_PASS)
+        cam_box_pass(cand, n_cand, lane, C, [&](int, const CamCand& q, int r, int c, float, float, float t) {
+            const int px = r * C.W + c;
+            if (t < __ldcg(dcam + px)) { dcam[px] = t; scam[px] = (uint8_t)(q.id_rpi & 255); }
+        });
+    if (RGBA) {
+        unsigned* const frame = reinterpret_cast<unsigned*>(rgba) + (size_t)cam * C.n_groups * 4;
+        const float ia2 = C.inv_a * C.inv_a, dic = fmaf(C.inv_c, C.inv_c, -ia2);
+        cam_box_pass(cand, n_cand, lane, C, [&](int k, const CamCand& q, int r, int c, float y, float z, float t) {
+            const float tf = noz * rcp_fast(fmaf(y, Ri[2][1], fmaf(z, Ri[2][2], Ri[2][0])));     // the floor, as the sweep forms it
+            bool win = t < ((tf >= C.znear && tf < C.zfar) ? tf : C.zfar);
+            for (unsigned others = shade[k].ovl; others; others &= others - 1u) {
+                const int k2 = __ffs((int)others) - 1;
+                const CamCand& q2 = cand[k2];
+                const int4 bb = q2.box;
+                float t2;
+                if (r >= bb.x && r <= bb.y && c >= bb.z && c <= bb.w && cam_hit(q2, y, z, t2) && t2 >= C.znear && (t2 < t || (t2 == t && k2 < k))) win = false;
             }
-        }
+            if (win) {
+                const int kd = (q.id_rpi & 255) - 2;                 // drone index -> albedo (Q53)
+                frame[r * C.W + c] = cam_shade_rgba((float)(250 - 22 * (kd & 7)), (float)(60 + 40 * ((kd >> 3) & 3)), (float)(40 + 26 * (kd & 7)),
+                                                    cam_ndotl(q, shade[k], y, z, ia2, dic));
+            }
+        });
     }
 }
 
