@@ -154,11 +154,25 @@ def camera_leg(stream, hbm_peak, n_envs=16384, n_drones=4, reps=20, cpu_envs=819
             env.render_depth(depth=depth, seg=seg)
         e1.record(stream)
         stream.synchronize()
+        rgba = env.render_rgba()
+        for _ in range(3):
+            env.render_rgba(rgba=rgba)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
+        for _ in range(reps):
+            env.render_rgba(rgba=rgba)
+        c1.record(stream)
+        stream.synchronize()
     sec = e0.elapsed_time(e1) / 1e3 / reps
+    sec_rgba = c0.elapsed_time(c1) / 1e3 / reps
     frames = n_envs * n_drones
     byt = frames * (48 * 64 * 5 + 32)
+    byt_rgba = frames * (48 * 64 * 4 + 32)
     out = {"workload": f"{n_envs} envs x {n_drones} drones, one 48 x 64 depth (fp32) + segmentation (u8) frame per drone, formation-circle scenes",
-           "frames_per_sec": frames / sec, "us_per_call": sec * 1e6, "gpu_launches": reps,
+           "frames_per_sec": frames / sec, "us_per_call": sec * 1e6, "gpu_launches": 2 * reps,
+           "rgba": {"workload": "the same scenes, one 48 x 64 x 4 uint8 colour frame per drone (mdg_render_rgba)", "frames_per_sec": frames / sec_rgba,
+                    "us_per_call": sec_rgba * 1e6, "bytes_per_launch": byt_rgba, "achieved_gbs": byt_rgba / sec_rgba / 1e9,
+                    "frac": byt_rgba / sec_rgba / 1e9 / hbm_peak, "kernel": "render_depth_kernel<rgba>"},
            "roofline": {"bound": "hbm", "achieved": byt / sec / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": byt / sec / 1e9 / hbm_peak,
                         "traffic": None, "kernel": "render_depth_kernel<two-pass>", "bytes_per_launch": byt,
                         "frac_of_nominal": byt / sec / 1e9 / 7700.0,
@@ -173,6 +187,7 @@ def camera_leg(stream, hbm_peak, n_envs=16384, n_drones=4, reps=20, cpu_envs=819
         pass
     from oracle import oracle as O
     cores = len(os.sched_getaffinity(0))
+    cpu_envs = max(1, min(n_envs, cpu_envs * 16 // (n_drones * n_drones)))     # the oracle's cost per frame grows with the drones per env
     sub = st[: cpu_envs * n_drones].astype(np.float64)
     t0 = time.perf_counter()
     O.render_depth(sub, cpu_envs, n_drones, n_threads=cores)
@@ -448,7 +463,7 @@ def run_ours(args, wl, c):
     if world == 1 and not args.no_camera:
         del envs, acts
         torch.cuda.empty_cache()
-        line["camera"] = camera_leg(stream, hbm_peak)
+        line["camera"] = camera_leg(stream, hbm_peak, n_envs=65536 // args.camera_drones, n_drones=args.camera_drones)
     print(json.dumps(line), flush=True)
     if dist:
         dist.destroy_process_group()
@@ -471,6 +486,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-camera", action="store_true", help="skip the secondary onboard-camera measurement")
+    ap.add_argument("--camera-drones", type=int, default=4, help="drones per env of the camera measurement (65,536 cameras in all)")
     ap.add_argument("--variant", default="", choices=["", "dyn", "table4", "noise", "paper_mjx"], help="secondary workload on the chosen config (see VARIANTS)")
     args = ap.parse_args()
     wl = W.config(args.config)
