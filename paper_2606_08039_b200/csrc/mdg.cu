@@ -59,6 +59,7 @@ struct mdg_env {
     float* stage = nullptr;              // device staging buffer of mdg_step_host (lazily allocated)
     cudaEvent_t order_event = nullptr;   // mdg_set_stream: orders the new stream behind work queued on the old one
     int n_sms = 0, step_grid = 0;        // persistent step kernel: one block per resident slot, looping over tiles
+    int step_grid_chained = 0;           // grid of a launch that chains to the previous step (configure_launch)
     int64_t launches = 0;
     std::map<std::tuple<const void*, int, int64_t>, cudaGraphExec_t> graphs;
 };
@@ -335,11 +336,19 @@ static int configure_launch(mdg_env* h) {
     const long long items = ((long long)h->N + epw - 1) / epw, blocks = (items + wpb - 1) / wpb;
     const long long slots = (long long)h->n_sms * resident;
     h->step_grid = (int)(blocks < slots ? blocks : slots);
+    // A launch that chains to the previous step shares the device with its neighbours in the stream anyway, so it need not
+    // bring a block for every slot: with one block per SM fewer (two envs per lane, four resident blocks) every warp handles
+    // more items per launch and pays its start-up and final fence less often, and the free slots are taken by the next
+    // launch's blocks (same-box A/B on config 5: 19.04 -> 18.63 us per step in the first 40 ms, 19.3 -> 19.1 once the power cap
+    // bites; its DYN variant 16.0 -> 15.2 and 16.4 -> 16.1; no gain with one env per lane, a 1 % loss when a warp has seven
+    // items per launch anyway).  A launch that waits for the whole stream (mdg_step) keeps the full grid.
+    h->step_grid_chained = h->step_grid;
+    if (h->lanes == 2 && resident >= 4 && items >= slots * wpb && items < 3 * slots * wpb) h->step_grid_chained = h->n_sms * (resident - 1);
     // Item-level chaining of consecutive steps.  A grid that fills every resident slot gives each warp the item of its own
-    // index first and hands the others out through a ticket dispenser (which therefore needs items >= warps); two dispensers
-    // alternate, which needs "at most two step kernels in flight": the successor's blocks can only start in slots this grid
-    // has vacated, and the successor's successor only once all of those have started (a warp of this grid would have to
-    // stall for a whole step to be still drawing then).  A smaller grid gives every warp exactly one item (its index), draws
+    // index first and hands the others out through a ticket dispenser (which therefore needs items >= warps); four dispensers
+    // take turns, which needs "at most four step kernels of a handle in flight": a successor's blocks can only start in free
+    // slots, and its own successor only once all of those have started, so for a fifth launch to draw from a dispenser a warp
+    // of the first is still using, three whole grids would have to start and largely finish while that warp stalls.  A smaller grid gives every warp exactly one item (its index), draws
     // nothing, and may therefore be chained to any depth.
     h->saturating = items >= slots * wpb;
     h->P.static_items = h->saturating ? 0u : 1u;                   // one warp per item, no dispenser: any depth of chained launches is safe
@@ -367,7 +376,7 @@ static int launch_step(mdg_env* h, const float* actions_dev, cudaStream_t s, boo
     h->P.chain = (want_chain && h->pdl && h->chainable && h->last_stream == s && h->last_capture == cap_id) ? 1u : 0u;
     h->chainable = true; h->last_stream = s; h->last_capture = cap_id;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)h->step_grid); cfg.blockDim = dim3((unsigned)h->block);
+    cfg.gridDim = dim3((unsigned)(h->P.chain ? h->step_grid_chained : h->step_grid)); cfg.blockDim = dim3((unsigned)h->block);
     cfg.dynamicSmemBytes = (size_t)h->smem; cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

@@ -96,7 +96,7 @@ struct DevBuffers {
     float4* E0;   // wind x y z, bits(ep_step)
     float4* E1;   // running gust impulse: velocity x y z, progress s (>= 1: none)
     uint32_t* gstep;
-    unsigned* ticket;   // [0..1] two work-item dispensers of the step kernel (0 between launches), used alternately; [2..3] their owner stamps
+    unsigned* ticket;   // [0..3] four work-item dispensers of the step kernel (0 between launches), used in turn
     unsigned* item_seq; // per work item: sequence number of the last step that finished it
     float* obs;
     float* reward;

@@ -357,10 +357,10 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
     // Every warp starts on the item of its own index (known without a memory round trip: the blocks of a launch start
     // within a microsecond of each other, whatever they wait for first is paid by all of them); the others are handed out
     // by an atomic ticket (item = tw + ticket; self-resetting: atomicInc wraps to 0 after the n_items grabs of one launch -
-    // n_items - tw items and one miss per warp; two dispensers alternate so that chained launches never share one), so SMs
+    // n_items - tw items and one miss per warp; four dispensers take turns so that chained launches never share one), so SMs
     // that run faster or host fewer long warps simply take more items.
     const unsigned wrap = n_items - 1u;
-    unsigned* const dispenser = B.ticket + (seq & 1u);
+    unsigned* const dispenser = B.ticket + (seq & 3u);
     // Everything with a long latency on the per-item path is issued one item early and consumed late: the ticket
     // of item n+2 is drawn (lane 0, atomic) when item n starts and read after its substeps; the "previous step
     // has published this item" flag of item n+2 is then probed (ld.acquire) and only re-polled at the prefetch
