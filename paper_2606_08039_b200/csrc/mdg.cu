@@ -175,7 +175,12 @@ static void make_dev_params(const mdg_params& p, int N, int M, int feat, DevPara
     for (int i = 0; i < 12; ++i) D.dr_alpha[i] = p.dr_alpha[i];
     for (int i = 0; i < 3; ++i) { D.reset_rpy_half[i] = p.reset_rpy_half[i]; D.reset_vel_half[i] = p.reset_vel_half[i]; }
     D.motor_lag_lo = p.motor_lag_lo; D.motor_lag_hi = p.motor_lag_hi;
-    for (int i = 0; i < 4; ++i) { D.obs_noise[i] = p.obs_noise[i]; D.obs_bias[i] = p.obs_bias[i]; }
+    D.sens_mask = 0u;
+    for (int i = 0; i < 4; ++i) {
+        D.obs_noise[i] = p.obs_noise[i]; D.obs_bias[i] = p.obs_bias[i];
+        if (p.obs_noise[i] != 0.0f) D.sens_mask |= 1u;
+        if (p.obs_bias[i] != 0.0f) D.sens_mask |= 2u;
+    }
     D.path_n = p.form_path_n; D.path_rate = (float)(dtc * p.form_speed);
     {   // moving formation centre (Q52): side lengths and perimeter of the closed polygon, in double
         double per = 0.0;

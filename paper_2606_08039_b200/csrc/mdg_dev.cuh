@@ -73,6 +73,7 @@ struct DevParams {
     int path_n; float path[24], path_len[8], path_perimeter, path_rate;   // moving formation centre: vertices, side lengths, form_speed dt_c
     int lat_a_lo, lat_a_n, lat_s_lo, lat_s_n;             // Table 4 latency rows in substeps: smallest delay and number of values (0 = off)
     float obs_noise[4], obs_bias[4];                      // Table 4 sensor rows: standard deviations for [position, velocity, RPY, body rates]
+    unsigned sens_mask;                                   // bit 0: some obs_noise is non-zero, bit 1: some obs_bias (what is all zero is not drawn)
     float chord[32];                                      // distance between circle slots i and k: chord[|i - k|]
 };
 

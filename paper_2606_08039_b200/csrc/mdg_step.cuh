@@ -249,12 +249,19 @@ struct Sensed { V3 p, eta, v, w; Q4 q; };                         // the kinemat
 __device__ __forceinline__ Sensed sensed(const DroneRegs& d, V3 eta) { Sensed s; s.p = d.p; s.eta = eta; s.v = d.v; s.w = d.w; s.q = d.q; return s; }
 __device__ __forceinline__ void sense(const DevParams& P, unsigned e, uint32_t j, uint32_t t, uint32_t ep_step, Sensed& s) {
     const uint32_t eg = e + P.env_base, t0 = t - ep_step;
-    const float4 n0 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE, P.seed_lo, P.seed_hi));
-    const float4 n1 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE + 1, P.seed_lo, P.seed_hi));
-    const float4 n2 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE + 2, P.seed_lo, P.seed_hi));
-    const float4 b0 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS, P.seed_lo, P.seed_hi));
-    const float4 b1 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS + 1, P.seed_lo, P.seed_hi));
-    const float4 b2 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS + 2, P.seed_lo, P.seed_hi));
+    // a set of standard deviations that is all zero multiplies its draws by zero: they are not made (warp-uniform branches;
+    // 0 stands in for the normals, which leaves every sum below what it was)
+    float4 n0 = make_float4(0.0f, 0.0f, 0.0f, 0.0f), n1 = n0, n2 = n0, b0 = n0, b1 = n0, b2 = n0;
+    if (P.sens_mask & 1u) {
+        n0 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE, P.seed_lo, P.seed_hi));
+        n1 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE + 1, P.seed_lo, P.seed_hi));
+        n2 = normals4(philox4x32_10(eg, j, t, STREAM_OBS_NOISE + 2, P.seed_lo, P.seed_hi));
+    }
+    if (P.sens_mask & 2u) {
+        b0 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS, P.seed_lo, P.seed_hi));
+        b1 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS + 1, P.seed_lo, P.seed_hi));
+        b2 = normals4(philox4x32_10(eg, j, t0, STREAM_OBS_BIAS + 2, P.seed_lo, P.seed_hi));
+    }
     const float sp = P.obs_noise[0], sv = P.obs_noise[1], se = P.obs_noise[2], sw = P.obs_noise[3];
     const float bp = P.obs_bias[0], bv = P.obs_bias[1], be = P.obs_bias[2], bw = P.obs_bias[3];
     s.p.x += fmaf(sp, n0.x, bp * b0.x); s.p.y += fmaf(sp, n0.y, bp * b0.y); s.p.z += fmaf(sp, n0.z, bp * b0.z);
