@@ -264,7 +264,8 @@ def run_ours(args, wl, c):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     K, Wm = args.steps, max(args.warmup, 3)
-    use_graph = args.mode == "graph" or (args.mode == "auto" and c != 5)    # the latency-bound configs: no host launch rate in the number
+    # the latency-bound batches (configs 1-4: at most 16,384 drones) go through one graph: no host launch rate in the number
+    use_graph = args.mode == "graph" or (args.mode == "auto" and wl.n_envs * wl.n_drones < 65536)
     if use_graph:
         K = -(-K // GRAPH_STEPS) * GRAPH_STEPS                              # whole graphs
     stream = torch.cuda.Stream()
