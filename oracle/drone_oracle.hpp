@@ -812,7 +812,10 @@ struct Sim {
                 for (int a = 0; a < 3; ++a) w[a] = w[a] + P.wind_const[a];
             if (P.wind_mask & WIND_GUST) {                         // PAPER.md:201, Q42
                 double* gs = &gust[(size_t)e * 4];
-                if (gs[3] >= 1.0) {                                // no impulse running: trigger with probability gust_prob
+                // an impulse is over once its phase has reached 1 - 1e-4 (Q42): the envelope is 3e-4 there, and a duration that is a
+                // whole number of control steps (the default 0.5 s = 24 steps) is not decided by the last bit of the accumulated phase
+                constexpr double GUST_END = 1.0 - 1e-4;
+                if (gs[3] >= GUST_END) {                           // no impulse running: trigger with probability gust_prob
                     const PhiloxOut r = philox4x32_10((uint32_t)e + (uint32_t)P.env_index_base, ENV_LEVEL, t, STREAM_GUST, k0, k1);
                     if (u01(r.x[0]) < P.gust_prob) {
                         const double amp = P.gust_max * u01(r.x[1]), z = 2.0 * u01(r.x[2]) - 1.0, ph = 2.0 * PI * u01(r.x[3]);
@@ -820,7 +823,7 @@ struct Sim {
                         gs[0] = amp * rxy * std::cos(ph); gs[1] = amp * rxy * std::sin(ph); gs[2] = amp * z; gs[3] = 0.0;
                     }
                 }
-                if (gs[3] < 1.0) {                                 // smooth envelope sin(pi s), s advancing by dt / duration
+                if (gs[3] < GUST_END) {                            // smooth envelope sin(pi s), s advancing by dt / duration
                     const R env_s = sin(R(PI * gs[3]));
                     for (int a = 0; a < 3; ++a) w[a] = w[a] + gs[a] * env_s;
                     gs[3] += D.dt_c / P.gust_duration;

@@ -504,7 +504,8 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
             if (wmask & 2) { u.x += P.wind_const[0]; u.y += P.wind_const[1]; u.z += P.wind_const[2]; }
             if (wmask & 4) {                                           // PAPER.md:201 impulses (Q42), state in E1
                 float4 gs = B.E1[e];
-                if (gs.w >= 1.0f) {                                    // none running: trigger with probability gust_prob
+                constexpr float GUST_END = 1.0f - 1e-4f;               // Q42: over at phase 1 - 1e-4, so that a duration of a whole number of steps is no rounding tie
+                if (gs.w >= GUST_END) {                                // none running: trigger with probability gust_prob
                     const uint4 r = philox4x32_10(e + P.env_base, 0xFFFFFFFFu, t, STREAM_GUST, P.seed_lo, P.seed_hi);
                     if (u01(r.x) < P.gust_prob) {
                         const float amp = P.gust_max * u01(r.y), z = fmaf(2.0f, u01(r.z), -1.0f);
@@ -514,7 +515,7 @@ __global__ void __launch_bounds__(128, MINB) step_kernel(const __grid_constant__
                         gs = make_float4(amp * rxy * cp, amp * rxy * sp, amp * z, 0.0f);
                     }
                 }
-                if (gs.w < 1.0f) {                                     // envelope sin(pi s), s advances by dt_c / duration
+                if (gs.w < GUST_END) {                                 // envelope sin(pi s), s advances by dt_c / duration
                     const float es = sinpif(gs.w);
                     u.x = fmaf(gs.x, es, u.x); u.y = fmaf(gs.y, es, u.y); u.z = fmaf(gs.z, es, u.z);
                     gs.w += P.gust_ds;

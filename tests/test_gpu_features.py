@@ -112,6 +112,12 @@ CASES = {
     # gust impulses (frequent, short) alone and the paper's COMBINED = all four wind components
     "m1_wind_gust": (wl("m1wg", 1500, 1, W.PHYS_MJC, W.ACT_VEL, dict(SINGLE, aero_mask=W.AERO_WIND, wind_mask=4, gust_prob=0.2,
                         gust_max=2.0, gust_duration=0.2), ("uniform", -0.5, 0.5)), {}),
+    # impulses that last a whole number of control steps (0.25 s = 12, and the default 0.5 s = 24): the end of an impulse must not
+    # hang on the last bit of the accumulated phase (Q42; a differential fuzz found fp32 and fp64 ending them one step apart)
+    "m1_wind_gust_whole_steps": (wl("m1wg12", 1500, 1, W.PHYS_MJC, W.ACT_VEL, dict(SINGLE, aero_mask=W.AERO_WIND, wind_mask=4, gust_prob=0.2,
+                                    gust_max=2.0, gust_duration=0.25), ("uniform", -0.5, 0.5)), {}),
+    "m2_wind_gust_default_duration": (wl("m2wg24", 900, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, aero_mask=W.AERO_WIND | W.AERO_DRAG,
+                                         wind_mask=4, gust_prob=0.3, gust_max=1.5), HOVER), {}),
     "m2_wind_combined": (wl("m2wall", 900, 2, W.PHYS_MJC_DRAG, W.ACT_RPM, dict(GRID, grid_cols=2, aero_mask=W.AERO_WIND | W.AERO_DRAG, wind_mask=15,
                             wind_const=[0.0, 0.9, 0.0], wind_sine_amp=0.01, wind_sine_omega=3.0, gust_prob=0.1, gust_max=1.5, gust_duration=0.3,
                             episode_len_s=0.5), HOVER), {}),
